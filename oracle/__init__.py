@@ -1,0 +1,178 @@
+"""CPU oracle for the Landau gauge-fixing hot path -- TEST INFRASTRUCTURE, not the product.
+
+Thin ctypes loader around ``oracle/lgf_oracle.c`` (plain C11, double precision, Algorithm 1 of
+arXiv:1206.0675 step by step; see the header of that file for conventions and citations).  Only
+``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline`` / ``--impl reference``
+legs may import this package.  It imports nothing from ``paper_1206_0675_b200`` and the CUDA path
+imports nothing from here.
+
+Array conventions (numpy, complex128, C-contiguous):
+  links U : shape (Lt, Lz, Ly, Lx, 4, 3, 3)   site-major, mu = 0..3 = x, y, z, t
+  Delta, w, g : shape (Lt, Lz, Ly, Lx, 3, 3)
+  scalar field : shape (Lt, Lz, Ly, Lx)
+  dims : (Lx, Ly, Lz, Lt)   (x fastest in memory)
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "lgf_oracle.c")
+_LIB = os.path.join(_HERE, "liblgf_oracle.so")
+CFLAGS = ["-O2", "-std=c11", "-fopenmp", "-fcx-limited-range", "-shared", "-fPIC"]
+
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle with gcc (idempotent).  Returns the path of the shared object."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        tmp = _LIB + ".tmp.%d" % os.getpid()
+        subprocess.run(["gcc", *CFLAGS, _SRC, "-o", tmp, "-lm"], check=True)
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        lib = ctypes.CDLL(build())
+        vp, i4 = ctypes.c_void_p, ctypes.POINTER(ctypes.c_int)
+        dp, d, lg = ctypes.POINTER(ctypes.c_double), ctypes.c_double, ctypes.c_long
+        lib.orc_num_threads.restype = ctypes.c_int
+        lib.orc_measure.argtypes = [i4, vp, vp, dp, dp]
+        lib.orc_dft4d.argtypes = [i4, vp, ctypes.c_int, vp]
+        lib.orc_p2.argtypes = [i4, i4]
+        lib.orc_p2.restype = d
+        lib.orc_accelerate.argtypes = [i4, vp, vp]
+        lib.orc_build_g.argtypes = [i4, vp, d, vp]
+        lib.orc_transform.argtypes = [i4, vp, vp]
+        lib.orc_iterate.argtypes = [i4, vp, d, lg, vp, vp]
+        lib.orc_fix.argtypes = [i4, vp, d, d, lg, vp, vp, lg]
+        lib.orc_fix.restype = lg
+        lib.orc_plaquette.argtypes = [i4, vp]
+        lib.orc_plaquette.restype = d
+        lib.orc_gs.argtypes = [vp, vp]
+        lib.orc_reconstruct_row3.argtypes = [vp, vp]
+        _lib = lib
+    return _lib
+
+
+def num_threads() -> int:
+    return int(_load().orc_num_threads())
+
+
+def _dims(dims):
+    dims = tuple(int(v) for v in dims)
+    assert len(dims) == 4
+    return dims, (ctypes.c_int * 4)(*dims)
+
+
+def _c128(a, shape):
+    a = np.ascontiguousarray(a, dtype=np.complex128)
+    assert a.shape == tuple(shape), (a.shape, shape)
+    return a
+
+
+def _site_shape(dims):
+    return (dims[3], dims[2], dims[1], dims[0])
+
+
+def _ptr(a):
+    return a.ctypes.data_as(ctypes.c_void_p)
+
+
+def measure(dims, U, want_delta: bool = True):
+    """Alg. 1 line 1 / 17.  Returns (Delta or None, F, theta)."""
+    dims, cd = _dims(dims)
+    U = _c128(U, _site_shape(dims) + (4, 3, 3))
+    Delta = np.empty(_site_shape(dims) + (3, 3), np.complex128) if want_delta else None
+    F, th = ctypes.c_double(), ctypes.c_double()
+    _load().orc_measure(cd, _ptr(U), _ptr(Delta) if want_delta else None, ctypes.byref(F), ctypes.byref(th))
+    return Delta, F.value, th.value
+
+
+def dft4d(dims, f, sign: int):
+    """Naive separable 4-D DFT of one complex scalar field; sign=-1 forward, +1 inverse, unnormalised."""
+    dims, cd = _dims(dims)
+    f = _c128(f, _site_shape(dims))
+    out = np.empty_like(f)
+    _load().orc_dft4d(cd, _ptr(f), int(sign), _ptr(out))
+    return out
+
+
+def p2(dims, k):
+    dims, cd = _dims(dims)
+    return float(_load().orc_p2(cd, (ctypes.c_int * 4)(*[int(v) for v in k])))
+
+
+def accelerate(dims, Delta):
+    """Alg. 1 lines 3-8: w = F^-1 (16/p^2) F Delta, zero mode removed, 1/V included."""
+    dims, cd = _dims(dims)
+    Delta = _c128(Delta, _site_shape(dims) + (3, 3))
+    w = np.empty_like(Delta)
+    _load().orc_accelerate(cd, _ptr(Delta), _ptr(w))
+    return w
+
+
+def build_g(dims, w, alpha: float):
+    dims, cd = _dims(dims)
+    w = _c128(w, _site_shape(dims) + (3, 3))
+    g = np.empty_like(w)
+    _load().orc_build_g(cd, _ptr(w), float(alpha), _ptr(g))
+    return g
+
+
+def transform(dims, U, g):
+    """Returns g(x) U_mu(x) g(x+mu)^dag as a new array."""
+    dims, cd = _dims(dims)
+    U = _c128(U, _site_shape(dims) + (4, 3, 3)).copy()
+    g = _c128(g, _site_shape(dims) + (3, 3))
+    _load().orc_transform(cd, _ptr(U), _ptr(g))
+    return U
+
+
+def iterate(dims, U, alpha: float, n: int):
+    """n updates.  Returns (U_after, F[0..n], theta[0..n]); entry i = after i updates (R12)."""
+    dims, cd = _dims(dims)
+    U = _c128(U, _site_shape(dims) + (4, 3, 3)).copy()
+    Fh = np.zeros(n + 1)
+    Th = np.zeros(n + 1)
+    _load().orc_iterate(cd, _ptr(U), float(alpha), int(n), _ptr(Fh), _ptr(Th))
+    return U, Fh, Th
+
+
+def fix(dims, U, alpha: float, tol: float, max_iter: int):
+    """Algorithm 1.  Returns (U_fixed, iterations, F[0..it], theta[0..it])."""
+    dims, cd = _dims(dims)
+    U = _c128(U, _site_shape(dims) + (4, 3, 3)).copy()
+    cap = int(max_iter) + 1
+    Fh = np.zeros(cap)
+    Th = np.zeros(cap)
+    it = int(_load().orc_fix(cd, _ptr(U), float(alpha), float(tol), int(max_iter), _ptr(Fh), _ptr(Th), cap))
+    return U, it, Fh[: it + 1].copy(), Th[: it + 1].copy()
+
+
+def plaquette(dims, U) -> float:
+    dims, cd = _dims(dims)
+    U = _c128(U, _site_shape(dims) + (4, 3, 3))
+    return float(_load().orc_plaquette(cd, _ptr(U)))
+
+
+def gs(M):
+    """Gram-Schmidt projection of one 3x3 complex matrix onto SU(3) (rows; R9)."""
+    M = _c128(M, (3, 3))
+    G = np.empty_like(M)
+    _load().orc_gs(_ptr(M), _ptr(G))
+    return G
+
+
+def reconstruct_row3(rows01):
+    rows01 = _c128(rows01, (2, 3))
+    out = np.empty(3, np.complex128)
+    _load().orc_reconstruct_row3(_ptr(rows01), _ptr(out))
+    return out
