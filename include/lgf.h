@@ -1,0 +1,145 @@
+/*
+ * lgf.h -- C ABI of liblgf: Fourier-accelerated steepest-descent Landau gauge fixing of a 4-D SU(3)
+ * lattice gauge configuration on one NVIDIA B200 (sm_100a).
+ *
+ * Method: Cardoso, Silva, Bicudo, Oliveira, "Landau Gauge Fixing on GPUs", arXiv:1206.0675.
+ * Citations below are "PAPER.md:<line>" of the extracted text plus the equation / algorithm line.
+ *
+ * One iteration (Algorithm 1) on the configuration {U_mu(x)}:
+ *   a1  A_mu(x)  = [(U_mu(x) - U_mu(x)^dag) / 2i] - (1/3) tr[.] 1                       (eq. 7, :75)
+ *       Delta(x) = sum_mu [A_mu(x - mu) - A_mu(x)]                                       (eq. 5, :63)
+ *       F        = sum_x sum_mu Re tr U_mu(x) / (4 * 3 * V)                              (eq. 3, :52)
+ *       theta    = sum_x tr[Delta(x) Delta(x)^dag] / (3 V)                               (eq. 6, :70)
+ *   a2  4-D forward FFT of every independent component of Delta                         (Alg. 1 line 4)
+ *   a3  multiply by p2max / p2(k), p2 = 4 sum_mu sin^2(pi k_mu / L_mu), p2max = 16, k = 0 -> 0 (line 5, :66)
+ *   a4  4-D inverse FFT, normalised by 1/V  ->  w(x)                                    (lines 6-7)
+ *   a5  g(x) = reunitarise(1 + i (alpha/2) w(x))   (first-order exp, Gram-Schmidt on rows, row 2 from eq. 8; :66, :148)
+ *   a6  U_mu(x) <- g(x) U_mu(x) g(x + mu)^dag  for all x, mu                            (eq. 2, :45; line 14)
+ *
+ * All of it runs in hand-written CUDA kernels; there is no CPU fallback: every entry point returns
+ * LGF_ECUDA if no usable device is present.
+ *
+ * Conventions
+ *   dims[4] = {Lx, Ly, Lz, Lt}; periodic; site index s = x + Lx*(y + Ly*(z + Lz*t)) (x fastest).
+ *   Each L_mu must be one of 2, 3, 4, 6, 8, 12, 16, 24, 32, 48, 64; otherwise LGF_EINVAL.
+ *   CANONICAL link layout (what callers pass in and get back): site-major array of structures
+ *     links[s][mu][i][j][re/im], mu = 0..3 = x, y, z, t, row-major 3x3, i.e. 72 reals per site,
+ *     of type float (LGF_FP32) or double (LGF_FP64) matching the context's precision.
+ *     As a torch tensor: shape [Lt, Lz, Ly, Lx, 4, 3, 3, 2].  Always 18 reals per link, whatever the
+ *     internal storage.  The library never keeps a caller pointer after the call returns.
+ *   Internally links live in a structure-of-arrays layout (18 or 12 reals per link; with
+ *     LGF_LINKS_12 only the first two rows are stored and the third is rebuilt as (row0 x row1)^*,
+ *     eq. 8); the context owns that storage, the FFT work fields, tables,
+ *     reduction scratch and the (F, theta) history.
+ *   "d_" arguments are DEVICE pointers, "h_" arguments are HOST pointers (pageable or pinned).
+ *   All work is enqueued on the context's stream (default: the legacy default stream 0; set it with
+ *     lgf_set_stream).  Calls that return values to the host synchronise that stream.
+ *   Error handling: every function returns LGF_OK (0) or a negative LGF_E* code (lgf_fix*: the number
+ *     of iterations >= 0, or a negative code); nothing throws or aborts across the ABI.  The message
+ *     of the last failure is available from lgf_last_error.  One context per host thread.
+ */
+#ifndef LGF_H
+#define LGF_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct lgf_ctx lgf_ctx; /* opaque */
+
+enum { LGF_FP32 = 4, LGF_FP64 = 8 };           /* precision = bytes per real                      */
+enum { LGF_LINKS_18 = 18, LGF_LINKS_12 = 12 }; /* internal reals per link      */
+enum {
+    LGF_OK = 0,
+    LGF_EINVAL = -1, /* bad argument (dims, precision, storage, null pointer, range)              */
+    LGF_ENOMEM = -2, /* device or host allocation failed                                          */
+    LGF_ECUDA = -3,  /* CUDA runtime error or no device; see lgf_last_error                       */
+    LGF_ESTATE = -4, /* call out of order (e.g. iterate before any links were set)                */
+    LGF_ENAN = -5    /* theta became NaN/Inf; iteration stopped                                   */
+};
+
+/* Create a context for a lattice of the given dims, arithmetic precision (LGF_FP32 / LGF_FP64; the
+ * kernels compute and store in that type, cross-site sums for F and theta are accumulated in fp64)
+ * and internal link storage.  Allocates all device buffers on the current CUDA device. */
+int lgf_create(const int dims[4], int precision, int link_storage, lgf_ctx **out);
+int lgf_destroy(lgf_ctx *ctx);
+
+/* cuda_stream is a cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream); the caller owns it. */
+int lgf_set_stream(lgf_ctx *ctx, void *cuda_stream);
+
+/* Copy a configuration in canonical layout into the context (converts to the internal layout) /
+ * copy the current configuration out.  Resets the iteration counter and the history (set only).
+ * Asynchronous on the context's stream for device pointers; the host variants return after the
+ * host buffer may be reused / has been filled. */
+int lgf_set_links(lgf_ctx *ctx, const void *d_links);
+int lgf_get_links(lgf_ctx *ctx, void *d_links);
+int lgf_set_links_host(lgf_ctx *ctx, const void *h_links);
+int lgf_get_links_host(lgf_ctx *ctx, void *h_links);
+
+/* n iterations of Algorithm 1's loop body [a1 -> a2..a4 -> a5/a6] on the internal configuration
+ * with step alpha (the paper uses 0.08), regardless of theta.  (F, theta) of the
+ * configuration BEFORE each update is appended to the history.  Never blocks the host. */
+int lgf_iterate(lgf_ctx *ctx, double alpha, int n);
+
+/* F, theta (a1) and the average plaquette
+ *   P = sum_x sum_{mu<nu} Re tr[U_mu(x) U_nu(x+mu) U_mu(x+nu)^dag U_nu(x)^dag] / (6 * 3 * V)
+ * of the current internal configuration.  Any of the out-pointers may be NULL.  Synchronises. */
+int lgf_measure(lgf_ctx *ctx, double *F, double *theta, double *plaquette);
+
+/* Algorithm 1: load the configuration at d_links / h_links, then
+ *   measure; while (theta >= tol && it < max_iter) { update; measure; ++it }
+ * and write the gauge-fixed configuration back to the same buffer.  Returns the number of updates
+ * applied (0 if the input already satisfies theta < tol; max_iter if it did not converge -- check
+ * with lgf_measure or lgf_history), or a negative LGF_E* code.  History entry n (n = 0..it) holds
+ * (F, theta) of the configuration after n updates.  Synchronises. */
+long long lgf_fix(lgf_ctx *ctx, void *d_links, double alpha, double tol, long long max_iter);
+long long lgf_fix_host(lgf_ctx *ctx, void *h_links, double alpha, double tol, long long max_iter);
+
+/* Copy history entries first .. first+count-1 into F[] and theta[] (host arrays, either may be
+ * NULL).  Entries are those recorded since the last set_links / fix.  Synchronises. */
+int lgf_history(lgf_ctx *ctx, long long first, long long count, double *F, double *theta);
+
+/* Number of updates applied since the last set_links / fix (synchronises), or a negative code. */
+long long lgf_iterations(lgf_ctx *ctx);
+/* Number of (F, theta) history entries recorded since the last set_links / fix (synchronises). */
+long long lgf_history_length(lgf_ctx *ctx);
+
+/* ---- single steps of the path, exposed so that each row of the hot path can be checked against
+ * ---- the oracle element by element (tests) and profiled on its own (bench) ---------------------- */
+
+/* a1 only: Delta(x) of the current configuration into the packed work field W (and F, theta, not
+ * recorded in the history).  F / theta may be NULL.  Synchronises if either is non-NULL. */
+int lgf_step_delta(lgf_ctx *ctx, double *F, double *theta);
+/* a2-a4 only: W <- F^-1 [(16/p2) F W] / V in place. */
+int lgf_step_accelerate(lgf_ctx *ctx);
+/* a5 + a6 only: g(x) from the current W with step alpha, then the link transform. */
+int lgf_step_update(lgf_ctx *ctx, double alpha);
+/* The work field as full 3x3 complex matrices, d_field[s][i][j][re/im] (18 reals per site, context
+ * precision).  get: unpack W (hermitian traceless by construction).  set: pack a hermitian
+ * traceless field into W (the anti-hermitian / trace parts of the argument are ignored). */
+int lgf_get_field(lgf_ctx *ctx, void *d_field);
+int lgf_set_field(lgf_ctx *ctx, const void *d_field);
+
+/* ---- instrumentation ------------------------------------------------------------------------- */
+
+/* Kernel classes for per-kernel timing. */
+enum { LGF_K_DELTA = 0, LGF_K_FFT = 1, LGF_K_UPDATE = 2, LGF_K_GBUILD = 3, LGF_K_CONVERT = 4,
+       LGF_K_PLAQ = 5, LGF_K_COUNT = 6 };
+/* When on != 0 every kernel launch is bracketed by CUDA events on the context's stream. */
+int lgf_set_profiling(lgf_ctx *ctx, int on);
+/* Sum of the event-measured durations (ms) and the number of launches per kernel class since
+ * profiling was switched on (arrays of LGF_K_COUNT entries, either may be NULL).  Synchronises. */
+int lgf_kernel_times(lgf_ctx *ctx, double *ms, long long *launches);
+/* Total number of kernels this context has launched since creation. */
+long long lgf_launch_count(const lgf_ctx *ctx);
+/* Algorithmic bytes one launch-set of the given kernel class must move for ONE iteration
+ * (DESIGN.md "Algorithmic bytes"): e.g. LGF_K_DELTA -> V * (4*n_l + 8) * bytes_per_real. */
+double lgf_algorithmic_bytes(const lgf_ctx *ctx, int kernel_class);
+
+const char *lgf_last_error(const lgf_ctx *ctx);
+const char *lgf_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LGF_H */

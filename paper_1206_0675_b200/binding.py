@@ -1,0 +1,272 @@
+"""ctypes binding of liblgf (include/lgf.h) -- argument marshalling only.
+
+Every function has the name and the meaning of the C entry point it wraps; every step of the hot path
+runs inside the CUDA kernels of liblgf.so.  PyTorch is used here only to own device memory and to
+provide the stream.  There is no CPU fallback: if liblgf.so is missing the import of the library
+fails with an instruction to build it, and without a CUDA device ``lgf_create`` raises ``LgfError``.
+
+Tensors passed as ``links`` are in the canonical layout of include/lgf.h: shape
+[Lt, Lz, Ly, Lx, 4, 3, 3, 2] real (or [Lt, Lz, Ly, Lx, 4, 3, 3] complex), dtype matching the
+context's precision, contiguous; CUDA tensors go to the device entry points, CPU tensors / numpy
+arrays to the ``*_host`` ones.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+
+LGF_FP32, LGF_FP64 = 4, 8
+LGF_LINKS_18, LGF_LINKS_12 = 18, 12
+LGF_OK, LGF_EINVAL, LGF_ENOMEM, LGF_ECUDA, LGF_ESTATE, LGF_ENAN = 0, -1, -2, -3, -4, -5
+LGF_K_DELTA, LGF_K_FFT, LGF_K_UPDATE, LGF_K_GBUILD, LGF_K_CONVERT, LGF_K_PLAQ, LGF_K_COUNT = 0, 1, 2, 3, 4, 5, 6
+KERNEL_CLASSES = ("delta", "fft", "update", "gbuild", "convert", "plaquette")
+
+_LIBPATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "liblgf.so")
+_lib = None
+
+# name -> (restype, argtypes); the list of symbols include/lgf.h declares
+_vp, _i, _d, _ll = ctypes.c_void_p, ctypes.c_int, ctypes.c_double, ctypes.c_longlong
+_dp, _llp = ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_longlong)
+SIGNATURES = {
+    "lgf_create": (_i, [ctypes.POINTER(ctypes.c_int), _i, _i, ctypes.POINTER(_vp)]),
+    "lgf_destroy": (_i, [_vp]),
+    "lgf_set_stream": (_i, [_vp, _vp]),
+    "lgf_set_links": (_i, [_vp, _vp]),
+    "lgf_get_links": (_i, [_vp, _vp]),
+    "lgf_set_links_host": (_i, [_vp, _vp]),
+    "lgf_get_links_host": (_i, [_vp, _vp]),
+    "lgf_iterate": (_i, [_vp, _d, _i]),
+    "lgf_measure": (_i, [_vp, _dp, _dp, _dp]),
+    "lgf_fix": (_ll, [_vp, _vp, _d, _d, _ll]),
+    "lgf_fix_host": (_ll, [_vp, _vp, _d, _d, _ll]),
+    "lgf_history": (_i, [_vp, _ll, _ll, _dp, _dp]),
+    "lgf_history_length": (_ll, [_vp]),
+    "lgf_iterations": (_ll, [_vp]),
+    "lgf_step_delta": (_i, [_vp, _dp, _dp]),
+    "lgf_step_accelerate": (_i, [_vp]),
+    "lgf_step_update": (_i, [_vp, _d]),
+    "lgf_get_field": (_i, [_vp, _vp]),
+    "lgf_set_field": (_i, [_vp, _vp]),
+    "lgf_set_profiling": (_i, [_vp, _i]),
+    "lgf_kernel_times": (_i, [_vp, _dp, _llp]),
+    "lgf_launch_count": (_ll, [_vp]),
+    "lgf_algorithmic_bytes": (_d, [_vp, _i]),
+    "lgf_last_error": (ctypes.c_char_p, [_vp]),
+    "lgf_version": (ctypes.c_char_p, []),
+}
+
+
+class LgfError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__("liblgf error %d: %s" % (code, msg))
+        self.code = code
+
+
+def library_path() -> str:
+    return _LIBPATH
+
+
+def load():
+    """Load liblgf.so (built by ``python -m paper_1206_0675_b200.build``).  Never falls back."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(_LIBPATH):
+            raise ImportError("%s is missing: build the CUDA library with `python -m paper_1206_0675_b200.build` "
+                              "(there is no CPU fallback)" % _LIBPATH)
+        lib = ctypes.CDLL(_LIBPATH)
+        for name, (res, args) in SIGNATURES.items():
+            fn = getattr(lib, name)
+            fn.restype, fn.argtypes = res, args
+        _lib = lib
+    return _lib
+
+
+def _check(ctx, rc):
+    if rc < 0:
+        msg = load().lgf_last_error(ctx)
+        raise LgfError(int(rc), msg.decode() if msg else "")
+    return rc
+
+
+def _dev_ptr(t, ctx_prec, nreal):
+    import torch
+
+    if not isinstance(t, torch.Tensor) or not t.is_cuda:
+        raise TypeError("expected a CUDA torch tensor")
+    if t.is_complex():
+        t = torch.view_as_real(t)
+    want = torch.float64 if ctx_prec == LGF_FP64 else torch.float32
+    if t.dtype != want or not t.is_contiguous() or t.numel() != nreal:
+        raise ValueError("tensor must be contiguous %s with %d reals (got %s, %d)" % (want, nreal, t.dtype, t.numel()))
+    return ctypes.c_void_p(t.data_ptr())
+
+
+def _host_ptr(a, ctx_prec, nreal):
+    import torch
+
+    if isinstance(a, torch.Tensor):
+        if a.is_cuda:
+            raise TypeError("expected host memory")
+        if a.is_complex():
+            a = torch.view_as_real(a)
+        want = torch.float64 if ctx_prec == LGF_FP64 else torch.float32
+        if a.dtype != want or not a.is_contiguous() or a.numel() != nreal:
+            raise ValueError("host tensor must be contiguous %s with %d reals" % (want, nreal))
+        return ctypes.c_void_p(a.data_ptr())
+    want = {LGF_FP64: (np.float64, np.complex128), LGF_FP32: (np.float32, np.complex64)}[ctx_prec]
+    if not isinstance(a, np.ndarray) or a.dtype not in want or not a.flags.c_contiguous:
+        raise ValueError("host array must be a C-contiguous numpy array of %s" % (want,))
+    if a.size * (2 if np.iscomplexobj(a) else 1) != nreal:
+        raise ValueError("host array has the wrong size")
+    return ctypes.c_void_p(a.ctypes.data)
+
+
+class Context:
+    """Owns one lgf_ctx.  Methods are the C entry points minus the ``lgf_`` prefix and ``ctx`` argument."""
+
+    def __init__(self, dims, precision=LGF_FP64, link_storage=LGF_LINKS_18, stream=None):
+        self.dims = tuple(int(v) for v in dims)
+        self.precision, self.link_storage = int(precision), int(link_storage)
+        self.V = int(np.prod(self.dims))
+        self._h = ctypes.c_void_p()
+        lib = load()
+        rc = lib.lgf_create((ctypes.c_int * 4)(*self.dims), self.precision, self.link_storage, ctypes.byref(self._h))
+        if rc < 0:
+            msg = lib.lgf_last_error(None)
+            raise LgfError(rc, msg.decode() if msg else "")
+        if stream is not None:
+            self.set_stream(stream)
+
+    # -- lifetime ---------------------------------------------------------------------------------
+    def destroy(self):
+        if self._h:
+            load().lgf_destroy(self._h)
+            self._h = ctypes.c_void_p()
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.destroy()
+
+    # -- plumbing ---------------------------------------------------------------------------------
+    def set_stream(self, stream):
+        ptr = stream.cuda_stream if hasattr(stream, "cuda_stream") else int(stream)
+        _check(self._h, load().lgf_set_stream(self._h, ctypes.c_void_p(ptr)))
+
+    def set_links(self, links):
+        _check(self._h, load().lgf_set_links(self._h, _dev_ptr(links, self.precision, self.V * 72)))
+
+    def get_links(self, out):
+        _check(self._h, load().lgf_get_links(self._h, _dev_ptr(out, self.precision, self.V * 72)))
+        return out
+
+    def set_links_host(self, links):
+        _check(self._h, load().lgf_set_links_host(self._h, _host_ptr(links, self.precision, self.V * 72)))
+
+    def get_links_host(self, out):
+        _check(self._h, load().lgf_get_links_host(self._h, _host_ptr(out, self.precision, self.V * 72)))
+        return out
+
+    # -- the path ---------------------------------------------------------------------------------
+    def iterate(self, alpha, n):
+        _check(self._h, load().lgf_iterate(self._h, float(alpha), int(n)))
+
+    def measure(self, plaquette=True):
+        F, th, P = ctypes.c_double(), ctypes.c_double(), ctypes.c_double()
+        _check(self._h, load().lgf_measure(self._h, ctypes.byref(F), ctypes.byref(th),
+                                           ctypes.byref(P) if plaquette else None))
+        return F.value, th.value, (P.value if plaquette else None)
+
+    def fix(self, links, alpha, tol, max_iter):
+        return int(_check(self._h, load().lgf_fix(self._h, _dev_ptr(links, self.precision, self.V * 72), float(alpha),
+                                                  float(tol), int(max_iter))))
+
+    def fix_host(self, links, alpha, tol, max_iter):
+        return int(_check(self._h, load().lgf_fix_host(self._h, _host_ptr(links, self.precision, self.V * 72),
+                                                       float(alpha), float(tol), int(max_iter))))
+
+    def history_length(self):
+        return int(_check(self._h, load().lgf_history_length(self._h)))
+
+    def history(self, first=0, count=None):
+        if count is None:
+            count = self.history_length() - first
+        F = np.zeros(count)
+        th = np.zeros(count)
+        _check(self._h, load().lgf_history(self._h, int(first), int(count), F.ctypes.data_as(_dp), th.ctypes.data_as(_dp)))
+        return F, th
+
+    def iterations(self):
+        return int(_check(self._h, load().lgf_iterations(self._h)))
+
+    # -- single steps -----------------------------------------------------------------------------
+    def step_delta(self, want_values=True):
+        if not want_values:
+            _check(self._h, load().lgf_step_delta(self._h, None, None))
+            return None
+        F, th = ctypes.c_double(), ctypes.c_double()
+        _check(self._h, load().lgf_step_delta(self._h, ctypes.byref(F), ctypes.byref(th)))
+        return F.value, th.value
+
+    def step_accelerate(self):
+        _check(self._h, load().lgf_step_accelerate(self._h))
+
+    def step_update(self, alpha):
+        _check(self._h, load().lgf_step_update(self._h, float(alpha)))
+
+    def get_field(self, out):
+        _check(self._h, load().lgf_get_field(self._h, _dev_ptr(out, self.precision, self.V * 18)))
+        return out
+
+    def set_field(self, field):
+        _check(self._h, load().lgf_set_field(self._h, _dev_ptr(field, self.precision, self.V * 18)))
+
+    # -- instrumentation --------------------------------------------------------------------------
+    def set_profiling(self, on):
+        _check(self._h, load().lgf_set_profiling(self._h, int(bool(on))))
+
+    def kernel_times(self):
+        ms = (ctypes.c_double * LGF_K_COUNT)()
+        n = (ctypes.c_longlong * LGF_K_COUNT)()
+        _check(self._h, load().lgf_kernel_times(self._h, ms, n))
+        return {k: (ms[i], int(n[i])) for i, k in enumerate(KERNEL_CLASSES)}
+
+    def launch_count(self):
+        return int(load().lgf_launch_count(self._h))
+
+    def algorithmic_bytes(self, kernel_class):
+        return float(load().lgf_algorithmic_bytes(self._h, int(kernel_class)))
+
+
+def lgf_version() -> str:
+    return load().lgf_version().decode()
+
+
+# C-style aliases with the header's names
+def lgf_create(dims, precision, link_storage):
+    return Context(dims, precision, link_storage)
+
+
+def lgf_destroy(ctx):
+    ctx.destroy()
+
+
+def lgf_iterate(ctx, alpha, n):
+    ctx.iterate(alpha, n)
+
+
+def lgf_measure(ctx):
+    return ctx.measure()
+
+
+def lgf_fix(ctx, links, alpha, tol, max_iter):
+    return ctx.fix(links, alpha, tol, max_iter)

@@ -1,0 +1,582 @@
+// lgf_api.cu -- the C ABI of liblgf (include/lgf.h): context, device buffers, tables, the FFT pass
+// plan and the Algorithm-1 driver.  Part of the CUDA path; shares nothing with
+// oracle/.  There is no CPU fallback anywhere in this file: without a CUDA device lgf_create fails.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/lgf.h"
+#include "lgf_state.cuh"
+
+using namespace lgf;
+
+struct lgf_ctx {
+    Geom g{};
+    int prec = 0;        // bytes per real
+    int nr = 3;          // stored rows per link
+    cudaStream_t stream = nullptr;
+    void *links = nullptr;       // C<R>[4][3*nr][V]
+    void *W = nullptr;           // C<R>[4][V]
+    double *partial = nullptr;   // per-block partial sums
+    int partial_cap = 0;
+    DevState *st = nullptr;
+    DevState *h_st = nullptr;    // pinned mirror
+    double *hist = nullptr;      // (F, theta) pairs
+    long long hist_cap = 0;
+    double *d_scalar = nullptr;
+    void *twiddle[4] = {nullptr, nullptr, nullptr, nullptr};   // C<R>[64] per axis, exp(-2 pi i m / L_mu)
+    void *p2tab = nullptr;                                     // R[4][64]
+    void *staging = nullptr;     // canonical-layout device buffer for the *_host entry points
+    std::vector<AxisPass> passes;
+    bool have_links = false;
+    bool profiling = false;
+    struct Stamp { cudaEvent_t a, b; int cls; };
+    std::vector<Stamp> stamps;
+    double prof_ms[LGF_K_COUNT] = {0};
+    long long prof_n[LGF_K_COUNT] = {0};
+    long long launches = 0;
+    std::string err;
+};
+
+static thread_local std::string g_err;   // errors with no context (lgf_create failures)
+
+static int fail(lgf_ctx *ctx, int code, const std::string &msg) {
+    if (ctx) ctx->err = msg;
+    g_err = msg;
+    return code;
+}
+static int cuda_fail(lgf_ctx *ctx, cudaError_t e, const char *what) {
+    return fail(ctx, e == cudaErrorMemoryAllocation ? LGF_ENOMEM : LGF_ECUDA,
+                std::string(what) + ": " + cudaGetErrorString(e));
+}
+#define CK(call)                                                     \
+    do {                                                             \
+        cudaError_t e_ = (call);                                     \
+        if (e_ != cudaSuccess) return cuda_fail(ctx, e_, #call);     \
+    } while (0)
+
+// ---- host-side tables -----------------------------------------------------------------------------
+static bool valid_len(int L) {
+    static const int ok[] = {2, 3, 4, 6, 8, 12, 16, 24, 32, 48, 64};
+    for (int v : ok) if (v == L) return true;
+    return false;
+}
+static void line_factor(int L, int &N1, int &N2) {     // must agree with lgf::LineFactor<L>
+    N1 = (L <= 8) ? L : ((L % 8 == 0) ? 8 : ((L % 4 == 0) ? 4 : ((L % 6 == 0) ? 6 : 3)));
+    N2 = L / N1;
+}
+// cos and sin of 2 pi m / L by exact octant reduction of the fraction, then libm in long double
+static void cossin_2pi(int m, int L, double &c, double &s) {
+    long num = 8L * (m % L), den = 8L * L;
+    double sc = 1.0, ss = 1.0;
+    bool swap = false;
+    if (2 * num > den) { num = den - num; ss = -ss; }
+    if (4 * num > den) { num = den / 2 - num; sc = -sc; }
+    if (8 * num > den) { num = den / 4 - num; swap = true; }
+    const long double x = 2.0L * 3.14159265358979323846264338327950288L * (long double)num / (long double)den;
+    long double cc = cosl(x), sv = sinl(x);
+    if (8 * num == den) { cc = 0.70710678118654752440084436210484904L; sv = cc; }
+    if (num == 0) { cc = 1.0L; sv = 0.0L; }
+    if (swap) { const long double t = cc; cc = sv; sv = t; }
+    c = sc * (double)cc;
+    s = ss * (double)sv;
+}
+
+template <class R>
+static int upload_tables(lgf_ctx *ctx) {
+    std::vector<R> p2(4 * 64, (R)0);
+    for (int mu = 0; mu < 4; mu++) {
+        const int L = ctx->g.L[mu];
+        std::vector<R> tw(2 * 64, (R)0);
+        for (int m = 0; m < L; m++) {
+            double c, s;
+            cossin_2pi(m, L, c, s);
+            tw[2 * m] = (R)c;
+            tw[2 * m + 1] = (R)(-s);                      // forward sign e^{-i}
+        }
+        CK(cudaMalloc(&ctx->twiddle[mu], sizeof(R) * 2 * 64));
+        CK(cudaMemcpy(ctx->twiddle[mu], tw.data(), sizeof(R) * 2 * 64, cudaMemcpyHostToDevice));
+        int N1, N2;
+        line_factor(L, N1, N2);
+        for (int p = 0; p < L; p++) {
+            const int k = (p / N2) + N1 * (p % N2);       // frequency held at position p (lgf_fft.cu header)
+            // 4 sin^2(pi k / L) = 2 (1 - cos(2 pi k / L))   -- use sin of the half angle for accuracy
+            double c, s;
+            cossin_2pi(k, 2 * L, c, s);                   // angle 2 pi k / (2L) = pi k / L
+            p2[mu * 64 + p] = (R)(4.0 * s * s);
+        }
+    }
+    CK(cudaMalloc(&ctx->p2tab, sizeof(R) * 4 * 64));
+    CK(cudaMemcpy(ctx->p2tab, p2.data(), sizeof(R) * 4 * 64, cudaMemcpyHostToDevice));
+    return LGF_OK;
+}
+
+static long long largest_divisor_le(long long n, long long cap) {
+    if (cap < 1) cap = 1;
+    for (long long d = (cap < n ? cap : n); d >= 1; d--)
+        if (n % d == 0) return d;
+    return 1;
+}
+
+// One pass per axis: forward x, y, z; forward + scale + inverse on t; inverse z, y, x.
+static void plan_passes(lgf_ctx *ctx) {
+    const long long T = 2048;     // target complex elements per tile
+    const size_t cbytes = 2 * (size_t)ctx->prec;
+    auto make = [&](int axis, int mode) {
+        AxisPass p{};
+        p.axis = axis;
+        p.L = ctx->g.L[axis];
+        p.mode = mode;
+        p.S = ctx->g.S[axis];
+        p.H = ctx->g.V / (p.S * p.L);
+        if (p.S == 1) {
+            p.nlo = 1;
+            p.nhi = (int)largest_divisor_le(p.H, T / p.L);
+            p.smem = (64 + (size_t)p.nhi * (p.L | 1)) * cbytes;
+        } else {
+            p.nlo = (int)largest_divisor_le(p.S, T / p.L);
+            p.nhi = (int)largest_divisor_le(p.H, T / ((long long)p.L * p.nlo));
+            p.smem = (64 + (size_t)p.nhi * p.L * p.nlo) * cbytes;
+        }
+        p.threads = 256;
+        return p;
+    };
+    ctx->passes.clear();
+    for (int a = 0; a < 3; a++) ctx->passes.push_back(make(a, FFT_FWD));
+    ctx->passes.push_back(make(3, FFT_FWD_SCALE_INV));
+    for (int a = 2; a >= 0; a--) ctx->passes.push_back(make(a, FFT_INV));
+}
+
+// ---- profiling brackets ---------------------------------------------------------------------------
+struct Bracket {
+    lgf_ctx *ctx;
+    int cls;
+    cudaEvent_t a = nullptr, b = nullptr;
+    Bracket(lgf_ctx *c, int k) : ctx(c), cls(k) {
+        ctx->launches++;
+        if (ctx->profiling) {
+            cudaEventCreate(&a);
+            cudaEventCreate(&b);
+            cudaEventRecord(a, ctx->stream);
+        }
+    }
+    ~Bracket() {
+        if (a) {
+            cudaEventRecord(b, ctx->stream);
+            ctx->stamps.push_back({a, b, cls});
+        }
+    }
+};
+static void drain_stamps(lgf_ctx *ctx) {
+    for (auto &s : ctx->stamps) {
+        float ms = 0.f;
+        if (cudaEventSynchronize(s.b) == cudaSuccess && cudaEventElapsedTime(&ms, s.a, s.b) == cudaSuccess) {
+            ctx->prof_ms[s.cls] += ms;
+            ctx->prof_n[s.cls] += 1;
+        }
+        cudaEventDestroy(s.a);
+        cudaEventDestroy(s.b);
+    }
+    ctx->stamps.clear();
+}
+
+// ---- typed steps ----------------------------------------------------------------------------------
+template <class R>
+static int step_delta(lgf_ctx *ctx, const int *stop, int *nblocks) {
+    Bracket br(ctx, LGF_K_DELTA);
+    CK(launch_delta<R>(ctx->nr, (const C<R> *)ctx->links, (C<R> *)ctx->W, ctx->g, ctx->partial, nblocks, stop,
+                       ctx->stream));
+    return LGF_OK;
+}
+template <class R>
+static int step_accelerate(lgf_ctx *ctx) {
+    const R scale = (R)(16.0 / (double)ctx->g.V);        // p2max / V      (Alg. 1 lines 5, 7; R5, R7)
+    for (const AxisPass &p : ctx->passes) {
+        Bracket br(ctx, LGF_K_FFT);
+        CK(launch_fft_pass<R>(p, (C<R> *)ctx->W, ctx->g, (const R *)ctx->twiddle[p.axis], (const R *)ctx->p2tab, scale,
+                              ctx->st, ctx->stream));
+    }
+    return LGF_OK;
+}
+template <class R>
+static int step_update(lgf_ctx *ctx, double alpha) {
+    Bracket br(ctx, LGF_K_UPDATE);
+    CK(launch_update<R>(ctx->nr, (C<R> *)ctx->links, (const C<R> *)ctx->W, ctx->g, (R)(0.5 * alpha), ctx->st,
+                        ctx->stream));
+    return LGF_OK;
+}
+static int step_finalize(lgf_ctx *ctx, int nblocks, double tol, int will_update, int record) {
+    ctx->launches++;
+    CK(launch_finalize(ctx->partial, nblocks, ctx->g.V, tol, will_update, record, ctx->st, ctx->hist, ctx->hist_cap,
+                       ctx->stream));
+    return LGF_OK;
+}
+
+// measure (a1 + finalize, recorded) then, unless stopped, accelerate and update: one pass of the
+// while-body of Algorithm 1 preceded by its loop test.
+template <class R>
+static int iteration(lgf_ctx *ctx, double alpha, double tol) {
+    int nb = 0, rc;
+    if ((rc = step_delta<R>(ctx, &ctx->st->done, &nb)) != LGF_OK) return rc;
+    if ((rc = step_finalize(ctx, nb, tol, 1, 1)) != LGF_OK) return rc;
+    if ((rc = step_accelerate<R>(ctx)) != LGF_OK) return rc;
+    return step_update<R>(ctx, alpha);
+}
+template <class R>
+static int measure_only(lgf_ctx *ctx, double tol, int record) {
+    int nb = 0, rc;
+    if ((rc = step_delta<R>(ctx, record ? &ctx->st->done : &ctx->st->zero, &nb)) != LGF_OK) return rc;
+    return step_finalize(ctx, nb, tol, 0, record);
+}
+
+#define DISPATCH(fn, ...) (ctx->prec == LGF_FP64 ? fn<double>(__VA_ARGS__) : fn<float>(__VA_ARGS__))
+
+static int fetch_state(lgf_ctx *ctx) {
+    CK(cudaMemcpyAsync(ctx->h_st, ctx->st, sizeof(DevState), cudaMemcpyDeviceToHost, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    return LGF_OK;
+}
+
+// ---- C ABI ----------------------------------------------------------------------------------------
+extern "C" {
+
+const char *lgf_version(void) { return "liblgf 0.1 (sm_100a)"; }
+
+const char *lgf_last_error(const lgf_ctx *ctx) { return ctx ? ctx->err.c_str() : g_err.c_str(); }
+
+int lgf_create(const int dims[4], int precision, int link_storage, lgf_ctx **out) {
+    if (!dims || !out) return fail(nullptr, LGF_EINVAL, "lgf_create: null argument");
+    *out = nullptr;
+    if (precision != LGF_FP32 && precision != LGF_FP64) return fail(nullptr, LGF_EINVAL, "lgf_create: bad precision");
+    if (link_storage != LGF_LINKS_18 && link_storage != LGF_LINKS_12)
+        return fail(nullptr, LGF_EINVAL, "lgf_create: bad link_storage");
+    for (int mu = 0; mu < 4; mu++)
+        if (!valid_len(dims[mu])) return fail(nullptr, LGF_EINVAL, "lgf_create: unsupported lattice extent");
+    int ndev = 0;
+    cudaError_t e = cudaGetDeviceCount(&ndev);
+    if (e != cudaSuccess || ndev == 0) {
+        cudaGetLastError();
+        return fail(nullptr, LGF_ECUDA, "lgf_create: no CUDA device (liblgf has no CPU path)");
+    }
+    lgf_ctx *ctx = new (std::nothrow) lgf_ctx();
+    if (!ctx) return fail(nullptr, LGF_ENOMEM, "lgf_create: host allocation failed");
+    ctx->prec = precision;
+    ctx->nr = link_storage == LGF_LINKS_18 ? 3 : 2;
+    long long S = 1;
+    for (int mu = 0; mu < 4; mu++) { ctx->g.L[mu] = dims[mu]; ctx->g.S[mu] = S; S *= dims[mu]; }
+    ctx->g.V = S;
+    const size_t V = (size_t)S, cb = 2 * (size_t)precision;
+    int rc = LGF_OK;
+    auto alloc = [&](void **p, size_t bytes) {
+        if (rc != LGF_OK) return;
+        cudaError_t ee = cudaMalloc(p, bytes);
+        if (ee != cudaSuccess) rc = cuda_fail(ctx, ee, "cudaMalloc");
+    };
+    alloc(&ctx->links, V * 4 * 3 * ctx->nr * cb);
+    alloc(&ctx->W, V * 4 * cb);
+    ctx->partial_cap = (int)((V + 255) / 256) + 1;
+    alloc((void **)&ctx->partial, sizeof(double) * 2 * ctx->partial_cap);
+    alloc((void **)&ctx->st, sizeof(DevState));
+    ctx->hist_cap = 1 << 20;
+    alloc((void **)&ctx->hist, sizeof(double) * 2 * ctx->hist_cap);
+    alloc((void **)&ctx->d_scalar, sizeof(double) * 4);
+    if (rc == LGF_OK) {
+        cudaError_t ee = cudaMallocHost((void **)&ctx->h_st, sizeof(DevState) + 4 * sizeof(double));
+        if (ee != cudaSuccess) rc = cuda_fail(ctx, ee, "cudaMallocHost");
+    }
+    if (rc == LGF_OK) rc = precision == LGF_FP64 ? upload_tables<double>(ctx) : upload_tables<float>(ctx);
+    if (rc == LGF_OK) {
+        plan_passes(ctx);
+        cudaError_t ee = launch_reset_state(ctx->st, ctx->stream);
+        if (ee == cudaSuccess) ee = cudaStreamSynchronize(ctx->stream);
+        if (ee != cudaSuccess) rc = cuda_fail(ctx, ee, "reset_state");
+    }
+    if (rc != LGF_OK) {
+        g_err = ctx->err;
+        lgf_destroy(ctx);
+        return rc;
+    }
+    *out = ctx;
+    return LGF_OK;
+}
+
+int lgf_destroy(lgf_ctx *ctx) {
+    if (!ctx) return LGF_EINVAL;
+    cudaStreamSynchronize(ctx->stream);
+    drain_stamps(ctx);
+    cudaFree(ctx->links);
+    cudaFree(ctx->W);
+    cudaFree(ctx->partial);
+    cudaFree(ctx->st);
+    cudaFree(ctx->hist);
+    cudaFree(ctx->d_scalar);
+    cudaFree(ctx->p2tab);
+    cudaFree(ctx->staging);
+    for (int mu = 0; mu < 4; mu++) cudaFree(ctx->twiddle[mu]);
+    if (ctx->h_st) cudaFreeHost(ctx->h_st);
+    cudaGetLastError();
+    delete ctx;
+    return LGF_OK;
+}
+
+int lgf_set_stream(lgf_ctx *ctx, void *cuda_stream) {
+    if (!ctx) return LGF_EINVAL;
+    CK(cudaStreamSynchronize(ctx->stream));
+    ctx->stream = (cudaStream_t)cuda_stream;
+    return LGF_OK;
+}
+
+int lgf_set_links(lgf_ctx *ctx, const void *d_links) {
+    if (!ctx || !d_links) return fail(ctx, LGF_EINVAL, "lgf_set_links: null argument");
+    {
+        Bracket br(ctx, LGF_K_CONVERT);
+        if (ctx->prec == LGF_FP64)
+            CK(launch_convert_in<double>(ctx->nr, (const double *)d_links, (C<double> *)ctx->links, ctx->g, ctx->stream));
+        else
+            CK(launch_convert_in<float>(ctx->nr, (const float *)d_links, (C<float> *)ctx->links, ctx->g, ctx->stream));
+    }
+    CK(launch_reset_state(ctx->st, ctx->stream));
+    ctx->have_links = true;
+    return LGF_OK;
+}
+
+int lgf_get_links(lgf_ctx *ctx, void *d_links) {
+    if (!ctx || !d_links) return fail(ctx, LGF_EINVAL, "lgf_get_links: null argument");
+    if (!ctx->have_links) return fail(ctx, LGF_ESTATE, "lgf_get_links: no configuration loaded");
+    Bracket br(ctx, LGF_K_CONVERT);
+    if (ctx->prec == LGF_FP64)
+        CK(launch_convert_out<double>(ctx->nr, (const C<double> *)ctx->links, (double *)d_links, ctx->g, ctx->stream));
+    else
+        CK(launch_convert_out<float>(ctx->nr, (const C<float> *)ctx->links, (float *)d_links, ctx->g, ctx->stream));
+    return LGF_OK;
+}
+
+static int ensure_staging(lgf_ctx *ctx) {
+    if (!ctx->staging) CK(cudaMalloc(&ctx->staging, (size_t)ctx->g.V * 72 * ctx->prec));
+    return LGF_OK;
+}
+
+int lgf_set_links_host(lgf_ctx *ctx, const void *h_links) {
+    if (!ctx || !h_links) return fail(ctx, LGF_EINVAL, "lgf_set_links_host: null argument");
+    int rc = ensure_staging(ctx);
+    if (rc != LGF_OK) return rc;
+    CK(cudaMemcpyAsync(ctx->staging, h_links, (size_t)ctx->g.V * 72 * ctx->prec, cudaMemcpyHostToDevice, ctx->stream));
+    rc = lgf_set_links(ctx, ctx->staging);
+    if (rc != LGF_OK) return rc;
+    CK(cudaStreamSynchronize(ctx->stream));
+    return LGF_OK;
+}
+
+int lgf_get_links_host(lgf_ctx *ctx, void *h_links) {
+    if (!ctx || !h_links) return fail(ctx, LGF_EINVAL, "lgf_get_links_host: null argument");
+    int rc = ensure_staging(ctx);
+    if (rc != LGF_OK) return rc;
+    rc = lgf_get_links(ctx, ctx->staging);
+    if (rc != LGF_OK) return rc;
+    CK(cudaMemcpyAsync(h_links, ctx->staging, (size_t)ctx->g.V * 72 * ctx->prec, cudaMemcpyDeviceToHost, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    return LGF_OK;
+}
+
+int lgf_iterate(lgf_ctx *ctx, double alpha, int n) {
+    if (!ctx || n < 0) return fail(ctx, LGF_EINVAL, "lgf_iterate: bad argument");
+    if (!ctx->have_links) return fail(ctx, LGF_ESTATE, "lgf_iterate: no configuration loaded");
+    ctx->launches++;
+    CK(launch_clear_done(ctx->st, ctx->stream));
+    for (int i = 0; i < n; i++) {
+        // tol = -1: theta >= 0 never stops the loop; only a NaN does
+        const int rc = DISPATCH(iteration, ctx, alpha, -1.0);
+        if (rc != LGF_OK) return rc;
+    }
+    return LGF_OK;
+}
+
+int lgf_measure(lgf_ctx *ctx, double *F, double *theta, double *plaquette) {
+    if (!ctx) return LGF_EINVAL;
+    if (!ctx->have_links) return fail(ctx, LGF_ESTATE, "lgf_measure: no configuration loaded");
+    if (F || theta) {
+        const int rc = DISPATCH(measure_only, ctx, -1.0, 0);
+        if (rc != LGF_OK) return rc;
+    }
+    if (plaquette) {
+        int nb = 0;
+        {
+            Bracket br(ctx, LGF_K_PLAQ);
+            if (ctx->prec == LGF_FP64)
+                CK(launch_plaquette<double>(ctx->nr, (const C<double> *)ctx->links, ctx->g, ctx->partial, &nb, ctx->stream));
+            else
+                CK(launch_plaquette<float>(ctx->nr, (const C<float> *)ctx->links, ctx->g, ctx->partial, &nb, ctx->stream));
+        }
+        ctx->launches++;
+        CK(launch_sum1(ctx->partial, nb, 1.0 / (18.0 * (double)ctx->g.V), ctx->d_scalar, ctx->stream));
+        double *hp = reinterpret_cast<double *>(ctx->h_st + 1);
+        CK(cudaMemcpyAsync(hp, ctx->d_scalar, sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    }
+    const int rc = fetch_state(ctx);
+    if (rc != LGF_OK) return rc;
+    if (F) *F = ctx->h_st->F;
+    if (theta) *theta = ctx->h_st->theta;
+    if (plaquette) *plaquette = *reinterpret_cast<double *>(ctx->h_st + 1);
+    return LGF_OK;
+}
+
+// Algorithm 1 on the configuration already loaded in the context.
+static long long fix_loaded(lgf_ctx *ctx, double alpha, double tol, long long max_iter) {
+    const int CHUNK = 16;      // iterations enqueued between two looks at the device-side stop flag
+    long long issued = 0;
+    bool done = false;
+    while (issued < max_iter && !done) {
+        const long long n = (max_iter - issued < CHUNK) ? (max_iter - issued) : CHUNK;
+        for (long long i = 0; i < n; i++) {
+            const int rc = DISPATCH(iteration, ctx, alpha, tol);
+            if (rc != LGF_OK) return rc;
+        }
+        issued += n;
+        const int rc = fetch_state(ctx);
+        if (rc != LGF_OK) return rc;
+        done = ctx->h_st->done != 0;
+    }
+    if (!done) {               // Alg. 1 line 17 after the last update
+        int rc = DISPATCH(measure_only, ctx, tol, 1);
+        if (rc != LGF_OK) return rc;
+        if ((rc = fetch_state(ctx)) != LGF_OK) return rc;
+    }
+    if (ctx->h_st->nan) return fail(ctx, LGF_ENAN, "lgf_fix: theta is NaN/Inf");
+    return ctx->h_st->n_updates;
+}
+
+long long lgf_fix(lgf_ctx *ctx, void *d_links, double alpha, double tol, long long max_iter) {
+    if (!ctx || !d_links || max_iter < 0) return fail(ctx, LGF_EINVAL, "lgf_fix: bad argument");
+    int rc = lgf_set_links(ctx, d_links);
+    if (rc != LGF_OK) return rc;
+    const long long it = fix_loaded(ctx, alpha, tol, max_iter);
+    if (it < 0) return it;
+    if ((rc = lgf_get_links(ctx, d_links)) != LGF_OK) return rc;
+    CK(cudaStreamSynchronize(ctx->stream));
+    return it;
+}
+
+long long lgf_fix_host(lgf_ctx *ctx, void *h_links, double alpha, double tol, long long max_iter) {
+    if (!ctx || !h_links || max_iter < 0) return fail(ctx, LGF_EINVAL, "lgf_fix_host: bad argument");
+    int rc = lgf_set_links_host(ctx, h_links);
+    if (rc != LGF_OK) return rc;
+    const long long it = fix_loaded(ctx, alpha, tol, max_iter);
+    if (it < 0) return it;
+    if ((rc = lgf_get_links_host(ctx, h_links)) != LGF_OK) return rc;
+    return it;
+}
+
+int lgf_history(lgf_ctx *ctx, long long first, long long count, double *F, double *theta) {
+    if (!ctx || first < 0 || count < 0) return fail(ctx, LGF_EINVAL, "lgf_history: bad argument");
+    int rc = fetch_state(ctx);
+    if (rc != LGF_OK) return rc;
+    const long long have = ctx->h_st->n_hist < ctx->hist_cap ? ctx->h_st->n_hist : ctx->hist_cap;
+    if (first + count > have) return fail(ctx, LGF_EINVAL, "lgf_history: range beyond the recorded entries");
+    if (count == 0) return LGF_OK;
+    std::vector<double> buf(2 * (size_t)count);
+    CK(cudaMemcpyAsync(buf.data(), ctx->hist + 2 * first, sizeof(double) * 2 * count, cudaMemcpyDeviceToHost, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    for (long long i = 0; i < count; i++) {
+        if (F) F[i] = buf[2 * i];
+        if (theta) theta[i] = buf[2 * i + 1];
+    }
+    return LGF_OK;
+}
+
+long long lgf_iterations(lgf_ctx *ctx) {
+    if (!ctx) return LGF_EINVAL;
+    const int rc = fetch_state(ctx);
+    if (rc != LGF_OK) return rc;
+    return ctx->h_st->n_updates;
+}
+
+long long lgf_history_length(lgf_ctx *ctx) {
+    if (!ctx) return LGF_EINVAL;
+    const int rc = fetch_state(ctx);
+    if (rc != LGF_OK) return rc;
+    return ctx->h_st->n_hist;
+}
+
+int lgf_step_delta(lgf_ctx *ctx, double *F, double *theta) {
+    if (!ctx) return LGF_EINVAL;
+    if (!ctx->have_links) return fail(ctx, LGF_ESTATE, "lgf_step_delta: no configuration loaded");
+    int rc = DISPATCH(measure_only, ctx, -1.0, 0);
+    if (rc != LGF_OK) return rc;
+    if (F || theta) {
+        if ((rc = fetch_state(ctx)) != LGF_OK) return rc;
+        if (F) *F = ctx->h_st->F;
+        if (theta) *theta = ctx->h_st->theta;
+    }
+    return LGF_OK;
+}
+
+int lgf_step_accelerate(lgf_ctx *ctx) {
+    if (!ctx) return LGF_EINVAL;
+    ctx->launches++;
+    CK(launch_clear_done(ctx->st, ctx->stream));
+    return DISPATCH(step_accelerate, ctx);
+}
+
+int lgf_step_update(lgf_ctx *ctx, double alpha) {
+    if (!ctx) return LGF_EINVAL;
+    if (!ctx->have_links) return fail(ctx, LGF_ESTATE, "lgf_step_update: no configuration loaded");
+    ctx->launches++;
+    CK(launch_clear_done(ctx->st, ctx->stream));
+    return DISPATCH(step_update, ctx, alpha);
+}
+
+int lgf_get_field(lgf_ctx *ctx, void *d_field) {
+    if (!ctx || !d_field) return fail(ctx, LGF_EINVAL, "lgf_get_field: null argument");
+    ctx->launches++;
+    if (ctx->prec == LGF_FP64) CK(launch_field_get<double>((const C<double> *)ctx->W, (double *)d_field, ctx->g, ctx->stream));
+    else CK(launch_field_get<float>((const C<float> *)ctx->W, (float *)d_field, ctx->g, ctx->stream));
+    return LGF_OK;
+}
+
+int lgf_set_field(lgf_ctx *ctx, const void *d_field) {
+    if (!ctx || !d_field) return fail(ctx, LGF_EINVAL, "lgf_set_field: null argument");
+    ctx->launches++;
+    if (ctx->prec == LGF_FP64) CK(launch_field_set<double>((C<double> *)ctx->W, (const double *)d_field, ctx->g, ctx->stream));
+    else CK(launch_field_set<float>((C<float> *)ctx->W, (const float *)d_field, ctx->g, ctx->stream));
+    return LGF_OK;
+}
+
+int lgf_set_profiling(lgf_ctx *ctx, int on) {
+    if (!ctx) return LGF_EINVAL;
+    CK(cudaStreamSynchronize(ctx->stream));
+    drain_stamps(ctx);
+    ctx->profiling = on != 0;
+    for (int k = 0; k < LGF_K_COUNT; k++) { ctx->prof_ms[k] = 0.0; ctx->prof_n[k] = 0; }
+    return LGF_OK;
+}
+
+int lgf_kernel_times(lgf_ctx *ctx, double *ms, long long *launches) {
+    if (!ctx) return LGF_EINVAL;
+    CK(cudaStreamSynchronize(ctx->stream));
+    drain_stamps(ctx);
+    for (int k = 0; k < LGF_K_COUNT; k++) {
+        if (ms) ms[k] = ctx->prof_ms[k];
+        if (launches) launches[k] = ctx->prof_n[k];
+    }
+    return LGF_OK;
+}
+
+long long lgf_launch_count(const lgf_ctx *ctx) { return ctx ? ctx->launches : LGF_EINVAL; }
+
+double lgf_algorithmic_bytes(const lgf_ctx *ctx, int kernel_class) {
+    if (!ctx) return 0.0;
+    const double V = (double)ctx->g.V, R = (double)ctx->prec, nl = 6.0 * ctx->nr;
+    switch (kernel_class) {
+        case LGF_K_DELTA: return V * (4.0 * nl + 8.0) * R;        // read 4 links, write packed Delta
+        case LGF_K_FFT: return V * 3.0 * 16.0 * R;                // three read+write sweeps of the packed field
+        case LGF_K_UPDATE: return V * (8.0 + 8.0 * nl) * R;       // read w and 4 links, write 4 links
+        case LGF_K_PLAQ: return V * 4.0 * nl * R;
+        case LGF_K_CONVERT: return V * (72.0 + 4.0 * nl) * R;
+        default: return 0.0;
+    }
+}
+
+}  // extern "C"

@@ -1,0 +1,284 @@
+// lgf_links.cu -- the link-side kernels of the gauge-fixing iteration:
+//   k_delta     a1: A_mu, Delta(x), per-block partial sums for F and theta   (eqs. 3, 5-7; Alg. 1 lines 1, 17)
+//   k_update    a5 + a6: g(x) = GS(1 + i (alpha/2) w(x)),  U_mu(x) <- g(x) U_mu(x) g(x+mu)^dag   (Alg. 1 lines 10, 14)
+//   k_plaquette average plaquette partial sums (gauge-invariant check)
+//   k_finalize  final fixed-order sum, F / theta normalisation, history, stop test (Alg. 1 line 2)
+//   layout conversion canonical AoS <-> internal SoA, packed field <-> full 3x3 field
+// Part of liblgf (CUDA path).  Shares nothing with oracle/.
+#include "lgf_state.cuh"
+
+namespace lgf {
+
+constexpr int SITE_THREADS = 256;
+
+// ---- a1 -------------------------------------------------------------------------------------------
+template <class R, int NR>
+__global__ void __launch_bounds__(SITE_THREADS) k_delta(const C<R> *__restrict__ links, C<R> *__restrict__ W, Geom g,
+                                                         double *__restrict__ partial,
+                                                         const int *__restrict__ stop) {
+    if (*stop) return;
+    __shared__ double scratch[SITE_THREADS / 32][2];
+    const long long s = (long long)blockIdx.x * SITE_THREADS + threadIdx.x;
+    double f = 0.0, t = 0.0;
+    if (s < g.V) {
+        int c[4];
+        site_coords(g, s, c);
+        Herm<R> d = herm_zero<R>();
+        R retr = 0;
+#pragma unroll
+        for (int mu = 0; mu < 4; mu++) {
+            C<R> u[9];
+            load_link<R, NR>(links, g.V, mu, s, u);
+            retr += u[0].x + u[4].x + u[8].x;                       // eq. 3: Re tr U_mu(x)
+            herm_sub(d, algebra_part(u));                           // - A_mu(x)
+            load_link<R, NR>(links, g.V, mu, site_bwd(g, s, c, mu), u);
+            herm_add(d, algebra_part(u));                           // + A_mu(x - mu)      (eq. 5)
+        }
+        store_herm(W, g.V, s, d);
+        f = (double)retr;
+        t = (double)herm_norm2(d);                                  // eq. 6: tr(Delta Delta^dag)
+    }
+    block_sum2(f, t, scratch);
+    if (threadIdx.x == 0) {
+        partial[2 * blockIdx.x] = f;
+        partial[2 * blockIdx.x + 1] = t;
+    }
+}
+
+// ---- a5 + a6 --------------------------------------------------------------------------------------
+template <class R, int NR>
+__global__ void __launch_bounds__(SITE_THREADS) k_update(C<R> *__restrict__ links, const C<R> *__restrict__ W, Geom g,
+                                                          R half_alpha, const DevState *__restrict__ st) {
+    if (st->done) return;
+    const long long s = (long long)blockIdx.x * SITE_THREADS + threadIdx.x;
+    if (s >= g.V) return;
+    int c[4];
+    site_coords(g, s, c);
+    C<R> gx[9];
+    build_g(load_herm(W, g.V, s), half_alpha, gx);
+#pragma unroll
+    for (int mu = 0; mu < 4; mu++) {
+        C<R> gf[9], u[9], tmp[9], r[9];
+        build_g(load_herm(W, g.V, site_fwd(g, s, c, mu)), half_alpha, gf);
+        load_link<R, NR>(links, g.V, mu, s, u);
+        mat_mul<NR>(gx, u, tmp);
+        mat_mul_dag<NR>(tmp, gf, r);
+        store_link<R, NR>(links, g.V, mu, s, r);
+    }
+}
+
+// ---- plaquette ------------------------------------------------------------------------------------
+template <class R, int NR>
+__global__ void __launch_bounds__(SITE_THREADS) k_plaquette(const C<R> *__restrict__ links, Geom g,
+                                                             double *__restrict__ partial) {
+    __shared__ double scratch[SITE_THREADS / 32][2];
+    const long long s = (long long)blockIdx.x * SITE_THREADS + threadIdx.x;
+    double p = 0.0, dummy = 0.0;
+    if (s < g.V) {
+        int c[4];
+        site_coords(g, s, c);
+        R acc = 0;
+        for (int mu = 0; mu < 4; mu++)
+            for (int nu = mu + 1; nu < 4; nu++) {
+                C<R> a[9], b[9], t1[9], t2[9];
+                load_link<R, NR>(links, g.V, mu, s, a);
+                load_link<R, NR>(links, g.V, nu, site_fwd(g, s, c, mu), b);
+                mat_mul<3>(a, b, t1);                                   // U_mu(x) U_nu(x+mu)
+                load_link<R, NR>(links, g.V, mu, site_fwd(g, s, c, nu), a);
+                mat_mul_dag<3>(t1, a, t2);                              // ... U_mu(x+nu)^dag
+                load_link<R, NR>(links, g.V, nu, s, b);
+                // Re tr(t2 b^dag) = sum_ij Re(t2_ij conj(b_ij))
+#pragma unroll
+                for (int e = 0; e < 9; e++) acc += t2[e].x * b[e].x + t2[e].y * b[e].y;
+            }
+        p = (double)acc;
+    }
+    block_sum2(p, dummy, scratch);
+    if (threadIdx.x == 0) partial[blockIdx.x] = p;
+}
+
+// ---- reductions' last stage -----------------------------------------------------------------------
+// One block; fixed summation order (thread i takes partials i, i+1024, ...), so F and theta are
+// bit-reproducible from run to run.
+__global__ void __launch_bounds__(1024) k_finalize(const double *__restrict__ partial, int nblocks, long long V,
+                                                    double tol, int will_update, int record, DevState *st,
+                                                    double *__restrict__ hist, long long hist_cap) {
+    if (record && st->done) return;
+    __shared__ double scratch[32][2];
+    double f = 0.0, t = 0.0;
+    for (int i = threadIdx.x; i < nblocks; i += 1024) {
+        f += partial[2 * i];
+        t += partial[2 * i + 1];
+    }
+    block_sum2(f, t, scratch);
+    if (threadIdx.x == 0) {
+        const double F = f / (12.0 * (double)V);          // eq. 3: 1 / (4 N_c V)
+        const double theta = t / (3.0 * (double)V);       // eq. 6: 1 / (N_c V)
+        st->F = F;
+        st->theta = theta;
+        if (record) {
+            const long long n = st->n_hist;
+            if (n < hist_cap) { hist[2 * n] = F; hist[2 * n + 1] = theta; }
+            st->n_hist = n + 1;
+            if (!(theta == theta) || theta > 1e300) { st->done = 1; st->nan = 1; }
+            else if (theta < tol) st->done = 1;           // Alg. 1 line 2: loop while theta >= eps
+            else if (will_update) st->n_updates += 1;
+        }
+    }
+}
+
+__global__ void __launch_bounds__(1024) k_sum1(const double *__restrict__ partial, int nblocks, double norm,
+                                                double *out) {
+    __shared__ double scratch[32][2];
+    double f = 0.0, t = 0.0;
+    for (int i = threadIdx.x; i < nblocks; i += 1024) f += partial[i];
+    block_sum2(f, t, scratch);
+    if (threadIdx.x == 0) *out = f * norm;
+}
+
+__global__ void k_reset_state(DevState *st) {
+    st->n_hist = 0; st->n_updates = 0; st->done = 0; st->nan = 0; st->F = 0.0; st->theta = 0.0; st->zero = 0;
+}
+__global__ void k_clear_done(DevState *st) { st->done = 0; }
+
+// ---- layout conversion ----------------------------------------------------------------------------
+// canonical: canon[((s*4 + mu)*9 + e)*2 + re/im]      (include/lgf.h)
+template <class R, int NR>
+__global__ void __launch_bounds__(SITE_THREADS) k_convert_in(const R *__restrict__ canon, C<R> *__restrict__ links,
+                                                              Geom g) {
+    const long long s = (long long)blockIdx.x * SITE_THREADS + threadIdx.x;
+    if (s >= g.V) return;
+    const C<R> *src = reinterpret_cast<const C<R> *>(canon) + s * 36;
+#pragma unroll
+    for (int mu = 0; mu < 4; mu++)
+#pragma unroll
+        for (int e = 0; e < 3 * NR; e++) links[((long long)mu * (3 * NR) + e) * g.V + s] = src[mu * 9 + e];
+}
+template <class R, int NR>
+__global__ void __launch_bounds__(SITE_THREADS) k_convert_out(const C<R> *__restrict__ links, R *__restrict__ canon,
+                                                               Geom g) {
+    const long long s = (long long)blockIdx.x * SITE_THREADS + threadIdx.x;
+    if (s >= g.V) return;
+    C<R> *dst = reinterpret_cast<C<R> *>(canon) + s * 36;
+#pragma unroll
+    for (int mu = 0; mu < 4; mu++) {
+        C<R> u[9];
+        load_link<R, NR>(links, g.V, mu, s, u);
+#pragma unroll
+        for (int e = 0; e < 9; e++) dst[mu * 9 + e] = u[e];
+    }
+}
+
+// packed hermitian traceless field <-> full 3x3 field  field[(s*9 + e)*2 + re/im]
+template <class R>
+__global__ void __launch_bounds__(SITE_THREADS) k_field_get(const C<R> *__restrict__ W, R *__restrict__ field, Geom g) {
+    const long long s = (long long)blockIdx.x * SITE_THREADS + threadIdx.x;
+    if (s >= g.V) return;
+    const Herm<R> h = load_herm(W, g.V, s);
+    C<R> *dst = reinterpret_cast<C<R> *>(field) + s * 9;
+    dst[0] = mk<R>(h.m00, 0); dst[1] = h.m01; dst[2] = h.m02;
+    dst[3] = conj(h.m01); dst[4] = mk<R>(h.m11, 0); dst[5] = h.m12;
+    dst[6] = conj(h.m02); dst[7] = conj(h.m12); dst[8] = mk<R>(-h.m00 - h.m11, 0);
+}
+template <class R>
+__global__ void __launch_bounds__(SITE_THREADS) k_field_set(C<R> *__restrict__ W, const R *__restrict__ field, Geom g) {
+    const long long s = (long long)blockIdx.x * SITE_THREADS + threadIdx.x;
+    if (s >= g.V) return;
+    const C<R> *m = reinterpret_cast<const C<R> *>(field) + s * 9;
+    // hermitian traceless part of m: (m + m^dag)/2 - tr/3
+    Herm<R> h;
+    const R hf = (R)0.5;
+    h.m01 = hf * (m[1] + conj(m[3]));
+    h.m02 = hf * (m[2] + conj(m[6]));
+    h.m12 = hf * (m[5] + conj(m[7]));
+    const R tr3 = (m[0].x + m[4].x + m[8].x) * (R)(1.0 / 3.0);
+    h.m00 = m[0].x - tr3;
+    h.m11 = m[4].x - tr3;
+    store_herm(W, g.V, s, h);
+}
+
+// ---- launchers ------------------------------------------------------------------------------------
+static inline int site_blocks(const Geom &g) { return (int)((g.V + SITE_THREADS - 1) / SITE_THREADS); }
+
+template <class R>
+cudaError_t launch_delta(int nr, const C<R> *links, C<R> *W, const Geom &g, double *partial, int *nblocks,
+                         const int *stop, cudaStream_t stream) {
+    const int nb = site_blocks(g);
+    *nblocks = nb;
+    if (nr == 3) k_delta<R, 3><<<nb, SITE_THREADS, 0, stream>>>(links, W, g, partial, stop);
+    else k_delta<R, 2><<<nb, SITE_THREADS, 0, stream>>>(links, W, g, partial, stop);
+    return cudaGetLastError();
+}
+template <class R>
+cudaError_t launch_update(int nr, C<R> *links, const C<R> *W, const Geom &g, R half_alpha, const DevState *st,
+                          cudaStream_t stream) {
+    const int nb = site_blocks(g);
+    if (nr == 3) k_update<R, 3><<<nb, SITE_THREADS, 0, stream>>>(links, W, g, half_alpha, st);
+    else k_update<R, 2><<<nb, SITE_THREADS, 0, stream>>>(links, W, g, half_alpha, st);
+    return cudaGetLastError();
+}
+template <class R>
+cudaError_t launch_plaquette(int nr, const C<R> *links, const Geom &g, double *partial, int *nblocks,
+                             cudaStream_t stream) {
+    const int nb = site_blocks(g);
+    *nblocks = nb;
+    if (nr == 3) k_plaquette<R, 3><<<nb, SITE_THREADS, 0, stream>>>(links, g, partial);
+    else k_plaquette<R, 2><<<nb, SITE_THREADS, 0, stream>>>(links, g, partial);
+    return cudaGetLastError();
+}
+template <class R>
+cudaError_t launch_convert_in(int nr, const R *canon, C<R> *links, const Geom &g, cudaStream_t stream) {
+    const int nb = site_blocks(g);
+    if (nr == 3) k_convert_in<R, 3><<<nb, SITE_THREADS, 0, stream>>>(canon, links, g);
+    else k_convert_in<R, 2><<<nb, SITE_THREADS, 0, stream>>>(canon, links, g);
+    return cudaGetLastError();
+}
+template <class R>
+cudaError_t launch_convert_out(int nr, const C<R> *links, R *canon, const Geom &g, cudaStream_t stream) {
+    const int nb = site_blocks(g);
+    if (nr == 3) k_convert_out<R, 3><<<nb, SITE_THREADS, 0, stream>>>(links, canon, g);
+    else k_convert_out<R, 2><<<nb, SITE_THREADS, 0, stream>>>(links, canon, g);
+    return cudaGetLastError();
+}
+template <class R>
+cudaError_t launch_field_get(const C<R> *W, R *field, const Geom &g, cudaStream_t stream) {
+    k_field_get<R><<<site_blocks(g), SITE_THREADS, 0, stream>>>(W, field, g);
+    return cudaGetLastError();
+}
+template <class R>
+cudaError_t launch_field_set(C<R> *W, const R *field, const Geom &g, cudaStream_t stream) {
+    k_field_set<R><<<site_blocks(g), SITE_THREADS, 0, stream>>>(W, field, g);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_finalize(const double *partial, int nblocks, long long V, double tol, int will_update, int record,
+                            DevState *st, double *hist, long long hist_cap, cudaStream_t stream) {
+    k_finalize<<<1, 1024, 0, stream>>>(partial, nblocks, V, tol, will_update, record, st, hist, hist_cap);
+    return cudaGetLastError();
+}
+cudaError_t launch_sum1(const double *partial, int nblocks, double norm, double *out, cudaStream_t stream) {
+    k_sum1<<<1, 1024, 0, stream>>>(partial, nblocks, norm, out);
+    return cudaGetLastError();
+}
+cudaError_t launch_reset_state(DevState *st, cudaStream_t stream) {
+    k_reset_state<<<1, 1, 0, stream>>>(st);
+    return cudaGetLastError();
+}
+cudaError_t launch_clear_done(DevState *st, cudaStream_t stream) {
+    k_clear_done<<<1, 1, 0, stream>>>(st);
+    return cudaGetLastError();
+}
+
+#define LGF_INST(R)                                                                                                   \
+    template cudaError_t launch_delta<R>(int, const C<R> *, C<R> *, const Geom &, double *, int *, const int *,        \
+                                         cudaStream_t);                                                                \
+    template cudaError_t launch_update<R>(int, C<R> *, const C<R> *, const Geom &, R, const DevState *, cudaStream_t); \
+    template cudaError_t launch_plaquette<R>(int, const C<R> *, const Geom &, double *, int *, cudaStream_t);          \
+    template cudaError_t launch_convert_in<R>(int, const R *, C<R> *, const Geom &, cudaStream_t);                     \
+    template cudaError_t launch_convert_out<R>(int, const C<R> *, R *, const Geom &, cudaStream_t);                    \
+    template cudaError_t launch_field_get<R>(const C<R> *, R *, const Geom &, cudaStream_t);                           \
+    template cudaError_t launch_field_set<R>(C<R> *, const R *, const Geom &, cudaStream_t);
+LGF_INST(float)
+LGF_INST(double)
+
+}  // namespace lgf

@@ -1,0 +1,66 @@
+// lgf_state.cuh -- device-resident control block of one context and the launch-side declarations
+// shared by the translation units of liblgf.  Part of the CUDA path; shares nothing with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include "lgf_su3.cuh"
+
+namespace lgf {
+
+// Lives in device memory; written only by k_finalize / k_reset, read by every kernel of the
+// iteration so that Algorithm 1's "while theta >= eps" needs no host round trip:
+// once `done` is set every later kernel of the enqueued iterations returns immediately.
+struct DevState {
+    long long n_hist;     // (F, theta) entries recorded since the last set_links
+    long long n_updates;  // link updates applied since the last set_links
+    int done;             // theta < tol seen (or NaN)
+    int nan;              // theta was NaN / Inf
+    double F, theta;      // last measured values
+    int zero;             // always 0: the `stop` word handed to kernels that must run regardless of `done`
+};
+
+enum FftMode { FFT_FWD = 0, FFT_INV = 1, FFT_FWD_SCALE_INV = 2 };
+
+// One FFT pass over one lattice axis (see lgf_fft.cu).
+struct AxisPass {
+    int axis;             // 0..3
+    int L;                // length of that axis
+    int mode;             // FftMode
+    long long S;          // global stride of the axis (elements)
+    long long H;          // number of "hi" blocks: V / (S * L)
+    int nlo, nhi;         // tile extents: nlo consecutive "lo" indices (lo < S), nhi "hi" indices
+    int threads;
+    size_t smem;
+};
+
+// launchers implemented in the .cu files (R = float / double)
+template <class R>
+cudaError_t launch_fft_pass(const AxisPass &p, C<R> *W, const Geom &g, const R *twiddle /*[2*L]*/,
+                            const R *p2tab /*[4][64] permuted 4 sin^2*/, R scale, const DevState *st,
+                            cudaStream_t stream);
+
+template <class R>
+cudaError_t launch_delta(int nr, const C<R> *links, C<R> *W, const Geom &g, double *partial, int *nblocks,
+                         const int *stop, cudaStream_t stream);
+template <class R>
+cudaError_t launch_update(int nr, C<R> *links, const C<R> *W, const Geom &g, R half_alpha, const DevState *st,
+                          cudaStream_t stream);
+template <class R>
+cudaError_t launch_plaquette(int nr, const C<R> *links, const Geom &g, double *partial, int *nblocks,
+                             cudaStream_t stream);
+template <class R>
+cudaError_t launch_convert_in(int nr, const R *canon, C<R> *links, const Geom &g, cudaStream_t stream);
+template <class R>
+cudaError_t launch_convert_out(int nr, const C<R> *links, R *canon, const Geom &g, cudaStream_t stream);
+template <class R>
+cudaError_t launch_field_get(const C<R> *W, R *field, const Geom &g, cudaStream_t stream);
+template <class R>
+cudaError_t launch_field_set(C<R> *W, const R *field, const Geom &g, cudaStream_t stream);
+
+// F / theta finalisation (precision independent)
+cudaError_t launch_finalize(const double *partial, int nblocks, long long V, double tol, int will_update, int record,
+                            DevState *st, double *hist, long long hist_cap, cudaStream_t stream);
+cudaError_t launch_sum1(const double *partial, int nblocks, double norm, double *out, cudaStream_t stream);
+cudaError_t launch_reset_state(DevState *st, cudaStream_t stream);
+cudaError_t launch_clear_done(DevState *st, cudaStream_t stream);
+
+}  // namespace lgf

@@ -1,0 +1,257 @@
+"""Parity of the CUDA path (through the C ABI of liblgf.so) with the CPU oracle, element by element
+on the same seeded inputs.  Tolerances are those BASELINE.json's north_star states:
+  per-iteration F and theta over the first 20 iterations: relative 1e-12 (fp64) / 1e-5 (fp32)
+  links after 20 iterations: max abs 1e-11 (fp64) / 2e-5 (fp32)
+  iterations to theta < 1e-15 (fp64): within 2 % of the oracle's count
+Every test here needs a GPU (-m gpu)."""
+import numpy as np
+import pytest
+
+import oracle
+from paper_1206_0675_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+ALPHA = 0.08
+TOL = {8: dict(scalar=1e-12, links=1e-11, field=1e-12), 4: dict(scalar=1e-5, links=2e-5, field=2e-5)}
+
+
+@pytest.fixture(scope="module")
+def lgf():
+    import torch
+
+    if not torch.cuda.is_available():
+        pytest.fail("no CUDA device: the gpu-marked tests must run on the B200 box")
+    from paper_1206_0675_b200 import binding
+
+    binding.load()
+    return binding
+
+
+def to_dev(a, prec):
+    import torch
+
+    cdt = torch.complex128 if prec == 8 else torch.complex64
+    return torch.from_numpy(np.ascontiguousarray(a)).to(cdt).cuda()
+
+
+def to_np(t):
+    return t.cpu().numpy().astype(np.complex128)
+
+
+def site_shape(dims):
+    return (dims[3], dims[2], dims[1], dims[0])
+
+
+def random_herm_field(dims, seed):
+    """Seeded hermitian traceless 3x3 field (input generator only: no method arithmetic)."""
+    V = int(np.prod(dims))
+    c = inputs.normals(seed, 7, 0, V * 8).reshape(V, 8).astype(np.complex128)
+    H = np.einsum("na,aij->nij", c, inputs.gell_mann())
+    return np.ascontiguousarray(H.reshape(site_shape(dims) + (3, 3)))
+
+
+SMALL = [("C1", (8, 8, 8, 8)), ("mixed", (12, 6, 16, 4)), ("odd", (3, 24, 2, 48))]
+VARIANTS = [(8, 18), (8, 12), (4, 18), (4, 12)]
+
+
+def small_config(name, dims):
+    if name == "C1":
+        return inputs.make_config("C1")
+    return inputs.smooth_config(dims, 0.25, 4242 + len(name), haar=True)
+
+
+@pytest.mark.parametrize("name,dims", SMALL)
+@pytest.mark.parametrize("prec,storage", VARIANTS)
+def test_delta_F_theta(lgf, name, dims, prec, storage):
+    """a1: Delta(x) element by element, F and theta (eqs. 3, 5-7)."""
+    import torch
+
+    U = small_config(name, dims)
+    D_o, F_o, th_o = oracle.measure(dims, U)
+    with lgf.Context(dims, prec, storage) as ctx:
+        ctx.set_links(to_dev(U, prec))
+        F, th = ctx.step_delta()
+        out = torch.empty(site_shape(dims) + (3, 3), dtype=torch.complex128 if prec == 8 else torch.complex64,
+                          device="cuda")
+        D = to_np(ctx.get_field(out))
+    tol = TOL[prec]
+    assert np.max(np.abs(D - D_o)) < tol["field"] * max(1.0, np.max(np.abs(D_o)))
+    assert abs(F - F_o) <= tol["scalar"] * abs(F_o)
+    assert abs(th - th_o) <= tol["scalar"] * abs(th_o)
+
+
+@pytest.mark.parametrize("dims", [(8, 8, 8, 8), (12, 6, 16, 4), (3, 24, 2, 48), (16, 16, 16, 16), (32, 8, 64, 4)])
+@pytest.mark.parametrize("prec", [8, 4])
+def test_accelerate(lgf, dims, prec):
+    """a2-a4: w = F^-1 (16/p^2) F Delta / V against the oracle's naive separable DFT."""
+    import torch
+
+    D = random_herm_field(dims, 99)
+    D -= D.mean(axis=(0, 1, 2, 3), keepdims=True)        # like a real Delta: zero lattice sum
+    w_o = oracle.accelerate(dims, D)
+    with lgf.Context(dims, prec, 18) as ctx:
+        ctx.set_field(to_dev(D, prec))
+        ctx.step_accelerate()
+        out = torch.empty(site_shape(dims) + (3, 3), dtype=torch.complex128 if prec == 8 else torch.complex64,
+                          device="cuda")
+        w = to_np(ctx.get_field(out))
+    scale = np.max(np.abs(w_o))
+    assert np.max(np.abs(w - w_o)) < (1e-12 if prec == 8 else 2e-5) * scale
+
+
+@pytest.mark.parametrize("name,dims", SMALL)
+@pytest.mark.parametrize("prec,storage", VARIANTS)
+def test_update(lgf, name, dims, prec, storage):
+    """a5 + a6: g = GS(1 + i alpha/2 w), U <- g U g^dag(x+mu), against the oracle on the same w."""
+    import torch
+
+    U = small_config(name, dims)
+    w = 3.0 * random_herm_field(dims, 5)
+    U_o = oracle.transform(dims, U, oracle.build_g(dims, w, ALPHA))
+    with lgf.Context(dims, prec, storage) as ctx:
+        d = to_dev(U, prec)
+        ctx.set_links(d)
+        ctx.set_field(to_dev(w, prec))
+        ctx.step_update(ALPHA)
+        out = to_np(ctx.get_links(torch.empty_like(d)))
+    assert np.max(np.abs(out - U_o)) < (1e-13 if prec == 8 else 2e-6)
+
+
+def run_trajectory(lgf, dims, U, prec, storage, n):
+    import torch
+
+    with lgf.Context(dims, prec, storage, stream=torch.cuda.current_stream()) as ctx:
+        d = to_dev(U, prec)
+        ctx.set_links(d)
+        ctx.iterate(ALPHA, n)
+        F, th, P = ctx.measure()
+        Fh, Th = ctx.history()
+        assert len(Fh) == n and ctx.iterations() == n
+        out = to_np(ctx.get_links(torch.empty_like(d)))
+    return np.append(Fh, F), np.append(Th, th), P, out
+
+
+@pytest.mark.parametrize("cfg", ["C1", "C2"])
+@pytest.mark.parametrize("prec,storage", VARIANTS)
+def test_trajectory_20(lgf, config_cache, cfg, prec, storage):
+    """north_star parity: (F_n, theta_n), n = 0..20, and the links after 20 iterations."""
+    dims = inputs.CONFIGS[cfg]["dims"]
+    U = config_cache(cfg)
+    U_o, F_o, T_o = oracle.iterate(dims, U, ALPHA, 20)
+    Fh, Th, P, out = run_trajectory(lgf, dims, U, prec, storage, 20)
+    tol = TOL[prec]
+    assert np.max(np.abs(Fh - F_o) / np.abs(F_o)) < tol["scalar"]
+    assert np.max(np.abs(Th - T_o) / np.abs(T_o)) < tol["scalar"]
+    assert np.max(np.abs(out - U_o)) < tol["links"]
+    assert abs(P - oracle.plaquette(dims, U)) < (1e-13 if prec == 8 else 1e-6)      # gauge invariant
+
+
+def test_trajectory_asymmetric(lgf):
+    """Radix-3 / mixed-length axes: 12 x 6 x 24 x 48, 10 iterations, fp64."""
+    dims = (12, 6, 24, 48)
+    U = inputs.smooth_config(dims, 0.3, 77, haar=True)
+    U_o, F_o, T_o = oracle.iterate(dims, U, ALPHA, 10)
+    Fh, Th, P, out = run_trajectory(lgf, dims, U, 8, 18, 10)
+    assert np.max(np.abs(Fh - F_o) / np.abs(F_o)) < 1e-12
+    assert np.max(np.abs(Th - T_o) / np.abs(T_o)) < 1e-12
+    assert np.max(np.abs(out - U_o)) < 1e-11
+
+
+@pytest.mark.parametrize("storage", [18, 12])
+def test_fix_c1_iteration_count(lgf, config_cache, storage):
+    """Algorithm 1 to theta < 1e-15 on C1: iteration count within 2 % of the oracle's, same final state."""
+    import torch
+
+    dims = inputs.CONFIGS["C1"]["dims"]
+    U = config_cache("C1")
+    U_o, it_o, F_o, T_o = oracle.fix(dims, U, ALPHA, 1e-15, 2000)
+    with lgf.Context(dims, 8, storage) as ctx:
+        d = to_dev(U, 8)
+        it = ctx.fix(d, ALPHA, 1e-15, 2000)
+        Fh, Th = ctx.history()
+        F, th, P = ctx.measure()
+    assert abs(it - it_o) <= max(1, round(0.02 * it_o))
+    assert len(Fh) == it + 1 and Th[-1] < 1e-15 and th < 1e-15
+    assert np.all(Th[:-1] >= 1e-15)
+    n = min(it, it_o)
+    assert np.max(np.abs(Fh[: n + 1] - F_o[: n + 1]) / np.abs(F_o[: n + 1])) < 1e-11
+    if it == it_o:
+        assert np.max(np.abs(to_np(d) - U_o)) < 1e-10
+    assert abs(P - oracle.plaquette(dims, U)) < 1e-13
+
+
+def test_fix_pure_gauge_reaches_F1(lgf, config_cache):
+    """Closed form: U = h(x) h(x+mu)^dag is driven to F -> 1, theta -> 0, U -> 1 (C2 pure-gauge variant)."""
+    dims = inputs.CONFIGS["C2pg"]["dims"]
+    U = config_cache("C2pg")
+    with lgf.Context(dims, 8, 18) as ctx:
+        d = to_dev(U, 8)
+        it = ctx.fix(d, ALPHA, 1e-15, 2000)
+        F, th, P = ctx.measure()
+    assert 0 < it < 200
+    assert abs(F - 1.0) < 1e-12 and th < 1e-15 and abs(P - 1.0) < 1e-12
+    eye = np.eye(3)
+    assert np.max(np.abs(to_np(d) - eye)) < 1e-6
+
+
+def test_fix_fp32_c2(lgf, config_cache):
+    """fp32 runs stop at theta < 1e-12 (BASELINE.json config C2); count close to the fp64 oracle's."""
+    dims = inputs.CONFIGS["C2"]["dims"]
+    U = config_cache("C2")
+    _, it_o, F_o, T_o = oracle.fix(dims, U, ALPHA, 1e-12, 2000)
+    with lgf.Context(dims, 4, 18) as ctx:
+        h = np.ascontiguousarray(U.astype(np.complex64))
+        it = ctx.fix_host(h, ALPHA, 1e-12, 2000)
+        F, th, _ = ctx.measure()
+    assert abs(it - it_o) <= max(2, round(0.05 * it_o))
+    assert th < 1e-12 and abs(F - F_o[-1]) < 1e-5 * abs(F_o[-1])
+    # the returned host array is still SU(3) to fp32 accuracy
+    UU = np.einsum("...ij,...kj->...ik", h.astype(np.complex128), h.astype(np.complex128).conj())
+    assert np.max(np.abs(UU - np.eye(3))) < 1e-4
+
+
+def test_edge_cases(lgf):
+    import torch
+
+    with pytest.raises(lgf.LgfError) as e:
+        lgf.Context((8, 8, 8, 10), 8, 18)
+    assert e.value.code == lgf.LGF_EINVAL
+    with pytest.raises(lgf.LgfError):
+        lgf.Context((8, 8, 8, 8), 2, 18)
+    with pytest.raises(lgf.LgfError):
+        lgf.Context((8, 8, 8, 8), 8, 8)
+    dims = (4, 4, 4, 4)
+    with lgf.Context(dims, 8, 18) as ctx:
+        with pytest.raises(lgf.LgfError) as e:
+            ctx.iterate(ALPHA, 1)
+        assert e.value.code == lgf.LGF_ESTATE
+        # unit links: already in Landau gauge, Delta = 0, F = 1, theta = 0 -> zero iterations
+        U = np.broadcast_to(np.eye(3, dtype=np.complex128), site_shape(dims) + (4, 3, 3)).copy()
+        d = to_dev(U, 8)
+        assert ctx.fix(d, ALPHA, 1e-15, 100) == 0
+        F, th, P = ctx.measure()
+        assert F == 1.0 and th == 0.0 and P == 1.0
+        assert np.array_equal(to_np(d), U)
+        # max_iter = 0: measure only, nothing changes
+        U2 = inputs.smooth_config(dims, 0.2, 5)
+        d2 = to_dev(U2, 8)
+        assert ctx.fix(d2, ALPHA, 1e-15, 0) == 0
+        assert np.array_equal(to_np(d2), U2)
+        assert ctx.history_length() == 1
+        # max_iter reached before convergence: returns max_iter, history has max_iter + 1 entries
+        assert ctx.fix(d2, ALPHA, 1e-15, 3) == 3
+        assert ctx.history_length() == 4
+        _, F_o, T_o = oracle.iterate(dims, U2, ALPHA, 3)
+        Fh, Th = ctx.history()
+        assert np.max(np.abs(Th - T_o) / T_o) < 1e-12
+
+
+def test_12_real_matches_18_real(lgf, config_cache):
+    """Third-row reconstruction (eq. 8) changes rounding only."""
+    dims = inputs.CONFIGS["C1"]["dims"]
+    U = config_cache("C1")
+    a = run_trajectory(lgf, dims, U, 8, 18, 8)
+    b = run_trajectory(lgf, dims, U, 8, 12, 8)
+    assert np.max(np.abs(a[3] - b[3])) < 1e-12
+    assert np.max(np.abs(a[1] - b[1]) / a[1]) < 1e-12
