@@ -1,0 +1,385 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the Landau gauge-fixing hot path (arXiv:1206.0675, Algorithm 1) on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C3] [--precision fp64] [--storage 18]
+    python -m torch.distributed.run --nnodes=1 --nproc-per-node N ... bench.py --gpus N --steps K --warmup W
+    python bench.py --impl reference [--steps K] [--warmup W]        # the CPU oracle, timed on the host cores
+
+A "step" is one pass of the whole hot path -- one iteration of Algorithm 1's loop body (Delta/F/theta ->
+forward FFT -> p2max/p2 -> inverse FFT -> g(x) -> link update) -- over one seeded
+synthetic 32^4 configuration (BASELINE.json configs[2] = C3, the lattice the metric is quoted on).  The
+headline line is fp64 / 18-real; the other precision x storage variants are timed the same way and listed
+under "variants".  Rank 0 prints ONE JSON line.  Multi-GPU = independent replicas (one configuration per
+GPU): no data-path collective, "scaling": "weak".
+
+Everything timed here goes through the C ABI of liblgf.so (paper_1206_0675_b200.binding); the oracle is
+executed only for the "cpu_baseline" object and for --impl reference.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "gauge_fix_iterations_per_s"
+UNIT = "iterations/s"
+ALPHA = 0.08
+FALLBACK_HBM_GBS = 6650.0          # /opt/skills/guides/B200_PROFILING.md fallback, used only if MEASURED_PEAKS.json is absent
+PREC = {"fp64": 8, "fp32": 4}
+
+
+def measured_peak():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+
+    REASONS = {0x8: "hw_slowdown", 0x40: "hw_thermal_slowdown", 0x20: "sw_thermal_slowdown", 0x4: "sw_power_cap",
+               0x80: "hw_power_brake_slowdown"}
+
+    def __init__(self, index, period=0.01):
+        self.period, self.samples, self.reasons, self._stop = period, [], set(), threading.Event()
+        self.max_mhz, self.ok = None, False
+        try:
+            import pynvml
+
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+            self.ok = True
+        except Exception as e:  # noqa: BLE001
+            self.err = repr(e)
+        self.thread = threading.Thread(target=self._run, daemon=True)
+
+    def _run(self):
+        while not self._stop.is_set():
+            try:
+                self.samples.append(int(self.nv.nvmlDeviceGetClockInfo(self.h, self.nv.NVML_CLOCK_SM)))
+                r = int(self.nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+                for bit, name in self.REASONS.items():
+                    if r & bit:
+                        self.reasons.add(name)
+            except Exception:  # noqa: BLE001
+                pass
+            time.sleep(self.period)
+
+    def __enter__(self):
+        if self.ok:
+            self.thread.start()
+        return self
+
+    def __exit__(self, *exc):
+        self._stop.set()
+        if self.ok:
+            self.thread.join()
+
+    def summary(self):
+        if not self.ok or not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": ["unavailable"]}
+        return {"sm_mhz": float(np.median(self.samples)), "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(self.samples)}
+
+
+def physical_gpu_index(local_rank):
+    vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+    if vis:
+        try:
+            return int(vis.split(",")[local_rank])
+        except Exception:  # noqa: BLE001
+            return local_rank
+    return local_rank
+
+
+# ---------------------------------------------------------------------------------------------------------
+def time_variant(binding, torch, U0, dims, prec_name, storage, steps, warmup, dist, sampler=None):
+    """Device-resident timing of `steps` iterations.  Returns dict(ms_per_step, launches, kernels...)."""
+    prec = PREC[prec_name]
+    cdt = torch.complex128 if prec == 8 else torch.complex64
+    stream = torch.cuda.current_stream()
+    out = {}
+    with binding.Context(dims, prec, storage, stream=stream) as ctx:
+        d = torch.from_numpy(U0).to(cdt).cuda()
+        ctx.set_links(d)
+        ctx.iterate(ALPHA, warmup)
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        n0 = ctx.launch_count()
+        if sampler is not None:
+            sampler.__enter__()
+        e0.record(stream)
+        ctx.iterate(ALPHA, steps)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        if sampler is not None:
+            sampler.__exit__()
+        if dist is not None:
+            dist.barrier()
+        ms = e0.elapsed_time(e1)
+        out["launches"] = ctx.launch_count() - n0
+        if dist is not None:
+            t = torch.tensor([ms], dtype=torch.float64, device="cuda")
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms = float(t.item())
+        out["ms_total"] = ms
+        out["ms_per_step"] = ms / steps
+        # per-kernel-class device times: every launch bracketed by CUDA events on the launching stream,
+        # over the same number of steps (a second region, so that the brackets do not perturb `value`)
+        ctx.set_profiling(True)
+        ctx.iterate(ALPHA, steps)
+        kt = ctx.kernel_times()
+        ctx.set_profiling(False)
+        kern = {}
+        for i, name in enumerate(binding.KERNEL_CLASSES):
+            ms_k, n_k = kt[name]
+            if n_k == 0:
+                continue
+            per_iter_launches = n_k / steps
+            bytes_iter = ctx.algorithmic_bytes(i)
+            kern[name] = {"ms_per_step": ms_k / steps, "launches_per_step": per_iter_launches,
+                          "avg_launch_us": 1e3 * ms_k / n_k, "algorithmic_bytes_per_step": bytes_iter,
+                          "gbs": bytes_iter / (ms_k / steps * 1e-3) / 1e9 if ms_k > 0 else None}
+        out["kernels"] = kern
+        F, th, P = ctx.measure()
+        out["F"], out["theta"], out["plaquette"] = F, th, P
+        out["iter_bytes"] = sum(ctx.algorithmic_bytes(i) for i in (binding.LGF_K_DELTA, binding.LGF_K_FFT,
+                                                                    binding.LGF_K_UPDATE))
+    del d
+    torch.cuda.empty_cache()
+    return out
+
+
+def time_e2e(binding, torch, U0, dims, prec_name, storage, tol, max_iter, dist):
+    """Algorithm 1 end to end through lgf_fix_host: pinned HOST buffer in, gauge-fixed HOST buffer out;
+    the H2D and D2H copies of the configuration are inside the timed region."""
+    prec = PREC[prec_name]
+    cdt = torch.complex128 if prec == 8 else torch.complex64
+    stream = torch.cuda.current_stream()
+    with binding.Context(dims, prec, storage, stream=stream) as ctx:
+        h = torch.from_numpy(U0).to(cdt).pin_memory()
+        warm = h.clone().pin_memory()
+        ctx.fix_host(warm, ALPHA, tol, 1)              # allocates the staging buffer, warms the kernels
+        del warm
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        t0 = time.perf_counter()
+        e0.record(stream)
+        it = ctx.fix_host(h, ALPHA, tol, max_iter)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        wall = time.perf_counter() - t0
+        ms = max(e0.elapsed_time(e1), 1e3 * wall)
+        if dist is not None:
+            dist.barrier()
+            t = torch.tensor([ms], dtype=torch.float64, device="cuda")
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms = float(t.item())
+        F, th, _ = ctx.measure(plaquette=False)
+        nbytes = h.numel() * h.element_size()
+    return {"iterations": it, "ms": ms, "bytes_each_way": nbytes, "theta": th, "F": F}
+
+
+def cpu_baseline(U0, dims, budget_s=30.0):
+    """The oracle as it stands, on the host cores, on a bounded sample: whole iterations of Algorithm 1
+    on the same configuration until ~budget_s have been spent (at least one)."""
+    import oracle
+
+    n, t = 0, 0.0
+    U = U0
+    while True:
+        t0 = time.perf_counter()
+        U, _, _ = oracle.iterate(dims, U, ALPHA, 1)
+        t += time.perf_counter() - t0
+        n += 1
+        if t + t / n > budget_s:
+            break
+    # orc_iterate(n=1) = measure + update + measure; one loop-body pass is update + measure, so correct by
+    # timing one extra measure
+    t0 = time.perf_counter()
+    oracle.measure(dims, U, want_delta=True)
+    tm = time.perf_counter() - t0
+    t_iter = t / n - tm
+    return {"value": 1.0 / t_iter, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+            "sample": "%d whole iteration(s) of Algorithm 1 on the full %s lattice, fp64, 9-component naive separable DFT "
+                      "(%.2f s each)" % (n, "x".join(str(v) for v in dims), t_iter)}
+
+
+# ---------------------------------------------------------------------------------------------------------
+def run_reference(args):
+    """--impl reference: the oracle, as it stands, timed on the host cores.  Rank 0 only."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return 0
+    import oracle
+    from paper_1206_0675_b200 import inputs
+
+    oracle.build()
+    cfg = inputs.CONFIGS[args.workload]
+    dims = cfg["dims"]
+    U = inputs.make_config(args.workload)
+    budget = float(args.reference_budget)
+    done_w, t_w = 0, 0.0
+    for _ in range(max(1, args.warmup)):                 # warm-up steps (bounded by the budget)
+        t0 = time.perf_counter()
+        U, _, _ = oracle.iterate(dims, U, ALPHA, 1)
+        t_w += time.perf_counter() - t0
+        done_w += 1
+        if t_w > 0.25 * budget:
+            break
+    per = t_w / done_w
+    k = int(max(1, min(args.steps, (budget - t_w) // per)))
+    t0 = time.perf_counter()
+    for _ in range(k):
+        U, _, _ = oracle.iterate(dims, U, ALPHA, 1)
+    t = time.perf_counter() - t0
+    value = k / t
+    sample = ("%d of the %d requested steps timed (%d warm-up); a step = one whole oracle iteration "
+              "(measure + 9-component DFT pair + g + update + measure) on the full %s lattice, fp64"
+              % (k, args.steps, done_w, "x".join(str(v) for v in dims)))
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": k,
+            "warmup": done_w, "ms_per_step": 1e3 * t / k, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": workload_name(args.workload, dims), "precision": "fp64", "alpha": ALPHA},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+                             "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+def workload_name(key, dims):
+    from paper_1206_0675_b200 import inputs
+
+    c = inputs.CONFIGS[key]
+    what = "hot start (Haar-random links)" if c["kind"] == "hot" else "smooth eps=%g with Haar h(x)" % c["eps"]
+    return "%s: %s periodic SU(3) lattice, %s, seed %d" % (key, "x".join(str(v) for v in dims), what, c["seed"])
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--workload", default="C3", choices=["C1", "C2", "C3", "C4", "C5"])
+    ap.add_argument("--precision", default="fp64", choices=["fp64", "fp32"])
+    ap.add_argument("--storage", type=int, default=18, choices=[18, 12])
+    ap.add_argument("--no-variants", action="store_true", help="time only the headline variant")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--cpu-budget", type=float, default=20.0)
+    ap.add_argument("--reference-budget", type=float, default=240.0)
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3)
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+
+    from paper_1206_0675_b200 import binding, inputs
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: liblgf has no CPU path")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist  # noqa: PLC0415
+
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    binding.load()
+
+    cfg = inputs.CONFIGS[args.workload]
+    dims = cfg["dims"]
+    V = int(np.prod(dims))
+    U0 = inputs.make_config(args.workload, seed_offset=rank)     # replicas: one ensemble member per GPU
+
+    sampler = ClockSampler(physical_gpu_index(local))
+    head = time_variant(binding, torch, U0, dims, args.precision, args.storage, args.steps, args.warmup, dist, sampler)
+    value = world * args.steps / (head["ms_total"] * 1e-3)
+    peak, peak_src = measured_peak()
+
+    # dominant kernel class of the iteration -> roofline object
+    hot = {k: v for k, v in head["kernels"].items() if k in ("delta", "fft", "update")}
+    dom = max(hot, key=lambda k: hot[k]["ms_per_step"])
+    dk = hot[dom]
+    bytes_per_launch = dk["algorithmic_bytes_per_step"] / dk["launches_per_step"]
+    achieved = bytes_per_launch / (dk["avg_launch_us"] * 1e-6) / 1e9
+    roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
+                "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": bytes_per_launch, "avg_launch_us": dk["avg_launch_us"],
+                "iteration": {"algorithmic_bytes": head["iter_bytes"],
+                              "achieved": head["iter_bytes"] / (head["ms_per_step"] * 1e-3) / 1e9,
+                              "frac": head["iter_bytes"] / (head["ms_per_step"] * 1e-3) / 1e9 / peak},
+                "kernels": {k: {"ms_per_step": round(v["ms_per_step"], 6), "launches_per_step": v["launches_per_step"],
+                                "gbs": v["gbs"], "frac": v["gbs"] / peak} for k, v in hot.items()}}
+
+    variants = {}
+    if not args.no_variants:
+        for pn in ("fp64", "fp32"):
+            for st in (18, 12):
+                if pn == args.precision and st == args.storage:
+                    r = head
+                else:
+                    r = time_variant(binding, torch, U0, dims, pn, st, args.steps, args.warmup, dist)
+                gbs = r["iter_bytes"] / (r["ms_per_step"] * 1e-3) / 1e9
+                variants["%s/%d" % (pn, st)] = {"iterations_per_s": world * 1e3 / r["ms_per_step"],
+                                                "site_updates_per_s": world * V * 1e3 / r["ms_per_step"],
+                                                "ms_per_step": r["ms_per_step"], "algorithmic_gbs": gbs,
+                                                "frac_of_peak": gbs / peak}
+
+    e2e = None
+    if not args.no_e2e:
+        tol = 1e-15 if args.precision == "fp64" else 1e-12
+        r = time_e2e(binding, torch, U0, dims, args.precision, args.storage, tol, 5000, dist)
+        its = max(1, r["iterations"])
+        e2e = {"value": world * its / (r["ms"] * 1e-3), "unit": UNIT,
+               "h2d_bytes_per_step": r["bytes_each_way"] / its, "d2h_bytes_per_step": r["bytes_each_way"] / its,
+               "call": "lgf_fix_host(pinned host links, alpha=0.08, tol=%g): H2D + %d iterations + D2H in %.1f ms"
+                       % (tol, r["iterations"], r["ms"]), "final_theta": r["theta"]}
+
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        cpu = cpu_baseline(U0, dims, args.cpu_budget)
+
+    if rank == 0:
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": args.warmup, "ms_per_step": head["ms_per_step"], "higher_is_better": True, "scaling": "weak",
+                "vs_baseline": None, "dtype": "f64" if args.precision == "fp64" else "f32", "data": "synthetic",
+                "config": {"workload": workload_name(args.workload, dims), "precision": args.precision,
+                           "link_storage": args.storage, "alpha": ALPHA, "sites": V, "parallelism": "replicas x%d" % world,
+                           "l2": "inputs larger than L2: one step streams %.0f MB of links and fields"
+                                 % (head["iter_bytes"] / 1e6)},
+                "site_updates_per_s": value * V, "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e,
+                "gpu_launches": head["launches"], "clocks": sampler.summary(), "variants": variants,
+                "state_after_timing": {"F": head["F"], "theta": head["theta"], "plaquette": head["plaquette"]}}
+        print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())
