@@ -120,6 +120,17 @@ int lgf_step_update(lgf_ctx *ctx, double alpha);
 int lgf_get_field(lgf_ctx *ctx, void *d_field);
 int lgf_set_field(lgf_ctx *ctx, const void *d_field);
 
+/* ---- tuning --------------------------------------------------------------------------------------- */
+
+/* Override a planner choice (takes effect from the next iteration; results are unchanged up to
+ * rounding).  Keys: "fft_two_axis" (1 = use the three-sweep two-axis FFT passes when the lattice
+ * allows, 0 = one pass per axis), "fft_xy_planes" ((x, y) planes per CTA, 0 = automatic),
+ * "fft_zt_xc" (consecutive (x, y) indices per CTA of the (z, t) pass, 0 = automatic).
+ * Unknown key or NULL: LGF_EINVAL.  Synchronises. */
+int lgf_tune(lgf_ctx *ctx, const char *key, int value);
+/* Number of FFT kernel launches per iteration under the current plan (3 or up to 7). */
+int lgf_fft_passes(const lgf_ctx *ctx);
+
 /* ---- instrumentation ------------------------------------------------------------------------- */
 
 /* Kernel classes for per-kernel timing. */

@@ -49,6 +49,8 @@ SIGNATURES = {
     "lgf_step_update": (_i, [_vp, _d]),
     "lgf_get_field": (_i, [_vp, _vp]),
     "lgf_set_field": (_i, [_vp, _vp]),
+    "lgf_tune": (_i, [_vp, ctypes.c_char_p, _i]),
+    "lgf_fft_passes": (_i, [_vp]),
     "lgf_set_profiling": (_i, [_vp, _i]),
     "lgf_kernel_times": (_i, [_vp, _dp, _llp]),
     "lgf_launch_count": (_ll, [_vp]),
@@ -229,6 +231,13 @@ class Context:
 
     def set_field(self, field):
         _check(self._h, load().lgf_set_field(self._h, _dev_ptr(field, self.precision, self.V * 18)))
+
+    # -- tuning -----------------------------------------------------------------------------------
+    def tune(self, key, value):
+        _check(self._h, load().lgf_tune(self._h, key.encode(), int(value)))
+
+    def fft_passes(self):
+        return int(load().lgf_fft_passes(self._h))
 
     # -- instrumentation --------------------------------------------------------------------------
     def set_profiling(self, on):

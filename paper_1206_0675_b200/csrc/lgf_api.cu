@@ -33,6 +33,9 @@ struct lgf_ctx {
     std::vector<AxisPass> passes;
     bool have_links = false;
     bool profiling = false;
+    int tune_two_axis = 1;       // lgf_tune: use the two-axis FFT passes when available
+    int tune_xy_planes = 0;      // lgf_tune: planes per CTA of the (x, y) pass (0 = planner's choice)
+    int tune_zt_xc = 0;          // lgf_tune: consecutive (x, y) indices per CTA of the (z, t) pass
     struct Stamp { cudaEvent_t a, b; int cls; };
     std::vector<Stamp> stamps;
     double prof_ms[LGF_K_COUNT] = {0};
@@ -121,17 +124,28 @@ static long long largest_divisor_le(long long n, long long cap) {
     return 1;
 }
 
-// One pass per axis: forward x, y, z; forward + scale + inverse on t; inverse z, y, x.
+static long long pow2_divisor_le(long long n, long long cap) {
+    long long d = 1;
+    while (d * 2 <= cap && n % (d * 2) == 0) d *= 2;
+    return d;
+}
+
+// FFT pass plan.  Preferred: three sweeps of the field -- (x, y) planes forward, (z, t) planes forward +
+// scale + inverse, (x, y) planes inverse -- when two-axis kernels exist for the lattice's lengths and
+// the tiles fit in shared memory; otherwise one pass per axis (forward x, y, z; forward + scale +
+// inverse on t; inverse z, y, x).  tune_xy_planes / tune_zt_xc (> 0) override the tile sizes.
 static void plan_passes(lgf_ctx *ctx) {
-    const long long T = 2048;     // target complex elements per tile
+    const long long T = 2048;     // target complex elements per tile of the one-axis passes
     const size_t cbytes = 2 * (size_t)ctx->prec;
+    const Geom &g = ctx->g;
     auto make = [&](int axis, int mode) {
         AxisPass p{};
+        p.kind = PASS_AXIS;
         p.axis = axis;
-        p.L = ctx->g.L[axis];
+        p.L = g.L[axis];
         p.mode = mode;
-        p.S = ctx->g.S[axis];
-        p.H = ctx->g.V / (p.S * p.L);
+        p.S = g.S[axis];
+        p.H = g.V / (p.S * p.L);
         if (p.S == 1) {
             p.nlo = 1;
             p.nhi = (int)largest_divisor_le(p.H, T / p.L);
@@ -144,10 +158,49 @@ static void plan_passes(lgf_ctx *ctx) {
         p.threads = 256;
         return p;
     };
+    const size_t SMEM_MAX = 200 * 1024;
+    const long long MIN_GRID = 2 * 148;
+    // (x, y) planes
+    AxisPass xy{};
+    bool have_xy = ctx->tune_two_axis && fft_pair_supported(PASS_XY, g.L[0], g.L[1]);
+    if (have_xy) {
+        const long long planes = 4LL * g.L[2] * g.L[3], psize = (long long)g.L[0] * g.L[1];
+        long long P = largest_divisor_le(planes, 2048 / psize > 0 ? 2048 / psize : 1);
+        while (P > 1 && planes / P < MIN_GRID) P = largest_divisor_le(planes, P - 1);
+        if (ctx->tune_xy_planes > 0 && planes % ctx->tune_xy_planes == 0) P = ctx->tune_xy_planes;
+        xy.kind = PASS_XY; xy.L = g.L[0]; xy.L2 = g.L[1]; xy.nhi = (int)P; xy.nlo = 1; xy.threads = 256;
+        xy.smem = (128 + (size_t)P * g.L[1] * (g.L[0] | 1)) * cbytes;
+        have_xy = xy.smem <= SMEM_MAX;
+    }
+    // (z, t) planes
+    AxisPass zt{};
+    bool have_zt = ctx->tune_two_axis && fft_pair_supported(PASS_ZT, g.L[2], g.L[3]);
+    if (have_zt) {
+        const long long plane = g.S[2], zsize = (long long)g.L[2] * g.L[3];
+        const long long phase = 128 / (long long)cbytes;             // lanes per shared-memory phase
+        const long long xc_min = pow2_divisor_le(plane, 32 / (long long)cbytes > 0 ? 32 / (long long)cbytes : 1);
+        long long XC = pow2_divisor_le(plane, (65536 / (long long)cbytes) / zsize > 0 ? (65536 / (long long)cbytes) / zsize : 1);
+        while (XC > xc_min && (plane / XC) * 4 < MIN_GRID) XC /= 2;
+        if (XC < xc_min) XC = xc_min;
+        if (ctx->tune_zt_xc > 0 && plane % ctx->tune_zt_xc == 0) XC = ctx->tune_zt_xc;
+        long long pitch = XC * g.L[2];
+        if (XC < phase && pitch % phase == 0) pitch += XC;           // lanes (xc, t) -> distinct banks
+        zt.kind = PASS_ZT; zt.L = g.L[2]; zt.L2 = g.L[3]; zt.mode = FFT_FWD_SCALE_INV; zt.nlo = (int)XC; zt.nhi = 1;
+        zt.pitch = (int)pitch; zt.threads = 256;
+        zt.smem = (128 + (size_t)pitch * g.L[3]) * cbytes;
+        have_zt = zt.smem <= SMEM_MAX;
+    }
     ctx->passes.clear();
-    for (int a = 0; a < 3; a++) ctx->passes.push_back(make(a, FFT_FWD));
-    ctx->passes.push_back(make(3, FFT_FWD_SCALE_INV));
-    for (int a = 2; a >= 0; a--) ctx->passes.push_back(make(a, FFT_INV));
+    if (have_xy) { xy.mode = FFT_FWD; ctx->passes.push_back(xy); }
+    else { ctx->passes.push_back(make(0, FFT_FWD)); ctx->passes.push_back(make(1, FFT_FWD)); }
+    if (have_zt) ctx->passes.push_back(zt);
+    else {
+        ctx->passes.push_back(make(2, FFT_FWD));
+        ctx->passes.push_back(make(3, FFT_FWD_SCALE_INV));
+        ctx->passes.push_back(make(2, FFT_INV));
+    }
+    if (have_xy) { xy.mode = FFT_INV; ctx->passes.push_back(xy); }
+    else { ctx->passes.push_back(make(1, FFT_INV)); ctx->passes.push_back(make(0, FFT_INV)); }
 }
 
 // ---- profiling brackets ---------------------------------------------------------------------------
@@ -196,8 +249,9 @@ static int step_accelerate(lgf_ctx *ctx) {
     const R scale = (R)(16.0 / (double)ctx->g.V);        // p2max / V      (Alg. 1 lines 5, 7; R5, R7)
     for (const AxisPass &p : ctx->passes) {
         Bracket br(ctx, LGF_K_FFT);
-        CK(launch_fft_pass<R>(p, (C<R> *)ctx->W, ctx->g, (const R *)ctx->twiddle[p.axis], (const R *)ctx->p2tab, scale,
-                              ctx->st, ctx->stream));
+        const R *tw[4] = {(const R *)ctx->twiddle[0], (const R *)ctx->twiddle[1], (const R *)ctx->twiddle[2],
+                          (const R *)ctx->twiddle[3]};
+        CK(launch_fft_pass<R>(p, (C<R> *)ctx->W, ctx->g, tw, (const R *)ctx->p2tab, scale, ctx->st, ctx->stream));
     }
     return LGF_OK;
 }
@@ -543,6 +597,20 @@ int lgf_set_field(lgf_ctx *ctx, const void *d_field) {
     else CK(launch_field_set<float>((C<float> *)ctx->W, (const float *)d_field, ctx->g, ctx->stream));
     return LGF_OK;
 }
+
+int lgf_tune(lgf_ctx *ctx, const char *key, int value) {
+    if (!ctx || !key) return fail(ctx, LGF_EINVAL, "lgf_tune: null argument");
+    const std::string k(key);
+    if (k == "fft_two_axis") ctx->tune_two_axis = value;
+    else if (k == "fft_xy_planes") ctx->tune_xy_planes = value;
+    else if (k == "fft_zt_xc") ctx->tune_zt_xc = value;
+    else return fail(ctx, LGF_EINVAL, "lgf_tune: unknown key " + k);
+    CK(cudaStreamSynchronize(ctx->stream));
+    plan_passes(ctx);
+    return LGF_OK;
+}
+
+int lgf_fft_passes(const lgf_ctx *ctx) { return ctx ? (int)ctx->passes.size() : LGF_EINVAL; }
 
 int lgf_set_profiling(lgf_ctx *ctx, int on) {
     if (!ctx) return LGF_EINVAL;

@@ -20,23 +20,35 @@ struct DevState {
 
 enum FftMode { FFT_FWD = 0, FFT_INV = 1, FFT_FWD_SCALE_INV = 2 };
 
-// One FFT pass over one lattice axis (see lgf_fft.cu).
+enum PassKind {
+    PASS_AXIS = 0,        // one lattice axis per pass (any supported length)
+    PASS_XY = 1,          // whole (x, y) planes: both axes transformed in one shared-memory tile
+    PASS_ZT = 2           // (z, t) planes of nlo consecutive (x, y) indices: forward z, t, scale, inverse t, z
+};
+
+// One FFT pass (see lgf_fft.cu).
 struct AxisPass {
-    int axis;             // 0..3
-    int L;                // length of that axis
+    int kind;             // PassKind
+    int axis;             // PASS_AXIS: 0..3
+    int L;                // PASS_AXIS: length of that axis; PASS_XY: Lx; PASS_ZT: Lz
+    int L2;               // PASS_XY: Ly; PASS_ZT: Lt
     int mode;             // FftMode
     long long S;          // global stride of the axis (elements)
     long long H;          // number of "hi" blocks: V / (S * L)
     int nlo, nhi;         // tile extents: nlo consecutive "lo" indices (lo < S), nhi "hi" indices
+                          // (PASS_XY: nhi = planes per CTA; PASS_ZT: nlo = consecutive (x, y) indices per CTA)
+    int pitch;            // PASS_ZT: shared-memory stride of t (nlo * Lz + padding)
     int threads;
     size_t smem;
 };
 
 // launchers implemented in the .cu files (R = float / double)
 template <class R>
-cudaError_t launch_fft_pass(const AxisPass &p, C<R> *W, const Geom &g, const R *twiddle /*[2*L]*/,
+cudaError_t launch_fft_pass(const AxisPass &p, C<R> *W, const Geom &g, const R *const twiddle[4] /*[2*64] per axis*/,
                             const R *p2tab /*[4][64] permuted 4 sin^2*/, R scale, const DevState *st,
                             cudaStream_t stream);
+// true if a PASS_XY (first two axes) / PASS_ZT (last two axes) kernel is instantiated for these lengths
+bool fft_pair_supported(int kind, int La, int Lb);
 
 template <class R>
 cudaError_t launch_delta(int nr, const C<R> *links, C<R> *W, const Geom &g, double *partial, int *nblocks,

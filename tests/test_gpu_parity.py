@@ -81,16 +81,25 @@ def test_delta_F_theta(lgf, name, dims, prec, storage):
     assert abs(th - th_o) <= tol["scalar"] * abs(th_o)
 
 
-@pytest.mark.parametrize("dims", [(8, 8, 8, 8), (12, 6, 16, 4), (3, 24, 2, 48), (16, 16, 16, 16), (32, 8, 64, 4)])
+ACC_DIMS = [(8, 8, 8, 8), (12, 6, 16, 4), (3, 24, 2, 48), (16, 16, 16, 16), (32, 8, 64, 4), (8, 8, 24, 48),
+            (24, 24, 24, 48), (32, 32, 16, 16), (64, 64, 8, 8), (8, 8, 64, 64)]
+
+
+@pytest.mark.parametrize("dims", ACC_DIMS)
 @pytest.mark.parametrize("prec", [8, 4])
-def test_accelerate(lgf, dims, prec):
-    """a2-a4: w = F^-1 (16/p^2) F Delta / V against the oracle's naive separable DFT."""
+@pytest.mark.parametrize("two_axis", [1, 0])
+def test_accelerate(lgf, dims, prec, two_axis):
+    """a2-a4: w = F^-1 (16/p^2) F Delta / V against the oracle's naive separable DFT, with the
+    three-sweep two-axis plan (where the lattice allows it) and with one pass per axis."""
     import torch
 
     D = random_herm_field(dims, 99)
     D -= D.mean(axis=(0, 1, 2, 3), keepdims=True)        # like a real Delta: zero lattice sum
     w_o = oracle.accelerate(dims, D)
     with lgf.Context(dims, prec, 18) as ctx:
+        ctx.tune("fft_two_axis", two_axis)
+        if not two_axis:
+            assert ctx.fft_passes() == 7
         ctx.set_field(to_dev(D, prec))
         ctx.step_accelerate()
         out = torch.empty(site_shape(dims) + (3, 3), dtype=torch.complex128 if prec == 8 else torch.complex64,
@@ -98,6 +107,32 @@ def test_accelerate(lgf, dims, prec):
         w = to_np(ctx.get_field(out))
     scale = np.max(np.abs(w_o))
     assert np.max(np.abs(w - w_o)) < (1e-12 if prec == 8 else 2e-5) * scale
+
+
+@pytest.mark.parametrize("dims,passes", [((32, 32, 32, 32), 3), ((24, 24, 24, 48), 3), ((8, 8, 8, 8), 3),
+                                         ((12, 6, 16, 4), 7), ((16, 16, 12, 6), 5), ((6, 12, 32, 32), 5)])
+def test_fft_plan_and_tile_overrides(lgf, dims, passes):
+    """The planner uses three sweeps where two-axis kernels exist; tile-size overrides change rounding only."""
+    import torch
+
+    D = random_herm_field(dims, 3)
+    D -= D.mean(axis=(0, 1, 2, 3), keepdims=True)
+    res = []
+    with lgf.Context(dims, 8, 18) as ctx:
+        assert ctx.fft_passes() == passes
+        for key, val in [(None, 0), ("fft_xy_planes", 1), ("fft_xy_planes", 4), ("fft_zt_xc", 2), ("fft_zt_xc", 8),
+                         ("fft_two_axis", 0)]:
+            if key:
+                ctx.tune(key, val)
+            ctx.set_field(to_dev(D, 8))
+            ctx.step_accelerate()
+            out = torch.empty(site_shape(dims) + (3, 3), dtype=torch.complex128, device="cuda")
+            res.append(to_np(ctx.get_field(out)))
+        with pytest.raises(lgf.LgfError):
+            ctx.tune("no_such_key", 1)
+    w_o = oracle.accelerate(dims, D)
+    for w in res:
+        assert np.max(np.abs(w - w_o)) < 1e-12 * np.max(np.abs(w_o))
 
 
 @pytest.mark.parametrize("name,dims", SMALL)
