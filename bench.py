@@ -160,8 +160,7 @@ def time_variant(binding, torch, U0, dims, prec_name, storage, steps, warmup, di
         out["kernels"] = kern
         F, th, P = ctx.measure()
         out["F"], out["theta"], out["plaquette"] = F, th, P
-        out["iter_bytes"] = sum(ctx.algorithmic_bytes(i) for i in (binding.LGF_K_DELTA, binding.LGF_K_FFT,
-                                                                    binding.LGF_K_UPDATE))
+        out["iter_bytes"] = ctx.algorithmic_bytes(binding.LGF_K_ITERATION)
     del d
     torch.cuda.empty_cache()
     return out
@@ -322,7 +321,7 @@ def main():
     peak, peak_src = measured_peak()
 
     # dominant kernel class of the iteration -> roofline object
-    hot = {k: v for k, v in head["kernels"].items() if k in ("delta", "fft", "update")}
+    hot = {k: v for k, v in head["kernels"].items() if k in ("delta", "fft", "update", "gbuild")}
     dom = max(hot, key=lambda k: hot[k]["ms_per_step"])
     dk = hot[dom]
     bytes_per_launch = dk["algorithmic_bytes_per_step"] / dk["launches_per_step"]

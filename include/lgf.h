@@ -76,9 +76,11 @@ int lgf_get_links(lgf_ctx *ctx, void *d_links);
 int lgf_set_links_host(lgf_ctx *ctx, const void *h_links);
 int lgf_get_links_host(lgf_ctx *ctx, void *h_links);
 
-/* n iterations of Algorithm 1's loop body [a1 -> a2..a4 -> a5/a6] on the internal configuration
- * with step alpha (the paper uses 0.08), regardless of theta.  (F, theta) of the
- * configuration BEFORE each update is appended to the history.  Never blocks the host. */
+/* n iterations of Algorithm 1's loop body [a2..a4 -> a5 -> a6 + a1 of the new links] on the internal
+ * configuration with step alpha (the paper uses 0.08), regardless of theta.  History
+ * entry k holds (F, theta) of the configuration after k updates since the last set_links (entry 0 =
+ * the loaded configuration, recorded by the first call), so n iterations from a fresh configuration
+ * leave n + 1 entries.  Never blocks the host. */
 int lgf_iterate(lgf_ctx *ctx, double alpha, int n);
 
 /* F, theta (a1) and the average plaquette
@@ -112,7 +114,8 @@ long long lgf_history_length(lgf_ctx *ctx);
 int lgf_step_delta(lgf_ctx *ctx, double *F, double *theta);
 /* a2-a4 only: W <- F^-1 [(16/p2) F W] / V in place. */
 int lgf_step_accelerate(lgf_ctx *ctx);
-/* a5 + a6 only: g(x) from the current W with step alpha, then the link transform. */
+/* a5 + a6 only: g(x) from the current W with step alpha, then the link transform (the fused sweep
+ * also leaves Delta of the new configuration in W; nothing is recorded in the history). */
 int lgf_step_update(lgf_ctx *ctx, double alpha);
 /* The work field as full 3x3 complex matrices, d_field[s][i][j][re/im] (18 reals per site, context
  * precision).  get: unpack W (hermitian traceless by construction).  set: pack a hermitian
@@ -124,7 +127,7 @@ int lgf_set_field(lgf_ctx *ctx, const void *d_field);
 
 /* Override a planner choice (takes effect from the next iteration; results are unchanged up to
  * rounding).  Keys: "fft_two_axis" (1 = use the three-sweep two-axis FFT passes when the lattice
- * allows, 0 = one pass per axis), "fft_xy_planes" ((x, y) planes per CTA, 0 = automatic),
+ * allows, 0 = one pass per axis), "fft_reg" (1 = use the register-line sweeps when the lattice allows), "fft_xy_planes" ((x, y) planes per CTA, 0 = automatic),
  * "fft_zt_xc" (consecutive (x, y) indices per CTA of the (z, t) pass, 0 = automatic).
  * Unknown key or NULL: LGF_EINVAL.  Synchronises. */
 int lgf_tune(lgf_ctx *ctx, const char *key, int value);
@@ -135,7 +138,8 @@ int lgf_fft_passes(const lgf_ctx *ctx);
 
 /* Kernel classes for per-kernel timing. */
 enum { LGF_K_DELTA = 0, LGF_K_FFT = 1, LGF_K_UPDATE = 2, LGF_K_GBUILD = 3, LGF_K_CONVERT = 4,
-       LGF_K_PLAQ = 5, LGF_K_COUNT = 6 };
+       LGF_K_PLAQ = 5, LGF_K_COUNT = 6,
+       LGF_K_ITERATION = 100 /* lgf_algorithmic_bytes only: the whole-iteration yard-stick */ };
 /* When on != 0 every kernel launch is bracketed by CUDA events on the context's stream. */
 int lgf_set_profiling(lgf_ctx *ctx, int on);
 /* Sum of the event-measured durations (ms) and the number of launches per kernel class since
@@ -144,7 +148,9 @@ int lgf_kernel_times(lgf_ctx *ctx, double *ms, long long *launches);
 /* Total number of kernels this context has launched since creation. */
 long long lgf_launch_count(const lgf_ctx *ctx);
 /* Algorithmic bytes one launch-set of the given kernel class must move for ONE iteration
- * (DESIGN.md "Algorithmic bytes"): e.g. LGF_K_DELTA -> V * (4*n_l + 8) * bytes_per_real. */
+ * (DESIGN.md "Algorithmic bytes"): e.g. LGF_K_DELTA -> V * (4*n_l + 8) * bytes_per_real;
+ * LGF_K_UPDATE is the fused sweep (a6 + a1): V * (8*n_l + 16); LGF_K_ITERATION the whole-iteration
+ * yard-stick V * (12*n_l + 64) of SURVEY.md section 8(d). */
 double lgf_algorithmic_bytes(const lgf_ctx *ctx, int kernel_class);
 
 const char *lgf_last_error(const lgf_ctx *ctx);

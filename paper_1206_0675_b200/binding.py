@@ -21,6 +21,7 @@ LGF_FP32, LGF_FP64 = 4, 8
 LGF_LINKS_18, LGF_LINKS_12 = 18, 12
 LGF_OK, LGF_EINVAL, LGF_ENOMEM, LGF_ECUDA, LGF_ESTATE, LGF_ENAN = 0, -1, -2, -3, -4, -5
 LGF_K_DELTA, LGF_K_FFT, LGF_K_UPDATE, LGF_K_GBUILD, LGF_K_CONVERT, LGF_K_PLAQ, LGF_K_COUNT = 0, 1, 2, 3, 4, 5, 6
+LGF_K_ITERATION = 100
 KERNEL_CLASSES = ("delta", "fft", "update", "gbuild", "convert", "plaquette")
 
 _LIBPATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "liblgf.so")

@@ -12,14 +12,18 @@
 #include "lgf_state.cuh"
 
 using namespace lgf;
+namespace lgf { extern int g_sweep_minb; }
 
 struct lgf_ctx {
     Geom g{};
     int prec = 0;        // bytes per real
     int nr = 3;          // stored rows per link
     cudaStream_t stream = nullptr;
-    void *links = nullptr;       // C<R>[4][3*nr][V]
-    void *W = nullptr;           // C<R>[4][V]
+    void *links[2] = {nullptr, nullptr};   // C<R>[4][3*nr][V] each: the sweep reads one and writes the other
+    void *W = nullptr;           // C<R>[4][V]   packed Delta / w
+    void *G = nullptr;           // C<R>[6][V]   rows 0, 1 of g(x)
+    bool w_is_delta = false;     // W holds Delta of the current configuration and `partial` its F / theta sums
+    int nb_partial = 0;          // number of per-block partial sums currently in `partial`
     double *partial = nullptr;   // per-block partial sums
     int partial_cap = 0;
     DevState *st = nullptr;
@@ -34,6 +38,7 @@ struct lgf_ctx {
     bool have_links = false;
     bool profiling = false;
     int tune_two_axis = 1;       // lgf_tune: use the two-axis FFT passes when available
+    int tune_reg = 1;            // lgf_tune: use the register-line FFT sweeps when available
     int tune_xy_planes = 0;      // lgf_tune: planes per CTA of the (x, y) pass (0 = planner's choice)
     int tune_zt_xc = 0;          // lgf_tune: consecutive (x, y) indices per CTA of the (z, t) pass
     struct Stamp { cudaEvent_t a, b; int cls; };
@@ -89,8 +94,7 @@ static void cossin_2pi(int m, int L, double &c, double &s) {
 }
 
 template <class R>
-static int upload_tables(lgf_ctx *ctx) {
-    std::vector<R> p2(4 * 64, (R)0);
+static int upload_twiddles(lgf_ctx *ctx) {
     for (int mu = 0; mu < 4; mu++) {
         const int L = ctx->g.L[mu];
         std::vector<R> tw(2 * 64, (R)0);
@@ -102,18 +106,30 @@ static int upload_tables(lgf_ctx *ctx) {
         }
         CK(cudaMalloc(&ctx->twiddle[mu], sizeof(R) * 2 * 64));
         CK(cudaMemcpy(ctx->twiddle[mu], tw.data(), sizeof(R) * 2 * 64, cudaMemcpyHostToDevice));
+    }
+    CK(cudaMalloc(&ctx->p2tab, sizeof(R) * 4 * 64));
+    return LGF_OK;
+}
+// p2tab[mu*64 + p] = 4 sin^2(pi k_mu(p) / L_mu), p = position along axis mu in k space: natural order
+// (k = p) for axes transformed in registers, the permuted order of the in-place two-step transform
+// (lgf_fft.cu header) otherwise.
+template <class R>
+static int upload_p2(lgf_ctx *ctx, const bool natural[4]) {
+    std::vector<R> p2(4 * 64, (R)0);
+    for (int mu = 0; mu < 4; mu++) {
+        const int L = ctx->g.L[mu];
         int N1, N2;
         line_factor(L, N1, N2);
         for (int p = 0; p < L; p++) {
-            const int k = (p / N2) + N1 * (p % N2);       // frequency held at position p (lgf_fft.cu header)
-            // 4 sin^2(pi k / L) = 2 (1 - cos(2 pi k / L))   -- use sin of the half angle for accuracy
+            const int k = natural[mu] ? p : (p / N2) + N1 * (p % N2);
+            // 4 sin^2(pi k / L): sine of the half angle, pi k / L = 2 pi k / (2L)
             double c, s;
-            cossin_2pi(k, 2 * L, c, s);                   // angle 2 pi k / (2L) = pi k / L
+            cossin_2pi(k, 2 * L, c, s);
             p2[mu * 64 + p] = (R)(4.0 * s * s);
         }
     }
-    CK(cudaMalloc(&ctx->p2tab, sizeof(R) * 4 * 64));
-    CK(cudaMemcpy(ctx->p2tab, p2.data(), sizeof(R) * 4 * 64, cudaMemcpyHostToDevice));
+    CK(cudaMemcpyAsync(ctx->p2tab, p2.data(), sizeof(R) * 4 * 64, cudaMemcpyHostToDevice, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
     return LGF_OK;
 }
 
@@ -134,7 +150,7 @@ static long long pow2_divisor_le(long long n, long long cap) {
 // scale + inverse, (x, y) planes inverse -- when two-axis kernels exist for the lattice's lengths and
 // the tiles fit in shared memory; otherwise one pass per axis (forward x, y, z; forward + scale +
 // inverse on t; inverse z, y, x).  tune_xy_planes / tune_zt_xc (> 0) override the tile sizes.
-static void plan_passes(lgf_ctx *ctx) {
+static int plan_passes(lgf_ctx *ctx) {
     const long long T = 2048;     // target complex elements per tile of the one-axis passes
     const size_t cbytes = 2 * (size_t)ctx->prec;
     const Geom &g = ctx->g;
@@ -158,6 +174,21 @@ static void plan_passes(lgf_ctx *ctx) {
         p.threads = 256;
         return p;
     };
+    auto finish = [&](const bool natural[4]) {
+        return ctx->prec == LGF_FP64 ? upload_p2<double>(ctx, natural) : upload_p2<float>(ctx, natural);
+    };
+    ctx->passes.clear();
+    if (ctx->tune_two_axis && ctx->tune_reg && fft_reg_supported(g)) {
+        for (int w = 0; w < 3; w++) {
+            AxisPass p{};
+            p.kind = PASS_REG;
+            p.axis = w;
+            ctx->passes.push_back(p);
+        }
+        const bool natural[4] = {true, true, true, fft_reg_t_natural(g)};
+        return finish(natural);
+    }
+    const bool permuted[4] = {false, false, false, false};
     const size_t SMEM_MAX = 200 * 1024;
     const long long MIN_GRID = 2 * 148;
     // (x, y) planes
@@ -190,7 +221,6 @@ static void plan_passes(lgf_ctx *ctx) {
         zt.smem = (128 + (size_t)pitch * g.L[3]) * cbytes;
         have_zt = zt.smem <= SMEM_MAX;
     }
-    ctx->passes.clear();
     if (have_xy) { xy.mode = FFT_FWD; ctx->passes.push_back(xy); }
     else { ctx->passes.push_back(make(0, FFT_FWD)); ctx->passes.push_back(make(1, FFT_FWD)); }
     if (have_zt) ctx->passes.push_back(zt);
@@ -201,6 +231,7 @@ static void plan_passes(lgf_ctx *ctx) {
     }
     if (have_xy) { xy.mode = FFT_INV; ctx->passes.push_back(xy); }
     else { ctx->passes.push_back(make(1, FFT_INV)); ctx->passes.push_back(make(0, FFT_INV)); }
+    return finish(permuted);
 }
 
 // ---- profiling brackets ---------------------------------------------------------------------------
@@ -238,9 +269,16 @@ static void drain_stamps(lgf_ctx *ctx) {
 
 // ---- typed steps ----------------------------------------------------------------------------------
 template <class R>
-static int step_delta(lgf_ctx *ctx, const int *stop, int *nblocks) {
+static LinkPair<R> link_pair(lgf_ctx *ctx) {
+    LinkPair<R> lp;
+    lp.buf[0] = (C<R> *)ctx->links[0];
+    lp.buf[1] = (C<R> *)ctx->links[1];
+    return lp;
+}
+template <class R>
+static int step_delta(lgf_ctx *ctx, const int *stop) {
     Bracket br(ctx, LGF_K_DELTA);
-    CK(launch_delta<R>(ctx->nr, (const C<R> *)ctx->links, (C<R> *)ctx->W, ctx->g, ctx->partial, nblocks, stop,
+    CK(launch_delta<R>(ctx->nr, link_pair<R>(ctx), (C<R> *)ctx->W, ctx->g, ctx->partial, &ctx->nb_partial, stop, ctx->st,
                        ctx->stream));
     return LGF_OK;
 }
@@ -249,41 +287,65 @@ static int step_accelerate(lgf_ctx *ctx) {
     const R scale = (R)(16.0 / (double)ctx->g.V);        // p2max / V      (Alg. 1 lines 5, 7; R5, R7)
     for (const AxisPass &p : ctx->passes) {
         Bracket br(ctx, LGF_K_FFT);
+        if (p.kind == PASS_REG) {
+            CK(launch_fft_reg<R>(p.axis, ctx->g, (C<R> *)ctx->W, (const R *)ctx->twiddle[3], (const R *)ctx->p2tab, scale,
+                                 ctx->st, ctx->stream));
+            continue;
+        }
         const R *tw[4] = {(const R *)ctx->twiddle[0], (const R *)ctx->twiddle[1], (const R *)ctx->twiddle[2],
                           (const R *)ctx->twiddle[3]};
         CK(launch_fft_pass<R>(p, (C<R> *)ctx->W, ctx->g, tw, (const R *)ctx->p2tab, scale, ctx->st, ctx->stream));
     }
     return LGF_OK;
 }
+// a5 then a6 + a1: g from the current W, then the fused sweep (new links into the other buffer, Delta of
+// the new links into W, partial sums of F and theta)
 template <class R>
 static int step_update(lgf_ctx *ctx, double alpha) {
+    {
+        Bracket br(ctx, LGF_K_GBUILD);
+        CK(launch_gbuild<R>((const C<R> *)ctx->W, (C<R> *)ctx->G, ctx->g, (R)(0.5 * alpha), ctx->st, ctx->stream));
+    }
     Bracket br(ctx, LGF_K_UPDATE);
-    CK(launch_update<R>(ctx->nr, (C<R> *)ctx->links, (const C<R> *)ctx->W, ctx->g, (R)(0.5 * alpha), ctx->st,
-                        ctx->stream));
+    CK(launch_sweep<R>(ctx->nr, link_pair<R>(ctx), (const C<R> *)ctx->G, (C<R> *)ctx->W, ctx->g, ctx->partial,
+                       &ctx->nb_partial, ctx->st, ctx->stream));
     return LGF_OK;
 }
-static int step_finalize(lgf_ctx *ctx, int nblocks, double tol, int will_update, int record) {
+static int step_finalize(lgf_ctx *ctx, double tol, int after_sweep, int record) {
     ctx->launches++;
-    CK(launch_finalize(ctx->partial, nblocks, ctx->g.V, tol, will_update, record, ctx->st, ctx->hist, ctx->hist_cap,
-                       ctx->stream));
+    CK(launch_finalize(ctx->partial, ctx->nb_partial, ctx->g.V, tol, after_sweep, record, ctx->st, ctx->hist,
+                       ctx->hist_cap, ctx->stream));
     return LGF_OK;
 }
 
-// measure (a1 + finalize, recorded) then, unless stopped, accelerate and update: one pass of the
-// while-body of Algorithm 1 preceded by its loop test.
+// Alg. 1 line 1: Delta, F, theta of the loaded configuration, recorded as history entry 0 with the stop
+// test of line 2.  Skipped when W already holds Delta of the current configuration (left there by the
+// previous sweep, whose finalize has recorded it).
+template <class R>
+static int first_measure(lgf_ctx *ctx, double tol) {
+    if (ctx->w_is_delta) return LGF_OK;
+    int rc;
+    if ((rc = step_delta<R>(ctx, &ctx->st->done)) != LGF_OK) return rc;
+    if ((rc = step_finalize(ctx, tol, 0, 1)) != LGF_OK) return rc;
+    ctx->w_is_delta = true;
+    return LGF_OK;
+}
+// One pass of the while-body of Algorithm 1 (lines 3-17): accelerate, g, sweep (update + measure), then
+// the finalize that makes the new configuration current, records (F, theta) and applies the loop test.
+// Every kernel returns immediately once the device-side `done` flag is set.
 template <class R>
 static int iteration(lgf_ctx *ctx, double alpha, double tol) {
-    int nb = 0, rc;
-    if ((rc = step_delta<R>(ctx, &ctx->st->done, &nb)) != LGF_OK) return rc;
-    if ((rc = step_finalize(ctx, nb, tol, 1, 1)) != LGF_OK) return rc;
+    int rc;
     if ((rc = step_accelerate<R>(ctx)) != LGF_OK) return rc;
-    return step_update<R>(ctx, alpha);
+    if ((rc = step_update<R>(ctx, alpha)) != LGF_OK) return rc;
+    return step_finalize(ctx, tol, 1, 1);
 }
+// a1 on the current configuration without touching the history or the stop flag
 template <class R>
-static int measure_only(lgf_ctx *ctx, double tol, int record) {
-    int nb = 0, rc;
-    if ((rc = step_delta<R>(ctx, record ? &ctx->st->done : &ctx->st->zero, &nb)) != LGF_OK) return rc;
-    return step_finalize(ctx, nb, tol, 0, record);
+static int measure_only(lgf_ctx *ctx) {
+    int rc;
+    if ((rc = step_delta<R>(ctx, &ctx->st->zero)) != LGF_OK) return rc;
+    return step_finalize(ctx, -1.0, 0, 0);
 }
 
 #define DISPATCH(fn, ...) (ctx->prec == LGF_FP64 ? fn<double>(__VA_ARGS__) : fn<float>(__VA_ARGS__))
@@ -329,10 +391,12 @@ int lgf_create(const int dims[4], int precision, int link_storage, lgf_ctx **out
         cudaError_t ee = cudaMalloc(p, bytes);
         if (ee != cudaSuccess) rc = cuda_fail(ctx, ee, "cudaMalloc");
     };
-    alloc(&ctx->links, V * 4 * 3 * ctx->nr * cb);
+    alloc(&ctx->links[0], V * 4 * 3 * ctx->nr * cb);
+    alloc(&ctx->links[1], V * 4 * 3 * ctx->nr * cb);
     alloc(&ctx->W, V * 4 * cb);
-    ctx->partial_cap = (int)((V + 255) / 256) + 1;
-    alloc((void **)&ctx->partial, sizeof(double) * 2 * ctx->partial_cap);
+    alloc(&ctx->G, V * 6 * cb);
+    ctx->partial_cap = (int)((V + 127) / 128) + 1;
+    alloc((void **)&ctx->partial, sizeof(double) * 4 * ctx->partial_cap);
     alloc((void **)&ctx->st, sizeof(DevState));
     ctx->hist_cap = 1 << 20;
     alloc((void **)&ctx->hist, sizeof(double) * 2 * ctx->hist_cap);
@@ -341,9 +405,9 @@ int lgf_create(const int dims[4], int precision, int link_storage, lgf_ctx **out
         cudaError_t ee = cudaMallocHost((void **)&ctx->h_st, sizeof(DevState) + 4 * sizeof(double));
         if (ee != cudaSuccess) rc = cuda_fail(ctx, ee, "cudaMallocHost");
     }
-    if (rc == LGF_OK) rc = precision == LGF_FP64 ? upload_tables<double>(ctx) : upload_tables<float>(ctx);
+    if (rc == LGF_OK) rc = precision == LGF_FP64 ? upload_twiddles<double>(ctx) : upload_twiddles<float>(ctx);
+    if (rc == LGF_OK) rc = plan_passes(ctx);
     if (rc == LGF_OK) {
-        plan_passes(ctx);
         cudaError_t ee = launch_reset_state(ctx->st, ctx->stream);
         if (ee == cudaSuccess) ee = cudaStreamSynchronize(ctx->stream);
         if (ee != cudaSuccess) rc = cuda_fail(ctx, ee, "reset_state");
@@ -361,8 +425,10 @@ int lgf_destroy(lgf_ctx *ctx) {
     if (!ctx) return LGF_EINVAL;
     cudaStreamSynchronize(ctx->stream);
     drain_stamps(ctx);
-    cudaFree(ctx->links);
+    cudaFree(ctx->links[0]);
+    cudaFree(ctx->links[1]);
     cudaFree(ctx->W);
+    cudaFree(ctx->G);
     cudaFree(ctx->partial);
     cudaFree(ctx->st);
     cudaFree(ctx->hist);
@@ -388,12 +454,14 @@ int lgf_set_links(lgf_ctx *ctx, const void *d_links) {
     {
         Bracket br(ctx, LGF_K_CONVERT);
         if (ctx->prec == LGF_FP64)
-            CK(launch_convert_in<double>(ctx->nr, (const double *)d_links, (C<double> *)ctx->links, ctx->g, ctx->stream));
+            CK(launch_convert_in<double>(ctx->nr, (const double *)d_links, (C<double> *)ctx->links[0], ctx->g, ctx->stream));
         else
-            CK(launch_convert_in<float>(ctx->nr, (const float *)d_links, (C<float> *)ctx->links, ctx->g, ctx->stream));
+            CK(launch_convert_in<float>(ctx->nr, (const float *)d_links, (C<float> *)ctx->links[0], ctx->g, ctx->stream));
     }
-    CK(launch_reset_state(ctx->st, ctx->stream));
+    ctx->launches++;
+    CK(launch_reset_state(ctx->st, ctx->stream));        // also makes buffer 0 the current one
     ctx->have_links = true;
+    ctx->w_is_delta = false;
     return LGF_OK;
 }
 
@@ -402,9 +470,9 @@ int lgf_get_links(lgf_ctx *ctx, void *d_links) {
     if (!ctx->have_links) return fail(ctx, LGF_ESTATE, "lgf_get_links: no configuration loaded");
     Bracket br(ctx, LGF_K_CONVERT);
     if (ctx->prec == LGF_FP64)
-        CK(launch_convert_out<double>(ctx->nr, (const C<double> *)ctx->links, (double *)d_links, ctx->g, ctx->stream));
+        CK(launch_convert_out<double>(ctx->nr, link_pair<double>(ctx), (double *)d_links, ctx->g, ctx->st, ctx->stream));
     else
-        CK(launch_convert_out<float>(ctx->nr, (const C<float> *)ctx->links, (float *)d_links, ctx->g, ctx->stream));
+        CK(launch_convert_out<float>(ctx->nr, link_pair<float>(ctx), (float *)d_links, ctx->g, ctx->st, ctx->stream));
     return LGF_OK;
 }
 
@@ -440,34 +508,36 @@ int lgf_iterate(lgf_ctx *ctx, double alpha, int n) {
     if (!ctx->have_links) return fail(ctx, LGF_ESTATE, "lgf_iterate: no configuration loaded");
     ctx->launches++;
     CK(launch_clear_done(ctx->st, ctx->stream));
-    for (int i = 0; i < n; i++) {
-        // tol = -1: theta >= 0 never stops the loop; only a NaN does
-        const int rc = DISPATCH(iteration, ctx, alpha, -1.0);
-        if (rc != LGF_OK) return rc;
-    }
+    // tol = -1: theta >= 0 never stops the loop; only a NaN does
+    int rc = DISPATCH(first_measure, ctx, -1.0);
+    if (rc != LGF_OK) return rc;
+    for (int i = 0; i < n; i++)
+        if ((rc = DISPATCH(iteration, ctx, alpha, -1.0)) != LGF_OK) return rc;
     return LGF_OK;
 }
 
 int lgf_measure(lgf_ctx *ctx, double *F, double *theta, double *plaquette) {
     if (!ctx) return LGF_EINVAL;
     if (!ctx->have_links) return fail(ctx, LGF_ESTATE, "lgf_measure: no configuration loaded");
-    if (F || theta) {
-        const int rc = DISPATCH(measure_only, ctx, -1.0, 0);
-        if (rc != LGF_OK) return rc;
-    }
-    if (plaquette) {
+    if (plaquette) {                 // uses the second half of the partial-sum buffer
         int nb = 0;
+        double *part = ctx->partial + 2 * ctx->partial_cap;
         {
             Bracket br(ctx, LGF_K_PLAQ);
             if (ctx->prec == LGF_FP64)
-                CK(launch_plaquette<double>(ctx->nr, (const C<double> *)ctx->links, ctx->g, ctx->partial, &nb, ctx->stream));
+                CK(launch_plaquette<double>(ctx->nr, link_pair<double>(ctx), ctx->g, part, &nb, ctx->st, ctx->stream));
             else
-                CK(launch_plaquette<float>(ctx->nr, (const C<float> *)ctx->links, ctx->g, ctx->partial, &nb, ctx->stream));
+                CK(launch_plaquette<float>(ctx->nr, link_pair<float>(ctx), ctx->g, part, &nb, ctx->st, ctx->stream));
         }
         ctx->launches++;
-        CK(launch_sum1(ctx->partial, nb, 1.0 / (18.0 * (double)ctx->g.V), ctx->d_scalar, ctx->stream));
+        CK(launch_sum1(part, nb, 1.0 / (18.0 * (double)ctx->g.V), ctx->d_scalar, ctx->stream));
         double *hp = reinterpret_cast<double *>(ctx->h_st + 1);
         CK(cudaMemcpyAsync(hp, ctx->d_scalar, sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    }
+    if (F || theta) {
+        const int rc = DISPATCH(measure_only, ctx);
+        if (rc != LGF_OK) return rc;
+        ctx->w_is_delta = true;
     }
     const int rc = fetch_state(ctx);
     if (rc != LGF_OK) return rc;
@@ -480,24 +550,19 @@ int lgf_measure(lgf_ctx *ctx, double *F, double *theta, double *plaquette) {
 // Algorithm 1 on the configuration already loaded in the context.
 static long long fix_loaded(lgf_ctx *ctx, double alpha, double tol, long long max_iter) {
     const int CHUNK = 16;      // iterations enqueued between two looks at the device-side stop flag
+    int rc = DISPATCH(first_measure, ctx, tol);                         // line 1 (+ the first loop test)
+    if (rc != LGF_OK) return rc;
     long long issued = 0;
     bool done = false;
     while (issued < max_iter && !done) {
         const long long n = (max_iter - issued < CHUNK) ? (max_iter - issued) : CHUNK;
-        for (long long i = 0; i < n; i++) {
-            const int rc = DISPATCH(iteration, ctx, alpha, tol);
-            if (rc != LGF_OK) return rc;
-        }
+        for (long long i = 0; i < n; i++)
+            if ((rc = DISPATCH(iteration, ctx, alpha, tol)) != LGF_OK) return rc;
         issued += n;
-        const int rc = fetch_state(ctx);
-        if (rc != LGF_OK) return rc;
+        if ((rc = fetch_state(ctx)) != LGF_OK) return rc;
         done = ctx->h_st->done != 0;
     }
-    if (!done) {               // Alg. 1 line 17 after the last update
-        int rc = DISPATCH(measure_only, ctx, tol, 1);
-        if (rc != LGF_OK) return rc;
-        if ((rc = fetch_state(ctx)) != LGF_OK) return rc;
-    }
+    if ((rc = fetch_state(ctx)) != LGF_OK) return rc;
     if (ctx->h_st->nan) return fail(ctx, LGF_ENAN, "lgf_fix: theta is NaN/Inf");
     return ctx->h_st->n_updates;
 }
@@ -557,8 +622,9 @@ long long lgf_history_length(lgf_ctx *ctx) {
 int lgf_step_delta(lgf_ctx *ctx, double *F, double *theta) {
     if (!ctx) return LGF_EINVAL;
     if (!ctx->have_links) return fail(ctx, LGF_ESTATE, "lgf_step_delta: no configuration loaded");
-    int rc = DISPATCH(measure_only, ctx, -1.0, 0);
+    int rc = DISPATCH(measure_only, ctx);
     if (rc != LGF_OK) return rc;
+    ctx->w_is_delta = true;
     if (F || theta) {
         if ((rc = fetch_state(ctx)) != LGF_OK) return rc;
         if (F) *F = ctx->h_st->F;
@@ -571,6 +637,7 @@ int lgf_step_accelerate(lgf_ctx *ctx) {
     if (!ctx) return LGF_EINVAL;
     ctx->launches++;
     CK(launch_clear_done(ctx->st, ctx->stream));
+    ctx->w_is_delta = false;
     return DISPATCH(step_accelerate, ctx);
 }
 
@@ -579,7 +646,10 @@ int lgf_step_update(lgf_ctx *ctx, double alpha) {
     if (!ctx->have_links) return fail(ctx, LGF_ESTATE, "lgf_step_update: no configuration loaded");
     ctx->launches++;
     CK(launch_clear_done(ctx->st, ctx->stream));
-    return DISPATCH(step_update, ctx, alpha);
+    const int rc = DISPATCH(step_update, ctx, alpha);
+    if (rc != LGF_OK) return rc;
+    ctx->w_is_delta = true;            // the sweep left Delta of the new links in W
+    return step_finalize(ctx, -1.0, 1, 0);
 }
 
 int lgf_get_field(lgf_ctx *ctx, void *d_field) {
@@ -595,6 +665,7 @@ int lgf_set_field(lgf_ctx *ctx, const void *d_field) {
     ctx->launches++;
     if (ctx->prec == LGF_FP64) CK(launch_field_set<double>((C<double> *)ctx->W, (const double *)d_field, ctx->g, ctx->stream));
     else CK(launch_field_set<float>((C<float> *)ctx->W, (const float *)d_field, ctx->g, ctx->stream));
+    ctx->w_is_delta = false;
     return LGF_OK;
 }
 
@@ -602,12 +673,13 @@ int lgf_tune(lgf_ctx *ctx, const char *key, int value) {
     if (!ctx || !key) return fail(ctx, LGF_EINVAL, "lgf_tune: null argument");
     const std::string k(key);
     if (k == "fft_two_axis") ctx->tune_two_axis = value;
+    else if (k == "fft_reg") ctx->tune_reg = value;
     else if (k == "fft_xy_planes") ctx->tune_xy_planes = value;
     else if (k == "fft_zt_xc") ctx->tune_zt_xc = value;
+    else if (k == "sweep_minb") lgf::g_sweep_minb = value;
     else return fail(ctx, LGF_EINVAL, "lgf_tune: unknown key " + k);
     CK(cudaStreamSynchronize(ctx->stream));
-    plan_passes(ctx);
-    return LGF_OK;
+    return plan_passes(ctx);
 }
 
 int lgf_fft_passes(const lgf_ctx *ctx) { return ctx ? (int)ctx->passes.size() : LGF_EINVAL; }
@@ -640,7 +712,9 @@ double lgf_algorithmic_bytes(const lgf_ctx *ctx, int kernel_class) {
     switch (kernel_class) {
         case LGF_K_DELTA: return V * (4.0 * nl + 8.0) * R;        // read 4 links, write packed Delta
         case LGF_K_FFT: return V * 3.0 * 16.0 * R;                // three read+write sweeps of the packed field
-        case LGF_K_UPDATE: return V * (8.0 + 8.0 * nl) * R;       // read w and 4 links, write 4 links
+        case LGF_K_UPDATE: return V * (8.0 * nl + 16.0) * R;      // fused sweep: read w-equivalent + 4 links, write 4 links + Delta
+        case LGF_K_GBUILD: return V * 20.0 * R;                   // read w (8), write rows 0, 1 of g (12)
+        case LGF_K_ITERATION: return V * (12.0 * nl + 64.0) * R;  // SURVEY.md section 8(d) yard-stick
         case LGF_K_PLAQ: return V * 4.0 * nl * R;
         case LGF_K_CONVERT: return V * (72.0 + 4.0 * nl) * R;
         default: return 0.0;

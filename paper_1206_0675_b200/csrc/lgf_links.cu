@@ -1,6 +1,9 @@
 // lgf_links.cu -- the link-side kernels of the gauge-fixing iteration:
-//   k_delta     a1: A_mu, Delta(x), per-block partial sums for F and theta   (eqs. 3, 5-7; Alg. 1 lines 1, 17)
-//   k_update    a5 + a6: g(x) = GS(1 + i (alpha/2) w(x)),  U_mu(x) <- g(x) U_mu(x) g(x+mu)^dag   (Alg. 1 lines 10, 14)
+//   k_delta     a1: A_mu, Delta(x), per-block partial sums for F and theta   (eqs. 3, 5-7; Alg. 1 line 1)
+//   k_gbuild    a5: g(x) = GS(1 + i (alpha/2) w(x))                          (Alg. 1 line 10)
+//   k_sweep     a6 + a1 fused: U'_mu(x) = g(x) U_mu(x) g(x+mu)^dag (Alg. 1 line 14) and, in the same pass,
+//               Delta, F, theta of the NEW configuration (Alg. 1 line 17) -- the links are read once
+//               and written once per iteration
 //   k_plaquette average plaquette partial sums (gauge-invariant check)
 //   k_finalize  final fixed-order sum, F / theta normalisation, history, stop test (Alg. 1 line 2)
 //   layout conversion canonical AoS <-> internal SoA, packed field <-> full 3x3 field
@@ -10,13 +13,16 @@
 namespace lgf {
 
 constexpr int SITE_THREADS = 256;
+constexpr int SWEEP_THREADS = 128;
+int g_sweep_minb = 3;   // experiment knob
 
 // ---- a1 -------------------------------------------------------------------------------------------
 template <class R, int NR>
-__global__ void __launch_bounds__(SITE_THREADS) k_delta(const C<R> *__restrict__ links, C<R> *__restrict__ W, Geom g,
-                                                         double *__restrict__ partial,
-                                                         const int *__restrict__ stop) {
+__global__ void __launch_bounds__(SITE_THREADS) k_delta(LinkPair<R> lp, C<R> *__restrict__ W, Geom g,
+                                                         double *__restrict__ partial, const int *__restrict__ stop,
+                                                         const DevState *__restrict__ st) {
     if (*stop) return;
+    const C<R> *__restrict__ links = lp.buf[st->cur];
     __shared__ double scratch[SITE_THREADS / 32][2];
     const long long s = (long long)blockIdx.x * SITE_THREADS + threadIdx.x;
     double f = 0.0, t = 0.0;
@@ -45,32 +51,95 @@ __global__ void __launch_bounds__(SITE_THREADS) k_delta(const C<R> *__restrict__
     }
 }
 
-// ---- a5 + a6 --------------------------------------------------------------------------------------
-template <class R, int NR>
-__global__ void __launch_bounds__(SITE_THREADS) k_update(C<R> *__restrict__ links, const C<R> *__restrict__ W, Geom g,
+// ---- a5 -------------------------------------------------------------------------------------------
+// g(x) from w(x); rows 0 and 1 are stored (G[e][s], e = 0..5), row 2 is (row0 x row1)^* by construction
+// (eq. 8), so rebuilding it on load reproduces it exactly.
+template <class R>
+__global__ void __launch_bounds__(SITE_THREADS) k_gbuild(const C<R> *__restrict__ W, C<R> *__restrict__ G, Geom g,
                                                           R half_alpha, const DevState *__restrict__ st) {
     if (st->done) return;
     const long long s = (long long)blockIdx.x * SITE_THREADS + threadIdx.x;
     if (s >= g.V) return;
-    int c[4];
-    site_coords(g, s, c);
     C<R> gx[9];
     build_g(load_herm(W, g.V, s), half_alpha, gx);
 #pragma unroll
-    for (int mu = 0; mu < 4; mu++) {
-        C<R> gf[9], u[9], tmp[9], r[9];
-        build_g(load_herm(W, g.V, site_fwd(g, s, c, mu)), half_alpha, gf);
-        load_link<R, NR>(links, g.V, mu, s, u);
-        mat_mul<NR>(gx, u, tmp);
-        mat_mul_dag<NR>(tmp, gf, r);
-        store_link<R, NR>(links, g.V, mu, s, r);
+    for (int e = 0; e < 6; e++) G[(long long)e * g.V + s] = gx[e];
+}
+
+template <class R>
+__device__ __forceinline__ void load_g(const C<R> *__restrict__ G, long long V, long long s, C<R> (&gx)[9]) {
+#pragma unroll
+    for (int e = 0; e < 6; e++) gx[e] = G[(long long)e * V + s];
+    reconstruct_row2(gx);
+}
+
+// out = a * b * c^dag as it will be seen by whoever loads the stored link later: with 12-real storage
+// only rows 0 and 1 are computed and row 2 is rebuilt from them (eq. 8), exactly as load_link does.
+template <int NR, class R>
+__device__ __forceinline__ void transform_link(const C<R> (&a)[9], const C<R> (&b)[9], const C<R> (&c)[9],
+                                               C<R> (&out)[9]) {
+    C<R> t[9];
+    mat_mul<NR>(a, b, t);
+    mat_mul_dag<NR>(t, c, out);
+    if constexpr (NR == 2) reconstruct_row2(out);
+}
+
+// ---- a6 + a1 fused --------------------------------------------------------------------------------
+// One thread per site x.  For every direction: the site's own new link U'_mu(x) = g(x) U_mu(x) g(x+mu)^dag
+// is computed, stored to the other link buffer and its algebra part subtracted from Delta(x); the new
+// link of the backward neighbour, U'_mu(x-mu) = g(x-mu) U_mu(x-mu) g(x)^dag, is recomputed (its inputs
+// are L1/L2 hits: the neighbouring thread reads the same lines) and its algebra part added.  Reads
+// buffer `cur`, writes buffer 1-cur (k_finalize flips `cur`), so no thread ever sees a half-updated
+// neighbourhood (Jacobi update, R10).
+template <class R, int NR, int MINB>
+__global__ void __launch_bounds__(SWEEP_THREADS, MINB) k_sweep(LinkPair<R> lp, const C<R> *__restrict__ G,
+                                                          C<R> *__restrict__ W, Geom g, double *__restrict__ partial,
+                                                          const DevState *__restrict__ st) {
+    if (st->done) return;
+    const int cur = st->cur;
+    const C<R> *__restrict__ src = lp.buf[cur];
+    C<R> *__restrict__ dst = lp.buf[1 - cur];
+    __shared__ double scratch[SWEEP_THREADS / 32][2];
+    const long long s = (long long)blockIdx.x * SWEEP_THREADS + threadIdx.x;
+    double f = 0.0, t = 0.0;
+    if (s < g.V) {
+        int c[4];
+        site_coords(g, s, c);
+        C<R> gx[9];
+        load_g(G, g.V, s, gx);
+        Herm<R> d = herm_zero<R>();
+        R retr = 0;
+#pragma unroll
+        for (int mu = 0; mu < 4; mu++) {
+            C<R> u[9], gn[9], p[9];
+            load_link<R, NR>(src, g.V, mu, s, u);
+            load_g(G, g.V, site_fwd(g, s, c, mu), gn);
+            transform_link<NR>(gx, u, gn, p);                       // Alg. 1 line 14, eq. 2
+            store_link<R, NR>(dst, g.V, mu, s, p);
+            retr += p[0].x + p[4].x + p[8].x;                       // eq. 3 on the new link
+            herm_sub(d, algebra_part(p));                           // - A'_mu(x)
+            const long long sb = site_bwd(g, s, c, mu);
+            load_link<R, NR>(src, g.V, mu, sb, u);
+            load_g(G, g.V, sb, gn);
+            transform_link<NR>(gn, u, gx, p);
+            herm_add(d, algebra_part(p));                           // + A'_mu(x - mu)     (eq. 5)
+        }
+        store_herm(W, g.V, s, d);
+        f = (double)retr;
+        t = (double)herm_norm2(d);
+    }
+    block_sum2(f, t, scratch);
+    if (threadIdx.x == 0) {
+        partial[2 * blockIdx.x] = f;
+        partial[2 * blockIdx.x + 1] = t;
     }
 }
 
 // ---- plaquette ------------------------------------------------------------------------------------
 template <class R, int NR>
-__global__ void __launch_bounds__(SITE_THREADS) k_plaquette(const C<R> *__restrict__ links, Geom g,
-                                                             double *__restrict__ partial) {
+__global__ void __launch_bounds__(SITE_THREADS) k_plaquette(LinkPair<R> lp, Geom g, double *__restrict__ partial,
+                                                             const DevState *__restrict__ st) {
+    const C<R> *__restrict__ links = lp.buf[st->cur];
     __shared__ double scratch[SITE_THREADS / 32][2];
     const long long s = (long long)blockIdx.x * SITE_THREADS + threadIdx.x;
     double p = 0.0, dummy = 0.0;
@@ -101,9 +170,9 @@ __global__ void __launch_bounds__(SITE_THREADS) k_plaquette(const C<R> *__restri
 // One block; fixed summation order (thread i takes partials i, i+1024, ...), so F and theta are
 // bit-reproducible from run to run.
 __global__ void __launch_bounds__(1024) k_finalize(const double *__restrict__ partial, int nblocks, long long V,
-                                                    double tol, int will_update, int record, DevState *st,
+                                                    double tol, int after_sweep, int record, DevState *st,
                                                     double *__restrict__ hist, long long hist_cap) {
-    if (record && st->done) return;
+    if ((record || after_sweep) && st->done) return;      // the kernels before this one did not run
     __shared__ double scratch[32][2];
     double f = 0.0, t = 0.0;
     for (int i = threadIdx.x; i < nblocks; i += 1024) {
@@ -116,13 +185,16 @@ __global__ void __launch_bounds__(1024) k_finalize(const double *__restrict__ pa
         const double theta = t / (3.0 * (double)V);       // eq. 6: 1 / (N_c V)
         st->F = F;
         st->theta = theta;
+        if (after_sweep) {                                // the sweep wrote the other buffer: make it current
+            st->cur = 1 - st->cur;
+            st->n_updates += 1;
+        }
         if (record) {
             const long long n = st->n_hist;
             if (n < hist_cap) { hist[2 * n] = F; hist[2 * n + 1] = theta; }
             st->n_hist = n + 1;
             if (!(theta == theta) || theta > 1e300) { st->done = 1; st->nan = 1; }
             else if (theta < tol) st->done = 1;           // Alg. 1 line 2: loop while theta >= eps
-            else if (will_update) st->n_updates += 1;
         }
     }
 }
@@ -138,6 +210,7 @@ __global__ void __launch_bounds__(1024) k_sum1(const double *__restrict__ partia
 
 __global__ void k_reset_state(DevState *st) {
     st->n_hist = 0; st->n_updates = 0; st->done = 0; st->nan = 0; st->F = 0.0; st->theta = 0.0; st->zero = 0;
+    st->cur = 0;
 }
 __global__ void k_clear_done(DevState *st) { st->done = 0; }
 
@@ -155,8 +228,9 @@ __global__ void __launch_bounds__(SITE_THREADS) k_convert_in(const R *__restrict
         for (int e = 0; e < 3 * NR; e++) links[((long long)mu * (3 * NR) + e) * g.V + s] = src[mu * 9 + e];
 }
 template <class R, int NR>
-__global__ void __launch_bounds__(SITE_THREADS) k_convert_out(const C<R> *__restrict__ links, R *__restrict__ canon,
-                                                               Geom g) {
+__global__ void __launch_bounds__(SITE_THREADS) k_convert_out(LinkPair<R> lp, R *__restrict__ canon, Geom g,
+                                                               const DevState *__restrict__ st) {
+    const C<R> *__restrict__ links = lp.buf[st->cur];
     const long long s = (long long)blockIdx.x * SITE_THREADS + threadIdx.x;
     if (s >= g.V) return;
     C<R> *dst = reinterpret_cast<C<R> *>(canon) + s * 36;
@@ -201,43 +275,58 @@ __global__ void __launch_bounds__(SITE_THREADS) k_field_set(C<R> *__restrict__ W
 static inline int site_blocks(const Geom &g) { return (int)((g.V + SITE_THREADS - 1) / SITE_THREADS); }
 
 template <class R>
-cudaError_t launch_delta(int nr, const C<R> *links, C<R> *W, const Geom &g, double *partial, int *nblocks,
-                         const int *stop, cudaStream_t stream) {
+cudaError_t launch_delta(int nr, LinkPair<R> links, C<R> *W, const Geom &g, double *partial, int *nblocks,
+                         const int *stop, const DevState *st, cudaStream_t stream) {
     const int nb = site_blocks(g);
     *nblocks = nb;
-    if (nr == 3) k_delta<R, 3><<<nb, SITE_THREADS, 0, stream>>>(links, W, g, partial, stop);
-    else k_delta<R, 2><<<nb, SITE_THREADS, 0, stream>>>(links, W, g, partial, stop);
+    if (nr == 3) k_delta<R, 3><<<nb, SITE_THREADS, 0, stream>>>(links, W, g, partial, stop, st);
+    else k_delta<R, 2><<<nb, SITE_THREADS, 0, stream>>>(links, W, g, partial, stop, st);
     return cudaGetLastError();
 }
 template <class R>
-cudaError_t launch_update(int nr, C<R> *links, const C<R> *W, const Geom &g, R half_alpha, const DevState *st,
-                          cudaStream_t stream) {
-    const int nb = site_blocks(g);
-    if (nr == 3) k_update<R, 3><<<nb, SITE_THREADS, 0, stream>>>(links, W, g, half_alpha, st);
-    else k_update<R, 2><<<nb, SITE_THREADS, 0, stream>>>(links, W, g, half_alpha, st);
+cudaError_t launch_gbuild(const C<R> *W, C<R> *G, const Geom &g, R half_alpha, const DevState *st, cudaStream_t stream) {
+    k_gbuild<R><<<site_blocks(g), SITE_THREADS, 0, stream>>>(W, G, g, half_alpha, st);
     return cudaGetLastError();
 }
 template <class R>
-cudaError_t launch_plaquette(int nr, const C<R> *links, const Geom &g, double *partial, int *nblocks,
-                             cudaStream_t stream) {
+cudaError_t launch_sweep(int nr, LinkPair<R> links, const C<R> *G, C<R> *W, const Geom &g, double *partial,
+                         int *nblocks, const DevState *st, cudaStream_t stream) {
+    const int nb = (int)((g.V + SWEEP_THREADS - 1) / SWEEP_THREADS);
+    *nblocks = nb;
+    switch (g_sweep_minb) {
+#define LGF_SW(M)                                                                                     \
+    case M:                                                                                           \
+        if (nr == 3) k_sweep<R, 3, M><<<nb, SWEEP_THREADS, 0, stream>>>(links, G, W, g, partial, st); \
+        else k_sweep<R, 2, M><<<nb, SWEEP_THREADS, 0, stream>>>(links, G, W, g, partial, st);         \
+        break;
+        LGF_SW(2) LGF_SW(3) LGF_SW(4) LGF_SW(5)
+#undef LGF_SW
+        default: return cudaErrorInvalidValue;
+    }
+    return cudaGetLastError();
+}
+template <class R>
+cudaError_t launch_plaquette(int nr, LinkPair<R> links, const Geom &g, double *partial, int *nblocks,
+                             const DevState *st, cudaStream_t stream) {
     const int nb = site_blocks(g);
     *nblocks = nb;
-    if (nr == 3) k_plaquette<R, 3><<<nb, SITE_THREADS, 0, stream>>>(links, g, partial);
-    else k_plaquette<R, 2><<<nb, SITE_THREADS, 0, stream>>>(links, g, partial);
+    if (nr == 3) k_plaquette<R, 3><<<nb, SITE_THREADS, 0, stream>>>(links, g, partial, st);
+    else k_plaquette<R, 2><<<nb, SITE_THREADS, 0, stream>>>(links, g, partial, st);
     return cudaGetLastError();
 }
 template <class R>
-cudaError_t launch_convert_in(int nr, const R *canon, C<R> *links, const Geom &g, cudaStream_t stream) {
+cudaError_t launch_convert_in(int nr, const R *canon, C<R> *links0, const Geom &g, cudaStream_t stream) {
     const int nb = site_blocks(g);
-    if (nr == 3) k_convert_in<R, 3><<<nb, SITE_THREADS, 0, stream>>>(canon, links, g);
-    else k_convert_in<R, 2><<<nb, SITE_THREADS, 0, stream>>>(canon, links, g);
+    if (nr == 3) k_convert_in<R, 3><<<nb, SITE_THREADS, 0, stream>>>(canon, links0, g);
+    else k_convert_in<R, 2><<<nb, SITE_THREADS, 0, stream>>>(canon, links0, g);
     return cudaGetLastError();
 }
 template <class R>
-cudaError_t launch_convert_out(int nr, const C<R> *links, R *canon, const Geom &g, cudaStream_t stream) {
+cudaError_t launch_convert_out(int nr, LinkPair<R> links, R *canon, const Geom &g, const DevState *st,
+                               cudaStream_t stream) {
     const int nb = site_blocks(g);
-    if (nr == 3) k_convert_out<R, 3><<<nb, SITE_THREADS, 0, stream>>>(links, canon, g);
-    else k_convert_out<R, 2><<<nb, SITE_THREADS, 0, stream>>>(links, canon, g);
+    if (nr == 3) k_convert_out<R, 3><<<nb, SITE_THREADS, 0, stream>>>(links, canon, g, st);
+    else k_convert_out<R, 2><<<nb, SITE_THREADS, 0, stream>>>(links, canon, g, st);
     return cudaGetLastError();
 }
 template <class R>
@@ -251,9 +340,9 @@ cudaError_t launch_field_set(C<R> *W, const R *field, const Geom &g, cudaStream_
     return cudaGetLastError();
 }
 
-cudaError_t launch_finalize(const double *partial, int nblocks, long long V, double tol, int will_update, int record,
+cudaError_t launch_finalize(const double *partial, int nblocks, long long V, double tol, int after_sweep, int record,
                             DevState *st, double *hist, long long hist_cap, cudaStream_t stream) {
-    k_finalize<<<1, 1024, 0, stream>>>(partial, nblocks, V, tol, will_update, record, st, hist, hist_cap);
+    k_finalize<<<1, 1024, 0, stream>>>(partial, nblocks, V, tol, after_sweep, record, st, hist, hist_cap);
     return cudaGetLastError();
 }
 cudaError_t launch_sum1(const double *partial, int nblocks, double norm, double *out, cudaStream_t stream) {
@@ -270,13 +359,16 @@ cudaError_t launch_clear_done(DevState *st, cudaStream_t stream) {
 }
 
 #define LGF_INST(R)                                                                                                   \
-    template cudaError_t launch_delta<R>(int, const C<R> *, C<R> *, const Geom &, double *, int *, const int *,        \
-                                         cudaStream_t);                                                                \
-    template cudaError_t launch_update<R>(int, C<R> *, const C<R> *, const Geom &, R, const DevState *, cudaStream_t); \
-    template cudaError_t launch_plaquette<R>(int, const C<R> *, const Geom &, double *, int *, cudaStream_t);          \
-    template cudaError_t launch_convert_in<R>(int, const R *, C<R> *, const Geom &, cudaStream_t);                     \
-    template cudaError_t launch_convert_out<R>(int, const C<R> *, R *, const Geom &, cudaStream_t);                    \
-    template cudaError_t launch_field_get<R>(const C<R> *, R *, const Geom &, cudaStream_t);                           \
+    template cudaError_t launch_delta<R>(int, LinkPair<R>, C<R> *, const Geom &, double *, int *, const int *,        \
+                                         const DevState *, cudaStream_t);                                             \
+    template cudaError_t launch_gbuild<R>(const C<R> *, C<R> *, const Geom &, R, const DevState *, cudaStream_t);     \
+    template cudaError_t launch_sweep<R>(int, LinkPair<R>, const C<R> *, C<R> *, const Geom &, double *, int *,       \
+                                         const DevState *, cudaStream_t);                                             \
+    template cudaError_t launch_plaquette<R>(int, LinkPair<R>, const Geom &, double *, int *, const DevState *,       \
+                                             cudaStream_t);                                                           \
+    template cudaError_t launch_convert_in<R>(int, const R *, C<R> *, const Geom &, cudaStream_t);                    \
+    template cudaError_t launch_convert_out<R>(int, LinkPair<R>, R *, const Geom &, const DevState *, cudaStream_t);  \
+    template cudaError_t launch_field_get<R>(const C<R> *, R *, const Geom &, cudaStream_t);                          \
     template cudaError_t launch_field_set<R>(C<R> *, const R *, const Geom &, cudaStream_t);
 LGF_INST(float)
 LGF_INST(double)

@@ -16,6 +16,15 @@ struct DevState {
     int nan;              // theta was NaN / Inf
     double F, theta;      // last measured values
     int zero;             // always 0: the `stop` word handed to kernels that must run regardless of `done`
+    int cur;              // which of the two link buffers holds the current configuration (0 / 1); the
+                          // sweep reads buffer `cur` and writes the other one, k_finalize flips it
+};
+
+// The two link buffers (ping-pong: the fused sweep needs U_mu(x - mu) of the OLD configuration while
+// other threads already write the new one).
+template <class R>
+struct LinkPair {
+    C<R> *buf[2];
 };
 
 enum FftMode { FFT_FWD = 0, FFT_INV = 1, FFT_FWD_SCALE_INV = 2 };
@@ -23,7 +32,9 @@ enum FftMode { FFT_FWD = 0, FFT_INV = 1, FFT_FWD_SCALE_INV = 2 };
 enum PassKind {
     PASS_AXIS = 0,        // one lattice axis per pass (any supported length)
     PASS_XY = 1,          // whole (x, y) planes: both axes transformed in one shared-memory tile
-    PASS_ZT = 2           // (z, t) planes of nlo consecutive (x, y) indices: forward z, t, scale, inverse t, z
+    PASS_ZT = 2,          // (z, t) planes of nlo consecutive (x, y) indices: forward z, t, scale, inverse t, z
+    PASS_REG = 3          // register-resident line transforms (lgf_fft_reg.cu); `axis` = 0: (x, y) forward,
+                          // 1: (z, t) forward + scale + inverse, 2: (x, y) inverse
 };
 
 // One FFT pass (see lgf_fft.cu).
@@ -47,29 +58,40 @@ template <class R>
 cudaError_t launch_fft_pass(const AxisPass &p, C<R> *W, const Geom &g, const R *const twiddle[4] /*[2*64] per axis*/,
                             const R *p2tab /*[4][64] permuted 4 sin^2*/, R scale, const DevState *st,
                             cudaStream_t stream);
+// register-line fast path (lgf_fft_reg.cu): available for this lattice?  is the t axis left in natural k order?
+bool fft_reg_supported(const Geom &g);
+bool fft_reg_t_natural(const Geom &g);
+template <class R>
+cudaError_t launch_fft_reg(int which, const Geom &g, C<R> *W, const R *twiddle_t, const R *p2tab, R scale,
+                           const DevState *st, cudaStream_t stream);
 // true if a PASS_XY (first two axes) / PASS_ZT (last two axes) kernel is instantiated for these lengths
 bool fft_pair_supported(int kind, int La, int Lb);
 
 template <class R>
-cudaError_t launch_delta(int nr, const C<R> *links, C<R> *W, const Geom &g, double *partial, int *nblocks,
-                         const int *stop, cudaStream_t stream);
+cudaError_t launch_delta(int nr, LinkPair<R> links, C<R> *W, const Geom &g, double *partial, int *nblocks,
+                         const int *stop, const DevState *st, cudaStream_t stream);
 template <class R>
-cudaError_t launch_update(int nr, C<R> *links, const C<R> *W, const Geom &g, R half_alpha, const DevState *st,
-                          cudaStream_t stream);
+cudaError_t launch_gbuild(const C<R> *W, C<R> *G, const Geom &g, R half_alpha, const DevState *st, cudaStream_t stream);
 template <class R>
-cudaError_t launch_plaquette(int nr, const C<R> *links, const Geom &g, double *partial, int *nblocks,
-                             cudaStream_t stream);
+cudaError_t launch_sweep(int nr, LinkPair<R> links, const C<R> *G, C<R> *W, const Geom &g, double *partial,
+                         int *nblocks, const DevState *st, cudaStream_t stream);
 template <class R>
-cudaError_t launch_convert_in(int nr, const R *canon, C<R> *links, const Geom &g, cudaStream_t stream);
+cudaError_t launch_plaquette(int nr, LinkPair<R> links, const Geom &g, double *partial, int *nblocks,
+                             const DevState *st, cudaStream_t stream);
 template <class R>
-cudaError_t launch_convert_out(int nr, const C<R> *links, R *canon, const Geom &g, cudaStream_t stream);
+cudaError_t launch_convert_in(int nr, const R *canon, C<R> *links0, const Geom &g, cudaStream_t stream);
+template <class R>
+cudaError_t launch_convert_out(int nr, LinkPair<R> links, R *canon, const Geom &g, const DevState *st,
+                               cudaStream_t stream);
 template <class R>
 cudaError_t launch_field_get(const C<R> *W, R *field, const Geom &g, cudaStream_t stream);
 template <class R>
 cudaError_t launch_field_set(C<R> *W, const R *field, const Geom &g, cudaStream_t stream);
 
 // F / theta finalisation (precision independent)
-cudaError_t launch_finalize(const double *partial, int nblocks, long long V, double tol, int will_update, int record,
+// after_sweep: the partial sums come from a sweep (flip `cur`, count the update); record: append (F, theta)
+// to the history and apply the stop test theta < tol
+cudaError_t launch_finalize(const double *partial, int nblocks, long long V, double tol, int after_sweep, int record,
                             DevState *st, double *hist, long long hist_cap, cudaStream_t stream);
 cudaError_t launch_sum1(const double *partial, int nblocks, double norm, double *out, cudaStream_t stream);
 cudaError_t launch_reset_state(DevState *st, cudaStream_t stream);

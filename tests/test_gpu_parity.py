@@ -82,23 +82,26 @@ def test_delta_F_theta(lgf, name, dims, prec, storage):
 
 
 ACC_DIMS = [(8, 8, 8, 8), (12, 6, 16, 4), (3, 24, 2, 48), (16, 16, 16, 16), (32, 8, 64, 4), (8, 8, 24, 48),
-            (24, 24, 24, 48), (32, 32, 16, 16), (64, 64, 8, 8), (8, 8, 64, 64)]
+            (24, 24, 24, 48), (32, 32, 16, 16), (64, 64, 8, 8), (8, 8, 64, 64), (16, 16, 32, 32), (24, 24, 8, 8),
+            (32, 32, 32, 32)]
 
 
 @pytest.mark.parametrize("dims", ACC_DIMS)
 @pytest.mark.parametrize("prec", [8, 4])
-@pytest.mark.parametrize("two_axis", [1, 0])
-def test_accelerate(lgf, dims, prec, two_axis):
-    """a2-a4: w = F^-1 (16/p^2) F Delta / V against the oracle's naive separable DFT, with the
-    three-sweep two-axis plan (where the lattice allows it) and with one pass per axis."""
+@pytest.mark.parametrize("plan", ["reg", "two_axis", "axis"])
+def test_accelerate(lgf, dims, prec, plan):
+    """a2-a4: w = F^-1 (16/p^2) F Delta / V against the oracle's naive separable DFT, with each FFT
+    plan: register-line sweeps and shared-memory two-axis sweeps (where the lattice allows them; the
+    planner falls back otherwise) and one pass per axis."""
     import torch
 
     D = random_herm_field(dims, 99)
     D -= D.mean(axis=(0, 1, 2, 3), keepdims=True)        # like a real Delta: zero lattice sum
     w_o = oracle.accelerate(dims, D)
     with lgf.Context(dims, prec, 18) as ctx:
-        ctx.tune("fft_two_axis", two_axis)
-        if not two_axis:
+        ctx.tune("fft_reg", int(plan == "reg"))
+        ctx.tune("fft_two_axis", int(plan != "axis"))
+        if plan == "axis":
             assert ctx.fft_passes() == 7
         ctx.set_field(to_dev(D, prec))
         ctx.step_accelerate()
@@ -120,8 +123,8 @@ def test_fft_plan_and_tile_overrides(lgf, dims, passes):
     res = []
     with lgf.Context(dims, 8, 18) as ctx:
         assert ctx.fft_passes() == passes
-        for key, val in [(None, 0), ("fft_xy_planes", 1), ("fft_xy_planes", 4), ("fft_zt_xc", 2), ("fft_zt_xc", 8),
-                         ("fft_two_axis", 0)]:
+        for key, val in [(None, 0), ("fft_reg", 0), ("fft_xy_planes", 1), ("fft_xy_planes", 4), ("fft_zt_xc", 2),
+                         ("fft_zt_xc", 8), ("fft_two_axis", 0)]:
             if key:
                 ctx.tune(key, val)
             ctx.set_field(to_dev(D, 8))
@@ -162,9 +165,12 @@ def run_trajectory(lgf, dims, U, prec, storage, n):
         ctx.iterate(ALPHA, n)
         F, th, P = ctx.measure()
         Fh, Th = ctx.history()
-        assert len(Fh) == n and ctx.iterations() == n
+        assert len(Fh) == n + 1 and ctx.iterations() == n        # entry k = after k updates (R12)
+        # the fused sweep's (F, theta) of the last configuration agree with a fresh a1 pass on it
+        rel = 1e-13 if prec == 8 else 1e-6
+        assert abs(F - Fh[-1]) <= rel * abs(F) and abs(th - Th[-1]) <= rel * abs(th)
         out = to_np(ctx.get_links(torch.empty_like(d)))
-    return np.append(Fh, F), np.append(Th, th), P, out
+    return Fh, Th, P, out
 
 
 @pytest.mark.parametrize("cfg", ["C1", "C2"])
