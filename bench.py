@@ -30,6 +30,8 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
+from paper_1206_0675_b200 import ensemble  # noqa: E402  (host-side replica bookkeeping only)
+
 METRIC = "gauge_fix_iterations_per_s"
 UNIT = "iterations/s"
 ALPHA = 0.08
@@ -135,10 +137,7 @@ def time_variant(binding, torch, U0, dims, prec_name, storage, steps, warmup, di
             dist.barrier()
         ms = e0.elapsed_time(e1)
         out["launches"] = ctx.launch_count() - n0
-        if dist is not None:
-            t = torch.tensor([ms], dtype=torch.float64, device="cuda")
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms = float(t.item())
+        ms = ensemble.max_over_ranks(dist, ms)          # the slowest replica bounds the whole job
         out["ms_total"] = ms
         out["ms_per_step"] = ms / steps
         # per-kernel-class device times: every launch bracketed by CUDA events on the launching stream,
@@ -190,9 +189,7 @@ def time_e2e(binding, torch, U0, dims, prec_name, storage, tol, max_iter, dist):
         ms = max(e0.elapsed_time(e1), 1e3 * wall)
         if dist is not None:
             dist.barrier()
-            t = torch.tensor([ms], dtype=torch.float64, device="cuda")
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms = float(t.item())
+        ms = ensemble.max_over_ranks(dist, ms)
         F, th, _ = ctx.measure(plaquette=False)
         nbytes = h.numel() * h.element_size()
     return {"iterations": it, "ms": ms, "bytes_each_way": nbytes, "theta": th, "F": F}
@@ -313,7 +310,8 @@ def main():
     cfg = inputs.CONFIGS[args.workload]
     dims = cfg["dims"]
     V = int(np.prod(dims))
-    U0 = inputs.make_config(args.workload, seed_offset=rank)     # replicas: one ensemble member per GPU
+    member = ensemble.member_indices(world, rank, world)[0]      # replicas: one ensemble member per GPU
+    U0 = inputs.make_config(args.workload, seed_offset=ensemble.member_seed_offset(member))
 
     sampler = ClockSampler(physical_gpu_index(local))
     head = time_variant(binding, torch, U0, dims, args.precision, args.storage, args.steps, args.warmup, dist, sampler)
