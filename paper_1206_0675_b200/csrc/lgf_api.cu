@@ -41,6 +41,10 @@ struct lgf_ctx {
     int tune_reg = 1;            // lgf_tune: use the register-line FFT sweeps when available
     int tune_xy_planes = 0;      // lgf_tune: planes per CTA of the (x, y) pass (0 = planner's choice)
     int tune_zt_xc = 0;          // lgf_tune: consecutive (x, y) indices per CTA of the (z, t) pass
+    int tune_fuse_g = 1;         // lgf_tune: end the last FFT sweep with the g-build (register-line plan only)
+    int tune_sweep_tiled = 0;    // lgf_tune: tiled sweep (shared-memory neighbour exchange, finalize folded in)
+    int tune_sweep_tt = 0;       // lgf_tune: t-march length of the tiled sweep (0 = automatic)
+    SweepTile tile{};
     struct Stamp { cudaEvent_t a, b; int cls; };
     std::vector<Stamp> stamps;
     double prof_ms[LGF_K_COUNT] = {0};
@@ -282,14 +286,20 @@ static int step_delta(lgf_ctx *ctx, const int *stop) {
                        ctx->stream));
     return LGF_OK;
 }
+// true if the plan's last sweep can end with the g-build (a5) and write G instead of W
+static bool can_fuse_g(const lgf_ctx *ctx) {
+    return ctx->tune_fuse_g && !ctx->passes.empty() && ctx->passes.back().kind == PASS_REG;
+}
+// a2-a4.  with_g: the last sweep also does a5 with step alpha (W is then NOT left holding w).
 template <class R>
-static int step_accelerate(lgf_ctx *ctx) {
+static int step_accelerate(lgf_ctx *ctx, bool with_g = false, double alpha = 0.0) {
     const R scale = (R)(16.0 / (double)ctx->g.V);        // p2max / V      (Alg. 1 lines 5, 7; R5, R7)
     for (const AxisPass &p : ctx->passes) {
         Bracket br(ctx, LGF_K_FFT);
         if (p.kind == PASS_REG) {
-            CK(launch_fft_reg<R>(p.axis, ctx->g, (C<R> *)ctx->W, (const R *)ctx->twiddle[3], (const R *)ctx->p2tab, scale,
-                                 ctx->st, ctx->stream));
+            const int which = (with_g && p.axis == 2) ? 3 : p.axis;
+            CK(launch_fft_reg<R>(which, ctx->g, (C<R> *)ctx->W, (const R *)ctx->twiddle[3], (const R *)ctx->p2tab, scale,
+                                 ctx->st, ctx->stream, (C<R> *)ctx->G, (R)(0.5 * alpha)));
             continue;
         }
         const R *tw[4] = {(const R *)ctx->twiddle[0], (const R *)ctx->twiddle[1], (const R *)ctx->twiddle[2],
@@ -300,22 +310,34 @@ static int step_accelerate(lgf_ctx *ctx) {
 }
 // a5 then a6 + a1: g from the current W, then the fused sweep (new links into the other buffer, Delta of
 // the new links into W, partial sums of F and theta)
-template <class R>
-static int step_update(lgf_ctx *ctx, double alpha) {
-    {
-        Bracket br(ctx, LGF_K_GBUILD);
-        CK(launch_gbuild<R>((const C<R> *)ctx->W, (C<R> *)ctx->G, ctx->g, (R)(0.5 * alpha), ctx->st, ctx->stream));
-    }
-    Bracket br(ctx, LGF_K_UPDATE);
-    CK(launch_sweep<R>(ctx->nr, link_pair<R>(ctx), (const C<R> *)ctx->G, (C<R> *)ctx->W, ctx->g, ctx->partial,
-                       &ctx->nb_partial, ctx->st, ctx->stream));
-    return LGF_OK;
-}
 static int step_finalize(lgf_ctx *ctx, double tol, int after_sweep, int record) {
     ctx->launches++;
     CK(launch_finalize(ctx->partial, ctx->nb_partial, ctx->g.V, tol, after_sweep, record, ctx->st, ctx->hist,
                        ctx->hist_cap, ctx->stream));
     return LGF_OK;
+}
+// The sweep also closes the iteration: it makes the new configuration current, and with record != 0 appends
+// (F, theta) to the history and applies the loop test theta < tol (a k_finalize launch after the default
+// sweep; inside the last CTA of the tiled one).
+template <class R>
+static int step_update(lgf_ctx *ctx, double alpha, double tol, int record, bool g_ready = false) {
+    if (!g_ready) {
+        Bracket br(ctx, LGF_K_GBUILD);
+        CK(launch_gbuild<R>((const C<R> *)ctx->W, (C<R> *)ctx->G, ctx->g, (R)(0.5 * alpha), ctx->st, ctx->stream));
+    }
+    if (ctx->tune_sweep_tiled) {
+        Bracket br(ctx, LGF_K_UPDATE);
+        CK(launch_sweep_tiled<R>(ctx->nr, link_pair<R>(ctx), (const C<R> *)ctx->G, (C<R> *)ctx->W, ctx->g, ctx->tile,
+                                 ctx->partial, &ctx->nb_partial, ctx->st, tol, record, ctx->hist, ctx->hist_cap,
+                                 ctx->stream));
+        return LGF_OK;
+    }
+    {
+        Bracket br(ctx, LGF_K_UPDATE);
+        CK(launch_sweep<R>(ctx->nr, link_pair<R>(ctx), (const C<R> *)ctx->G, (C<R> *)ctx->W, ctx->g, ctx->partial,
+                           &ctx->nb_partial, ctx->st, ctx->stream));
+    }
+    return step_finalize(ctx, tol, 1, record);
 }
 
 // Alg. 1 line 1: Delta, F, theta of the loaded configuration, recorded as history entry 0 with the stop
@@ -336,9 +358,9 @@ static int first_measure(lgf_ctx *ctx, double tol) {
 template <class R>
 static int iteration(lgf_ctx *ctx, double alpha, double tol) {
     int rc;
-    if ((rc = step_accelerate<R>(ctx)) != LGF_OK) return rc;
-    if ((rc = step_update<R>(ctx, alpha)) != LGF_OK) return rc;
-    return step_finalize(ctx, tol, 1, 1);
+    const bool fuse = can_fuse_g(ctx);
+    if ((rc = step_accelerate<R>(ctx, fuse, alpha)) != LGF_OK) return rc;
+    return step_update<R>(ctx, alpha, tol, 1, fuse);
 }
 // a1 on the current configuration without touching the history or the stop flag
 template <class R>
@@ -395,7 +417,11 @@ int lgf_create(const int dims[4], int precision, int link_storage, lgf_ctx **out
     alloc(&ctx->links[1], V * 4 * 3 * ctx->nr * cb);
     alloc(&ctx->W, V * 4 * cb);
     alloc(&ctx->G, V * 6 * cb);
-    ctx->partial_cap = (int)((V + 127) / 128) + 1;
+    ctx->tile = choose_sweep_tile(ctx->g, 0);
+    {   // >= the CTA count of every kernel that writes per-CTA partial sums (tiled sweep: at most V / threads)
+        const size_t a = (V + 127) / 128, b = V / (size_t)ctx->tile.threads;
+        ctx->partial_cap = (int)(a > b ? a : b) + 1;
+    }
     alloc((void **)&ctx->partial, sizeof(double) * 4 * ctx->partial_cap);
     alloc((void **)&ctx->st, sizeof(DevState));
     ctx->hist_cap = 1 << 20;
@@ -638,7 +664,7 @@ int lgf_step_accelerate(lgf_ctx *ctx) {
     ctx->launches++;
     CK(launch_clear_done(ctx->st, ctx->stream));
     ctx->w_is_delta = false;
-    return DISPATCH(step_accelerate, ctx);
+    return DISPATCH(step_accelerate, ctx, false, 0.0);
 }
 
 int lgf_step_update(lgf_ctx *ctx, double alpha) {
@@ -646,10 +672,10 @@ int lgf_step_update(lgf_ctx *ctx, double alpha) {
     if (!ctx->have_links) return fail(ctx, LGF_ESTATE, "lgf_step_update: no configuration loaded");
     ctx->launches++;
     CK(launch_clear_done(ctx->st, ctx->stream));
-    const int rc = DISPATCH(step_update, ctx, alpha);
+    const int rc = DISPATCH(step_update, ctx, alpha, -1.0, 0, false);
     if (rc != LGF_OK) return rc;
     ctx->w_is_delta = true;            // the sweep left Delta of the new links in W
-    return step_finalize(ctx, -1.0, 1, 0);
+    return LGF_OK;
 }
 
 int lgf_get_field(lgf_ctx *ctx, void *d_field) {
@@ -677,6 +703,9 @@ int lgf_tune(lgf_ctx *ctx, const char *key, int value) {
     else if (k == "fft_xy_planes") ctx->tune_xy_planes = value;
     else if (k == "fft_zt_xc") ctx->tune_zt_xc = value;
     else if (k == "sweep_minb") lgf::g_sweep_minb = value;
+    else if (k == "sweep_tiled") ctx->tune_sweep_tiled = value;
+    else if (k == "fuse_g") ctx->tune_fuse_g = value;
+    else if (k == "sweep_tt") { ctx->tune_sweep_tt = value; ctx->tile = choose_sweep_tile(ctx->g, value); }
     else return fail(ctx, LGF_EINVAL, "lgf_tune: unknown key " + k);
     CK(cudaStreamSynchronize(ctx->stream));
     return plan_passes(ctx);

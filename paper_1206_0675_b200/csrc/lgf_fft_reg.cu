@@ -15,7 +15,8 @@
 //                    smem -> t lines: forward, times p2max / (V p2(k)) (Alg. 1 lines 5, 7), inverse ->
 //                    smem -> z lines inverse -> global.
 //   k_fftr_xy<INV>   kx lines from global (transposed layout) -> smem -> ky lines -> global, natural
-//                    (x, y) layout again.
+//                    (x, y) layout again; inside an iteration the GOUT variant ends with the g-build (a5)
+//                    and writes g(x) instead of w(x).
 //
 // One shared-memory round trip per sweep in (x, y), two in (z, t), against five and ten for the
 // in-place two-step passes of lgf_fft.cu, which remain the path for lines that do not fit in registers.
@@ -25,14 +26,22 @@ namespace lgf {
 
 // ---- (x, y) planes --------------------------------------------------------------------------------
 // P planes per CTA, L threads per plane.  Plane q (q = c*Lz*Lt + z + Lz*t) starts at W + q*L*L.
-template <class R, int L, int MODE, int P>
-__global__ void __launch_bounds__(P *L) k_fftr_xy(C<R> *__restrict__ W, const DevState *__restrict__ st) {
+// GOUT (inverse sweep only): the CTA's P planes are the four packed components of P/4 (z, t) slices, so
+// all of w(x) is on chip when the sweep ends; instead of storing w it builds g(x) = GS(1 + i (alpha/2) w(x))
+// (a5, Alg. 1 line 10) and stores rows 0, 1 of g to G -- the separate g-build pass over the field disappears.
+template <class R, int L, int MODE, int P, bool GOUT>
+__global__ void __launch_bounds__(P *L) k_fftr_xy(C<R> *__restrict__ W, const DevState *__restrict__ st,
+                                                  C<R> *__restrict__ G, long long V, int nzt, R half_alpha) {
     if (st->done) return;
+    static_assert(!GOUT || (MODE == FFT_INV && P % 4 == 0 && L % 4 == 0), "g output needs all four components on chip");
     constexpr int PX = L | 1;                    // odd row pitch: lanes over rows hit distinct banks
     extern __shared__ __align__(16) unsigned char smem_raw[];
     C<R> *tile_all = reinterpret_cast<C<R> *>(smem_raw);
     const int p = threadIdx.x / L, i = threadIdx.x % L;
-    C<R> *base = W + ((long long)blockIdx.x * P + p) * (L * L);
+    // plane number: GOUT: component p % 4 of slice blockIdx.x * (P/4) + p / 4; otherwise consecutive planes
+    const long long q = GOUT ? (long long)(p % 4) * nzt + (long long)blockIdx.x * (P / 4) + p / 4
+                             : (long long)blockIdx.x * P + p;
+    C<R> *base = W + q * (L * L);
     C<R> *tile = tile_all + p * (L * PX);
     C<R> v[L];
 #pragma unroll
@@ -54,8 +63,33 @@ __global__ void __launch_bounds__(P *L) k_fftr_xy(C<R> *__restrict__ W, const De
         for (int n = 0; n < L; n++) v[n] = tile[n * PX + i];            // column x = i, ky = n
         Dft<L, +1, R>::run(v);                                          // over ky  ->  y = n
     }
+    if constexpr (!GOUT) {
 #pragma unroll
-    for (int n = 0; n < L; n++) base[n * L + i] = v[n];                 // FWD: (kx = n, ky = i); INV: (y = n, x = i)
+        for (int n = 0; n < L; n++) base[n * L + i] = v[n];             // FWD: (kx = n, ky = i); INV: (y = n, x = i)
+    } else {
+        __syncthreads();                                                // everyone has read its column
+#pragma unroll
+        for (int n = 0; n < L; n++) tile[n * PX + i] = v[n];            // tile[y][x] of component p % 4
+        __syncthreads();
+        const C<R> *t4 = tile_all + (p / 4) * 4 * (L * PX);             // the four component tiles of this slice
+        const long long s0 = ((long long)blockIdx.x * (P / 4) + p / 4) * (L * L);
+#pragma unroll
+        for (int m = 0; m < L / 4; m++) {
+            const int y = (p % 4) + 4 * m;
+            Herm<R> w;
+            w.m01 = t4[y * PX + i];
+            w.m02 = t4[L * PX + y * PX + i];
+            w.m12 = t4[2 * L * PX + y * PX + i];
+            const C<R> dg = t4[3 * L * PX + y * PX + i];
+            w.m00 = dg.x;
+            w.m11 = dg.y;
+            C<R> gx[9];
+            build_g(w, half_alpha, gx);
+            const long long s = s0 + y * L + i;
+#pragma unroll
+            for (int e = 0; e < 6; e++) G[(long long)e * V + s] = gx[e];
+        }
+    }
 }
 
 // ---- (z, t) planes --------------------------------------------------------------------------------
@@ -70,10 +104,13 @@ struct ZtShape {
     static constexpr int PITCH = XC * LZ + ((XC < PHASE && (XC * LZ) % PHASE == 0) ? XC : 0);
     static constexpr int THREADS = XC * (LZ > LT ? LZ : LT);
     static constexpr size_t SMEM = sizeof(C<R>) * ((size_t)PITCH * LT + (TREG ? 0 : 64));
+    // resident CTAs per SM the register allocation is asked to allow.  Asking for 3 at 32 x 32 fp64 (168
+    // registers, 280 B of spills) made the sweep slower (50 -> 65 us on B200), so the compiler is left alone.
+    static constexpr int MINB = 1;
 };
 
 template <class R, int LZ, int LT, int XC, bool TREG>
-__global__ void __launch_bounds__((ZtShape<R, LZ, LT, XC, TREG>::THREADS))
+__global__ void __launch_bounds__((ZtShape<R, LZ, LT, XC, TREG>::THREADS), (ZtShape<R, LZ, LT, XC, TREG>::MINB))
     k_fftr_zt(C<R> *__restrict__ W, Geom g, const C<R> *__restrict__ twt_g, const R *__restrict__ p2tab, R scale,
               const DevState *__restrict__ st) {
     if (st->done) return;
@@ -176,22 +213,23 @@ bool fft_reg_t_natural(const Geom &g) {
 
 template <class R>
 cudaError_t launch_fft_reg(int which, const Geom &g, C<R> *W, const R *twiddle_t, const R *p2tab, R scale,
-                           const DevState *st, cudaStream_t stream) {
-    if (which == 0 || which == 2) {                                     // (x, y) forward / inverse
+                           const DevState *st, cudaStream_t stream, C<R> *G, R half_alpha) {
+    if (which == 0 || which == 2 || which == 3) {                       // (x, y) forward / inverse / inverse + g
         const long long planes = 4LL * g.L[2] * g.L[3];
+        const int nzt = g.L[2] * g.L[3];
 #define LGF_GO(LEN)                                                                                       \
     if (g.L[0] == LEN) {                                                                                   \
         constexpr int P = XyPlanes<LEN>::P;                                                                \
         constexpr size_t SM = sizeof(C<R>) * P * LEN * (LEN | 1);                                            \
-        auto kf = k_fftr_xy<R, LEN, FFT_FWD, P>;                                                           \
-        auto ki = k_fftr_xy<R, LEN, FFT_INV, P>;                                                           \
+        auto kf = k_fftr_xy<R, LEN, FFT_FWD, P, false>;                                                    \
+        auto ki = k_fftr_xy<R, LEN, FFT_INV, P, false>;                                                    \
+        auto kg = k_fftr_xy<R, LEN, FFT_INV, P, true>;                                                     \
+        auto kern = which == 0 ? kf : (which == 2 ? ki : kg);                                              \
         if (SM > 48 * 1024) {                                                                            \
-            cudaError_t e = cudaFuncSetAttribute(which == 0 ? kf : ki,                                   \
-                                                 cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SM);  \
+            cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SM); \
             if (e != cudaSuccess) return e;                                                              \
         }                                                                                                \
-        if (which == 0) kf<<<(unsigned)(planes / P), P * LEN, SM, stream>>>(W, st);                        \
-        else ki<<<(unsigned)(planes / P), P * LEN, SM, stream>>>(W, st);                                   \
+        kern<<<(unsigned)(planes / P), P * LEN, SM, stream>>>(W, st, G, g.V, nzt, half_alpha);             \
         return cudaGetLastError();                                                                       \
     }
         LGF_REG_XY(LGF_GO)
@@ -217,8 +255,8 @@ cudaError_t launch_fft_reg(int which, const Geom &g, C<R> *W, const R *twiddle_t
 }
 
 template cudaError_t launch_fft_reg<float>(int, const Geom &, C<float> *, const float *, const float *, float,
-                                           const DevState *, cudaStream_t);
+                                           const DevState *, cudaStream_t, C<float> *, float);
 template cudaError_t launch_fft_reg<double>(int, const Geom &, C<double> *, const double *, const double *, double,
-                                            const DevState *, cudaStream_t);
+                                            const DevState *, cudaStream_t, C<double> *, double);
 
 }  // namespace lgf

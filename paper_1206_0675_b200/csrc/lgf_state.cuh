@@ -18,7 +18,17 @@ struct DevState {
     int zero;             // always 0: the `stop` word handed to kernels that must run regardless of `done`
     int cur;              // which of the two link buffers holds the current configuration (0 / 1); the
                           // sweep reads buffer `cur` and writes the other one, k_finalize flips it
+    unsigned int ticket;  // CTAs of the running tiled sweep that have delivered their partial sums
 };
+
+// Tile of the tiled sweep (lgf_links.cu): TX x TY x TZ threads, marching TT slices in t.
+struct SweepTile {
+    int T[4];             // tile extents TX, TY, TZ (one thread per site) and TT (march length)
+    int nt[4];            // tiles per axis
+    int threads;          // TX * TY * TZ
+};
+// tile choice for a lattice (host)
+SweepTile choose_sweep_tile(const Geom &g, int tt_override);
 
 // The two link buffers (ping-pong: the fused sweep needs U_mu(x - mu) of the OLD configuration while
 // other threads already write the new one).
@@ -34,7 +44,8 @@ enum PassKind {
     PASS_XY = 1,          // whole (x, y) planes: both axes transformed in one shared-memory tile
     PASS_ZT = 2,          // (z, t) planes of nlo consecutive (x, y) indices: forward z, t, scale, inverse t, z
     PASS_REG = 3          // register-resident line transforms (lgf_fft_reg.cu); `axis` = 0: (x, y) forward,
-                          // 1: (z, t) forward + scale + inverse, 2: (x, y) inverse
+                          // 1: (z, t) forward + scale + inverse, 2: (x, y) inverse, 3: (x, y) inverse ending in the
+                      // g-build (writes G, not W)
 };
 
 // One FFT pass (see lgf_fft.cu).
@@ -63,7 +74,7 @@ bool fft_reg_supported(const Geom &g);
 bool fft_reg_t_natural(const Geom &g);
 template <class R>
 cudaError_t launch_fft_reg(int which, const Geom &g, C<R> *W, const R *twiddle_t, const R *p2tab, R scale,
-                           const DevState *st, cudaStream_t stream);
+                           const DevState *st, cudaStream_t stream, C<R> *G = nullptr, R half_alpha = 0);
 // true if a PASS_XY (first two axes) / PASS_ZT (last two axes) kernel is instantiated for these lengths
 bool fft_pair_supported(int kind, int La, int Lb);
 
@@ -75,6 +86,11 @@ cudaError_t launch_gbuild(const C<R> *W, C<R> *G, const Geom &g, R half_alpha, c
 template <class R>
 cudaError_t launch_sweep(int nr, LinkPair<R> links, const C<R> *G, C<R> *W, const Geom &g, double *partial,
                          int *nblocks, const DevState *st, cudaStream_t stream);
+// tiled sweep with the finalize folded in (last CTA): record / tol / hist as for launch_finalize
+template <class R>
+cudaError_t launch_sweep_tiled(int nr, LinkPair<R> links, const C<R> *G, C<R> *W, const Geom &g, const SweepTile &tl,
+                               double *partial, int *nblocks, DevState *st, double tol, int record, double *hist,
+                               long long hist_cap, cudaStream_t stream);
 template <class R>
 cudaError_t launch_plaquette(int nr, LinkPair<R> links, const Geom &g, double *partial, int *nblocks,
                              const DevState *st, cudaStream_t stream);
