@@ -138,6 +138,65 @@ def hot_config(dims, seed: int, chunk: int = 1 << 20) -> np.ndarray:
     return U.reshape(_site_shape(dims) + (4, 3, 3))
 
 
+# ---- the same counter-based streams with torch ops (CPU or CUDA) -- for the 64^4 hot start ------------
+# The numpy QR above needs minutes for the 67 M links of C5.  These functions draw the SAME uniform and
+# normal streams (bit-identical integers; log / cos may differ from numpy's in the last ulp) and
+# orthonormalise the Ginibre matrix by classical Gram-Schmidt on its columns, which is the QR factor with a
+# positive diagonal, i.e. the same Haar recipe (R21).  Still no method arithmetic: input construction only.
+def _torch_uniforms(torch, seed: int, stream: int, start: int, count: int, device):
+    key = int(_stream_key(seed, stream))
+    key = key - (1 << 64) if key >= (1 << 63) else key
+    golden = int(_GOLDEN) - (1 << 64)
+    m1, m2 = int(_M1) - (1 << 64), int(_M2) - (1 << 64)
+
+    def lsr(z, k):                                    # logical shift right of an int64 bit pattern
+        return (z >> k) & ((1 << (64 - k)) - 1)
+
+    ctr = torch.arange(start + 1, start + count + 1, dtype=torch.int64, device=device)
+    z = key + ctr * golden
+    z = (z ^ lsr(z, 30)) * m1
+    z = (z ^ lsr(z, 27)) * m2
+    z = z ^ lsr(z, 31)
+    return (lsr(z, 11).to(torch.float64) + 0.5) * (1.0 / 9007199254740992.0)
+
+
+def _torch_normals(torch, seed: int, stream: int, start: int, count: int, device):
+    u = _torch_uniforms(torch, seed, stream, 2 * start, 2 * count, device)
+    return torch.sqrt(-2.0 * torch.log(u[0::2])) * torch.cos(2.0 * np.pi * u[1::2])
+
+
+def haar_su3_torch(seed: int, stream: int, start: int, count: int, device="cpu"):
+    """count Haar-random SU(3) matrices as a torch complex128 tensor (count, 3, 3) on `device`."""
+    import torch
+
+    n = _torch_normals(torch, seed, stream, 18 * start, 18 * count, device).reshape(count, 3, 3, 2)
+    Z = torch.complex(n[..., 0], n[..., 1]) / np.sqrt(2.0)
+    cols = []
+    for j in range(3):                                # Gram-Schmidt on columns = Q of QR with R_jj > 0
+        v = Z[:, :, j]
+        for _ in range(2):                            # orthogonalise twice: unitary to rounding
+            for q in cols:
+                v = v - q * (q.conj() * v).sum(dim=1, keepdim=True)
+        cols.append(v / torch.linalg.vector_norm(v, dim=1, keepdim=True))
+    Q = torch.stack(cols, dim=2)
+    det = torch.linalg.det(Q)
+    return Q / (det ** (1.0 / 3.0))[:, None, None]
+
+
+def hot_config_torch(dims, seed: int, device="cpu", chunk: int = 1 << 22):
+    """hot_config with torch ops: every link Haar-random; returns a torch complex128 tensor of shape
+    (Lt, Lz, Ly, Lx, 4, 3, 3) on `device`.  Same streams as hot_config, Gram-Schmidt instead of LAPACK QR."""
+    import torch
+
+    dims = tuple(int(v) for v in dims)
+    V = dims[0] * dims[1] * dims[2] * dims[3]
+    U = torch.empty((V * 4, 3, 3), dtype=torch.complex128, device=device)
+    for s in range(0, V * 4, chunk):
+        e = min(s + chunk, V * 4)
+        U[s:e] = haar_su3_torch(seed, STREAM_HOT, s, e - s, device)
+    return U.reshape(_site_shape(dims) + (4, 3, 3))
+
+
 def abelian_config(dims, amp: float, seed: int) -> np.ndarray:
     """Diagonal links U = diag(e^{i p1}, e^{i p2}, e^{-i(p1+p2)}) with phases p ~ amp * N(0,1):
     a small-field abelian configuration on which the linearised iteration is exactly solvable."""
