@@ -48,6 +48,27 @@ def measured_peak():
         return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
 
 
+def captured_traffic(workload, precision, storage, kernel_class):
+    """DRAM bytes per launch of the dominant kernel from the committed ncu --set full capture
+    (profiles/*_traffic.csv: dram__bytes_read.sum + dram__bytes_write.sum), or None if that workload /
+    variant / kernel has not been captured.  A stored measurement, read as data; nothing here runs ncu."""
+    import csv
+    import glob
+
+    best = None
+    for path in sorted(glob.glob(os.path.join(ROOT, "profiles", "*_traffic.csv"))):
+        try:
+            with open(path, newline="") as f:
+                for row in csv.DictReader(f):
+                    if (row["workload"] == workload and row["precision"] == precision
+                            and int(row["link_storage"]) == int(storage) and row["kernel_class"] == kernel_class):
+                        best = {"bytes": float(row["dram_bytes_per_launch"]), "kernel": row["kernel"],
+                                "source": "profiles/" + os.path.basename(path)}
+        except Exception:  # noqa: BLE001
+            continue
+    return best
+
+
 class ClockSampler:
     """Samples SM clock and throttle reasons through NVML while the timed region runs."""
 
@@ -324,8 +345,10 @@ def main():
     dk = hot[dom]
     bytes_per_launch = dk["algorithmic_bytes_per_step"] / dk["launches_per_step"]
     achieved = bytes_per_launch / (dk["avg_launch_us"] * 1e-6) / 1e9
+    cap = captured_traffic(args.workload, args.precision, args.storage, dom)
     roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+                "frac": achieved / peak, "traffic": cap["bytes"] if cap else None,
+                "traffic_source": cap["source"] if cap else None, "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": bytes_per_launch, "avg_launch_us": dk["avg_launch_us"],
                 "iteration": {"algorithmic_bytes": head["iter_bytes"],
                               "achieved": head["iter_bytes"] / (head["ms_per_step"] * 1e-3) / 1e9,

@@ -23,6 +23,7 @@ struct lgf_ctx {
     void *W = nullptr;           // C<R>[4][V]   packed Delta / w
     void *G = nullptr;           // C<R>[6][V]   rows 0, 1 of g(x)
     bool w_is_delta = false;     // W holds Delta of the current configuration and `partial` its F / theta sums
+    bool recorded = false;       // the current configuration's (F, theta) is already in the history
     int nb_partial = 0;          // number of per-block partial sums currently in `partial`
     double *partial = nullptr;   // per-block partial sums
     int partial_cap = 0;
@@ -345,11 +346,17 @@ static int step_update(lgf_ctx *ctx, double alpha, double tol, int record, bool 
 // previous sweep, whose finalize has recorded it).
 template <class R>
 static int first_measure(lgf_ctx *ctx, double tol) {
-    if (ctx->w_is_delta) return LGF_OK;
     int rc;
-    if ((rc = step_delta<R>(ctx, &ctx->st->done)) != LGF_OK) return rc;
-    if ((rc = step_finalize(ctx, tol, 0, 1)) != LGF_OK) return rc;
-    ctx->w_is_delta = true;
+    if (!ctx->w_is_delta) {
+        if ((rc = step_delta<R>(ctx, &ctx->st->done)) != LGF_OK) return rc;
+        ctx->w_is_delta = true;
+    }
+    // W / `partial` may have been filled by lgf_measure or lgf_step_delta, which record nothing: the
+    // history entry of this configuration (and the loop test) is still owed
+    if (!ctx->recorded) {
+        if ((rc = step_finalize(ctx, tol, 0, 1)) != LGF_OK) return rc;
+        ctx->recorded = true;
+    }
     return LGF_OK;
 }
 // One pass of the while-body of Algorithm 1 (lines 3-17): accelerate, g, sweep (update + measure), then
@@ -360,7 +367,9 @@ static int iteration(lgf_ctx *ctx, double alpha, double tol) {
     int rc;
     const bool fuse = can_fuse_g(ctx);
     if ((rc = step_accelerate<R>(ctx, fuse, alpha)) != LGF_OK) return rc;
-    return step_update<R>(ctx, alpha, tol, 1, fuse);
+    if ((rc = step_update<R>(ctx, alpha, tol, 1, fuse)) != LGF_OK) return rc;
+    ctx->recorded = true;                                // the sweep's finalize appended the new configuration
+    return LGF_OK;
 }
 // a1 on the current configuration without touching the history or the stop flag
 template <class R>
@@ -488,6 +497,7 @@ int lgf_set_links(lgf_ctx *ctx, const void *d_links) {
     CK(launch_reset_state(ctx->st, ctx->stream));        // also makes buffer 0 the current one
     ctx->have_links = true;
     ctx->w_is_delta = false;
+    ctx->recorded = false;
     return LGF_OK;
 }
 
@@ -675,6 +685,7 @@ int lgf_step_update(lgf_ctx *ctx, double alpha) {
     const int rc = DISPATCH(step_update, ctx, alpha, -1.0, 0, false);
     if (rc != LGF_OK) return rc;
     ctx->w_is_delta = true;            // the sweep left Delta of the new links in W
+    ctx->recorded = false;             // ... but nothing about them in the history
     return LGF_OK;
 }
 

@@ -330,6 +330,33 @@ def test_edge_cases(lgf):
         assert np.max(np.abs(Th - T_o) / T_o) < 1e-12
 
 
+@pytest.mark.parametrize("probe", ["measure", "measure_no_plaquette", "step_delta", "none"])
+def test_history_entry0_survives_a_measurement_before_iterate(lgf, config_cache, probe):
+    """lgf_measure / lgf_step_delta fill W and the partial sums but record nothing; the first lgf_iterate
+    after them must still record entry 0 = the loaded configuration (include/lgf.h, R12).  Found at 64^4:
+    measure() before iterate() used to leave the history one entry short."""
+    dims = inputs.CONFIGS["C1"]["dims"]
+    U = config_cache("C1")
+    _, F_o, T_o = oracle.iterate(dims, U, ALPHA, 3)
+    with lgf.Context(dims, 8, 18) as ctx:
+        ctx.set_links(to_dev(U, 8))
+        if probe == "measure":
+            ctx.measure()
+        elif probe == "measure_no_plaquette":
+            ctx.measure(plaquette=False)
+        elif probe == "step_delta":
+            ctx.step_delta()
+        assert ctx.history_length() == 0
+        ctx.iterate(ALPHA, 1)
+        assert ctx.history_length() == 2 and ctx.iterations() == 1
+        ctx.measure()                                   # between two iterate calls: no duplicate entry either
+        ctx.iterate(ALPHA, 2)
+        Fh, Th = ctx.history()
+    assert len(Fh) == 4
+    assert np.max(np.abs(Fh - F_o) / np.abs(F_o)) < 1e-12
+    assert np.max(np.abs(Th - T_o) / np.abs(T_o)) < 1e-12
+
+
 def test_12_real_matches_18_real(lgf, config_cache):
     """Third-row reconstruction (eq. 8) changes rounding only."""
     dims = inputs.CONFIGS["C1"]["dims"]
