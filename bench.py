@@ -139,24 +139,46 @@ def time_variant(binding, torch, U0, dims, prec_name, storage, steps, warmup, di
     with binding.Context(dims, prec, storage, stream=stream) as ctx:
         d = torch.from_numpy(U0).to(cdt).cuda()
         ctx.set_links(d)
-        ctx.iterate(ALPHA, warmup)
+        # warm-up, itself timed on the device: gives the per-step estimate the stall check below uses
+        w0, w1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ctx.iterate(ALPHA, 1)
+        w0.record(stream)
+        ctx.iterate(ALPHA, max(1, warmup - 1))
+        w1.record(stream)
         torch.cuda.synchronize()
-        if dist is not None:
-            dist.barrier()
-        torch.cuda.synchronize()
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        warm_ms_per_step = w0.elapsed_time(w1) / max(1, warmup - 1)
+
+        def timed_region():
+            if dist is not None:
+                dist.barrier()
+            torch.cuda.synchronize()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream)
+            ctx.iterate(ALPHA, steps)
+            b.record(stream)
+            torch.cuda.synchronize()
+            if dist is not None:
+                dist.barrier()
+            return a.elapsed_time(b)
+
         n0 = ctx.launch_count()
         if sampler is not None:
             sampler.__enter__()
-        e0.record(stream)
-        ctx.iterate(ALPHA, steps)
-        e1.record(stream)
-        torch.cuda.synchronize()
+        ms = timed_region()
+        # A timed region far slower than the warm-up steps of the same kernels is a stall of the launching
+        # host thread, not kernel time (seen once on a fresh box: 35 s for 3 steps, not reproducible, cause
+        # unknown).  It is re-measured ONCE and both numbers are reported; nothing is dropped silently.
+        out["remeasured"] = None
+        stalled = ms / steps > 20.0 * warm_ms_per_step
+        # every rank takes the same branch (the timed region contains barriers): any rank stalled -> all re-measure
+        if ensemble.max_over_ranks(dist, 1.0 if stalled else 0.0) > 0.5:
+            first = ms
+            n0 = ctx.launch_count()
+            ms = timed_region()
+            out["remeasured"] = {"reason": "first timed region stalled", "first_ms_per_step": first / steps,
+                                 "warmup_ms_per_step": warm_ms_per_step, "second_ms_per_step": ms / steps}
         if sampler is not None:
             sampler.__exit__()
-        if dist is not None:
-            dist.barrier()
-        ms = e0.elapsed_time(e1)
         out["launches"] = ctx.launch_count() - n0
         ms = ensemble.max_over_ranks(dist, ms)          # the slowest replica bounds the whole job
         out["ms_total"] = ms
@@ -393,7 +415,8 @@ def main():
                            "l2": "inputs larger than L2: one step streams %.0f MB of links and fields"
                                  % (head["iter_bytes"] / 1e6)},
                 "site_updates_per_s": value * V, "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e,
-                "gpu_launches": head["launches"], "clocks": sampler.summary(), "variants": variants,
+                "gpu_launches": head["launches"], "clocks": sampler.summary(), "remeasured": head.get("remeasured"),
+                "variants": variants,
                 "state_after_timing": {"F": head["F"], "theta": head["theta"], "plaquette": head["plaquette"]}}
         print(json.dumps(line), flush=True)
     if dist is not None:
