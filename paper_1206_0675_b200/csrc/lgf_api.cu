@@ -44,6 +44,7 @@ struct lgf_ctx {
     int tune_zt_xc = 0;          // lgf_tune: consecutive (x, y) indices per CTA of the (z, t) pass
     int tune_fuse_g = 1;         // lgf_tune: end the last FFT sweep with the g-build (register-line plan only)
     int tune_sweep_tiled = 0;    // lgf_tune: tiled sweep (shared-memory neighbour exchange, finalize folded in)
+    int tune_sweep_tz = 0;       // lgf_tune: z-planes per (z, t) tile of the sweep's block order (0 = automatic, 1 = plain)
     int tune_sweep_tt = 0;       // lgf_tune: t-march length of the tiled sweep (0 = automatic)
     SweepTile tile{};
     struct Stamp { cudaEvent_t a, b; int cls; };
@@ -214,7 +215,10 @@ static int plan_passes(lgf_ctx *ctx) {
     if (have_zt) {
         const long long plane = g.S[2], zsize = (long long)g.L[2] * g.L[3];
         const long long phase = 128 / (long long)cbytes;             // lanes per shared-memory phase
-        const long long xc_min = pow2_divisor_le(plane, 32 / (long long)cbytes > 0 ? 32 / (long long)cbytes : 1);
+        // shortest run the planner accepts: 2 complex elements (32 B in fp64, 16 B in fp32).  Measured at 64^4
+        // on B200: fp64 XC = 2 (128 KB tile) beats XC = 1 (2.87 vs 2.97 ms per FFT), fp32 XC = 2 (64 KB tile,
+        // 3 CTAs per SM) beats the 32-byte rule's XC = 4 (1.62 vs 1.92 ms).
+        const long long xc_min = pow2_divisor_le(plane, 2);
         long long XC = pow2_divisor_le(plane, (65536 / (long long)cbytes) / zsize > 0 ? (65536 / (long long)cbytes) / zsize : 1);
         while (XC > xc_min && (plane / XC) * 4 < MIN_GRID) XC /= 2;
         if (XC < xc_min) XC = xc_min;
@@ -336,7 +340,7 @@ static int step_update(lgf_ctx *ctx, double alpha, double tol, int record, bool 
     {
         Bracket br(ctx, LGF_K_UPDATE);
         CK(launch_sweep<R>(ctx->nr, link_pair<R>(ctx), (const C<R> *)ctx->G, (C<R> *)ctx->W, ctx->g, ctx->partial,
-                           &ctx->nb_partial, ctx->st, ctx->stream));
+                           &ctx->nb_partial, ctx->st, ctx->stream, ctx->tune_sweep_tz));
     }
     return step_finalize(ctx, tol, 1, record);
 }
@@ -716,6 +720,7 @@ int lgf_tune(lgf_ctx *ctx, const char *key, int value) {
     else if (k == "sweep_minb") lgf::g_sweep_minb = value;
     else if (k == "sweep_tiled") ctx->tune_sweep_tiled = value;
     else if (k == "fuse_g") ctx->tune_fuse_g = value;
+    else if (k == "sweep_tz") ctx->tune_sweep_tz = value;
     else if (k == "sweep_tt") { ctx->tune_sweep_tt = value; ctx->tile = choose_sweep_tile(ctx->g, value); }
     else return fail(ctx, LGF_EINVAL, "lgf_tune: unknown key " + k);
     CK(cudaStreamSynchronize(ctx->stream));
