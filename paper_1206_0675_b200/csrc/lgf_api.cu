@@ -40,6 +40,8 @@ struct lgf_ctx {
     bool profiling = false;
     int tune_two_axis = 1;       // lgf_tune: use the two-axis FFT passes when available
     int tune_reg = 1;            // lgf_tune: use the register-line FFT sweeps when available
+    int tune_reg2 = -1;          // lgf_tune: two-threads-per-line sweeps: 1 = prefer, 0 = never, -1 = where the
+                                 // one-thread kernels do not exist (64-point axes)
     int tune_xy_planes = 0;      // lgf_tune: planes per CTA of the (x, y) pass (0 = planner's choice)
     int tune_zt_xc = 0;          // lgf_tune: consecutive (x, y) indices per CTA of the (z, t) pass
     int tune_fuse_g = 1;         // lgf_tune: end the last FFT sweep with the g-build (register-line plan only)
@@ -184,6 +186,17 @@ static int plan_passes(lgf_ctx *ctx) {
         return ctx->prec == LGF_FP64 ? upload_p2<double>(ctx, natural) : upload_p2<float>(ctx, natural);
     };
     ctx->passes.clear();
+    auto plan_reg2 = [&]() {
+        for (int w = 0; w < 3; w++) {
+            AxisPass p{};
+            p.kind = PASS_REG2;
+            p.axis = w;
+            ctx->passes.push_back(p);
+        }
+        const bool natural[4] = {true, true, true, true};
+        return finish(natural);
+    };
+    if (ctx->tune_two_axis && ctx->tune_reg2 == 1 && fft_reg2_supported(g)) return plan_reg2();
     if (ctx->tune_two_axis && ctx->tune_reg && fft_reg_supported(g)) {
         for (int w = 0; w < 3; w++) {
             AxisPass p{};
@@ -194,6 +207,7 @@ static int plan_passes(lgf_ctx *ctx) {
         const bool natural[4] = {true, true, true, fft_reg_t_natural(g)};
         return finish(natural);
     }
+    if (ctx->tune_two_axis && ctx->tune_reg2 != 0 && fft_reg2_supported(g)) return plan_reg2();
     const bool permuted[4] = {false, false, false, false};
     const size_t SMEM_MAX = 200 * 1024;
     const long long MIN_GRID = 2 * 148;
@@ -293,7 +307,9 @@ static int step_delta(lgf_ctx *ctx, const int *stop) {
 }
 // true if the plan's last sweep can end with the g-build (a5) and write G instead of W
 static bool can_fuse_g(const lgf_ctx *ctx) {
-    return ctx->tune_fuse_g && !ctx->passes.empty() && ctx->passes.back().kind == PASS_REG;
+    if (!ctx->tune_fuse_g || ctx->passes.empty()) return false;
+    const int kind = ctx->passes.back().kind;
+    return kind == PASS_REG || (kind == PASS_REG2 && fft_reg2_gout(ctx->g, ctx->prec));
 }
 // a2-a4.  with_g: the last sweep also does a5 with step alpha (W is then NOT left holding w).
 template <class R>
@@ -305,6 +321,12 @@ static int step_accelerate(lgf_ctx *ctx, bool with_g = false, double alpha = 0.0
             const int which = (with_g && p.axis == 2) ? 3 : p.axis;
             CK(launch_fft_reg<R>(which, ctx->g, (C<R> *)ctx->W, (const R *)ctx->twiddle[3], (const R *)ctx->p2tab, scale,
                                  ctx->st, ctx->stream, (C<R> *)ctx->G, (R)(0.5 * alpha)));
+            continue;
+        }
+        if (p.kind == PASS_REG2) {
+            const int which = (with_g && p.axis == 2) ? 3 : p.axis;
+            CK(launch_fft_reg2<R>(which, ctx->g, (C<R> *)ctx->W, (const R *)ctx->p2tab, scale, ctx->st, ctx->stream,
+                                  (C<R> *)ctx->G, (R)(0.5 * alpha)));
             continue;
         }
         const R *tw[4] = {(const R *)ctx->twiddle[0], (const R *)ctx->twiddle[1], (const R *)ctx->twiddle[2],
@@ -715,6 +737,7 @@ int lgf_tune(lgf_ctx *ctx, const char *key, int value) {
     const std::string k(key);
     if (k == "fft_two_axis") ctx->tune_two_axis = value;
     else if (k == "fft_reg") ctx->tune_reg = value;
+    else if (k == "fft_reg2") ctx->tune_reg2 = value;
     else if (k == "fft_xy_planes") ctx->tune_xy_planes = value;
     else if (k == "fft_zt_xc") ctx->tune_zt_xc = value;
     else if (k == "sweep_minb") lgf::g_sweep_minb = value;

@@ -1,0 +1,259 @@
+// lgf_fft_reg2.cu -- register-line sweeps of the batched 4-D FFT (Alg. 1 lines 3-8) with
+// TWO threads per line (lgf_fft_split.cuh): the same three sweeps as lgf_fft_reg.cu,
+//   k_fftr2_xy<FWD>, k_fftr2_zt (forward z, t; times p2max / (V p2(k)); inverse t, z), k_fftr2_xy<INV[, GOUT]>,
+// but each thread holds half a line, so a 32-point fp64 line costs 64 data registers per thread instead of
+// 128 (more warps in flight) and 64-point lines fit at all.  All four axes end up in natural k order.
+// Part of liblgf (CUDA path); no cuFFT; shares nothing with oracle/.
+//
+// Thread layout: a warp owns 16 lines; lane = q + 16 h, q = line within the warp, h = which half of the
+// line.  The pair (q, 0), (q, 1) exchanges with __shfl_xor(.., 16).  Lanes q run over the contiguous
+// index of every global and shared-memory access.
+#include "lgf_fft_split.cuh"
+#include "lgf_state.cuh"
+
+namespace lgf {
+
+constexpr int PAIR_MASK = 16;
+
+// ---- (x, y) planes --------------------------------------------------------------------------------
+// P planes per CTA, 2 L threads per plane (L / 16 warps).  Plane q starts at W + q L^2.  The k-space plane
+// is stored transposed, element (kx, ky) at kx L + ky, as in lgf_fft_reg.cu.
+// GOUT (inverse only): the P planes are the four packed components of P / 4 (z, t) slices; the sweep ends
+// with a5, g = GS(1 + i (alpha/2) w), and stores rows 0, 1 of g instead of w.
+template <class R, int L, int MODE, int P, bool GOUT>
+__global__ void __launch_bounds__(2 * P * L) k_fftr2_xy(C<R> *__restrict__ W, const DevState *__restrict__ st,
+                                                        C<R> *__restrict__ G, long long V, int nzt, R half_alpha) {
+    if (st->done) return;
+    static_assert(L % 16 == 0, "16 lines per warp");
+    static_assert(!GOUT || (MODE == FFT_INV && P % 4 == 0), "g output needs all four components on chip");
+    constexpr int M = L / 2;
+    constexpr int PX = L | 1;                    // odd row pitch
+    using S = SplitDft<L, PAIR_MASK, R>;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    C<R> *tile_all = reinterpret_cast<C<R> *>(smem_raw);
+    const int tid = threadIdx.x;
+    const int p = tid / (2 * L), tp = tid % (2 * L);          // plane, thread within the plane
+    const int h = (tp >> 4) & 1;                               // lane = q + 16 h
+    const int i = (tp >> 5) * 16 + (tp & 15);                  // line number 0 .. L-1
+    const long long q = GOUT ? (long long)(p % 4) * nzt + (long long)blockIdx.x * (P / 4) + p / 4
+                             : (long long)blockIdx.x * P + p;
+    C<R> *base = W + q * (L * L);
+    C<R> *tile = tile_all + p * (L * PX);
+    C<R> v[M];
+    if constexpr (MODE == FFT_FWD) {
+#pragma unroll
+        for (int m = 0; m < M; m++) v[m] = base[(m + M * h) * L + i];        // y = m + M h at x = i
+        S::forward(v, h);                                                    // -> ky = 2 j + h
+#pragma unroll
+        for (int j = 0; j < M; j++) tile[(2 * j + h) * PX + i] = v[j];       // tile[ky][x]
+        __syncthreads();
+#pragma unroll
+        for (int m = 0; m < M; m++) v[m] = tile[i * PX + m + M * h];         // row ky = i, x = m + M h
+        S::forward(v, h);                                                    // -> kx = 2 j + h
+#pragma unroll
+        for (int j = 0; j < M; j++) base[(2 * j + h) * L + i] = v[j];        // (kx, ky = i), transposed plane
+    } else {
+#pragma unroll
+        for (int j = 0; j < M; j++) v[j] = base[(2 * j + h) * L + i];        // kx = 2 j + h at ky = i
+        S::inverse(v, h);                                                    // -> x = m + M h
+#pragma unroll
+        for (int m = 0; m < M; m++) tile[i * PX + m + M * h] = v[m];         // tile[ky][x]
+        __syncthreads();
+#pragma unroll
+        for (int j = 0; j < M; j++) v[j] = tile[(2 * j + h) * PX + i];       // column x = i, ky = 2 j + h
+        S::inverse(v, h);                                                    // -> y = m + M h
+        if constexpr (!GOUT) {
+#pragma unroll
+            for (int m = 0; m < M; m++) base[(m + M * h) * L + i] = v[m];    // (y, x = i)
+        } else {
+            __syncthreads();                                                 // everyone has read its column
+#pragma unroll
+            for (int m = 0; m < M; m++) tile[(m + M * h) * PX + i] = v[m];   // tile[y][x] of component p % 4
+            __syncthreads();
+            const C<R> *t4 = tile_all + (p / 4) * 4 * (L * PX);
+            const long long s0 = ((long long)blockIdx.x * (P / 4) + p / 4) * (L * L);
+            // the 8 L threads of a slice share its L^2 sites: thread (p % 4, h, i) takes rows y = (p%4) + 4 h' ...
+            const int sub = (p % 4) * 2 + h;                                 // 0 .. 7
+#pragma unroll
+            for (int mm = 0; mm < L / 8; mm++) {
+                const int y = sub + 8 * mm;
+                Herm<R> w;
+                w.m01 = t4[y * PX + i];
+                w.m02 = t4[L * PX + y * PX + i];
+                w.m12 = t4[2 * L * PX + y * PX + i];
+                const C<R> dg = t4[3 * L * PX + y * PX + i];
+                w.m00 = dg.x;
+                w.m11 = dg.y;
+                C<R> gx[9];
+                build_g(w, half_alpha, gx);
+                const long long s = s0 + y * L + i;
+#pragma unroll
+                for (int e = 0; e < 6; e++) G[(long long)e * V + s] = gx[e];
+            }
+        }
+    }
+}
+
+// ---- (z, t) planes --------------------------------------------------------------------------------
+// grid = ((Lx Ly) / XC, 4 components).  Shared-memory element (xc, z, t) at xc + XC z + PITCH t, PITCH =
+// XC LZ + padding (the 8-lane phases of the z-line stores, lanes (xc, t), land on distinct banks).
+// z lines: line l -> (xc = l % XC, t = l / XC); t lines: line l = xc + XC kz.  Two threads per line.
+template <class R, int LZ, int LT, int XC>
+struct Zt2Shape {
+    static constexpr int PHASE = 128 / (int)sizeof(C<R>);
+    static constexpr int PITCH = XC * LZ + ((XC < PHASE && (XC * LZ) % PHASE == 0) ? XC : 0);
+    static constexpr int LINES = XC * (LZ > LT ? LZ : LT);
+    static constexpr int THREADS = 2 * LINES;
+    static constexpr size_t SMEM = sizeof(C<R>) * (size_t)PITCH * LT;
+    static_assert((XC * LZ) % 16 == 0 && (XC * LT) % 16 == 0, "16 lines per warp");
+};
+
+template <class R, int LZ, int LT, int XC>
+__global__ void __launch_bounds__((Zt2Shape<R, LZ, LT, XC>::THREADS))
+    k_fftr2_zt(C<R> *__restrict__ W, Geom g, const R *__restrict__ p2tab, R scale, const DevState *__restrict__ st) {
+    if (st->done) return;
+    using Sh = Zt2Shape<R, LZ, LT, XC>;
+    constexpr int PITCH = Sh::PITCH, MZ = LZ / 2, MT = LT / 2;
+    using SZ = SplitDft<LZ, PAIR_MASK, R>;
+    using ST = SplitDft<LT, PAIR_MASK, R>;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    C<R> *tile = reinterpret_cast<C<R> *>(smem_raw);
+    const long long plane = g.S[2];
+    const int lo0 = blockIdx.x * XC;
+    C<R> *Wc = W + (long long)blockIdx.y * g.V + lo0;
+    const int tid = threadIdx.x;
+    const int h = (tid >> 4) & 1;
+    const int l = (tid >> 5) * 16 + (tid & 15);               // line number
+    const int xc = l % XC, r = l / XC;                        // z-line steps: t = r; t-line step: kz = r
+
+    // whole warps take each branch (the line counts are multiples of 16), so the shuffles inside are safe
+    if (l < XC * LT) {                                        // forward z at (xc, t = r)
+        C<R> v[MZ];
+        const C<R> *src = Wc + xc + plane * ((long long)LZ * r);
+#pragma unroll
+        for (int m = 0; m < MZ; m++) v[m] = src[plane * (m + MZ * h)];
+        SZ::forward(v, h);                                    // -> kz = 2 j + h
+#pragma unroll
+        for (int j = 0; j < MZ; j++) tile[r * PITCH + (2 * j + h) * XC + xc] = v[j];
+    }
+    __syncthreads();
+    if (l < XC * LZ) {                                        // t line at (xc, kz = r): forward, scale, inverse
+        C<R> v[MT];
+#pragma unroll
+        for (int m = 0; m < MT; m++) v[m] = tile[(m + MT * h) * PITCH + l];
+        ST::forward(v, h);                                    // -> kt = 2 j + h
+        // k-space (x, y) index of this column: the forward (x, y) sweep wrote the plane transposed
+        const int lo = lo0 + xc, kx = lo / g.L[1], ky = lo % g.L[1];
+        const R p2xyz = p2tab[kx] + p2tab[64 + ky] + p2tab[128 + r];
+#pragma unroll
+        for (int j = 0; j < MT; j++) {
+            const R p2 = p2xyz + p2tab[192 + 2 * j + h];
+            const R f = (p2 == (R)0) ? (R)0 : scale / p2;     // Alg. 1 lines 5, 7; zero mode -> 0 (R6)
+            v[j] = f * v[j];
+        }
+        ST::inverse(v, h);                                    // -> t = m + MT h
+#pragma unroll
+        for (int m = 0; m < MT; m++) tile[(m + MT * h) * PITCH + l] = v[m];
+    }
+    __syncthreads();
+    if (l < XC * LT) {                                        // inverse z at (xc, t = r)
+        C<R> v[MZ];
+#pragma unroll
+        for (int j = 0; j < MZ; j++) v[j] = tile[r * PITCH + (2 * j + h) * XC + xc];
+        SZ::inverse(v, h);                                    // -> z = m + MZ h
+        C<R> *dst = Wc + xc + plane * ((long long)LZ * r);
+#pragma unroll
+        for (int m = 0; m < MZ; m++) dst[plane * (m + MZ * h)] = v[m];
+    }
+}
+
+// ---- configuration and launchers --------------------------------------------------------------------
+// planes per CTA of the (x, y) sweeps (a multiple of 4 allows the g output) and consecutive (kx, ky) indices
+// per CTA of the (z, t) sweep
+template <class R, int L> struct Xy2Cfg;
+template <> struct Xy2Cfg<double, 16> { static constexpr int P = 8; };
+template <> struct Xy2Cfg<double, 32> { static constexpr int P = 4; };
+template <> struct Xy2Cfg<double, 64> { static constexpr int P = 1; };     // 4 planes of 64 x 64 fp64 exceed shared memory
+template <> struct Xy2Cfg<float, 16> { static constexpr int P = 8; };
+template <> struct Xy2Cfg<float, 32> { static constexpr int P = 4; };
+template <> struct Xy2Cfg<float, 64> { static constexpr int P = 4; };
+template <class R, int L> struct Zt2Cfg;
+template <> struct Zt2Cfg<double, 16> { static constexpr int XC = 4; };
+template <> struct Zt2Cfg<double, 32> { static constexpr int XC = 4; };
+template <> struct Zt2Cfg<double, 64> { static constexpr int XC = 2; };
+template <> struct Zt2Cfg<float, 16> { static constexpr int XC = 8; };
+template <> struct Zt2Cfg<float, 32> { static constexpr int XC = 4; };
+template <> struct Zt2Cfg<float, 64> { static constexpr int XC = 2; };
+
+#define LGF_REG2_LEN(X) X(16) X(32) X(64)
+
+static bool reg2_len(int L) { return L == 16 || L == 32 || L == 64; }
+
+bool fft_reg2_supported(const Geom &g) {
+    if (!(g.L[0] == g.L[1] && g.L[2] == g.L[3] && reg2_len(g.L[0]) && reg2_len(g.L[2]))) return false;
+    const long long planes = 4LL * g.L[2] * g.L[3];
+    return planes % 8 == 0 && g.S[2] % 8 == 0;
+}
+// can the inverse (x, y) sweep end with the g-build for this lattice and precision (bytes per real)?
+bool fft_reg2_gout(const Geom &g, int prec) {
+    if (!fft_reg2_supported(g)) return false;
+    if (g.L[0] == 64) return prec == 4;
+    return true;
+}
+
+template <class R, int L>
+static cudaError_t launch_xy2(int which, const Geom &g, C<R> *W, const DevState *st, cudaStream_t stream, C<R> *G,
+                              R half_alpha) {
+    constexpr int P = Xy2Cfg<R, L>::P;
+    constexpr size_t SM = sizeof(C<R>) * P * L * (L | 1);
+    const long long planes = 4LL * g.L[2] * g.L[3];
+    const int nzt = g.L[2] * g.L[3];
+    void (*kern)(C<R> *, const DevState *, C<R> *, long long, int, R) = nullptr;
+    if (which == 0) kern = k_fftr2_xy<R, L, FFT_FWD, P, false>;
+    else if (which == 2) kern = k_fftr2_xy<R, L, FFT_INV, P, false>;
+    else if constexpr (P % 4 == 0) kern = k_fftr2_xy<R, L, FFT_INV, P, true>;
+    if (!kern) return cudaErrorInvalidValue;
+    if (SM > 40 * 1024) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SM);
+        if (e != cudaSuccess) return e;
+    }
+    kern<<<(unsigned)(planes / P), 2 * P * L, SM, stream>>>(W, st, G, g.V, nzt, half_alpha);
+    return cudaGetLastError();
+}
+
+template <class R, int L>
+static cudaError_t launch_zt2(const Geom &g, C<R> *W, const R *p2tab, R scale, const DevState *st, cudaStream_t stream) {
+    constexpr int XC = Zt2Cfg<R, L>::XC;
+    using Sh = Zt2Shape<R, L, L, XC>;
+    auto kern = k_fftr2_zt<R, L, L, XC>;
+    if (Sh::SMEM > 40 * 1024) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Sh::SMEM);
+        if (e != cudaSuccess) return e;
+    }
+    dim3 grid((unsigned)(g.S[2] / XC), 4);
+    kern<<<grid, Sh::THREADS, Sh::SMEM, stream>>>(W, g, p2tab, scale, st);
+    return cudaGetLastError();
+}
+
+// which: 0 = (x, y) forward, 1 = (z, t) forward + scale + inverse, 2 = (x, y) inverse, 3 = (x, y) inverse + g
+template <class R>
+cudaError_t launch_fft_reg2(int which, const Geom &g, C<R> *W, const R *p2tab, R scale, const DevState *st,
+                            cudaStream_t stream, C<R> *G, R half_alpha) {
+    if (which == 1) {
+#define LGF_GO(LEN) if (g.L[2] == LEN) return launch_zt2<R, LEN>(g, W, p2tab, scale, st, stream);
+        LGF_REG2_LEN(LGF_GO)
+#undef LGF_GO
+        return cudaErrorInvalidValue;
+    }
+#define LGF_GO(LEN) if (g.L[0] == LEN) return launch_xy2<R, LEN>(which, g, W, st, stream, G, half_alpha);
+    LGF_REG2_LEN(LGF_GO)
+#undef LGF_GO
+    return cudaErrorInvalidValue;
+}
+
+template cudaError_t launch_fft_reg2<float>(int, const Geom &, C<float> *, const float *, float, const DevState *,
+                                            cudaStream_t, C<float> *, float);
+template cudaError_t launch_fft_reg2<double>(int, const Geom &, C<double> *, const double *, double, const DevState *,
+                                             cudaStream_t, C<double> *, double);
+
+}  // namespace lgf

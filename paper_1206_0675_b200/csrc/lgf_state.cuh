@@ -39,10 +39,12 @@ struct LinkPair {
 
 enum FftMode { FFT_FWD = 0, FFT_INV = 1, FFT_FWD_SCALE_INV = 2 };
 
+// (PASS_REG2: the two-threads-per-line register sweeps of lgf_fft_reg2.cu; `axis` as for PASS_REG)
 enum PassKind {
     PASS_AXIS = 0,        // one lattice axis per pass (any supported length)
     PASS_XY = 1,          // whole (x, y) planes: both axes transformed in one shared-memory tile
     PASS_ZT = 2,          // (z, t) planes of nlo consecutive (x, y) indices: forward z, t, scale, inverse t, z
+    PASS_REG2 = 4,
     PASS_REG = 3          // register-resident line transforms (lgf_fft_reg.cu); `axis` = 0: (x, y) forward,
                           // 1: (z, t) forward + scale + inverse, 2: (x, y) inverse, 3: (x, y) inverse ending in the
                       // g-build (writes G, not W)
@@ -75,6 +77,12 @@ bool fft_reg_t_natural(const Geom &g);
 template <class R>
 cudaError_t launch_fft_reg(int which, const Geom &g, C<R> *W, const R *twiddle_t, const R *p2tab, R scale,
                            const DevState *st, cudaStream_t stream, C<R> *G = nullptr, R half_alpha = 0);
+// two-threads-per-line register sweeps (lgf_fft_reg2.cu)
+bool fft_reg2_supported(const Geom &g);
+bool fft_reg2_gout(const Geom &g, int prec);
+template <class R>
+cudaError_t launch_fft_reg2(int which, const Geom &g, C<R> *W, const R *p2tab, R scale, const DevState *st,
+                            cudaStream_t stream, C<R> *G, R half_alpha);
 // true if a PASS_XY (first two axes) / PASS_ZT (last two axes) kernel is instantiated for these lengths
 bool fft_pair_supported(int kind, int La, int Lb);
 

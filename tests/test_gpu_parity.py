@@ -83,16 +83,16 @@ def test_delta_F_theta(lgf, name, dims, prec, storage):
 
 ACC_DIMS = [(8, 8, 8, 8), (12, 6, 16, 4), (3, 24, 2, 48), (16, 16, 16, 16), (32, 8, 64, 4), (8, 8, 24, 48),
             (24, 24, 24, 48), (32, 32, 16, 16), (64, 64, 8, 8), (8, 8, 64, 64), (16, 16, 32, 32), (24, 24, 8, 8),
-            (32, 32, 32, 32)]
+            (32, 32, 32, 32), (64, 64, 16, 16), (16, 16, 64, 64)]
 
 
 @pytest.mark.parametrize("dims", ACC_DIMS)
 @pytest.mark.parametrize("prec", [8, 4])
-@pytest.mark.parametrize("plan", ["reg", "two_axis", "axis"])
+@pytest.mark.parametrize("plan", ["reg", "reg2", "two_axis", "axis"])
 def test_accelerate(lgf, dims, prec, plan):
     """a2-a4: w = F^-1 (16/p^2) F Delta / V against the oracle's naive separable DFT, with each FFT
-    plan: register-line sweeps and shared-memory two-axis sweeps (where the lattice allows them; the
-    planner falls back otherwise) and one pass per axis."""
+    plan: register-line sweeps with one and with two threads per line, shared-memory two-axis sweeps
+    (where the lattice allows them; the planner falls back otherwise) and one pass per axis."""
     import torch
 
     D = random_herm_field(dims, 99)
@@ -100,6 +100,7 @@ def test_accelerate(lgf, dims, prec, plan):
     w_o = oracle.accelerate(dims, D)
     with lgf.Context(dims, prec, 18) as ctx:
         ctx.tune("fft_reg", int(plan == "reg"))
+        ctx.tune("fft_reg2", int(plan == "reg2"))
         ctx.tune("fft_two_axis", int(plan != "axis"))
         if plan == "axis":
             assert ctx.fft_passes() == 7
@@ -228,6 +229,20 @@ def test_trajectory_tiled_sweep(lgf, config_cache):
     assert np.max(np.abs(Fh - F_o) / np.abs(F_o)) < 1e-12
     assert np.max(np.abs(Th - T_o) / np.abs(T_o)) < 1e-12
     assert np.max(np.abs(out - U_o)) < 1e-11
+
+
+@pytest.mark.parametrize("prec,storage", VARIANTS)
+def test_trajectory_two_thread_fft(lgf, config_cache, prec, storage):
+    """20 iterations of C2 with the two-threads-per-line FFT sweeps (lgf_fft_reg2.cu), whose inverse
+    (x, y) sweep ends with the g-build: the same parity bar as the default plan."""
+    dims = inputs.CONFIGS["C2"]["dims"]
+    U = config_cache("C2")
+    U_o, F_o, T_o = oracle.iterate(dims, U, ALPHA, 20)
+    Fh, Th, P, out = run_trajectory(lgf, dims, U, prec, storage, 20, tune={"fft_reg2": 1})
+    tol = TOL[prec]
+    assert np.max(np.abs(Fh - F_o) / np.abs(F_o)) < tol["scalar"]
+    assert np.max(np.abs(Th - T_o) / np.abs(T_o)) < tol["scalar"]
+    assert np.max(np.abs(out - U_o)) < tol["links"]
 
 
 def test_trajectory_asymmetric(lgf):
