@@ -40,8 +40,7 @@ struct lgf_ctx {
     bool profiling = false;
     int tune_two_axis = 1;       // lgf_tune: use the two-axis FFT passes when available
     int tune_reg = 1;            // lgf_tune: use the register-line FFT sweeps when available
-    int tune_reg2 = -1;          // lgf_tune: two-threads-per-line sweeps: 1 = prefer, 0 = never, -1 = where the
-                                 // one-thread kernels do not exist (64-point axes)
+    int tune_reg2 = 1;           // lgf_tune: two-threads-per-line FFT sweeps where the lattice allows (0 = never)
     int tune_xy_planes = 0;      // lgf_tune: planes per CTA of the (x, y) pass (0 = planner's choice)
     int tune_zt_xc = 0;          // lgf_tune: consecutive (x, y) indices per CTA of the (z, t) pass
     int tune_fuse_g = 1;         // lgf_tune: end the last FFT sweep with the g-build (register-line plan only)
@@ -196,7 +195,11 @@ static int plan_passes(lgf_ctx *ctx) {
         const bool natural[4] = {true, true, true, true};
         return finish(natural);
     };
-    if (ctx->tune_two_axis && ctx->tune_reg2 == 1 && fft_reg2_supported(g)) return plan_reg2();
+    // Two threads per line wherever those kernels exist (16-, 32-, 64-point axes).  Measured on B200 against
+    // the one-thread family at 32^4 (warm, CUDA events): fp64 iteration 0.3886 -> 0.3854 ms, fp32 0.2402 ->
+    // 0.2335 ms; at 64^4 (against the shared-memory passes) fp64 7.60 -> 6.72 ms, fp32 4.48 -> 3.78 ms.  A
+    // per-sweep mix of the two families was tried and is not better (0.3908 ms).
+    if (ctx->tune_two_axis && ctx->tune_reg2 != 0 && fft_reg2_supported(g)) return plan_reg2();
     if (ctx->tune_two_axis && ctx->tune_reg && fft_reg_supported(g)) {
         for (int w = 0; w < 3; w++) {
             AxisPass p{};
@@ -207,7 +210,6 @@ static int plan_passes(lgf_ctx *ctx) {
         const bool natural[4] = {true, true, true, fft_reg_t_natural(g)};
         return finish(natural);
     }
-    if (ctx->tune_two_axis && ctx->tune_reg2 != 0 && fft_reg2_supported(g)) return plan_reg2();
     const bool permuted[4] = {false, false, false, false};
     const size_t SMEM_MAX = 200 * 1024;
     const long long MIN_GRID = 2 * 148;

@@ -124,8 +124,10 @@ def test_fft_plan_and_tile_overrides(lgf, dims, passes):
     res = []
     with lgf.Context(dims, 8, 18) as ctx:
         assert ctx.fft_passes() == passes
-        for key, val in [(None, 0), ("fft_reg", 0), ("fft_xy_planes", 1), ("fft_xy_planes", 4), ("fft_zt_xc", 2),
-                         ("fft_zt_xc", 8), ("fft_two_axis", 0)]:
+        # default plan -> one-thread register lines -> shared-memory two-axis passes (with tile overrides) -> one
+        # pass per axis
+        for key, val in [(None, 0), ("fft_reg2", 0), ("fft_reg", 0), ("fft_xy_planes", 1), ("fft_xy_planes", 4),
+                         ("fft_zt_xc", 2), ("fft_zt_xc", 8), ("fft_two_axis", 0)]:
             if key:
                 ctx.tune(key, val)
             ctx.set_field(to_dev(D, 8))
