@@ -123,12 +123,29 @@ int lgf_step_update(lgf_ctx *ctx, double alpha);
 int lgf_get_field(lgf_ctx *ctx, void *d_field);
 int lgf_set_field(lgf_ctx *ctx, const void *d_field);
 
+/* ---- accumulated gauge transformation ----------------------------- */
+
+/* on != 0: keep G(x) = g_n(x) ... g_1(x), the product of the rotations g_k(x) (a5) of all updates applied
+ * since the last set_links / fix, so that the current configuration is
+ *   U_mu(x) = G(x) U0_mu(x) G(x + mu)^dag        (eq. 2, composed over the iterations)
+ * with U0 the loaded one -- what a user needs to carry other fields (quark sources, propagators,
+ * PAPER.md:21) into the same gauge.  Costs one extra pass per iteration (12 + 18 + 18 reals per site) and
+ * 18 reals per site of device memory.  G is reset to 1 by set_links / fix and by this call.  on == 0
+ * frees the storage.  Synchronises. */
+int lgf_track_transform(lgf_ctx *ctx, int on);
+/* Copy G out: d_transform[s][i][j][re/im], 18 reals per site in the context's precision (as a torch tensor:
+ * [Lt, Lz, Ly, Lx, 3, 3] complex).  LGF_ESTATE if tracking is off.  Asynchronous on the context's stream. */
+int lgf_get_transform(lgf_ctx *ctx, void *d_transform);
+
 /* ---- tuning --------------------------------------------------------------------------------------- */
 
 /* Override a planner choice (takes effect from the next iteration; results are unchanged up to
  * rounding).  Keys: "fft_two_axis" (1 = use the three-sweep two-axis FFT passes when the lattice
  * allows, 0 = one pass per axis), "fft_reg" (1 = use the register-line sweeps when the lattice allows), "fft_xy_planes" ((x, y) planes per CTA, 0 = automatic),
- * "fft_zt_xc" (consecutive (x, y) indices per CTA of the (z, t) pass, 0 = automatic).
+ * "fft_zt_xc" (consecutive (x, y) indices per CTA of the (z, t) pass, 0 = automatic), "fft_reg2" (1 = two
+ * threads per line where the lattice allows), "fuse_g" (1 = the last FFT sweep ends with the g-build),
+ * "sweep_tz" (z-planes per (z, t) tile of the sweep's CTA order, 0 = automatic, 1 = plain order),
+ * "sweep_tiled" (1 = tiled sweep variant), "sweep_tt" (its t-march length).
  * Unknown key or NULL: LGF_EINVAL.  Synchronises. */
 int lgf_tune(lgf_ctx *ctx, const char *key, int value);
 /* Number of FFT kernel launches per iteration under the current plan (3 or up to 7). */

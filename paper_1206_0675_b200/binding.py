@@ -50,6 +50,8 @@ SIGNATURES = {
     "lgf_step_update": (_i, [_vp, _d]),
     "lgf_get_field": (_i, [_vp, _vp]),
     "lgf_set_field": (_i, [_vp, _vp]),
+    "lgf_track_transform": (_i, [_vp, _i]),
+    "lgf_get_transform": (_i, [_vp, _vp]),
     "lgf_tune": (_i, [_vp, ctypes.c_char_p, _i]),
     "lgf_fft_passes": (_i, [_vp]),
     "lgf_set_profiling": (_i, [_vp, _i]),
@@ -232,6 +234,14 @@ class Context:
 
     def set_field(self, field):
         _check(self._h, load().lgf_set_field(self._h, _dev_ptr(field, self.precision, self.V * 18)))
+
+    # -- accumulated gauge transformation ----------------------------------------------------------
+    def track_transform(self, on=True):
+        _check(self._h, load().lgf_track_transform(self._h, int(bool(on))))
+
+    def get_transform(self, out):
+        _check(self._h, load().lgf_get_transform(self._h, _dev_ptr(out, self.precision, self.V * 18)))
+        return out
 
     # -- tuning -----------------------------------------------------------------------------------
     def tune(self, key, value):

@@ -22,6 +22,7 @@ struct lgf_ctx {
     void *links[2] = {nullptr, nullptr};   // C<R>[4][3*nr][V] each: the sweep reads one and writes the other
     void *W = nullptr;           // C<R>[4][V]   packed Delta / w
     void *G = nullptr;           // C<R>[6][V]   rows 0, 1 of g(x)
+    void *Gacc = nullptr;        // C<R>[9][V]   accumulated transformation g_n ... g_1 (lgf_track_transform), or null
     bool w_is_delta = false;     // W holds Delta of the current configuration and `partial` its F / theta sums
     bool recorded = false;       // the current configuration's (F, theta) is already in the history
     int nb_partial = 0;          // number of per-block partial sums currently in `partial`
@@ -354,6 +355,10 @@ static int step_update(lgf_ctx *ctx, double alpha, double tol, int record, bool 
         Bracket br(ctx, LGF_K_GBUILD);
         CK(launch_gbuild<R>((const C<R> *)ctx->W, (C<R> *)ctx->G, ctx->g, (R)(0.5 * alpha), ctx->st, ctx->stream));
     }
+    if (ctx->Gacc) {                                      // Gacc <- g Gacc, with the g this update applies
+        Bracket br(ctx, LGF_K_GBUILD);
+        CK(launch_gacc<R>(1, (const C<R> *)ctx->G, (C<R> *)ctx->Gacc, (R *)nullptr, ctx->g, ctx->st, ctx->stream));
+    }
     if (ctx->tune_sweep_tiled) {
         Bracket br(ctx, LGF_K_UPDATE);
         CK(launch_sweep_tiled<R>(ctx->nr, link_pair<R>(ctx), (const C<R> *)ctx->G, (C<R> *)ctx->W, ctx->g, ctx->tile,
@@ -492,6 +497,7 @@ int lgf_destroy(lgf_ctx *ctx) {
     cudaFree(ctx->links[1]);
     cudaFree(ctx->W);
     cudaFree(ctx->G);
+    cudaFree(ctx->Gacc);
     cudaFree(ctx->partial);
     cudaFree(ctx->st);
     cudaFree(ctx->hist);
@@ -520,6 +526,13 @@ int lgf_set_links(lgf_ctx *ctx, const void *d_links) {
             CK(launch_convert_in<double>(ctx->nr, (const double *)d_links, (C<double> *)ctx->links[0], ctx->g, ctx->stream));
         else
             CK(launch_convert_in<float>(ctx->nr, (const float *)d_links, (C<float> *)ctx->links[0], ctx->g, ctx->stream));
+    }
+    if (ctx->Gacc) {
+        ctx->launches++;
+        if (ctx->prec == LGF_FP64)
+            CK(launch_gacc<double>(0, nullptr, (C<double> *)ctx->Gacc, nullptr, ctx->g, ctx->st, ctx->stream));
+        else
+            CK(launch_gacc<float>(0, nullptr, (C<float> *)ctx->Gacc, nullptr, ctx->g, ctx->st, ctx->stream));
     }
     ctx->launches++;
     CK(launch_reset_state(ctx->st, ctx->stream));        // also makes buffer 0 the current one
@@ -731,6 +744,34 @@ int lgf_set_field(lgf_ctx *ctx, const void *d_field) {
     if (ctx->prec == LGF_FP64) CK(launch_field_set<double>((C<double> *)ctx->W, (const double *)d_field, ctx->g, ctx->stream));
     else CK(launch_field_set<float>((C<float> *)ctx->W, (const float *)d_field, ctx->g, ctx->stream));
     ctx->w_is_delta = false;
+    return LGF_OK;
+}
+
+int lgf_track_transform(lgf_ctx *ctx, int on) {
+    if (!ctx) return LGF_EINVAL;
+    CK(cudaStreamSynchronize(ctx->stream));
+    if (!on) {
+        cudaFree(ctx->Gacc);
+        ctx->Gacc = nullptr;
+        return LGF_OK;
+    }
+    if (!ctx->Gacc) CK(cudaMalloc(&ctx->Gacc, (size_t)ctx->g.V * 9 * 2 * ctx->prec));
+    ctx->launches++;
+    if (ctx->prec == LGF_FP64)
+        CK(launch_gacc<double>(0, nullptr, (C<double> *)ctx->Gacc, nullptr, ctx->g, ctx->st, ctx->stream));
+    else
+        CK(launch_gacc<float>(0, nullptr, (C<float> *)ctx->Gacc, nullptr, ctx->g, ctx->st, ctx->stream));
+    return LGF_OK;
+}
+
+int lgf_get_transform(lgf_ctx *ctx, void *d_transform) {
+    if (!ctx || !d_transform) return fail(ctx, LGF_EINVAL, "lgf_get_transform: null argument");
+    if (!ctx->Gacc) return fail(ctx, LGF_ESTATE, "lgf_get_transform: tracking is off (lgf_track_transform)");
+    ctx->launches++;
+    if (ctx->prec == LGF_FP64)
+        CK(launch_gacc<double>(2, nullptr, (C<double> *)ctx->Gacc, (double *)d_transform, ctx->g, ctx->st, ctx->stream));
+    else
+        CK(launch_gacc<float>(2, nullptr, (C<float> *)ctx->Gacc, (float *)d_transform, ctx->g, ctx->st, ctx->stream));
     return LGF_OK;
 }
 

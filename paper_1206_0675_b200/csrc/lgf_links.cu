@@ -337,6 +337,42 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB)
     close_sweep(f, t, partial, scratch, g.V, tol, record, st, hist, hist_cap, ticket);
 }
 
+// ---- accumulated gauge transformation ------------------------------
+// Gacc(x) <- g(x) Gacc(x): after n updates Gacc(x) = g_n(x) ... g_1(x), the transformation that takes the
+// loaded configuration to the current one, U_mu(x) = Gacc(x) U0_mu(x) Gacc(x + mu)^dag (eq. 2, PAPER.md:45,
+// composed).  Gacc is stored like a link plane set: Gacc[e][s], e = 0..8 (all three rows: products of
+// many g drift off SU(3) by rounding, which eq. 8 would hide rather than carry).
+template <class R>
+__global__ void __launch_bounds__(SITE_THREADS) k_gacc(const C<R> *__restrict__ G, C<R> *__restrict__ A, Geom g,
+                                                        const DevState *__restrict__ st) {
+    if (st->done) return;
+    const long long s = (long long)blockIdx.x * SITE_THREADS + threadIdx.x;
+    if (s >= g.V) return;
+    C<R> gx[9], a[9], out[9];
+    load_g(G, g.V, s, gx);
+#pragma unroll
+    for (int e = 0; e < 9; e++) a[e] = A[(long long)e * g.V + s];
+    mat_mul<3>(gx, a, out);
+#pragma unroll
+    for (int e = 0; e < 9; e++) A[(long long)e * g.V + s] = out[e];
+}
+template <class R>
+__global__ void __launch_bounds__(SITE_THREADS) k_gacc_identity(C<R> *__restrict__ A, Geom g) {
+    const long long s = (long long)blockIdx.x * SITE_THREADS + threadIdx.x;
+    if (s >= g.V) return;
+#pragma unroll
+    for (int e = 0; e < 9; e++) A[(long long)e * g.V + s] = mk<R>((e % 4 == 0) ? (R)1 : (R)0, (R)0);
+}
+// canonical output: out[s][i][j] complex, 18 reals per site
+template <class R>
+__global__ void __launch_bounds__(SITE_THREADS) k_gacc_get(const C<R> *__restrict__ A, R *__restrict__ out, Geom g) {
+    const long long s = (long long)blockIdx.x * SITE_THREADS + threadIdx.x;
+    if (s >= g.V) return;
+    C<R> *dst = reinterpret_cast<C<R> *>(out) + s * 9;
+#pragma unroll
+    for (int e = 0; e < 9; e++) dst[e] = A[(long long)e * g.V + s];
+}
+
 // ---- plaquette ------------------------------------------------------------------------------------
 template <class R, int NR>
 __global__ void __launch_bounds__(SITE_THREADS) k_plaquette(LinkPair<R> lp, Geom g, double *__restrict__ partial,
@@ -594,6 +630,14 @@ cudaError_t launch_convert_out(int nr, LinkPair<R> links, R *canon, const Geom &
     return cudaGetLastError();
 }
 template <class R>
+cudaError_t launch_gacc(int op, const C<R> *G, C<R> *A, R *out, const Geom &g, const DevState *st, cudaStream_t stream) {
+    const int nb = site_blocks(g);
+    if (op == 0) k_gacc_identity<R><<<nb, SITE_THREADS, 0, stream>>>(A, g);
+    else if (op == 1) k_gacc<R><<<nb, SITE_THREADS, 0, stream>>>(G, A, g, st);
+    else k_gacc_get<R><<<nb, SITE_THREADS, 0, stream>>>(A, out, g);
+    return cudaGetLastError();
+}
+template <class R>
 cudaError_t launch_field_get(const C<R> *W, R *field, const Geom &g, cudaStream_t stream) {
     k_field_get<R><<<site_blocks(g), SITE_THREADS, 0, stream>>>(W, field, g);
     return cudaGetLastError();
@@ -635,6 +679,7 @@ cudaError_t launch_clear_done(DevState *st, cudaStream_t stream) {
                                              cudaStream_t);                                                           \
     template cudaError_t launch_convert_in<R>(int, const R *, C<R> *, const Geom &, cudaStream_t);                    \
     template cudaError_t launch_convert_out<R>(int, LinkPair<R>, R *, const Geom &, const DevState *, cudaStream_t);  \
+    template cudaError_t launch_gacc<R>(int, const C<R> *, C<R> *, R *, const Geom &, const DevState *, cudaStream_t); \
     template cudaError_t launch_field_get<R>(const C<R> *, R *, const Geom &, cudaStream_t);                          \
     template cudaError_t launch_field_set<R>(C<R> *, const R *, const Geom &, cudaStream_t);
 LGF_INST(float)

@@ -374,6 +374,51 @@ def test_history_entry0_survives_a_measurement_before_iterate(lgf, config_cache,
     assert np.max(np.abs(Th - T_o) / np.abs(T_o)) < 1e-12
 
 
+@pytest.mark.parametrize("dims", [(8, 8, 8, 8), (12, 6, 16, 4), (16, 16, 16, 16)])
+@pytest.mark.parametrize("prec,storage", [(8, 18), (8, 12), (4, 18)])
+def test_accumulated_transformation(lgf, dims, prec, storage):
+    """NEXT-2: lgf_track_transform / lgf_get_transform.  G(x) = g_n(x) ... g_1(x) against the product of the
+    oracle's g fields, and the defining property G U0 G(x+mu)^dag = U_n on the CUDA side's own output."""
+    import torch
+
+    U0 = inputs.smooth_config(dims, 0.3, 97, haar=True)
+    n = 8
+    U, G = U0.copy(), np.broadcast_to(np.eye(3, dtype=np.complex128), site_shape(dims) + (3, 3)).copy()
+    for _ in range(n):
+        D, _, _ = oracle.measure(dims, U)
+        g = oracle.build_g(dims, oracle.accelerate(dims, D), ALPHA)
+        U = oracle.transform(dims, U, g)
+        G = g @ G
+    tol = TOL[prec]["links"]
+    cdt = torch.complex128 if prec == 8 else torch.complex64
+    with lgf.Context(dims, prec, storage) as ctx:
+        with pytest.raises(lgf.LgfError) as e:
+            ctx.get_transform(torch.empty(site_shape(dims) + (3, 3), dtype=cdt, device="cuda"))
+        assert e.value.code == lgf.LGF_ESTATE
+        ctx.track_transform(True)
+        d = to_dev(U0, prec)
+        ctx.set_links(d)
+        ctx.iterate(ALPHA, 3)
+        ctx.step_accelerate()                 # the single-step entry points accumulate too
+        ctx.step_update(ALPHA)
+        ctx.iterate(ALPHA, n - 4)
+        Gd = to_np(ctx.get_transform(torch.empty(site_shape(dims) + (3, 3), dtype=cdt, device="cuda")))
+        out = to_np(ctx.get_links(torch.empty_like(d)))
+        assert np.max(np.abs(Gd - G)) < tol
+        assert np.max(np.abs(out - U)) < tol
+        assert np.max(np.abs(oracle.transform(dims, U0, Gd) - out)) < tol
+        # set_links resets G to the identity
+        ctx.set_links(d)
+        G1 = to_np(ctx.get_transform(torch.empty(site_shape(dims) + (3, 3), dtype=cdt, device="cuda")))
+        assert np.array_equal(G1, np.broadcast_to(np.eye(3), G1.shape))
+        # a converged fix stops accumulating when the iteration stops
+        it = ctx.fix(d, ALPHA, 1e-15 if prec == 8 else 1e-12, 500)
+        Gf = to_np(ctx.get_transform(torch.empty(site_shape(dims) + (3, 3), dtype=cdt, device="cuda")))
+        assert 0 < it < 500
+        assert np.max(np.abs(oracle.transform(dims, U0, Gf) - to_np(d))) < tol * (1 + it / 20)
+        ctx.track_transform(False)
+
+
 def test_12_real_matches_18_real(lgf, config_cache):
     """Third-row reconstruction (eq. 8) changes rounding only."""
     dims = inputs.CONFIGS["C1"]["dims"]

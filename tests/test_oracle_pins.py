@@ -405,3 +405,25 @@ def test_iterate_and_fix_agree_and_count_updates():
     # max_iter cap
     _, it3, _, _ = oracle.fix(dims, U, 0.08, 1e-15, 5)
     assert it3 == 5
+
+
+def test_accumulated_transformation_carries_U0_to_Un():
+    """with G(x) = g_n(x) ... g_1(x) (left multiplication, newest factor first) the
+    configuration after n updates is G(x) U0_mu(x) G(x+mu)^dag (eq. 2 composed).  Built here from the oracle's
+    single steps; it must reproduce oracle.iterate's configuration, and G must stay in SU(3)."""
+    dims = (4, 6, 4, 8)
+    U0 = inputs.smooth_config(dims, 0.3, 31, haar=True)
+    n = 6
+    U = U0.copy()
+    G = np.broadcast_to(np.eye(3, dtype=np.complex128), U0.shape[:4] + (3, 3)).copy()
+    for _ in range(n):
+        D, _, _ = oracle.measure(dims, U)
+        g = oracle.build_g(dims, oracle.accelerate(dims, D), 0.08)
+        U = oracle.transform(dims, U, g)
+        G = g @ G
+    U_n, _, _ = oracle.iterate(dims, U0, 0.08, n)
+    assert np.max(np.abs(U - U_n)) < 1e-13
+    assert np.max(np.abs(oracle.transform(dims, U0, G) - U_n)) < 1e-13
+    # the other order of the product is NOT the transformation (the g_k do not commute)
+    assert np.max(np.abs(G @ np.conj(np.swapaxes(G, -1, -2)) - np.eye(3))) < 1e-14
+    assert np.max(np.abs(np.linalg.det(G) - 1)) < 1e-14
