@@ -22,6 +22,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "lgf_oracle.c")
+_SRC_HB = os.path.join(_HERE, "lgf_heatbath_oracle.c")      # thermalisation oracle
 _LIB = os.path.join(_HERE, "liblgf_oracle.so")
 CFLAGS = ["-O2", "-std=c11", "-fopenmp", "-fcx-limited-range", "-shared", "-fPIC"]
 
@@ -30,9 +31,10 @@ _lib = None
 
 def build(force: bool = False) -> str:
     """Compile the oracle with gcc (idempotent).  Returns the path of the shared object."""
-    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+    newest = max(os.path.getmtime(_SRC), os.path.getmtime(_SRC_HB))
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < newest:
         tmp = _LIB + ".tmp.%d" % os.getpid()
-        subprocess.run(["gcc", *CFLAGS, _SRC, "-o", tmp, "-lm"], check=True)
+        subprocess.run(["gcc", *CFLAGS, _SRC, _SRC_HB, "-o", tmp, "-lm"], check=True)
         os.replace(tmp, _LIB)
     return _LIB
 
@@ -176,3 +178,39 @@ def reconstruct_row3(rows01):
     out = np.empty(3, np.complex128)
     _load().orc_reconstruct_row3(_ptr(rows01), _ptr(out))
     return out
+
+
+# ---- thermalisation oracle (lgf_heatbath_oracle.c) -------------------------
+def hb_staples(dims, U):
+    """Staple sums A_mu(x) of every link: shape (Lt, Lz, Ly, Lx, 4, 3, 3); Re tr[U A] sums the plaquettes
+    that contain the link."""
+    dims, cd = _dims(dims)
+    U = _c128(U, _site_shape(dims) + (4, 3, 3))
+    A = np.empty_like(U)
+    _load().orc_hb_staples(cd, _ptr(U), _ptr(A))
+    return A
+
+
+def hb_kp_sample(a: float, seed: int, n: int):
+    """n Kennedy-Pendleton draws X ~ exp(a x0) sqrt(1 - x0^2) dx0 dOmega.  Returns (X[n, 4], attempts[n])."""
+    X = np.empty((n, 4), np.float64)
+    att = np.empty(n, np.int32)
+    lib = _load()
+    lib.orc_hb_kp_sample.argtypes = [ctypes.c_double, ctypes.c_ulonglong, ctypes.c_long, ctypes.c_void_p, ctypes.c_void_p]
+    lib.orc_hb_kp_sample(float(a), int(seed), int(n), X.ctypes.data, att.ctypes.data)
+    return X, att
+
+
+def heatbath(dims, U, beta: float, seed: int, sweep0: int, nsweeps: int):
+    """nsweeps Cabibbo-Marinari heat-bath sweeps (numbered from sweep0) of the Wilson action at beta.
+    Returns the new configuration."""
+    dims, cd = _dims(dims)
+    U = _c128(U, _site_shape(dims) + (4, 3, 3)).copy()
+    lib = _load()
+    lib.orc_heatbath.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_double, ctypes.c_ulonglong, ctypes.c_long,
+                                 ctypes.c_long]
+    lib.orc_heatbath.restype = ctypes.c_int
+    rc = lib.orc_heatbath(cd, _ptr(U), float(beta), int(seed), int(sweep0), int(nsweeps))
+    if rc != 0:
+        raise ValueError("heatbath needs even lattice extents")
+    return U
