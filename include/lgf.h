@@ -123,6 +123,20 @@ int lgf_step_update(lgf_ctx *ctx, double alpha);
 int lgf_get_field(lgf_ctx *ctx, void *d_field);
 int lgf_set_field(lgf_ctx *ctx, const void *d_field);
 
+/* ---- thermalisation ------------------------------------------------ */
+
+/* nsweeps heat-bath sweeps of the internal configuration with the SU(3) Wilson action
+ *   S = beta sum_p [1 - Re tr U_p / 3]
+ * -- the producer of the paper's kind of input ("generated via importance sampling using, for example, the
+ * Wilson action"; beta = 5.8, 6.0, 6.2, :211).  The paper names no algorithm; this is the
+ * Cabibbo-Marinari pseudo-heat-bath over the three SU(2) subgroups with Creutz / Kennedy-Pendleton sampling
+ * in checkerboard order, driven by counter-based uniform numbers (readings R24-R27), so that the
+ * result is a deterministic function of (loaded configuration, beta, seed, number of sweeps applied since
+ * set_links) whatever the split into calls.  Arithmetic in double whatever the context's precision.  All
+ * extents must be even (LGF_EINVAL otherwise).  Resets the history, the iteration counter and the
+ * accumulated transformation, as loading a new configuration would.  Asynchronous. */
+int lgf_thermalize(lgf_ctx *ctx, double beta, int nsweeps, unsigned long long seed);
+
 /* ---- accumulated gauge transformation ----------------------------- */
 
 /* on != 0: keep G(x) = g_n(x) ... g_1(x), the product of the rotations g_k(x) (a5) of all updates applied
@@ -155,7 +169,7 @@ int lgf_fft_passes(const lgf_ctx *ctx);
 
 /* Kernel classes for per-kernel timing. */
 enum { LGF_K_DELTA = 0, LGF_K_FFT = 1, LGF_K_UPDATE = 2, LGF_K_GBUILD = 3, LGF_K_CONVERT = 4,
-       LGF_K_PLAQ = 5, LGF_K_COUNT = 6,
+       LGF_K_PLAQ = 5, LGF_K_HEATBATH = 6, LGF_K_COUNT = 7,
        LGF_K_ITERATION = 100 /* lgf_algorithmic_bytes only: the whole-iteration yard-stick */ };
 /* When on != 0 every kernel launch is bracketed by CUDA events on the context's stream. */
 int lgf_set_profiling(lgf_ctx *ctx, int on);

@@ -20,9 +20,9 @@ import numpy as np
 LGF_FP32, LGF_FP64 = 4, 8
 LGF_LINKS_18, LGF_LINKS_12 = 18, 12
 LGF_OK, LGF_EINVAL, LGF_ENOMEM, LGF_ECUDA, LGF_ESTATE, LGF_ENAN = 0, -1, -2, -3, -4, -5
-LGF_K_DELTA, LGF_K_FFT, LGF_K_UPDATE, LGF_K_GBUILD, LGF_K_CONVERT, LGF_K_PLAQ, LGF_K_COUNT = 0, 1, 2, 3, 4, 5, 6
+LGF_K_DELTA, LGF_K_FFT, LGF_K_UPDATE, LGF_K_GBUILD, LGF_K_CONVERT, LGF_K_PLAQ, LGF_K_HEATBATH, LGF_K_COUNT = 0, 1, 2, 3, 4, 5, 6, 7
 LGF_K_ITERATION = 100
-KERNEL_CLASSES = ("delta", "fft", "update", "gbuild", "convert", "plaquette")
+KERNEL_CLASSES = ("delta", "fft", "update", "gbuild", "convert", "plaquette", "heatbath")
 
 _LIBPATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "liblgf.so")
 _lib = None
@@ -50,6 +50,7 @@ SIGNATURES = {
     "lgf_step_update": (_i, [_vp, _d]),
     "lgf_get_field": (_i, [_vp, _vp]),
     "lgf_set_field": (_i, [_vp, _vp]),
+    "lgf_thermalize": (_i, [_vp, _d, _i, ctypes.c_ulonglong]),
     "lgf_track_transform": (_i, [_vp, _i]),
     "lgf_get_transform": (_i, [_vp, _vp]),
     "lgf_tune": (_i, [_vp, ctypes.c_char_p, _i]),
@@ -234,6 +235,10 @@ class Context:
 
     def set_field(self, field):
         _check(self._h, load().lgf_set_field(self._h, _dev_ptr(field, self.precision, self.V * 18)))
+
+    # -- thermalisation --------------------------------------------------------------------------
+    def thermalize(self, beta, nsweeps, seed):
+        _check(self._h, load().lgf_thermalize(self._h, float(beta), int(nsweeps), int(seed)))
 
     # -- accumulated gauge transformation ----------------------------------------------------------
     def track_transform(self, on=True):

@@ -37,6 +37,7 @@ struct lgf_ctx {
     void *p2tab = nullptr;                                     // R[4][64]
     void *staging = nullptr;     // canonical-layout device buffer for the *_host entry points
     std::vector<AxisPass> passes;
+    unsigned long long hb_sweeps = 0;   // heat-bath sweeps applied since the last set_links (selects the random stream)
     bool have_links = false;
     bool profiling = false;
     int tune_two_axis = 1;       // lgf_tune: use the two-axis FFT passes when available
@@ -539,6 +540,7 @@ int lgf_set_links(lgf_ctx *ctx, const void *d_links) {
     ctx->have_links = true;
     ctx->w_is_delta = false;
     ctx->recorded = false;
+    ctx->hb_sweeps = 0;
     return LGF_OK;
 }
 
@@ -747,6 +749,38 @@ int lgf_set_field(lgf_ctx *ctx, const void *d_field) {
     return LGF_OK;
 }
 
+int lgf_thermalize(lgf_ctx *ctx, double beta, int nsweeps, unsigned long long seed) {
+    if (!ctx || nsweeps < 0 || !(beta > 0.0)) return fail(ctx, LGF_EINVAL, "lgf_thermalize: bad argument");
+    if (!ctx->have_links) return fail(ctx, LGF_ESTATE, "lgf_thermalize: no configuration loaded");
+    for (int mu = 0; mu < 4; mu++)
+        if (ctx->g.L[mu] % 2) return fail(ctx, LGF_EINVAL, "lgf_thermalize: the checkerboard needs even extents");
+    const unsigned long long key = heatbath_key(seed);
+    for (int sw = 0; sw < nsweeps; sw++, ctx->hb_sweeps++)
+        for (int mu = 0; mu < 4; mu++)
+            for (int parity = 0; parity < 2; parity++) {
+                Bracket br(ctx, LGF_K_HEATBATH);
+                if (ctx->prec == LGF_FP64)
+                    CK(launch_heatbath<double>(ctx->nr, link_pair<double>(ctx), ctx->g, ctx->st, beta, key, ctx->hb_sweeps,
+                                               mu, parity, ctx->stream));
+                else
+                    CK(launch_heatbath<float>(ctx->nr, link_pair<float>(ctx), ctx->g, ctx->st, beta, key, ctx->hb_sweeps, mu,
+                                              parity, ctx->stream));
+            }
+    // a new configuration: the history, the counters and the accumulated transformation start again
+    ctx->launches++;
+    CK(launch_reset_counters(ctx->st, ctx->stream));
+    ctx->w_is_delta = false;
+    ctx->recorded = false;
+    if (ctx->Gacc) {
+        ctx->launches++;
+        if (ctx->prec == LGF_FP64)
+            CK(launch_gacc<double>(0, nullptr, (C<double> *)ctx->Gacc, nullptr, ctx->g, ctx->st, ctx->stream));
+        else
+            CK(launch_gacc<float>(0, nullptr, (C<float> *)ctx->Gacc, nullptr, ctx->g, ctx->st, ctx->stream));
+    }
+    return LGF_OK;
+}
+
 int lgf_track_transform(lgf_ctx *ctx, int on) {
     if (!ctx) return LGF_EINVAL;
     CK(cudaStreamSynchronize(ctx->stream));
@@ -827,6 +861,8 @@ double lgf_algorithmic_bytes(const lgf_ctx *ctx, int kernel_class) {
         case LGF_K_GBUILD: return V * 20.0 * R;                   // read w (8), write rows 0, 1 of g (12)
         case LGF_K_ITERATION: return V * (12.0 * nl + 64.0) * R;  // SURVEY.md section 8(d) yard-stick
         case LGF_K_PLAQ: return V * 4.0 * nl * R;
+        case LGF_K_HEATBATH: return V * 36.0 * nl * R;            // one SWEEP = 8 class passes, each reading every
+                                                                  // link once (4 V) and writing V / 2
         case LGF_K_CONVERT: return V * (72.0 + 4.0 * nl) * R;
         default: return 0.0;
     }

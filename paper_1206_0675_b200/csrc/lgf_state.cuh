@@ -115,6 +115,13 @@ cudaError_t launch_field_get(const C<R> *W, R *field, const Geom &g, cudaStream_
 template <class R>
 cudaError_t launch_field_set(C<R> *W, const R *field, const Geom &g, cudaStream_t stream);
 
+// thermalisation (lgf_heatbath.cu): one class (mu, parity) of heat-bath sweep number `sweep`
+unsigned long long heatbath_key(unsigned long long seed);
+template <class R>
+cudaError_t launch_heatbath(int nr, LinkPair<R> links, const Geom &g, const DevState *st, double beta,
+                            unsigned long long key, unsigned long long sweep, int mu, int parity, cudaStream_t stream);
+cudaError_t launch_reset_counters(DevState *st, cudaStream_t stream);
+
 // F / theta finalisation (precision independent)
 // after_sweep: the partial sums come from a sweep (flip `cur`, count the update); record: append (F, theta)
 // to the history and apply the stop test theta < tol
