@@ -40,7 +40,11 @@
  *     delta, clipped to [0, 2], is used.
  *   uniforms: u_n = ((mix64(key + (idx + 1) G) >> 11) + 0.5) 2^-53, key = mix64(seed ^ G), G = 0x9E3779B97F4A7C15,
  *     mix64 = the splitmix64 finaliser, idx = (((((sweep 8 + mu 2 + parity) V + site) 3 + k) 32 + t) 6 + n).   (R27)
- *   No reunitarisation is applied (the products stay in SU(3) to rounding: ~1e-15 per sweep).
+ *   After its three subgroup updates the link is re-projected onto SU(3): Gram-Schmidt on rows 0, 1, row 2 =
+ *     (row0 x row1)^* (the same projection as the gauge fixer's, eq. 8).  On a unitary matrix this
+ *     changes the last bits only, but it is needed: with 12-real link storage (row 2 rebuilt on every load) the
+ *     norm error of rows 0, 1 is fed back through the rebuilt row by the (0,2) and (1,2) updates and grows
+ *     exponentially -- 5e-13 after 25 sweeps, 7.5e-7 after 100, overflow before 300 on the CUDA side.      (R26)
  */
 #include <complex.h>
 #include <math.h>
@@ -192,6 +196,8 @@ void orc_hb_kp_sample(double a, unsigned long long seed, long n, double *X, int 
 /* ------------------------------------------------------------------------------------------ */
 /* the sweep                                                                                  */
 /* ------------------------------------------------------------------------------------------ */
+void orc_gs(const cplx *M, cplx *G);      /* lgf_oracle.c: Gram-Schmidt projection onto SU(3), pinned there */
+
 static void hb_update_link(cplx *U, const cplx *A, double beta, uint64_t seed, uint64_t link_idx)
 {
     static const int PAIR[3][2] = {{0, 1}, {0, 2}, {1, 2}};
@@ -221,6 +227,9 @@ static void hb_update_link(cplx *U, const cplx *A, double beta, uint64_t seed, u
             W[3 * j + col] = e_ji * wi + e_jj * wj;
         }
     }
+    cplx P[9];
+    orc_gs(U, P);                                            /* back onto SU(3) */
+    memcpy(U, P, sizeof(P));
 }
 
 /* nsweeps sweeps, numbered sweep0, sweep0 + 1, ... (the number selects the random stream, so a run may be

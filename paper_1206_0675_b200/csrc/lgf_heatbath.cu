@@ -10,6 +10,8 @@
 //   staples only contain links of other classes, so the update is done in place                      (R25)
 //   W = U A; for (i, j) = (0,1), (0,2), (1,2): quaternion r of the 2x2 block of W, kk = |r|,
 //   X ~ exp(a x0) sqrt(1 - x0^2), a = 2 beta kk / 3; alpha = X (r/kk)^dag; U <- E(alpha) U, W <- E(alpha) W  (R26)
+//   then U is re-projected onto SU(3) (Gram-Schmidt rows 0, 1; row 2 = (row0 x row1)^*): without it the norm
+//   error of rows 0, 1 grows exponentially over the sweeps in 12-real storage (overflow before 300 sweeps)  (R26)
 //   uniforms u_n = ((mix64(key + (idx+1) G) >> 11) + 0.5) 2^-53, idx = ((((class V + site) 3 + k) 32 + t) 6 + n) (R27)
 // The arithmetic is double precision whatever the storage precision of the links.
 #include "lgf_state.cuh"
@@ -177,6 +179,17 @@ __global__ void __launch_bounds__(HB_THREADS) k_heatbath(LinkPair<R> lp, Geom g,
             W[3 * i + col] = e_ii * wi + e_ij * wj;
             W[3 * j + col] = e_ji * wi + e_jj * wj;
         }
+    }
+    {   // back onto SU(3): a <- row0 / |row0|; b <- row1 - (a^dag . row1) a, normalised; row2 = (a x b)^*
+        const double ia = 1.0 / sqrt(norm2(U[0]) + norm2(U[1]) + norm2(U[2]));
+        U[0] = ia * U[0]; U[1] = ia * U[1]; U[2] = ia * U[2];
+        Z ab = mulc(U[3], U[0]);
+        ab = ab + mulc(U[4], U[1]);
+        ab = ab + mulc(U[5], U[2]);
+        U[3] = U[3] - ab * U[0]; U[4] = U[4] - ab * U[1]; U[5] = U[5] - ab * U[2];
+        const double ib = 1.0 / sqrt(norm2(U[3]) + norm2(U[4]) + norm2(U[5]));
+        U[3] = ib * U[3]; U[4] = ib * U[4]; U[5] = ib * U[5];
+        reconstruct_row2(U);
     }
     C<R> out[9];
 #pragma unroll

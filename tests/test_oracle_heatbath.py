@@ -73,6 +73,8 @@ def test_heatbath_keeps_links_in_su3_and_is_counter_based():
     dims = (4, 4, 4, 4)
     U0 = inputs.hot_config(dims, 5)
     U2 = oracle.heatbath(dims, U0, 5.7, 99, 0, 2)
+    U40 = oracle.heatbath(dims, U2, 5.7, 99, 2, 38)          # re-projected after every update (R26): no drift
+    assert np.max(np.abs(U40 @ _dag(U40) - np.eye(3))) < 5e-15
     assert np.max(np.abs(U2 @ _dag(U2) - np.eye(3))) < 1e-14
     assert np.max(np.abs(np.linalg.det(U2) - 1)) < 1e-14
     assert not np.allclose(U2, U0)
