@@ -159,7 +159,10 @@ int lgf_get_transform(lgf_ctx *ctx, void *d_transform);
  * "fft_zt_xc" (consecutive (x, y) indices per CTA of the (z, t) pass, 0 = automatic), "fft_reg2" (1 = two
  * threads per line where the lattice allows), "fuse_g" (1 = the last FFT sweep ends with the g-build),
  * "sweep_tz" (z-planes per (z, t) tile of the sweep's CTA order, 0 = automatic, 1 = plain order),
- * "sweep_tiled" (1 = tiled sweep variant), "sweep_tt" (its t-march length).
+ * "sweep_tiled" (1 = tiled sweep variant), "sweep_tt" (its t-march length), "reunit_every" (N > 0: in every
+ * N-th update the new links are projected back onto SU(3) inside the sweep; 0 = never, the method as the
+ * paper states it -- this key DOES change the result, by the rounding drift it removes; meant for fp32 runs
+ * of thousands of iterations).
  * Unknown key or NULL: LGF_EINVAL.  Synchronises. */
 int lgf_tune(lgf_ctx *ctx, const char *key, int value);
 /* Number of FFT kernel launches per iteration under the current plan (3 or up to 7). */

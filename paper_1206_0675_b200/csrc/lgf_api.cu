@@ -49,6 +49,8 @@ struct lgf_ctx {
     int tune_zt_xc = 0;          // lgf_tune: consecutive (x, y) indices per CTA of the (z, t) pass
     int tune_fuse_g = 1;         // lgf_tune: end the last FFT sweep with the g-build (register-line plan only)
     int tune_sweep_tiled = 0;    // lgf_tune: tiled sweep (shared-memory neighbour exchange, finalize folded in)
+    int tune_reunit = 0;         // lgf_tune "reunit_every": project the new links onto SU(3) in every N-th update (0 = never)
+    long long updates_enqueued = 0;   // host-side count of updates enqueued since the last set_links / thermalize
     int tune_sweep_tz = 0;       // lgf_tune: z-planes per (z, t) tile of the sweep's block order (0 = automatic, 1 = plain)
     int tune_sweep_tt = 0;       // lgf_tune: t-march length of the tiled sweep (0 = automatic)
     SweepTile tile{};
@@ -362,7 +364,9 @@ static int step_update(lgf_ctx *ctx, double alpha, double tol, int record, bool 
         Bracket br(ctx, LGF_K_GBUILD);
         CK(launch_gacc<R>(1, (const C<R> *)ctx->G, (C<R> *)ctx->Gacc, (R *)nullptr, ctx->g, ctx->st, ctx->stream));
     }
-    if (ctx->tune_sweep_tiled) {
+    ctx->updates_enqueued++;
+    const bool reunit = ctx->tune_reunit > 0 && ctx->updates_enqueued % ctx->tune_reunit == 0;
+    if (ctx->tune_sweep_tiled && !reunit) {
         Bracket br(ctx, LGF_K_UPDATE);
         CK(launch_sweep_tiled<R>(ctx->nr, link_pair<R>(ctx), (const C<R> *)ctx->G, (C<R> *)ctx->W, ctx->g, ctx->tile,
                                  ctx->partial, &ctx->nb_partial, ctx->st, tol, record, ctx->hist, ctx->hist_cap,
@@ -372,7 +376,7 @@ static int step_update(lgf_ctx *ctx, double alpha, double tol, int record, bool 
     {
         Bracket br(ctx, LGF_K_UPDATE);
         CK(launch_sweep<R>(ctx->nr, link_pair<R>(ctx), (const C<R> *)ctx->G, (C<R> *)ctx->W, ctx->g, ctx->partial,
-                           &ctx->nb_partial, ctx->st, ctx->stream, ctx->tune_sweep_tz));
+                           &ctx->nb_partial, ctx->st, ctx->stream, ctx->tune_sweep_tz, reunit));
     }
     return step_finalize(ctx, tol, 1, record);
 }
@@ -550,6 +554,7 @@ int lgf_set_links(lgf_ctx *ctx, const void *d_links) {
     ctx->w_is_delta = false;
     ctx->recorded = false;
     ctx->hb_sweeps = 0;
+    ctx->updates_enqueued = 0;
     return LGF_OK;
 }
 
@@ -842,6 +847,7 @@ int lgf_tune(lgf_ctx *ctx, const char *key, int value) {
     else if (k == "sweep_tiled") ctx->tune_sweep_tiled = value;
     else if (k == "fuse_g") ctx->tune_fuse_g = value;
     else if (k == "sweep_tz") ctx->tune_sweep_tz = value;
+    else if (k == "reunit_every") ctx->tune_reunit = value < 0 ? 0 : value;
     else if (k == "sweep_tt") { ctx->tune_sweep_tt = value; ctx->tile = choose_sweep_tile(ctx->g, value); }
     else return fail(ctx, LGF_EINVAL, "lgf_tune: unknown key " + k);
     CK(cudaStreamSynchronize(ctx->stream));

@@ -158,6 +158,24 @@ __device__ __forceinline__ long long block_base(const BlockOrder &bo, unsigned i
     return (long long)bxy + (long long)bo.nxy * ((ztile * bo.tz + zi) + (long long)bo.Lz * t);
 }
 
+// Opt-in (lgf_tune "reunit_every"): put a freshly transformed link back onto SU(3) -- Gram-Schmidt on rows 0, 1,
+// row 2 = (row0 x row1)^* (eq. 8).  The method as the paper states it never does this (R13), and in
+// fp64 it need not; in fp32 the links of a run of thousands of iterations drift far enough to move the
+// gauge-invariant plaquette in the fourth digit.  Done inside the sweep, on every copy of the new link it
+// computes, so Delta, F and theta stay those of the links that are stored and no extra pass is needed.
+template <class R>
+__device__ __forceinline__ void project_su3(C<R> (&u)[9]) {
+    const R ia = (R)1 / sqrt(norm2(u[0]) + norm2(u[1]) + norm2(u[2]));
+    u[0] = ia * u[0]; u[1] = ia * u[1]; u[2] = ia * u[2];
+    C<R> ab = mulc(u[3], u[0]);
+    ab = ab + mulc(u[4], u[1]);
+    ab = ab + mulc(u[5], u[2]);
+    u[3] = u[3] - ab * u[0]; u[4] = u[4] - ab * u[1]; u[5] = u[5] - ab * u[2];
+    const R ib = (R)1 / sqrt(norm2(u[3]) + norm2(u[4]) + norm2(u[5]));
+    u[3] = ib * u[3]; u[4] = ib * u[4]; u[5] = ib * u[5];
+    reconstruct_row2(u);
+}
+
 // ---- a6 + a1 fused --------------------------------------------------------------------------------
 // One thread per site x.  For every direction: the site's own new link U'_mu(x) = g(x) U_mu(x) g(x+mu)^dag
 // is computed, stored to the other link buffer and its algebra part subtracted from Delta(x); the new
@@ -165,7 +183,7 @@ __device__ __forceinline__ long long block_base(const BlockOrder &bo, unsigned i
 // are L1/L2 hits: the neighbouring thread reads the same lines) and its algebra part added.  Reads
 // buffer `cur`, writes buffer 1-cur (k_finalize flips `cur`), so no thread ever sees a half-updated
 // neighbourhood (Jacobi update, R10).
-template <class R, int NR, int MINB>
+template <class R, int NR, int MINB, bool REUNIT>
 __global__ void __launch_bounds__(SWEEP_THREADS, MINB)
     k_sweep(LinkPair<R> lp, const C<R> *__restrict__ G, C<R> *__restrict__ W, Geom g, double *__restrict__ partial,
             const DevState *__restrict__ st, BlockOrder bo) {
@@ -189,6 +207,7 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB)
             load_link<R, NR>(src, g.V, mu, s, u);
             load_g(G, g.V, site_fwd(g, s, c, mu), gn);
             transform_link<NR>(gx, u, gn, p);                       // Alg. 1 line 14, eq. 2
+            if constexpr (REUNIT) project_su3(p);
             store_link<R, NR>(dst, g.V, mu, s, p);
             retr += p[0].x + p[4].x + p[8].x;                       // eq. 3 on the new link
             herm_sub(d, algebra_part(p));                           // - A'_mu(x)
@@ -196,6 +215,7 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB)
             load_link<R, NR>(src, g.V, mu, sb, u);
             load_g(G, g.V, sb, gn);
             transform_link<NR>(gn, u, gx, p);
+            if constexpr (REUNIT) project_su3(p);                   // the same link the neighbour stores
             herm_add(d, algebra_part(p));                           // + A'_mu(x - mu)     (eq. 5)
         }
         store_herm(W, g.V, s, d);
@@ -512,7 +532,7 @@ cudaError_t launch_gbuild(const C<R> *W, C<R> *G, const Geom &g, R half_alpha, c
 }
 template <class R>
 cudaError_t launch_sweep(int nr, LinkPair<R> links, const C<R> *G, C<R> *W, const Geom &g, double *partial,
-                         int *nblocks, const DevState *st, cudaStream_t stream, int order_tz) {
+                         int *nblocks, const DevState *st, cudaStream_t stream, int order_tz, bool reunit) {
     const int nb = (int)((g.V + SWEEP_THREADS - 1) / SWEEP_THREADS);
     *nblocks = nb;
     // (z, t)-tiled block order when the (x, y) plane is a whole number of CTAs; TZ: about 24 MB of traffic
@@ -534,10 +554,13 @@ cudaError_t launch_sweep(int nr, LinkPair<R> links, const C<R> *G, C<R> *W, cons
     switch (g_sweep_minb) {
 #define LGF_SW(M)                                                                                     \
     case M:                                                                                           \
-        if (nr == 3) k_sweep<R, 3, M><<<nb, SWEEP_THREADS, 0, stream>>>(links, G, W, g, partial, st, bo); \
-        else k_sweep<R, 2, M><<<nb, SWEEP_THREADS, 0, stream>>>(links, G, W, g, partial, st, bo);         \
+        if (reunit) {                                                                                     \
+            if (nr == 3) k_sweep<R, 3, M, true><<<nb, SWEEP_THREADS, 0, stream>>>(links, G, W, g, partial, st, bo); \
+            else k_sweep<R, 2, M, true><<<nb, SWEEP_THREADS, 0, stream>>>(links, G, W, g, partial, st, bo);         \
+        } else if (nr == 3) k_sweep<R, 3, M, false><<<nb, SWEEP_THREADS, 0, stream>>>(links, G, W, g, partial, st, bo); \
+        else k_sweep<R, 2, M, false><<<nb, SWEEP_THREADS, 0, stream>>>(links, G, W, g, partial, st, bo);         \
         break;
-        LGF_SW(2) LGF_SW(3) LGF_SW(4) LGF_SW(5)
+        LGF_SW(2) LGF_SW(3) LGF_SW(4)
 #undef LGF_SW
         default: return cudaErrorInvalidValue;
     }
@@ -671,7 +694,7 @@ cudaError_t launch_clear_done(DevState *st, cudaStream_t stream) {
                                          const DevState *, cudaStream_t);                                             \
     template cudaError_t launch_gbuild<R>(const C<R> *, C<R> *, const Geom &, R, const DevState *, cudaStream_t);     \
     template cudaError_t launch_sweep<R>(int, LinkPair<R>, const C<R> *, C<R> *, const Geom &, double *, int *,       \
-                                         const DevState *, cudaStream_t, int);                                             \
+                                         const DevState *, cudaStream_t, int, bool);                                             \
     template cudaError_t launch_sweep_tiled<R>(int, LinkPair<R>, const C<R> *, C<R> *, const Geom &, const SweepTile &, \
                                                double *, int *, DevState *, double, int, double *, long long,         \
                                                cudaStream_t);                                                         \

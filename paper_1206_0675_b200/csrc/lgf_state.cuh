@@ -93,7 +93,8 @@ template <class R>
 cudaError_t launch_gbuild(const C<R> *W, C<R> *G, const Geom &g, R half_alpha, const DevState *st, cudaStream_t stream);
 template <class R>
 cudaError_t launch_sweep(int nr, LinkPair<R> links, const C<R> *G, C<R> *W, const Geom &g, double *partial,
-                         int *nblocks, const DevState *st, cudaStream_t stream, int order_tz /* 0 auto, 1 plain */);
+                         int *nblocks, const DevState *st, cudaStream_t stream, int order_tz /* 0 auto, 1 plain */,
+                         bool reunit /* project every new link onto SU(3) */);
 // tiled sweep with the finalize folded in (last CTA): record / tol / hist as for launch_finalize
 template <class R>
 cudaError_t launch_sweep_tiled(int nr, LinkPair<R> links, const C<R> *G, C<R> *W, const Geom &g, const SweepTile &tl,

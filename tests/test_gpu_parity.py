@@ -419,6 +419,48 @@ def test_accumulated_transformation(lgf, dims, prec, storage):
         ctx.track_transform(False)
 
 
+@pytest.mark.parametrize("storage", [18, 12])
+def test_reunit_every_update_keeps_fp64_parity(lgf, config_cache, storage):
+    """lgf_tune("reunit_every", 1): every new link is projected onto SU(3) inside the sweep -- on the stored copy
+    and on the copy recomputed for the backward neighbour alike.  In fp64 the projection moves the last bits
+    only, so the 20-iteration parity bar against the (never projecting) oracle must still hold; it would not
+    if Delta were computed from differently projected copies."""
+    dims = inputs.CONFIGS["C2"]["dims"]
+    U = config_cache("C2")
+    U_o, F_o, T_o = oracle.iterate(dims, U, ALPHA, 20)
+    Fh, Th, P, out = run_trajectory(lgf, dims, U, 8, storage, 20, tune={"reunit_every": 1})
+    assert np.max(np.abs(Fh - F_o) / np.abs(F_o)) < 1e-12
+    assert np.max(np.abs(Th - T_o) / np.abs(T_o)) < 1e-12
+    assert np.max(np.abs(out - U_o)) < 1e-11
+    assert np.max(np.abs(out @ np.conj(np.swapaxes(out, -1, -2)) - np.eye(3))) < 2e-15      # tighter than R13's drift
+
+
+@pytest.mark.parametrize("storage", [18, 12])
+def test_reunit_holds_fp32_links_on_su3(lgf, storage):
+    """fp32, 1500 updates of a rough (hot-start) 8^4 configuration: without projection the links drift and
+    take the gauge-invariant plaquette with them; with reunit_every = 10 both stay at float rounding."""
+    import torch
+
+    dims = (8, 8, 8, 8)
+    U = inputs.hot_config(dims, 4711)
+    P0 = oracle.plaquette(dims, U.astype(np.complex64).astype(np.complex128))
+    res = {}
+    for every in (0, 10):
+        with lgf.Context(dims, 4, storage) as ctx:
+            ctx.tune("reunit_every", every)
+            d = to_dev(U, 4)
+            ctx.set_links(d)
+            ctx.iterate(ALPHA, 1500)
+            _, th, P = ctx.measure()
+            out = to_np(ctx.get_links(torch.empty_like(d)))
+        res[every] = (abs(P - P0), np.max(np.abs(out @ np.conj(np.swapaxes(out, -1, -2)) - np.eye(3))), th)
+    assert res[10][1] < 2e-6 and res[10][0] < 5e-6
+    assert res[0][1] > 5 * res[10][1]                # the drift the projection removes is real
+    # the projection does not disturb the iteration: same theta as the unprojected run to within a factor 2
+    # (a hot start converges slowly: theta ~ 1e-5 after 1500 updates, down from 3.6)
+    assert res[10][2] < 1e-3 and 0.5 < res[10][2] / res[0][2] < 2.0
+
+
 def test_12_real_matches_18_real(lgf, config_cache):
     """Third-row reconstruction (eq. 8) changes rounding only."""
     dims = inputs.CONFIGS["C1"]["dims"]
