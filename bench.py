@@ -306,6 +306,61 @@ def run_reference(args):
     return 0
 
 
+def run_thermal(args):
+    """--thermal BETA: the paper's kind of input.  Thermalise a cold 32^4 lattice with
+    lgf_thermalize (heat bath, Wilson action) and gauge-fix it with lgf_fix: iterations and seconds to
+    theta < 1e-15 (fp64) / 1e-12 (fp32), to set beside the paper's Table 3.  Prints one JSON
+    line of its own; not the contract line."""
+    import torch
+
+    from paper_1206_0675_b200 import binding
+
+    torch.cuda.set_device(0)
+    binding.load()
+    dims, prec = (32, 32, 32, 32), PREC[args.precision]
+    cdt = torch.complex128 if prec == 8 else torch.complex64
+    stream = torch.cuda.current_stream()
+    with binding.Context(dims, prec, args.storage, stream=stream) as ctx:
+        ctx.tune("reunit_every", args.reunit_every)
+        cold = torch.zeros((32, 32, 32, 32, 4, 3, 3), dtype=cdt, device="cuda")
+        for i in range(3):
+            cold[..., i, i] = 1
+        ctx.set_links(cold)
+        ctx.thermalize(args.thermal, 5, args.thermal_seed)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        ctx.thermalize(args.thermal, args.thermal_sweeps - 5, args.thermal_seed)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        ms_sweep = e0.elapsed_time(e1) / (args.thermal_sweeps - 5)
+        _, theta0, P0 = ctx.measure()
+        links = ctx.get_links(torch.empty_like(cold))
+        dev0 = float((links @ links.conj().transpose(-1, -2) - torch.eye(3, dtype=cdt, device="cuda")).abs().max())
+        tol = 1e-15 if prec == 8 else 1e-12
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        it = ctx.fix(links, ALPHA, tol, 200000)
+        torch.cuda.synchronize()
+        sec = time.perf_counter() - t0
+        F, theta, P1 = ctx.measure()
+        Fh, _ = ctx.history()
+        hb_bytes = ctx.algorithmic_bytes(binding.LGF_K_HEATBATH)
+    peak, _ = measured_peak()
+    print(json.dumps({
+        "mode": "thermal", "beta": args.thermal, "lattice": "32x32x32x32", "precision": args.precision,
+        "link_storage": args.storage, "reunit_every": args.reunit_every, "heatbath_sweeps": args.thermal_sweeps,
+        "seed": args.thermal_seed, "heatbath_ms_per_sweep": ms_sweep,
+        "heatbath_algorithmic_gbs": hb_bytes / (ms_sweep * 1e-3) / 1e9, "heatbath_frac_of_peak": hb_bytes / (ms_sweep * 1e-3) / 1e9 / peak,
+        "plaquette_thermalised": P0, "su3_deviation_thermalised": dev0, "theta_before": theta0,
+        "iterations_to_tol": it, "tol": tol, "seconds_to_fix": sec, "ms_per_iteration": 1e3 * sec / max(it, 1),
+        "F_final": F, "theta_final": theta, "plaquette_after_fix": P1, "plaquette_drift": abs(P1 - P0),
+        "F_min_step": float(np.min(np.diff(Fh))) if len(Fh) > 1 else None,
+        "paper_table3": "32^4 dp, C2070: 765-10427 iterations, 61.1 ms/iteration (12-real tex) -- other hardware, context"}),
+        flush=True)
+    return 0
+
+
 def workload_name(key, dims):
     from paper_1206_0675_b200 import inputs
 
@@ -328,10 +383,17 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--cpu-budget", type=float, default=20.0)
     ap.add_argument("--reference-budget", type=float, default=240.0)
+    ap.add_argument("--thermal", type=float, default=None, metavar="BETA",
+                    help="thermalise a cold 32^4 lattice at BETA and gauge-fix it (own JSON line, not the contract line)")
+    ap.add_argument("--thermal-sweeps", type=int, default=300)
+    ap.add_argument("--thermal-seed", type=int, default=1234)
+    ap.add_argument("--reunit-every", type=int, default=0)
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)
     if args.impl == "reference":
         return run_reference(args)
+    if args.thermal is not None:
+        return run_thermal(args)
 
     import torch
 
