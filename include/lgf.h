@@ -153,13 +153,14 @@ int lgf_get_transform(lgf_ctx *ctx, void *d_transform);
 
 /* ---- tuning --------------------------------------------------------------------------------------- */
 
-/* Override a planner choice (takes effect from the next iteration; results are unchanged up to
- * rounding).  Keys: "fft_two_axis" (1 = use the three-sweep two-axis FFT passes when the lattice
+/* Override a planner choice of THIS context (takes effect from the next iteration; results are unchanged up
+ * to rounding, except for "reunit_every").  Keys: "fft_two_axis" (1 = use the three-sweep two-axis FFT passes when the lattice
  * allows, 0 = one pass per axis), "fft_reg" (1 = use the register-line sweeps when the lattice allows), "fft_xy_planes" ((x, y) planes per CTA, 0 = automatic),
  * "fft_zt_xc" (consecutive (x, y) indices per CTA of the (z, t) pass, 0 = automatic), "fft_reg2" (1 = two
  * threads per line where the lattice allows), "fuse_g" (1 = the last FFT sweep ends with the g-build),
  * "sweep_tz" (z-planes per (z, t) tile of the sweep's CTA order, 0 = automatic, 1 = plain order),
- * "sweep_tiled" (1 = tiled sweep variant), "sweep_tt" (its t-march length), "reunit_every" (N > 0: in every
+ * "sweep_tiled" (1 = tiled sweep variant), "sweep_tt" (its t-march length), "sweep_minb" (2, 3 or 4: resident
+ * CTAs per SM the sweep's register allocation is asked to allow), "reunit_every" (N > 0: in every
  * N-th update the new links are projected back onto SU(3) inside the sweep; 0 = never, the method as the
  * paper states it -- this key DOES change the result, by the rounding drift it removes; meant for fp32 runs
  * of thousands of iterations).

@@ -12,7 +12,6 @@
 #include "lgf_state.cuh"
 
 using namespace lgf;
-namespace lgf { extern int g_sweep_minb; }
 
 struct lgf_ctx {
     Geom g{};
@@ -49,6 +48,7 @@ struct lgf_ctx {
     int tune_zt_xc = 0;          // lgf_tune: consecutive (x, y) indices per CTA of the (z, t) pass
     int tune_fuse_g = 1;         // lgf_tune: end the last FFT sweep with the g-build (register-line plan only)
     int tune_sweep_tiled = 0;    // lgf_tune: tiled sweep (shared-memory neighbour exchange, finalize folded in)
+    int tune_sweep_minb = 3;     // lgf_tune: resident CTAs per SM the sweep's register allocation is asked to allow
     int tune_reunit = 0;         // lgf_tune "reunit_every": project the new links onto SU(3) in every N-th update (0 = never)
     long long updates_enqueued = 0;   // host-side count of updates enqueued since the last set_links / thermalize
     int tune_sweep_tz = 0;       // lgf_tune: z-planes per (z, t) tile of the sweep's block order (0 = automatic, 1 = plain)
@@ -370,13 +370,13 @@ static int step_update(lgf_ctx *ctx, double alpha, double tol, int record, bool 
         Bracket br(ctx, LGF_K_UPDATE);
         CK(launch_sweep_tiled<R>(ctx->nr, link_pair<R>(ctx), (const C<R> *)ctx->G, (C<R> *)ctx->W, ctx->g, ctx->tile,
                                  ctx->partial, &ctx->nb_partial, ctx->st, tol, record, ctx->hist, ctx->hist_cap,
-                                 ctx->stream));
+                                 ctx->stream, ctx->tune_sweep_minb));
         return LGF_OK;
     }
     {
         Bracket br(ctx, LGF_K_UPDATE);
         CK(launch_sweep<R>(ctx->nr, link_pair<R>(ctx), (const C<R> *)ctx->G, (C<R> *)ctx->W, ctx->g, ctx->partial,
-                           &ctx->nb_partial, ctx->st, ctx->stream, ctx->tune_sweep_tz, reunit));
+                           &ctx->nb_partial, ctx->st, ctx->stream, ctx->tune_sweep_tz, reunit, ctx->tune_sweep_minb));
     }
     return step_finalize(ctx, tol, 1, record);
 }
@@ -843,7 +843,10 @@ int lgf_tune(lgf_ctx *ctx, const char *key, int value) {
     else if (k == "fft_reg2") ctx->tune_reg2 = value;
     else if (k == "fft_xy_planes") ctx->tune_xy_planes = value;
     else if (k == "fft_zt_xc") ctx->tune_zt_xc = value;
-    else if (k == "sweep_minb") lgf::g_sweep_minb = value;
+    else if (k == "sweep_minb") {
+        if (value < 2 || value > 4) return fail(ctx, LGF_EINVAL, "lgf_tune: sweep_minb must be 2, 3 or 4");
+        ctx->tune_sweep_minb = value;
+    }
     else if (k == "sweep_tiled") ctx->tune_sweep_tiled = value;
     else if (k == "fuse_g") ctx->tune_fuse_g = value;
     else if (k == "sweep_tz") ctx->tune_sweep_tz = value;

@@ -14,7 +14,6 @@ namespace lgf {
 
 constexpr int SITE_THREADS = 256;
 constexpr int SWEEP_THREADS = 128;
-int g_sweep_minb = 3;   // experiment knob
 
 // ---- a1 -------------------------------------------------------------------------------------------
 template <class R, int NR>
@@ -532,7 +531,7 @@ cudaError_t launch_gbuild(const C<R> *W, C<R> *G, const Geom &g, R half_alpha, c
 }
 template <class R>
 cudaError_t launch_sweep(int nr, LinkPair<R> links, const C<R> *G, C<R> *W, const Geom &g, double *partial,
-                         int *nblocks, const DevState *st, cudaStream_t stream, int order_tz, bool reunit) {
+                         int *nblocks, const DevState *st, cudaStream_t stream, int order_tz, bool reunit, int minb) {
     const int nb = (int)((g.V + SWEEP_THREADS - 1) / SWEEP_THREADS);
     *nblocks = nb;
     // (z, t)-tiled block order when the (x, y) plane is a whole number of CTAs; TZ: about 24 MB of traffic
@@ -551,7 +550,7 @@ cudaError_t launch_sweep(int nr, LinkPair<R> links, const C<R> *G, C<R> *W, cons
         }
         if (tz > 1 && g.L[2] % tz == 0) { bo.nxy = (int)(plane / SWEEP_THREADS); bo.tz = tz; }
     }
-    switch (g_sweep_minb) {
+    switch (minb) {
 #define LGF_SW(M)                                                                                     \
     case M:                                                                                           \
         if (reunit) {                                                                                     \
@@ -603,12 +602,12 @@ SweepTile choose_sweep_tile(const Geom &g, int tt_override) {
 template <class R>
 cudaError_t launch_sweep_tiled(int nr, LinkPair<R> links, const C<R> *G, C<R> *W, const Geom &g, const SweepTile &tl,
                                double *partial, int *nblocks, DevState *st, double tol, int record, double *hist,
-                               long long hist_cap, cudaStream_t stream) {
+                               long long hist_cap, cudaStream_t stream, int minb) {
     const int nb = tl.nt[0] * tl.nt[1] * tl.nt[2] * tl.nt[3];
     *nblocks = nb;
     const int threads = (tl.threads + 31) / 32 * 32;
     const size_t smem = sizeof(R) * 2 * 32 * (size_t)tl.threads;
-    switch (g_sweep_minb) {
+    switch (minb) {
 #define LGF_SW(M)                                                                                              \
     case M: {                                                                                                  \
         auto k3 = k_sweep_tiled<R, 3, M>;                                                                      \
@@ -694,10 +693,10 @@ cudaError_t launch_clear_done(DevState *st, cudaStream_t stream) {
                                          const DevState *, cudaStream_t);                                             \
     template cudaError_t launch_gbuild<R>(const C<R> *, C<R> *, const Geom &, R, const DevState *, cudaStream_t);     \
     template cudaError_t launch_sweep<R>(int, LinkPair<R>, const C<R> *, C<R> *, const Geom &, double *, int *,       \
-                                         const DevState *, cudaStream_t, int, bool);                                             \
+                                         const DevState *, cudaStream_t, int, bool, int);                                             \
     template cudaError_t launch_sweep_tiled<R>(int, LinkPair<R>, const C<R> *, C<R> *, const Geom &, const SweepTile &, \
                                                double *, int *, DevState *, double, int, double *, long long,         \
-                                               cudaStream_t);                                                         \
+                                               cudaStream_t, int);                                                         \
     template cudaError_t launch_plaquette<R>(int, LinkPair<R>, const Geom &, double *, int *, const DevState *,       \
                                              cudaStream_t);                                                           \
     template cudaError_t launch_convert_in<R>(int, const R *, C<R> *, const Geom &, cudaStream_t);                    \

@@ -94,12 +94,13 @@ cudaError_t launch_gbuild(const C<R> *W, C<R> *G, const Geom &g, R half_alpha, c
 template <class R>
 cudaError_t launch_sweep(int nr, LinkPair<R> links, const C<R> *G, C<R> *W, const Geom &g, double *partial,
                          int *nblocks, const DevState *st, cudaStream_t stream, int order_tz /* 0 auto, 1 plain */,
-                         bool reunit /* project every new link onto SU(3) */);
+                         bool reunit /* project every new link onto SU(3) */, int minb /* CTAs per SM asked of the
+                         register allocation: 2, 3 or 4 */);
 // tiled sweep with the finalize folded in (last CTA): record / tol / hist as for launch_finalize
 template <class R>
 cudaError_t launch_sweep_tiled(int nr, LinkPair<R> links, const C<R> *G, C<R> *W, const Geom &g, const SweepTile &tl,
                                double *partial, int *nblocks, DevState *st, double tol, int record, double *hist,
-                               long long hist_cap, cudaStream_t stream);
+                               long long hist_cap, cudaStream_t stream, int minb);
 template <class R>
 cudaError_t launch_plaquette(int nr, LinkPair<R> links, const Geom &g, double *partial, int *nblocks,
                              const DevState *st, cudaStream_t stream);
