@@ -340,7 +340,7 @@ def run_thermal(args):
         tol = 1e-15 if prec == 8 else 1e-12
         torch.cuda.synchronize()
         t0 = time.perf_counter()
-        it = ctx.fix(links, ALPHA, tol, 200000)
+        it = ctx.fix(links, args.alpha, tol, args.thermal_max_iter)
         torch.cuda.synchronize()
         sec = time.perf_counter() - t0
         F, theta, P1 = ctx.measure()
@@ -349,7 +349,8 @@ def run_thermal(args):
     peak, _ = measured_peak()
     print(json.dumps({
         "mode": "thermal", "beta": args.thermal, "lattice": "32x32x32x32", "precision": args.precision,
-        "link_storage": args.storage, "reunit_every": args.reunit_every, "heatbath_sweeps": args.thermal_sweeps,
+        "link_storage": args.storage, "alpha": args.alpha, "reunit_every": args.reunit_every,
+        "heatbath_sweeps": args.thermal_sweeps,
         "seed": args.thermal_seed, "heatbath_ms_per_sweep": ms_sweep,
         "heatbath_algorithmic_gbs": hb_bytes / (ms_sweep * 1e-3) / 1e9, "heatbath_frac_of_peak": hb_bytes / (ms_sweep * 1e-3) / 1e9 / peak,
         "plaquette_thermalised": P0, "su3_deviation_thermalised": dev0, "theta_before": theta0,
@@ -388,6 +389,8 @@ def main():
     ap.add_argument("--thermal-sweeps", type=int, default=300)
     ap.add_argument("--thermal-seed", type=int, default=1234)
     ap.add_argument("--reunit-every", type=int, default=0)
+    ap.add_argument("--alpha", type=float, default=ALPHA, help="step size of the --thermal fix (the paper uses 0.08)")
+    ap.add_argument("--thermal-max-iter", type=int, default=200000)
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)
     if args.impl == "reference":
