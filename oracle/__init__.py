@@ -214,3 +214,15 @@ def heatbath(dims, U, beta: float, seed: int, sweep0: int, nsweeps: int):
     if rc != 0:
         raise ValueError("heatbath needs even lattice extents")
     return U
+
+
+def overrelax(dims, U, nsweeps: int):
+    """nsweeps microcanonical overrelaxation sweeps (R28): the action is conserved.  Returns the new configuration."""
+    dims, cd = _dims(dims)
+    U = _c128(U, _site_shape(dims) + (4, 3, 3)).copy()
+    lib = _load()
+    lib.orc_overrelax.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_long]
+    lib.orc_overrelax.restype = ctypes.c_int
+    if lib.orc_overrelax(cd, _ptr(U), int(nsweeps)) != 0:
+        raise ValueError("overrelax needs even lattice extents")
+    return U

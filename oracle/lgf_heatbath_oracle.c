@@ -38,6 +38,9 @@
  *     strong-coupling pin P = beta/18 fails by 30 %), Creutz alone not at large a_kp.  With the switch at 2 the
  *     rejection probability per attempt stays below 0.5; after HB_MAXATT = 32 rejections (< 1e-9) the last
  *     delta, clipped to [0, 2], is used.
+ *   overrelaxation sweep (microcanonical, no random numbers): same class order and subgroups, with
+ *     alpha = (V^dag)^2 instead of the heat-bath draw: alpha V = V^dag has the same x0 as V, so Re tr[U A] -- and
+ *     with it the action -- is unchanged by every single step; then the same re-projection.            (R28)
  *   uniforms: u_n = ((mix64(key + (idx + 1) G) >> 11) + 0.5) 2^-53, key = mix64(seed ^ G), G = 0x9E3779B97F4A7C15,
  *     mix64 = the splitmix64 finaliser, idx = (((((sweep 8 + mu 2 + parity) V + site) 3 + k) 32 + t) 6 + n).   (R27)
  *   After its three subgroup updates the link is re-projected onto SU(3): Gram-Schmidt on rows 0, 1, row 2 =
@@ -198,7 +201,8 @@ void orc_hb_kp_sample(double a, unsigned long long seed, long n, double *X, int 
 /* ------------------------------------------------------------------------------------------ */
 void orc_gs(const cplx *M, cplx *G);      /* lgf_oracle.c: Gram-Schmidt projection onto SU(3), pinned there */
 
-static void hb_update_link(cplx *U, const cplx *A, double beta, uint64_t seed, uint64_t link_idx)
+/* overrelax != 0: alpha = (V^dag)^2 (R28), beta / seed / link_idx unused */
+static void hb_update_link(cplx *U, const cplx *A, double beta, uint64_t seed, uint64_t link_idx, int overrelax)
 {
     static const int PAIR[3][2] = {{0, 1}, {0, 2}, {1, 2}};
     cplx W[9];
@@ -209,10 +213,11 @@ static void hb_update_link(cplx *U, const cplx *A, double beta, uint64_t seed, u
         const double r0 = 0.5 * creal(a + d), r1 = 0.5 * cimag(b + c), r2 = 0.5 * creal(b - c), r3 = 0.5 * cimag(a - d);
         const double kk = sqrt(r0 * r0 + r1 * r1 + r2 * r2 + r3 * r3);
         if (!(kk > 1e-300)) continue;                       /* degenerate staple: leave this subgroup alone */
-        double x[4];
-        hb_kp(2.0 * beta * kk / 3.0, seed, ((link_idx * 3 + (uint64_t)k) * HB_MAXATT) * 6, x);
         /* alpha = X V^dag, V^dag = (r0, -r) / kk; quaternion product (p0, p)(q0, q) = (p0 q0 - p.q, p0 q + q0 p - p x q) */
         const double q0 = r0 / kk, q1 = -r1 / kk, q2 = -r2 / kk, q3 = -r3 / kk;
+        double x[4];
+        if (overrelax) { x[0] = q0; x[1] = q1; x[2] = q2; x[3] = q3; }      /* X = V^dag: alpha = V^dag V^dag */
+        else hb_kp(2.0 * beta * kk / 3.0, seed, ((link_idx * 3 + (uint64_t)k) * HB_MAXATT) * 6, x);
         const double al0 = x[0] * q0 - (x[1] * q1 + x[2] * q2 + x[3] * q3);
         const double al1 = x[0] * q1 + q0 * x[1] - (x[2] * q3 - x[3] * q2);
         const double al2 = x[0] * q2 + q0 * x[2] - (x[3] * q1 - x[1] * q3);
@@ -250,7 +255,29 @@ int orc_heatbath(const int L[4], cplx *U, double beta, unsigned long long seed, 
                     cplx A[9];
                     hb_staple(L, U, s, mu, A);
                     const uint64_t link_idx = ((uint64_t)sw * 8 + (uint64_t)(mu * 2 + parity)) * (uint64_t)V + (uint64_t)s;
-                    hb_update_link(U + (s * 4 + mu) * 9, A, beta, (uint64_t)seed, link_idx);
+                    hb_update_link(U + (s * 4 + mu) * 9, A, beta, (uint64_t)seed, link_idx, 0);
+                }
+            }
+    return 0;
+}
+
+/* nsweeps overrelaxation sweeps (R28).  Returns 0, or -1 if an extent is odd. */
+int orc_overrelax(const int L[4], cplx *U, long nsweeps)
+{
+    for (int mu = 0; mu < 4; mu++)
+        if (L[mu] % 2) return -1;
+    const long V = hb_volume(L);
+    for (long sw = 0; sw < nsweeps; sw++)
+        for (int mu = 0; mu < 4; mu++)
+            for (int parity = 0; parity < 2; parity++) {
+#pragma omp parallel for schedule(static)
+                for (long s = 0; s < V; s++) {
+                    int c[4];
+                    hb_coords(L, s, c);
+                    if (((c[0] + c[1] + c[2] + c[3]) & 1) != parity) continue;
+                    cplx A[9];
+                    hb_staple(L, U, s, mu, A);
+                    hb_update_link(U + (s * 4 + mu) * 9, A, 0.0, 0, 0, 1);
                 }
             }
     return 0;

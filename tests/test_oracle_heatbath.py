@@ -108,3 +108,31 @@ def test_weak_coupling_limit():
     cold = np.broadcast_to(np.eye(3, dtype=np.complex128), (4, 4, 4, 4, 4, 3, 3)).copy()
     P, err = _mean_plaquette(dims, cold, beta, 23, 40, 60)
     assert abs((1.0 - P) * beta / 2.0 - 1.0) < 0.06          # finite-volume zero modes and O(1/beta) terms: a few per cent
+
+
+def test_overrelaxation_conserves_the_action_and_moves_the_links():
+    """R28: every overrelaxation step leaves Re tr[U A] unchanged, so the plaquette is conserved to rounding by
+    whole sweeps -- on a rough configuration, where the links move by O(1)."""
+    dims = (4, 6, 4, 4)
+    U0 = oracle.heatbath(dims, inputs.hot_config(dims, 8), 5.7, 3, 0, 3)
+    P0 = oracle.plaquette(dims, U0)
+    U1 = oracle.overrelax(dims, U0, 1)
+    U3 = oracle.overrelax(dims, U1, 2)
+    assert abs(oracle.plaquette(dims, U1) - P0) < 1e-14 and abs(oracle.plaquette(dims, U3) - P0) < 1e-14
+    assert np.mean(np.abs(U1 - U0)) > 0.1                      # not a small move
+    assert np.max(np.abs(U3 @ _dag(U3) - np.eye(3))) < 5e-15
+    assert np.array_equal(oracle.overrelax(dims, U0, 3), U3)   # deterministic, no random numbers
+    with pytest.raises(ValueError):
+        oracle.overrelax((4, 4, 3, 4), inputs.hot_config((4, 4, 3, 4), 5), 1)
+
+
+def test_heatbath_with_overrelaxation_keeps_the_equilibrium():
+    """Mixing in microcanonical sweeps must not move the equilibrium: same weak-coupling limit 1 - P = 2/beta."""
+    dims, beta = (4, 4, 4, 4), 80.0
+    U = np.broadcast_to(np.eye(3, dtype=np.complex128), (4, 4, 4, 4, 4, 3, 3)).copy()
+    vals = []
+    for k in range(70):
+        U = oracle.overrelax(dims, oracle.heatbath(dims, U, beta, 31, k, 1), 2)
+        if k >= 25:
+            vals.append(oracle.plaquette(dims, U))
+    assert abs((1.0 - np.mean(vals)) * beta / 2.0 - 1.0) < 0.06
