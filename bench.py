@@ -326,14 +326,20 @@ def run_thermal(args):
         for i in range(3):
             cold[..., i, i] = 1
         ctx.set_links(cold)
-        ctx.thermalize(args.thermal, 5, args.thermal_seed)
+        def cycles(n):                                   # one heat-bath sweep + K overrelaxation sweeps each
+            for _ in range(n):
+                ctx.thermalize(args.thermal, 1, args.thermal_seed)
+                if args.thermal_overrelax > 0:
+                    ctx.overrelax(args.thermal_overrelax)
+
+        cycles(5)
         torch.cuda.synchronize()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record(stream)
-        ctx.thermalize(args.thermal, args.thermal_sweeps - 5, args.thermal_seed)
+        cycles(args.thermal_sweeps - 5)
         e1.record(stream)
         torch.cuda.synchronize()
-        ms_sweep = e0.elapsed_time(e1) / (args.thermal_sweeps - 5)
+        ms_sweep = e0.elapsed_time(e1) / ((args.thermal_sweeps - 5) * (1 + args.thermal_overrelax))
         _, theta0, P0 = ctx.measure()
         links = ctx.get_links(torch.empty_like(cold))
         dev0 = float((links @ links.conj().transpose(-1, -2) - torch.eye(3, dtype=cdt, device="cuda")).abs().max())
@@ -350,7 +356,7 @@ def run_thermal(args):
     print(json.dumps({
         "mode": "thermal", "beta": args.thermal, "lattice": "32x32x32x32", "precision": args.precision,
         "link_storage": args.storage, "alpha": args.alpha, "reunit_every": args.reunit_every,
-        "heatbath_sweeps": args.thermal_sweeps,
+        "heatbath_sweeps": args.thermal_sweeps, "overrelax_per_heatbath": args.thermal_overrelax,
         "seed": args.thermal_seed, "heatbath_ms_per_sweep": ms_sweep,
         "heatbath_algorithmic_gbs": hb_bytes / (ms_sweep * 1e-3) / 1e9, "heatbath_frac_of_peak": hb_bytes / (ms_sweep * 1e-3) / 1e9 / peak,
         "plaquette_thermalised": P0, "su3_deviation_thermalised": dev0, "theta_before": theta0,
@@ -388,6 +394,7 @@ def main():
                     help="thermalise a cold 32^4 lattice at BETA and gauge-fix it (own JSON line, not the contract line)")
     ap.add_argument("--thermal-sweeps", type=int, default=300)
     ap.add_argument("--thermal-seed", type=int, default=1234)
+    ap.add_argument("--thermal-overrelax", type=int, default=0, help="overrelaxation sweeps after each heat-bath sweep")
     ap.add_argument("--reunit-every", type=int, default=0)
     ap.add_argument("--alpha", type=float, default=ALPHA, help="step size of the --thermal fix (the paper uses 0.08)")
     ap.add_argument("--thermal-max-iter", type=int, default=200000)

@@ -136,6 +136,11 @@ int lgf_set_field(lgf_ctx *ctx, const void *d_field);
  * extents must be even (LGF_EINVAL otherwise).  Resets the history, the iteration counter and the
  * accumulated transformation, as loading a new configuration would.  Asynchronous. */
 int lgf_thermalize(lgf_ctx *ctx, double beta, int nsweeps, unsigned long long seed);
+/* nsweeps microcanonical overrelaxation sweeps (same order and subgroups, alpha = (V^dag)^2 instead of the
+ * heat-bath draw, R28): every step leaves the action unchanged, no random numbers are used, so the
+ * plaquette is conserved to rounding while the links move by O(1) -- interleaved with lgf_thermalize it
+ * shortens the autocorrelation of the ensemble.  Same state reset and error behaviour as lgf_thermalize. */
+int lgf_overrelax(lgf_ctx *ctx, int nsweeps);
 
 /* ---- accumulated gauge transformation ----------------------------- */
 

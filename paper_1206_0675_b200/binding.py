@@ -51,6 +51,7 @@ SIGNATURES = {
     "lgf_get_field": (_i, [_vp, _vp]),
     "lgf_set_field": (_i, [_vp, _vp]),
     "lgf_thermalize": (_i, [_vp, _d, _i, ctypes.c_ulonglong]),
+    "lgf_overrelax": (_i, [_vp, _i]),
     "lgf_track_transform": (_i, [_vp, _i]),
     "lgf_get_transform": (_i, [_vp, _vp]),
     "lgf_tune": (_i, [_vp, ctypes.c_char_p, _i]),
@@ -239,6 +240,9 @@ class Context:
     # -- thermalisation --------------------------------------------------------------------------
     def thermalize(self, beta, nsweeps, seed):
         _check(self._h, load().lgf_thermalize(self._h, float(beta), int(nsweeps), int(seed)))
+
+    def overrelax(self, nsweeps):
+        _check(self._h, load().lgf_overrelax(self._h, int(nsweeps)))
 
     # -- accumulated gauge transformation ----------------------------------------------------------
     def track_transform(self, on=True):

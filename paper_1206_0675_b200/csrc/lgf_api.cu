@@ -775,28 +775,30 @@ int lgf_set_field(lgf_ctx *ctx, const void *d_field) {
     return LGF_OK;
 }
 
-int lgf_thermalize(lgf_ctx *ctx, double beta, int nsweeps, unsigned long long seed) {
-    if (!ctx || nsweeps < 0 || !(beta > 0.0)) return fail(ctx, LGF_EINVAL, "lgf_thermalize: bad argument");
-    if (!ctx->have_links) return fail(ctx, LGF_ESTATE, "lgf_thermalize: no configuration loaded");
+// heat-bath (overrelax = false) or overrelaxation sweeps of the internal configuration
+static int monte_carlo_sweeps(lgf_ctx *ctx, double beta, int nsweeps, unsigned long long seed, bool overrelax) {
     for (int mu = 0; mu < 4; mu++)
-        if (ctx->g.L[mu] % 2) return fail(ctx, LGF_EINVAL, "lgf_thermalize: the checkerboard needs even extents");
+        if (ctx->g.L[mu] % 2) return fail(ctx, LGF_EINVAL, "the checkerboard update needs even extents");
     const unsigned long long key = heatbath_key(seed);
-    for (int sw = 0; sw < nsweeps; sw++, ctx->hb_sweeps++)
+    for (int sw = 0; sw < nsweeps; sw++) {
         for (int mu = 0; mu < 4; mu++)
             for (int parity = 0; parity < 2; parity++) {
                 Bracket br(ctx, LGF_K_HEATBATH);
                 if (ctx->prec == LGF_FP64)
                     CK(launch_heatbath<double>(ctx->nr, link_pair<double>(ctx), ctx->g, ctx->st, beta, key, ctx->hb_sweeps,
-                                               mu, parity, ctx->stream));
+                                               mu, parity, ctx->stream, overrelax));
                 else
                     CK(launch_heatbath<float>(ctx->nr, link_pair<float>(ctx), ctx->g, ctx->st, beta, key, ctx->hb_sweeps, mu,
-                                              parity, ctx->stream));
+                                              parity, ctx->stream, overrelax));
             }
+        if (!overrelax) ctx->hb_sweeps++;                // only heat-bath sweeps consume random numbers
+    }
     // a new configuration: the history, the counters and the accumulated transformation start again
     ctx->launches++;
     CK(launch_reset_counters(ctx->st, ctx->stream));
     ctx->w_is_delta = false;
     ctx->recorded = false;
+    ctx->updates_enqueued = 0;
     if (ctx->Gacc) {
         ctx->launches++;
         if (ctx->prec == LGF_FP64)
@@ -805,6 +807,18 @@ int lgf_thermalize(lgf_ctx *ctx, double beta, int nsweeps, unsigned long long se
             CK(launch_gacc<float>(0, nullptr, (C<float> *)ctx->Gacc, nullptr, ctx->g, ctx->st, ctx->stream));
     }
     return LGF_OK;
+}
+
+int lgf_thermalize(lgf_ctx *ctx, double beta, int nsweeps, unsigned long long seed) {
+    if (!ctx || nsweeps < 0 || !(beta > 0.0)) return fail(ctx, LGF_EINVAL, "lgf_thermalize: bad argument");
+    if (!ctx->have_links) return fail(ctx, LGF_ESTATE, "lgf_thermalize: no configuration loaded");
+    return monte_carlo_sweeps(ctx, beta, nsweeps, seed, false);
+}
+
+int lgf_overrelax(lgf_ctx *ctx, int nsweeps) {
+    if (!ctx || nsweeps < 0) return fail(ctx, LGF_EINVAL, "lgf_overrelax: bad argument");
+    if (!ctx->have_links) return fail(ctx, LGF_ESTATE, "lgf_overrelax: no configuration loaded");
+    return monte_carlo_sweeps(ctx, 0.0, nsweeps, 0, true);
 }
 
 int lgf_track_transform(lgf_ctx *ctx, int on) {

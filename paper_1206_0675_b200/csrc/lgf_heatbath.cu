@@ -12,6 +12,8 @@
 //   X ~ exp(a x0) sqrt(1 - x0^2), a = 2 beta kk / 3; alpha = X (r/kk)^dag; U <- E(alpha) U, W <- E(alpha) W  (R26)
 //   then U is re-projected onto SU(3) (Gram-Schmidt rows 0, 1; row 2 = (row0 x row1)^*): without it the norm
 //   error of rows 0, 1 grows exponentially over the sweeps in 12-real storage (overflow before 300 sweeps)  (R26)
+//   overrelaxation (OVERRELAX): alpha = (V^dag)^2 instead of the draw -- alpha V = V^dag has the same x0 as V, the
+//   action is unchanged by every step; no random numbers                                                    (R28)
 //   uniforms u_n = ((mix64(key + (idx+1) G) >> 11) + 0.5) 2^-53, idx = ((((class V + site) 3 + k) 32 + t) 6 + n) (R27)
 // The arithmetic is double precision whatever the storage precision of the links.
 #include "lgf_state.cuh"
@@ -106,7 +108,7 @@ __device__ __forceinline__ void hb_sample(double a, unsigned long long key, unsi
 }
 
 // One class (mu, parity) of one sweep.  class_id = sweep * 8 + mu * 2 + parity selects the random stream.
-template <class R, int NR>
+template <class R, int NR, bool OVERRELAX>
 __global__ void __launch_bounds__(HB_THREADS) k_heatbath(LinkPair<R> lp, Geom g, const DevState *__restrict__ st,
                                                          double beta, unsigned long long key,
                                                          unsigned long long class_id, int mu, int parity) {
@@ -160,10 +162,11 @@ __global__ void __launch_bounds__(HB_THREADS) k_heatbath(LinkPair<R> lp, Geom g,
         const double r0 = 0.5 * (a.x + d.x), r1 = 0.5 * (b.y + cc.y), r2 = 0.5 * (b.x - cc.x), r3 = 0.5 * (a.y - d.y);
         const double kk = sqrt(r0 * r0 + r1 * r1 + r2 * r2 + r3 * r3);
         if (!(kk > 1e-300)) continue;
-        double x[4];
-        hb_sample(2.0 * beta * kk / 3.0, key, ((link_idx * 3ULL + (unsigned long long)k) * HB_MAXATT) * 6ULL, x);
         // alpha = X V^dag, V^dag = (r0, -r) / kk
         const double q0 = r0 / kk, q1 = -r1 / kk, q2 = -r2 / kk, q3 = -r3 / kk;
+        double x[4];
+        if constexpr (OVERRELAX) { x[0] = q0; x[1] = q1; x[2] = q2; x[3] = q3; }       // X = V^dag
+        else hb_sample(2.0 * beta * kk / 3.0, key, ((link_idx * 3ULL + (unsigned long long)k) * HB_MAXATT) * 6ULL, x);
         const double al0 = x[0] * q0 - (x[1] * q1 + x[2] * q2 + x[3] * q3);
         const double al1 = x[0] * q1 + q0 * x[1] - (x[2] * q3 - x[3] * q2);
         const double al2 = x[0] * q2 + q0 * x[2] - (x[3] * q1 - x[1] * q3);
@@ -211,11 +214,15 @@ unsigned long long heatbath_key(unsigned long long seed) {
 
 template <class R>
 cudaError_t launch_heatbath(int nr, LinkPair<R> links, const Geom &g, const DevState *st, double beta,
-                            unsigned long long key, unsigned long long sweep, int mu, int parity, cudaStream_t stream) {
+                            unsigned long long key, unsigned long long sweep, int mu, int parity, cudaStream_t stream,
+                            bool overrelax) {
     const int nb = (int)((g.V / 2 + HB_THREADS - 1) / HB_THREADS);
     const unsigned long long class_id = sweep * 8ULL + (unsigned long long)(mu * 2 + parity);
-    if (nr == 3) k_heatbath<R, 3><<<nb, HB_THREADS, 0, stream>>>(links, g, st, beta, key, class_id, mu, parity);
-    else k_heatbath<R, 2><<<nb, HB_THREADS, 0, stream>>>(links, g, st, beta, key, class_id, mu, parity);
+    if (overrelax) {
+        if (nr == 3) k_heatbath<R, 3, true><<<nb, HB_THREADS, 0, stream>>>(links, g, st, beta, key, class_id, mu, parity);
+        else k_heatbath<R, 2, true><<<nb, HB_THREADS, 0, stream>>>(links, g, st, beta, key, class_id, mu, parity);
+    } else if (nr == 3) k_heatbath<R, 3, false><<<nb, HB_THREADS, 0, stream>>>(links, g, st, beta, key, class_id, mu, parity);
+    else k_heatbath<R, 2, false><<<nb, HB_THREADS, 0, stream>>>(links, g, st, beta, key, class_id, mu, parity);
     return cudaGetLastError();
 }
 cudaError_t launch_reset_counters(DevState *st, cudaStream_t stream) {
@@ -224,8 +231,8 @@ cudaError_t launch_reset_counters(DevState *st, cudaStream_t stream) {
 }
 
 template cudaError_t launch_heatbath<float>(int, LinkPair<float>, const Geom &, const DevState *, double,
-                                            unsigned long long, unsigned long long, int, int, cudaStream_t);
+                                            unsigned long long, unsigned long long, int, int, cudaStream_t, bool);
 template cudaError_t launch_heatbath<double>(int, LinkPair<double>, const Geom &, const DevState *, double,
-                                             unsigned long long, unsigned long long, int, int, cudaStream_t);
+                                             unsigned long long, unsigned long long, int, int, cudaStream_t, bool);
 
 }  // namespace lgf

@@ -121,7 +121,8 @@ cudaError_t launch_field_set(C<R> *W, const R *field, const Geom &g, cudaStream_
 unsigned long long heatbath_key(unsigned long long seed);
 template <class R>
 cudaError_t launch_heatbath(int nr, LinkPair<R> links, const Geom &g, const DevState *st, double beta,
-                            unsigned long long key, unsigned long long sweep, int mu, int parity, cudaStream_t stream);
+                            unsigned long long key, unsigned long long sweep, int mu, int parity, cudaStream_t stream,
+                            bool overrelax /* R28: alpha = (V^dag)^2, no random numbers */);
 cudaError_t launch_reset_counters(DevState *st, cudaStream_t stream);
 
 // F / theta finalisation (precision independent)

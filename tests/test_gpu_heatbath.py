@@ -166,3 +166,35 @@ def test_many_sweeps_stay_in_su3(lgf, prec, storage):
     assert bool(torch.isfinite(torch.view_as_real(out)).all())
     assert dev < (1e-14 if prec == 8 else 1e-6)
     assert 0.55 < P < 0.64            # thermalised at beta = 6 (8^4: large fluctuations around 0.594)
+
+
+@pytest.mark.parametrize("prec,storage", [(8, 18), (8, 12), (4, 18)])
+def test_overrelaxation_matches_the_oracle_and_conserves_the_action(lgf, prec, storage):
+    """R28 on the CUDA side: one and two sweeps against the oracle, the plaquette conserved, history reset."""
+    dims = (8, 4, 6, 8)
+    U0 = oracle.heatbath(dims, inputs.hot_config(dims, 41), 5.7, 3, 0, 2)
+    if prec == 4:
+        U0 = U0.astype(np.complex64).astype(np.complex128)
+    U1 = oracle.overrelax(dims, U0, 1)
+    U2 = oracle.overrelax(dims, U1, 1)
+    with lgf.Context(dims, prec, storage) as ctx:
+        d = _dev(U0, prec)
+        ctx.set_links(d)
+        _, _, P0 = ctx.measure()
+        ctx.iterate(0.08, 1)
+        ctx.set_links(d)
+        ctx.overrelax(1)
+        assert ctx.history_length() == 0
+        e1 = np.abs(_links(ctx, d) - U1)
+        ctx.overrelax(1)
+        e2 = np.abs(_links(ctx, d) - U2)
+        _, _, P2 = ctx.measure()
+        ctx.thermalize(5.7, 1, 3)                     # overrelaxation consumes no random numbers: this is sweep 0
+        e3 = np.abs(_links(ctx, d) - oracle.heatbath(dims, U2, 5.7, 3, 0, 1))
+    if prec == 8:
+        assert e1.max() < TOL1 and np.quantile(e2, 0.999) < TOL1 * growth(5.7) and e2.max() < NO_FLIP
+        assert np.quantile(e3, 0.999) < TOL1 * growth(5.7) ** 2 and e3.max() < NO_FLIP
+        assert abs(P2 - P0) < 1e-13
+    else:
+        assert e1.max() < 1e-5 and e2.max() < 1e-4
+        assert abs(P2 - P0) < 2e-6
