@@ -168,15 +168,17 @@ __global__ void __launch_bounds__((Zt2Shape<R, LZ, LT, XC>::THREADS))
 }
 
 // ---- configuration and launchers --------------------------------------------------------------------
-// planes per CTA of the (x, y) sweeps (a multiple of 4 allows the g output) and consecutive (kx, ky) indices
-// per CTA of the (z, t) sweep
+// planes per CTA of the inverse (P; a multiple of 4 allows the g output) and of the forward (PF) (x, y) sweep,
+// and consecutive (kx, ky) indices per CTA of the (z, t) sweep.  Measured at 32^4 on B200 (FFT time per
+// iteration): PF = 4 -> 2: fp64 0.1129 -> 0.1091 ms, fp32 0.0643 -> 0.0628 ms (smaller CTAs, shorter last
+// wave; PF = 1 the same as 2); XC = 4 against 2 / 1 / 8: fp64 0.1129 against 0.1189 / 0.1438 / 0.1226 ms.
 template <class R, int L> struct Xy2Cfg;
-template <> struct Xy2Cfg<double, 16> { static constexpr int P = 8; };
-template <> struct Xy2Cfg<double, 32> { static constexpr int P = 4; };
-template <> struct Xy2Cfg<double, 64> { static constexpr int P = 1; };     // 4 planes of 64 x 64 fp64 exceed shared memory
-template <> struct Xy2Cfg<float, 16> { static constexpr int P = 8; };
-template <> struct Xy2Cfg<float, 32> { static constexpr int P = 4; };
-template <> struct Xy2Cfg<float, 64> { static constexpr int P = 4; };
+template <> struct Xy2Cfg<double, 16> { static constexpr int P = 8, PF = 8; };
+template <> struct Xy2Cfg<double, 32> { static constexpr int P = 4, PF = 2; };
+template <> struct Xy2Cfg<double, 64> { static constexpr int P = 1, PF = 1; };   // 4 planes of 64 x 64 fp64 exceed shared memory
+template <> struct Xy2Cfg<float, 16> { static constexpr int P = 8, PF = 8; };
+template <> struct Xy2Cfg<float, 32> { static constexpr int P = 4, PF = 2; };
+template <> struct Xy2Cfg<float, 64> { static constexpr int P = 4, PF = 4; };
 template <class R, int L> struct Zt2Cfg;
 template <> struct Zt2Cfg<double, 16> { static constexpr int XC = 4; };
 template <> struct Zt2Cfg<double, 32> { static constexpr int XC = 4; };
@@ -201,24 +203,26 @@ bool fft_reg2_gout(const Geom &g, int prec) {
     return true;
 }
 
-template <class R, int L>
-static cudaError_t launch_xy2(int which, const Geom &g, C<R> *W, const DevState *st, cudaStream_t stream, C<R> *G,
-                              R half_alpha) {
-    constexpr int P = Xy2Cfg<R, L>::P;
+template <class R, int L, int MODE, int P, bool GOUT>
+static cudaError_t launch_xy2_as(const Geom &g, C<R> *W, const DevState *st, cudaStream_t stream, C<R> *G, R half_alpha) {
     constexpr size_t SM = sizeof(C<R>) * P * L * (L | 1);
     const long long planes = 4LL * g.L[2] * g.L[3];
-    const int nzt = g.L[2] * g.L[3];
-    void (*kern)(C<R> *, const DevState *, C<R> *, long long, int, R) = nullptr;
-    if (which == 0) kern = k_fftr2_xy<R, L, FFT_FWD, P, false>;
-    else if (which == 2) kern = k_fftr2_xy<R, L, FFT_INV, P, false>;
-    else if constexpr (P % 4 == 0) kern = k_fftr2_xy<R, L, FFT_INV, P, true>;
-    if (!kern) return cudaErrorInvalidValue;
+    auto kern = k_fftr2_xy<R, L, MODE, P, GOUT>;
     if (SM > 40 * 1024) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SM);
         if (e != cudaSuccess) return e;
     }
-    kern<<<(unsigned)(planes / P), 2 * P * L, SM, stream>>>(W, st, G, g.V, nzt, half_alpha);
+    kern<<<(unsigned)(planes / P), 2 * P * L, SM, stream>>>(W, st, G, g.V, g.L[2] * g.L[3], half_alpha);
     return cudaGetLastError();
+}
+template <class R, int L>
+static cudaError_t launch_xy2(int which, const Geom &g, C<R> *W, const DevState *st, cudaStream_t stream, C<R> *G,
+                              R half_alpha) {
+    constexpr int P = Xy2Cfg<R, L>::P, PF = Xy2Cfg<R, L>::PF;
+    if (which == 0) return launch_xy2_as<R, L, FFT_FWD, PF, false>(g, W, st, stream, G, half_alpha);
+    if (which == 2) return launch_xy2_as<R, L, FFT_INV, P, false>(g, W, st, stream, G, half_alpha);
+    if constexpr (P % 4 == 0) return launch_xy2_as<R, L, FFT_INV, P, true>(g, W, st, stream, G, half_alpha);
+    return cudaErrorInvalidValue;
 }
 
 template <class R, int L>
