@@ -164,7 +164,8 @@ int lgf_get_transform(lgf_ctx *ctx, void *d_transform);
  * "fft_zt_xc" (consecutive (x, y) indices per CTA of the (z, t) pass, 0 = automatic), "fft_reg2" (1 = two
  * threads per line where the lattice allows), "fuse_g" (1 = the last FFT sweep ends with the g-build),
  * "sweep_tz" (z-planes per (z, t) tile of the sweep's CTA order, 0 = automatic, 1 = plain order),
- * "sweep_tiled" (1 = tiled sweep variant), "sweep_tt" (its t-march length), "sweep_minb" (2, 3 or 4: resident
+ * "sweep_share" (1 / 0 / -1 = automatic: backward x, y neighbours of the same CTA hand over their algebra parts
+ * through shared memory instead of being recomputed), "sweep_tiled" (1 = tiled sweep variant), "sweep_tt" (its t-march length), "sweep_minb" (2, 3 or 4: resident
  * CTAs per SM the sweep's register allocation is asked to allow), "reunit_every" (N > 0: in every
  * N-th update the new links are projected back onto SU(3) inside the sweep; 0 = never, the method as the
  * paper states it -- this key DOES change the result, by the rounding drift it removes; meant for fp32 runs

@@ -49,6 +49,8 @@ struct lgf_ctx {
     int tune_fuse_g = 1;         // lgf_tune: end the last FFT sweep with the g-build (register-line plan only)
     int tune_sweep_tiled = 0;    // lgf_tune: tiled sweep (shared-memory neighbour exchange, finalize folded in)
     int tune_sweep_minb = 3;     // lgf_tune: resident CTAs per SM the sweep's register allocation is asked to allow
+    int tune_sweep_share = -1;   // lgf_tune: hand A'_x, A'_y to the forward neighbours of the same CTA through shared
+                                 // memory (1 / 0; -1 = automatic: 18-real and fp32 or a lattice beyond L2)
     int tune_reunit = 0;         // lgf_tune "reunit_every": project the new links onto SU(3) in every N-th update (0 = never)
     long long updates_enqueued = 0;   // host-side count of updates enqueued since the last set_links / thermalize
     int tune_sweep_tz = 0;       // lgf_tune: z-planes per (z, t) tile of the sweep's block order (0 = automatic, 1 = plain)
@@ -376,7 +378,8 @@ static int step_update(lgf_ctx *ctx, double alpha, double tol, int record, bool 
     {
         Bracket br(ctx, LGF_K_UPDATE);
         CK(launch_sweep<R>(ctx->nr, link_pair<R>(ctx), (const C<R> *)ctx->G, (C<R> *)ctx->W, ctx->g, ctx->partial,
-                           &ctx->nb_partial, ctx->st, ctx->stream, ctx->tune_sweep_tz, reunit, ctx->tune_sweep_minb));
+                           &ctx->nb_partial, ctx->st, ctx->stream, ctx->tune_sweep_tz, reunit, ctx->tune_sweep_minb,
+                           ctx->tune_sweep_share));
     }
     return step_finalize(ctx, tol, 1, record);
 }
@@ -864,6 +867,7 @@ int lgf_tune(lgf_ctx *ctx, const char *key, int value) {
     else if (k == "sweep_tiled") ctx->tune_sweep_tiled = value;
     else if (k == "fuse_g") ctx->tune_fuse_g = value;
     else if (k == "sweep_tz") ctx->tune_sweep_tz = value;
+    else if (k == "sweep_share") ctx->tune_sweep_share = value;
     else if (k == "reunit_every") ctx->tune_reunit = value < 0 ? 0 : value;
     else if (k == "sweep_tt") { ctx->tune_sweep_tt = value; ctx->tile = choose_sweep_tile(ctx->g, value); }
     else return fail(ctx, LGF_EINVAL, "lgf_tune: unknown key " + k);

@@ -175,6 +175,22 @@ __device__ __forceinline__ void project_su3(C<R> (&u)[9]) {
     reconstruct_row2(u);
 }
 
+template <class R>
+__device__ __forceinline__ void herm_to_smem(R *__restrict__ slot, int stride, const Herm<R> &a) {
+    slot[0] = a.m01.x; slot[stride] = a.m01.y; slot[2 * stride] = a.m02.x; slot[3 * stride] = a.m02.y;
+    slot[4 * stride] = a.m12.x; slot[5 * stride] = a.m12.y; slot[6 * stride] = a.m00; slot[7 * stride] = a.m11;
+}
+template <class R>
+__device__ __forceinline__ Herm<R> herm_from_smem(const R *__restrict__ slot, int stride) {
+    Herm<R> a;
+    a.m01 = mk<R>(slot[0], slot[stride]);
+    a.m02 = mk<R>(slot[2 * stride], slot[3 * stride]);
+    a.m12 = mk<R>(slot[4 * stride], slot[5 * stride]);
+    a.m00 = slot[6 * stride];
+    a.m11 = slot[7 * stride];
+    return a;
+}
+
 // ---- a6 + a1 fused --------------------------------------------------------------------------------
 // One thread per site x.  For every direction: the site's own new link U'_mu(x) = g(x) U_mu(x) g(x+mu)^dag
 // is computed, stored to the other link buffer and its algebra part subtracted from Delta(x); the new
@@ -182,7 +198,12 @@ __device__ __forceinline__ void project_su3(C<R> (&u)[9]) {
 // are L1/L2 hits: the neighbouring thread reads the same lines) and its algebra part added.  Reads
 // buffer `cur`, writes buffer 1-cur (k_finalize flips `cur`), so no thread ever sees a half-updated
 // neighbourhood (Jacobi update, R10).
-template <class R, int NR, int MINB, bool REUNIT>
+// SHARE: a CTA's 128 consecutive sites are whole x lines when Lx divides 128 (four lines at 32^4), so the
+// backward x neighbour of a site, and for most lines the backward y neighbour, belongs to the same CTA and has
+// just computed the very A'_mu the site needs.  Those two are handed over through shared memory (one barrier
+// per CTA, flat indexing) instead of being recomputed; neighbours outside the CTA, and z and t, are recomputed
+// as before.  At 32^4: 6.25 link transforms per site instead of 8.
+template <class R, int NR, int MINB, bool REUNIT, bool SHARE>
 __global__ void __launch_bounds__(SWEEP_THREADS, MINB)
     k_sweep(LinkPair<R> lp, const C<R> *__restrict__ G, C<R> *__restrict__ W, Geom g, double *__restrict__ partial,
             const DevState *__restrict__ st, BlockOrder bo) {
@@ -191,32 +212,70 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB)
     const C<R> *__restrict__ src = lp.buf[cur];
     C<R> *__restrict__ dst = lp.buf[1 - cur];
     __shared__ double scratch[SWEEP_THREADS / 32][2];
-    const long long s = block_base(bo, blockIdx.x) * SWEEP_THREADS + threadIdx.x;
+    __shared__ R sA[SHARE ? 2 * 8 * SWEEP_THREADS : 1];          // A'_x, A'_y of the CTA's sites
+    const long long base = block_base(bo, blockIdx.x) * SWEEP_THREADS;
+    const long long s = base + threadIdx.x;
+    const bool live = s < g.V;
     double f = 0.0, t = 0.0;
-    if (s < g.V) {
-        int c[4];
+    int c[4] = {0, 0, 0, 0};
+    C<R> gx[9];
+    Herm<R> d = herm_zero<R>();
+    R retr = 0;
+    // the site's own new link in direction mu: transformed, stored, - A'_mu(x) into d; returns A'_mu(x)
+    auto own = [&](int mu) {
+        C<R> u[9], gn[9], p[9];
+        load_link<R, NR>(src, g.V, mu, s, u);
+        load_g(G, g.V, site_fwd(g, s, c, mu), gn);
+        transform_link<NR>(gx, u, gn, p);                           // Alg. 1 line 14, eq. 2
+        if constexpr (REUNIT) project_su3(p);
+        store_link<R, NR>(dst, g.V, mu, s, p);
+        retr += p[0].x + p[4].x + p[8].x;                           // eq. 3 on the new link
+        const Herm<R> a = algebra_part(p);
+        herm_sub(d, a);                                             // - A'_mu(x)
+        return a;
+    };
+    // + A'_mu(x - mu): the backward neighbour's new link recomputed (its inputs are L1 / L2 hits)
+    auto bwd = [&](int mu, long long sb) {
+        C<R> u[9], gn[9], p[9];
+        load_link<R, NR>(src, g.V, mu, sb, u);
+        load_g(G, g.V, sb, gn);
+        transform_link<NR>(gn, u, gx, p);
+        if constexpr (REUNIT) project_su3(p);                       // the same link the neighbour stores
+        herm_add(d, algebra_part(p));                               // eq. 5
+    };
+    if (live) {
         site_coords(g, s, c);
-        C<R> gx[9];
         load_g(G, g.V, s, gx);
-        Herm<R> d = herm_zero<R>();
-        R retr = 0;
+    }
+    if constexpr (!SHARE) {
+        if (live) {
 #pragma unroll
-        for (int mu = 0; mu < 4; mu++) {
-            C<R> u[9], gn[9], p[9];
-            load_link<R, NR>(src, g.V, mu, s, u);
-            load_g(G, g.V, site_fwd(g, s, c, mu), gn);
-            transform_link<NR>(gx, u, gn, p);                       // Alg. 1 line 14, eq. 2
-            if constexpr (REUNIT) project_su3(p);
-            store_link<R, NR>(dst, g.V, mu, s, p);
-            retr += p[0].x + p[4].x + p[8].x;                       // eq. 3 on the new link
-            herm_sub(d, algebra_part(p));                           // - A'_mu(x)
-            const long long sb = site_bwd(g, s, c, mu);
-            load_link<R, NR>(src, g.V, mu, sb, u);
-            load_g(G, g.V, sb, gn);
-            transform_link<NR>(gn, u, gx, p);
-            if constexpr (REUNIT) project_su3(p);                   // the same link the neighbour stores
-            herm_add(d, algebra_part(p));                           // + A'_mu(x - mu)     (eq. 5)
+            for (int mu = 0; mu < 4; mu++) {                        // own and backward link interleaved: the two
+                own(mu);                                            // touch neighbouring cache lines
+                bwd(mu, site_bwd(g, s, c, mu));
+            }
         }
+    } else {
+        if (live) {
+#pragma unroll
+            for (int mu = 0; mu < 2; mu++)
+                herm_to_smem(sA + mu * 8 * SWEEP_THREADS + threadIdx.x, SWEEP_THREADS, own(mu));
+        }
+        __syncthreads();
+        if (live) {
+#pragma unroll
+            for (int mu = 0; mu < 4; mu++) {
+                if (mu >= 2) own(mu);
+                const long long sb = site_bwd(g, s, c, mu);
+                const long long off = sb - base;
+                if (mu < 2 && off >= 0 && off < SWEEP_THREADS)
+                    herm_add(d, herm_from_smem(sA + mu * 8 * SWEEP_THREADS + (int)off, SWEEP_THREADS));
+                else
+                    bwd(mu, sb);
+            }
+        }
+    }
+    if (live) {
         store_herm(W, g.V, s, d);
         f = (double)retr;
         t = (double)herm_norm2(d);
@@ -243,22 +302,6 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB)
 // F and theta partial sums are reduced per CTA; the last CTA to finish (ticket counter) adds the per-CTA
 // partials in fixed order and does what k_finalize does, so one iteration needs no separate
 // finalize launch and the sums stay bit-reproducible.
-
-template <class R>
-__device__ __forceinline__ void herm_to_smem(R *__restrict__ slot, int stride, const Herm<R> &a) {
-    slot[0] = a.m01.x; slot[stride] = a.m01.y; slot[2 * stride] = a.m02.x; slot[3 * stride] = a.m02.y;
-    slot[4 * stride] = a.m12.x; slot[5 * stride] = a.m12.y; slot[6 * stride] = a.m00; slot[7 * stride] = a.m11;
-}
-template <class R>
-__device__ __forceinline__ Herm<R> herm_from_smem(const R *__restrict__ slot, int stride) {
-    Herm<R> a;
-    a.m01 = mk<R>(slot[0], slot[stride]);
-    a.m02 = mk<R>(slot[2 * stride], slot[3 * stride]);
-    a.m12 = mk<R>(slot[4 * stride], slot[5 * stride]);
-    a.m00 = slot[6 * stride];
-    a.m11 = slot[7 * stride];
-    return a;
-}
 
 template <class R, int NR, int MINB>
 __global__ void __launch_bounds__(SWEEP_THREADS, MINB)
@@ -531,13 +574,20 @@ cudaError_t launch_gbuild(const C<R> *W, C<R> *G, const Geom &g, R half_alpha, c
 }
 template <class R>
 cudaError_t launch_sweep(int nr, LinkPair<R> links, const C<R> *G, C<R> *W, const Geom &g, double *partial,
-                         int *nblocks, const DevState *st, cudaStream_t stream, int order_tz, bool reunit, int minb) {
+                         int *nblocks, const DevState *st, cudaStream_t stream, int order_tz, bool reunit, int minb,
+                         int share_mode) {
     const int nb = (int)((g.V + SWEEP_THREADS - 1) / SWEEP_THREADS);
     *nblocks = nb;
     // (z, t)-tiled block order when the (x, y) plane is a whole number of CTAs; TZ: about 24 MB of traffic
     // (1.3 kB per site in fp64 / 18-real) between a site and its t-neighbour
     BlockOrder bo{0, 1, g.L[2], g.L[3]};
     const long long plane = (long long)g.L[0] * g.L[1];
+    const bool beyond_l2 = (double)plane * (8.0 * 6.0 * nr + 28.0) * sizeof(R) * g.L[2] > 64.0e6;   // one t slice of traffic
+    // A'_x, A'_y through shared memory (SHARE): automatic where it measured faster on B200 -- 18-real storage,
+    // x lines that divide the CTA, and fp32 (32^4: 0.1718 -> 0.1601 ms; 64^4: 2.61 -> 2.42 ms) or a lattice beyond
+    // L2 (64^4 fp64: 4.42 -> 4.26 ms); neutral within 1.5 % otherwise, +1.7 % at 24^3 x 48.
+    const bool share = share_mode >= 0 ? share_mode != 0
+                                       : (nr == 3 && SWEEP_THREADS % g.L[0] == 0 && (sizeof(R) == 4 || beyond_l2));
     if (order_tz != 1 && plane % SWEEP_THREADS == 0) {
         int tz = order_tz;
         if (tz <= 0) {
@@ -545,22 +595,25 @@ cudaError_t launch_sweep(int nr, LinkPair<R> links, const C<R> *G, C<R> *W, cons
             // 32^4 where it fits, -4 % sweep time at 64^4 where it does not)
             const double per_plane = (double)plane * (8.0 * 6.0 * nr + 28.0) * sizeof(R);
             tz = 1;
-            if (per_plane * g.L[2] > 64.0e6)
+            if (beyond_l2)
                 while (tz * 2 <= g.L[2] && g.L[2] % (tz * 2) == 0 && per_plane * tz * 2 <= 24.0e6) tz *= 2;
         }
         if (tz > 1 && g.L[2] % tz == 0) { bo.nxy = (int)(plane / SWEEP_THREADS); bo.tz = tz; }
     }
     switch (minb) {
-#define LGF_SW(M)                                                                                     \
-    case M:                                                                                           \
-        if (reunit) {                                                                                     \
-            if (nr == 3) k_sweep<R, 3, M, true><<<nb, SWEEP_THREADS, 0, stream>>>(links, G, W, g, partial, st, bo); \
-            else k_sweep<R, 2, M, true><<<nb, SWEEP_THREADS, 0, stream>>>(links, G, W, g, partial, st, bo);         \
-        } else if (nr == 3) k_sweep<R, 3, M, false><<<nb, SWEEP_THREADS, 0, stream>>>(links, G, W, g, partial, st, bo); \
-        else k_sweep<R, 2, M, false><<<nb, SWEEP_THREADS, 0, stream>>>(links, G, W, g, partial, st, bo);         \
+#define LGF_SWK(M, RU, SH)                                                                                  \
+    if (nr == 3) k_sweep<R, 3, M, RU, SH><<<nb, SWEEP_THREADS, 0, stream>>>(links, G, W, g, partial, st, bo); \
+    else k_sweep<R, 2, M, RU, SH><<<nb, SWEEP_THREADS, 0, stream>>>(links, G, W, g, partial, st, bo);
+#define LGF_SW(M)                                                  \
+    case M:                                                        \
+        if (reunit && share) { LGF_SWK(M, true, true) }            \
+        else if (reunit) { LGF_SWK(M, true, false) }               \
+        else if (share) { LGF_SWK(M, false, true) }                \
+        else { LGF_SWK(M, false, false) }                          \
         break;
         LGF_SW(2) LGF_SW(3) LGF_SW(4)
 #undef LGF_SW
+#undef LGF_SWK
         default: return cudaErrorInvalidValue;
     }
     return cudaGetLastError();
@@ -693,7 +746,7 @@ cudaError_t launch_clear_done(DevState *st, cudaStream_t stream) {
                                          const DevState *, cudaStream_t);                                             \
     template cudaError_t launch_gbuild<R>(const C<R> *, C<R> *, const Geom &, R, const DevState *, cudaStream_t);     \
     template cudaError_t launch_sweep<R>(int, LinkPair<R>, const C<R> *, C<R> *, const Geom &, double *, int *,       \
-                                         const DevState *, cudaStream_t, int, bool, int);                                             \
+                                         const DevState *, cudaStream_t, int, bool, int, int);                                             \
     template cudaError_t launch_sweep_tiled<R>(int, LinkPair<R>, const C<R> *, C<R> *, const Geom &, const SweepTile &, \
                                                double *, int *, DevState *, double, int, double *, long long,         \
                                                cudaStream_t, int);                                                         \

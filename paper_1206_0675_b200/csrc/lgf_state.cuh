@@ -95,7 +95,7 @@ template <class R>
 cudaError_t launch_sweep(int nr, LinkPair<R> links, const C<R> *G, C<R> *W, const Geom &g, double *partial,
                          int *nblocks, const DevState *st, cudaStream_t stream, int order_tz /* 0 auto, 1 plain */,
                          bool reunit /* project every new link onto SU(3) */, int minb /* CTAs per SM asked of the
-                         register allocation: 2, 3 or 4 */);
+                         register allocation: 2, 3 or 4 */, int share_mode /* A'_x, A'_y through shared memory: 1 / 0 / -1 = where it measured faster */);
 // tiled sweep with the finalize folded in (last CTA): record / tol / hist as for launch_finalize
 template <class R>
 cudaError_t launch_sweep_tiled(int nr, LinkPair<R> links, const C<R> *G, C<R> *W, const Geom &g, const SweepTile &tl,

@@ -247,6 +247,22 @@ def test_trajectory_two_thread_fft(lgf, config_cache, prec, storage):
     assert np.max(np.abs(out - U_o)) < tol["links"]
 
 
+@pytest.mark.parametrize("name,dims", SMALL + [("tiny", (2, 4, 2, 6)), ("C2", (16, 16, 16, 16))])
+@pytest.mark.parametrize("prec,storage", VARIANTS)
+def test_trajectory_shared_neighbour_sweep(lgf, config_cache, name, dims, prec, storage):
+    """lgf_tune("sweep_share", 1): A'_x and A'_y of backward neighbours inside the same CTA come through shared
+    memory, the others are recomputed.  Lattices whose x lines do not divide the CTA's 128 sites (12, 3, 2) mix
+    both paths inside a warp.  Same parity bar as the default sweep."""
+    U = config_cache("C2") if name == "C2" else small_config(name, dims)
+    n = 12
+    U_o, F_o, T_o = oracle.iterate(dims, U, ALPHA, n)
+    Fh, Th, P, out = run_trajectory(lgf, dims, U, prec, storage, n, tune={"sweep_share": 1})
+    tol = TOL[prec]
+    assert np.max(np.abs(Fh - F_o) / np.abs(F_o)) < tol["scalar"]
+    assert np.max(np.abs(Th - T_o) / np.abs(T_o)) < tol["scalar"]
+    assert np.max(np.abs(out - U_o)) < tol["links"]
+
+
 def test_trajectory_asymmetric(lgf):
     """Radix-3 / mixed-length axes: 12 x 6 x 24 x 48, 10 iterations, fp64."""
     dims = (12, 6, 24, 48)
