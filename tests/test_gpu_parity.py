@@ -477,6 +477,36 @@ def test_reunit_holds_fp32_links_on_su3(lgf, storage):
     assert res[10][2] < 1e-3 and 0.5 < res[10][2] / res[0][2] < 2.0
 
 
+@pytest.mark.parametrize("prec", [8, 4])
+def test_nan_input_stops_the_iteration(lgf, config_cache, prec):
+    """include/lgf.h: theta NaN/Inf -> the device-side flag stops the loop, lgf_fix returns LGF_ENAN (at its next
+    look at the flag, not after max_iter), lgf_iterate stops recording; nothing hangs or aborts."""
+    import time
+
+    import torch
+
+    dims = inputs.CONFIGS["C1"]["dims"]
+    U = config_cache("C1").copy()
+    U[3, 2, 1, 0, 2, 1, 1] = np.nan
+    with lgf.Context(dims, prec, 18) as ctx:
+        d = to_dev(U, prec)
+        t0 = time.perf_counter()
+        with pytest.raises(lgf.LgfError) as e:
+            ctx.fix(d, ALPHA, 1e-15, 10 ** 6)
+        assert e.value.code == lgf.LGF_ENAN
+        assert time.perf_counter() - t0 < 5.0                 # a million iterations would take half a minute
+        ctx.set_links(to_dev(U, prec))
+        ctx.iterate(ALPHA, 50)
+        torch.cuda.synchronize()
+        n = ctx.history_length()
+        Fh, Th = ctx.history()
+        assert 1 <= n <= 3 and not np.isfinite(Th[-1])        # the NaN reaches theta within an iteration or two
+        # a clean configuration afterwards works as usual
+        ctx.set_links(to_dev(config_cache("C1"), prec))
+        ctx.iterate(ALPHA, 2)
+        assert ctx.history_length() == 3 and np.all(np.isfinite(ctx.history()[1]))
+
+
 def test_12_real_matches_18_real(lgf, config_cache):
     """Third-row reconstruction (eq. 8) changes rounding only."""
     dims = inputs.CONFIGS["C1"]["dims"]
