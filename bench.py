@@ -347,6 +347,7 @@ def run_thermal(args):
         ms_sweep = e0.elapsed_time(e1) / ((args.thermal_sweeps - 5) * (1 + args.thermal_overrelax))
         _, theta0, P0 = ctx.measure()
         links = ctx.get_links(torch.empty_like(cold))
+        ctx_thermalised = links.clone() if args.mixed else None
         dev0 = float((links @ links.conj().transpose(-1, -2) - torch.eye(3, dtype=cdt, device="cuda")).abs().max())
         tol = 1e-15 if prec == 8 else 1e-12
         torch.cuda.synchronize()
@@ -357,6 +358,32 @@ def run_thermal(args):
         F, theta, P1 = ctx.measure()
         Fh, _ = ctx.history()
         hb_bytes = ctx.algorithmic_bytes(binding.LGF_K_HEATBATH)
+        thermalised = ctx_thermalised if args.mixed else None
+    mixed = None
+    if args.mixed:
+        # NEXT-4 ablation, orbit-preserving: an fp32 context finds the accumulated transformation G (tracked, links
+        # projected every 20 updates, theta < 1e-12); G is applied to the ORIGINAL fp64 links with
+        # lgf_apply_transform (an exact gauge transformation: the plaquette is kept to fp64 rounding); lgf_fix
+        # polishes in fp64 to 1e-15.  Timed against the fp64-only fix above.  The float -> double cast of G is a
+        # dtype conversion of the exchange buffer.
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        with binding.Context(dims, binding.LGF_FP32, args.storage, stream=stream) as c32:
+            c32.tune("reunit_every", 20)
+            c32.track_transform(True)
+            it32 = c32.fix(thermalised.to(torch.complex64), args.alpha, 1e-12, args.thermal_max_iter)
+            G32 = c32.get_transform(torch.empty((32, 32, 32, 32, 3, 3), dtype=torch.complex64, device="cuda"))
+        with binding.Context(dims, binding.LGF_FP64, args.storage, stream=stream) as c64:
+            c64.set_links(thermalised)
+            c64.apply_transform(G32.to(torch.complex128))
+            l64 = c64.get_links(torch.empty_like(thermalised))
+            it64 = c64.fix(l64, args.alpha, 1e-15, args.thermal_max_iter)
+            torch.cuda.synchronize()
+            sec_mixed = time.perf_counter() - t0
+            Fm, thm, Pm = c64.measure()
+        mixed = {"iterations_fp32": it32, "iterations_fp64_polish": it64, "seconds": sec_mixed, "F_final": Fm,
+                 "theta_final": thm, "plaquette_after": Pm, "plaquette_drift": abs(Pm - P0),
+                 "speedup_vs_fp64_only": sec / sec_mixed}
     peak, _ = measured_peak()
     print(json.dumps({
         "mode": "thermal", "beta": args.thermal, "lattice": "32x32x32x32", "precision": args.precision,
@@ -367,7 +394,7 @@ def run_thermal(args):
         "plaquette_thermalised": P0, "su3_deviation_thermalised": dev0, "theta_before": theta0,
         "iterations_to_tol": it, "tol": tol, "seconds_to_fix": sec, "ms_per_iteration": 1e3 * sec / max(it, 1),
         "F_final": F, "theta_final": theta, "plaquette_after_fix": P1, "plaquette_drift": abs(P1 - P0),
-        "F_min_step": float(np.min(np.diff(Fh))) if len(Fh) > 1 else None,
+        "F_min_step": float(np.min(np.diff(Fh))) if len(Fh) > 1 else None, "mixed_precision": mixed,
         "paper_table3": "32^4 dp, C2070: 765-10427 iterations, 61.1 ms/iteration (12-real tex) -- other hardware, context"}),
         flush=True)
     return 0
@@ -403,6 +430,7 @@ def main():
     ap.add_argument("--reunit-every", type=int, default=0)
     ap.add_argument("--alpha", type=float, default=ALPHA, help="step size of the --thermal fix (the paper uses 0.08)")
     ap.add_argument("--thermal-max-iter", type=int, default=200000)
+    ap.add_argument("--mixed", action="store_true", help="--thermal (fp64 only): also time fp32 iterations + fp64 polish")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)
     if args.impl == "reference":

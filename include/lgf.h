@@ -156,6 +156,16 @@ int lgf_track_transform(lgf_ctx *ctx, int on);
  * [Lt, Lz, Ly, Lx, 3, 3] complex).  LGF_ESTATE if tracking is off.  Asynchronous on the context's stream. */
 int lgf_get_transform(lgf_ctx *ctx, void *d_transform);
 
+/* Apply a given gauge transformation to the internal configuration: U_mu(x) <- G(x) U_mu(x) G(x + mu)^dag
+ * (eq. 2) with d_transform[s][i][j][re/im] in the layout lgf_get_transform writes (18 reals per
+ * site, the context's precision).  Each G(x) is first projected onto SU(3) (Gram-Schmidt on rows 0, 1, row 2
+ * from eq. 8), so a transformation accumulated in float and converted to double may be passed: the result is
+ * an exact gauge transform of the loaded links -- every gauge-invariant quantity is preserved to rounding.
+ * Use: find G cheaply (an fp32 context with lgf_track_transform), apply it to the original fp64 links here,
+ * finish with lgf_fix in fp64.  Restarts the history and the counters like loading a configuration; an
+ * accumulated transformation that is being tracked is multiplied by G.  Asynchronous. */
+int lgf_apply_transform(lgf_ctx *ctx, const void *d_transform);
+
 /* ---- tuning --------------------------------------------------------------------------------------- */
 
 /* Override a planner choice of THIS context (takes effect from the next iteration; results are unchanged up

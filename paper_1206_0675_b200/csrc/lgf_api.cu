@@ -422,6 +422,23 @@ static int measure_only(lgf_ctx *ctx) {
     return step_finalize(ctx, -1.0, 0, 0);
 }
 
+template <class R>
+static int apply_transform(lgf_ctx *ctx, const void *d_transform) {
+    ctx->launches++;
+    CK(launch_gacc<R>(3, nullptr, (C<R> *)ctx->G, (R *)const_cast<void *>(d_transform), ctx->g, ctx->st, ctx->stream));
+    ctx->launches++;
+    CK(launch_clear_done(ctx->st, ctx->stream));
+    // the fused sweep with the given field in the place of g: U <- G U G(x+mu)^dag, Delta / F / theta of the result
+    const int rc = step_update<R>(ctx, 0.0, -1.0, 0, true);
+    if (rc != LGF_OK) return rc;
+    ctx->launches++;
+    CK(launch_reset_counters(ctx->st, ctx->stream));       // a new starting configuration: history and counters restart
+    ctx->w_is_delta = true;                                  // ... whose Delta and partial sums the sweep has left behind
+    ctx->recorded = false;
+    ctx->updates_enqueued = 0;
+    return LGF_OK;
+}
+
 #define DISPATCH(fn, ...) (ctx->prec == LGF_FP64 ? fn<double>(__VA_ARGS__) : fn<float>(__VA_ARGS__))
 
 static int fetch_state(lgf_ctx *ctx) {
@@ -850,6 +867,12 @@ int lgf_get_transform(lgf_ctx *ctx, void *d_transform) {
     else
         CK(launch_gacc<float>(2, nullptr, (C<float> *)ctx->Gacc, (float *)d_transform, ctx->g, ctx->st, ctx->stream));
     return LGF_OK;
+}
+
+int lgf_apply_transform(lgf_ctx *ctx, const void *d_transform) {
+    if (!ctx || !d_transform) return fail(ctx, LGF_EINVAL, "lgf_apply_transform: null argument");
+    if (!ctx->have_links) return fail(ctx, LGF_ESTATE, "lgf_apply_transform: no configuration loaded");
+    return ctx->prec == LGF_FP64 ? apply_transform<double>(ctx, d_transform) : apply_transform<float>(ctx, d_transform);
 }
 
 int lgf_tune(lgf_ctx *ctx, const char *key, int value) {

@@ -425,6 +425,20 @@ __global__ void __launch_bounds__(SITE_THREADS) k_gacc_identity(C<R> *__restrict
 #pragma unroll
     for (int e = 0; e < 9; e++) A[(long long)e * g.V + s] = mk<R>((e % 4 == 0) ? (R)1 : (R)0, (R)0);
 }
+// canonical transformation field in[s][i][j] -> rows 0, 1 of its projection onto SU(3) in the layout of G
+// (lgf_apply_transform: the given matrices may be a float product converted to double, i.e. off SU(3) by 1e-7)
+template <class R>
+__global__ void __launch_bounds__(SITE_THREADS) k_g_from_canonical(const R *__restrict__ in, C<R> *__restrict__ G, Geom g) {
+    const long long s = (long long)blockIdx.x * SITE_THREADS + threadIdx.x;
+    if (s >= g.V) return;
+    const C<R> *src = reinterpret_cast<const C<R> *>(in) + s * 9;
+    C<R> m[9];
+#pragma unroll
+    for (int e = 0; e < 9; e++) m[e] = src[e];
+    project_su3(m);
+#pragma unroll
+    for (int e = 0; e < 6; e++) G[(long long)e * g.V + s] = m[e];
+}
 // canonical output: out[s][i][j] complex, 18 reals per site
 template <class R>
 __global__ void __launch_bounds__(SITE_THREADS) k_gacc_get(const C<R> *__restrict__ A, R *__restrict__ out, Geom g) {
@@ -707,7 +721,8 @@ cudaError_t launch_convert_out(int nr, LinkPair<R> links, R *canon, const Geom &
 template <class R>
 cudaError_t launch_gacc(int op, const C<R> *G, C<R> *A, R *out, const Geom &g, const DevState *st, cudaStream_t stream) {
     const int nb = site_blocks(g);
-    if (op == 0) k_gacc_identity<R><<<nb, SITE_THREADS, 0, stream>>>(A, g);
+    if (op == 3) k_g_from_canonical<R><<<nb, SITE_THREADS, 0, stream>>>(out, A, g);      // out = input field, A = G
+    else if (op == 0) k_gacc_identity<R><<<nb, SITE_THREADS, 0, stream>>>(A, g);
     else if (op == 1) k_gacc<R><<<nb, SITE_THREADS, 0, stream>>>(G, A, g, st);
     else k_gacc_get<R><<<nb, SITE_THREADS, 0, stream>>>(A, out, g);
     return cudaGetLastError();

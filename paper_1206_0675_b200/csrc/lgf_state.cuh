@@ -109,7 +109,8 @@ cudaError_t launch_convert_in(int nr, const R *canon, C<R> *links0, const Geom &
 template <class R>
 cudaError_t launch_convert_out(int nr, LinkPair<R> links, R *canon, const Geom &g, const DevState *st,
                                cudaStream_t stream);
-// accumulated gauge transformation: op 0 = set to identity, 1 = Gacc <- g Gacc, 2 = copy out (canonical [s][3][3])
+// accumulated gauge transformation: op 0 = set to identity, 1 = Gacc <- g Gacc, 2 = copy out (canonical [s][3][3]),
+// 3 = (A = G, out = canonical input field) rows 0, 1 of the SU(3) projection of a given transformation into G
 template <class R>
 cudaError_t launch_gacc(int op, const C<R> *G, C<R> *A, R *out, const Geom &g, const DevState *st, cudaStream_t stream);
 template <class R>

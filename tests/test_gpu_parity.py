@@ -477,6 +477,73 @@ def test_reunit_holds_fp32_links_on_su3(lgf, storage):
     assert res[10][2] < 1e-3 and 0.5 < res[10][2] / res[0][2] < 2.0
 
 
+@pytest.mark.parametrize("dims", [(8, 8, 8, 8), (12, 6, 16, 4)])
+@pytest.mark.parametrize("prec,storage", [(8, 18), (8, 12), (4, 18)])
+def test_apply_transform(lgf, dims, prec, storage):
+    """lgf_apply_transform: U <- G U G(x+mu)^dag for a given field G against the oracle's transform; G off SU(3)
+    is projected first (row-wise Gram-Schmidt, the oracle's pinned orc_gs); history restarts; a tracked
+    accumulated transformation picks the factor up."""
+    import torch
+
+    V = int(np.prod(dims))
+    U = small_config("x", dims) if dims != (8, 8, 8, 8) else inputs.make_config("C1")
+    h = inputs.haar_su3(606, inputs.STREAM_HAAR, 0, V).reshape(site_shape(dims) + (3, 3))
+    noisy = h * (1.0 + 1e-3 * inputs.normals(607, 5, 0, V).reshape(site_shape(dims) + (1, 1)))      # off SU(3)
+    h_proj = np.stack([oracle.gs(m) for m in noisy.reshape(-1, 3, 3)]).reshape(h.shape)
+    U_o = oracle.transform(dims, U, h_proj)
+    D_o, F_o, T_o = oracle.measure(dims, U_o)
+    tol = 1e-13 if prec == 8 else 2e-6
+    cdt = torch.complex128 if prec == 8 else torch.complex64
+    with lgf.Context(dims, prec, storage) as ctx:
+        ctx.track_transform(True)
+        d = to_dev(U, prec)
+        ctx.set_links(d)
+        ctx.iterate(ALPHA, 2)
+        ctx.set_links(d)
+        _, _, P0 = ctx.measure()
+        ctx.apply_transform(to_dev(noisy, prec))
+        assert ctx.history_length() == 0 and ctx.iterations() == 0
+        out = to_np(ctx.get_links(torch.empty_like(d)))
+        Gt = to_np(ctx.get_transform(torch.empty(site_shape(dims) + (3, 3), dtype=cdt, device="cuda")))
+        ctx.iterate(ALPHA, 0)                                   # records entry 0 from what the sweep left behind
+        Fh, Th = ctx.history()
+        _, _, P1 = ctx.measure()
+    assert np.max(np.abs(out - U_o)) < tol
+    assert np.max(np.abs(Gt - h_proj)) < tol
+    assert len(Fh) == 1
+    assert abs(Fh[0] - F_o) < (1e-12 if prec == 8 else 1e-5) * abs(F_o)
+    assert abs(Th[0] - T_o) < (1e-12 if prec == 8 else 1e-5) * abs(T_o)
+    assert abs(P1 - P0) < (1e-13 if prec == 8 else 1e-6)        # gauge invariant
+
+
+def test_mixed_precision_workflow_preserves_the_orbit(lgf, config_cache):
+    """Find G in fp32 (tracked), apply it to the ORIGINAL fp64 links, polish in fp64: theta < 1e-15 with the
+    plaquette of the original configuration preserved to fp64 rounding, in far fewer fp64 iterations."""
+    import torch
+
+    dims = inputs.CONFIGS["C2"]["dims"]
+    U = config_cache("C2")
+    P_o = oracle.plaquette(dims, U)
+    with lgf.Context(dims, 4, 18) as c32:
+        c32.track_transform(True)
+        l32 = to_dev(U, 4)
+        it32 = c32.fix(l32, ALPHA, 1e-12, 2000)
+        G32 = c32.get_transform(torch.empty(site_shape(dims) + (3, 3), dtype=torch.complex64, device="cuda"))
+    with lgf.Context(dims, 8, 18) as c64:
+        d = to_dev(U, 8)
+        it_only = c64.fix(d.clone(), ALPHA, 1e-15, 2000)
+        c64.set_links(d)
+        c64.apply_transform(G32.to(torch.complex128))
+        _, th_start, P_start = c64.measure()
+        out = c64.get_links(torch.empty_like(d))
+        it_polish = c64.fix(out, ALPHA, 1e-15, 2000)
+        F, th, P = c64.measure()
+    assert 0 < it32 < 2000 and 0 < it_only < 2000
+    assert th_start < 1e-10                         # the float transformation already fixes the gauge to float accuracy
+    assert abs(P_start - P_o) < 1e-13 and abs(P - P_o) < 1e-13
+    assert th < 1e-15 and it_polish < it_only // 2
+
+
 @pytest.mark.parametrize("prec", [8, 4])
 def test_nan_input_stops_the_iteration(lgf, config_cache, prec):
     """include/lgf.h: theta NaN/Inf -> the device-side flag stops the loop, lgf_fix returns LGF_ENAN (at its next
