@@ -459,7 +459,14 @@ def main():
     dims = cfg["dims"]
     V = int(np.prod(dims))
     member = ensemble.member_indices(world, rank, world)[0]      # replicas: one ensemble member per GPU
-    U0 = inputs.make_config(args.workload, seed_offset=ensemble.member_seed_offset(member))
+    if cfg["kind"] == "hot":
+        # 64^4 hot start: the torch back end of the same counter-based streams (seconds on the GPU instead of
+        # minutes of numpy QR for 67 M links), brought to the host like every other input
+        seed = cfg["seed"] + 7919 * ensemble.member_seed_offset(member)
+        U0 = inputs.hot_config_torch(dims, seed, device="cuda").cpu().numpy()
+        torch.cuda.empty_cache()
+    else:
+        U0 = inputs.make_config(args.workload, seed_offset=ensemble.member_seed_offset(member))
 
     sampler = ClockSampler(physical_gpu_index(local))
     head = time_variant(binding, torch, U0, dims, args.precision, args.storage, args.steps, args.warmup, dist, sampler)
@@ -500,12 +507,14 @@ def main():
     e2e = None
     if not args.no_e2e:
         tol = 1e-15 if args.precision == "fp64" else 1e-12
-        r = time_e2e(binding, torch, U0, dims, args.precision, args.storage, tol, 5000, dist)
+        # a hot start is not run to convergence: BASELINE.json's C5 is a fixed 200 iterations
+        max_iter = 200 if cfg["kind"] == "hot" else 5000
+        r = time_e2e(binding, torch, U0, dims, args.precision, args.storage, tol, max_iter, dist)
         its = max(1, r["iterations"])
         e2e = {"value": world * its / (r["ms"] * 1e-3), "unit": UNIT,
                "h2d_bytes_per_step": r["bytes_each_way"] / its, "d2h_bytes_per_step": r["bytes_each_way"] / its,
-               "call": "lgf_fix_host(pinned host links, alpha=0.08, tol=%g): H2D + %d iterations + D2H in %.1f ms"
-                       % (tol, r["iterations"], r["ms"]), "final_theta": r["theta"]}
+               "call": "lgf_fix_host(pinned host links, alpha=0.08, tol=%g, max_iter=%d): H2D + %d iterations + D2H in %.1f ms"
+                       % (tol, max_iter, r["iterations"], r["ms"]), "final_theta": r["theta"]}
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
