@@ -47,15 +47,12 @@ struct lgf_ctx {
     int tune_xy_planes = 0;      // lgf_tune: planes per CTA of the (x, y) pass (0 = planner's choice)
     int tune_zt_xc = 0;          // lgf_tune: consecutive (x, y) indices per CTA of the (z, t) pass
     int tune_fuse_g = 1;         // lgf_tune: end the last FFT sweep with the g-build (register-line plan only)
-    int tune_sweep_tiled = 0;    // lgf_tune: tiled sweep (shared-memory neighbour exchange, finalize folded in)
     int tune_sweep_minb = 3;     // lgf_tune: resident CTAs per SM the sweep's register allocation is asked to allow
     int tune_sweep_share = -1;   // lgf_tune: hand A'_x, A'_y to the forward neighbours of the same CTA through shared
                                  // memory (1 / 0; -1 = automatic: 18-real and fp32 or a lattice beyond L2)
     int tune_reunit = 0;         // lgf_tune "reunit_every": project the new links onto SU(3) in every N-th update (0 = never)
     long long updates_enqueued = 0;   // host-side count of updates enqueued since the last set_links / thermalize
     int tune_sweep_tz = 0;       // lgf_tune: z-planes per (z, t) tile of the sweep's block order (0 = automatic, 1 = plain)
-    int tune_sweep_tt = 0;       // lgf_tune: t-march length of the tiled sweep (0 = automatic)
-    SweepTile tile{};
     struct Stamp { cudaEvent_t a, b; int cls; };
     std::vector<Stamp> stamps;
     double prof_ms[LGF_K_COUNT] = {0};
@@ -354,8 +351,7 @@ static int step_finalize(lgf_ctx *ctx, double tol, int after_sweep, int record) 
     return LGF_OK;
 }
 // The sweep also closes the iteration: it makes the new configuration current, and with record != 0 appends
-// (F, theta) to the history and applies the loop test theta < tol (a k_finalize launch after the default
-// sweep; inside the last CTA of the tiled one).
+// (F, theta) to the history and applies the loop test theta < tol (the k_finalize launch after the sweep).
 template <class R>
 static int step_update(lgf_ctx *ctx, double alpha, double tol, int record, bool g_ready = false) {
     if (!g_ready) {
@@ -368,13 +364,6 @@ static int step_update(lgf_ctx *ctx, double alpha, double tol, int record, bool 
     }
     ctx->updates_enqueued++;
     const bool reunit = ctx->tune_reunit > 0 && ctx->updates_enqueued % ctx->tune_reunit == 0;
-    if (ctx->tune_sweep_tiled && !reunit) {
-        Bracket br(ctx, LGF_K_UPDATE);
-        CK(launch_sweep_tiled<R>(ctx->nr, link_pair<R>(ctx), (const C<R> *)ctx->G, (C<R> *)ctx->W, ctx->g, ctx->tile,
-                                 ctx->partial, &ctx->nb_partial, ctx->st, tol, record, ctx->hist, ctx->hist_cap,
-                                 ctx->stream, ctx->tune_sweep_minb));
-        return LGF_OK;
-    }
     {
         Bracket br(ctx, LGF_K_UPDATE);
         CK(launch_sweep<R>(ctx->nr, link_pair<R>(ctx), (const C<R> *)ctx->G, (C<R> *)ctx->W, ctx->g, ctx->partial,
@@ -486,11 +475,7 @@ int lgf_create(const int dims[4], int precision, int link_storage, lgf_ctx **out
     alloc(&ctx->links[1], V * 4 * 3 * ctx->nr * cb);
     alloc(&ctx->W, V * 4 * cb);
     alloc(&ctx->G, V * 6 * cb);
-    ctx->tile = choose_sweep_tile(ctx->g, 0);
-    {   // >= the CTA count of every kernel that writes per-CTA partial sums (tiled sweep: at most V / threads)
-        const size_t a = (V + 127) / 128, b = V / (size_t)ctx->tile.threads;
-        ctx->partial_cap = (int)(a > b ? a : b) + 1;
-    }
+    ctx->partial_cap = (int)((V + 127) / 128) + 1;   // >= the CTA count of every kernel that writes per-CTA partial sums
     alloc((void **)&ctx->partial, sizeof(double) * 4 * ctx->partial_cap);
     alloc((void **)&ctx->st, sizeof(DevState));
     ctx->hist_cap = 1 << 20;
@@ -887,12 +872,10 @@ int lgf_tune(lgf_ctx *ctx, const char *key, int value) {
         if (value < 2 || value > 4) return fail(ctx, LGF_EINVAL, "lgf_tune: sweep_minb must be 2, 3 or 4");
         ctx->tune_sweep_minb = value;
     }
-    else if (k == "sweep_tiled") ctx->tune_sweep_tiled = value;
     else if (k == "fuse_g") ctx->tune_fuse_g = value;
     else if (k == "sweep_tz") ctx->tune_sweep_tz = value;
     else if (k == "sweep_share") ctx->tune_sweep_share = value;
     else if (k == "reunit_every") ctx->tune_reunit = value < 0 ? 0 : value;
-    else if (k == "sweep_tt") { ctx->tune_sweep_tt = value; ctx->tile = choose_sweep_tile(ctx->g, value); }
     else return fail(ctx, LGF_EINVAL, "lgf_tune: unknown key " + k);
     CK(cudaStreamSynchronize(ctx->stream));
     return plan_passes(ctx);

@@ -202,7 +202,7 @@ __global__ void __launch_bounds__(HB_THREADS) k_heatbath(LinkPair<R> lp, Geom g,
 
 // a changed configuration: forget the history and the counters, keep which link buffer is current
 __global__ void k_reset_counters(DevState *st) {
-    st->n_hist = 0; st->n_updates = 0; st->done = 0; st->nan = 0; st->F = 0.0; st->theta = 0.0; st->ticket = 0;
+    st->n_hist = 0; st->n_updates = 0; st->done = 0; st->nan = 0; st->F = 0.0; st->theta = 0.0;
 }
 
 unsigned long long heatbath_key(unsigned long long seed) {

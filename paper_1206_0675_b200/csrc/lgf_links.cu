@@ -102,42 +102,6 @@ __device__ __forceinline__ void finalize_tail(double f, double t, long long V, d
     }
 }
 
-// End of a sweep kernel: per-CTA partial sums of F and theta; the last CTA to deliver (ticket counter) adds
-// all partials in a fixed order -- bit-reproducible -- and closes the iteration as k_finalize would
-// (new buffer current, history, stop test).  Used by the tiled sweep, whose CTAs live long enough to
-// amortise the release fence.
-// Every thread of the block must call this.
-__device__ __forceinline__ void close_sweep(double f, double t, double *__restrict__ partial, double (*scratch)[2],
-                                            long long V, double tol, int record, DevState *st,
-                                            double *__restrict__ hist, long long hist_cap, unsigned int *ticket) {
-    __shared__ int is_last;
-    block_sum2(f, t, scratch);
-    if (threadIdx.x == 0) {
-        partial[2 * blockIdx.x] = f;
-        partial[2 * blockIdx.x + 1] = t;
-        // release only: orders the two stores above before the ticket without the L1 invalidation that a
-        // full __threadfence() (acquire side, CCTL.IVALL) would inflict on the CTAs still running on this SM
-        unsigned int n;
-        asm volatile("atom.add.release.gpu.global.u32 %0, [%1], 1;" : "=r"(n) : "l"(ticket) : "memory");
-        is_last = (n == gridDim.x - 1);
-    }
-    __syncthreads();
-    if (is_last) {
-        __threadfence();                                  // acquire side, this one CTA only
-        f = 0.0; t = 0.0;
-        for (int i = threadIdx.x; i < (int)gridDim.x; i += blockDim.x) {
-            f += __ldcg(partial + 2 * i);
-            t += __ldcg(partial + 2 * i + 1);
-        }
-        __syncthreads();
-        block_sum2(f, t, scratch);
-        if (threadIdx.x == 0) {
-            *ticket = 0;
-            finalize_tail(f, t, V, tol, 1, record, st, hist, hist_cap);
-        }
-    }
-}
-
 // Order in which the CTAs of the sweep walk the lattice.  With the plain order (block b = sites
 // 128 b .. 128 b + 127) the t-backward neighbour of a site was touched a whole t slice earlier: 43 MB of
 // traffic at 32^3, 340 MB at 64^3 -- beyond L2, so U_t(x - t), g(x - t) and g(x) come from DRAM a second
@@ -280,123 +244,14 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB)
         f = (double)retr;
         t = (double)herm_norm2(d);
     }
-    // k_finalize closes the iteration in a launch of its own: folding it in here (close_sweep) costs more
-    // than that launch, because the release fence holds each of the 8192 short-lived CTAs until its link
-    // stores are acknowledged (measured 0.271 -> 0.317 ms at 32^4 fp64)
+    // k_finalize closes the iteration in a launch of its own: folding it in here (release fence + ticket per
+    // CTA, last CTA finalises) costs more than that launch, because the fence holds each of the 8192
+    // short-lived CTAs until its link stores are acknowledged (measured 0.271 -> 0.317 ms at 32^4 fp64)
     block_sum2(f, t, scratch);
     if (threadIdx.x == 0) {
         partial[2 * blockIdx.x] = f;
         partial[2 * blockIdx.x + 1] = t;
     }
-}
-
-// ---- a6 + a1 fused, tiled -------------------------------------------------------------------------
-// The same computation as k_sweep with each new link computed (almost) once.  A CTA owns a tile of
-// TX x TY x TZ sites of one t slice (one thread per site) and marches TT slices forward in t.  Per slice a
-// thread computes its own four new links U'_mu(x), stores them, and publishes their algebra parts
-// A'_mu(x) (8 reals each) in shared memory (double-buffered by slice parity).
-// Delta(x) = sum_mu [A'_mu(x - mu) - A'_mu(x)] (eq. 5) then takes A'_mu(x - mu) from the neighbouring
-// thread's shared-memory slot (A'_t: from this thread's own slot of the previous slice) -- also across the periodic wrap when the tile spans the whole axis -- and
-// recomputes it (as k_sweep does for every direction) only on the low faces of the tile and on the first
-// slice of the march.  Link transforms per site: 4 + 1/TY + 1/TZ + 1/TT (+ 1/TX) instead of 8.
-// F and theta partial sums are reduced per CTA; the last CTA to finish (ticket counter) adds the per-CTA
-// partials in fixed order and does what k_finalize does, so one iteration needs no separate
-// finalize launch and the sums stay bit-reproducible.
-
-template <class R, int NR, int MINB>
-__global__ void __launch_bounds__(SWEEP_THREADS, MINB)
-    k_sweep_tiled(LinkPair<R> lp, const C<R> *__restrict__ G, C<R> *__restrict__ W, Geom g, SweepTile tl,
-                  double *__restrict__ partial, DevState *st, double tol, int record, double *__restrict__ hist,
-                  long long hist_cap, unsigned int *__restrict__ ticket) {
-    if (st->done) return;
-    const int cur = st->cur;
-    const C<R> *__restrict__ src = lp.buf[cur];
-    C<R> *__restrict__ dst = lp.buf[1 - cur];
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    R *sA = reinterpret_cast<R *>(smem_raw);                  // [2 buffers][4 directions][8 reals][threads]
-    __shared__ double scratch[SWEEP_THREADS / 32][2];
-    const int nth = tl.threads;
-    // the block is padded to whole warps; the padding threads shadow thread 0 (same loads, same barriers)
-    // and store nothing
-    const bool active = (int)threadIdx.x < nth;
-    const int tid = active ? (int)threadIdx.x : 0;
-    // tile origin and this thread's site in the first slice
-    int b = blockIdx.x;
-    const int bx = b % tl.nt[0]; b /= tl.nt[0];
-    const int by = b % tl.nt[1]; b /= tl.nt[1];
-    const int bz = b % tl.nt[2];
-    const int bt = b / tl.nt[2];
-    int l[3];
-    l[0] = tid % tl.T[0];
-    l[1] = (tid / tl.T[0]) % tl.T[1];
-    l[2] = tid / (tl.T[0] * tl.T[1]);
-    const int lstride[3] = {1, tl.T[0], tl.T[0] * tl.T[1]};
-    int c[4];
-    c[0] = bx * tl.T[0] + l[0];
-    c[1] = by * tl.T[1] + l[1];
-    c[2] = bz * tl.T[2] + l[2];
-    c[3] = bt * tl.T[3];
-    double f = 0.0, t = 0.0;
-    {
-        long long s = c[0] + g.S[1] * c[1] + g.S[2] * c[2] + g.S[3] * c[3];
-        // where A'_mu(x - mu) comes from, mu = x, y, z: >= 0: that thread's slot; -1: recompute (tile face)
-        int nbr[3];
-#pragma unroll
-        for (int mu = 0; mu < 3; mu++)
-            nbr[mu] = l[mu] > 0 ? tid - lstride[mu] : (tl.T[mu] == g.L[mu] ? tid + (tl.T[mu] - 1) * lstride[mu] : -1);
-        for (int k = 0; k < tl.T[3]; k++) {
-            R *buf = sA + (k & 1) * (32 * nth);
-            const R *prev = sA + ((k & 1) ^ 1) * (32 * nth);       // the previous slice's slots
-            C<R> gx[9];
-            load_g(G, g.V, s, gx);
-            Herm<R> d = herm_zero<R>();
-            R retr = 0;
-#pragma unroll
-            for (int mu = 0; mu < 4; mu++) {
-                C<R> u[9], gn[9], p[9];
-                load_link<R, NR>(src, g.V, mu, s, u);
-                load_g(G, g.V, site_fwd(g, s, c, mu), gn);
-                transform_link<NR>(gx, u, gn, p);                   // Alg. 1 line 14, eq. 2
-                if (active) store_link<R, NR>(dst, g.V, mu, s, p);
-                retr += p[0].x + p[4].x + p[8].x;                   // eq. 3 on the new link
-                const Herm<R> a = algebra_part(p);
-                herm_sub(d, a);                                     // - A'_mu(x)
-                if (active) herm_to_smem(buf + mu * 8 * nth + tid, nth, a);     // slot 3 (A'_t) is read back by this thread only
-            }
-            __syncthreads();
-#pragma unroll
-            for (int mu = 0; mu < 3; mu++) {
-                if (nbr[mu] >= 0) {
-                    herm_add(d, herm_from_smem(buf + mu * 8 * nth + nbr[mu], nth));
-                } else {
-                    C<R> u[9], gn[9], p[9];
-                    const long long sb = site_bwd(g, s, c, mu);
-                    load_link<R, NR>(src, g.V, mu, sb, u);
-                    load_g(G, g.V, sb, gn);
-                    transform_link<NR>(gn, u, gx, p);
-                    herm_add(d, algebra_part(p));                   // + A'_mu(x - mu)     (eq. 5)
-                }
-            }
-            if (k == 0) {
-                C<R> u[9], gn[9], p[9];
-                const long long sb = site_bwd(g, s, c, 3);
-                load_link<R, NR>(src, g.V, 3, sb, u);
-                load_g(G, g.V, sb, gn);
-                transform_link<NR>(gn, u, gx, p);
-                herm_add(d, algebra_part(p));
-            } else {
-                herm_add(d, herm_from_smem(prev + 3 * 8 * nth + tid, nth));   // A'_t(x - t) of the previous slice
-            }
-            if (active) {
-                store_herm(W, g.V, s, d);
-                f += (double)retr;
-                t += (double)herm_norm2(d);
-            }                             // eq. 6
-            s += g.S[3];
-            c[3] += 1;
-        }
-    }
-    close_sweep(f, t, partial, scratch, g.V, tol, record, st, hist, hist_cap, ticket);
 }
 
 // ---- accumulated gauge transformation ------------------------------
@@ -508,7 +363,7 @@ __global__ void __launch_bounds__(1024) k_sum1(const double *__restrict__ partia
 
 __global__ void k_reset_state(DevState *st) {
     st->n_hist = 0; st->n_updates = 0; st->done = 0; st->nan = 0; st->F = 0.0; st->theta = 0.0; st->zero = 0;
-    st->cur = 0; st->ticket = 0;
+    st->cur = 0;
 }
 __global__ void k_clear_done(DevState *st) { st->done = 0; }
 
@@ -632,68 +487,6 @@ cudaError_t launch_sweep(int nr, LinkPair<R> links, const C<R> *G, C<R> *W, cons
     }
     return cudaGetLastError();
 }
-static int largest_div_le(int n, int cap) {
-    for (int d = (cap < n ? cap : n); d >= 1; d--)
-        if (n % d == 0) return d;
-    return 1;
-}
-// TX covers as much of an x line as fits a warp, TY / TZ share the remaining threads as evenly as the
-// divisors allow (the recomputed faces cost 1/TY + 1/TZ), TT is the longest march that still leaves the
-// grid a few waves deep.
-SweepTile choose_sweep_tile(const Geom &g, int tt_override) {
-    SweepTile tl{};
-    tl.T[0] = largest_div_le(g.L[0], 32);
-    const int rest = SWEEP_THREADS / tl.T[0];
-    int best_y = 1, best_z = 1;
-    double best_cost = 1e30;
-    for (int ty = 1; ty <= rest; ty++) {
-        if (g.L[1] % ty) continue;
-        const int tz = largest_div_le(g.L[2], rest / ty);
-        const double cost = (ty == g.L[1] ? 0.0 : 1.0 / ty) + (tz == g.L[2] ? 0.0 : 1.0 / tz) +
-                            4.0 * (double)(SWEEP_THREADS - tl.T[0] * ty * tz) / SWEEP_THREADS;   // idle threads
-        if (cost < best_cost - 1e-12) { best_cost = cost; best_y = ty; best_z = tz; }
-    }
-    tl.T[1] = best_y;
-    tl.T[2] = best_z;
-    tl.threads = tl.T[0] * tl.T[1] * tl.T[2];
-    const long long slices = (g.V / g.L[3]) / tl.threads;           // tiles per t slice
-    int tt = 1;
-    for (int cand = 1; cand <= g.L[3] && cand <= 16; cand++)
-        if (g.L[3] % cand == 0 && slices * (g.L[3] / cand) >= 4LL * 148 * 3) tt = cand;
-    if (tt_override > 0 && g.L[3] % tt_override == 0) tt = tt_override;
-    tl.T[3] = tt;
-    for (int mu = 0; mu < 4; mu++) tl.nt[mu] = g.L[mu] / tl.T[mu];
-    return tl;
-}
-
-template <class R>
-cudaError_t launch_sweep_tiled(int nr, LinkPair<R> links, const C<R> *G, C<R> *W, const Geom &g, const SweepTile &tl,
-                               double *partial, int *nblocks, DevState *st, double tol, int record, double *hist,
-                               long long hist_cap, cudaStream_t stream, int minb) {
-    const int nb = tl.nt[0] * tl.nt[1] * tl.nt[2] * tl.nt[3];
-    *nblocks = nb;
-    const int threads = (tl.threads + 31) / 32 * 32;
-    const size_t smem = sizeof(R) * 2 * 32 * (size_t)tl.threads;
-    switch (minb) {
-#define LGF_SW(M)                                                                                              \
-    case M: {                                                                                                  \
-        auto k3 = k_sweep_tiled<R, 3, M>;                                                                      \
-        auto k2 = k_sweep_tiled<R, 2, M>;                                                                      \
-        if (smem > 40 * 1024) {   /* static + dynamic may exceed the 48 KB default */                          \
-            cudaError_t e = cudaFuncSetAttribute(nr == 3 ? k3 : k2, cudaFuncAttributeMaxDynamicSharedMemorySize, \
-                                                 (int)smem);                                                   \
-            if (e != cudaSuccess) return e;                                                                    \
-        }                                                                                                      \
-        if (nr == 3) k3<<<nb, threads, smem, stream>>>(links, G, W, g, tl, partial, st, tol, record, hist, hist_cap, &st->ticket); \
-        else k2<<<nb, threads, smem, stream>>>(links, G, W, g, tl, partial, st, tol, record, hist, hist_cap, &st->ticket);         \
-        break;                                                                                                 \
-    }
-        LGF_SW(2) LGF_SW(3) LGF_SW(4)
-#undef LGF_SW
-        default: return cudaErrorInvalidValue;
-    }
-    return cudaGetLastError();
-}
 template <class R>
 cudaError_t launch_plaquette(int nr, LinkPair<R> links, const Geom &g, double *partial, int *nblocks,
                              const DevState *st, cudaStream_t stream) {
@@ -762,9 +555,6 @@ cudaError_t launch_clear_done(DevState *st, cudaStream_t stream) {
     template cudaError_t launch_gbuild<R>(const C<R> *, C<R> *, const Geom &, R, const DevState *, cudaStream_t);     \
     template cudaError_t launch_sweep<R>(int, LinkPair<R>, const C<R> *, C<R> *, const Geom &, double *, int *,       \
                                          const DevState *, cudaStream_t, int, bool, int, int);                                             \
-    template cudaError_t launch_sweep_tiled<R>(int, LinkPair<R>, const C<R> *, C<R> *, const Geom &, const SweepTile &, \
-                                               double *, int *, DevState *, double, int, double *, long long,         \
-                                               cudaStream_t, int);                                                         \
     template cudaError_t launch_plaquette<R>(int, LinkPair<R>, const Geom &, double *, int *, const DevState *,       \
                                              cudaStream_t);                                                           \
     template cudaError_t launch_convert_in<R>(int, const R *, C<R> *, const Geom &, cudaStream_t);                    \

@@ -18,17 +18,9 @@ struct DevState {
     int zero;             // always 0: the `stop` word handed to kernels that must run regardless of `done`
     int cur;              // which of the two link buffers holds the current configuration (0 / 1); the
                           // sweep reads buffer `cur` and writes the other one, k_finalize flips it
-    unsigned int ticket;  // CTAs of the running tiled sweep that have delivered their partial sums
 };
 
-// Tile of the tiled sweep (lgf_links.cu): TX x TY x TZ threads, marching TT slices in t.
-struct SweepTile {
-    int T[4];             // tile extents TX, TY, TZ (one thread per site) and TT (march length)
-    int nt[4];            // tiles per axis
-    int threads;          // TX * TY * TZ
-};
-// tile choice for a lattice (host)
-SweepTile choose_sweep_tile(const Geom &g, int tt_override);
+
 
 // The two link buffers (ping-pong: the fused sweep needs U_mu(x - mu) of the OLD configuration while
 // other threads already write the new one).
@@ -96,11 +88,6 @@ cudaError_t launch_sweep(int nr, LinkPair<R> links, const C<R> *G, C<R> *W, cons
                          int *nblocks, const DevState *st, cudaStream_t stream, int order_tz /* 0 auto, 1 plain */,
                          bool reunit /* project every new link onto SU(3) */, int minb /* CTAs per SM asked of the
                          register allocation: 2, 3 or 4 */, int share_mode /* A'_x, A'_y through shared memory: 1 / 0 / -1 = where it measured faster */);
-// tiled sweep with the finalize folded in (last CTA): record / tol / hist as for launch_finalize
-template <class R>
-cudaError_t launch_sweep_tiled(int nr, LinkPair<R> links, const C<R> *G, C<R> *W, const Geom &g, const SweepTile &tl,
-                               double *partial, int *nblocks, DevState *st, double tol, int record, double *hist,
-                               long long hist_cap, cudaStream_t stream, int minb);
 template <class R>
 cudaError_t launch_plaquette(int nr, LinkPair<R> links, const Geom &g, double *partial, int *nblocks,
                              const DevState *st, cudaStream_t stream);

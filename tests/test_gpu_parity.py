@@ -159,35 +159,6 @@ def test_update(lgf, name, dims, prec, storage):
     assert np.max(np.abs(out - U_o)) < (1e-13 if prec == 8 else 2e-6)
 
 
-@pytest.mark.parametrize("name,dims", SMALL + [("tiny", (2, 4, 2, 6)), ("long-t", (8, 4, 4, 32))])
-@pytest.mark.parametrize("prec,storage", [(8, 18), (4, 12)])
-@pytest.mark.parametrize("tt", [0, 2])
-def test_update_tiled_sweep(lgf, name, dims, prec, storage, tt):
-    """The tiled variant of the sweep (shared-memory neighbour exchange, t march, partial warps, periodic
-    wrap inside a tile): same links, Delta, F and theta as the oracle's transform + measure."""
-    import torch
-
-    U = small_config(name, dims)
-    w = 3.0 * random_herm_field(dims, 6)
-    U_o = oracle.transform(dims, U, oracle.build_g(dims, w, ALPHA))
-    D_o, F_o, T_o = oracle.measure(dims, U_o, want_delta=True)
-    with lgf.Context(dims, prec, storage) as ctx:
-        ctx.tune("sweep_tiled", 1)
-        ctx.tune("sweep_tt", tt)
-        d = to_dev(U, prec)
-        ctx.set_links(d)
-        ctx.set_field(to_dev(w, prec))
-        ctx.step_update(ALPHA)
-        field = to_np(ctx.get_field(torch.empty(site_shape(dims) + (3, 3), dtype=d.dtype, device="cuda")))
-        out = to_np(ctx.get_links(torch.empty_like(d)))
-        assert ctx.iterations() == 1
-        F, th, _ = ctx.measure(plaquette=False)
-    assert np.max(np.abs(out - U_o)) < (1e-13 if prec == 8 else 2e-6)
-    assert np.max(np.abs(field - D_o)) < (1e-12 if prec == 8 else 2e-5) * max(1.0, np.max(np.abs(D_o)))
-    assert abs(F - F_o) <= (1e-12 if prec == 8 else 1e-5) * abs(F_o)
-    assert abs(th - T_o) <= (1e-12 if prec == 8 else 1e-5) * abs(T_o)
-
-
 def run_trajectory(lgf, dims, U, prec, storage, n, tune=None):
     import torch
 
@@ -220,17 +191,6 @@ def test_trajectory_20(lgf, config_cache, cfg, prec, storage):
     assert np.max(np.abs(Th - T_o) / np.abs(T_o)) < tol["scalar"]
     assert np.max(np.abs(out - U_o)) < tol["links"]
     assert abs(P - oracle.plaquette(dims, U)) < (1e-13 if prec == 8 else 1e-6)      # gauge invariant
-
-
-def test_trajectory_tiled_sweep(lgf, config_cache):
-    """20 iterations of C2 with the tiled sweep: the same parity bar as the default path."""
-    dims = inputs.CONFIGS["C2"]["dims"]
-    U = config_cache("C2")
-    U_o, F_o, T_o = oracle.iterate(dims, U, ALPHA, 20)
-    Fh, Th, P, out = run_trajectory(lgf, dims, U, 8, 18, 20, tune={"sweep_tiled": 1})
-    assert np.max(np.abs(Fh - F_o) / np.abs(F_o)) < 1e-12
-    assert np.max(np.abs(Th - T_o) / np.abs(T_o)) < 1e-12
-    assert np.max(np.abs(out - U_o)) < 1e-11
 
 
 @pytest.mark.parametrize("prec,storage", VARIANTS)
