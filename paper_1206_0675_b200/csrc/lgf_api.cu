@@ -47,7 +47,6 @@ struct lgf_ctx {
     int tune_xy_planes = 0;      // lgf_tune: planes per CTA of the (x, y) pass (0 = planner's choice)
     int tune_zt_xc = 0;          // lgf_tune: consecutive (x, y) indices per CTA of the (z, t) pass
     int tune_fuse_g = 1;         // lgf_tune: end the last FFT sweep with the g-build (register-line plan only)
-    int tune_sweep_minb = 3;     // lgf_tune: resident CTAs per SM the sweep's register allocation is asked to allow
     int tune_sweep_share = -1;   // lgf_tune: hand A'_x, A'_y to the forward neighbours of the same CTA through shared
                                  // memory (1 / 0; -1 = automatic: 18-real and fp32 or a lattice beyond L2)
     int tune_reunit = 0;         // lgf_tune "reunit_every": project the new links onto SU(3) in every N-th update (0 = never)
@@ -367,8 +366,7 @@ static int step_update(lgf_ctx *ctx, double alpha, double tol, int record, bool 
     {
         Bracket br(ctx, LGF_K_UPDATE);
         CK(launch_sweep<R>(ctx->nr, link_pair<R>(ctx), (const C<R> *)ctx->G, (C<R> *)ctx->W, ctx->g, ctx->partial,
-                           &ctx->nb_partial, ctx->st, ctx->stream, ctx->tune_sweep_tz, reunit, ctx->tune_sweep_minb,
-                           ctx->tune_sweep_share));
+                           &ctx->nb_partial, ctx->st, ctx->stream, ctx->tune_sweep_tz, reunit, ctx->tune_sweep_share));
     }
     return step_finalize(ctx, tol, 1, record);
 }
@@ -868,10 +866,6 @@ int lgf_tune(lgf_ctx *ctx, const char *key, int value) {
     else if (k == "fft_reg2") ctx->tune_reg2 = value;
     else if (k == "fft_xy_planes") ctx->tune_xy_planes = value;
     else if (k == "fft_zt_xc") ctx->tune_zt_xc = value;
-    else if (k == "sweep_minb") {
-        if (value < 2 || value > 4) return fail(ctx, LGF_EINVAL, "lgf_tune: sweep_minb must be 2, 3 or 4");
-        ctx->tune_sweep_minb = value;
-    }
     else if (k == "fuse_g") ctx->tune_fuse_g = value;
     else if (k == "sweep_tz") ctx->tune_sweep_tz = value;
     else if (k == "sweep_share") ctx->tune_sweep_share = value;

@@ -167,8 +167,11 @@ __device__ __forceinline__ Herm<R> herm_from_smem(const R *__restrict__ slot, in
 // just computed the very A'_mu the site needs.  Those two are handed over through shared memory (one barrier
 // per CTA, flat indexing) instead of being recomputed; neighbours outside the CTA, and z and t, are recomputed
 // as before.  At 32^4: 6.25 link transforms per site instead of 8.
-template <class R, int NR, int MINB, bool REUNIT, bool SHARE>
-__global__ void __launch_bounds__(SWEEP_THREADS, MINB)
+// The register allocation is asked to allow 3 CTAs per SM: 168 registers, no spills in fp64 / 18-real (2 would
+// allow 255 registers at 8 warps per SM, 4 would force spills at 128).
+constexpr int SWEEP_MINB = 3;
+template <class R, int NR, bool REUNIT, bool SHARE>
+__global__ void __launch_bounds__(SWEEP_THREADS, SWEEP_MINB)
     k_sweep(LinkPair<R> lp, const C<R> *__restrict__ G, C<R> *__restrict__ W, Geom g, double *__restrict__ partial,
             const DevState *__restrict__ st, BlockOrder bo) {
     if (st->done) return;
@@ -443,8 +446,7 @@ cudaError_t launch_gbuild(const C<R> *W, C<R> *G, const Geom &g, R half_alpha, c
 }
 template <class R>
 cudaError_t launch_sweep(int nr, LinkPair<R> links, const C<R> *G, C<R> *W, const Geom &g, double *partial,
-                         int *nblocks, const DevState *st, cudaStream_t stream, int order_tz, bool reunit, int minb,
-                         int share_mode) {
+                         int *nblocks, const DevState *st, cudaStream_t stream, int order_tz, bool reunit, int share_mode) {
     const int nb = (int)((g.V + SWEEP_THREADS - 1) / SWEEP_THREADS);
     *nblocks = nb;
     // (z, t)-tiled block order when the (x, y) plane is a whole number of CTAs; TZ: about 24 MB of traffic
@@ -469,22 +471,14 @@ cudaError_t launch_sweep(int nr, LinkPair<R> links, const C<R> *G, C<R> *W, cons
         }
         if (tz > 1 && g.L[2] % tz == 0) { bo.nxy = (int)(plane / SWEEP_THREADS); bo.tz = tz; }
     }
-    switch (minb) {
-#define LGF_SWK(M, RU, SH)                                                                                  \
-    if (nr == 3) k_sweep<R, 3, M, RU, SH><<<nb, SWEEP_THREADS, 0, stream>>>(links, G, W, g, partial, st, bo); \
-    else k_sweep<R, 2, M, RU, SH><<<nb, SWEEP_THREADS, 0, stream>>>(links, G, W, g, partial, st, bo);
-#define LGF_SW(M)                                                  \
-    case M:                                                        \
-        if (reunit && share) { LGF_SWK(M, true, true) }            \
-        else if (reunit) { LGF_SWK(M, true, false) }               \
-        else if (share) { LGF_SWK(M, false, true) }                \
-        else { LGF_SWK(M, false, false) }                          \
-        break;
-        LGF_SW(2) LGF_SW(3) LGF_SW(4)
-#undef LGF_SW
+#define LGF_SWK(RU, SH)                                                                                  \
+    if (nr == 3) k_sweep<R, 3, RU, SH><<<nb, SWEEP_THREADS, 0, stream>>>(links, G, W, g, partial, st, bo); \
+    else k_sweep<R, 2, RU, SH><<<nb, SWEEP_THREADS, 0, stream>>>(links, G, W, g, partial, st, bo);
+    if (reunit && share) { LGF_SWK(true, true) }
+    else if (reunit) { LGF_SWK(true, false) }
+    else if (share) { LGF_SWK(false, true) }
+    else { LGF_SWK(false, false) }
 #undef LGF_SWK
-        default: return cudaErrorInvalidValue;
-    }
     return cudaGetLastError();
 }
 template <class R>
@@ -554,7 +548,7 @@ cudaError_t launch_clear_done(DevState *st, cudaStream_t stream) {
                                          const DevState *, cudaStream_t);                                             \
     template cudaError_t launch_gbuild<R>(const C<R> *, C<R> *, const Geom &, R, const DevState *, cudaStream_t);     \
     template cudaError_t launch_sweep<R>(int, LinkPair<R>, const C<R> *, C<R> *, const Geom &, double *, int *,       \
-                                         const DevState *, cudaStream_t, int, bool, int, int);                                             \
+                                         const DevState *, cudaStream_t, int, bool, int);                                             \
     template cudaError_t launch_plaquette<R>(int, LinkPair<R>, const Geom &, double *, int *, const DevState *,       \
                                              cudaStream_t);                                                           \
     template cudaError_t launch_convert_in<R>(int, const R *, C<R> *, const Geom &, cudaStream_t);                    \

@@ -86,8 +86,8 @@ cudaError_t launch_gbuild(const C<R> *W, C<R> *G, const Geom &g, R half_alpha, c
 template <class R>
 cudaError_t launch_sweep(int nr, LinkPair<R> links, const C<R> *G, C<R> *W, const Geom &g, double *partial,
                          int *nblocks, const DevState *st, cudaStream_t stream, int order_tz /* 0 auto, 1 plain */,
-                         bool reunit /* project every new link onto SU(3) */, int minb /* CTAs per SM asked of the
-                         register allocation: 2, 3 or 4 */, int share_mode /* A'_x, A'_y through shared memory: 1 / 0 / -1 = where it measured faster */);
+                         bool reunit /* project every new link onto SU(3) */,
+                         int share_mode /* A'_x, A'_y through shared memory: 1 / 0 / -1 = where it measured faster */);
 template <class R>
 cudaError_t launch_plaquette(int nr, LinkPair<R> links, const Geom &g, double *partial, int *nblocks,
                              const DevState *st, cudaStream_t stream);
