@@ -107,6 +107,15 @@ def dft4d(dims, f, sign: int):
     return out
 
 
+def gluon_field(dims, U, mu: int):
+    """A_mu(k) = sum_x exp(-2 pi i k.x/L) A_mu(x), unnormalised: shape (Lt, Lz, Ly, Lx, 3, 3) indexed by (kt, kz, ky, kx)."""
+    dims, cd = _dims(dims)
+    U = _c128(U, _site_shape(dims) + (4, 3, 3))
+    Ak = np.empty(_site_shape(dims) + (3, 3), np.complex128)
+    _load().orc_gluon_field(cd, _ptr(U), int(mu), _ptr(Ak))
+    return Ak
+
+
 def p2(dims, k):
     dims, cd = _dims(dims)
     return float(_load().orc_p2(cd, (ctypes.c_int * 4)(*[int(v) for v in k])))

@@ -225,6 +225,26 @@ void orc_dft4d(const int L[4], const cplx *in, int sign, cplx *out)
     free(b);
 }
 
+/* Gluon field in momentum space (the quantity gauge-fixed configurations are
+ * made for):  Ak[k][i][j] = sum_x exp(-2 pi i sum_nu k_nu x_nu / L_nu) A_mu(x)_ij  with A_mu(x) the
+ * hermitian traceless algebra part of U_mu(x) (eq. 7 as read in R1, R4), k = kx + Lx (ky + Ly (kz + Lz kt)),
+ * unnormalised, the link's field taken at the site x (no mid-point phase exp(-i pi k_mu / L_mu)).
+ * With this convention eq. 5 reads  F[Delta](k) = sum_mu (exp(-2 pi i k_mu / L_mu) - 1) Ak_mu(k). */
+void orc_gluon_field(const int L[4], const cplx *U, int mu, cplx *Ak)
+{
+    const long V = volume(L);
+    cplx *f = (cplx *)malloc(sizeof(cplx) * V);
+    cplx *g = (cplx *)malloc(sizeof(cplx) * V);
+    cplx *A = (cplx *)malloc(sizeof(cplx) * V * 9);
+    for (long s = 0; s < V; s++) algebra_part(U + (s * 4 + mu) * 9, A + s * 9);
+    for (int e = 0; e < 9; e++) {
+        for (long s = 0; s < V; s++) f[s] = A[s * 9 + e];
+        orc_dft4d(L, f, -1, g);
+        for (long s = 0; s < V; s++) Ak[s * 9 + e] = g[s];
+    }
+    free(f); free(g); free(A);
+}
+
 /* p^2(k) = 4 sum_mu sin^2(pi k_mu / L_mu): eigenvalues of the lattice -d^2 (R5) */
 double orc_p2(const int L[4], const int k[4])
 {

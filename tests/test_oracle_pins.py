@@ -427,3 +427,54 @@ def test_accumulated_transformation_carries_U0_to_Un():
     # the other order of the product is NOT the transformation (the g_k do not commute)
     assert np.max(np.abs(G @ np.conj(np.swapaxes(G, -1, -2)) - np.eye(3))) < 1e-14
     assert np.max(np.abs(np.linalg.det(G) - 1)) < 1e-14
+
+
+def _phase_minus_one(dims, mu):
+    """exp(-2 pi i k_mu / L_mu) - 1 on the (kt, kz, ky, kx) grid."""
+    L = dims[mu]
+    ph = np.exp(-2j * np.pi * np.arange(L) / L) - 1.0
+    shape = [1, 1, 1, 1]
+    shape[3 - mu] = L
+    return ph.reshape(shape + [1, 1])
+
+
+def test_gluon_field_divergence_identity_and_symmetries():
+    """NEXT-2: A_mu(k).  From eq. 5, F[Delta](k) = sum_mu (exp(-2 pi i k_mu/L_mu) - 1) A_mu(k) for ANY configuration
+    -- it ties the new function to the pinned Delta and the pinned DFT (sign of the shift, site convention,
+    normalisation).  A_mu(x) hermitian traceless  =>  A_mu(-k) = A_mu(k)^dag, tr A_mu(k) = 0."""
+    dims = (4, 6, 2, 8)
+    U = inputs.smooth_config(dims, 0.4, 58, haar=True)
+    Delta, _, _ = oracle.measure(dims, U)
+    lhs = np.stack([oracle.dft4d(dims, np.ascontiguousarray(Delta[..., i, j]), -1) for i in range(3) for j in range(3)],
+                   axis=-1).reshape(Delta.shape)
+    A = [oracle.gluon_field(dims, U, mu) for mu in range(4)]
+    rhs = sum(_phase_minus_one(dims, mu) * A[mu] for mu in range(4))
+    assert np.max(np.abs(lhs - rhs)) < 1e-11 * max(1.0, np.max(np.abs(lhs)))
+    for mu in range(4):
+        Am = A[mu]
+        minus_k = np.roll(Am[::-1, ::-1, ::-1, ::-1], 1, axis=(0, 1, 2, 3))          # A(-k)
+        assert np.max(np.abs(minus_k - np.conj(np.swapaxes(Am, -1, -2)))) < 1e-11
+        assert np.max(np.abs(np.trace(Am, axis1=-2, axis2=-1))) < 1e-11
+    # k = 0 is the plain lattice sum; constant links give a single non-zero mode
+    const = np.broadcast_to(U[0, 0, 0, 0], U.shape).copy()
+    Ac = oracle.gluon_field(dims, const, 1)
+    assert np.max(np.abs(Ac.reshape(-1, 3, 3)[1:])) < 1e-10 and np.max(np.abs(Ac[0, 0, 0, 0])) > 1.0
+
+
+def test_gluon_field_is_transverse_in_landau_gauge():
+    """What the gauge fixing is for: after Algorithm 1 has driven theta below 1e-15 the lattice divergence of the
+    gluon field vanishes mode by mode, sum_mu (exp(-2 pi i k_mu/L_mu) - 1) A_mu(k) = 0, while before it does not."""
+    dims = (4, 4, 4, 8)
+    U = inputs.smooth_config(dims, 0.3, 59, haar=True)
+    V = int(np.prod(dims))
+
+    def div(Ucfg):
+        return sum(_phase_minus_one(dims, mu) * oracle.gluon_field(dims, Ucfg, mu) for mu in range(4))
+
+    before = np.abs(div(U)).max()
+    Ufix, it, F, th = oracle.fix(dims, U, 0.08, 1e-15, 2000)
+    after = div(Ufix)
+    assert th[-1] < 1e-15 and before > 1.0
+    # Parseval: sum_k |F[Delta](k)|^2 = V sum_x |Delta(x)|^2 = V * 3 V theta
+    assert abs(np.sum(np.abs(after) ** 2) - 3.0 * V * V * th[-1]) < 1e-3 * 3.0 * V * V * th[-1] + 1e-20
+    assert np.abs(after).max() < np.sqrt(3.0 * V * V * 1e-15)
