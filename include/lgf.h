@@ -156,6 +156,17 @@ int lgf_track_transform(lgf_ctx *ctx, int on);
  * [Lt, Lz, Ly, Lx, 3, 3] complex).  LGF_ESTATE if tracking is off.  Asynchronous on the context's stream. */
 int lgf_get_transform(lgf_ctx *ctx, void *d_transform);
 
+/* Gluon field of direction mu (0..3) in momentum space -- what a Landau-gauge configuration is fixed for
+ * (gluon propagator):
+ *   d_out[k][i][j] = sum_x exp(-2 pi i sum_nu k_nu x_nu / L_nu) A_mu(x)_ij,   k = kx + Lx (ky + Ly (kz + Lz kt)),
+ * A_mu(x) the hermitian traceless algebra part of the current U_mu(x) (eq. 7), unnormalised, the link's field
+ * taken at the site x (multiply by exp(-i pi k_mu / L_mu) for the mid-point convention); 18 reals per k in the
+ * context's precision (as a torch tensor: [Lt, Lz, Ly, Lx, 3, 3] complex indexed by (kt, kz, ky, kx)).
+ * With this convention eq. 5 reads F[Delta](k) = sum_mu (exp(-2 pi i k_mu / L_mu) - 1) A_mu(k): in Landau gauge
+ * the field is transverse mode by mode.  Uses the work field (a following lgf_iterate recomputes Delta).
+ * Asynchronous. */
+int lgf_gluon_field(lgf_ctx *ctx, int mu, void *d_out);
+
 /* Apply a given gauge transformation to the internal configuration: U_mu(x) <- G(x) U_mu(x) G(x + mu)^dag
  * (eq. 2) with d_transform[s][i][j][re/im] in the layout lgf_get_transform writes (18 reals per
  * site, the context's precision).  Each G(x) is first projected onto SU(3) (Gram-Schmidt on rows 0, 1, row 2

@@ -54,6 +54,7 @@ SIGNATURES = {
     "lgf_overrelax": (_i, [_vp, _i]),
     "lgf_track_transform": (_i, [_vp, _i]),
     "lgf_get_transform": (_i, [_vp, _vp]),
+    "lgf_gluon_field": (_i, [_vp, _i, _vp]),
     "lgf_apply_transform": (_i, [_vp, _vp]),
     "lgf_tune": (_i, [_vp, ctypes.c_char_p, _i]),
     "lgf_fft_passes": (_i, [_vp]),
@@ -251,6 +252,10 @@ class Context:
 
     def get_transform(self, out):
         _check(self._h, load().lgf_get_transform(self._h, _dev_ptr(out, self.precision, self.V * 18)))
+        return out
+
+    def gluon_field(self, mu, out):
+        _check(self._h, load().lgf_gluon_field(self._h, int(mu), _dev_ptr(out, self.precision, self.V * 18)))
         return out
 
     def apply_transform(self, transform):

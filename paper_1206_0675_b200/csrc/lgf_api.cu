@@ -161,30 +161,35 @@ static long long pow2_divisor_le(long long n, long long cap) {
 // scale + inverse, (x, y) planes inverse -- when two-axis kernels exist for the lattice's lengths and
 // the tiles fit in shared memory; otherwise one pass per axis (forward x, y, z; forward + scale +
 // inverse on t; inverse z, y, x).  tune_xy_planes / tune_zt_xc (> 0) override the tile sizes.
-static int plan_passes(lgf_ctx *ctx) {
-    const long long T = 2048;     // target complex elements per tile of the one-axis passes
+// one in-place shared-memory pass over one axis (k_fft_axis; any supported length)
+static AxisPass make_axis_pass(const lgf_ctx *ctx, int axis, int mode) {
+    const long long T = 2048;     // target complex elements per tile
     const size_t cbytes = 2 * (size_t)ctx->prec;
     const Geom &g = ctx->g;
-    auto make = [&](int axis, int mode) {
-        AxisPass p{};
-        p.kind = PASS_AXIS;
-        p.axis = axis;
-        p.L = g.L[axis];
-        p.mode = mode;
-        p.S = g.S[axis];
-        p.H = g.V / (p.S * p.L);
-        if (p.S == 1) {
-            p.nlo = 1;
-            p.nhi = (int)largest_divisor_le(p.H, T / p.L);
-            p.smem = (64 + (size_t)p.nhi * (p.L | 1)) * cbytes;
-        } else {
-            p.nlo = (int)largest_divisor_le(p.S, T / p.L);
-            p.nhi = (int)largest_divisor_le(p.H, T / ((long long)p.L * p.nlo));
-            p.smem = (64 + (size_t)p.nhi * p.L * p.nlo) * cbytes;
-        }
-        p.threads = 256;
-        return p;
-    };
+    AxisPass p{};
+    p.kind = PASS_AXIS;
+    p.axis = axis;
+    p.L = g.L[axis];
+    p.mode = mode;
+    p.S = g.S[axis];
+    p.H = g.V / (p.S * p.L);
+    if (p.S == 1) {
+        p.nlo = 1;
+        p.nhi = (int)largest_divisor_le(p.H, T / p.L);
+        p.smem = (64 + (size_t)p.nhi * (p.L | 1)) * cbytes;
+    } else {
+        p.nlo = (int)largest_divisor_le(p.S, T / p.L);
+        p.nhi = (int)largest_divisor_le(p.H, T / ((long long)p.L * p.nlo));
+        p.smem = (64 + (size_t)p.nhi * p.L * p.nlo) * cbytes;
+    }
+    p.threads = 256;
+    return p;
+}
+
+static int plan_passes(lgf_ctx *ctx) {
+    const size_t cbytes = 2 * (size_t)ctx->prec;
+    const Geom &g = ctx->g;
+    auto make = [&](int axis, int mode) { return make_axis_pass(ctx, axis, mode); };
     auto finish = [&](const bool natural[4]) {
         return ctx->prec == LGF_FP64 ? upload_p2<double>(ctx, natural) : upload_p2<float>(ctx, natural);
     };
@@ -423,6 +428,30 @@ static int apply_transform(lgf_ctx *ctx, const void *d_transform) {
     ctx->w_is_delta = true;                                  // ... whose Delta and partial sums the sweep has left behind
     ctx->recorded = false;
     ctx->updates_enqueued = 0;
+    return LGF_OK;
+}
+
+// A_mu(k): packed algebra part of direction mu into W, forward transform with one pass per axis (works on every
+// supported lattice; leaves each axis in the permuted order of the two-step line transform), unpack to natural
+// order.  W is overwritten.
+template <class R>
+static int gluon_field(lgf_ctx *ctx, int mu, void *d_out) {
+    ctx->launches++;
+    CK(launch_algebra<R>(ctx->nr, link_pair<R>(ctx), (C<R> *)ctx->W, ctx->g, mu, ctx->st, ctx->stream));
+    ctx->launches++;
+    CK(launch_clear_done(ctx->st, ctx->stream));          // the FFT passes return at once while `done` is set
+    const R *tw[4] = {(const R *)ctx->twiddle[0], (const R *)ctx->twiddle[1], (const R *)ctx->twiddle[2],
+                      (const R *)ctx->twiddle[3]};
+    int N1[4], N2[4];
+    for (int axis = 0; axis < 4; axis++) {
+        line_factor(ctx->g.L[axis], N1[axis], N2[axis]);
+        const AxisPass p = make_axis_pass(ctx, axis, FFT_FWD);
+        Bracket br(ctx, LGF_K_FFT);
+        CK(launch_fft_pass<R>(p, (C<R> *)ctx->W, ctx->g, tw, (const R *)ctx->p2tab, (R)1, ctx->st, ctx->stream));
+    }
+    ctx->launches++;
+    CK(launch_gluon_unpack<R>((const C<R> *)ctx->W, (R *)d_out, ctx->g, N1, N2, ctx->stream));
+    ctx->w_is_delta = false;
     return LGF_OK;
 }
 
@@ -850,6 +879,12 @@ int lgf_get_transform(lgf_ctx *ctx, void *d_transform) {
     else
         CK(launch_gacc<float>(2, nullptr, (C<float> *)ctx->Gacc, (float *)d_transform, ctx->g, ctx->st, ctx->stream));
     return LGF_OK;
+}
+
+int lgf_gluon_field(lgf_ctx *ctx, int mu, void *d_out) {
+    if (!ctx || !d_out || mu < 0 || mu > 3) return fail(ctx, LGF_EINVAL, "lgf_gluon_field: bad argument");
+    if (!ctx->have_links) return fail(ctx, LGF_ESTATE, "lgf_gluon_field: no configuration loaded");
+    return ctx->prec == LGF_FP64 ? gluon_field<double>(ctx, mu, d_out) : gluon_field<float>(ctx, mu, d_out);
 }
 
 int lgf_apply_transform(lgf_ctx *ctx, const void *d_transform) {

@@ -307,6 +307,54 @@ __global__ void __launch_bounds__(SITE_THREADS) k_gacc_get(const C<R> *__restric
     for (int e = 0; e < 9; e++) dst[e] = A[(long long)e * g.V + s];
 }
 
+// ---- gluon field in momentum space ---------------------------------
+// k_algebra: W <- packed A_mu(x), the hermitian traceless algebra part of the links of ONE direction (eq. 7).
+// k_gluon_unpack: after the forward transform of W (one pass per axis, lgf_fft.cu, which leaves position
+// p = N2 k1 + k2 of a line holding frequency k = k1 + N1 k2), rebuild the full 3 x 3 matrix A_mu(k) in natural
+// k order.  The packing put two REAL fields into W[3] = M00 + i M11 and kept only the upper off-diagonals, so
+//   A01(k) = W0(k), A10(k) = conj(W0(-k))   (M10(x) = conj(M01(x)));  likewise 02 / 20 from W1, 12 / 21 from W2;
+//   A00(k) = (W3(k) + conj(W3(-k))) / 2,  A11(k) = (W3(k) - conj(W3(-k))) / (2i),  A22 = -A00 - A11.
+template <class R, int NR>
+__global__ void __launch_bounds__(SITE_THREADS) k_algebra(LinkPair<R> lp, C<R> *__restrict__ W, Geom g, int mu,
+                                                           const DevState *__restrict__ st) {
+    const C<R> *__restrict__ links = lp.buf[st->cur];
+    const long long s = (long long)blockIdx.x * SITE_THREADS + threadIdx.x;
+    if (s >= g.V) return;
+    C<R> u[9];
+    load_link<R, NR>(links, g.V, mu, s, u);
+    store_herm(W, g.V, s, algebra_part(u));
+}
+struct AxisPerm {
+    int N1[4], N2[4];          // line factorisation of each axis (LineFactor<L>)
+};
+__device__ __forceinline__ long long kspace_pos(const Geom &g, const AxisPerm &pm, const int (&k)[4]) {
+    long long p = 0;
+#pragma unroll
+    for (int mu = 0; mu < 4; mu++) p += g.S[mu] * (long long)(pm.N2[mu] * (k[mu] % pm.N1[mu]) + k[mu] / pm.N1[mu]);
+    return p;
+}
+template <class R>
+__global__ void __launch_bounds__(SITE_THREADS) k_gluon_unpack(const C<R> *__restrict__ W, R *__restrict__ out, Geom g,
+                                                                AxisPerm pm) {
+    const long long s = (long long)blockIdx.x * SITE_THREADS + threadIdx.x;      // natural k index
+    if (s >= g.V) return;
+    int k[4], m[4];
+    site_coords(g, s, k);
+#pragma unroll
+    for (int mu = 0; mu < 4; mu++) m[mu] = k[mu] == 0 ? 0 : g.L[mu] - k[mu];         // -k
+    const long long pk = kspace_pos(g, pm, k), pm_k = kspace_pos(g, pm, m);
+    const C<R> w0 = W[pk], w1 = W[g.V + pk], w2 = W[2 * g.V + pk], w3 = W[3 * g.V + pk];
+    const C<R> c0 = conj(W[pm_k]), c1 = conj(W[g.V + pm_k]), c2 = conj(W[2 * g.V + pm_k]), c3 = conj(W[3 * g.V + pm_k]);
+    const R h = (R)0.5;
+    const C<R> a00 = h * (w3 + c3);
+    const C<R> dif = h * (w3 - c3);
+    const C<R> a11 = mk<R>(dif.y, -dif.x);                                            // dif / i
+    C<R> *dst = reinterpret_cast<C<R> *>(out) + s * 9;
+    dst[0] = a00; dst[1] = w0; dst[2] = w1;
+    dst[3] = c0; dst[4] = a11; dst[5] = w2;
+    dst[6] = c1; dst[7] = c2; dst[8] = mk<R>(-a00.x - a11.x, -a00.y - a11.y);
+}
+
 // ---- plaquette ------------------------------------------------------------------------------------
 template <class R, int NR>
 __global__ void __launch_bounds__(SITE_THREADS) k_plaquette(LinkPair<R> lp, Geom g, double *__restrict__ partial,
@@ -515,6 +563,20 @@ cudaError_t launch_gacc(int op, const C<R> *G, C<R> *A, R *out, const Geom &g, c
     return cudaGetLastError();
 }
 template <class R>
+cudaError_t launch_algebra(int nr, LinkPair<R> links, C<R> *W, const Geom &g, int mu, const DevState *st, cudaStream_t stream) {
+    const int nb = site_blocks(g);
+    if (nr == 3) k_algebra<R, 3><<<nb, SITE_THREADS, 0, stream>>>(links, W, g, mu, st);
+    else k_algebra<R, 2><<<nb, SITE_THREADS, 0, stream>>>(links, W, g, mu, st);
+    return cudaGetLastError();
+}
+template <class R>
+cudaError_t launch_gluon_unpack(const C<R> *W, R *out, const Geom &g, const int N1[4], const int N2[4], cudaStream_t stream) {
+    AxisPerm pm;
+    for (int mu = 0; mu < 4; mu++) { pm.N1[mu] = N1[mu]; pm.N2[mu] = N2[mu]; }
+    k_gluon_unpack<R><<<site_blocks(g), SITE_THREADS, 0, stream>>>(W, out, g, pm);
+    return cudaGetLastError();
+}
+template <class R>
 cudaError_t launch_field_get(const C<R> *W, R *field, const Geom &g, cudaStream_t stream) {
     k_field_get<R><<<site_blocks(g), SITE_THREADS, 0, stream>>>(W, field, g);
     return cudaGetLastError();
@@ -554,6 +616,8 @@ cudaError_t launch_clear_done(DevState *st, cudaStream_t stream) {
     template cudaError_t launch_convert_in<R>(int, const R *, C<R> *, const Geom &, cudaStream_t);                    \
     template cudaError_t launch_convert_out<R>(int, LinkPair<R>, R *, const Geom &, const DevState *, cudaStream_t);  \
     template cudaError_t launch_gacc<R>(int, const C<R> *, C<R> *, R *, const Geom &, const DevState *, cudaStream_t); \
+    template cudaError_t launch_algebra<R>(int, LinkPair<R>, C<R> *, const Geom &, int, const DevState *, cudaStream_t); \
+    template cudaError_t launch_gluon_unpack<R>(const C<R> *, R *, const Geom &, const int[4], const int[4], cudaStream_t); \
     template cudaError_t launch_field_get<R>(const C<R> *, R *, const Geom &, cudaStream_t);                          \
     template cudaError_t launch_field_set<R>(C<R> *, const R *, const Geom &, cudaStream_t);
 LGF_INST(float)

@@ -100,6 +100,11 @@ cudaError_t launch_convert_out(int nr, LinkPair<R> links, R *canon, const Geom &
 // 3 = (A = G, out = canonical input field) rows 0, 1 of the SU(3) projection of a given transformation into G
 template <class R>
 cudaError_t launch_gacc(int op, const C<R> *G, C<R> *A, R *out, const Geom &g, const DevState *st, cudaStream_t stream);
+// gluon field: W <- packed A_mu(x) of one direction; unpack of its forward transform into natural-order 3 x 3 A_mu(k)
+template <class R>
+cudaError_t launch_algebra(int nr, LinkPair<R> links, C<R> *W, const Geom &g, int mu, const DevState *st, cudaStream_t stream);
+template <class R>
+cudaError_t launch_gluon_unpack(const C<R> *W, R *out, const Geom &g, const int N1[4], const int N2[4], cudaStream_t stream);
 template <class R>
 cudaError_t launch_field_get(const C<R> *W, R *field, const Geom &g, cudaStream_t stream);
 template <class R>

@@ -437,6 +437,65 @@ def test_reunit_holds_fp32_links_on_su3(lgf, storage):
     assert res[10][2] < 1e-3 and 0.5 < res[10][2] / res[0][2] < 2.0
 
 
+@pytest.mark.parametrize("dims", [(8, 8, 8, 8), (12, 6, 16, 4), (3, 24, 2, 48), (16, 16, 16, 16), (6, 4, 32, 2)])
+@pytest.mark.parametrize("prec,storage", [(8, 18), (8, 12), (4, 18)])
+def test_gluon_field(lgf, dims, prec, storage):
+    """lgf_gluon_field: A_mu(k) for every direction against the oracle (naive DFT of the algebra part), natural k
+    order out of the permuted order the one-axis passes leave, both halves of the packed real fields."""
+    import torch
+
+    U = inputs.smooth_config(dims, 0.35, 808, haar=True)
+    cdt = torch.complex128 if prec == 8 else torch.complex64
+    with lgf.Context(dims, prec, storage) as ctx:
+        d = to_dev(U, prec)
+        ctx.set_links(d)
+        ctx.iterate(ALPHA, 1)                                   # W holds Delta: the call must not depend on that
+        U1 = to_np(ctx.get_links(torch.empty_like(d)))
+        got = [to_np(ctx.gluon_field(mu, torch.empty(site_shape(dims) + (3, 3), dtype=cdt, device="cuda")))
+               for mu in range(4)]
+        ctx.iterate(ALPHA, 1)                                   # ... and the iteration must still work after it
+        assert ctx.history_length() == 3
+        Fh, Th = ctx.history()
+    _, F_o, T_o = oracle.iterate(dims, U, ALPHA, 2)
+    rel = 1e-12 if prec == 8 else 1e-5
+    assert np.max(np.abs(Th - T_o) / T_o) < rel and np.max(np.abs(Fh - F_o) / np.abs(F_o)) < rel
+    for mu in range(4):
+        ref = oracle.gluon_field(dims, U1, mu)
+        scale = np.max(np.abs(ref))
+        assert np.max(np.abs(got[mu] - ref)) < (1e-12 if prec == 8 else 2e-5) * scale, "mu = %d" % mu
+
+
+def test_gluon_field_is_transverse_after_fixing(lgf, config_cache):
+    """The point of it all, on the CUDA path's own output: fix C2 to theta < 1e-15, then
+    sum_mu (exp(-2 pi i k_mu/L_mu) - 1) A_mu(k) = F[Delta](k) vanishes mode by mode (Parseval: 3 V^2 theta)."""
+    import torch
+
+    dims = inputs.CONFIGS["C2"]["dims"]
+    V = int(np.prod(dims))
+    U = config_cache("C2")
+
+    def divergence(ctx):
+        tot = 0
+        for mu in range(4):
+            A = to_np(ctx.gluon_field(mu, torch.empty(site_shape(dims) + (3, 3), dtype=torch.complex128, device="cuda")))
+            ph = np.exp(-2j * np.pi * np.arange(dims[mu]) / dims[mu]) - 1.0
+            shape = [1, 1, 1, 1, 1, 1]
+            shape[3 - mu] = dims[mu]
+            tot = tot + ph.reshape(shape) * A
+        return tot
+
+    with lgf.Context(dims, 8, 18) as ctx:
+        d = to_dev(U, 8)
+        ctx.set_links(d)
+        before = np.abs(divergence(ctx)).max()
+        it = ctx.fix(d, ALPHA, 1e-15, 2000)
+        after = divergence(ctx)
+        _, th, _ = ctx.measure(plaquette=False)
+    assert 0 < it < 2000 and th < 1e-15 and before > 1.0
+    assert abs(np.sum(np.abs(after) ** 2) - 3.0 * V * V * th) < 1e-3 * 3.0 * V * V * th
+    assert np.abs(after).max() < np.sqrt(3.0 * V * V * 1e-15)
+
+
 @pytest.mark.parametrize("dims", [(8, 8, 8, 8), (12, 6, 16, 4)])
 @pytest.mark.parametrize("prec,storage", [(8, 18), (8, 12), (4, 18)])
 def test_apply_transform(lgf, dims, prec, storage):
