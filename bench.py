@@ -322,12 +322,13 @@ def run_thermal(args):
 
     torch.cuda.set_device(0)
     binding.load()
-    dims, prec = (32, 32, 32, 32), PREC[args.precision]
+    L = int(args.thermal_size)
+    dims, prec = (L, L, L, L), PREC[args.precision]
     cdt = torch.complex128 if prec == 8 else torch.complex64
     stream = torch.cuda.current_stream()
     with binding.Context(dims, prec, args.storage, stream=stream) as ctx:
         ctx.tune("reunit_every", args.reunit_every)
-        cold = torch.zeros((32, 32, 32, 32, 4, 3, 3), dtype=cdt, device="cuda")
+        cold = torch.zeros((L, L, L, L, 4, 3, 3), dtype=cdt, device="cuda")
         for i in range(3):
             cold[..., i, i] = 1
         ctx.set_links(cold)
@@ -348,7 +349,11 @@ def run_thermal(args):
         _, theta0, P0 = ctx.measure()
         links = ctx.get_links(torch.empty_like(cold))
         ctx_thermalised = links.clone() if args.mixed else None
-        dev0 = float((links @ links.conj().transpose(-1, -2) - torch.eye(3, dtype=cdt, device="cuda")).abs().max())
+        dev0 = 0.0                                        # deviation from SU(3), one t slice at a time (64^4: 9.7 GB)
+        eye = torch.eye(3, dtype=cdt, device="cuda")
+        for t in range(L):
+            sl = links[t]
+            dev0 = max(dev0, float((sl @ sl.conj().transpose(-1, -2) - eye).abs().max()))
         tol = 1e-15 if prec == 8 else 1e-12
         torch.cuda.synchronize()
         t0 = time.perf_counter()
@@ -372,7 +377,7 @@ def run_thermal(args):
             c32.tune("reunit_every", 20)
             c32.track_transform(True)
             it32 = c32.fix(thermalised.to(torch.complex64), args.alpha, 1e-12, args.thermal_max_iter)
-            G32 = c32.get_transform(torch.empty((32, 32, 32, 32, 3, 3), dtype=torch.complex64, device="cuda"))
+            G32 = c32.get_transform(torch.empty((L, L, L, L, 3, 3), dtype=torch.complex64, device="cuda"))
         with binding.Context(dims, binding.LGF_FP64, args.storage, stream=stream) as c64:
             c64.set_links(thermalised)
             c64.apply_transform(G32.to(torch.complex128))
@@ -386,7 +391,7 @@ def run_thermal(args):
                  "speedup_vs_fp64_only": sec / sec_mixed}
     peak, _ = measured_peak()
     print(json.dumps({
-        "mode": "thermal", "beta": args.thermal, "lattice": "32x32x32x32", "precision": args.precision,
+        "mode": "thermal", "beta": args.thermal, "lattice": "x".join([str(L)] * 4), "precision": args.precision,
         "link_storage": args.storage, "alpha": args.alpha, "reunit_every": args.reunit_every,
         "heatbath_sweeps": args.thermal_sweeps, "overrelax_per_heatbath": args.thermal_overrelax,
         "seed": args.thermal_seed, "heatbath_ms_per_sweep": ms_sweep,
@@ -424,6 +429,7 @@ def main():
     ap.add_argument("--reference-budget", type=float, default=240.0)
     ap.add_argument("--thermal", type=float, default=None, metavar="BETA",
                     help="thermalise a cold 32^4 lattice at BETA and gauge-fix it (own JSON line, not the contract line)")
+    ap.add_argument("--thermal-size", type=int, default=32, choices=[8, 16, 32, 64], help="lattice extent L of --thermal (L^4)")
     ap.add_argument("--thermal-sweeps", type=int, default=300)
     ap.add_argument("--thermal-seed", type=int, default=1234)
     ap.add_argument("--thermal-overrelax", type=int, default=0, help="overrelaxation sweeps after each heat-bath sweep")
