@@ -13,7 +13,9 @@
  * hermiticity/tracelessness/zero-sum of Delta, hand-computed single-link case, the first-order
  * identity dF = (alpha/2)/(12V) sum tr[w Delta], the abelian contraction ratio (1-8 alpha)^2,
  * library QR for the Gram-Schmidt projection, plaquette invariance, the pure-gauge closed form
- * (F -> 1, theta -> 0).  Parity status: no function here is "parity unpinned" except the
+ * (F -> 1, theta -> 0); for orc_gluon_field the identity F[Delta](k) = sum_mu (exp(-2 pi i k_mu/L_mu) - 1) A_mu(k)
+ * against the pinned Delta and DFT, hermiticity in k space and transversality after fixing; for the product of
+ * the g fields the defining property G U0 G(x+mu)^dag = U_n.  Parity status: no function here is "parity unpinned" except the
  * iteration COUNTS on the synthetic configurations (the paper prints none for inputs we have).
  *
  * Conventions:
