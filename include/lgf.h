@@ -186,7 +186,9 @@ int lgf_apply_transform(lgf_ctx *ctx, const void *d_transform);
  * threads per line where the lattice allows), "fuse_g" (1 = the last FFT sweep ends with the g-build),
  * "sweep_tz" (z-planes per (z, t) tile of the sweep's CTA order, 0 = automatic, 1 = plain order),
  * "sweep_share" (1 / 0 / -1 = automatic: backward x, y neighbours of the same CTA hand over their algebra parts
- * through shared memory instead of being recomputed), "reunit_every" (N > 0: in every
+ * through shared memory instead of being recomputed), "pdl" (1 / 0: programmatic dependent launch of the
+ * iteration's kernels, so that each kernel's launch overlaps the tail of the one before -- the one key that is
+ * process-wide rather than per context), "reunit_every" (N > 0: in every
  * N-th update the new links are projected back onto SU(3) inside the sweep; 0 = never, the method as the
  * paper states it -- this key DOES change the result, by the rounding drift it removes; meant for fp32 runs
  * of thousands of iterations).

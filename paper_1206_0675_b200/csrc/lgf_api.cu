@@ -12,6 +12,7 @@
 #include "lgf_state.cuh"
 
 using namespace lgf;
+namespace lgf { int g_pdl_enabled = 1; }   // programmatic dependent launch of the iteration's kernels (lgf_pdl.cuh)
 
 struct lgf_ctx {
     Geom g{};
@@ -902,6 +903,7 @@ int lgf_tune(lgf_ctx *ctx, const char *key, int value) {
     else if (k == "fft_xy_planes") ctx->tune_xy_planes = value;
     else if (k == "fft_zt_xc") ctx->tune_zt_xc = value;
     else if (k == "fuse_g") ctx->tune_fuse_g = value;
+    else if (k == "pdl") lgf::g_pdl_enabled = value != 0;          // a launch attribute: process-wide, not per context
     else if (k == "sweep_tz") ctx->tune_sweep_tz = value;
     else if (k == "sweep_share") ctx->tune_sweep_share = value;
     else if (k == "reunit_every") ctx->tune_reunit = value < 0 ? 0 : value;

@@ -21,6 +21,7 @@
 // One shared-memory round trip per sweep in (x, y), two in (z, t), against five and ten for the
 // in-place two-step passes of lgf_fft.cu, which remain the path for lines that do not fit in registers.
 #include "lgf_fft_steps.cuh"
+#include "lgf_pdl.cuh"
 
 namespace lgf {
 
@@ -32,6 +33,7 @@ namespace lgf {
 template <class R, int L, int MODE, int P, bool GOUT>
 __global__ void __launch_bounds__(P *L) k_fftr_xy(C<R> *__restrict__ W, const DevState *__restrict__ st,
                                                   C<R> *__restrict__ G, long long V, int nzt, R half_alpha) {
+    pdl_enter();
     if (st->done) return;
     static_assert(!GOUT || (MODE == FFT_INV && P % 4 == 0 && L % 4 == 0), "g output needs all four components on chip");
     constexpr int PX = L | 1;                    // odd row pitch: lanes over rows hit distinct banks
@@ -113,6 +115,7 @@ template <class R, int LZ, int LT, int XC, bool TREG>
 __global__ void __launch_bounds__((ZtShape<R, LZ, LT, XC, TREG>::THREADS), (ZtShape<R, LZ, LT, XC, TREG>::MINB))
     k_fftr_zt(C<R> *__restrict__ W, Geom g, const C<R> *__restrict__ twt_g, const R *__restrict__ p2tab, R scale,
               const DevState *__restrict__ st) {
+    pdl_enter();
     if (st->done) return;
     using S = ZtShape<R, LZ, LT, XC, TREG>;
     constexpr int PITCH = S::PITCH;
@@ -229,8 +232,7 @@ cudaError_t launch_fft_reg(int which, const Geom &g, C<R> *W, const R *twiddle_t
             cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SM); \
             if (e != cudaSuccess) return e;                                                              \
         }                                                                                                \
-        kern<<<(unsigned)(planes / P), P * LEN, SM, stream>>>(W, st, G, g.V, nzt, half_alpha);             \
-        return cudaGetLastError();                                                                       \
+        return launch_pdl(kern, dim3((unsigned)(planes / P)), dim3(P * LEN), SM, stream, W, st, G, g.V, nzt, half_alpha); \
     }
         LGF_REG_XY(LGF_GO)
 #undef LGF_GO
@@ -246,8 +248,8 @@ cudaError_t launch_fft_reg(int which, const Geom &g, C<R> *W, const R *twiddle_t
             if (e != cudaSuccess) return e;                                                                   \
         }                                                                                                     \
         dim3 grid((unsigned)(g.S[2] / XC), 4);                                                                \
-        kern<<<grid, S::THREADS, S::SMEM, stream>>>(W, g, reinterpret_cast<const C<R> *>(twiddle_t), p2tab, scale, st); \
-        return cudaGetLastError();                                                                            \
+        return launch_pdl(kern, grid, dim3(S::THREADS), S::SMEM, stream, W, g, reinterpret_cast<const C<R> *>(twiddle_t), \
+                          p2tab, scale, st);                                                                  \
     }
     LGF_REG_ZT(LGF_GO)
 #undef LGF_GO

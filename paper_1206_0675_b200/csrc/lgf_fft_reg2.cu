@@ -10,6 +10,7 @@
 // index of every global and shared-memory access.
 #include "lgf_fft_split.cuh"
 #include "lgf_state.cuh"
+#include "lgf_pdl.cuh"
 
 namespace lgf {
 
@@ -23,6 +24,7 @@ constexpr int PAIR_MASK = 16;
 template <class R, int L, int MODE, int P, bool GOUT>
 __global__ void __launch_bounds__(2 * P * L) k_fftr2_xy(C<R> *__restrict__ W, const DevState *__restrict__ st,
                                                         C<R> *__restrict__ G, long long V, int nzt, R half_alpha) {
+    pdl_enter();
     if (st->done) return;
     static_assert(L % 16 == 0, "16 lines per warp");
     static_assert(!GOUT || (MODE == FFT_INV && P % 4 == 0), "g output needs all four components on chip");
@@ -111,6 +113,7 @@ struct Zt2Shape {
 template <class R, int LZ, int LT, int XC>
 __global__ void __launch_bounds__((Zt2Shape<R, LZ, LT, XC>::THREADS))
     k_fftr2_zt(C<R> *__restrict__ W, Geom g, const R *__restrict__ p2tab, R scale, const DevState *__restrict__ st) {
+    pdl_enter();
     if (st->done) return;
     using Sh = Zt2Shape<R, LZ, LT, XC>;
     constexpr int PITCH = Sh::PITCH, MZ = LZ / 2, MT = LT / 2;
@@ -212,8 +215,8 @@ static cudaError_t launch_xy2_as(const Geom &g, C<R> *W, const DevState *st, cud
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SM);
         if (e != cudaSuccess) return e;
     }
-    kern<<<(unsigned)(planes / P), 2 * P * L, SM, stream>>>(W, st, G, g.V, g.L[2] * g.L[3], half_alpha);
-    return cudaGetLastError();
+    return launch_pdl(kern, dim3((unsigned)(planes / P)), dim3(2 * P * L), SM, stream, W, st, G, g.V, g.L[2] * g.L[3],
+                      half_alpha);
 }
 template <class R, int L>
 static cudaError_t launch_xy2(int which, const Geom &g, C<R> *W, const DevState *st, cudaStream_t stream, C<R> *G,
@@ -235,8 +238,7 @@ static cudaError_t launch_zt2(const Geom &g, C<R> *W, const R *p2tab, R scale, c
         if (e != cudaSuccess) return e;
     }
     dim3 grid((unsigned)(g.S[2] / XC), 4);
-    kern<<<grid, Sh::THREADS, Sh::SMEM, stream>>>(W, g, p2tab, scale, st);
-    return cudaGetLastError();
+    return launch_pdl(kern, grid, dim3(Sh::THREADS), Sh::SMEM, stream, W, g, p2tab, scale, st);
 }
 
 // which: 0 = (x, y) forward, 1 = (z, t) forward + scale + inverse, 2 = (x, y) inverse, 3 = (x, y) inverse + g

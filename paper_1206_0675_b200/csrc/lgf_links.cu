@@ -9,6 +9,7 @@
 //   layout conversion canonical AoS <-> internal SoA, packed field <-> full 3x3 field
 // Part of liblgf (CUDA path).  Shares nothing with oracle/.
 #include "lgf_state.cuh"
+#include "lgf_pdl.cuh"
 
 namespace lgf {
 
@@ -56,6 +57,7 @@ __global__ void __launch_bounds__(SITE_THREADS) k_delta(LinkPair<R> lp, C<R> *__
 template <class R>
 __global__ void __launch_bounds__(SITE_THREADS) k_gbuild(const C<R> *__restrict__ W, C<R> *__restrict__ G, Geom g,
                                                           R half_alpha, const DevState *__restrict__ st) {
+    pdl_enter();
     if (st->done) return;
     const long long s = (long long)blockIdx.x * SITE_THREADS + threadIdx.x;
     if (s >= g.V) return;
@@ -174,6 +176,7 @@ template <class R, int NR, bool REUNIT, bool SHARE>
 __global__ void __launch_bounds__(SWEEP_THREADS, SWEEP_MINB)
     k_sweep(LinkPair<R> lp, const C<R> *__restrict__ G, C<R> *__restrict__ W, Geom g, double *__restrict__ partial,
             const DevState *__restrict__ st, BlockOrder bo) {
+    pdl_enter();
     if (st->done) return;
     const int cur = st->cur;
     const C<R> *__restrict__ src = lp.buf[cur];
@@ -265,6 +268,7 @@ __global__ void __launch_bounds__(SWEEP_THREADS, SWEEP_MINB)
 template <class R>
 __global__ void __launch_bounds__(SITE_THREADS) k_gacc(const C<R> *__restrict__ G, C<R> *__restrict__ A, Geom g,
                                                         const DevState *__restrict__ st) {
+    pdl_enter();
     if (st->done) return;
     const long long s = (long long)blockIdx.x * SITE_THREADS + threadIdx.x;
     if (s >= g.V) return;
@@ -392,6 +396,7 @@ __global__ void __launch_bounds__(SITE_THREADS) k_plaquette(LinkPair<R> lp, Geom
 __global__ void __launch_bounds__(1024) k_finalize(const double *__restrict__ partial, int nblocks, long long V,
                                                     double tol, int after_sweep, int record, DevState *st,
                                                     double *__restrict__ hist, long long hist_cap) {
+    pdl_enter();
     if ((record || after_sweep) && st->done) return;      // the kernels before this one did not run
     __shared__ double scratch[32][2];
     double f = 0.0, t = 0.0;
@@ -489,8 +494,7 @@ cudaError_t launch_delta(int nr, LinkPair<R> links, C<R> *W, const Geom &g, doub
 }
 template <class R>
 cudaError_t launch_gbuild(const C<R> *W, C<R> *G, const Geom &g, R half_alpha, const DevState *st, cudaStream_t stream) {
-    k_gbuild<R><<<site_blocks(g), SITE_THREADS, 0, stream>>>(W, G, g, half_alpha, st);
-    return cudaGetLastError();
+    return launch_pdl(k_gbuild<R>, dim3(site_blocks(g)), dim3(SITE_THREADS), 0, stream, W, G, g, half_alpha, st);
 }
 template <class R>
 cudaError_t launch_sweep(int nr, LinkPair<R> links, const C<R> *G, C<R> *W, const Geom &g, double *partial,
@@ -520,8 +524,8 @@ cudaError_t launch_sweep(int nr, LinkPair<R> links, const C<R> *G, C<R> *W, cons
         if (tz > 1 && g.L[2] % tz == 0) { bo.nxy = (int)(plane / SWEEP_THREADS); bo.tz = tz; }
     }
 #define LGF_SWK(RU, SH)                                                                                  \
-    if (nr == 3) k_sweep<R, 3, RU, SH><<<nb, SWEEP_THREADS, 0, stream>>>(links, G, W, g, partial, st, bo); \
-    else k_sweep<R, 2, RU, SH><<<nb, SWEEP_THREADS, 0, stream>>>(links, G, W, g, partial, st, bo);
+    if (nr == 3) return launch_pdl(k_sweep<R, 3, RU, SH>, dim3(nb), dim3(SWEEP_THREADS), 0, stream, links, G, W, g, partial, st, bo); \
+    else return launch_pdl(k_sweep<R, 2, RU, SH>, dim3(nb), dim3(SWEEP_THREADS), 0, stream, links, G, W, g, partial, st, bo);
     if (reunit && share) { LGF_SWK(true, true) }
     else if (reunit) { LGF_SWK(true, false) }
     else if (share) { LGF_SWK(false, true) }
@@ -558,7 +562,7 @@ cudaError_t launch_gacc(int op, const C<R> *G, C<R> *A, R *out, const Geom &g, c
     const int nb = site_blocks(g);
     if (op == 3) k_g_from_canonical<R><<<nb, SITE_THREADS, 0, stream>>>(out, A, g);      // out = input field, A = G
     else if (op == 0) k_gacc_identity<R><<<nb, SITE_THREADS, 0, stream>>>(A, g);
-    else if (op == 1) k_gacc<R><<<nb, SITE_THREADS, 0, stream>>>(G, A, g, st);
+    else if (op == 1) return launch_pdl(k_gacc<R>, dim3(nb), dim3(SITE_THREADS), 0, stream, G, A, g, st);
     else k_gacc_get<R><<<nb, SITE_THREADS, 0, stream>>>(A, out, g);
     return cudaGetLastError();
 }
@@ -589,8 +593,8 @@ cudaError_t launch_field_set(C<R> *W, const R *field, const Geom &g, cudaStream_
 
 cudaError_t launch_finalize(const double *partial, int nblocks, long long V, double tol, int after_sweep, int record,
                             DevState *st, double *hist, long long hist_cap, cudaStream_t stream) {
-    k_finalize<<<1, 1024, 0, stream>>>(partial, nblocks, V, tol, after_sweep, record, st, hist, hist_cap);
-    return cudaGetLastError();
+    return launch_pdl(k_finalize, dim3(1), dim3(1024), 0, stream, partial, nblocks, V, tol, after_sweep, record, st, hist,
+                      hist_cap);
 }
 cudaError_t launch_sum1(const double *partial, int nblocks, double norm, double *out, cudaStream_t stream) {
     k_sum1<<<1, 1024, 0, stream>>>(partial, nblocks, norm, out);
