@@ -13,6 +13,7 @@
 //   backwards with conjugate twiddles; no reordering pass, no second buffer (the paper's k3 kernel and
 //   reorder array, are not needed).
 #include "lgf_fft_steps.cuh"
+#include "lgf_pdl.cuh"
 
 namespace lgf {
 
@@ -23,6 +24,7 @@ __global__ void __launch_bounds__(256) k_fft_axis(C<R> *__restrict__ W, Geom g, 
                                                    int lo_blocks, const C<R> *__restrict__ twiddle,
                                                    const R *__restrict__ p2tab, R scale,
                                                    const DevState *__restrict__ st) {
+    pdl_enter();
     if (st->done) return;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     C<R> *tw = reinterpret_cast<C<R> *>(smem_raw);          // [L] forward twiddles exp(-2 pi i m / L)
@@ -76,6 +78,7 @@ __global__ void __launch_bounds__(256) k_fft_axis(C<R> *__restrict__ W, Geom g, 
 template <class R, int LX, int LY, int MODE>
 __global__ void __launch_bounds__(256) k_fft_xy(C<R> *__restrict__ W, int P, const C<R> *__restrict__ twx_g,
                                                  const C<R> *__restrict__ twy_g, const DevState *__restrict__ st) {
+    pdl_enter();
     if (st->done) return;
     constexpr int PX = LX | 1;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -117,6 +120,7 @@ __global__ void __launch_bounds__(256) k_fft_zt(C<R> *__restrict__ W, Geom g, in
                                                  const C<R> *__restrict__ twz_g, const C<R> *__restrict__ twt_g,
                                                  const R *__restrict__ p2tab, R scale,
                                                  const DevState *__restrict__ st) {
+    pdl_enter();
     if (st->done) return;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     C<R> *twz = reinterpret_cast<C<R> *>(smem_raw);
@@ -172,8 +176,7 @@ static cudaError_t launch_L(const AxisPass &p, C<R> *W, const Geom &g, const R *
     auto go = [&](auto kern) {
         cudaError_t e = set_smem(kern, p.smem);
         if (e != cudaSuccess) return e;
-        kern<<<grid, p.threads, p.smem, stream>>>(W, g, p.S, p.nlo, p.nhi, lo_blocks, tw, p2tab, scale, st);
-        return cudaGetLastError();
+        return launch_pdl(kern, grid, dim3(p.threads), p.smem, stream, W, g, p.S, p.nlo, p.nhi, lo_blocks, tw, p2tab, scale, st);
     };
     switch (p.mode) {
         case FFT_FWD: return go(k_fft_axis<R, L, FFT_FWD>);
@@ -191,8 +194,7 @@ static cudaError_t launch_xy(const AxisPass &p, C<R> *W, const Geom &g, const R 
     auto go = [&](auto kern) {
         cudaError_t e = set_smem(kern, p.smem);
         if (e != cudaSuccess) return e;
-        kern<<<grid, p.threads, p.smem, stream>>>(W, p.nhi, twx, twy, st);
-        return cudaGetLastError();
+        return launch_pdl(kern, dim3(grid), dim3(p.threads), p.smem, stream, W, p.nhi, twx, twy, st);
     };
     return p.mode == FFT_FWD ? go(k_fft_xy<R, LX, LY, FFT_FWD>) : go(k_fft_xy<R, LX, LY, FFT_INV>);
 }
@@ -205,8 +207,7 @@ static cudaError_t launch_zt(const AxisPass &p, C<R> *W, const Geom &g, const R 
     auto kern = k_fft_zt<R, LZ, LT>;
     cudaError_t e = set_smem(kern, p.smem);
     if (e != cudaSuccess) return e;
-    kern<<<grid, p.threads, p.smem, stream>>>(W, g, p.nlo, p.pitch, twz, twt, p2tab, scale, st);
-    return cudaGetLastError();
+    return launch_pdl(kern, grid, dim3(p.threads), p.smem, stream, W, g, p.nlo, p.pitch, twz, twt, p2tab, scale, st);
 }
 
 // the (La, Lb) pairs for which two-axis kernels are instantiated: BASELINE.json's lattices
