@@ -184,7 +184,8 @@ int lgf_apply_transform(lgf_ctx *ctx, const void *d_transform);
  * allows, 0 = one pass per axis), "fft_reg" (1 = use the register-line sweeps when the lattice allows), "fft_xy_planes" ((x, y) planes per CTA, 0 = automatic),
  * "fft_zt_xc" (consecutive (x, y) indices per CTA of the (z, t) pass, 0 = automatic), "fft_reg2" (1 = two
  * threads per line where the lattice allows), "fuse_g" (1 = the last FFT sweep ends with the g-build),
- * "sweep_tz" (z-planes per (z, t) tile of the sweep's CTA order, 0 = automatic, 1 = plain order),
+ * "sweep_tz" (z-planes per (z, t) tile of the sweep's CTA order, 0 = automatic, 1 = plain order), "hb_tz" (the
+ * same for the thread order of lgf_thermalize / lgf_overrelax, 0 = automatic),
  * "sweep_share" (1 / 0 / -1 = automatic: backward x, y neighbours of the same CTA hand over their algebra parts
  * through shared memory instead of being recomputed), "pdl" (1 / 0: programmatic dependent launch of the
  * iteration's kernels, so that each kernel's launch overlaps the tail of the one before -- the one key that is

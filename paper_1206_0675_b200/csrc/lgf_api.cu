@@ -50,6 +50,7 @@ struct lgf_ctx {
     int tune_fuse_g = 1;         // lgf_tune: end the last FFT sweep with the g-build (register-line plan only)
     int tune_sweep_share = -1;   // lgf_tune: hand A'_x, A'_y to the forward neighbours of the same CTA through shared
                                  // memory (1 / 0; -1 = automatic: 18-real and fp32 or a lattice beyond L2)
+    int tune_hb_tz = 0;          // lgf_tune: z-planes per (z, t) tile of the heat-bath thread order (0 = automatic)
     int tune_reunit = 0;         // lgf_tune "reunit_every": project the new links onto SU(3) in every N-th update (0 = never)
     long long updates_enqueued = 0;   // host-side count of updates enqueued since the last set_links / thermalize
     int tune_sweep_tz = 0;       // lgf_tune: z-planes per (z, t) tile of the sweep's block order (0 = automatic, 1 = plain)
@@ -819,10 +820,10 @@ static int monte_carlo_sweeps(lgf_ctx *ctx, double beta, int nsweeps, unsigned l
                 Bracket br(ctx, LGF_K_HEATBATH);
                 if (ctx->prec == LGF_FP64)
                     CK(launch_heatbath<double>(ctx->nr, link_pair<double>(ctx), ctx->g, ctx->st, beta, key, ctx->hb_sweeps,
-                                               mu, parity, ctx->stream, overrelax));
+                                               mu, parity, ctx->stream, overrelax, ctx->tune_hb_tz));
                 else
                     CK(launch_heatbath<float>(ctx->nr, link_pair<float>(ctx), ctx->g, ctx->st, beta, key, ctx->hb_sweeps, mu,
-                                              parity, ctx->stream, overrelax));
+                                              parity, ctx->stream, overrelax, ctx->tune_hb_tz));
             }
         if (!overrelax) ctx->hb_sweeps++;                // only heat-bath sweeps consume random numbers
     }
@@ -905,6 +906,7 @@ int lgf_tune(lgf_ctx *ctx, const char *key, int value) {
     else if (k == "fuse_g") ctx->tune_fuse_g = value;
     else if (k == "pdl") lgf::g_pdl_enabled = value != 0;          // a launch attribute: process-wide, not per context
     else if (k == "sweep_tz") ctx->tune_sweep_tz = value;
+    else if (k == "hb_tz") ctx->tune_hb_tz = value;
     else if (k == "sweep_share") ctx->tune_sweep_share = value;
     else if (k == "reunit_every") ctx->tune_reunit = value < 0 ? 0 : value;
     else return fail(ctx, LGF_EINVAL, "lgf_tune: unknown key " + k);

@@ -115,7 +115,8 @@ unsigned long long heatbath_key(unsigned long long seed);
 template <class R>
 cudaError_t launch_heatbath(int nr, LinkPair<R> links, const Geom &g, const DevState *st, double beta,
                             unsigned long long key, unsigned long long sweep, int mu, int parity, cudaStream_t stream,
-                            bool overrelax /* R28: alpha = (V^dag)^2, no random numbers */);
+                            bool overrelax /* R28: alpha = (V^dag)^2, no random numbers */,
+                            int order_tz /* z-planes per (z, t) tile of the thread order: 0 = automatic */);
 cudaError_t launch_reset_counters(DevState *st, cudaStream_t stream);
 
 // F / theta finalisation (precision independent)

@@ -198,3 +198,30 @@ def test_overrelaxation_matches_the_oracle_and_conserves_the_action(lgf, prec, s
     else:
         assert e1.max() < 1e-5 and e2.max() < 1e-4
         assert abs(P2 - P0) < 2e-6
+
+
+@pytest.mark.parametrize("prec,storage", [(8, 18), (4, 12)])
+def test_tiled_thread_order_is_bit_identical(lgf, prec, storage):
+    """lgf_tune("hb_tz"): the (z, t)-tiled order in which the threads walk the lattice (used automatically when a
+    t slice exceeds L2, i.e. at 64^4) only changes WHICH thread updates a site; sites, staples and random numbers
+    are the same, so heat-bath and overrelaxation sweeps must come out bit for bit as in the plain order."""
+    import torch
+
+    dims = (8, 4, 8, 6)
+    U0 = inputs.hot_config(dims, 77)
+    res = []
+    for tz in (8, 2, 4, 1):                                  # 8 = Lz: the plain order
+        with lgf.Context(dims, prec, storage) as ctx:
+            ctx.tune("hb_tz", tz)
+            d = _dev(U0, prec)
+            ctx.set_links(d)
+            ctx.thermalize(5.9, 2, 13)
+            ctx.overrelax(1)
+            ctx.thermalize(5.9, 1, 13)
+            res.append(ctx.get_links(torch.empty_like(d)).clone())
+    for r in res[1:]:
+        assert torch.equal(res[0], r)
+    if prec == 8:
+        ref = oracle.heatbath(dims, oracle.overrelax(dims, oracle.heatbath(dims, U0, 5.9, 13, 0, 2), 1), 5.9, 13, 2, 1)
+        err = np.abs(res[1].cpu().numpy() - ref)
+        assert np.quantile(err, 0.999) < TOL1 * growth(5.9) ** 3 and err.max() < NO_FLIP
