@@ -130,6 +130,14 @@ def physical_gpu_index(local_rank):
 
 
 # ---------------------------------------------------------------------------------------------------------
+TUNE = {}          # --tune key=value[,key=value]: lgf_tune overrides applied to every context (ablations)
+
+
+def apply_tune(ctx):
+    for k, v in TUNE.items():
+        ctx.tune(k, v)
+
+
 def time_variant(binding, torch, U0, dims, prec_name, storage, steps, warmup, dist, sampler=None):
     """Device-resident timing of `steps` iterations.  Returns dict(ms_per_step, launches, kernels...)."""
     prec = PREC[prec_name]
@@ -137,6 +145,7 @@ def time_variant(binding, torch, U0, dims, prec_name, storage, steps, warmup, di
     stream = torch.cuda.current_stream()
     out = {}
     with binding.Context(dims, prec, storage, stream=stream) as ctx:
+        apply_tune(ctx)
         d = torch.from_numpy(U0).to(cdt).cuda()
         ctx.set_links(d)
         # warm-up, itself timed on the device: gives the per-step estimate the stall check below uses
@@ -215,6 +224,7 @@ def time_e2e(binding, torch, U0, dims, prec_name, storage, tol, max_iter, dist):
     cdt = torch.complex128 if prec == 8 else torch.complex64
     stream = torch.cuda.current_stream()
     with binding.Context(dims, prec, storage, stream=stream) as ctx:
+        apply_tune(ctx)
         h = torch.from_numpy(U0).to(cdt).pin_memory()
         warm = h.clone().pin_memory()
         ctx.fix_host(warm, ALPHA, tol, 1)              # allocates the staging buffer, warms the kernels
@@ -427,6 +437,8 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--cpu-budget", type=float, default=20.0)
     ap.add_argument("--reference-budget", type=float, default=240.0)
+    ap.add_argument("--tune", default="", metavar="KEY=VALUE[,KEY=VALUE]",
+                    help="lgf_tune overrides for every context (ablations; the default line uses none)")
     ap.add_argument("--thermal", type=float, default=None, metavar="BETA",
                     help="thermalise a cold 32^4 lattice at BETA and gauge-fix it (own JSON line, not the contract line)")
     ap.add_argument("--thermal-size", type=int, default=32, choices=[8, 16, 32, 64], help="lattice extent L of --thermal (L^4)")
@@ -439,6 +451,9 @@ def main():
     ap.add_argument("--mixed", action="store_true", help="--thermal (fp64 only): also time fp32 iterations + fp64 polish")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)
+    for kv in [x for x in args.tune.split(",") if x]:
+        k, v = kv.split("=")
+        TUNE[k.strip()] = int(v)
     if args.impl == "reference":
         return run_reference(args)
     if args.thermal is not None:
@@ -531,7 +546,7 @@ def main():
                 "warmup": args.warmup, "ms_per_step": head["ms_per_step"], "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": None, "dtype": "f64" if args.precision == "fp64" else "f32", "data": "synthetic",
                 "config": {"workload": workload_name(args.workload, dims), "precision": args.precision,
-                           "link_storage": args.storage, "alpha": ALPHA, "sites": V, "parallelism": "replicas x%d" % world,
+                           "tune": dict(TUNE), "link_storage": args.storage, "alpha": ALPHA, "sites": V, "parallelism": "replicas x%d" % world,
                            "l2": "inputs larger than L2: one step streams %.0f MB of links and fields"
                                  % (head["iter_bytes"] / 1e6)},
                 "site_updates_per_s": value * V, "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e,
