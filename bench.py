@@ -337,6 +337,7 @@ def run_thermal(args):
     cdt = torch.complex128 if prec == 8 else torch.complex64
     stream = torch.cuda.current_stream()
     with binding.Context(dims, prec, args.storage, stream=stream) as ctx:
+        apply_tune(ctx)
         ctx.tune("reunit_every", args.reunit_every)
         cold = torch.zeros((L, L, L, L, 4, 3, 3), dtype=cdt, device="cuda")
         for i in range(3):
@@ -402,7 +403,7 @@ def run_thermal(args):
     peak, _ = measured_peak()
     print(json.dumps({
         "mode": "thermal", "beta": args.thermal, "lattice": "x".join([str(L)] * 4), "precision": args.precision,
-        "link_storage": args.storage, "alpha": args.alpha, "reunit_every": args.reunit_every,
+        "link_storage": args.storage, "tune": dict(TUNE), "alpha": args.alpha, "reunit_every": args.reunit_every,
         "heatbath_sweeps": args.thermal_sweeps, "overrelax_per_heatbath": args.thermal_overrelax,
         "seed": args.thermal_seed, "heatbath_ms_per_sweep": ms_sweep,
         "heatbath_algorithmic_gbs": hb_bytes / (ms_sweep * 1e-3) / 1e9, "heatbath_frac_of_peak": hb_bytes / (ms_sweep * 1e-3) / 1e9 / peak,
