@@ -118,3 +118,52 @@ def test_c5_hot_start_one_iteration(lgf):
         assert err < tol["links"]
         assert np.all(np.diff(Fh5) > 0)
         assert abs(P5 - P0) < (1e-13 if prec == 8 else 1e-6)
+
+
+def test_section_8f_rows_at_full_size(lgf, config_cache):
+    """The SURVEY.md 8(f) rows at the bench lattice (32^4, fp64 / 18-real, default plan): two heat-bath sweeps and
+    one overrelaxation sweep link by link against the thermalisation oracle; then, on the smooth C3 configuration,
+    five updates with the accumulated transformation tracked -- G against the product of the oracle's g fields,
+    G U0 G(x+mu)^dag against the CUDA path's own links -- and the gluon field A_t(k) against the oracle's."""
+    import torch
+
+    dims = inputs.CONFIGS["C3"]["dims"]
+    V = int(np.prod(dims))
+    # -- thermalisation (NEXT-1)
+    hot = inputs.hot_config_torch(dims, 4242, device="cuda")
+    U0 = hot.cpu().numpy()
+    U1 = oracle.heatbath(dims, U0, 6.0, 55, 0, 1)
+    U2 = oracle.overrelax(dims, oracle.heatbath(dims, U1, 6.0, 55, 1, 1), 1)
+    with lgf.Context(dims, 8, 18, stream=torch.cuda.current_stream()) as ctx:
+        ctx.set_links(hot)
+        ctx.thermalize(6.0, 1, 55)
+        e1 = np.abs(ctx.get_links(torch.empty_like(hot)).cpu().numpy() - U1)
+        ctx.thermalize(6.0, 1, 55)
+        ctx.overrelax(1)
+        e2 = np.abs(ctx.get_links(torch.empty_like(hot)).cpu().numpy() - U2)
+        _, _, P = ctx.measure()
+    assert e1.max() < 1e-12
+    assert np.quantile(e2, 0.999) < 1e-12 * 3.0 ** 2 and e2.max() < 1e-6        # see tests/test_gpu_heatbath.py
+    assert abs(P - oracle.plaquette(dims, U2)) < 1e-12
+    del hot, U0, U1, U2, e1, e2
+    # -- accumulated transformation and gluon field (NEXT-2)
+    U = config_cache("C3")
+    Uo, G = U.copy(), np.broadcast_to(np.eye(3, dtype=np.complex128), U.shape[:4] + (3, 3)).copy()
+    for _ in range(5):
+        D, _, _ = oracle.measure(dims, Uo)
+        g = oracle.build_g(dims, oracle.accelerate(dims, D), ALPHA)
+        Uo = oracle.transform(dims, Uo, g)
+        G = g @ G
+    with lgf.Context(dims, 8, 18, stream=torch.cuda.current_stream()) as ctx:
+        ctx.track_transform(True)
+        d = torch.from_numpy(U).cuda()
+        ctx.set_links(d)
+        ctx.iterate(ALPHA, 5)
+        Gd = ctx.get_transform(torch.empty(U.shape[:4] + (3, 3), dtype=torch.complex128, device="cuda")).cpu().numpy()
+        out = ctx.get_links(torch.empty_like(d)).cpu().numpy()
+        At = ctx.gluon_field(3, torch.empty(U.shape[:4] + (3, 3), dtype=torch.complex128, device="cuda")).cpu().numpy()
+    assert np.max(np.abs(Gd - G)) < 1e-11 and np.max(np.abs(out - Uo)) < 1e-11
+    assert np.max(np.abs(oracle.transform(dims, U, Gd) - out)) < 1e-11
+    ref = oracle.gluon_field(dims, out, 3)
+    assert np.max(np.abs(At - ref)) < 1e-12 * np.max(np.abs(ref))
+    assert V == 32 ** 4
