@@ -17,6 +17,7 @@
 //   uniforms u_n = ((mix64(key + (idx+1) G) >> 11) + 0.5) 2^-53, idx = ((((class V + site) 3 + k) 32 + t) 6 + n) (R27)
 // The arithmetic is double precision whatever the storage precision of the links.
 #include "lgf_state.cuh"
+#include "lgf_pdl.cuh"
 
 namespace lgf {
 
@@ -112,6 +113,7 @@ template <class R, int NR, bool OVERRELAX>
 __global__ void __launch_bounds__(HB_THREADS) k_heatbath(LinkPair<R> lp, Geom g, const DevState *__restrict__ st,
                                                          double beta, unsigned long long key,
                                                          unsigned long long class_id, int mu, int parity, int tz) {
+    pdl_enter();                                        // the eight class passes of a sweep are chained (lgf_pdl.cuh)
     C<R> *links = lp.buf[st->cur];                      // updated in place (no __restrict__: read and written)
     const long long h = (long long)blockIdx.x * HB_THREADS + threadIdx.x;
     if (h >= g.V / 2) return;
@@ -235,12 +237,15 @@ cudaError_t launch_heatbath(int nr, LinkPair<R> links, const Geom &g, const DevS
         }
     }
     const unsigned long long class_id = sweep * 8ULL + (unsigned long long)(mu * 2 + parity);
+#define LGF_HB(NRV, ORV) \
+    return launch_pdl(k_heatbath<R, NRV, ORV>, dim3(nb), dim3(HB_THREADS), 0, stream, links, g, st, beta, key, class_id, mu, parity, tz)
     if (overrelax) {
-        if (nr == 3) k_heatbath<R, 3, true><<<nb, HB_THREADS, 0, stream>>>(links, g, st, beta, key, class_id, mu, parity, tz);
-        else k_heatbath<R, 2, true><<<nb, HB_THREADS, 0, stream>>>(links, g, st, beta, key, class_id, mu, parity, tz);
-    } else if (nr == 3) k_heatbath<R, 3, false><<<nb, HB_THREADS, 0, stream>>>(links, g, st, beta, key, class_id, mu, parity, tz);
-    else k_heatbath<R, 2, false><<<nb, HB_THREADS, 0, stream>>>(links, g, st, beta, key, class_id, mu, parity, tz);
-    return cudaGetLastError();
+        if (nr == 3) LGF_HB(3, true);
+        LGF_HB(2, true);
+    }
+    if (nr == 3) LGF_HB(3, false);
+    LGF_HB(2, false);
+#undef LGF_HB
 }
 cudaError_t launch_reset_counters(DevState *st, cudaStream_t stream) {
     k_reset_counters<<<1, 1, 0, stream>>>(st);
