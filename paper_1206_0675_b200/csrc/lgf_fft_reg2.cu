@@ -182,20 +182,31 @@ template <> struct Xy2Cfg<double, 64> { static constexpr int P = 1, PF = 1; };  
 template <> struct Xy2Cfg<float, 16> { static constexpr int P = 8, PF = 8; };
 template <> struct Xy2Cfg<float, 32> { static constexpr int P = 4, PF = 2; };
 template <> struct Xy2Cfg<float, 64> { static constexpr int P = 4, PF = 4; };
-template <class R, int L> struct Zt2Cfg;
-template <> struct Zt2Cfg<double, 16> { static constexpr int XC = 4; };
-template <> struct Zt2Cfg<double, 32> { static constexpr int XC = 4; };
-template <> struct Zt2Cfg<double, 64> { static constexpr int XC = 2; };
-template <> struct Zt2Cfg<float, 16> { static constexpr int XC = 8; };
-template <> struct Zt2Cfg<float, 32> { static constexpr int XC = 4; };
-template <> struct Zt2Cfg<float, 64> { static constexpr int XC = 2; };
+// (Lz, Lt) pairs of the (z, t) sweep: Lt = Lz, and Lt = 2 Lz -- the usual shape of a lattice QCD volume (the
+// paper tunes on 32^3 x n) -- with the consecutive (kx, ky) indices per CTA
+template <class R, int LZ, int LT> struct Zt2Cfg;
+template <> struct Zt2Cfg<double, 16, 16> { static constexpr int XC = 4; };
+template <> struct Zt2Cfg<double, 32, 32> { static constexpr int XC = 4; };
+template <> struct Zt2Cfg<double, 64, 64> { static constexpr int XC = 2; };
+template <> struct Zt2Cfg<double, 16, 32> { static constexpr int XC = 4; };
+template <> struct Zt2Cfg<double, 32, 64> { static constexpr int XC = 2; };
+template <> struct Zt2Cfg<float, 16, 16> { static constexpr int XC = 8; };
+template <> struct Zt2Cfg<float, 32, 32> { static constexpr int XC = 4; };
+template <> struct Zt2Cfg<float, 64, 64> { static constexpr int XC = 2; };
+template <> struct Zt2Cfg<float, 16, 32> { static constexpr int XC = 4; };
+template <> struct Zt2Cfg<float, 32, 64> { static constexpr int XC = 2; };
+#define LGF_REG2_ZT(X) X(16, 16) X(32, 32) X(64, 64) X(16, 32) X(32, 64)
 
 #define LGF_REG2_LEN(X) X(16) X(32) X(64)
 
 static bool reg2_len(int L) { return L == 16 || L == 32 || L == 64; }
 
 bool fft_reg2_supported(const Geom &g) {
-    if (!(g.L[0] == g.L[1] && g.L[2] == g.L[3] && reg2_len(g.L[0]) && reg2_len(g.L[2]))) return false;
+    bool zt = false;
+#define LGF_C(A, B) if (g.L[2] == A && g.L[3] == B) zt = true;
+    LGF_REG2_ZT(LGF_C)
+#undef LGF_C
+    if (!(g.L[0] == g.L[1] && reg2_len(g.L[0]) && zt)) return false;
     const long long planes = 4LL * g.L[2] * g.L[3];
     return planes % 8 == 0 && g.S[2] % 8 == 0;
 }
@@ -228,11 +239,11 @@ static cudaError_t launch_xy2(int which, const Geom &g, C<R> *W, const DevState 
     return cudaErrorInvalidValue;
 }
 
-template <class R, int L>
+template <class R, int LZ, int LT>
 static cudaError_t launch_zt2(const Geom &g, C<R> *W, const R *p2tab, R scale, const DevState *st, cudaStream_t stream) {
-    constexpr int XC = Zt2Cfg<R, L>::XC;
-    using Sh = Zt2Shape<R, L, L, XC>;
-    auto kern = k_fftr2_zt<R, L, L, XC>;
+    constexpr int XC = Zt2Cfg<R, LZ, LT>::XC;
+    using Sh = Zt2Shape<R, LZ, LT, XC>;
+    auto kern = k_fftr2_zt<R, LZ, LT, XC>;
     if (Sh::SMEM > 40 * 1024) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Sh::SMEM);
         if (e != cudaSuccess) return e;
@@ -246,8 +257,8 @@ template <class R>
 cudaError_t launch_fft_reg2(int which, const Geom &g, C<R> *W, const R *p2tab, R scale, const DevState *st,
                             cudaStream_t stream, C<R> *G, R half_alpha) {
     if (which == 1) {
-#define LGF_GO(LEN) if (g.L[2] == LEN) return launch_zt2<R, LEN>(g, W, p2tab, scale, st, stream);
-        LGF_REG2_LEN(LGF_GO)
+#define LGF_GO(A, B) if (g.L[2] == A && g.L[3] == B) return launch_zt2<R, A, B>(g, W, p2tab, scale, st, stream);
+        LGF_REG2_ZT(LGF_GO)
 #undef LGF_GO
         return cudaErrorInvalidValue;
     }

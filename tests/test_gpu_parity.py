@@ -83,7 +83,7 @@ def test_delta_F_theta(lgf, name, dims, prec, storage):
 
 ACC_DIMS = [(8, 8, 8, 8), (12, 6, 16, 4), (3, 24, 2, 48), (16, 16, 16, 16), (32, 8, 64, 4), (8, 8, 24, 48),
             (24, 24, 24, 48), (32, 32, 16, 16), (64, 64, 8, 8), (8, 8, 64, 64), (16, 16, 32, 32), (24, 24, 8, 8),
-            (32, 32, 32, 32), (64, 64, 16, 16), (16, 16, 64, 64)]
+            (32, 32, 32, 32), (64, 64, 16, 16), (16, 16, 64, 64), (16, 16, 16, 32), (32, 32, 32, 64)]
 
 
 @pytest.mark.parametrize("dims", ACC_DIMS)
@@ -113,7 +113,7 @@ def test_accelerate(lgf, dims, prec, plan):
     assert np.max(np.abs(w - w_o)) < (1e-12 if prec == 8 else 2e-5) * scale
 
 
-@pytest.mark.parametrize("dims,passes", [((32, 32, 32, 32), 3), ((24, 24, 24, 48), 3), ((8, 8, 8, 8), 3),
+@pytest.mark.parametrize("dims,passes", [((32, 32, 32, 32), 3), ((24, 24, 24, 48), 3), ((8, 8, 8, 8), 3), ((16, 16, 16, 32), 3),
                                          ((12, 6, 16, 4), 7), ((16, 16, 12, 6), 5), ((6, 12, 32, 32), 5)])
 def test_fft_plan_and_tile_overrides(lgf, dims, passes):
     """The planner uses three sweeps where two-axis kernels exist; tile-size overrides change rounding only."""
@@ -217,6 +217,20 @@ def test_trajectory_shared_neighbour_sweep(lgf, config_cache, name, dims, prec, 
     n = 12
     U_o, F_o, T_o = oracle.iterate(dims, U, ALPHA, n)
     Fh, Th, P, out = run_trajectory(lgf, dims, U, prec, storage, n, tune={"sweep_share": 1})
+    tol = TOL[prec]
+    assert np.max(np.abs(Fh - F_o) / np.abs(F_o)) < tol["scalar"]
+    assert np.max(np.abs(Th - T_o) / np.abs(T_o)) < tol["scalar"]
+    assert np.max(np.abs(out - U_o)) < tol["links"]
+
+
+@pytest.mark.parametrize("prec,storage", VARIANTS)
+def test_trajectory_time_extent_twice_the_spatial_one(lgf, prec, storage):
+    """16^3 x 32 -- the usual shape of a lattice QCD volume (the paper tunes on 32^3 x n): 20
+    iterations through the register-line sweeps with Lt = 2 Lz, every precision x storage variant."""
+    dims = (16, 16, 16, 32)
+    U = inputs.smooth_config(dims, 0.3, 3216, haar=True)
+    U_o, F_o, T_o = oracle.iterate(dims, U, ALPHA, 20)
+    Fh, Th, P, out = run_trajectory(lgf, dims, U, prec, storage, 20)
     tol = TOL[prec]
     assert np.max(np.abs(Fh - F_o) / np.abs(F_o)) < tol["scalar"]
     assert np.max(np.abs(Th - T_o) / np.abs(T_o)) < tol["scalar"]
