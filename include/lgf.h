@@ -220,6 +220,64 @@ double lgf_algorithmic_bytes(const lgf_ctx *ctx, int kernel_class);
 const char *lgf_last_error(const lgf_ctx *ctx);
 const char *lgf_version(void);
 
+/* ---- one configuration sharded over several GPUs ------
+ *
+ * Slab decomposition over t: rank r of nranks owns the slices t = r T .. (r+1) T - 1, T = Lt / nranks -- a
+ * contiguous piece of the canonical configuration, [T, Lz, Ly, Lx, 4, 3, 3, 2] as a tensor.  nranks must divide
+ * Lt and Lz (LGF_EINVAL otherwise): for the t lines of the 4-D FFT the field is redistributed into z-slabs
+ * (rank r: z = r Zl .. (r+1) Zl - 1, Zl = Lz / nranks, all t) by an all-to-all.  Every entry point below is
+ * LOCAL to one rank: it works on that rank's slab and on device buffers the caller passes in, and the caller
+ * moves those buffers between ranks (NCCL send/recv, all-to-all, all-reduce through torch.distributed in
+ * paper_1206_0675_b200/slab.py) -- no kernel waits on another rank.  One iteration of Algorithm 1
+ * is, on every rank:
+ *   halo_pack(LINKS) -> [send to r+1, receive from r-1] -> halo_unpack(LINKS) -> delta(sums) -> [all-reduce sums:
+ *   F = sums[0] / (12 V), theta = sums[1] / (3 V), V the GLOBAL volume (eqs. 3, 6)] -> fft_local(0) ->
+ *   transpose(0, send) -> [all-to-all] -> transpose(1, recv) -> fft_t -> transpose(2, send) -> [all-to-all] ->
+ *   transpose(3, recv) -> fft_local(1) -> gbuild(alpha) -> halo_pack(G) -> [send to r-1, receive from r+1] ->
+ *   halo_unpack(G) -> update.
+ * With nranks = 1 the "exchanges" are copies of a rank's send buffer into its own receive buffer (periodic wrap).
+ * The result equals the one-GPU path's up to the rounding order of the F / theta sums and of the FFT passes.
+ * Same precision / storage / error conventions as above; messages from lgf_slab_last_error.  All calls are
+ * asynchronous on the context's stream (default: stream 0). */
+typedef struct lgf_slab lgf_slab; /* opaque */
+enum { LGF_HALO_LINKS = 0, /* U_t on one 3-D slice: 18 or 12 reals per site (the context's link storage)       */
+       LGF_HALO_G = 1      /* rows 0, 1 of g(x) on one 3-D slice: 12 reals per site                             */ };
+
+int lgf_slab_create(const int dims[4] /* GLOBAL extents */, int precision, int link_storage, int rank, int nranks,
+                    lgf_slab **out);
+int lgf_slab_destroy(lgf_slab *ctx);
+int lgf_slab_set_stream(lgf_slab *ctx, void *cuda_stream);
+/* this rank's slab in canonical layout (72 reals per site, Lx Ly Lz T sites, t slowest) */
+int lgf_slab_set_links(lgf_slab *ctx, const void *d_links);
+int lgf_slab_get_links(lgf_slab *ctx, void *d_links);
+/* number of REALS of one halo buffer (Lx Ly Lz sites times the reals per site above) */
+long long lgf_slab_halo_elems(const lgf_slab *ctx, int which);
+/* pack: LGF_HALO_LINKS = U_t of the slab's LAST slice (the rank above needs it as U_t(x - t), eq. 5);
+ * LGF_HALO_G = g of the slab's FIRST slice (the rank below needs it as g(x + t), eq. 2) into d_send.
+ * unpack: take the neighbour's packed slice from d_recv into the context's halo storage. */
+int lgf_slab_halo_pack(lgf_slab *ctx, int which, void *d_send);
+int lgf_slab_halo_unpack(lgf_slab *ctx, int which, const void *d_recv);
+/* a1 on the slab: Delta(x) into the work field; d_sums[0] = sum Re tr U_mu(x), d_sums[1] = sum tr(Delta Delta^dag)
+ * over the slab's sites (device doubles, fixed summation order). */
+int lgf_slab_delta(lgf_slab *ctx, double *d_sums);
+/* the x, y, z passes of the 4-D FFT on the slab's work field: inverse == 0 forward (x, y, z), else inverse (z, y, x) */
+int lgf_slab_fft_local(lgf_slab *ctx, int inverse);
+/* the two sides of the two all-to-alls; d_buf holds 8 reals per local site, ordered [q][c][tl][zl][y][x] with
+ * chunk q (1 / nranks of the buffer) the part that goes to / came from rank q:
+ *   stage 0: work field (t-slabs) -> send buffer      stage 1: receive buffer -> z-slab field
+ *   stage 2: z-slab field -> send buffer              stage 3: receive buffer -> work field (t-slabs) */
+int lgf_slab_transpose(lgf_slab *ctx, int stage, void *d_buf);
+/* on the z-slab field: forward t, times p2max / (V p2(k)) with the zero mode set to 0, inverse t (Alg. 1 lines 4-7) */
+int lgf_slab_fft_t(lgf_slab *ctx);
+/* a5: g(x) = GS(1 + i (alpha / 2) w(x)) on the slab */
+int lgf_slab_gbuild(lgf_slab *ctx, double alpha);
+/* a6: U_mu(x) <- g(x) U_mu(x) g(x + mu)^dag on the slab, in place */
+int lgf_slab_update(lgf_slab *ctx);
+/* the slab's work field as full 3 x 3 matrices, 18 reals per local site (as lgf_get_field) */
+int lgf_slab_get_field(lgf_slab *ctx, void *d_field);
+long long lgf_slab_launch_count(const lgf_slab *ctx);
+const char *lgf_slab_last_error(const lgf_slab *ctx);
+
 #ifdef __cplusplus
 }
 #endif

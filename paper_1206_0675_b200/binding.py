@@ -64,7 +64,26 @@ SIGNATURES = {
     "lgf_algorithmic_bytes": (_d, [_vp, _i]),
     "lgf_last_error": (ctypes.c_char_p, [_vp]),
     "lgf_version": (ctypes.c_char_p, []),
+    # one configuration sharded over several GPUs (per-rank entry points; exchanges in slab.py)
+    "lgf_slab_create": (_i, [ctypes.POINTER(ctypes.c_int), _i, _i, _i, _i, ctypes.POINTER(_vp)]),
+    "lgf_slab_destroy": (_i, [_vp]),
+    "lgf_slab_set_stream": (_i, [_vp, _vp]),
+    "lgf_slab_set_links": (_i, [_vp, _vp]),
+    "lgf_slab_get_links": (_i, [_vp, _vp]),
+    "lgf_slab_halo_elems": (_ll, [_vp, _i]),
+    "lgf_slab_halo_pack": (_i, [_vp, _i, _vp]),
+    "lgf_slab_halo_unpack": (_i, [_vp, _i, _vp]),
+    "lgf_slab_delta": (_i, [_vp, _vp]),
+    "lgf_slab_fft_local": (_i, [_vp, _i]),
+    "lgf_slab_transpose": (_i, [_vp, _i, _vp]),
+    "lgf_slab_fft_t": (_i, [_vp]),
+    "lgf_slab_gbuild": (_i, [_vp, _d]),
+    "lgf_slab_update": (_i, [_vp]),
+    "lgf_slab_get_field": (_i, [_vp, _vp]),
+    "lgf_slab_launch_count": (_ll, [_vp]),
+    "lgf_slab_last_error": (ctypes.c_char_p, [_vp]),
 }
+LGF_HALO_LINKS, LGF_HALO_G = 0, 1
 
 
 class LgfError(RuntimeError):
@@ -283,6 +302,90 @@ class Context:
 
     def algorithmic_bytes(self, kernel_class):
         return float(load().lgf_algorithmic_bytes(self._h, int(kernel_class)))
+
+
+class SlabContext:
+    """Owns one lgf_slab: rank `rank` of `nranks` of ONE configuration sharded over t (include/lgf.h, last section).
+    Methods are the C entry points minus the ``lgf_slab_`` prefix; all local to this rank -- the exchanges
+    between ranks are paper_1206_0675_b200.slab's."""
+
+    def __init__(self, dims, precision, link_storage, rank, nranks, stream=None):
+        self.dims = tuple(int(v) for v in dims)
+        self.precision, self.link_storage = int(precision), int(link_storage)
+        self.rank, self.nranks = int(rank), int(nranks)
+        self._h = ctypes.c_void_p()
+        lib = load()
+        rc = lib.lgf_slab_create((ctypes.c_int * 4)(*self.dims), self.precision, self.link_storage, self.rank,
+                                 self.nranks, ctypes.byref(self._h))
+        if rc < 0:
+            msg = lib.lgf_slab_last_error(None)
+            raise LgfError(rc, msg.decode() if msg else "")
+        self.T = self.dims[3] // self.nranks
+        self.V = self.dims[0] * self.dims[1] * self.dims[2] * self.T       # local sites
+        if stream is not None:
+            self.set_stream(stream)
+
+    def destroy(self):
+        if self._h:
+            load().lgf_slab_destroy(self._h)
+            self._h = ctypes.c_void_p()
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+    def _ck(self, rc):
+        if rc < 0:
+            msg = load().lgf_slab_last_error(self._h)
+            raise LgfError(int(rc), msg.decode() if msg else "")
+        return rc
+
+    def set_stream(self, stream):
+        ptr = stream.cuda_stream if hasattr(stream, "cuda_stream") else int(stream)
+        self._ck(load().lgf_slab_set_stream(self._h, ctypes.c_void_p(ptr)))
+
+    def set_links(self, links):
+        self._ck(load().lgf_slab_set_links(self._h, _dev_ptr(links, self.precision, self.V * 72)))
+
+    def get_links(self, out):
+        self._ck(load().lgf_slab_get_links(self._h, _dev_ptr(out, self.precision, self.V * 72)))
+        return out
+
+    def halo_elems(self, which):
+        return int(self._ck(load().lgf_slab_halo_elems(self._h, int(which))))
+
+    def halo_pack(self, which, send):
+        self._ck(load().lgf_slab_halo_pack(self._h, int(which), _dev_ptr(send, self.precision, self.halo_elems(which))))
+
+    def halo_unpack(self, which, recv):
+        self._ck(load().lgf_slab_halo_unpack(self._h, int(which), _dev_ptr(recv, self.precision, self.halo_elems(which))))
+
+    def delta(self, sums):
+        self._ck(load().lgf_slab_delta(self._h, _dev_ptr(sums, LGF_FP64, 2)))
+
+    def fft_local(self, inverse):
+        self._ck(load().lgf_slab_fft_local(self._h, int(bool(inverse))))
+
+    def transpose(self, stage, buf):
+        self._ck(load().lgf_slab_transpose(self._h, int(stage), _dev_ptr(buf, self.precision, self.V * 8)))
+
+    def fft_t(self):
+        self._ck(load().lgf_slab_fft_t(self._h))
+
+    def gbuild(self, alpha):
+        self._ck(load().lgf_slab_gbuild(self._h, float(alpha)))
+
+    def update(self):
+        self._ck(load().lgf_slab_update(self._h))
+
+    def get_field(self, out):
+        self._ck(load().lgf_slab_get_field(self._h, _dev_ptr(out, self.precision, self.V * 18)))
+        return out
+
+    def launch_count(self):
+        return int(load().lgf_slab_launch_count(self._h))
 
 
 def lgf_version() -> str:

@@ -106,6 +106,13 @@ static void cossin_2pi(int m, int L, double &c, double &s) {
     s = ss * (double)sv;
 }
 
+// the same tables for the slab-decomposed path (lgf_slab.cu)
+namespace lgf {
+bool host_valid_len(int L) { return valid_len(L); }
+void host_line_factor(int L, int &N1, int &N2) { line_factor(L, N1, N2); }
+void host_cossin_2pi(int m, int L, double &c, double &s) { cossin_2pi(m, L, c, s); }
+}
+
 template <class R>
 static int upload_twiddles(lgf_ctx *ctx) {
     for (int mu = 0; mu < 4; mu++) {

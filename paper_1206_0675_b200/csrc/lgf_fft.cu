@@ -56,7 +56,8 @@ __global__ void __launch_bounds__(256) k_fft_axis(C<R> *__restrict__ W, Geom g, 
             int c[4];
             site_coords(g, s, c);
             const R p2 = p2tab[c[0]] + p2tab[64 + c[1]] + p2tab[128 + c[2]] + p2tab[192 + c[3]];
-            const R f = (s == 0) ? (R)0 : scale / p2;
+            const R f = (p2 == (R)0) ? (R)0 : scale / p2;            // p2 = 0 only at k = 0 (R6); also right for a
+                                                                     // z-slab of k space (lgf_slab.cu), where s = 0 is not k = 0
             C<R> *e = tile + hi * ts.sHi + n * ts.sN + lo;
             *e = f * (*e);
         }

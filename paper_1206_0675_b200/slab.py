@@ -1,0 +1,270 @@
+"""ONE configuration sharded over several GPUs: t-slab decomposition of Algorithm 1.
+
+SURVEY.md section 8(e) / 8(f) NEXT-3; the paper's stated future work (its CPU code does the same
+decomposition with PFFT over MPI, :124).  Rank r of N owns the slices t = r T .. (r+1) T - 1 of the lattice.
+Every arithmetic step runs in liblgf's kernels through the per-rank entry points ``lgf_slab_*`` (include/lgf.h);
+this module only sequences them and moves the buffers between ranks.  Per iteration there are exactly four
+exchanges plus one two-double all-reduce:
+
+  halo LINKS  U_t of a rank's last slice     -> rank r+1   (a1: A_t(x - t), eq. 5)          S3 * n_l reals
+  all-to-all  t-slabs -> z-slabs of F_xyz[Delta]            (a2: the t lines of the 4-D FFT)  8 * V/N * (N-1)/N
+  all-to-all  z-slabs -> t-slabs                            (a4)                              the same
+  halo G      g of a rank's first slice      -> rank r-1   (a6: g(x + t), eq. 2)            S3 * 12 reals
+  all-reduce  (sum Re tr U, sum tr Delta Delta^dag)         (F, theta, eqs. 3, 6)             2 doubles
+
+Two exchange objects implement them:
+
+* ``DistExchange``: one process per GPU, torch.distributed (NCCL over NVLink / NVSwitch: batched isend / irecv for
+  the halos, ``all_to_all_single`` for the transposition, ``all_reduce`` for the sums).  On gloo it moves CPU
+  tensors the same way (tests/test_slab_gloo.py, world_size 2).
+* ``LocalExchange``: all N ranks emulated in ONE process on one GPU.  Each phase is run for every rank in turn and
+  the exchange is a set of device copies between the ranks' buffers, so no kernel ever waits on another rank
+  (B200_PROFILING.md: emulate ranks as successive launches over all ranks' data, never as concurrently waiting
+  kernels).  This is how the path is checked against the oracle on the one-GPU box (tests/test_gpu_slab.py).
+
+Both have the same three methods over LISTS of per-local-rank tensors (length N for LocalExchange, 1 for
+DistExchange), so ``SlabFixer`` is the same code in both cases.  No CPU fallback: the kernels need liblgf.so and
+a CUDA device.  This module never touches the oracle.
+"""
+from __future__ import annotations
+
+from typing import List, Sequence
+
+from . import binding as B
+
+
+class LocalExchange:
+    """N ranks emulated in one process (see module docstring)."""
+
+    def __init__(self, world: int):
+        if world < 1:
+            raise ValueError("world must be >= 1")
+        self.world = int(world)
+        self.local_ranks = list(range(self.world))
+
+    def shift(self, send: Sequence, recv: Sequence, step: int) -> None:
+        """recv[r] <- send[(r - step) mod N]: every rank sends to rank r + step."""
+        n = self.world
+        for r in range(n):
+            recv[r].copy_(send[(r - step) % n])
+
+    def all_to_all(self, send: Sequence, recv: Sequence) -> None:
+        """Chunk q of rank r's send buffer becomes chunk r of rank q's receive buffer (equal chunks)."""
+        n = self.world
+        for r in range(n):
+            dst = recv[r].view(n, -1)
+            for q in range(n):
+                dst[q].copy_(send[q].view(n, -1)[r])
+
+    def all_reduce_sum(self, vals: Sequence) -> None:
+        total = vals[0].clone()
+        for v in vals[1:]:
+            total += v                      # fixed order: rank 0, 1, ..., N-1
+        for v in vals:
+            v.copy_(total)
+
+
+class DistExchange:
+    """One process per rank over torch.distributed (nccl on the GPUs, gloo on the CPU)."""
+
+    def __init__(self, dist, group=None):
+        self.dist, self.group = dist, group
+        self.world = dist.get_world_size(group)
+        self.rank = dist.get_rank(group)
+        self.local_ranks = [self.rank]
+
+    def _global(self, r: int) -> int:
+        return r if self.group is None else self.dist.get_global_rank(self.group, r)
+
+    def shift(self, send, recv, step: int) -> None:
+        n, r, dist = self.world, self.rank, self.dist
+        if n == 1:
+            recv[0].copy_(send[0])
+            return
+        ops = [dist.P2POp(dist.isend, send[0], self._global((r + step) % n), self.group),
+               dist.P2POp(dist.irecv, recv[0], self._global((r - step) % n), self.group)]
+        for w in dist.batch_isend_irecv(ops):
+            w.wait()
+
+    def all_to_all(self, send, recv) -> None:
+        if self.world == 1:
+            recv[0].copy_(send[0])
+            return
+        self.dist.all_to_all_single(recv[0].view(-1), send[0].view(-1), group=self.group)
+
+    def all_reduce_sum(self, vals) -> None:
+        if self.world > 1:
+            self.dist.all_reduce(vals[0], group=self.group)
+
+
+def slab_of(links, rank: int, world: int):
+    """Rank `rank`'s t-slab of a canonical configuration [Lt, Lz, Ly, Lx, 4, 3, 3(, 2)] (a contiguous slice)."""
+    Lt = links.shape[0]
+    if Lt % world:
+        raise ValueError("world must divide Lt")
+    T = Lt // world
+    return links[rank * T:(rank + 1) * T]
+
+
+class SlabFixer:
+    """Algorithm 1 on one configuration sharded over ``exchange.world`` ranks.
+
+    dims = GLOBAL (Lx, Ly, Lz, Lt); world must divide Lt and Lz.  History entry n = (F, theta) of the configuration
+    after n updates since ``set_links`` (as lgf_iterate / lgf_fix, include/lgf.h)."""
+
+    def __init__(self, dims, precision=B.LGF_FP64, link_storage=B.LGF_LINKS_18, exchange=None, device=None):
+        import torch
+
+        self.torch = torch
+        self.ex = exchange if exchange is not None else LocalExchange(1)
+        self.dims = tuple(int(v) for v in dims)
+        self.precision, self.link_storage = int(precision), int(link_storage)
+        self.device = torch.device(device) if device is not None else torch.device("cuda", torch.cuda.current_device())
+        self.V = self.dims[0] * self.dims[1] * self.dims[2] * self.dims[3]
+        world = self.ex.world
+        stream = torch.cuda.current_stream(self.device)
+        self.ranks: List[B.SlabContext] = [B.SlabContext(self.dims, precision, link_storage, r, world, stream=stream)
+                                           for r in self.ex.local_ranks]
+        rdt = torch.float64 if precision == B.LGF_FP64 else torch.float32
+        mk = lambda n, dt=rdt: [torch.empty(n, dtype=dt, device=self.device) for _ in self.ranks]
+        c0 = self.ranks[0]
+        self._u_send, self._u_recv = mk(c0.halo_elems(B.LGF_HALO_LINKS)), mk(c0.halo_elems(B.LGF_HALO_LINKS))
+        self._g_send, self._g_recv = mk(c0.halo_elems(B.LGF_HALO_G)), mk(c0.halo_elems(B.LGF_HALO_G))
+        self._a_send, self._a_recv = mk(c0.V * 8), mk(c0.V * 8)
+        self._sums = mk(2, torch.float64)
+        self._hist = []                 # device tensors [2]: (sum Re tr U, sum tr Delta Delta^dag), all-reduced
+        self._measured = False          # W of every rank holds Delta of the current links and _hist[-1] their sums
+        self.updates = 0
+        self.exchanged_bytes = 0        # per rank, what the last iterate() sent (bench / DESIGN.md figures)
+
+    # -- configuration ----------------------------------------------------------------------------
+    def set_links(self, slabs: Sequence) -> None:
+        """One canonical slab per local rank ([T, Lz, Ly, Lx, 4, 3, 3, 2] real or [..., 3, 3] complex, on the device)."""
+        if len(slabs) != len(self.ranks):
+            raise ValueError("expected %d slab(s)" % len(self.ranks))
+        for c, s in zip(self.ranks, slabs):
+            c.set_links(s.contiguous())
+        self._hist, self._measured, self.updates = [], False, 0
+
+    def set_links_global(self, links) -> None:
+        self.set_links([slab_of(links, r, self.ex.world) for r in self.ex.local_ranks])
+
+    def get_links(self) -> list:
+        rdt = self.torch.float64 if self.precision == B.LGF_FP64 else self.torch.float32
+        out = []
+        for c in self.ranks:
+            t = self.torch.empty((c.T, self.dims[2], self.dims[1], self.dims[0], 4, 3, 3, 2), dtype=rdt, device=self.device)
+            out.append(c.get_links(t))
+        return out
+
+    # -- the steps of one iteration ---------------------------------------------------------------
+    def _step_delta(self) -> None:
+        """a1 (+ halo of U_t, all-reduce of the sums): Delta into every rank's work field, sums into the history."""
+        for c, s in zip(self.ranks, self._u_send):
+            c.halo_pack(B.LGF_HALO_LINKS, s)
+        self.ex.shift(self._u_send, self._u_recv, +1)
+        for c, r, sm in zip(self.ranks, self._u_recv, self._sums):
+            c.halo_unpack(B.LGF_HALO_LINKS, r)
+            c.delta(sm)
+        self.ex.all_reduce_sum(self._sums)
+        self._hist.append(self._sums[0].clone())
+        self._measured = True
+
+    def _step_accelerate(self) -> None:
+        """a2-a4: w = F^-1[(p2max / p2) F Delta] / V with the t lines gathered by two all-to-alls."""
+        for c, s in zip(self.ranks, self._a_send):
+            c.fft_local(False)
+            c.transpose(0, s)
+        self.ex.all_to_all(self._a_send, self._a_recv)
+        for c, s, r in zip(self.ranks, self._a_send, self._a_recv):
+            c.transpose(1, r)
+            c.fft_t()
+            c.transpose(2, s)
+        self.ex.all_to_all(self._a_send, self._a_recv)
+        for c, r in zip(self.ranks, self._a_recv):
+            c.transpose(3, r)
+            c.fft_local(True)
+
+    def _step_update(self, alpha: float) -> None:
+        """a5 + a6 (+ halo of g)."""
+        for c, s in zip(self.ranks, self._g_send):
+            c.gbuild(alpha)
+            c.halo_pack(B.LGF_HALO_G, s)
+        self.ex.shift(self._g_send, self._g_recv, -1)
+        for c, r in zip(self.ranks, self._g_recv):
+            c.halo_unpack(B.LGF_HALO_G, r)
+            c.update()
+        self._measured = False
+        self.updates += 1
+
+    def _bytes_per_iteration(self) -> int:
+        n, es = self.ex.world, self._a_send[0].element_size()
+        if n == 1:
+            return 0
+        a2a = 2 * self._a_send[0].numel() * es * (n - 1) // n
+        return a2a + (self._u_send[0].numel() + self._g_send[0].numel()) * es + 16
+
+    # -- public: same meaning as lgf_measure / lgf_iterate / lgf_fix ---------------------------------
+    def measure(self):
+        """(F, theta) of the current configuration (eqs. 3, 6); synchronises."""
+        if not self._measured:
+            self._step_delta()
+            sums = self._hist.pop()           # a measurement records nothing ...
+            self._measured = False            # ... so the next iterate measures (and records) again
+        else:
+            sums = self._hist[-1]
+        f, t = sums.tolist()
+        return f / (12.0 * self.V), t / (3.0 * self.V)
+
+    def iterate(self, alpha: float, n: int) -> None:
+        """n updates regardless of theta; leaves n + 1 history entries from a fresh configuration.  Never reads
+        a value back to the host."""
+        for _ in range(int(n)):
+            if not self._measured:
+                self._step_delta()
+            self._step_accelerate()
+            self._step_update(alpha)
+        if not self._measured:
+            self._step_delta()
+        self.exchanged_bytes = self._bytes_per_iteration() * int(n)
+
+    def fix(self, alpha: float, tol: float, max_iter: int) -> int:
+        """measure; while theta >= tol and it < max_iter: update; measure.  Returns the number of updates."""
+        it = 0
+        while True:
+            if not self._measured:
+                self._step_delta()
+            theta = float(self._hist[-1][1].item()) / (3.0 * self.V)
+            if theta != theta:
+                raise B.LgfError(B.LGF_ENAN, "theta became NaN")
+            if theta < tol or it >= max_iter:
+                return it
+            self._step_accelerate()
+            self._step_update(alpha)
+            it += 1
+
+    def history(self):
+        """(F[], theta[]) numpy arrays of the recorded entries; synchronises."""
+        import numpy as np
+
+        if not self._hist:
+            return np.zeros(0), np.zeros(0)
+        h = self.torch.stack(self._hist).cpu().numpy()
+        return h[:, 0] / (12.0 * self.V), h[:, 1] / (3.0 * self.V)
+
+    def work_field(self) -> list:
+        """Every local rank's work field (Delta after a measurement) as [T, Lz, Ly, Lx, 3, 3, 2] tensors."""
+        rdt = self.torch.float64 if self.precision == B.LGF_FP64 else self.torch.float32
+        out = []
+        for c in self.ranks:
+            t = self.torch.empty((c.T, self.dims[2], self.dims[1], self.dims[0], 3, 3, 2), dtype=rdt, device=self.device)
+            out.append(c.get_field(t))
+        return out
+
+    def launch_count(self) -> int:
+        return sum(c.launch_count() for c in self.ranks)
+
+    def destroy(self) -> None:
+        for c in self.ranks:
+            c.destroy()
+        self.ranks = []
