@@ -231,10 +231,9 @@ const char *lgf_version(void);
  * paper_1206_0675_b200/slab.py) -- no kernel waits on another rank.  One iteration of Algorithm 1
  * is, on every rank:
  *   halo_pack(LINKS) -> [send to r+1, receive from r-1] -> halo_unpack(LINKS) -> delta(sums) -> [all-reduce sums:
- *   F = sums[0] / (12 V), theta = sums[1] / (3 V), V the GLOBAL volume (eqs. 3, 6)] -> fft_local(0) ->
- *   transpose(0, send) -> [all-to-all] -> transpose(1, recv) -> fft_t -> transpose(2, send) -> [all-to-all] ->
- *   transpose(3, recv) -> fft_local(1) -> gbuild(alpha) -> halo_pack(G) -> [send to r-1, receive from r+1] ->
- *   halo_unpack(G) -> update.
+ *   F = sums[0] / (12 V), theta = sums[1] / (3 V), V the GLOBAL volume (eqs. 3, 6)] -> fft_forward(send) ->
+ *   [all-to-all] -> fft_t(recv, send) -> [all-to-all] -> fft_inverse_g(recv, alpha) -> halo_pack(G) ->
+ *   [send to r-1, receive from r+1] -> halo_unpack(G) -> update.
  * With nranks = 1 the "exchanges" are copies of a rank's send buffer into its own receive buffer (periodic wrap).
  * The result equals the one-GPU path's up to the rounding order of the F / theta sums and of the FFT passes.
  * Same precision / storage / error conventions as above; messages from lgf_slab_last_error.  All calls are
@@ -260,15 +259,20 @@ int lgf_slab_halo_unpack(lgf_slab *ctx, int which, const void *d_recv);
 /* a1 on the slab: Delta(x) into the work field; d_sums[0] = sum Re tr U_mu(x), d_sums[1] = sum tr(Delta Delta^dag)
  * over the slab's sites (device doubles, fixed summation order). */
 int lgf_slab_delta(lgf_slab *ctx, double *d_sums);
-/* the x, y, z passes of the 4-D FFT on the slab's work field: inverse == 0 forward (x, y, z), else inverse (z, y, x) */
-int lgf_slab_fft_local(lgf_slab *ctx, int inverse);
-/* the two sides of the two all-to-alls; d_buf holds 8 reals per local site, ordered [q][c][tl][zl][y][x] with
- * chunk q (1 / nranks of the buffer) the part that goes to / came from rank q:
- *   stage 0: work field (t-slabs) -> send buffer      stage 1: receive buffer -> z-slab field
- *   stage 2: z-slab field -> send buffer              stage 3: receive buffer -> work field (t-slabs) */
-int lgf_slab_transpose(lgf_slab *ctx, int stage, void *d_buf);
-/* on the z-slab field: forward t, times p2max / (V p2(k)) with the zero mode set to 0, inverse t (Alg. 1 lines 4-7) */
-int lgf_slab_fft_t(lgf_slab *ctx);
+/* The 4-D FFT around the two all-to-alls.  An all-to-all buffer holds 8 reals per local site, ordered
+ * [q][c][tl][zl][y][x]: chunk q (1 / nranks of the buffer) is the part that goes to / came from rank q, c = 0..3 the
+ * packed component of the work field, tl / zl the t / z index inside the chunk (t = q T + tl on the t-slab side's
+ * peer, z = q Zl + zl).  The passes next to an all-to-all read and write these buffers directly:
+ *   fft_forward:   forward x, y in place, forward z from the work field into d_send                (Alg. 1 line 4)
+ *   fft_t:         t lines of this rank's z-slab, d_recv -> d_send (distinct buffers): forward t, times
+ *                  p2max / (V p2(k)) with the zero mode set to 0, inverse t                       (lines 4-7)
+ *   fft_inverse:   inverse z from d_recv into the work field, inverse y, x: w(x) in the work field  (line 6)
+ *   fft_inverse_g: the same, ending in a5, g(x) = GS(1 + i (alpha / 2) w(x)) (line 10) -- fused into the last
+ *                  sweep where the lattice allows (the work field then does not hold w) */
+int lgf_slab_fft_forward(lgf_slab *ctx, void *d_send);
+int lgf_slab_fft_t(lgf_slab *ctx, const void *d_recv, void *d_send);
+int lgf_slab_fft_inverse(lgf_slab *ctx, const void *d_recv);
+int lgf_slab_fft_inverse_g(lgf_slab *ctx, const void *d_recv, double alpha);
 /* a5: g(x) = GS(1 + i (alpha / 2) w(x)) on the slab */
 int lgf_slab_gbuild(lgf_slab *ctx, double alpha);
 /* a6: U_mu(x) <- g(x) U_mu(x) g(x + mu)^dag on the slab, in place */

@@ -74,9 +74,10 @@ SIGNATURES = {
     "lgf_slab_halo_pack": (_i, [_vp, _i, _vp]),
     "lgf_slab_halo_unpack": (_i, [_vp, _i, _vp]),
     "lgf_slab_delta": (_i, [_vp, _vp]),
-    "lgf_slab_fft_local": (_i, [_vp, _i]),
-    "lgf_slab_transpose": (_i, [_vp, _i, _vp]),
-    "lgf_slab_fft_t": (_i, [_vp]),
+    "lgf_slab_fft_forward": (_i, [_vp, _vp]),
+    "lgf_slab_fft_t": (_i, [_vp, _vp, _vp]),
+    "lgf_slab_fft_inverse": (_i, [_vp, _vp]),
+    "lgf_slab_fft_inverse_g": (_i, [_vp, _vp, _d]),
     "lgf_slab_gbuild": (_i, [_vp, _d]),
     "lgf_slab_update": (_i, [_vp]),
     "lgf_slab_get_field": (_i, [_vp, _vp]),
@@ -365,14 +366,18 @@ class SlabContext:
     def delta(self, sums):
         self._ck(load().lgf_slab_delta(self._h, _dev_ptr(sums, LGF_FP64, 2)))
 
-    def fft_local(self, inverse):
-        self._ck(load().lgf_slab_fft_local(self._h, int(bool(inverse))))
+    def fft_forward(self, send):
+        self._ck(load().lgf_slab_fft_forward(self._h, _dev_ptr(send, self.precision, self.V * 8)))
 
-    def transpose(self, stage, buf):
-        self._ck(load().lgf_slab_transpose(self._h, int(stage), _dev_ptr(buf, self.precision, self.V * 8)))
+    def fft_t(self, recv, send):
+        self._ck(load().lgf_slab_fft_t(self._h, _dev_ptr(recv, self.precision, self.V * 8),
+                                       _dev_ptr(send, self.precision, self.V * 8)))
 
-    def fft_t(self):
-        self._ck(load().lgf_slab_fft_t(self._h))
+    def fft_inverse(self, recv):
+        self._ck(load().lgf_slab_fft_inverse(self._h, _dev_ptr(recv, self.precision, self.V * 8)))
+
+    def fft_inverse_g(self, recv, alpha):
+        self._ck(load().lgf_slab_fft_inverse_g(self._h, _dev_ptr(recv, self.precision, self.V * 8), float(alpha)))
 
     def gbuild(self, alpha):
         self._ck(load().lgf_slab_gbuild(self._h, float(alpha)))

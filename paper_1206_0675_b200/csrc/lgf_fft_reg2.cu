@@ -210,6 +210,13 @@ bool fft_reg2_supported(const Geom &g) {
     const long long planes = 4LL * g.L[2] * g.L[3];
     return planes % 8 == 0 && g.S[2] % 8 == 0;
 }
+// the (x, y) sweeps alone (which = 0, 2, 3) for a geometry whose last two extents are arbitrary -- a t-slab of the
+// sharded path (lgf_slab.cu): square planes of a supported length, whole CTAs of planes, and for the g output
+// the four components of P / 4 (z, t) slices per CTA
+bool fft_reg2_xy_supported(const Geom &g) {
+    return g.L[0] == g.L[1] && reg2_len(g.L[0]) && (4LL * g.L[2] * g.L[3]) % 8 == 0 && ((long long)g.L[2] * g.L[3]) % 2 == 0;
+}
+bool fft_reg2_xy_gout(const Geom &g, int prec) { return fft_reg2_xy_supported(g) && !(g.L[0] == 64 && prec == 8); }
 // can the inverse (x, y) sweep end with the g-build for this lattice and precision (bytes per real)?
 bool fft_reg2_gout(const Geom &g, int prec) {
     if (!fft_reg2_supported(g)) return false;

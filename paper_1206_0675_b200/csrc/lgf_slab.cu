@@ -4,9 +4,11 @@
 // Rank r of N owns the t-slab  t = r T .. (r+1) T - 1,  T = Lt / N  (all x, y, z), i.e. a contiguous slice of the
 // canonical configuration.  One iteration of Algorithm 1 then needs exactly these exchanges:
 //   a1    Delta(x) wants U_t(x - t) of the slice below the slab: one 3-D slice of U_t from rank r-1   (halo, LINKS)
-//   a2-a4 x, y, z are whole inside the slab: transformed locally (lgf_fft.cu, one pass per axis); the t lines are
-//         gathered by an ALL-TO-ALL that turns t-slabs into z-slabs (rank r gets z = r Zl .. (r+1) Zl - 1 of every
-//         t, Zl = Lz / N), the t pass does forward + p2max / (V p2(k)) + inverse there, a second all-to-all goes back
+//   a2-a4 x, y, z are whole inside the slab: (x, y) planes by the register-line sweeps of lgf_fft_reg2.cu (else one pass
+//         per axis, lgf_fft.cu); the t lines are gathered by an ALL-TO-ALL that turns t-slabs into z-slabs (rank r gets
+//         z = r Zl .. (r+1) Zl - 1 of every t, Zl = Lz / N).  The passes next to it work straight on its buffers: forward z
+//         writes the send buffer, the t pass (forward, times p2max / (V p2(k)), inverse) reads the receive buffer and writes
+//         the send buffer of the second all-to-all, inverse z reads its receive buffer -- no pack / unpack pass
 //   a6    U_t(x) g(x + t)^dag wants g of the slice above the slab: one slice of g from rank r+1          (halo, G)
 //   F, theta: per-rank sums, all-reduced by the caller (two doubles).
 // This file holds the kernels and the per-rank context; the exchanges themselves are the caller's (NCCL through
@@ -20,6 +22,7 @@
 #include <vector>
 
 #include "../../include/lgf.h"
+#include "lgf_fft_steps.cuh"
 #include "lgf_state.cuh"
 
 namespace lgf {
@@ -102,26 +105,91 @@ __global__ void __launch_bounds__(SLAB_THREADS) k_slab_update(C<R> *__restrict__
     }
 }
 
-// The two index maps of the all-to-all.  Buffer element b = (((q 4 + c) T + tl) Zl + zl) Sxy + xy  (chunk q goes to /
-// came from rank q; c = packed component of W; tl, zl local to the chunk).
-//   side 0 (t-slab field  [c][tl][z][xy],  z = q Zl + zl):    w = c V + (tl Lz + q Zl + zl) Sxy + xy
-//   side 1 (z-slab field  [c][t][zl][xy],  t = q T + tl):     w = c V + ((q T + tl) Zl + zl) Sxy + xy
-// dir 0: buf[b] = field[w];  dir 1: field[w] = buf[b].
+// Where element n of a line lives: base + (n / D) strideQ + (n % D) strideN.  The all-to-all buffers are ordered
+// [q][c][tl][zl][xy] (chunk q goes to / came from rank q; c = packed component of W; tl, zl local to the chunk), so
+//   a z line in a buffer   (z = q Zl + zl):  D = Zl, strideQ = chunk, strideN = Sxy,     base = (c T + tl) Zl Sxy + xy
+//   a t line in a buffer   (t = q T + tl):   D = T,  strideQ = chunk, strideN = Zl Sxy,  base = (c T Zl + zl) Sxy + xy
+//   a z line in the field W[c][tl][z][xy]:   D = Lz (one piece),      strideN = Sxy,     base = c V + tl Lz Sxy + xy
+// with chunk = 4 T Zl Sxy elements.  blockIdx.y = the "other" local index (tl for z lines, zl for t lines), blockIdx.z = c.
+struct LineAddr {
+    long long stride_c, stride_o, strideQ, strideN;
+    int D;
+};
+__device__ __forceinline__ long long line_elem(const LineAddr &a, long long base, int n) {
+    return base + (long long)(n / a.D) * a.strideQ + (long long)(n % a.D) * a.strideN;
+}
+
+// One line pass of the 4-D FFT (Alg. 1 lines 3-8) that reads with one address map and writes with another, so that
+// the passes next to an all-to-all work straight on its buffers and no separate pack / unpack pass exists:
+//   z forward   FFT_FWD             src = W (t-slab)        dst = send buffer
+//   t           FFT_FWD_SCALE_INV   src = receive buffer    dst = send buffer     (times p2max / (V p2(k)), k = 0 -> 0)
+//   z inverse   FFT_INV             src = receive buffer    dst = W
+// A CTA takes nlo consecutive (x, y) indices of one line bundle; the transform itself is lgf_fft_steps.cuh's.
+template <class R, int L, int MODE>
+__global__ void __launch_bounds__(256) k_slab_fft_line(const C<R> *__restrict__ src, C<R> *__restrict__ dst, LineAddr as,
+                                                       LineAddr ad, int nlo, int Lx, const C<R> *__restrict__ twiddle,
+                                                       const R *__restrict__ p2tab, R scale) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    C<R> *tw = reinterpret_cast<C<R> *>(smem_raw);
+    C<R> *tile = tw + 64;
+    TileShape ts;
+    ts.nlo = nlo; ts.nhi = 1; ts.sN = nlo; ts.sHi = 0;
+    const long long xy0 = (long long)blockIdx.x * nlo;
+    const long long bs = (long long)blockIdx.z * as.stride_c + (long long)blockIdx.y * as.stride_o + xy0;
+    const long long bd = (long long)blockIdx.z * ad.stride_c + (long long)blockIdx.y * ad.stride_o + xy0;
+    for (int m = threadIdx.x; m < L; m += blockDim.x) tw[m] = twiddle[m];
+    const int nelem = L * nlo;
+    for (int idx = threadIdx.x; idx < nelem; idx += blockDim.x) {
+        const int lo = idx % nlo, n = idx / nlo;
+        tile[idx] = src[line_elem(as, bs, n) + lo];
+    }
+    __syncthreads();
+    if constexpr (MODE == FFT_FWD || MODE == FFT_FWD_SCALE_INV) line_fft_forward<R, L>(tile, tw, ts);
+    if constexpr (MODE == FFT_FWD_SCALE_INV) {
+        // t lines: blockIdx.y = zl; p2tab[128 + zl] is this rank's z-slab of the z table (positions, not frequencies)
+        for (int idx = threadIdx.x; idx < nelem; idx += blockDim.x) {
+            const int lo = idx % nlo, n = idx / nlo;
+            const int xy = (int)xy0 + lo, x = xy % Lx, y = xy / Lx;
+            const R p2 = p2tab[x] + p2tab[64 + y] + p2tab[128 + blockIdx.y] + p2tab[192 + n];
+            const R f = (p2 == (R)0) ? (R)0 : scale / p2;           // p2 = 0 only at k = 0 (R6)
+            tile[idx] = f * tile[idx];
+        }
+        __syncthreads();
+    }
+    if constexpr (MODE == FFT_INV || MODE == FFT_FWD_SCALE_INV) line_fft_inverse<R, L>(tile, tw, ts);
+    for (int idx = threadIdx.x; idx < nelem; idx += blockDim.x) {
+        const int lo = idx % nlo, n = idx / nlo;
+        dst[line_elem(ad, bd, n) + lo] = tile[idx];
+    }
+}
+
+template <class R, int L>
+static cudaError_t launch_line_L(int mode, const C<R> *src, C<R> *dst, const LineAddr &as, const LineAddr &ad, int nlo,
+                                 dim3 grid, int Lx, const R *twiddle, const R *p2tab, R scale, cudaStream_t stream) {
+    const size_t smem = (64 + (size_t)L * nlo) * sizeof(C<R>);
+    const C<R> *tw = reinterpret_cast<const C<R> *>(twiddle);
+    auto go = [&](auto kern) {
+        if (smem > 48 * 1024) {
+            cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            if (e != cudaSuccess) return e;
+        }
+        kern<<<grid, 256, smem, stream>>>(src, dst, as, ad, nlo, Lx, tw, p2tab, scale);
+        return cudaGetLastError();
+    };
+    if (mode == FFT_FWD) return go(k_slab_fft_line<R, L, FFT_FWD>);
+    if (mode == FFT_INV) return go(k_slab_fft_line<R, L, FFT_INV>);
+    return go(k_slab_fft_line<R, L, FFT_FWD_SCALE_INV>);
+}
 template <class R>
-__global__ void __launch_bounds__(SLAB_THREADS) k_slab_transpose(C<R> *__restrict__ field, C<R> *__restrict__ buf, long long V,
-                                                                 int Sxy, int T, int Zl, int N, int side, int dir) {
-    const long long b = (long long)blockIdx.x * SLAB_THREADS + threadIdx.x;
-    if (b >= 4 * V) return;
-    long long r = b;
-    const int xy = (int)(r % Sxy); r /= Sxy;
-    const int zl = (int)(r % Zl); r /= Zl;
-    const int tl = (int)(r % T); r /= T;
-    const int c = (int)(r % 4);
-    const int q = (int)(r / 4);
-    const long long w = side == 0 ? (long long)c * V + ((long long)tl * (Zl * N) + q * Zl + zl) * Sxy + xy
-                                  : (long long)c * V + (((long long)q * T + tl) * Zl + zl) * Sxy + xy;
-    if (dir == 0) buf[b] = field[w];
-    else field[w] = buf[b];
+static cudaError_t launch_line(int L, int mode, const C<R> *src, C<R> *dst, const LineAddr &as, const LineAddr &ad, int nlo,
+                               dim3 grid, int Lx, const R *twiddle, const R *p2tab, R scale, cudaStream_t stream) {
+    switch (L) {
+#define LGF_CASE(LEN) case LEN: return launch_line_L<R, LEN>(mode, src, dst, as, ad, nlo, grid, Lx, twiddle, p2tab, scale, stream);
+        LGF_CASE(2) LGF_CASE(3) LGF_CASE(4) LGF_CASE(6) LGF_CASE(8) LGF_CASE(12) LGF_CASE(16) LGF_CASE(24)
+        LGF_CASE(32) LGF_CASE(48) LGF_CASE(64)
+#undef LGF_CASE
+        default: return cudaErrorInvalidValue;
+    }
 }
 
 }  // namespace lgf
@@ -133,13 +201,11 @@ struct lgf_slab {
     int rank = 0, N = 1, T = 0, Zl = 0;
     int prec = 0, nr = 3;
     Geom gl{};                   // the slab: (Lx, Ly, Lz, T)
-    Geom gt{};                   // the z-slab the t pass works on: (Lx, Ly, Zl, Lt); same number of sites
     long long Vglobal = 0;
     cudaStream_t stream = nullptr;
     void *links = nullptr;       // C<R>[4][3 nr][Vl]
     void *uhalo = nullptr;       // C<R>[3 nr][S3]   U_t of the slice below the slab
     void *W = nullptr;           // C<R>[4][Vl]      packed Delta / w, t-slab order
-    void *Wt = nullptr;          // C<R>[4][Vl]      the same field in z-slab order
     void *G = nullptr;           // C<R>[6][Vl]
     void *ghalo = nullptr;       // C<R>[6][S3]      g of the slice above the slab
     double *partial = nullptr;
@@ -147,7 +213,11 @@ struct lgf_slab {
     DevState *st = nullptr;      // all zero: the kernels shared with the one-GPU path look at st->done
     void *twiddle[4] = {nullptr, nullptr, nullptr, nullptr};
     void *p2tab = nullptr;       // R[4][64], z section shifted to this rank's z-slab
-    AxisPass pass_fwd[3], pass_inv[3], pass_t;
+    AxisPass pass_fwd[2], pass_inv[2];   // x, y one axis per pass (any supported length), used unless xy_reg
+    bool xy_reg = false;         // (x, y) planes by the register-line sweeps of lgf_fft_reg2.cu (square planes of 16 / 32 / 64)
+    bool xy_gout = false;        // ... and the inverse one can end with the g-build (a5)
+    int nlo_z = 1, nlo_t = 1;    // consecutive (x, y) indices per CTA of the z / t line passes
+    LineAddr a_w{}, a_zbuf{}, a_tbuf{};
     bool have_links = false;
     long long launches = 0;
     std::string err;
@@ -221,8 +291,9 @@ static int slab_tables(lgf_slab *ctx) {
         int N1, N2;
         host_line_factor(L, N1, N2);
         const int first = mu == 2 ? ctx->rank * ctx->Zl : 0, count = mu == 2 ? ctx->Zl : L;
+        const bool natural = mu < 2 && ctx->xy_reg;        // the register-line sweeps leave kx, ky in natural order
         for (int i = 0; i < count; i++) {
-            const int p = first + i, k = (p / N2) + N1 * (p % N2);
+            const int p = first + i, k = natural ? p : (p / N2) + N1 * (p % N2);
             double c, s;
             host_cossin_2pi(k, 2 * L, c, s);
             p2[mu * 64 + i] = (R)(4.0 * s * s);
@@ -233,23 +304,62 @@ static int slab_tables(lgf_slab *ctx) {
     return LGF_OK;
 }
 
+// forward x, y (in place in W), then forward z from W into the send buffer of the first all-to-all
 template <class R>
-static int slab_fft_local(lgf_slab *ctx, int inverse) {
+static int slab_fft_forward(lgf_slab *ctx, void *d_send) {
     const R *tw[4] = {(const R *)ctx->twiddle[0], (const R *)ctx->twiddle[1], (const R *)ctx->twiddle[2], (const R *)ctx->twiddle[3]};
-    for (int i = 0; i < 3; i++) {
-        const AxisPass &p = inverse ? ctx->pass_inv[i] : ctx->pass_fwd[i];
-        SCK(launch_fft_pass<R>(p, (C<R> *)ctx->W, ctx->gl, tw, (const R *)ctx->p2tab, (R)0, ctx->st, ctx->stream));
+    if (ctx->xy_reg) {
+        SCK(launch_fft_reg2<R>(0, ctx->gl, (C<R> *)ctx->W, (const R *)ctx->p2tab, (R)0, ctx->st, ctx->stream, nullptr, (R)0));
         ctx->launches++;
+    } else {
+        for (int i = 0; i < 2; i++) {
+            SCK(launch_fft_pass<R>(ctx->pass_fwd[i], (C<R> *)ctx->W, ctx->gl, tw, (const R *)ctx->p2tab, (R)0, ctx->st, ctx->stream));
+            ctx->launches++;
+        }
     }
+    const dim3 grid((unsigned)(ctx->gl.S[2] / ctx->nlo_z), ctx->T, 4);
+    SCK(launch_line<R>(ctx->dims[2], FFT_FWD, (const C<R> *)ctx->W, (C<R> *)d_send, ctx->a_w, ctx->a_zbuf, ctx->nlo_z, grid,
+                       ctx->dims[0], tw[2], (const R *)ctx->p2tab, (R)0, ctx->stream));
+    ctx->launches++;
     return LGF_OK;
 }
 
+// the t lines, from the receive buffer of the first all-to-all into the send buffer of the second
 template <class R>
-static int slab_fft_t(lgf_slab *ctx) {
-    const R *tw[4] = {(const R *)ctx->twiddle[0], (const R *)ctx->twiddle[1], (const R *)ctx->twiddle[2], (const R *)ctx->twiddle[3]};
+static int slab_fft_t(lgf_slab *ctx, const void *d_recv, void *d_send) {
     const R scale = (R)(16.0 / (double)ctx->Vglobal);              // p2max / V (Alg. 1 lines 5, 7; R5)
-    SCK(launch_fft_pass<R>(ctx->pass_t, (C<R> *)ctx->Wt, ctx->gt, tw, (const R *)ctx->p2tab, scale, ctx->st, ctx->stream));
+    const dim3 grid((unsigned)(ctx->gl.S[2] / ctx->nlo_t), ctx->Zl, 4);
+    SCK(launch_line<R>(ctx->dims[3], FFT_FWD_SCALE_INV, (const C<R> *)d_recv, (C<R> *)d_send, ctx->a_tbuf, ctx->a_tbuf, ctx->nlo_t,
+                       grid, ctx->dims[0], (const R *)ctx->twiddle[3], (const R *)ctx->p2tab, scale, ctx->stream));
     ctx->launches++;
+    return LGF_OK;
+}
+
+// inverse z from the receive buffer of the second all-to-all into W, then inverse y, x; with_g: ending in a5
+template <class R>
+static int slab_fft_inverse(lgf_slab *ctx, const void *d_recv, bool with_g, double alpha) {
+    const R *tw[4] = {(const R *)ctx->twiddle[0], (const R *)ctx->twiddle[1], (const R *)ctx->twiddle[2], (const R *)ctx->twiddle[3]};
+    const dim3 grid((unsigned)(ctx->gl.S[2] / ctx->nlo_z), ctx->T, 4);
+    SCK(launch_line<R>(ctx->dims[2], FFT_INV, (const C<R> *)d_recv, (C<R> *)ctx->W, ctx->a_zbuf, ctx->a_w, ctx->nlo_z, grid,
+                       ctx->dims[0], tw[2], (const R *)ctx->p2tab, (R)0, ctx->stream));
+    ctx->launches++;
+    const R ha = (R)(0.5 * alpha);
+    if (ctx->xy_reg) {
+        const bool fuse = with_g && ctx->xy_gout;
+        SCK(launch_fft_reg2<R>(fuse ? 3 : 2, ctx->gl, (C<R> *)ctx->W, (const R *)ctx->p2tab, (R)0, ctx->st, ctx->stream,
+                               (C<R> *)ctx->G, ha));
+        ctx->launches++;
+        if (fuse) return LGF_OK;
+    } else {
+        for (int i = 0; i < 2; i++) {
+            SCK(launch_fft_pass<R>(ctx->pass_inv[i], (C<R> *)ctx->W, ctx->gl, tw, (const R *)ctx->p2tab, (R)0, ctx->st, ctx->stream));
+            ctx->launches++;
+        }
+    }
+    if (with_g) {
+        SCK(launch_gbuild<R>((const C<R> *)ctx->W, (C<R> *)ctx->G, ctx->gl, ha, ctx->st, ctx->stream));
+        ctx->launches++;
+    }
     return LGF_OK;
 }
 
@@ -281,19 +391,6 @@ static int slab_update(lgf_slab *ctx) {
     return LGF_OK;
 }
 
-template <class R>
-static int slab_transpose(lgf_slab *ctx, int stage, void *d_buf) {
-    // stage 0: W (t-slabs) -> send buffer;  1: receive buffer -> Wt (z-slabs);  2: Wt -> send buffer;  3: receive buffer -> W
-    const int side = (stage == 0 || stage == 3) ? 0 : 1, dir = (stage == 0 || stage == 2) ? 0 : 1;
-    C<R> *field = (C<R> *)(side == 0 ? ctx->W : ctx->Wt);
-    const long long n = 4 * ctx->gl.V;
-    k_slab_transpose<R><<<(unsigned)((n + SLAB_THREADS - 1) / SLAB_THREADS), SLAB_THREADS, 0, ctx->stream>>>(
-        field, (C<R> *)d_buf, ctx->gl.V, (int)ctx->gl.S[2], ctx->T, ctx->Zl, ctx->N, side, dir);
-    SCK(cudaGetLastError());
-    ctx->launches++;
-    return LGF_OK;
-}
-
 extern "C" {
 
 const char *lgf_slab_last_error(const lgf_slab *ctx) { return ctx ? ctx->err.c_str() : g_slab_err.c_str(); }
@@ -301,7 +398,7 @@ const char *lgf_slab_last_error(const lgf_slab *ctx) { return ctx ? ctx->err.c_s
 int lgf_slab_destroy(lgf_slab *ctx) {
     if (!ctx) return LGF_EINVAL;
     cudaStreamSynchronize(ctx->stream);
-    void *bufs[] = {ctx->links, ctx->uhalo, ctx->W, ctx->Wt, ctx->G, ctx->ghalo, ctx->partial, ctx->st, ctx->p2tab,
+    void *bufs[] = {ctx->links, ctx->uhalo, ctx->W, ctx->G, ctx->ghalo, ctx->partial, ctx->st, ctx->p2tab,
                     ctx->twiddle[0], ctx->twiddle[1], ctx->twiddle[2], ctx->twiddle[3]};
     for (void *b : bufs) cudaFree(b);
     cudaGetLastError();
@@ -336,14 +433,20 @@ int lgf_slab_create(const int dims[4], int precision, int link_storage, int rank
     ctx->Zl = dims[2] / nranks;
     ctx->Vglobal = 1;
     for (int mu = 0; mu < 4; mu++) { ctx->dims[mu] = dims[mu]; ctx->Vglobal *= dims[mu]; }
-    const int Ll[4] = {dims[0], dims[1], dims[2], ctx->T}, Lt[4] = {dims[0], dims[1], ctx->Zl, dims[3]};
-    long long Sl = 1, St = 1;
-    for (int mu = 0; mu < 4; mu++) {
-        ctx->gl.L[mu] = Ll[mu]; ctx->gl.S[mu] = Sl; Sl *= Ll[mu];
-        ctx->gt.L[mu] = Lt[mu]; ctx->gt.S[mu] = St; St *= Lt[mu];
-    }
+    const int Ll[4] = {dims[0], dims[1], dims[2], ctx->T};
+    long long Sl = 1;
+    for (int mu = 0; mu < 4; mu++) { ctx->gl.L[mu] = Ll[mu]; ctx->gl.S[mu] = Sl; Sl *= Ll[mu]; }
     ctx->gl.V = Sl;
-    ctx->gt.V = St;
+    ctx->xy_reg = fft_reg2_xy_supported(ctx->gl);
+    ctx->xy_gout = fft_reg2_xy_gout(ctx->gl, precision);
+    {   // address maps of the line passes (LineAddr) and their tiles: about 2048 complex elements per CTA
+        const long long Sxy = ctx->gl.S[2], chunk = 4LL * ctx->T * ctx->Zl * Sxy;
+        ctx->a_w = LineAddr{Sl, (long long)dims[2] * Sxy, 0, Sxy, dims[2]};
+        ctx->a_zbuf = LineAddr{(long long)ctx->T * ctx->Zl * Sxy, (long long)ctx->Zl * Sxy, chunk, Sxy, ctx->Zl};
+        ctx->a_tbuf = LineAddr{(long long)ctx->T * ctx->Zl * Sxy, Sxy, chunk, (long long)ctx->Zl * Sxy, ctx->T};
+        ctx->nlo_z = (int)divisor_le(Sxy, 2048 / dims[2]);
+        ctx->nlo_t = (int)divisor_le(Sxy, 2048 / dims[3]);
+    }
     const size_t V = (size_t)Sl, S3 = (size_t)ctx->gl.S[3], cb = 2 * (size_t)precision;
     ctx->nb = (int)((V + SLAB_THREADS - 1) / SLAB_THREADS);
     int rc = LGF_OK;
@@ -356,7 +459,6 @@ int lgf_slab_create(const int dims[4], int precision, int link_storage, int rank
     alloc(&ctx->links, V * 4 * 3 * ctx->nr * cb);
     alloc(&ctx->uhalo, S3 * 3 * ctx->nr * cb);
     alloc(&ctx->W, V * 4 * cb);
-    alloc(&ctx->Wt, V * 4 * cb);
     alloc(&ctx->G, V * 6 * cb);
     alloc(&ctx->ghalo, S3 * 6 * cb);
     alloc((void **)&ctx->partial, sizeof(double) * 2 * ctx->nb);
@@ -371,11 +473,10 @@ int lgf_slab_create(const int dims[4], int precision, int link_storage, int rank
         lgf_slab_destroy(ctx);
         return rc;
     }
-    for (int a = 0; a < 3; a++) {
+    for (int a = 0; a < 2; a++) {
         ctx->pass_fwd[a] = slab_axis_pass(ctx->gl, precision, a, FFT_FWD);
-        ctx->pass_inv[a] = slab_axis_pass(ctx->gl, precision, 2 - a, FFT_INV);
+        ctx->pass_inv[a] = slab_axis_pass(ctx->gl, precision, 1 - a, FFT_INV);
     }
-    ctx->pass_t = slab_axis_pass(ctx->gt, precision, 3, FFT_FWD_SCALE_INV);
     *out = ctx;
     return LGF_OK;
 }
@@ -442,19 +543,24 @@ int lgf_slab_delta(lgf_slab *ctx, double *d_sums) {
     return ctx->prec == LGF_FP64 ? slab_delta<double>(ctx, d_sums) : slab_delta<float>(ctx, d_sums);
 }
 
-int lgf_slab_fft_local(lgf_slab *ctx, int inverse) {
-    if (!ctx) return LGF_EINVAL;
-    return ctx->prec == LGF_FP64 ? slab_fft_local<double>(ctx, inverse) : slab_fft_local<float>(ctx, inverse);
+int lgf_slab_fft_forward(lgf_slab *ctx, void *d_send) {
+    if (!ctx || !d_send) return sfail(ctx, LGF_EINVAL, "lgf_slab_fft_forward: null argument");
+    return ctx->prec == LGF_FP64 ? slab_fft_forward<double>(ctx, d_send) : slab_fft_forward<float>(ctx, d_send);
 }
 
-int lgf_slab_transpose(lgf_slab *ctx, int stage, void *d_buf) {
-    if (!ctx || !d_buf || stage < 0 || stage > 3) return sfail(ctx, LGF_EINVAL, "lgf_slab_transpose: bad argument");
-    return ctx->prec == LGF_FP64 ? slab_transpose<double>(ctx, stage, d_buf) : slab_transpose<float>(ctx, stage, d_buf);
+int lgf_slab_fft_t(lgf_slab *ctx, const void *d_recv, void *d_send) {
+    if (!ctx || !d_recv || !d_send || d_recv == d_send) return sfail(ctx, LGF_EINVAL, "lgf_slab_fft_t: bad argument");
+    return ctx->prec == LGF_FP64 ? slab_fft_t<double>(ctx, d_recv, d_send) : slab_fft_t<float>(ctx, d_recv, d_send);
 }
 
-int lgf_slab_fft_t(lgf_slab *ctx) {
-    if (!ctx) return LGF_EINVAL;
-    return ctx->prec == LGF_FP64 ? slab_fft_t<double>(ctx) : slab_fft_t<float>(ctx);
+int lgf_slab_fft_inverse(lgf_slab *ctx, const void *d_recv) {
+    if (!ctx || !d_recv) return sfail(ctx, LGF_EINVAL, "lgf_slab_fft_inverse: null argument");
+    return ctx->prec == LGF_FP64 ? slab_fft_inverse<double>(ctx, d_recv, false, 0.0) : slab_fft_inverse<float>(ctx, d_recv, false, 0.0);
+}
+
+int lgf_slab_fft_inverse_g(lgf_slab *ctx, const void *d_recv, double alpha) {
+    if (!ctx || !d_recv) return sfail(ctx, LGF_EINVAL, "lgf_slab_fft_inverse_g: null argument");
+    return ctx->prec == LGF_FP64 ? slab_fft_inverse<double>(ctx, d_recv, true, alpha) : slab_fft_inverse<float>(ctx, d_recv, true, alpha);
 }
 
 int lgf_slab_gbuild(lgf_slab *ctx, double alpha) {

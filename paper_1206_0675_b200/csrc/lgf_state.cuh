@@ -72,6 +72,8 @@ cudaError_t launch_fft_reg(int which, const Geom &g, C<R> *W, const R *twiddle_t
 // two-threads-per-line register sweeps (lgf_fft_reg2.cu)
 bool fft_reg2_supported(const Geom &g);
 bool fft_reg2_gout(const Geom &g, int prec);
+bool fft_reg2_xy_supported(const Geom &g);      // the (x, y) sweeps alone, any (Lz, Lt): the slabs of lgf_slab.cu
+bool fft_reg2_xy_gout(const Geom &g, int prec);
 template <class R>
 cudaError_t launch_fft_reg2(int which, const Geom &g, C<R> *W, const R *p2tab, R scale, const DevState *st,
                             cudaStream_t stream, C<R> *G, R half_alpha);

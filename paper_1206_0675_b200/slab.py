@@ -170,25 +170,25 @@ class SlabFixer:
         self._hist.append(self._sums[0].clone())
         self._measured = True
 
-    def _step_accelerate(self) -> None:
-        """a2-a4: w = F^-1[(p2max / p2) F Delta] / V with the t lines gathered by two all-to-alls."""
+    def _fft_to_second_exchange(self) -> None:
         for c, s in zip(self.ranks, self._a_send):
-            c.fft_local(False)
-            c.transpose(0, s)
+            c.fft_forward(s)
         self.ex.all_to_all(self._a_send, self._a_recv)
         for c, s, r in zip(self.ranks, self._a_send, self._a_recv):
-            c.transpose(1, r)
-            c.fft_t()
-            c.transpose(2, s)
+            c.fft_t(r, s)
         self.ex.all_to_all(self._a_send, self._a_recv)
-        for c, r in zip(self.ranks, self._a_recv):
-            c.transpose(3, r)
-            c.fft_local(True)
 
-    def _step_update(self, alpha: float) -> None:
+    def _step_accelerate(self) -> None:
+        """a2-a4: w = F^-1[(p2max / p2) F Delta] / V with the t lines gathered by two all-to-alls; w into the work field."""
+        self._fft_to_second_exchange()
+        for c, r in zip(self.ranks, self._a_recv):
+            c.fft_inverse(r)
+
+    def _step_update(self, alpha: float, g_ready: bool = False) -> None:
         """a5 + a6 (+ halo of g)."""
         for c, s in zip(self.ranks, self._g_send):
-            c.gbuild(alpha)
+            if not g_ready:
+                c.gbuild(alpha)
             c.halo_pack(B.LGF_HALO_G, s)
         self.ex.shift(self._g_send, self._g_recv, -1)
         for c, r in zip(self.ranks, self._g_recv):
@@ -196,6 +196,13 @@ class SlabFixer:
             c.update()
         self._measured = False
         self.updates += 1
+
+    def _step_iteration(self, alpha: float) -> None:
+        """a2-a6 with the g-build at the end of the last FFT sweep (what iterate / fix run)."""
+        self._fft_to_second_exchange()
+        for c, r in zip(self.ranks, self._a_recv):
+            c.fft_inverse_g(r, alpha)
+        self._step_update(alpha, g_ready=True)
 
     def _bytes_per_iteration(self) -> int:
         n, es = self.ex.world, self._a_send[0].element_size()
@@ -222,8 +229,7 @@ class SlabFixer:
         for _ in range(int(n)):
             if not self._measured:
                 self._step_delta()
-            self._step_accelerate()
-            self._step_update(alpha)
+            self._step_iteration(alpha)
         if not self._measured:
             self._step_delta()
         self.exchanged_bytes = self._bytes_per_iteration() * int(n)
@@ -239,8 +245,7 @@ class SlabFixer:
                 raise B.LgfError(B.LGF_ENAN, "theta became NaN")
             if theta < tol or it >= max_iter:
                 return it
-            self._step_accelerate()
-            self._step_update(alpha)
+            self._step_iteration(alpha)
             it += 1
 
     def history(self):

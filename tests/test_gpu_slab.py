@@ -44,7 +44,8 @@ def gathered(slabs):
 
 # (dims, world): T = Lt / world from the whole lattice down to ONE slice per rank; Zl = Lz / world down to 1
 CASES = [((8, 8, 8, 8), 1), ((8, 8, 8, 8), 2), ((8, 8, 8, 8), 4), ((8, 8, 8, 8), 8), ((12, 6, 16, 4), 2),
-         ((12, 6, 16, 4), 4), ((16, 16, 12, 6), 3), ((16, 16, 12, 6), 6), ((3, 24, 2, 48), 2)]
+         ((12, 6, 16, 4), 4), ((16, 16, 12, 6), 3), ((16, 16, 12, 6), 6), ((3, 24, 2, 48), 2), ((32, 32, 8, 4), 4),
+         ((64, 64, 4, 2), 2)]
 
 
 @pytest.mark.parametrize("dims,world", CASES)

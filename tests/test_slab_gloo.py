@@ -1,6 +1,6 @@
 """The exchanges of the sharded path (paper_1206_0675_b200/slab.py) on the CPU:
 world_size 2 and 3 over gloo against the in-process LocalExchange, and the all-to-all against the buffer layout
-include/lgf.h documents for lgf_slab_transpose ([q][c][tl][zl][y][x], chunk q <-> rank q), modelled here as
+include/lgf.h documents for lgf_slab_fft_forward / _t / _inverse ([q][c][tl][zl][y][x], chunk q <-> rank q), modelled here as
 plain numpy index shuffles -- data movement only, none of the method's arithmetic.  The kernels that fill and
 read those buffers are checked on the GPU (tests/test_gpu_slab.py, with LocalExchange); this file checks that
 the torch.distributed plumbing delivers the same chunks to the same places."""
