@@ -416,6 +416,77 @@ def run_thermal(args):
     return 0
 
 
+def run_shard(args):
+    """--shard K: ONE configuration sharded over ranks (t-slabs, paper_1206_0675_b200/slab.py).
+    Under torchrun (WORLD_SIZE = N > 1) the ranks are the processes and the exchanges go over NCCL: strong scaling,
+    value = iterations/s of the one configuration, max-over-ranks device time.  In a single process K ranks are
+    emulated one after the other on the one GPU (exchanges = device copies): the time is then the SUM of the K
+    ranks' kernel times plus the copies -- a per-rank cost figure, NOT a scaling measurement; the NVLink time is a
+    model from the bytes each rank sends (stated as such).  Prints one JSON line of its own; not the contract line."""
+    import torch
+
+    from paper_1206_0675_b200 import binding, inputs, slab
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: liblgf has no CPU path")
+    torch.cuda.set_device(local)
+    binding.load()
+    dist = None
+    if world > 1:
+        import torch.distributed as dist  # noqa: PLC0415
+
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        ex, nranks, mode = slab.DistExchange(dist), world, "nccl"
+    else:
+        ex, nranks, mode = slab.LocalExchange(args.shard), args.shard, "emulated on one GPU, ranks in turn"
+    cfg = inputs.CONFIGS[args.workload]
+    dims = cfg["dims"]
+    V = int(np.prod(dims))
+    prec = PREC[args.precision]
+    if cfg["kind"] == "hot":
+        U0 = inputs.hot_config_torch(dims, cfg["seed"], device="cuda")
+    else:
+        U0 = torch.from_numpy(inputs.make_config(args.workload)).cuda()
+    U0 = torch.view_as_real(U0.to(torch.complex128 if prec == 8 else torch.complex64)).contiguous()
+    fx = slab.SlabFixer(dims, prec, args.storage, ex)
+    fx.set_links_global(U0)
+    del U0
+    fx.iterate(ALPHA, args.warmup)
+    n0 = fx.launch_count()
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record()
+    fx.iterate(ALPHA, args.steps)
+    b.record()
+    torch.cuda.synchronize()
+    ms = ensemble.max_over_ranks(dist, a.elapsed_time(b), torch.device("cuda", local)) / args.steps
+    F, theta = fx.measure()
+    sent = fx.exchanged_bytes / args.steps
+    if rank == 0:
+        line = {"metric": METRIC, "value": 1e3 / ms, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+                "ms_per_step": ms, "higher_is_better": True, "scaling": "strong" if world > 1 else "none (emulation)",
+                "dtype": "f64" if prec == 8 else "f32", "data": "synthetic",
+                "config": {"workload": workload_name(args.workload, dims), "precision": args.precision,
+                           "link_storage": args.storage, "alpha": ALPHA, "sites": V,
+                           "parallelism": "one configuration in %d t-slabs (%s)" % (nranks, mode)},
+                "slab": {"ranks": nranks, "sites_per_rank": V // nranks, "sent_bytes_per_rank_per_iteration": sent,
+                         "ms_per_rank_kernels_and_copies": ms / (nranks if world == 1 else 1),
+                         "launches_per_iteration": (fx.launch_count() - n0) / args.steps,
+                         "nvlink_model_ms": sent / 900e9 * 1e3,
+                         "nvlink_model": "sent bytes / 900 GB/s per direction per GPU (B200 NVLink 5); not measured"},
+                "state_after_timing": {"F": F, "theta": theta}}
+        print(json.dumps(line), flush=True)
+    fx.destroy()
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
 def workload_name(key, dims):
     from paper_1206_0675_b200 import inputs
 
@@ -449,6 +520,9 @@ def main():
     ap.add_argument("--reunit-every", type=int, default=0)
     ap.add_argument("--alpha", type=float, default=ALPHA, help="step size of the --thermal fix (the paper uses 0.08)")
     ap.add_argument("--thermal-max-iter", type=int, default=200000)
+    ap.add_argument("--shard", type=int, default=0, metavar="K",
+                    help="ONE configuration sharded over t-slabs: K emulated ranks in a single process; under torchrun the "
+                         "ranks are the processes (any K > 0)")
     ap.add_argument("--mixed", action="store_true", help="--thermal (fp64 only): also time fp32 iterations + fp64 polish")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)
@@ -459,6 +533,8 @@ def main():
         return run_reference(args)
     if args.thermal is not None:
         return run_thermal(args)
+    if args.shard > 0:
+        return run_shard(args)
 
     import torch
 

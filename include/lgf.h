@@ -233,14 +233,18 @@ const char *lgf_version(void);
  *   halo_pack(LINKS) -> [send to r+1, receive from r-1] -> halo_unpack(LINKS) -> delta(sums) -> [all-reduce sums:
  *   F = sums[0] / (12 V), theta = sums[1] / (3 V), V the GLOBAL volume (eqs. 3, 6)] -> fft_forward(send) ->
  *   [all-to-all] -> fft_t(recv, send) -> [all-to-all] -> fft_inverse_g(recv, alpha) -> halo_pack(G) ->
- *   [send to r-1, receive from r+1] -> halo_unpack(G) -> update.
+ *   [send to r-1, receive from r+1] -> halo_unpack(G) -> update,
+ * or, with the fused form of the last step (what paper_1206_0675_b200/slab.py iterates with): one such round of
+ * halo(LINKS) + delta at the start, then per iteration fft_forward .. fft_inverse_g -> halo_pack(G), halo_pack(G_UP)
+ * -> [exchange both ways] -> halo_unpack(G), halo_unpack(G_UP) -> sweep(sums) -> [all-reduce sums].
  * With nranks = 1 the "exchanges" are copies of a rank's send buffer into its own receive buffer (periodic wrap).
  * The result equals the one-GPU path's up to the rounding order of the F / theta sums and of the FFT passes.
  * Same precision / storage / error conventions as above; messages from lgf_slab_last_error.  All calls are
  * asynchronous on the context's stream (default: stream 0). */
 typedef struct lgf_slab lgf_slab; /* opaque */
 enum { LGF_HALO_LINKS = 0, /* U_t on one 3-D slice: 18 or 12 reals per site (the context's link storage)       */
-       LGF_HALO_G = 1      /* rows 0, 1 of g(x) on one 3-D slice: 12 reals per site                             */ };
+       LGF_HALO_G = 1,     /* rows 0, 1 of g(x) on one 3-D slice: 12 reals per site                             */
+       LGF_HALO_G_UP = 2   /* the same, travelling the other way (fused sweep)                                  */ };
 
 int lgf_slab_create(const int dims[4] /* GLOBAL extents */, int precision, int link_storage, int rank, int nranks,
                     lgf_slab **out);
@@ -277,6 +281,15 @@ int lgf_slab_fft_inverse_g(lgf_slab *ctx, const void *d_recv, double alpha);
 int lgf_slab_gbuild(lgf_slab *ctx, double alpha);
 /* a6: U_mu(x) <- g(x) U_mu(x) g(x + mu)^dag on the slab, in place */
 int lgf_slab_update(lgf_slab *ctx);
+/* a6 + a1 fused (the iteration loop's form): the new links go to the context's second link buffer, and Delta, F
+ * and theta of the NEW configuration (Alg. 1 line 17) come out of the same pass -- work field and d_sums as for
+ * lgf_slab_delta.  Needs g of BOTH neighbouring slices: halo_pack(LGF_HALO_G) -> rank r-1 (as before) and
+ * halo_pack(LGF_HALO_G_UP) = g of the slab's LAST slice -> rank r+1, each followed by halo_unpack with the same id
+ * on the receiver; and the U_t halo of the current configuration, which must have been exchanged once
+ * (halo_pack / halo_unpack(LGF_HALO_LINKS), e.g. by the first lgf_slab_delta round) after set_links or after an
+ * lgf_slab_update -- LGF_ESTATE otherwise.  The sweep itself keeps that halo current from then on, so an iteration
+ * of sweeps exchanges 24 reals per boundary site instead of 12 + 18 (or 12 + 12). */
+int lgf_slab_sweep(lgf_slab *ctx, double *d_sums);
 /* the slab's work field as full 3 x 3 matrices, 18 reals per local site (as lgf_get_field) */
 int lgf_slab_get_field(lgf_slab *ctx, void *d_field);
 long long lgf_slab_launch_count(const lgf_slab *ctx);

@@ -80,11 +80,12 @@ SIGNATURES = {
     "lgf_slab_fft_inverse_g": (_i, [_vp, _vp, _d]),
     "lgf_slab_gbuild": (_i, [_vp, _d]),
     "lgf_slab_update": (_i, [_vp]),
+    "lgf_slab_sweep": (_i, [_vp, _vp]),
     "lgf_slab_get_field": (_i, [_vp, _vp]),
     "lgf_slab_launch_count": (_ll, [_vp]),
     "lgf_slab_last_error": (ctypes.c_char_p, [_vp]),
 }
-LGF_HALO_LINKS, LGF_HALO_G = 0, 1
+LGF_HALO_LINKS, LGF_HALO_G, LGF_HALO_G_UP = 0, 1, 2
 
 
 class LgfError(RuntimeError):
@@ -384,6 +385,9 @@ class SlabContext:
 
     def update(self):
         self._ck(load().lgf_slab_update(self._h))
+
+    def sweep(self, sums):
+        self._ck(load().lgf_slab_sweep(self._h, _dev_ptr(sums, LGF_FP64, 2)))
 
     def get_field(self, out):
         self._ck(load().lgf_slab_get_field(self._h, _dev_ptr(out, self.precision, self.V * 18)))

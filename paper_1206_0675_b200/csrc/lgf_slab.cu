@@ -13,9 +13,9 @@
 //   F, theta: per-rank sums, all-reduced by the caller (two doubles).
 // This file holds the kernels and the per-rank context; the exchanges themselves are the caller's (NCCL through
 // torch.distributed, paper_1206_0675_b200/slab.py): every entry point here is local to one rank and works on
-// buffers the caller hands in, so no kernel ever waits on another rank.  The links are updated in place (a link
-// transform reads no other link); Delta is recomputed by a pass of its own (the fused sweep of lgf_links.cu needs
-// g(x - mu) as well, i.e. a second g halo: left for later).
+// buffers the caller hands in, so no kernel ever waits on another rank.  Two forms of a6: k_slab_update transforms
+// the links in place (a link transform reads no other link) and leaves a1 to a pass of its own; k_slab_sweep is the
+// fused a6 + a1 pass of the iteration loop (second g halo instead of the U_t halo, two link buffers).
 // Part of liblgf (CUDA path).  Shares nothing with oracle/.
 #include <new>
 #include <string>
@@ -102,6 +102,73 @@ __global__ void __launch_bounds__(SLAB_THREADS) k_slab_update(C<R> *__restrict__
         mat_mul<NR>(gx, u, t);
         mat_mul_dag<NR>(t, gn, p);
         store_link<R, NR>(links, g.V, mu, s, p);                    // with 12-real storage row 2 is rebuilt on load (eq. 8)
+    }
+}
+
+// a6 + a1 fused on a slab (the slab form of k_sweep, lgf_links.cu): every site writes its own new links
+// U'_mu(x) = g(x) U_mu(x) g(x + mu)^dag into the OTHER link buffer and recomputes the new links of its backward
+// neighbours, U'_mu(x - mu) = g(x - mu) U_mu(x - mu) g(x)^dag, for Delta, F, theta of the new configuration
+// (Alg. 1 lines 14, 17) -- the links are read once and written once per iteration, and no separate Delta pass runs.
+// Across the slab boundary it needs g of the slice above (ghi) and of the slice below (glo), and the OLD U_t of the
+// slice below (uhalo); the first local slice also stores the new U_t(x - t) back into uhalo, which thereby stays
+// the neighbour's current U_t without ever being exchanged again.
+constexpr int SLAB_SWEEP_THREADS = 128;
+template <class R, int NR>
+__global__ void __launch_bounds__(SLAB_SWEEP_THREADS, 3)
+    k_slab_sweep(const C<R> *__restrict__ src, C<R> *__restrict__ dst, const C<R> *__restrict__ G,
+                 const C<R> *__restrict__ ghi, const C<R> *__restrict__ glo, C<R> *__restrict__ uhalo,
+                 C<R> *__restrict__ W, Geom g, double *__restrict__ partial) {
+    __shared__ double scratch[SLAB_SWEEP_THREADS / 32][2];
+    const long long s = (long long)blockIdx.x * SLAB_SWEEP_THREADS + threadIdx.x;
+    double f = 0.0, t = 0.0;
+    if (s < g.V) {
+        int c[4];
+        site_coords(g, s, c);
+        const long long S3 = g.S[3];
+        C<R> gx[9];
+        slab_load_g(G, g.V, s, gx);
+        Herm<R> d = herm_zero<R>();
+        R retr = 0;
+#pragma unroll
+        for (int mu = 0; mu < 4; mu++) {
+            {   // the site's own new link
+                C<R> u[9], gn[9], tmp[9], p[9];
+                load_link<R, NR>(src, g.V, mu, s, u);
+                if (mu == 3 && c[3] == g.L[3] - 1) slab_load_g(ghi, S3, s - S3 * (long long)(g.L[3] - 1), gn);
+                else slab_load_g(G, g.V, site_fwd(g, s, c, mu), gn);
+                mat_mul<NR>(gx, u, tmp);
+                mat_mul_dag<NR>(tmp, gn, p);
+                if constexpr (NR == 2) reconstruct_row2(p);        // as whoever loads the stored link will see it (eq. 8)
+                store_link<R, NR>(dst, g.V, mu, s, p);
+                retr += p[0].x + p[4].x + p[8].x;                   // eq. 3 on the new link
+                herm_sub(d, algebra_part(p));                       // - A'_mu(x)
+            }
+            {   // + A'_mu(x - mu): the backward neighbour's new link recomputed
+                C<R> u[9], gb[9], tmp[9], p[9];
+                const bool below = (mu == 3 && c[3] == 0);          // the neighbour is on the rank below
+                if (below) {
+                    load_link<R, NR>(uhalo, S3, 0, s, u);           // s < S3: the (x, y, z) index
+                    slab_load_g(glo, S3, s, gb);
+                } else {
+                    const long long sb = site_bwd(g, s, c, mu);
+                    load_link<R, NR>(src, g.V, mu, sb, u);
+                    slab_load_g(G, g.V, sb, gb);
+                }
+                mat_mul<NR>(gb, u, tmp);
+                mat_mul_dag<NR>(tmp, gx, p);
+                if constexpr (NR == 2) reconstruct_row2(p);
+                if (below) store_link<R, NR>(uhalo, S3, 0, s, p);   // keep the halo copy of U_t current
+                herm_add(d, algebra_part(p));                       // eq. 5
+            }
+        }
+        store_herm(W, g.V, s, d);
+        f = (double)retr;
+        t = (double)herm_norm2(d);                                  // eq. 6
+    }
+    block_sum2(f, t, scratch);
+    if (threadIdx.x == 0) {
+        partial[2 * blockIdx.x] = f;
+        partial[2 * blockIdx.x + 1] = t;
     }
 }
 
@@ -203,11 +270,15 @@ struct lgf_slab {
     Geom gl{};                   // the slab: (Lx, Ly, Lz, T)
     long long Vglobal = 0;
     cudaStream_t stream = nullptr;
-    void *links = nullptr;       // C<R>[4][3 nr][Vl]
+    void *lbuf[2] = {nullptr, nullptr};   // C<R>[4][3 nr][Vl] each: the fused sweep reads one and writes the other
+    int cur = 0;                 // which one holds the current configuration (`links` below points at it)
+    void *links = nullptr;
     void *uhalo = nullptr;       // C<R>[3 nr][S3]   U_t of the slice below the slab
     void *W = nullptr;           // C<R>[4][Vl]      packed Delta / w, t-slab order
     void *G = nullptr;           // C<R>[6][Vl]
     void *ghalo = nullptr;       // C<R>[6][S3]      g of the slice above the slab
+    void *glo = nullptr;         // C<R>[6][S3]      g of the slice below the slab (fused sweep only)
+    bool uhalo_valid = false;    // uhalo holds U_t of the slice below for the CURRENT configuration
     double *partial = nullptr;
     int nb = 0;
     DevState *st = nullptr;      // all zero: the kernels shared with the one-GPU path look at st->done
@@ -391,6 +462,28 @@ static int slab_update(lgf_slab *ctx) {
     return LGF_OK;
 }
 
+template <class R>
+static int slab_sweep(lgf_slab *ctx, double *d_sums) {
+    const int nb = (int)((ctx->gl.V + SLAB_SWEEP_THREADS - 1) / SLAB_SWEEP_THREADS);      // <= 2 * ctx->nb: partial is sized for it
+    const C<R> *src = (const C<R> *)ctx->lbuf[ctx->cur];
+    C<R> *dst = (C<R> *)ctx->lbuf[1 - ctx->cur];
+    if (ctx->nr == 3)
+        k_slab_sweep<R, 3><<<nb, SLAB_SWEEP_THREADS, 0, ctx->stream>>>(src, dst, (const C<R> *)ctx->G, (const C<R> *)ctx->ghalo,
+                                                                       (const C<R> *)ctx->glo, (C<R> *)ctx->uhalo, (C<R> *)ctx->W,
+                                                                       ctx->gl, ctx->partial);
+    else
+        k_slab_sweep<R, 2><<<nb, SLAB_SWEEP_THREADS, 0, ctx->stream>>>(src, dst, (const C<R> *)ctx->G, (const C<R> *)ctx->ghalo,
+                                                                       (const C<R> *)ctx->glo, (C<R> *)ctx->uhalo, (C<R> *)ctx->W,
+                                                                       ctx->gl, ctx->partial);
+    SCK(cudaGetLastError());
+    k_slab_sum2<<<1, SLAB_THREADS, 0, ctx->stream>>>(ctx->partial, nb, d_sums);
+    SCK(cudaGetLastError());
+    ctx->cur = 1 - ctx->cur;
+    ctx->links = ctx->lbuf[ctx->cur];
+    ctx->launches += 2;
+    return LGF_OK;
+}
+
 extern "C" {
 
 const char *lgf_slab_last_error(const lgf_slab *ctx) { return ctx ? ctx->err.c_str() : g_slab_err.c_str(); }
@@ -398,7 +491,7 @@ const char *lgf_slab_last_error(const lgf_slab *ctx) { return ctx ? ctx->err.c_s
 int lgf_slab_destroy(lgf_slab *ctx) {
     if (!ctx) return LGF_EINVAL;
     cudaStreamSynchronize(ctx->stream);
-    void *bufs[] = {ctx->links, ctx->uhalo, ctx->W, ctx->G, ctx->ghalo, ctx->partial, ctx->st, ctx->p2tab,
+    void *bufs[] = {ctx->lbuf[0], ctx->lbuf[1], ctx->uhalo, ctx->W, ctx->G, ctx->ghalo, ctx->glo, ctx->partial, ctx->st, ctx->p2tab,
                     ctx->twiddle[0], ctx->twiddle[1], ctx->twiddle[2], ctx->twiddle[3]};
     for (void *b : bufs) cudaFree(b);
     cudaGetLastError();
@@ -456,12 +549,15 @@ int lgf_slab_create(const int dims[4], int precision, int link_storage, int rank
         if (ee != cudaSuccess) rc = sfail(ctx, ee == cudaErrorMemoryAllocation ? LGF_ENOMEM : LGF_ECUDA,
                                           std::string("cudaMalloc: ") + cudaGetErrorString(ee));
     };
-    alloc(&ctx->links, V * 4 * 3 * ctx->nr * cb);
+    alloc(&ctx->lbuf[0], V * 4 * 3 * ctx->nr * cb);
+    alloc(&ctx->lbuf[1], V * 4 * 3 * ctx->nr * cb);
+    ctx->links = ctx->lbuf[0];
     alloc(&ctx->uhalo, S3 * 3 * ctx->nr * cb);
     alloc(&ctx->W, V * 4 * cb);
     alloc(&ctx->G, V * 6 * cb);
     alloc(&ctx->ghalo, S3 * 6 * cb);
-    alloc((void **)&ctx->partial, sizeof(double) * 2 * ctx->nb);
+    alloc(&ctx->glo, S3 * 6 * cb);
+    alloc((void **)&ctx->partial, sizeof(double) * 2 * (2 * ctx->nb + 1));
     alloc((void **)&ctx->st, sizeof(DevState));
     if (rc == LGF_OK) {
         cudaError_t ee = cudaMemset(ctx->st, 0, sizeof(DevState));
@@ -489,6 +585,9 @@ int lgf_slab_set_stream(lgf_slab *ctx, void *cuda_stream) {
 
 int lgf_slab_set_links(lgf_slab *ctx, const void *d_links) {
     if (!ctx || !d_links) return sfail(ctx, LGF_EINVAL, "lgf_slab_set_links: null argument");
+    ctx->cur = 0;
+    ctx->links = ctx->lbuf[0];
+    ctx->uhalo_valid = false;
     if (ctx->prec == LGF_FP64) SCK(launch_convert_in<double>(ctx->nr, (const double *)d_links, (C<double> *)ctx->links, ctx->gl, ctx->stream));
     else SCK(launch_convert_in<float>(ctx->nr, (const float *)d_links, (C<float> *)ctx->links, ctx->gl, ctx->stream));
     ctx->launches++;
@@ -511,7 +610,7 @@ int lgf_slab_get_links(lgf_slab *ctx, void *d_links) {
 }
 
 long long lgf_slab_halo_elems(const lgf_slab *ctx, int which) {
-    if (!ctx || (which != LGF_HALO_LINKS && which != LGF_HALO_G)) return LGF_EINVAL;
+    if (!ctx || (which != LGF_HALO_LINKS && which != LGF_HALO_G && which != LGF_HALO_G_UP)) return LGF_EINVAL;
     return (long long)ctx->gl.S[3] * (which == LGF_HALO_LINKS ? 3 * ctx->nr : 6) * 2;
 }
 
@@ -524,6 +623,9 @@ int lgf_slab_halo_pack(lgf_slab *ctx, int which, void *d_send) {
         SCK(cudaMemcpy2DAsync(d_send, S3 * cb, src, V * cb, S3 * cb, 3 * ctx->nr, cudaMemcpyDeviceToDevice, ctx->stream));
     } else if (which == LGF_HALO_G) {       // g of the FIRST local slice, for the rank below
         SCK(cudaMemcpy2DAsync(d_send, S3 * cb, ctx->G, V * cb, S3 * cb, 6, cudaMemcpyDeviceToDevice, ctx->stream));
+    } else if (which == LGF_HALO_G_UP) {    // g of the LAST local slice, for the rank above (fused sweep)
+        const char *src = (const char *)ctx->G + S3 * (ctx->T - 1) * cb;
+        SCK(cudaMemcpy2DAsync(d_send, S3 * cb, src, V * cb, S3 * cb, 6, cudaMemcpyDeviceToDevice, ctx->stream));
     } else return sfail(ctx, LGF_EINVAL, "lgf_slab_halo_pack: bad halo id");
     return LGF_OK;
 }
@@ -531,7 +633,10 @@ int lgf_slab_halo_pack(lgf_slab *ctx, int which, void *d_send) {
 int lgf_slab_halo_unpack(lgf_slab *ctx, int which, const void *d_recv) {
     if (!ctx || !d_recv) return sfail(ctx, LGF_EINVAL, "lgf_slab_halo_unpack: null argument");
     const size_t cb = 2 * (size_t)ctx->prec, S3 = (size_t)ctx->gl.S[3];
-    if (which == LGF_HALO_LINKS) SCK(cudaMemcpyAsync(ctx->uhalo, d_recv, S3 * 3 * ctx->nr * cb, cudaMemcpyDeviceToDevice, ctx->stream));
+    if (which == LGF_HALO_LINKS) {
+        SCK(cudaMemcpyAsync(ctx->uhalo, d_recv, S3 * 3 * ctx->nr * cb, cudaMemcpyDeviceToDevice, ctx->stream));
+        ctx->uhalo_valid = true;
+    } else if (which == LGF_HALO_G_UP) SCK(cudaMemcpyAsync(ctx->glo, d_recv, S3 * 6 * cb, cudaMemcpyDeviceToDevice, ctx->stream));
     else if (which == LGF_HALO_G) SCK(cudaMemcpyAsync(ctx->ghalo, d_recv, S3 * 6 * cb, cudaMemcpyDeviceToDevice, ctx->stream));
     else return sfail(ctx, LGF_EINVAL, "lgf_slab_halo_unpack: bad halo id");
     return LGF_OK;
@@ -576,7 +681,16 @@ int lgf_slab_gbuild(lgf_slab *ctx, double alpha) {
 int lgf_slab_update(lgf_slab *ctx) {
     if (!ctx) return LGF_EINVAL;
     if (!ctx->have_links) return sfail(ctx, LGF_ESTATE, "lgf_slab_update: no configuration loaded");
+    ctx->uhalo_valid = false;                // the neighbour's U_t changed too: exchange it again before the next delta
     return ctx->prec == LGF_FP64 ? slab_update<double>(ctx) : slab_update<float>(ctx);
+}
+
+int lgf_slab_sweep(lgf_slab *ctx, double *d_sums) {
+    if (!ctx || !d_sums) return sfail(ctx, LGF_EINVAL, "lgf_slab_sweep: null argument");
+    if (!ctx->have_links) return sfail(ctx, LGF_ESTATE, "lgf_slab_sweep: no configuration loaded");
+    if (!ctx->uhalo_valid)
+        return sfail(ctx, LGF_ESTATE, "lgf_slab_sweep: the U_t halo is not current (halo_unpack(LGF_HALO_LINKS) after set_links / update)");
+    return ctx->prec == LGF_FP64 ? slab_sweep<double>(ctx, d_sums) : slab_sweep<float>(ctx, d_sums);
 }
 
 int lgf_slab_get_field(lgf_slab *ctx, void *d_field) {

@@ -3,13 +3,14 @@
 SURVEY.md section 8(e) / 8(f) NEXT-3; the paper's stated future work (its CPU code does the same
 decomposition with PFFT over MPI, :124).  Rank r of N owns the slices t = r T .. (r+1) T - 1 of the lattice.
 Every arithmetic step runs in liblgf's kernels through the per-rank entry points ``lgf_slab_*`` (include/lgf.h);
-this module only sequences them and moves the buffers between ranks.  Per iteration there are exactly four
-exchanges plus one two-double all-reduce:
+this module only sequences them and moves the buffers between ranks.  The exchanges (the U_t halo only once per
+loaded configuration -- the fused sweep keeps it current -- the others once per iteration):
 
   halo LINKS  U_t of a rank's last slice     -> rank r+1   (a1: A_t(x - t), eq. 5)          S3 * n_l reals
   all-to-all  t-slabs -> z-slabs of F_xyz[Delta]            (a2: the t lines of the 4-D FFT)  8 * V/N * (N-1)/N
   all-to-all  z-slabs -> t-slabs                            (a4)                              the same
   halo G      g of a rank's first slice      -> rank r-1   (a6: g(x + t), eq. 2)            S3 * 12 reals
+  halo G_UP   g of a rank's last slice       -> rank r+1   (fused a6 + a1: g(x - t))        S3 * 12 reals
   all-reduce  (sum Re tr U, sum tr Delta Delta^dag)         (F, theta, eqs. 3, 6)             2 doubles
 
 Two exchange objects implement them:
@@ -130,6 +131,7 @@ class SlabFixer:
         c0 = self.ranks[0]
         self._u_send, self._u_recv = mk(c0.halo_elems(B.LGF_HALO_LINKS)), mk(c0.halo_elems(B.LGF_HALO_LINKS))
         self._g_send, self._g_recv = mk(c0.halo_elems(B.LGF_HALO_G)), mk(c0.halo_elems(B.LGF_HALO_G))
+        self._g2_send, self._g2_recv = mk(c0.halo_elems(B.LGF_HALO_G_UP)), mk(c0.halo_elems(B.LGF_HALO_G_UP))
         self._a_send, self._a_recv = mk(c0.V * 8), mk(c0.V * 8)
         self._sums = mk(2, torch.float64)
         self._hist = []                 # device tensors [2]: (sum Re tr U, sum tr Delta Delta^dag), all-reduced
@@ -198,18 +200,31 @@ class SlabFixer:
         self.updates += 1
 
     def _step_iteration(self, alpha: float) -> None:
-        """a2-a6 with the g-build at the end of the last FFT sweep (what iterate / fix run)."""
+        """a2-a6 + a1 of the new links, as iterate / fix run them: the g-build at the end of the last FFT sweep, g halos
+        both ways, the fused sweep (new links, their Delta and sums in one pass), all-reduce.  Wants the work fields
+        to hold Delta of the current links (``_measured``), which also means the U_t halos are current."""
         self._fft_to_second_exchange()
-        for c, r in zip(self.ranks, self._a_recv):
+        for c, r, dn, up in zip(self.ranks, self._a_recv, self._g_send, self._g2_send):
             c.fft_inverse_g(r, alpha)
-        self._step_update(alpha, g_ready=True)
+            c.halo_pack(B.LGF_HALO_G, dn)
+            c.halo_pack(B.LGF_HALO_G_UP, up)
+        self.ex.shift(self._g_send, self._g_recv, -1)
+        self.ex.shift(self._g2_send, self._g2_recv, +1)
+        for c, dn, up, sm in zip(self.ranks, self._g_recv, self._g2_recv, self._sums):
+            c.halo_unpack(B.LGF_HALO_G, dn)
+            c.halo_unpack(B.LGF_HALO_G_UP, up)
+            c.sweep(sm)
+        self.ex.all_reduce_sum(self._sums)
+        self._hist.append(self._sums[0].clone())
+        self._measured = True
+        self.updates += 1
 
     def _bytes_per_iteration(self) -> int:
         n, es = self.ex.world, self._a_send[0].element_size()
         if n == 1:
             return 0
         a2a = 2 * self._a_send[0].numel() * es * (n - 1) // n
-        return a2a + (self._u_send[0].numel() + self._g_send[0].numel()) * es + 16
+        return a2a + (self._g_send[0].numel() + self._g2_send[0].numel()) * es + 16
 
     # -- public: same meaning as lgf_measure / lgf_iterate / lgf_fix ---------------------------------
     def measure(self):

@@ -92,6 +92,51 @@ def test_slab_trajectory(slab, dims, world, prec, storage):
     fx.destroy()
 
 
+@pytest.mark.parametrize("dims,world", [((8, 8, 8, 8), 2), ((16, 16, 12, 6), 6), ((12, 6, 16, 4), 4)])
+@pytest.mark.parametrize("prec,storage", [(8, 18), (4, 12)])
+def test_slab_single_steps_make_the_same_trajectory(slab, dims, world, prec, storage):
+    """The single-step entry points (delta / fft_inverse + gbuild / in-place update with the U_t halo re-exchanged
+    every iteration) against the oracle, and a mix of both forms of a6 in one run."""
+    n = 6
+    U = inputs.smooth_config(dims, 0.25, 515 + world, haar=True)
+    U_o, F_o, T_o = oracle.iterate(dims, U, ALPHA, n)
+    fx = slab.SlabFixer(dims, prec, storage, slab.LocalExchange(world))
+    fx.set_links_global(to_dev(U, prec))
+    for k in range(n):
+        fx._step_delta()
+        if k % 3 == 2:
+            fx._step_iteration(ALPHA)          # fused sweep in between: records the next entry itself
+            fx._hist.pop()
+            fx._measured = False
+        else:
+            fx._step_accelerate()
+            fx._step_update(ALPHA)
+    fx._step_delta()
+    Fh, Th = fx.history()
+    tol = TOL[prec]
+    assert len(Th) == n + 1
+    assert np.max(np.abs(Fh - F_o) / np.abs(F_o)) < tol["scalar"]
+    assert np.max(np.abs(Th - T_o) / np.abs(T_o)) < tol["scalar"]
+    assert np.max(np.abs(gathered(fx.get_links()) - U_o)) < tol["links"]
+    fx.destroy()
+
+
+def test_slab_sweep_refuses_a_stale_link_halo(slab):
+    from paper_1206_0675_b200 import binding
+
+    dims = (8, 8, 8, 8)
+    fx = slab.SlabFixer(dims, 8, 18, slab.LocalExchange(2))
+    fx.set_links_global(to_dev(inputs.make_config("C1"), 8))
+    with pytest.raises(binding.LgfError):
+        fx.ranks[0].sweep(fx._sums[0])         # no U_t halo yet
+    fx._step_delta()
+    fx._step_accelerate()
+    fx._step_update(ALPHA)                      # in-place update: the halo is stale again
+    with pytest.raises(binding.LgfError):
+        fx.ranks[0].sweep(fx._sums[0])
+    fx.destroy()
+
+
 def test_slab_equals_one_gpu_path_on_c2(slab):
     """16^4 (C2) over 4 ranks against the oracle over 20 iterations, and against the one-GPU path of liblgf."""
     import torch
