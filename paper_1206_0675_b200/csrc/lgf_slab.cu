@@ -22,6 +22,7 @@
 #include <vector>
 
 #include "../../include/lgf.h"
+#include "lgf_fft_split.cuh"
 #include "lgf_fft_steps.cuh"
 #include "lgf_state.cuh"
 
@@ -181,6 +182,7 @@ __global__ void __launch_bounds__(SLAB_SWEEP_THREADS, 3)
 struct LineAddr {
     long long stride_c, stride_o, strideQ, strideN;
     int D;
+    int shift;      // log2(D) when D is a power of two (always, for the lengths the register-line passes take), else -1
 };
 __device__ __forceinline__ long long line_elem(const LineAddr &a, long long base, int n) {
     return base + (long long)(n / a.D) * a.strideQ + (long long)(n % a.D) * a.strideN;
@@ -228,6 +230,67 @@ __global__ void __launch_bounds__(256) k_slab_fft_line(const C<R> *__restrict__ 
         const int lo = idx % nlo, n = idx / nlo;
         dst[line_elem(ad, bd, n) + lo] = tile[idx];
     }
+}
+
+// The same three passes with the line in REGISTERS, two threads per line (lgf_fft_split.cuh; lengths 16, 32, 64 with
+// whole CTAs of 128 consecutive (x, y) indices): no shared memory, every element is loaded once into the register
+// that transforms it, and the axis ends in NATURAL frequency order (the p2 table of that axis is stored accordingly).
+// Thread layout as in lgf_fft_reg2.cu: a warp owns 16 lines, lane = q + 16 h, q runs over the contiguous index.
+__device__ __forceinline__ long long line_elem2(const LineAddr &a, long long base, int n) {
+    return base + (long long)(n >> a.shift) * a.strideQ + (long long)(n & (a.D - 1)) * a.strideN;
+}
+template <class R, int L, int MODE>
+__global__ void __launch_bounds__(256) k_slab_fft_line2(const C<R> *__restrict__ src, C<R> *__restrict__ dst, LineAddr as,
+                                                        LineAddr ad, int Lx, const R *__restrict__ p2tab, R scale) {
+    constexpr int M = L / 2;
+    using S = SplitDft<L, 16, R>;
+    const int tid = threadIdx.x;
+    const int h = (tid >> 4) & 1;
+    const long long xy = (long long)blockIdx.x * 128 + (tid >> 5) * 16 + (tid & 15);
+    const long long bs = (long long)blockIdx.z * as.stride_c + (long long)blockIdx.y * as.stride_o + xy;
+    const long long bd = (long long)blockIdx.z * ad.stride_c + (long long)blockIdx.y * ad.stride_o + xy;
+    C<R> v[M];
+    if constexpr (MODE == FFT_INV) {
+#pragma unroll
+        for (int j = 0; j < M; j++) v[j] = src[line_elem2(as, bs, 2 * j + h)];          // frequency k = 2 j + h
+    } else {
+#pragma unroll
+        for (int m = 0; m < M; m++) v[m] = src[line_elem2(as, bs, m + M * h)];
+        S::forward(v, h);                                                                // -> k = 2 j + h
+    }
+    if constexpr (MODE == FFT_FWD_SCALE_INV) {
+        // t lines: blockIdx.y = zl (p2tab[128 + zl] = this rank's z-slab of the z table); Alg. 1 lines 5, 7
+        const int x = (int)(xy % Lx), y = (int)(xy / Lx);
+        const R p2xyz = p2tab[x] + p2tab[64 + y] + p2tab[128 + blockIdx.y];
+#pragma unroll
+        for (int j = 0; j < M; j++) {
+            const R p2 = p2xyz + p2tab[192 + 2 * j + h];
+            const R f = (p2 == (R)0) ? (R)0 : scale / p2;                                // p2 = 0 only at k = 0 (R6)
+            v[j] = f * v[j];
+        }
+    }
+    if constexpr (MODE == FFT_FWD) {
+#pragma unroll
+        for (int j = 0; j < M; j++) dst[line_elem2(ad, bd, 2 * j + h)] = v[j];
+    } else {
+        S::inverse(v, h);                                                                // -> position m + M h
+#pragma unroll
+        for (int m = 0; m < M; m++) dst[line_elem2(ad, bd, m + M * h)] = v[m];
+    }
+}
+template <class R>
+static cudaError_t launch_line2(int L, int mode, const C<R> *src, C<R> *dst, const LineAddr &as, const LineAddr &ad,
+                                dim3 grid, int Lx, const R *p2tab, R scale, cudaStream_t stream) {
+#define LGF_GO(LEN)                                                                                              \
+    if (L == LEN) {                                                                                              \
+        if (mode == FFT_FWD) k_slab_fft_line2<R, LEN, FFT_FWD><<<grid, 256, 0, stream>>>(src, dst, as, ad, Lx, p2tab, scale); \
+        else if (mode == FFT_INV) k_slab_fft_line2<R, LEN, FFT_INV><<<grid, 256, 0, stream>>>(src, dst, as, ad, Lx, p2tab, scale); \
+        else k_slab_fft_line2<R, LEN, FFT_FWD_SCALE_INV><<<grid, 256, 0, stream>>>(src, dst, as, ad, Lx, p2tab, scale); \
+        return cudaGetLastError();                                                                               \
+    }
+    LGF_GO(16) LGF_GO(32) LGF_GO(64)
+#undef LGF_GO
+    return cudaErrorInvalidValue;
 }
 
 template <class R, int L>
@@ -288,6 +351,7 @@ struct lgf_slab {
     bool xy_reg = false;         // (x, y) planes by the register-line sweeps of lgf_fft_reg2.cu (square planes of 16 / 32 / 64)
     bool xy_gout = false;        // ... and the inverse one can end with the g-build (a5)
     int nlo_z = 1, nlo_t = 1;    // consecutive (x, y) indices per CTA of the z / t line passes
+    bool z_reg = false, t_reg = false;   // z / t lines in registers (k_slab_fft_line2): natural frequency order on that axis
     LineAddr a_w{}, a_zbuf{}, a_tbuf{};
     bool have_links = false;
     long long launches = 0;
@@ -362,7 +426,7 @@ static int slab_tables(lgf_slab *ctx) {
         int N1, N2;
         host_line_factor(L, N1, N2);
         const int first = mu == 2 ? ctx->rank * ctx->Zl : 0, count = mu == 2 ? ctx->Zl : L;
-        const bool natural = mu < 2 && ctx->xy_reg;        // the register-line sweeps leave kx, ky in natural order
+        const bool natural = mu < 2 ? ctx->xy_reg : (mu == 2 ? ctx->z_reg : ctx->t_reg);   // register-line passes: natural order
         for (int i = 0; i < count; i++) {
             const int p = first + i, k = natural ? p : (p / N2) + N1 * (p % N2);
             double c, s;
@@ -388,6 +452,12 @@ static int slab_fft_forward(lgf_slab *ctx, void *d_send) {
             ctx->launches++;
         }
     }
+    if (ctx->z_reg) {
+        SCK(launch_line2<R>(ctx->dims[2], FFT_FWD, (const C<R> *)ctx->W, (C<R> *)d_send, ctx->a_w, ctx->a_zbuf,
+                            dim3((unsigned)(ctx->gl.S[2] / 128), ctx->T, 4), ctx->dims[0], (const R *)ctx->p2tab, (R)0, ctx->stream));
+        ctx->launches++;
+        return LGF_OK;
+    }
     const dim3 grid((unsigned)(ctx->gl.S[2] / ctx->nlo_z), ctx->T, 4);
     SCK(launch_line<R>(ctx->dims[2], FFT_FWD, (const C<R> *)ctx->W, (C<R> *)d_send, ctx->a_w, ctx->a_zbuf, ctx->nlo_z, grid,
                        ctx->dims[0], tw[2], (const R *)ctx->p2tab, (R)0, ctx->stream));
@@ -399,6 +469,12 @@ static int slab_fft_forward(lgf_slab *ctx, void *d_send) {
 template <class R>
 static int slab_fft_t(lgf_slab *ctx, const void *d_recv, void *d_send) {
     const R scale = (R)(16.0 / (double)ctx->Vglobal);              // p2max / V (Alg. 1 lines 5, 7; R5)
+    if (ctx->t_reg) {
+        SCK(launch_line2<R>(ctx->dims[3], FFT_FWD_SCALE_INV, (const C<R> *)d_recv, (C<R> *)d_send, ctx->a_tbuf, ctx->a_tbuf,
+                            dim3((unsigned)(ctx->gl.S[2] / 128), ctx->Zl, 4), ctx->dims[0], (const R *)ctx->p2tab, scale, ctx->stream));
+        ctx->launches++;
+        return LGF_OK;
+    }
     const dim3 grid((unsigned)(ctx->gl.S[2] / ctx->nlo_t), ctx->Zl, 4);
     SCK(launch_line<R>(ctx->dims[3], FFT_FWD_SCALE_INV, (const C<R> *)d_recv, (C<R> *)d_send, ctx->a_tbuf, ctx->a_tbuf, ctx->nlo_t,
                        grid, ctx->dims[0], (const R *)ctx->twiddle[3], (const R *)ctx->p2tab, scale, ctx->stream));
@@ -410,9 +486,14 @@ static int slab_fft_t(lgf_slab *ctx, const void *d_recv, void *d_send) {
 template <class R>
 static int slab_fft_inverse(lgf_slab *ctx, const void *d_recv, bool with_g, double alpha) {
     const R *tw[4] = {(const R *)ctx->twiddle[0], (const R *)ctx->twiddle[1], (const R *)ctx->twiddle[2], (const R *)ctx->twiddle[3]};
-    const dim3 grid((unsigned)(ctx->gl.S[2] / ctx->nlo_z), ctx->T, 4);
-    SCK(launch_line<R>(ctx->dims[2], FFT_INV, (const C<R> *)d_recv, (C<R> *)ctx->W, ctx->a_zbuf, ctx->a_w, ctx->nlo_z, grid,
-                       ctx->dims[0], tw[2], (const R *)ctx->p2tab, (R)0, ctx->stream));
+    if (ctx->z_reg) {
+        SCK(launch_line2<R>(ctx->dims[2], FFT_INV, (const C<R> *)d_recv, (C<R> *)ctx->W, ctx->a_zbuf, ctx->a_w,
+                            dim3((unsigned)(ctx->gl.S[2] / 128), ctx->T, 4), ctx->dims[0], (const R *)ctx->p2tab, (R)0, ctx->stream));
+    } else {
+        const dim3 grid((unsigned)(ctx->gl.S[2] / ctx->nlo_z), ctx->T, 4);
+        SCK(launch_line<R>(ctx->dims[2], FFT_INV, (const C<R> *)d_recv, (C<R> *)ctx->W, ctx->a_zbuf, ctx->a_w, ctx->nlo_z, grid,
+                           ctx->dims[0], tw[2], (const R *)ctx->p2tab, (R)0, ctx->stream));
+    }
     ctx->launches++;
     const R ha = (R)(0.5 * alpha);
     if (ctx->xy_reg) {
@@ -534,9 +615,13 @@ int lgf_slab_create(const int dims[4], int precision, int link_storage, int rank
     ctx->xy_gout = fft_reg2_xy_gout(ctx->gl, precision);
     {   // address maps of the line passes (LineAddr) and their tiles: about 2048 complex elements per CTA
         const long long Sxy = ctx->gl.S[2], chunk = 4LL * ctx->T * ctx->Zl * Sxy;
-        ctx->a_w = LineAddr{Sl, (long long)dims[2] * Sxy, 0, Sxy, dims[2]};
-        ctx->a_zbuf = LineAddr{(long long)ctx->T * ctx->Zl * Sxy, (long long)ctx->Zl * Sxy, chunk, Sxy, ctx->Zl};
-        ctx->a_tbuf = LineAddr{(long long)ctx->T * ctx->Zl * Sxy, Sxy, chunk, (long long)ctx->Zl * Sxy, ctx->T};
+        auto lg2 = [](int d) { int sh = 0; while ((1 << sh) < d) sh++; return (1 << sh) == d ? sh : -1; };
+        ctx->a_w = LineAddr{Sl, (long long)dims[2] * Sxy, 0, Sxy, dims[2], lg2(dims[2])};
+        ctx->a_zbuf = LineAddr{(long long)ctx->T * ctx->Zl * Sxy, (long long)ctx->Zl * Sxy, chunk, Sxy, ctx->Zl, lg2(ctx->Zl)};
+        ctx->a_tbuf = LineAddr{(long long)ctx->T * ctx->Zl * Sxy, Sxy, chunk, (long long)ctx->Zl * Sxy, ctx->T, lg2(ctx->T)};
+        auto reg_len = [](int L) { return L == 16 || L == 32 || L == 64; };
+        ctx->z_reg = reg_len(dims[2]) && Sxy % 128 == 0;          // nranks | L then makes Zl, T powers of two
+        ctx->t_reg = reg_len(dims[3]) && Sxy % 128 == 0;
         ctx->nlo_z = (int)divisor_le(Sxy, 2048 / dims[2]);
         ctx->nlo_t = (int)divisor_le(Sxy, 2048 / dims[3]);
     }

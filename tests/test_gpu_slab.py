@@ -45,7 +45,7 @@ def gathered(slabs):
 # (dims, world): T = Lt / world from the whole lattice down to ONE slice per rank; Zl = Lz / world down to 1
 CASES = [((8, 8, 8, 8), 1), ((8, 8, 8, 8), 2), ((8, 8, 8, 8), 4), ((8, 8, 8, 8), 8), ((12, 6, 16, 4), 2),
          ((12, 6, 16, 4), 4), ((16, 16, 12, 6), 3), ((16, 16, 12, 6), 6), ((3, 24, 2, 48), 2), ((32, 32, 8, 4), 4),
-         ((64, 64, 4, 2), 2)]
+         ((64, 64, 4, 2), 2), ((16, 16, 16, 32), 8), ((32, 32, 16, 16), 4)]
 
 
 @pytest.mark.parametrize("dims,world", CASES)
@@ -134,6 +134,22 @@ def test_slab_sweep_refuses_a_stale_link_halo(slab):
     fx._step_update(ALPHA)                      # in-place update: the halo is stale again
     with pytest.raises(binding.LgfError):
         fx.ranks[0].sweep(fx._sums[0])
+    fx.destroy()
+
+
+@pytest.mark.parametrize("prec", [8, 4])
+def test_slab_64_point_t_lines_in_registers(slab, prec):
+    """Lt = 64: the t pass with 32 complex registers per thread (k_slab_fft_line2<64>), 3 iterations over 4 ranks."""
+    dims, n = (16, 16, 16, 64), 3
+    U = inputs.smooth_config(dims, 0.25, 6464, haar=True)
+    U_o, F_o, T_o = oracle.iterate(dims, U, ALPHA, n)
+    fx = slab.SlabFixer(dims, prec, 18, slab.LocalExchange(4))
+    fx.set_links_global(to_dev(U, prec))
+    fx.iterate(ALPHA, n)
+    Fh, Th = fx.history()
+    tol = TOL[prec]
+    assert np.max(np.abs(Th - T_o) / np.abs(T_o)) < tol["scalar"]
+    assert np.max(np.abs(gathered(fx.get_links()) - U_o)) < tol["links"]
     fx.destroy()
 
 
