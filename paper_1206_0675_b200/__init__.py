@@ -7,5 +7,5 @@ package loads nothing; the binding loads the CUDA library on first use and fails
 missing -- there is no CPU fallback.
 """
 
-__all__ = ["binding", "build", "inputs", "ensemble"]
+__all__ = ["binding", "build", "inputs", "ensemble", "slab"]
 __version__ = "0.1.0"
