@@ -233,20 +233,21 @@ __global__ void __launch_bounds__(256) k_slab_fft_line(const C<R> *__restrict__ 
 }
 
 // The same three passes with the line in REGISTERS, two threads per line (lgf_fft_split.cuh; lengths 16, 32, 64 with
-// whole CTAs of 128 consecutive (x, y) indices): no shared memory, every element is loaded once into the register
+// whole CTAs of LINE2_LINES consecutive (x, y) indices): no shared memory, every element is loaded once into the register
 // that transforms it, and the axis ends in NATURAL frequency order (the p2 table of that axis is stored accordingly).
 // Thread layout as in lgf_fft_reg2.cu: a warp owns 16 lines, lane = q + 16 h, q runs over the contiguous index.
+constexpr int LINE2_LINES = 64;       // lines per CTA (two threads each); with 128 the 512 CTAs of a 32^4 half lattice leave a 0.73 wave tail (iteration 2 % slower)
 __device__ __forceinline__ long long line_elem2(const LineAddr &a, long long base, int n) {
     return base + (long long)(n >> a.shift) * a.strideQ + (long long)(n & (a.D - 1)) * a.strideN;
 }
 template <class R, int L, int MODE>
-__global__ void __launch_bounds__(256) k_slab_fft_line2(const C<R> *__restrict__ src, C<R> *__restrict__ dst, LineAddr as,
+__global__ void __launch_bounds__(2 * LINE2_LINES) k_slab_fft_line2(const C<R> *__restrict__ src, C<R> *__restrict__ dst, LineAddr as,
                                                         LineAddr ad, int Lx, const R *__restrict__ p2tab, R scale) {
     constexpr int M = L / 2;
     using S = SplitDft<L, 16, R>;
     const int tid = threadIdx.x;
     const int h = (tid >> 4) & 1;
-    const long long xy = (long long)blockIdx.x * 128 + (tid >> 5) * 16 + (tid & 15);
+    const long long xy = (long long)blockIdx.x * LINE2_LINES + (tid >> 5) * 16 + (tid & 15);
     const long long bs = (long long)blockIdx.z * as.stride_c + (long long)blockIdx.y * as.stride_o + xy;
     const long long bd = (long long)blockIdx.z * ad.stride_c + (long long)blockIdx.y * ad.stride_o + xy;
     C<R> v[M];
@@ -283,9 +284,9 @@ static cudaError_t launch_line2(int L, int mode, const C<R> *src, C<R> *dst, con
                                 dim3 grid, int Lx, const R *p2tab, R scale, cudaStream_t stream) {
 #define LGF_GO(LEN)                                                                                              \
     if (L == LEN) {                                                                                              \
-        if (mode == FFT_FWD) k_slab_fft_line2<R, LEN, FFT_FWD><<<grid, 256, 0, stream>>>(src, dst, as, ad, Lx, p2tab, scale); \
-        else if (mode == FFT_INV) k_slab_fft_line2<R, LEN, FFT_INV><<<grid, 256, 0, stream>>>(src, dst, as, ad, Lx, p2tab, scale); \
-        else k_slab_fft_line2<R, LEN, FFT_FWD_SCALE_INV><<<grid, 256, 0, stream>>>(src, dst, as, ad, Lx, p2tab, scale); \
+        if (mode == FFT_FWD) k_slab_fft_line2<R, LEN, FFT_FWD><<<grid, 2 * LINE2_LINES, 0, stream>>>(src, dst, as, ad, Lx, p2tab, scale); \
+        else if (mode == FFT_INV) k_slab_fft_line2<R, LEN, FFT_INV><<<grid, 2 * LINE2_LINES, 0, stream>>>(src, dst, as, ad, Lx, p2tab, scale); \
+        else k_slab_fft_line2<R, LEN, FFT_FWD_SCALE_INV><<<grid, 2 * LINE2_LINES, 0, stream>>>(src, dst, as, ad, Lx, p2tab, scale); \
         return cudaGetLastError();                                                                               \
     }
     LGF_GO(16) LGF_GO(32) LGF_GO(64)
@@ -454,7 +455,7 @@ static int slab_fft_forward(lgf_slab *ctx, void *d_send) {
     }
     if (ctx->z_reg) {
         SCK(launch_line2<R>(ctx->dims[2], FFT_FWD, (const C<R> *)ctx->W, (C<R> *)d_send, ctx->a_w, ctx->a_zbuf,
-                            dim3((unsigned)(ctx->gl.S[2] / 128), ctx->T, 4), ctx->dims[0], (const R *)ctx->p2tab, (R)0, ctx->stream));
+                            dim3((unsigned)(ctx->gl.S[2] / LINE2_LINES), ctx->T, 4), ctx->dims[0], (const R *)ctx->p2tab, (R)0, ctx->stream));
         ctx->launches++;
         return LGF_OK;
     }
@@ -471,7 +472,7 @@ static int slab_fft_t(lgf_slab *ctx, const void *d_recv, void *d_send) {
     const R scale = (R)(16.0 / (double)ctx->Vglobal);              // p2max / V (Alg. 1 lines 5, 7; R5)
     if (ctx->t_reg) {
         SCK(launch_line2<R>(ctx->dims[3], FFT_FWD_SCALE_INV, (const C<R> *)d_recv, (C<R> *)d_send, ctx->a_tbuf, ctx->a_tbuf,
-                            dim3((unsigned)(ctx->gl.S[2] / 128), ctx->Zl, 4), ctx->dims[0], (const R *)ctx->p2tab, scale, ctx->stream));
+                            dim3((unsigned)(ctx->gl.S[2] / LINE2_LINES), ctx->Zl, 4), ctx->dims[0], (const R *)ctx->p2tab, scale, ctx->stream));
         ctx->launches++;
         return LGF_OK;
     }
@@ -488,7 +489,7 @@ static int slab_fft_inverse(lgf_slab *ctx, const void *d_recv, bool with_g, doub
     const R *tw[4] = {(const R *)ctx->twiddle[0], (const R *)ctx->twiddle[1], (const R *)ctx->twiddle[2], (const R *)ctx->twiddle[3]};
     if (ctx->z_reg) {
         SCK(launch_line2<R>(ctx->dims[2], FFT_INV, (const C<R> *)d_recv, (C<R> *)ctx->W, ctx->a_zbuf, ctx->a_w,
-                            dim3((unsigned)(ctx->gl.S[2] / 128), ctx->T, 4), ctx->dims[0], (const R *)ctx->p2tab, (R)0, ctx->stream));
+                            dim3((unsigned)(ctx->gl.S[2] / LINE2_LINES), ctx->T, 4), ctx->dims[0], (const R *)ctx->p2tab, (R)0, ctx->stream));
     } else {
         const dim3 grid((unsigned)(ctx->gl.S[2] / ctx->nlo_z), ctx->T, 4);
         SCK(launch_line<R>(ctx->dims[2], FFT_INV, (const C<R> *)d_recv, (C<R> *)ctx->W, ctx->a_zbuf, ctx->a_w, ctx->nlo_z, grid,
@@ -620,8 +621,8 @@ int lgf_slab_create(const int dims[4], int precision, int link_storage, int rank
         ctx->a_zbuf = LineAddr{(long long)ctx->T * ctx->Zl * Sxy, (long long)ctx->Zl * Sxy, chunk, Sxy, ctx->Zl, lg2(ctx->Zl)};
         ctx->a_tbuf = LineAddr{(long long)ctx->T * ctx->Zl * Sxy, Sxy, chunk, (long long)ctx->Zl * Sxy, ctx->T, lg2(ctx->T)};
         auto reg_len = [](int L) { return L == 16 || L == 32 || L == 64; };
-        ctx->z_reg = reg_len(dims[2]) && Sxy % 128 == 0;          // nranks | L then makes Zl, T powers of two
-        ctx->t_reg = reg_len(dims[3]) && Sxy % 128 == 0;
+        ctx->z_reg = reg_len(dims[2]) && Sxy % LINE2_LINES == 0;          // nranks | L then makes Zl, T powers of two
+        ctx->t_reg = reg_len(dims[3]) && Sxy % LINE2_LINES == 0;
         ctx->nlo_z = (int)divisor_le(Sxy, 2048 / dims[2]);
         ctx->nlo_t = (int)divisor_le(Sxy, 2048 / dims[3]);
     }
