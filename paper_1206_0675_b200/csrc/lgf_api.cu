@@ -53,6 +53,8 @@ struct lgf_ctx {
     int tune_hb_tz = 0;          // lgf_tune: z-planes per (z, t) tile of the heat-bath thread order (0 = automatic)
     int tune_reunit = 0;         // lgf_tune "reunit_every": project the new links onto SU(3) in every N-th update (0 = never)
     long long updates_enqueued = 0;   // host-side count of updates enqueued since the last set_links / thermalize
+    int tune_sweep_ahead = 0;    // lgf_tune "sweep_prefetch": CTAs ahead of which the sweep prefetches its tile into L2 (0 = off)
+    int tune_sweep_minb = 3;     // lgf_tune "sweep_minb": resident CTAs per SM the sweep's register allocation allows (3 / 2)
     int tune_sweep_tz = 0;       // lgf_tune: z-planes per (z, t) tile of the sweep's block order (0 = automatic, 1 = plain)
     struct Stamp { cudaEvent_t a, b; int cls; };
     std::vector<Stamp> stamps;
@@ -380,7 +382,8 @@ static int step_update(lgf_ctx *ctx, double alpha, double tol, int record, bool 
     {
         Bracket br(ctx, LGF_K_UPDATE);
         CK(launch_sweep<R>(ctx->nr, link_pair<R>(ctx), (const C<R> *)ctx->G, (C<R> *)ctx->W, ctx->g, ctx->partial,
-                           &ctx->nb_partial, ctx->st, ctx->stream, ctx->tune_sweep_tz, reunit, ctx->tune_sweep_share));
+                           &ctx->nb_partial, ctx->st, ctx->stream, ctx->tune_sweep_tz, reunit, ctx->tune_sweep_share,
+                           ctx->tune_sweep_ahead, ctx->tune_sweep_minb));
     }
     return step_finalize(ctx, tol, 1, record);
 }
@@ -915,6 +918,8 @@ int lgf_tune(lgf_ctx *ctx, const char *key, int value) {
     else if (k == "sweep_tz") ctx->tune_sweep_tz = value;
     else if (k == "hb_tz") ctx->tune_hb_tz = value;
     else if (k == "sweep_share") ctx->tune_sweep_share = value;
+    else if (k == "sweep_prefetch") ctx->tune_sweep_ahead = value < 0 ? 0 : value;
+    else if (k == "sweep_minb") ctx->tune_sweep_minb = value == 2 ? 2 : 3;
     else if (k == "reunit_every") ctx->tune_reunit = value < 0 ? 0 : value;
     else return fail(ctx, LGF_EINVAL, "lgf_tune: unknown key " + k);
     CK(cudaStreamSynchronize(ctx->stream));

@@ -31,22 +31,28 @@ struct SplitDft {
 
     // all 32 lanes of the warp must call (shuffles); h = this thread's half (0 / 1)
     static __device__ __forceinline__ void forward(C<R> (&v)[M], int h) {
+        // one fused multiply-add per real makes both halves' butterfly, o + s v with s = +1 (thread 0: x[m] +
+        // x[m + M]) or -1 (thread 1: x[m] - x[m + M], o being the partner's x[m]); exact, since s v is.  Computing
+        // sum and difference in both threads and selecting cost 4 double-precision adds per element instead of 2.
+        const R s = h ? (R)-1 : (R)1;
         static_for<0, M>([&](auto mc) {
             constexpr int m = decltype(mc)::value;
             const C<R> o = shfl_xor_c(v[m], PMASK);
-            const C<R> sum = v[m] + o;                                   // thread 0: x[m] + x[m + M]
-            const C<R> dif = twiddle_mul<L, m, -1, R>(o - v[m]);         // thread 1: (x[m] - x[m + M]) w^m
-            v[m] = h ? dif : sum;
+            const C<R> t = mk<R>(fma(s, v[m].x, o.x), fma(s, v[m].y, o.y));
+            if constexpr (m == 0) v[m] = t;
+            else v[m] = h ? twiddle_mul<L, m, -1, R>(t) : t;             // thread 1: (x[m] - x[m + M]) w^m
         });
         Dft<M, -1, R>::run(v);
     }
     static __device__ __forceinline__ void inverse(C<R> (&v)[M], int h) {
         Dft<M, +1, R>::run(v);
+        const R s = h ? (R)-1 : (R)1;
         static_for<0, M>([&](auto mc) {
             constexpr int m = decltype(mc)::value;
-            const C<R> y = h ? twiddle_mul<L, m, +1, R>(v[m]) : v[m];    // thread 1: y1[m] conj(w)^m
+            C<R> y = v[m];
+            if constexpr (m != 0) y = h ? twiddle_mul<L, m, +1, R>(v[m]) : v[m];   // thread 1: y1[m] conj(w)^m
             const C<R> o = shfl_xor_c(y, PMASK);
-            v[m] = h ? (o - y) : (y + o);                                // y0 + y1  /  y0 - y1
+            v[m] = mk<R>(fma(s, y.x, o.x), fma(s, y.y, o.y));           // y0 + y1  /  y0 - y1
         });
     }
 };

@@ -172,17 +172,35 @@ __device__ __forceinline__ Herm<R> herm_from_smem(const R *__restrict__ slot, in
 // The register allocation is asked to allow 3 CTAs per SM: 168 registers, no spills in fp64 / 18-real (2 would
 // allow 255 registers at 8 warps per SM, 4 would force spills at 128).
 constexpr int SWEEP_MINB = 3;
-template <class R, int NR, bool REUNIT, bool SHARE>
-__global__ void __launch_bounds__(SWEEP_THREADS, SWEEP_MINB)
+// L2 prefetch (sm_90+ bulk prefetch, SASS UBLKPF): one instruction asks the memory system to bring `bytes`
+// contiguous bytes into L2; nothing is written to the SM, no register or shared memory is held.
+__device__ __forceinline__ void prefetch_l2_bulk(const void *p, unsigned bytes) {
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
+}
+template <class R, int NR, bool REUNIT, bool SHARE, int MINB>
+__global__ void __launch_bounds__(SWEEP_THREADS, MINB)
     k_sweep(LinkPair<R> lp, const C<R> *__restrict__ G, C<R> *__restrict__ W, Geom g, double *__restrict__ partial,
-            const DevState *__restrict__ st, BlockOrder bo) {
+            const DevState *__restrict__ st, BlockOrder bo, int ahead) {
     pdl_enter();
     if (st->done) return;
     const int cur = st->cur;
-    const C<R> *__restrict__ src = lp.buf[cur];
-    C<R> *__restrict__ dst = lp.buf[1 - cur];
+    // (a select between the two kernel parameters, not an indexed load of the parameter array: the pointers stay
+    // in the global address space -- LDG / STG instead of generic LD / ST -- and the array is not copied to the stack)
+    const C<R> *__restrict__ src = cur ? lp.buf[1] : lp.buf[0];
+    C<R> *__restrict__ dst = cur ? lp.buf[0] : lp.buf[1];
     __shared__ double scratch[SWEEP_THREADS / 32][2];
     __shared__ R sA[SHARE ? 2 * 8 * SWEEP_THREADS : 1];          // A'_x, A'_y of the CTA's sites
+    // The kernel is latency-bound (12 warps per SM, half of their time waiting on DRAM): the CTA that will run
+    // `ahead` blocks later finds its own links and g(x) -- 4 * 3 NR + 6 planes of 128 consecutive sites -- in L2
+    // already, because this CTA asks for them now: one bulk prefetch per plane, issued by the first threads.
+    if (ahead > 0 && blockIdx.x + ahead < gridDim.x) {
+        constexpr int NP = 4 * 3 * NR;
+        const long long pb = block_base(bo, blockIdx.x + ahead) * SWEEP_THREADS;
+        const long long left = g.V - pb;
+        const unsigned bytes = (unsigned)((left < SWEEP_THREADS ? left : SWEEP_THREADS) * sizeof(C<R>));
+        if (threadIdx.x < NP) prefetch_l2_bulk(src + (long long)threadIdx.x * g.V + pb, bytes);
+        else if (threadIdx.x < NP + 6) prefetch_l2_bulk(G + (long long)(threadIdx.x - NP) * g.V + pb, bytes);
+    }
     const long long base = block_base(bo, blockIdx.x) * SWEEP_THREADS;
     const long long s = base + threadIdx.x;
     const bool live = s < g.V;
@@ -498,7 +516,8 @@ cudaError_t launch_gbuild(const C<R> *W, C<R> *G, const Geom &g, R half_alpha, c
 }
 template <class R>
 cudaError_t launch_sweep(int nr, LinkPair<R> links, const C<R> *G, C<R> *W, const Geom &g, double *partial,
-                         int *nblocks, const DevState *st, cudaStream_t stream, int order_tz, bool reunit, int share_mode) {
+                         int *nblocks, const DevState *st, cudaStream_t stream, int order_tz, bool reunit, int share_mode,
+                         int ahead, int minb) {
     const int nb = (int)((g.V + SWEEP_THREADS - 1) / SWEEP_THREADS);
     *nblocks = nb;
     // (z, t)-tiled block order when the (x, y) plane is a whole number of CTAs; TZ: about 24 MB of traffic
@@ -523,13 +542,17 @@ cudaError_t launch_sweep(int nr, LinkPair<R> links, const C<R> *G, C<R> *W, cons
         }
         if (tz > 1 && g.L[2] % tz == 0) { bo.nxy = (int)(plane / SWEEP_THREADS); bo.tz = tz; }
     }
-#define LGF_SWK(RU, SH)                                                                                  \
-    if (nr == 3) return launch_pdl(k_sweep<R, 3, RU, SH>, dim3(nb), dim3(SWEEP_THREADS), 0, stream, links, G, W, g, partial, st, bo); \
-    else return launch_pdl(k_sweep<R, 2, RU, SH>, dim3(nb), dim3(SWEEP_THREADS), 0, stream, links, G, W, g, partial, st, bo);
-    if (reunit && share) { LGF_SWK(true, true) }
-    else if (reunit) { LGF_SWK(true, false) }
-    else if (share) { LGF_SWK(false, true) }
-    else { LGF_SWK(false, false) }
+#define LGF_SWK(RU, SH, MB)                                                                              \
+    if (nr == 3) return launch_pdl(k_sweep<R, 3, RU, SH, MB>, dim3(nb), dim3(SWEEP_THREADS), 0, stream, links, G, W, g, partial, st, bo, ahead); \
+    else return launch_pdl(k_sweep<R, 2, RU, SH, MB>, dim3(nb), dim3(SWEEP_THREADS), 0, stream, links, G, W, g, partial, st, bo, ahead);
+    if (minb == 2) {
+        if (share) { LGF_SWK(false, true, 2) }
+        else { LGF_SWK(false, false, 2) }
+    }
+    if (reunit && share) { LGF_SWK(true, true, SWEEP_MINB) }
+    else if (reunit) { LGF_SWK(true, false, SWEEP_MINB) }
+    else if (share) { LGF_SWK(false, true, SWEEP_MINB) }
+    else { LGF_SWK(false, false, SWEEP_MINB) }
 #undef LGF_SWK
     return cudaGetLastError();
 }
@@ -614,7 +637,7 @@ cudaError_t launch_clear_done(DevState *st, cudaStream_t stream) {
                                          const DevState *, cudaStream_t);                                             \
     template cudaError_t launch_gbuild<R>(const C<R> *, C<R> *, const Geom &, R, const DevState *, cudaStream_t);     \
     template cudaError_t launch_sweep<R>(int, LinkPair<R>, const C<R> *, C<R> *, const Geom &, double *, int *,       \
-                                         const DevState *, cudaStream_t, int, bool, int);                                             \
+                                         const DevState *, cudaStream_t, int, bool, int, int, int);                                   \
     template cudaError_t launch_plaquette<R>(int, LinkPair<R>, const Geom &, double *, int *, const DevState *,       \
                                              cudaStream_t);                                                           \
     template cudaError_t launch_convert_in<R>(int, const R *, C<R> *, const Geom &, cudaStream_t);                    \

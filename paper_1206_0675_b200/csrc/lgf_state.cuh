@@ -89,7 +89,9 @@ template <class R>
 cudaError_t launch_sweep(int nr, LinkPair<R> links, const C<R> *G, C<R> *W, const Geom &g, double *partial,
                          int *nblocks, const DevState *st, cudaStream_t stream, int order_tz /* 0 auto, 1 plain */,
                          bool reunit /* project every new link onto SU(3) */,
-                         int share_mode /* A'_x, A'_y through shared memory: 1 / 0 / -1 = where it measured faster */);
+                         int share_mode /* A'_x, A'_y through shared memory: 1 / 0 / -1 = where it measured faster */,
+                         int ahead /* L2 bulk prefetch of the tile `ahead` CTAs later (0 = none) */,
+                         int minb /* resident CTAs per SM the register allocation allows: 3 (168 registers) or 2 (255) */);
 template <class R>
 cudaError_t launch_plaquette(int nr, LinkPair<R> links, const Geom &g, double *partial, int *nblocks,
                              const DevState *st, cudaStream_t stream);
