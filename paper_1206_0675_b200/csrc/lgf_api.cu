@@ -12,7 +12,6 @@
 #include "lgf_state.cuh"
 
 using namespace lgf;
-namespace lgf { int g_pdl_enabled = 1; }   // programmatic dependent launch of the iteration's kernels (lgf_pdl.cuh)
 
 struct lgf_ctx {
     Geom g{};
@@ -53,6 +52,7 @@ struct lgf_ctx {
     int tune_hb_tz = 0;          // lgf_tune: z-planes per (z, t) tile of the heat-bath thread order (0 = automatic)
     int tune_reunit = 0;         // lgf_tune "reunit_every": project the new links onto SU(3) in every N-th update (0 = never)
     long long updates_enqueued = 0;   // host-side count of updates enqueued since the last set_links / thermalize
+    int tune_pdl = 1;            // lgf_tune "pdl": launch the iteration's kernels with programmatic stream serialization
     int tune_sweep_ahead = 0;    // lgf_tune "sweep_prefetch": CTAs ahead of which the sweep prefetches its tile into L2 (0 = off)
     int tune_sweep_minb = 3;     // lgf_tune "sweep_minb": resident CTAs per SM the sweep's register allocation allows (3 / 2)
     int tune_sweep_tz = 0;       // lgf_tune: z-planes per (z, t) tile of the sweep's block order (0 = automatic, 1 = plain)
@@ -80,6 +80,9 @@ static int cuda_fail(lgf_ctx *ctx, cudaError_t e, const char *what) {
         cudaError_t e_ = (call);                                     \
         if (e_ != cudaSuccess) return cuda_fail(ctx, e_, #call);     \
     } while (0)
+
+// the context's stream with its dependent-launch setting, for the launchers
+#define STRM(ctx) (lgf::LaunchStream((ctx)->stream, (ctx)->tune_pdl != 0))
 
 // ---- host-side tables -----------------------------------------------------------------------------
 static bool valid_len(int L) {
@@ -324,7 +327,7 @@ template <class R>
 static int step_delta(lgf_ctx *ctx, const int *stop) {
     Bracket br(ctx, LGF_K_DELTA);
     CK(launch_delta<R>(ctx->nr, link_pair<R>(ctx), (C<R> *)ctx->W, ctx->g, ctx->partial, &ctx->nb_partial, stop, ctx->st,
-                       ctx->stream));
+                       STRM(ctx)));
     return LGF_OK;
 }
 // true if the plan's last sweep can end with the g-build (a5) and write G instead of W
@@ -342,18 +345,18 @@ static int step_accelerate(lgf_ctx *ctx, bool with_g = false, double alpha = 0.0
         if (p.kind == PASS_REG) {
             const int which = (with_g && p.axis == 2) ? 3 : p.axis;
             CK(launch_fft_reg<R>(which, ctx->g, (C<R> *)ctx->W, (const R *)ctx->twiddle[3], (const R *)ctx->p2tab, scale,
-                                 ctx->st, ctx->stream, (C<R> *)ctx->G, (R)(0.5 * alpha)));
+                                 ctx->st, STRM(ctx), (C<R> *)ctx->G, (R)(0.5 * alpha)));
             continue;
         }
         if (p.kind == PASS_REG2) {
             const int which = (with_g && p.axis == 2) ? 3 : p.axis;
-            CK(launch_fft_reg2<R>(which, ctx->g, (C<R> *)ctx->W, (const R *)ctx->p2tab, scale, ctx->st, ctx->stream,
+            CK(launch_fft_reg2<R>(which, ctx->g, (C<R> *)ctx->W, (const R *)ctx->p2tab, scale, ctx->st, STRM(ctx),
                                   (C<R> *)ctx->G, (R)(0.5 * alpha)));
             continue;
         }
         const R *tw[4] = {(const R *)ctx->twiddle[0], (const R *)ctx->twiddle[1], (const R *)ctx->twiddle[2],
                           (const R *)ctx->twiddle[3]};
-        CK(launch_fft_pass<R>(p, (C<R> *)ctx->W, ctx->g, tw, (const R *)ctx->p2tab, scale, ctx->st, ctx->stream));
+        CK(launch_fft_pass<R>(p, (C<R> *)ctx->W, ctx->g, tw, (const R *)ctx->p2tab, scale, ctx->st, STRM(ctx)));
     }
     return LGF_OK;
 }
@@ -362,7 +365,7 @@ static int step_accelerate(lgf_ctx *ctx, bool with_g = false, double alpha = 0.0
 static int step_finalize(lgf_ctx *ctx, double tol, int after_sweep, int record) {
     ctx->launches++;
     CK(launch_finalize(ctx->partial, ctx->nb_partial, ctx->g.V, tol, after_sweep, record, ctx->st, ctx->hist,
-                       ctx->hist_cap, ctx->stream));
+                       ctx->hist_cap, STRM(ctx)));
     return LGF_OK;
 }
 // The sweep also closes the iteration: it makes the new configuration current, and with record != 0 appends
@@ -371,18 +374,18 @@ template <class R>
 static int step_update(lgf_ctx *ctx, double alpha, double tol, int record, bool g_ready = false) {
     if (!g_ready) {
         Bracket br(ctx, LGF_K_GBUILD);
-        CK(launch_gbuild<R>((const C<R> *)ctx->W, (C<R> *)ctx->G, ctx->g, (R)(0.5 * alpha), ctx->st, ctx->stream));
+        CK(launch_gbuild<R>((const C<R> *)ctx->W, (C<R> *)ctx->G, ctx->g, (R)(0.5 * alpha), ctx->st, STRM(ctx)));
     }
     if (ctx->Gacc) {                                      // Gacc <- g Gacc, with the g this update applies
         Bracket br(ctx, LGF_K_GBUILD);
-        CK(launch_gacc<R>(1, (const C<R> *)ctx->G, (C<R> *)ctx->Gacc, (R *)nullptr, ctx->g, ctx->st, ctx->stream));
+        CK(launch_gacc<R>(1, (const C<R> *)ctx->G, (C<R> *)ctx->Gacc, (R *)nullptr, ctx->g, ctx->st, STRM(ctx)));
     }
     ctx->updates_enqueued++;
     const bool reunit = ctx->tune_reunit > 0 && ctx->updates_enqueued % ctx->tune_reunit == 0;
     {
         Bracket br(ctx, LGF_K_UPDATE);
         CK(launch_sweep<R>(ctx->nr, link_pair<R>(ctx), (const C<R> *)ctx->G, (C<R> *)ctx->W, ctx->g, ctx->partial,
-                           &ctx->nb_partial, ctx->st, ctx->stream, ctx->tune_sweep_tz, reunit, ctx->tune_sweep_share,
+                           &ctx->nb_partial, ctx->st, STRM(ctx), ctx->tune_sweep_tz, reunit, ctx->tune_sweep_share,
                            ctx->tune_sweep_ahead, ctx->tune_sweep_minb));
     }
     return step_finalize(ctx, tol, 1, record);
@@ -429,14 +432,14 @@ static int measure_only(lgf_ctx *ctx) {
 template <class R>
 static int apply_transform(lgf_ctx *ctx, const void *d_transform) {
     ctx->launches++;
-    CK(launch_gacc<R>(3, nullptr, (C<R> *)ctx->G, (R *)const_cast<void *>(d_transform), ctx->g, ctx->st, ctx->stream));
+    CK(launch_gacc<R>(3, nullptr, (C<R> *)ctx->G, (R *)const_cast<void *>(d_transform), ctx->g, ctx->st, STRM(ctx)));
     ctx->launches++;
-    CK(launch_clear_done(ctx->st, ctx->stream));
+    CK(launch_clear_done(ctx->st, STRM(ctx)));
     // the fused sweep with the given field in the place of g: U <- G U G(x+mu)^dag, Delta / F / theta of the result
     const int rc = step_update<R>(ctx, 0.0, -1.0, 0, true);
     if (rc != LGF_OK) return rc;
     ctx->launches++;
-    CK(launch_reset_counters(ctx->st, ctx->stream));       // a new starting configuration: history and counters restart
+    CK(launch_reset_counters(ctx->st, STRM(ctx)));       // a new starting configuration: history and counters restart
     ctx->w_is_delta = true;                                  // ... whose Delta and partial sums the sweep has left behind
     ctx->recorded = false;
     ctx->updates_enqueued = 0;
@@ -449,9 +452,9 @@ static int apply_transform(lgf_ctx *ctx, const void *d_transform) {
 template <class R>
 static int gluon_field(lgf_ctx *ctx, int mu, void *d_out) {
     ctx->launches++;
-    CK(launch_algebra<R>(ctx->nr, link_pair<R>(ctx), (C<R> *)ctx->W, ctx->g, mu, ctx->st, ctx->stream));
+    CK(launch_algebra<R>(ctx->nr, link_pair<R>(ctx), (C<R> *)ctx->W, ctx->g, mu, ctx->st, STRM(ctx)));
     ctx->launches++;
-    CK(launch_clear_done(ctx->st, ctx->stream));          // the FFT passes return at once while `done` is set
+    CK(launch_clear_done(ctx->st, STRM(ctx)));          // the FFT passes return at once while `done` is set
     const R *tw[4] = {(const R *)ctx->twiddle[0], (const R *)ctx->twiddle[1], (const R *)ctx->twiddle[2],
                       (const R *)ctx->twiddle[3]};
     int N1[4], N2[4];
@@ -459,10 +462,10 @@ static int gluon_field(lgf_ctx *ctx, int mu, void *d_out) {
         line_factor(ctx->g.L[axis], N1[axis], N2[axis]);
         const AxisPass p = make_axis_pass(ctx, axis, FFT_FWD);
         Bracket br(ctx, LGF_K_FFT);
-        CK(launch_fft_pass<R>(p, (C<R> *)ctx->W, ctx->g, tw, (const R *)ctx->p2tab, (R)1, ctx->st, ctx->stream));
+        CK(launch_fft_pass<R>(p, (C<R> *)ctx->W, ctx->g, tw, (const R *)ctx->p2tab, (R)1, ctx->st, STRM(ctx)));
     }
     ctx->launches++;
-    CK(launch_gluon_unpack<R>((const C<R> *)ctx->W, (R *)d_out, ctx->g, N1, N2, ctx->stream));
+    CK(launch_gluon_unpack<R>((const C<R> *)ctx->W, (R *)d_out, ctx->g, N1, N2, STRM(ctx)));
     ctx->w_is_delta = false;
     return LGF_OK;
 }
@@ -532,7 +535,7 @@ int lgf_create(const int dims[4], int precision, int link_storage, lgf_ctx **out
     if (rc == LGF_OK) rc = precision == LGF_FP64 ? upload_twiddles<double>(ctx) : upload_twiddles<float>(ctx);
     if (rc == LGF_OK) rc = plan_passes(ctx);
     if (rc == LGF_OK) {
-        cudaError_t ee = launch_reset_state(ctx->st, ctx->stream);
+        cudaError_t ee = launch_reset_state(ctx->st, STRM(ctx));
         if (ee == cudaSuccess) ee = cudaStreamSynchronize(ctx->stream);
         if (ee != cudaSuccess) rc = cuda_fail(ctx, ee, "reset_state");
     }
@@ -581,19 +584,19 @@ int lgf_set_links(lgf_ctx *ctx, const void *d_links) {
     {
         Bracket br(ctx, LGF_K_CONVERT);
         if (ctx->prec == LGF_FP64)
-            CK(launch_convert_in<double>(ctx->nr, (const double *)d_links, (C<double> *)ctx->links[0], ctx->g, ctx->stream));
+            CK(launch_convert_in<double>(ctx->nr, (const double *)d_links, (C<double> *)ctx->links[0], ctx->g, STRM(ctx)));
         else
-            CK(launch_convert_in<float>(ctx->nr, (const float *)d_links, (C<float> *)ctx->links[0], ctx->g, ctx->stream));
+            CK(launch_convert_in<float>(ctx->nr, (const float *)d_links, (C<float> *)ctx->links[0], ctx->g, STRM(ctx)));
     }
     if (ctx->Gacc) {
         ctx->launches++;
         if (ctx->prec == LGF_FP64)
-            CK(launch_gacc<double>(0, nullptr, (C<double> *)ctx->Gacc, nullptr, ctx->g, ctx->st, ctx->stream));
+            CK(launch_gacc<double>(0, nullptr, (C<double> *)ctx->Gacc, nullptr, ctx->g, ctx->st, STRM(ctx)));
         else
-            CK(launch_gacc<float>(0, nullptr, (C<float> *)ctx->Gacc, nullptr, ctx->g, ctx->st, ctx->stream));
+            CK(launch_gacc<float>(0, nullptr, (C<float> *)ctx->Gacc, nullptr, ctx->g, ctx->st, STRM(ctx)));
     }
     ctx->launches++;
-    CK(launch_reset_state(ctx->st, ctx->stream));        // also makes buffer 0 the current one
+    CK(launch_reset_state(ctx->st, STRM(ctx)));        // also makes buffer 0 the current one
     ctx->have_links = true;
     ctx->w_is_delta = false;
     ctx->recorded = false;
@@ -607,9 +610,9 @@ int lgf_get_links(lgf_ctx *ctx, void *d_links) {
     if (!ctx->have_links) return fail(ctx, LGF_ESTATE, "lgf_get_links: no configuration loaded");
     Bracket br(ctx, LGF_K_CONVERT);
     if (ctx->prec == LGF_FP64)
-        CK(launch_convert_out<double>(ctx->nr, link_pair<double>(ctx), (double *)d_links, ctx->g, ctx->st, ctx->stream));
+        CK(launch_convert_out<double>(ctx->nr, link_pair<double>(ctx), (double *)d_links, ctx->g, ctx->st, STRM(ctx)));
     else
-        CK(launch_convert_out<float>(ctx->nr, link_pair<float>(ctx), (float *)d_links, ctx->g, ctx->st, ctx->stream));
+        CK(launch_convert_out<float>(ctx->nr, link_pair<float>(ctx), (float *)d_links, ctx->g, ctx->st, STRM(ctx)));
     return LGF_OK;
 }
 
@@ -644,7 +647,7 @@ int lgf_iterate(lgf_ctx *ctx, double alpha, int n) {
     if (!ctx || n < 0) return fail(ctx, LGF_EINVAL, "lgf_iterate: bad argument");
     if (!ctx->have_links) return fail(ctx, LGF_ESTATE, "lgf_iterate: no configuration loaded");
     ctx->launches++;
-    CK(launch_clear_done(ctx->st, ctx->stream));
+    CK(launch_clear_done(ctx->st, STRM(ctx)));
     // tol = -1: theta >= 0 never stops the loop; only a NaN does
     int rc = DISPATCH(first_measure, ctx, -1.0);
     if (rc != LGF_OK) return rc;
@@ -662,12 +665,12 @@ int lgf_measure(lgf_ctx *ctx, double *F, double *theta, double *plaquette) {
         {
             Bracket br(ctx, LGF_K_PLAQ);
             if (ctx->prec == LGF_FP64)
-                CK(launch_plaquette<double>(ctx->nr, link_pair<double>(ctx), ctx->g, part, &nb, ctx->st, ctx->stream));
+                CK(launch_plaquette<double>(ctx->nr, link_pair<double>(ctx), ctx->g, part, &nb, ctx->st, STRM(ctx)));
             else
-                CK(launch_plaquette<float>(ctx->nr, link_pair<float>(ctx), ctx->g, part, &nb, ctx->st, ctx->stream));
+                CK(launch_plaquette<float>(ctx->nr, link_pair<float>(ctx), ctx->g, part, &nb, ctx->st, STRM(ctx)));
         }
         ctx->launches++;
-        CK(launch_sum1(part, nb, 1.0 / (18.0 * (double)ctx->g.V), ctx->d_scalar, ctx->stream));
+        CK(launch_sum1(part, nb, 1.0 / (18.0 * (double)ctx->g.V), ctx->d_scalar, STRM(ctx)));
         double *hp = reinterpret_cast<double *>(ctx->h_st + 1);
         CK(cudaMemcpyAsync(hp, ctx->d_scalar, sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
     }
@@ -785,7 +788,7 @@ int lgf_step_delta(lgf_ctx *ctx, double *F, double *theta) {
 int lgf_step_accelerate(lgf_ctx *ctx) {
     if (!ctx) return LGF_EINVAL;
     ctx->launches++;
-    CK(launch_clear_done(ctx->st, ctx->stream));
+    CK(launch_clear_done(ctx->st, STRM(ctx)));
     ctx->w_is_delta = false;
     return DISPATCH(step_accelerate, ctx, false, 0.0);
 }
@@ -794,7 +797,7 @@ int lgf_step_update(lgf_ctx *ctx, double alpha) {
     if (!ctx) return LGF_EINVAL;
     if (!ctx->have_links) return fail(ctx, LGF_ESTATE, "lgf_step_update: no configuration loaded");
     ctx->launches++;
-    CK(launch_clear_done(ctx->st, ctx->stream));
+    CK(launch_clear_done(ctx->st, STRM(ctx)));
     const int rc = DISPATCH(step_update, ctx, alpha, -1.0, 0, false);
     if (rc != LGF_OK) return rc;
     ctx->w_is_delta = true;            // the sweep left Delta of the new links in W
@@ -805,16 +808,16 @@ int lgf_step_update(lgf_ctx *ctx, double alpha) {
 int lgf_get_field(lgf_ctx *ctx, void *d_field) {
     if (!ctx || !d_field) return fail(ctx, LGF_EINVAL, "lgf_get_field: null argument");
     ctx->launches++;
-    if (ctx->prec == LGF_FP64) CK(launch_field_get<double>((const C<double> *)ctx->W, (double *)d_field, ctx->g, ctx->stream));
-    else CK(launch_field_get<float>((const C<float> *)ctx->W, (float *)d_field, ctx->g, ctx->stream));
+    if (ctx->prec == LGF_FP64) CK(launch_field_get<double>((const C<double> *)ctx->W, (double *)d_field, ctx->g, STRM(ctx)));
+    else CK(launch_field_get<float>((const C<float> *)ctx->W, (float *)d_field, ctx->g, STRM(ctx)));
     return LGF_OK;
 }
 
 int lgf_set_field(lgf_ctx *ctx, const void *d_field) {
     if (!ctx || !d_field) return fail(ctx, LGF_EINVAL, "lgf_set_field: null argument");
     ctx->launches++;
-    if (ctx->prec == LGF_FP64) CK(launch_field_set<double>((C<double> *)ctx->W, (const double *)d_field, ctx->g, ctx->stream));
-    else CK(launch_field_set<float>((C<float> *)ctx->W, (const float *)d_field, ctx->g, ctx->stream));
+    if (ctx->prec == LGF_FP64) CK(launch_field_set<double>((C<double> *)ctx->W, (const double *)d_field, ctx->g, STRM(ctx)));
+    else CK(launch_field_set<float>((C<float> *)ctx->W, (const float *)d_field, ctx->g, STRM(ctx)));
     ctx->w_is_delta = false;
     return LGF_OK;
 }
@@ -830,25 +833,25 @@ static int monte_carlo_sweeps(lgf_ctx *ctx, double beta, int nsweeps, unsigned l
                 Bracket br(ctx, LGF_K_HEATBATH);
                 if (ctx->prec == LGF_FP64)
                     CK(launch_heatbath<double>(ctx->nr, link_pair<double>(ctx), ctx->g, ctx->st, beta, key, ctx->hb_sweeps,
-                                               mu, parity, ctx->stream, overrelax, ctx->tune_hb_tz));
+                                               mu, parity, STRM(ctx), overrelax, ctx->tune_hb_tz));
                 else
                     CK(launch_heatbath<float>(ctx->nr, link_pair<float>(ctx), ctx->g, ctx->st, beta, key, ctx->hb_sweeps, mu,
-                                              parity, ctx->stream, overrelax, ctx->tune_hb_tz));
+                                              parity, STRM(ctx), overrelax, ctx->tune_hb_tz));
             }
         if (!overrelax) ctx->hb_sweeps++;                // only heat-bath sweeps consume random numbers
     }
     // a new configuration: the history, the counters and the accumulated transformation start again
     ctx->launches++;
-    CK(launch_reset_counters(ctx->st, ctx->stream));
+    CK(launch_reset_counters(ctx->st, STRM(ctx)));
     ctx->w_is_delta = false;
     ctx->recorded = false;
     ctx->updates_enqueued = 0;
     if (ctx->Gacc) {
         ctx->launches++;
         if (ctx->prec == LGF_FP64)
-            CK(launch_gacc<double>(0, nullptr, (C<double> *)ctx->Gacc, nullptr, ctx->g, ctx->st, ctx->stream));
+            CK(launch_gacc<double>(0, nullptr, (C<double> *)ctx->Gacc, nullptr, ctx->g, ctx->st, STRM(ctx)));
         else
-            CK(launch_gacc<float>(0, nullptr, (C<float> *)ctx->Gacc, nullptr, ctx->g, ctx->st, ctx->stream));
+            CK(launch_gacc<float>(0, nullptr, (C<float> *)ctx->Gacc, nullptr, ctx->g, ctx->st, STRM(ctx)));
     }
     return LGF_OK;
 }
@@ -876,9 +879,9 @@ int lgf_track_transform(lgf_ctx *ctx, int on) {
     if (!ctx->Gacc) CK(cudaMalloc(&ctx->Gacc, (size_t)ctx->g.V * 9 * 2 * ctx->prec));
     ctx->launches++;
     if (ctx->prec == LGF_FP64)
-        CK(launch_gacc<double>(0, nullptr, (C<double> *)ctx->Gacc, nullptr, ctx->g, ctx->st, ctx->stream));
+        CK(launch_gacc<double>(0, nullptr, (C<double> *)ctx->Gacc, nullptr, ctx->g, ctx->st, STRM(ctx)));
     else
-        CK(launch_gacc<float>(0, nullptr, (C<float> *)ctx->Gacc, nullptr, ctx->g, ctx->st, ctx->stream));
+        CK(launch_gacc<float>(0, nullptr, (C<float> *)ctx->Gacc, nullptr, ctx->g, ctx->st, STRM(ctx)));
     return LGF_OK;
 }
 
@@ -887,9 +890,9 @@ int lgf_get_transform(lgf_ctx *ctx, void *d_transform) {
     if (!ctx->Gacc) return fail(ctx, LGF_ESTATE, "lgf_get_transform: tracking is off (lgf_track_transform)");
     ctx->launches++;
     if (ctx->prec == LGF_FP64)
-        CK(launch_gacc<double>(2, nullptr, (C<double> *)ctx->Gacc, (double *)d_transform, ctx->g, ctx->st, ctx->stream));
+        CK(launch_gacc<double>(2, nullptr, (C<double> *)ctx->Gacc, (double *)d_transform, ctx->g, ctx->st, STRM(ctx)));
     else
-        CK(launch_gacc<float>(2, nullptr, (C<float> *)ctx->Gacc, (float *)d_transform, ctx->g, ctx->st, ctx->stream));
+        CK(launch_gacc<float>(2, nullptr, (C<float> *)ctx->Gacc, (float *)d_transform, ctx->g, ctx->st, STRM(ctx)));
     return LGF_OK;
 }
 
@@ -914,7 +917,7 @@ int lgf_tune(lgf_ctx *ctx, const char *key, int value) {
     else if (k == "fft_xy_planes") ctx->tune_xy_planes = value;
     else if (k == "fft_zt_xc") ctx->tune_zt_xc = value;
     else if (k == "fuse_g") ctx->tune_fuse_g = value;
-    else if (k == "pdl") lgf::g_pdl_enabled = value != 0;          // a launch attribute: process-wide, not per context
+    else if (k == "pdl") ctx->tune_pdl = value != 0;               // programmatic dependent launch of this context's kernels
     else if (k == "sweep_tz") ctx->tune_sweep_tz = value;
     else if (k == "hb_tz") ctx->tune_hb_tz = value;
     else if (k == "sweep_share") ctx->tune_sweep_share = value;

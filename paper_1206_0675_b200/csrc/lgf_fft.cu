@@ -169,7 +169,7 @@ static cudaError_t set_smem(K kern, size_t smem) {
 
 template <class R, int L>
 static cudaError_t launch_L(const AxisPass &p, C<R> *W, const Geom &g, const R *twiddle, const R *p2tab, R scale,
-                            const DevState *st, cudaStream_t stream) {
+                            const DevState *st, LaunchStream stream) {
     const int lo_blocks = (int)(p.S / p.nlo);
     const long long tiles = (long long)lo_blocks * (p.H / p.nhi);
     dim3 grid((unsigned)tiles, 4);
@@ -188,7 +188,7 @@ static cudaError_t launch_L(const AxisPass &p, C<R> *W, const Geom &g, const R *
 
 template <class R, int LX, int LY>
 static cudaError_t launch_xy(const AxisPass &p, C<R> *W, const Geom &g, const R *const twiddle[4], const DevState *st,
-                             cudaStream_t stream) {
+                             LaunchStream stream) {
     const long long planes = 4LL * g.L[2] * g.L[3];
     const unsigned grid = (unsigned)(planes / p.nhi);
     const C<R> *twx = reinterpret_cast<const C<R> *>(twiddle[0]), *twy = reinterpret_cast<const C<R> *>(twiddle[1]);
@@ -202,7 +202,7 @@ static cudaError_t launch_xy(const AxisPass &p, C<R> *W, const Geom &g, const R 
 
 template <class R, int LZ, int LT>
 static cudaError_t launch_zt(const AxisPass &p, C<R> *W, const Geom &g, const R *const twiddle[4], const R *p2tab,
-                             R scale, const DevState *st, cudaStream_t stream) {
+                             R scale, const DevState *st, LaunchStream stream) {
     dim3 grid((unsigned)(g.S[2] / p.nlo), 4);
     const C<R> *twz = reinterpret_cast<const C<R> *>(twiddle[2]), *twt = reinterpret_cast<const C<R> *>(twiddle[3]);
     auto kern = k_fft_zt<R, LZ, LT>;
@@ -225,7 +225,7 @@ bool fft_pair_supported(int kind, int La, int Lb) {
 
 template <class R>
 cudaError_t launch_fft_pass(const AxisPass &p, C<R> *W, const Geom &g, const R *const twiddle[4], const R *p2tab,
-                            R scale, const DevState *st, cudaStream_t stream) {
+                            R scale, const DevState *st, LaunchStream stream) {
     if (p.kind == PASS_XY) {
 #define LGF_GO(A, B) if (p.L == A && p.L2 == B) return launch_xy<R, A, B>(p, W, g, twiddle, st, stream);
         LGF_XY_PAIRS(LGF_GO)
@@ -248,8 +248,8 @@ cudaError_t launch_fft_pass(const AxisPass &p, C<R> *W, const Geom &g, const R *
 }
 
 template cudaError_t launch_fft_pass<float>(const AxisPass &, C<float> *, const Geom &, const float *const[4],
-                                            const float *, float, const DevState *, cudaStream_t);
+                                            const float *, float, const DevState *, LaunchStream);
 template cudaError_t launch_fft_pass<double>(const AxisPass &, C<double> *, const Geom &, const double *const[4],
-                                             const double *, double, const DevState *, cudaStream_t);
+                                             const double *, double, const DevState *, LaunchStream);
 
 }  // namespace lgf

@@ -216,7 +216,7 @@ bool fft_reg_t_natural(const Geom &g) {
 
 template <class R>
 cudaError_t launch_fft_reg(int which, const Geom &g, C<R> *W, const R *twiddle_t, const R *p2tab, R scale,
-                           const DevState *st, cudaStream_t stream, C<R> *G, R half_alpha) {
+                           const DevState *st, LaunchStream stream, C<R> *G, R half_alpha) {
     if (which == 0 || which == 2 || which == 3) {                       // (x, y) forward / inverse / inverse + g
         const long long planes = 4LL * g.L[2] * g.L[3];
         const int nzt = g.L[2] * g.L[3];
@@ -257,8 +257,8 @@ cudaError_t launch_fft_reg(int which, const Geom &g, C<R> *W, const R *twiddle_t
 }
 
 template cudaError_t launch_fft_reg<float>(int, const Geom &, C<float> *, const float *, const float *, float,
-                                           const DevState *, cudaStream_t, C<float> *, float);
+                                           const DevState *, LaunchStream, C<float> *, float);
 template cudaError_t launch_fft_reg<double>(int, const Geom &, C<double> *, const double *, const double *, double,
-                                            const DevState *, cudaStream_t, C<double> *, double);
+                                            const DevState *, LaunchStream, C<double> *, double);
 
 }  // namespace lgf

@@ -225,7 +225,7 @@ bool fft_reg2_gout(const Geom &g, int prec) {
 }
 
 template <class R, int L, int MODE, int P, bool GOUT>
-static cudaError_t launch_xy2_as(const Geom &g, C<R> *W, const DevState *st, cudaStream_t stream, C<R> *G, R half_alpha) {
+static cudaError_t launch_xy2_as(const Geom &g, C<R> *W, const DevState *st, LaunchStream stream, C<R> *G, R half_alpha) {
     constexpr size_t SM = sizeof(C<R>) * P * L * (L | 1);
     const long long planes = 4LL * g.L[2] * g.L[3];
     auto kern = k_fftr2_xy<R, L, MODE, P, GOUT>;
@@ -237,7 +237,7 @@ static cudaError_t launch_xy2_as(const Geom &g, C<R> *W, const DevState *st, cud
                       half_alpha);
 }
 template <class R, int L>
-static cudaError_t launch_xy2(int which, const Geom &g, C<R> *W, const DevState *st, cudaStream_t stream, C<R> *G,
+static cudaError_t launch_xy2(int which, const Geom &g, C<R> *W, const DevState *st, LaunchStream stream, C<R> *G,
                               R half_alpha) {
     constexpr int P = Xy2Cfg<R, L>::P, PF = Xy2Cfg<R, L>::PF;
     if (which == 0) return launch_xy2_as<R, L, FFT_FWD, PF, false>(g, W, st, stream, G, half_alpha);
@@ -247,7 +247,7 @@ static cudaError_t launch_xy2(int which, const Geom &g, C<R> *W, const DevState 
 }
 
 template <class R, int LZ, int LT>
-static cudaError_t launch_zt2(const Geom &g, C<R> *W, const R *p2tab, R scale, const DevState *st, cudaStream_t stream) {
+static cudaError_t launch_zt2(const Geom &g, C<R> *W, const R *p2tab, R scale, const DevState *st, LaunchStream stream) {
     constexpr int XC = Zt2Cfg<R, LZ, LT>::XC;
     using Sh = Zt2Shape<R, LZ, LT, XC>;
     auto kern = k_fftr2_zt<R, LZ, LT, XC>;
@@ -262,7 +262,7 @@ static cudaError_t launch_zt2(const Geom &g, C<R> *W, const R *p2tab, R scale, c
 // which: 0 = (x, y) forward, 1 = (z, t) forward + scale + inverse, 2 = (x, y) inverse, 3 = (x, y) inverse + g
 template <class R>
 cudaError_t launch_fft_reg2(int which, const Geom &g, C<R> *W, const R *p2tab, R scale, const DevState *st,
-                            cudaStream_t stream, C<R> *G, R half_alpha) {
+                            LaunchStream stream, C<R> *G, R half_alpha) {
     if (which == 1) {
 #define LGF_GO(A, B) if (g.L[2] == A && g.L[3] == B) return launch_zt2<R, A, B>(g, W, p2tab, scale, st, stream);
         LGF_REG2_ZT(LGF_GO)
@@ -276,8 +276,8 @@ cudaError_t launch_fft_reg2(int which, const Geom &g, C<R> *W, const R *p2tab, R
 }
 
 template cudaError_t launch_fft_reg2<float>(int, const Geom &, C<float> *, const float *, float, const DevState *,
-                                            cudaStream_t, C<float> *, float);
+                                            LaunchStream, C<float> *, float);
 template cudaError_t launch_fft_reg2<double>(int, const Geom &, C<double> *, const double *, double, const DevState *,
-                                             cudaStream_t, C<double> *, double);
+                                             LaunchStream, C<double> *, double);
 
 }  // namespace lgf

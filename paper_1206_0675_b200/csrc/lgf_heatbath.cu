@@ -220,7 +220,7 @@ unsigned long long heatbath_key(unsigned long long seed) {
 
 template <class R>
 cudaError_t launch_heatbath(int nr, LinkPair<R> links, const Geom &g, const DevState *st, double beta,
-                            unsigned long long key, unsigned long long sweep, int mu, int parity, cudaStream_t stream,
+                            unsigned long long key, unsigned long long sweep, int mu, int parity, LaunchStream stream,
                             bool overrelax, int order_tz) {
     const int nb = (int)((g.V / 2 + HB_THREADS - 1) / HB_THREADS);
     // z-planes per (z, t) tile: automatic = plain order unless one t slice of a class pass's traffic (every link
@@ -247,14 +247,14 @@ cudaError_t launch_heatbath(int nr, LinkPair<R> links, const Geom &g, const DevS
     LGF_HB(2, false);
 #undef LGF_HB
 }
-cudaError_t launch_reset_counters(DevState *st, cudaStream_t stream) {
+cudaError_t launch_reset_counters(DevState *st, LaunchStream stream) {
     k_reset_counters<<<1, 1, 0, stream>>>(st);
     return cudaGetLastError();
 }
 
 template cudaError_t launch_heatbath<float>(int, LinkPair<float>, const Geom &, const DevState *, double,
-                                            unsigned long long, unsigned long long, int, int, cudaStream_t, bool, int);
+                                            unsigned long long, unsigned long long, int, int, LaunchStream, bool, int);
 template cudaError_t launch_heatbath<double>(int, LinkPair<double>, const Geom &, const DevState *, double,
-                                             unsigned long long, unsigned long long, int, int, cudaStream_t, bool, int);
+                                             unsigned long long, unsigned long long, int, int, LaunchStream, bool, int);
 
 }  // namespace lgf

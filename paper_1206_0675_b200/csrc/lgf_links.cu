@@ -20,9 +20,9 @@ constexpr int SWEEP_THREADS = 128;
 template <class R, int NR>
 __global__ void __launch_bounds__(SITE_THREADS) k_delta(LinkPair<R> lp, C<R> *__restrict__ W, Geom g,
                                                          double *__restrict__ partial, const int *__restrict__ stop,
-                                                         const DevState *__restrict__ st) {
+                                                         const DevState *__restrict__ st, SweepHalo<R> halo) {
     if (*stop) return;
-    const C<R> *__restrict__ links = lp.buf[st->cur];
+    const C<R> *__restrict__ links = st->cur ? lp.buf[1] : lp.buf[0];
     __shared__ double scratch[SITE_THREADS / 32][2];
     const long long s = (long long)blockIdx.x * SITE_THREADS + threadIdx.x;
     double f = 0.0, t = 0.0;
@@ -37,7 +37,9 @@ __global__ void __launch_bounds__(SITE_THREADS) k_delta(LinkPair<R> lp, C<R> *__
             load_link<R, NR>(links, g.V, mu, s, u);
             retr += u[0].x + u[4].x + u[8].x;                       // eq. 3: Re tr U_mu(x)
             herm_sub(d, algebra_part(u));                           // - A_mu(x)
-            load_link<R, NR>(links, g.V, mu, site_bwd(g, s, c, mu), u);
+            // (t-slab: the slice below the slab lives on another rank; its U_t is in the halo copy, s < S3 there)
+            if (mu == 3 && halo.uhalo && c[3] == 0) load_link<R, NR>(halo.uhalo, g.S[3], 0, s, u);
+            else load_link<R, NR>(links, g.V, mu, site_bwd(g, s, c, mu), u);
             herm_add(d, algebra_part(u));                           // + A_mu(x - mu)      (eq. 5)
         }
         store_herm(W, g.V, s, d);
@@ -67,24 +69,6 @@ __global__ void __launch_bounds__(SITE_THREADS) k_gbuild(const C<R> *__restrict_
     for (int e = 0; e < 6; e++) G[(long long)e * g.V + s] = gx[e];
 }
 
-template <class R>
-__device__ __forceinline__ void load_g(const C<R> *__restrict__ G, long long V, long long s, C<R> (&gx)[9]) {
-#pragma unroll
-    for (int e = 0; e < 6; e++) gx[e] = G[(long long)e * V + s];
-    reconstruct_row2(gx);
-}
-
-// out = a * b * c^dag as it will be seen by whoever loads the stored link later: with 12-real storage
-// only rows 0 and 1 are computed and row 2 is rebuilt from them (eq. 8), exactly as load_link does.
-template <int NR, class R>
-__device__ __forceinline__ void transform_link(const C<R> (&a)[9], const C<R> (&b)[9], const C<R> (&c)[9],
-                                               C<R> (&out)[9]) {
-    C<R> t[9];
-    mat_mul<NR>(a, b, t);
-    mat_mul_dag<NR>(t, c, out);
-    if constexpr (NR == 2) reconstruct_row2(out);
-}
-
 __device__ __forceinline__ void finalize_tail(double f, double t, long long V, double tol, int after_sweep, int record,
                                               DevState *st, double *__restrict__ hist, long long hist_cap) {
     const double F = f / (12.0 * (double)V);          // eq. 3: 1 / (4 N_c V)
@@ -102,43 +86,6 @@ __device__ __forceinline__ void finalize_tail(double f, double t, long long V, d
         if (!(theta == theta) || theta > 1e300) { st->done = 1; st->nan = 1; }
         else if (theta < tol) st->done = 1;           // Alg. 1 line 2: loop while theta >= eps
     }
-}
-
-// Order in which the CTAs of the sweep walk the lattice.  With the plain order (block b = sites
-// 128 b .. 128 b + 127) the t-backward neighbour of a site was touched a whole t slice earlier: 43 MB of
-// traffic at 32^3, 340 MB at 64^3 -- beyond L2, so U_t(x - t), g(x - t) and g(x) come from DRAM a second
-// time (17 GB read instead of 11 at 64^4).  The tiled order walks (z, t) tiles of TZ z-planes: inside a
-// tile t runs slower than z, so the t-neighbour is only TZ (x, y) planes of traffic away.
-//   enumeration b' -> bxy = b' % nxy, zi = (b' / nxy) % TZ, t = (b' / (nxy TZ)) % Lt, ztile = b' / (nxy TZ Lt)
-//   block base  = bxy + nxy * ((ztile TZ + zi) + Lz t)
-struct BlockOrder {
-    int nxy;      // CTAs per (x, y) plane; 0 = plain order
-    int tz, Lz, Lt;
-};
-__device__ __forceinline__ long long block_base(const BlockOrder &bo, unsigned int b) {
-    if (bo.nxy == 0) return b;
-    const unsigned int bxy = b % bo.nxy; unsigned int r = b / bo.nxy;
-    const unsigned int zi = r % bo.tz; r /= bo.tz;
-    const unsigned int t = r % bo.Lt, ztile = r / bo.Lt;
-    return (long long)bxy + (long long)bo.nxy * ((ztile * bo.tz + zi) + (long long)bo.Lz * t);
-}
-
-// Opt-in (lgf_tune "reunit_every"): put a freshly transformed link back onto SU(3) -- Gram-Schmidt on rows 0, 1,
-// row 2 = (row0 x row1)^* (eq. 8).  The method as the paper states it never does this (R13), and in
-// fp64 it need not; in fp32 the links of a run of thousands of iterations drift far enough to move the
-// gauge-invariant plaquette in the fourth digit.  Done inside the sweep, on every copy of the new link it
-// computes, so Delta, F and theta stay those of the links that are stored and no extra pass is needed.
-template <class R>
-__device__ __forceinline__ void project_su3(C<R> (&u)[9]) {
-    const R ia = (R)1 / sqrt(norm2(u[0]) + norm2(u[1]) + norm2(u[2]));
-    u[0] = ia * u[0]; u[1] = ia * u[1]; u[2] = ia * u[2];
-    C<R> ab = mulc(u[3], u[0]);
-    ab = ab + mulc(u[4], u[1]);
-    ab = ab + mulc(u[5], u[2]);
-    u[3] = u[3] - ab * u[0]; u[4] = u[4] - ab * u[1]; u[5] = u[5] - ab * u[2];
-    const R ib = (R)1 / sqrt(norm2(u[3]) + norm2(u[4]) + norm2(u[5]));
-    u[3] = ib * u[3]; u[4] = ib * u[4]; u[5] = ib * u[5];
-    reconstruct_row2(u);
 }
 
 template <class R>
@@ -180,7 +127,7 @@ __device__ __forceinline__ void prefetch_l2_bulk(const void *p, unsigned bytes) 
 template <class R, int NR, bool REUNIT, bool SHARE, int MINB>
 __global__ void __launch_bounds__(SWEEP_THREADS, MINB)
     k_sweep(LinkPair<R> lp, const C<R> *__restrict__ G, C<R> *__restrict__ W, Geom g, double *__restrict__ partial,
-            const DevState *__restrict__ st, BlockOrder bo, int ahead) {
+            const DevState *__restrict__ st, BlockOrder bo, int ahead, SweepHalo<R> halo) {
     pdl_enter();
     if (st->done) return;
     const int cur = st->cur;
@@ -213,7 +160,9 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB)
     auto own = [&](int mu) {
         C<R> u[9], gn[9], p[9];
         load_link<R, NR>(src, g.V, mu, s, u);
-        load_g(G, g.V, site_fwd(g, s, c, mu), gn);
+        // (t-slab: g of the slice above the slab comes from the neighbour's halo copy)
+        if (mu == 3 && halo.ghi && c[3] == g.L[3] - 1) load_g(halo.ghi, g.S[3], s - g.S[3] * (long long)(g.L[3] - 1), gn);
+        else load_g(G, g.V, site_fwd(g, s, c, mu), gn);
         transform_link<NR>(gx, u, gn, p);                           // Alg. 1 line 14, eq. 2
         if constexpr (REUNIT) project_su3(p);
         store_link<R, NR>(dst, g.V, mu, s, p);
@@ -225,10 +174,19 @@ __global__ void __launch_bounds__(SWEEP_THREADS, MINB)
     // + A'_mu(x - mu): the backward neighbour's new link recomputed (its inputs are L1 / L2 hits)
     auto bwd = [&](int mu, long long sb) {
         C<R> u[9], gn[9], p[9];
-        load_link<R, NR>(src, g.V, mu, sb, u);
-        load_g(G, g.V, sb, gn);
+        // (t-slab: the slice below lives on another rank -- its old U_t and its g are in the halo copies, and the
+        // new U_t is stored back, so that the halo copy stays the neighbour's current link without another exchange)
+        const bool below = mu == 3 && halo.uhalo && c[3] == 0;
+        if (below) {
+            load_link<R, NR>(halo.uhalo, g.S[3], 0, s, u);          // s < S3 here: the (x, y, z) index
+            load_g(halo.glo, g.S[3], s, gn);
+        } else {
+            load_link<R, NR>(src, g.V, mu, sb, u);
+            load_g(G, g.V, sb, gn);
+        }
         transform_link<NR>(gn, u, gx, p);
         if constexpr (REUNIT) project_su3(p);                       // the same link the neighbour stores
+        if (below) store_link<R, NR>(halo.uhalo, g.S[3], 0, s, p);
         herm_add(d, algebra_part(p));                               // eq. 5
     };
     if (live) {
@@ -503,21 +461,21 @@ static inline int site_blocks(const Geom &g) { return (int)((g.V + SITE_THREADS 
 
 template <class R>
 cudaError_t launch_delta(int nr, LinkPair<R> links, C<R> *W, const Geom &g, double *partial, int *nblocks,
-                         const int *stop, const DevState *st, cudaStream_t stream) {
+                         const int *stop, const DevState *st, LaunchStream stream, const SweepHalo<R> &halo) {
     const int nb = site_blocks(g);
     *nblocks = nb;
-    if (nr == 3) k_delta<R, 3><<<nb, SITE_THREADS, 0, stream>>>(links, W, g, partial, stop, st);
-    else k_delta<R, 2><<<nb, SITE_THREADS, 0, stream>>>(links, W, g, partial, stop, st);
+    if (nr == 3) k_delta<R, 3><<<nb, SITE_THREADS, 0, stream>>>(links, W, g, partial, stop, st, halo);
+    else k_delta<R, 2><<<nb, SITE_THREADS, 0, stream>>>(links, W, g, partial, stop, st, halo);
     return cudaGetLastError();
 }
 template <class R>
-cudaError_t launch_gbuild(const C<R> *W, C<R> *G, const Geom &g, R half_alpha, const DevState *st, cudaStream_t stream) {
+cudaError_t launch_gbuild(const C<R> *W, C<R> *G, const Geom &g, R half_alpha, const DevState *st, LaunchStream stream) {
     return launch_pdl(k_gbuild<R>, dim3(site_blocks(g)), dim3(SITE_THREADS), 0, stream, W, G, g, half_alpha, st);
 }
 template <class R>
 cudaError_t launch_sweep(int nr, LinkPair<R> links, const C<R> *G, C<R> *W, const Geom &g, double *partial,
-                         int *nblocks, const DevState *st, cudaStream_t stream, int order_tz, bool reunit, int share_mode,
-                         int ahead, int minb) {
+                         int *nblocks, const DevState *st, LaunchStream stream, int order_tz, bool reunit, int share_mode,
+                         int ahead, int minb, const SweepHalo<R> &halo) {
     const int nb = (int)((g.V + SWEEP_THREADS - 1) / SWEEP_THREADS);
     *nblocks = nb;
     // (z, t)-tiled block order when the (x, y) plane is a whole number of CTAs; TZ: about 24 MB of traffic
@@ -543,8 +501,8 @@ cudaError_t launch_sweep(int nr, LinkPair<R> links, const C<R> *G, C<R> *W, cons
         if (tz > 1 && g.L[2] % tz == 0) { bo.nxy = (int)(plane / SWEEP_THREADS); bo.tz = tz; }
     }
 #define LGF_SWK(RU, SH, MB)                                                                              \
-    if (nr == 3) return launch_pdl(k_sweep<R, 3, RU, SH, MB>, dim3(nb), dim3(SWEEP_THREADS), 0, stream, links, G, W, g, partial, st, bo, ahead); \
-    else return launch_pdl(k_sweep<R, 2, RU, SH, MB>, dim3(nb), dim3(SWEEP_THREADS), 0, stream, links, G, W, g, partial, st, bo, ahead);
+    if (nr == 3) return launch_pdl(k_sweep<R, 3, RU, SH, MB>, dim3(nb), dim3(SWEEP_THREADS), 0, stream, links, G, W, g, partial, st, bo, ahead, halo); \
+    else return launch_pdl(k_sweep<R, 2, RU, SH, MB>, dim3(nb), dim3(SWEEP_THREADS), 0, stream, links, G, W, g, partial, st, bo, ahead, halo);
     if (minb == 2) {
         if (share) { LGF_SWK(false, true, 2) }
         else { LGF_SWK(false, false, 2) }
@@ -558,7 +516,7 @@ cudaError_t launch_sweep(int nr, LinkPair<R> links, const C<R> *G, C<R> *W, cons
 }
 template <class R>
 cudaError_t launch_plaquette(int nr, LinkPair<R> links, const Geom &g, double *partial, int *nblocks,
-                             const DevState *st, cudaStream_t stream) {
+                             const DevState *st, LaunchStream stream) {
     const int nb = site_blocks(g);
     *nblocks = nb;
     if (nr == 3) k_plaquette<R, 3><<<nb, SITE_THREADS, 0, stream>>>(links, g, partial, st);
@@ -566,7 +524,7 @@ cudaError_t launch_plaquette(int nr, LinkPair<R> links, const Geom &g, double *p
     return cudaGetLastError();
 }
 template <class R>
-cudaError_t launch_convert_in(int nr, const R *canon, C<R> *links0, const Geom &g, cudaStream_t stream) {
+cudaError_t launch_convert_in(int nr, const R *canon, C<R> *links0, const Geom &g, LaunchStream stream) {
     const int nb = site_blocks(g);
     if (nr == 3) k_convert_in<R, 3><<<nb, SITE_THREADS, 0, stream>>>(canon, links0, g);
     else k_convert_in<R, 2><<<nb, SITE_THREADS, 0, stream>>>(canon, links0, g);
@@ -574,14 +532,14 @@ cudaError_t launch_convert_in(int nr, const R *canon, C<R> *links0, const Geom &
 }
 template <class R>
 cudaError_t launch_convert_out(int nr, LinkPair<R> links, R *canon, const Geom &g, const DevState *st,
-                               cudaStream_t stream) {
+                               LaunchStream stream) {
     const int nb = site_blocks(g);
     if (nr == 3) k_convert_out<R, 3><<<nb, SITE_THREADS, 0, stream>>>(links, canon, g, st);
     else k_convert_out<R, 2><<<nb, SITE_THREADS, 0, stream>>>(links, canon, g, st);
     return cudaGetLastError();
 }
 template <class R>
-cudaError_t launch_gacc(int op, const C<R> *G, C<R> *A, R *out, const Geom &g, const DevState *st, cudaStream_t stream) {
+cudaError_t launch_gacc(int op, const C<R> *G, C<R> *A, R *out, const Geom &g, const DevState *st, LaunchStream stream) {
     const int nb = site_blocks(g);
     if (op == 3) k_g_from_canonical<R><<<nb, SITE_THREADS, 0, stream>>>(out, A, g);      // out = input field, A = G
     else if (op == 0) k_gacc_identity<R><<<nb, SITE_THREADS, 0, stream>>>(A, g);
@@ -590,63 +548,63 @@ cudaError_t launch_gacc(int op, const C<R> *G, C<R> *A, R *out, const Geom &g, c
     return cudaGetLastError();
 }
 template <class R>
-cudaError_t launch_algebra(int nr, LinkPair<R> links, C<R> *W, const Geom &g, int mu, const DevState *st, cudaStream_t stream) {
+cudaError_t launch_algebra(int nr, LinkPair<R> links, C<R> *W, const Geom &g, int mu, const DevState *st, LaunchStream stream) {
     const int nb = site_blocks(g);
     if (nr == 3) k_algebra<R, 3><<<nb, SITE_THREADS, 0, stream>>>(links, W, g, mu, st);
     else k_algebra<R, 2><<<nb, SITE_THREADS, 0, stream>>>(links, W, g, mu, st);
     return cudaGetLastError();
 }
 template <class R>
-cudaError_t launch_gluon_unpack(const C<R> *W, R *out, const Geom &g, const int N1[4], const int N2[4], cudaStream_t stream) {
+cudaError_t launch_gluon_unpack(const C<R> *W, R *out, const Geom &g, const int N1[4], const int N2[4], LaunchStream stream) {
     AxisPerm pm;
     for (int mu = 0; mu < 4; mu++) { pm.N1[mu] = N1[mu]; pm.N2[mu] = N2[mu]; }
     k_gluon_unpack<R><<<site_blocks(g), SITE_THREADS, 0, stream>>>(W, out, g, pm);
     return cudaGetLastError();
 }
 template <class R>
-cudaError_t launch_field_get(const C<R> *W, R *field, const Geom &g, cudaStream_t stream) {
+cudaError_t launch_field_get(const C<R> *W, R *field, const Geom &g, LaunchStream stream) {
     k_field_get<R><<<site_blocks(g), SITE_THREADS, 0, stream>>>(W, field, g);
     return cudaGetLastError();
 }
 template <class R>
-cudaError_t launch_field_set(C<R> *W, const R *field, const Geom &g, cudaStream_t stream) {
+cudaError_t launch_field_set(C<R> *W, const R *field, const Geom &g, LaunchStream stream) {
     k_field_set<R><<<site_blocks(g), SITE_THREADS, 0, stream>>>(W, field, g);
     return cudaGetLastError();
 }
 
 cudaError_t launch_finalize(const double *partial, int nblocks, long long V, double tol, int after_sweep, int record,
-                            DevState *st, double *hist, long long hist_cap, cudaStream_t stream) {
+                            DevState *st, double *hist, long long hist_cap, LaunchStream stream) {
     return launch_pdl(k_finalize, dim3(1), dim3(1024), 0, stream, partial, nblocks, V, tol, after_sweep, record, st, hist,
                       hist_cap);
 }
-cudaError_t launch_sum1(const double *partial, int nblocks, double norm, double *out, cudaStream_t stream) {
+cudaError_t launch_sum1(const double *partial, int nblocks, double norm, double *out, LaunchStream stream) {
     k_sum1<<<1, 1024, 0, stream>>>(partial, nblocks, norm, out);
     return cudaGetLastError();
 }
-cudaError_t launch_reset_state(DevState *st, cudaStream_t stream) {
+cudaError_t launch_reset_state(DevState *st, LaunchStream stream) {
     k_reset_state<<<1, 1, 0, stream>>>(st);
     return cudaGetLastError();
 }
-cudaError_t launch_clear_done(DevState *st, cudaStream_t stream) {
+cudaError_t launch_clear_done(DevState *st, LaunchStream stream) {
     k_clear_done<<<1, 1, 0, stream>>>(st);
     return cudaGetLastError();
 }
 
 #define LGF_INST(R)                                                                                                   \
     template cudaError_t launch_delta<R>(int, LinkPair<R>, C<R> *, const Geom &, double *, int *, const int *,        \
-                                         const DevState *, cudaStream_t);                                             \
-    template cudaError_t launch_gbuild<R>(const C<R> *, C<R> *, const Geom &, R, const DevState *, cudaStream_t);     \
+                                         const DevState *, LaunchStream, const SweepHalo<R> &);                       \
+    template cudaError_t launch_gbuild<R>(const C<R> *, C<R> *, const Geom &, R, const DevState *, LaunchStream);     \
     template cudaError_t launch_sweep<R>(int, LinkPair<R>, const C<R> *, C<R> *, const Geom &, double *, int *,       \
-                                         const DevState *, cudaStream_t, int, bool, int, int, int);                                   \
+                                         const DevState *, LaunchStream, int, bool, int, int, int, const SweepHalo<R> &);                                   \
     template cudaError_t launch_plaquette<R>(int, LinkPair<R>, const Geom &, double *, int *, const DevState *,       \
-                                             cudaStream_t);                                                           \
-    template cudaError_t launch_convert_in<R>(int, const R *, C<R> *, const Geom &, cudaStream_t);                    \
-    template cudaError_t launch_convert_out<R>(int, LinkPair<R>, R *, const Geom &, const DevState *, cudaStream_t);  \
-    template cudaError_t launch_gacc<R>(int, const C<R> *, C<R> *, R *, const Geom &, const DevState *, cudaStream_t); \
-    template cudaError_t launch_algebra<R>(int, LinkPair<R>, C<R> *, const Geom &, int, const DevState *, cudaStream_t); \
-    template cudaError_t launch_gluon_unpack<R>(const C<R> *, R *, const Geom &, const int[4], const int[4], cudaStream_t); \
-    template cudaError_t launch_field_get<R>(const C<R> *, R *, const Geom &, cudaStream_t);                          \
-    template cudaError_t launch_field_set<R>(C<R> *, const R *, const Geom &, cudaStream_t);
+                                             LaunchStream);                                                           \
+    template cudaError_t launch_convert_in<R>(int, const R *, C<R> *, const Geom &, LaunchStream);                    \
+    template cudaError_t launch_convert_out<R>(int, LinkPair<R>, R *, const Geom &, const DevState *, LaunchStream);  \
+    template cudaError_t launch_gacc<R>(int, const C<R> *, C<R> *, R *, const Geom &, const DevState *, LaunchStream); \
+    template cudaError_t launch_algebra<R>(int, LinkPair<R>, C<R> *, const Geom &, int, const DevState *, LaunchStream); \
+    template cudaError_t launch_gluon_unpack<R>(const C<R> *, R *, const Geom &, const int[4], const int[4], LaunchStream); \
+    template cudaError_t launch_field_get<R>(const C<R> *, R *, const Geom &, LaunchStream);                          \
+    template cudaError_t launch_field_set<R>(C<R> *, const R *, const Geom &, LaunchStream);
 LGF_INST(float)
 LGF_INST(double)
 

@@ -23,19 +23,26 @@ __device__ __forceinline__ void pdl_enter() {
 #endif
 }
 
-extern int g_pdl_enabled;      // lgf_api.cu: 1 unless switched off (lgf_tune "pdl", process-wide: a launch attribute)
+// A stream plus the context's programmatic-dependent-launch setting (lgf_tune "pdl", per context).  Converts from
+// and to cudaStream_t, so launchers that do not care keep passing a plain stream (dependent launch allowed).
+struct LaunchStream {
+    cudaStream_t s;
+    bool pdl;
+    LaunchStream(cudaStream_t stream = nullptr, bool allow = true) : s(stream), pdl(allow) {}
+    operator cudaStream_t() const { return s; }
+};
 
 // kernel<<<grid, block, smem, stream>>>(args...) with the attribute that lets it start while its predecessor drains
 template <class... KArgs, class... Args>
-cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t stream, Args... args) {
+cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, LaunchStream stream, Args... args) {
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = grid;
     cfg.blockDim = block;
     cfg.dynamicSmemBytes = smem;
-    cfg.stream = stream;
+    cfg.stream = stream.s;
     cudaLaunchAttribute attr;
     attr.id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    attr.val.programmaticStreamSerializationAllowed = g_pdl_enabled ? 1 : 0;
+    attr.val.programmaticStreamSerializationAllowed = stream.pdl ? 1 : 0;
     cfg.attrs = &attr;
     cfg.numAttrs = 1;
     return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);

@@ -281,7 +281,7 @@ __global__ void __launch_bounds__(2 * LINE2_LINES) k_slab_fft_line2(const C<R> *
 }
 template <class R>
 static cudaError_t launch_line2(int L, int mode, const C<R> *src, C<R> *dst, const LineAddr &as, const LineAddr &ad,
-                                dim3 grid, int Lx, const R *p2tab, R scale, cudaStream_t stream) {
+                                dim3 grid, int Lx, const R *p2tab, R scale, LaunchStream stream) {
 #define LGF_GO(LEN)                                                                                              \
     if (L == LEN) {                                                                                              \
         if (mode == FFT_FWD) k_slab_fft_line2<R, LEN, FFT_FWD><<<grid, 2 * LINE2_LINES, 0, stream>>>(src, dst, as, ad, Lx, p2tab, scale); \
@@ -296,7 +296,7 @@ static cudaError_t launch_line2(int L, int mode, const C<R> *src, C<R> *dst, con
 
 template <class R, int L>
 static cudaError_t launch_line_L(int mode, const C<R> *src, C<R> *dst, const LineAddr &as, const LineAddr &ad, int nlo,
-                                 dim3 grid, int Lx, const R *twiddle, const R *p2tab, R scale, cudaStream_t stream) {
+                                 dim3 grid, int Lx, const R *twiddle, const R *p2tab, R scale, LaunchStream stream) {
     const size_t smem = (64 + (size_t)L * nlo) * sizeof(C<R>);
     const C<R> *tw = reinterpret_cast<const C<R> *>(twiddle);
     auto go = [&](auto kern) {
@@ -313,7 +313,7 @@ static cudaError_t launch_line_L(int mode, const C<R> *src, C<R> *dst, const Lin
 }
 template <class R>
 static cudaError_t launch_line(int L, int mode, const C<R> *src, C<R> *dst, const LineAddr &as, const LineAddr &ad, int nlo,
-                               dim3 grid, int Lx, const R *twiddle, const R *p2tab, R scale, cudaStream_t stream) {
+                               dim3 grid, int Lx, const R *twiddle, const R *p2tab, R scale, LaunchStream stream) {
     switch (L) {
 #define LGF_CASE(LEN) case LEN: return launch_line_L<R, LEN>(mode, src, dst, as, ad, nlo, grid, Lx, twiddle, p2tab, scale, stream);
         LGF_CASE(2) LGF_CASE(3) LGF_CASE(4) LGF_CASE(6) LGF_CASE(8) LGF_CASE(12) LGF_CASE(16) LGF_CASE(24)

@@ -3,6 +3,7 @@
 #pragma once
 #include <cuda_runtime.h>
 #include "lgf_su3.cuh"
+#include "lgf_pdl.cuh"
 
 namespace lgf {
 
@@ -58,17 +59,26 @@ struct AxisPass {
     size_t smem;
 };
 
+// Where g and U_t across the ends of the t range come from: all null on one GPU (periodic inside the buffers);
+// on a t-slab (lgf_slab.cu) the neighbouring ranks' halo copies.  One sweep / Delta kernel serves both paths.
+template <class R>
+struct SweepHalo {
+    const C<R> *ghi = nullptr;   // rows 0, 1 of g on the slice above the slab, C<R>[6][S3]
+    const C<R> *glo = nullptr;   // ... on the slice below
+    C<R> *uhalo = nullptr;       // U_t of the slice below, C<R>[3 NR][S3]; the sweep stores its new value back
+};
+
 // launchers implemented in the .cu files (R = float / double)
 template <class R>
 cudaError_t launch_fft_pass(const AxisPass &p, C<R> *W, const Geom &g, const R *const twiddle[4] /*[2*64] per axis*/,
                             const R *p2tab /*[4][64] permuted 4 sin^2*/, R scale, const DevState *st,
-                            cudaStream_t stream);
+                            LaunchStream stream);
 // register-line fast path (lgf_fft_reg.cu): available for this lattice?  is the t axis left in natural k order?
 bool fft_reg_supported(const Geom &g);
 bool fft_reg_t_natural(const Geom &g);
 template <class R>
 cudaError_t launch_fft_reg(int which, const Geom &g, C<R> *W, const R *twiddle_t, const R *p2tab, R scale,
-                           const DevState *st, cudaStream_t stream, C<R> *G = nullptr, R half_alpha = 0);
+                           const DevState *st, LaunchStream stream, C<R> *G = nullptr, R half_alpha = 0);
 // two-threads-per-line register sweeps (lgf_fft_reg2.cu)
 bool fft_reg2_supported(const Geom &g);
 bool fft_reg2_gout(const Geom &g, int prec);
@@ -76,60 +86,62 @@ bool fft_reg2_xy_supported(const Geom &g);      // the (x, y) sweeps alone, any 
 bool fft_reg2_xy_gout(const Geom &g, int prec);
 template <class R>
 cudaError_t launch_fft_reg2(int which, const Geom &g, C<R> *W, const R *p2tab, R scale, const DevState *st,
-                            cudaStream_t stream, C<R> *G, R half_alpha);
+                            LaunchStream stream, C<R> *G, R half_alpha);
 // true if a PASS_XY (first two axes) / PASS_ZT (last two axes) kernel is instantiated for these lengths
 bool fft_pair_supported(int kind, int La, int Lb);
 
 template <class R>
 cudaError_t launch_delta(int nr, LinkPair<R> links, C<R> *W, const Geom &g, double *partial, int *nblocks,
-                         const int *stop, const DevState *st, cudaStream_t stream);
+                         const int *stop, const DevState *st, LaunchStream stream,
+                         const SweepHalo<R> &halo = SweepHalo<R>());
 template <class R>
-cudaError_t launch_gbuild(const C<R> *W, C<R> *G, const Geom &g, R half_alpha, const DevState *st, cudaStream_t stream);
+cudaError_t launch_gbuild(const C<R> *W, C<R> *G, const Geom &g, R half_alpha, const DevState *st, LaunchStream stream);
 template <class R>
 cudaError_t launch_sweep(int nr, LinkPair<R> links, const C<R> *G, C<R> *W, const Geom &g, double *partial,
-                         int *nblocks, const DevState *st, cudaStream_t stream, int order_tz /* 0 auto, 1 plain */,
+                         int *nblocks, const DevState *st, LaunchStream stream, int order_tz /* 0 auto, 1 plain */,
                          bool reunit /* project every new link onto SU(3) */,
                          int share_mode /* A'_x, A'_y through shared memory: 1 / 0 / -1 = where it measured faster */,
                          int ahead /* L2 bulk prefetch of the tile `ahead` CTAs later (0 = none) */,
-                         int minb /* resident CTAs per SM the register allocation allows: 3 (168 registers) or 2 (255) */);
+                         int minb /* resident CTAs per SM the register allocation allows: 3 (168 registers) or 2 (255) */,
+                         const SweepHalo<R> &halo = SweepHalo<R>());
 template <class R>
 cudaError_t launch_plaquette(int nr, LinkPair<R> links, const Geom &g, double *partial, int *nblocks,
-                             const DevState *st, cudaStream_t stream);
+                             const DevState *st, LaunchStream stream);
 template <class R>
-cudaError_t launch_convert_in(int nr, const R *canon, C<R> *links0, const Geom &g, cudaStream_t stream);
+cudaError_t launch_convert_in(int nr, const R *canon, C<R> *links0, const Geom &g, LaunchStream stream);
 template <class R>
 cudaError_t launch_convert_out(int nr, LinkPair<R> links, R *canon, const Geom &g, const DevState *st,
-                               cudaStream_t stream);
+                               LaunchStream stream);
 // accumulated gauge transformation: op 0 = set to identity, 1 = Gacc <- g Gacc, 2 = copy out (canonical [s][3][3]),
 // 3 = (A = G, out = canonical input field) rows 0, 1 of the SU(3) projection of a given transformation into G
 template <class R>
-cudaError_t launch_gacc(int op, const C<R> *G, C<R> *A, R *out, const Geom &g, const DevState *st, cudaStream_t stream);
+cudaError_t launch_gacc(int op, const C<R> *G, C<R> *A, R *out, const Geom &g, const DevState *st, LaunchStream stream);
 // gluon field: W <- packed A_mu(x) of one direction; unpack of its forward transform into natural-order 3 x 3 A_mu(k)
 template <class R>
-cudaError_t launch_algebra(int nr, LinkPair<R> links, C<R> *W, const Geom &g, int mu, const DevState *st, cudaStream_t stream);
+cudaError_t launch_algebra(int nr, LinkPair<R> links, C<R> *W, const Geom &g, int mu, const DevState *st, LaunchStream stream);
 template <class R>
-cudaError_t launch_gluon_unpack(const C<R> *W, R *out, const Geom &g, const int N1[4], const int N2[4], cudaStream_t stream);
+cudaError_t launch_gluon_unpack(const C<R> *W, R *out, const Geom &g, const int N1[4], const int N2[4], LaunchStream stream);
 template <class R>
-cudaError_t launch_field_get(const C<R> *W, R *field, const Geom &g, cudaStream_t stream);
+cudaError_t launch_field_get(const C<R> *W, R *field, const Geom &g, LaunchStream stream);
 template <class R>
-cudaError_t launch_field_set(C<R> *W, const R *field, const Geom &g, cudaStream_t stream);
+cudaError_t launch_field_set(C<R> *W, const R *field, const Geom &g, LaunchStream stream);
 
 // thermalisation (lgf_heatbath.cu): one class (mu, parity) of heat-bath sweep number `sweep`
 unsigned long long heatbath_key(unsigned long long seed);
 template <class R>
 cudaError_t launch_heatbath(int nr, LinkPair<R> links, const Geom &g, const DevState *st, double beta,
-                            unsigned long long key, unsigned long long sweep, int mu, int parity, cudaStream_t stream,
+                            unsigned long long key, unsigned long long sweep, int mu, int parity, LaunchStream stream,
                             bool overrelax /* R28: alpha = (V^dag)^2, no random numbers */,
                             int order_tz /* z-planes per (z, t) tile of the thread order: 0 = automatic */);
-cudaError_t launch_reset_counters(DevState *st, cudaStream_t stream);
+cudaError_t launch_reset_counters(DevState *st, LaunchStream stream);
 
 // F / theta finalisation (precision independent)
 // after_sweep: the partial sums come from a sweep (flip `cur`, count the update); record: append (F, theta)
 // to the history and apply the stop test theta < tol
 cudaError_t launch_finalize(const double *partial, int nblocks, long long V, double tol, int after_sweep, int record,
-                            DevState *st, double *hist, long long hist_cap, cudaStream_t stream);
-cudaError_t launch_sum1(const double *partial, int nblocks, double norm, double *out, cudaStream_t stream);
-cudaError_t launch_reset_state(DevState *st, cudaStream_t stream);
-cudaError_t launch_clear_done(DevState *st, cudaStream_t stream);
+                            DevState *st, double *hist, long long hist_cap, LaunchStream stream);
+cudaError_t launch_sum1(const double *partial, int nblocks, double norm, double *out, LaunchStream stream);
+cudaError_t launch_reset_state(DevState *st, LaunchStream stream);
+cudaError_t launch_clear_done(DevState *st, LaunchStream stream);
 
 }  // namespace lgf

@@ -159,6 +159,62 @@ __device__ __forceinline__ void mat_mul_dag(const C<R> (&a)[9], const C<R> (&b)[
         }
 }
 
+// rows 0, 1 of g(x) are stored (G[e][s], e = 0..5); row 2 is (row0 x row1)^* by construction (eq. 8)
+template <class R>
+__device__ __forceinline__ void load_g(const C<R> *__restrict__ G, long long V, long long s, C<R> (&gx)[9]) {
+#pragma unroll
+    for (int e = 0; e < 6; e++) gx[e] = G[(long long)e * V + s];
+    reconstruct_row2(gx);
+}
+
+// out = a * b * c^dag as it will be seen by whoever loads the stored link later: with 12-real storage
+// only rows 0 and 1 are computed and row 2 is rebuilt from them (eq. 8), exactly as load_link does.
+template <int NR, class R>
+__device__ __forceinline__ void transform_link(const C<R> (&a)[9], const C<R> (&b)[9], const C<R> (&c)[9],
+                                               C<R> (&out)[9]) {
+    C<R> t[9];
+    mat_mul<NR>(a, b, t);
+    mat_mul_dag<NR>(t, c, out);
+    if constexpr (NR == 2) reconstruct_row2(out);
+}
+
+// Opt-in (lgf_tune "reunit_every"): put a freshly transformed link back onto SU(3) -- Gram-Schmidt on rows 0, 1,
+// row 2 = (row0 x row1)^* (eq. 8).  The method as the paper states it never does this (R13), and in
+// fp64 it need not; in fp32 the links of a run of thousands of iterations drift far enough to move the
+// gauge-invariant plaquette in the fourth digit.  Done inside the sweep, on every copy of the new link it
+// computes, so Delta, F and theta stay those of the links that are stored and no extra pass is needed.
+template <class R>
+__device__ __forceinline__ void project_su3(C<R> (&u)[9]) {
+    const R ia = (R)1 / sqrt(norm2(u[0]) + norm2(u[1]) + norm2(u[2]));
+    u[0] = ia * u[0]; u[1] = ia * u[1]; u[2] = ia * u[2];
+    C<R> ab = mulc(u[3], u[0]);
+    ab = ab + mulc(u[4], u[1]);
+    ab = ab + mulc(u[5], u[2]);
+    u[3] = u[3] - ab * u[0]; u[4] = u[4] - ab * u[1]; u[5] = u[5] - ab * u[2];
+    const R ib = (R)1 / sqrt(norm2(u[3]) + norm2(u[4]) + norm2(u[5]));
+    u[3] = ib * u[3]; u[4] = ib * u[4]; u[5] = ib * u[5];
+    reconstruct_row2(u);
+}
+
+// Order in which the CTAs of the sweep walk the lattice.  With the plain order (block b = sites
+// 128 b .. 128 b + 127) the t-backward neighbour of a site was touched a whole t slice earlier: 43 MB of
+// traffic at 32^3, 340 MB at 64^3 -- beyond L2, so U_t(x - t), g(x - t) and g(x) come from DRAM a second
+// time (17 GB read instead of 11 at 64^4).  The tiled order walks (z, t) tiles of TZ z-planes: inside a
+// tile t runs slower than z, so the t-neighbour is only TZ (x, y) planes of traffic away.
+//   enumeration b' -> bxy = b' % nxy, zi = (b' / nxy) % TZ, t = (b' / (nxy TZ)) % Lt, ztile = b' / (nxy TZ Lt)
+//   block base  = bxy + nxy * ((ztile TZ + zi) + Lz t)
+struct BlockOrder {
+    int nxy;      // CTAs per (x, y) plane; 0 = plain order
+    int tz, Lz, Lt;
+};
+__device__ __forceinline__ long long block_base(const BlockOrder &bo, unsigned int b) {
+    if (bo.nxy == 0) return b;
+    const unsigned int bxy = b % bo.nxy; unsigned int r = b / bo.nxy;
+    const unsigned int zi = r % bo.tz; r /= bo.tz;
+    const unsigned int t = r % bo.Lt, ztile = r / bo.Lt;
+    return (long long)bxy + (long long)bo.nxy * ((ztile * bo.tz + zi) + (long long)bo.Lz * t);
+}
+
 // ---- lattice geometry ----------------------------------------------------------------------------
 struct Geom {
     int L[4];          // Lx, Ly, Lz, Lt
