@@ -290,6 +290,28 @@ int lgf_slab_update(lgf_slab *ctx);
  * lgf_slab_update -- LGF_ESTATE otherwise.  The sweep itself keeps that halo current from then on, so an iteration
  * of sweeps exchanges 24 reals per boundary site instead of 12 + 18 (or 12 + 12). */
 int lgf_slab_sweep(lgf_slab *ctx, double *d_sums);
+/* Algorithm 1's control on the device (lines 1, 2, 17), the slab twin of what lgf_iterate /
+ * lgf_fix do inside: d_sums (device, 2 doubles) = the sums of lgf_slab_delta / lgf_slab_sweep AFTER the all-reduce
+ * over the ranks.  Computes F = sums[0] / (12 V_global) (eq. 3) and theta = sums[1] / (3 V_global) (eq. 6) into the
+ * context's device-resident state; record != 0: appends (F, theta) to the history and applies the loop test --
+ * theta < tol, or a NaN / Inf theta, sets the `done` flag, after which every iteration kernel of this context
+ * (FFT passes, g-build, update, sweep, the sum of the partial sums, finalize itself) returns at once, so iterations
+ * enqueued past convergence cost nothing and the host needs no per-iteration read-back.  after_sweep != 0: the sums
+ * come from lgf_slab_sweep -- the second link buffer becomes the current one and the update counter advances;
+ * REQUIRED after every lgf_slab_sweep (the sweep itself flips nothing).  Every rank calls it with the same sums, so
+ * every rank takes the same decision.  lgf_slab_delta always runs (it is a measurement). */
+int lgf_slab_finalize(lgf_slab *ctx, const double *d_sums, double tol, int after_sweep, int record);
+/* clears the `done` flag (start of a new iterate / fix) */
+int lgf_slab_clear_done(lgf_slab *ctx);
+/* lgf_slab_poll enqueues an asynchronous copy of the state into pinned host memory and returns at once (at most two
+ * outstanding, LGF_ESTATE beyond); lgf_slab_poll_wait waits for the OLDEST outstanding one and reports what it saw
+ * (any out-pointer may be NULL).  A driver that enqueues a chunk of iterations, polls, enqueues the next chunk and
+ * only then waits for the first look never lets the GPU idle on the host. */
+int lgf_slab_poll(lgf_slab *ctx);
+int lgf_slab_poll_wait(lgf_slab *ctx, int *done, int *nan_seen, long long *n_updates, double *F, double *theta);
+/* the recorded (F, theta) entries, as lgf_history / lgf_history_length; synchronise the stream */
+long long lgf_slab_history_length(lgf_slab *ctx);
+int lgf_slab_history(lgf_slab *ctx, long long first, long long count, double *F, double *theta);
 /* the slab's work field as full 3 x 3 matrices, 18 reals per local site (as lgf_get_field) */
 int lgf_slab_get_field(lgf_slab *ctx, void *d_field);
 long long lgf_slab_launch_count(const lgf_slab *ctx);

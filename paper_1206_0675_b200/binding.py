@@ -81,6 +81,12 @@ SIGNATURES = {
     "lgf_slab_gbuild": (_i, [_vp, _d]),
     "lgf_slab_update": (_i, [_vp]),
     "lgf_slab_sweep": (_i, [_vp, _vp]),
+    "lgf_slab_finalize": (_i, [_vp, _vp, _d, _i, _i]),
+    "lgf_slab_clear_done": (_i, [_vp]),
+    "lgf_slab_poll": (_i, [_vp]),
+    "lgf_slab_poll_wait": (_i, [_vp, ctypes.POINTER(ctypes.c_int), ctypes.POINTER(ctypes.c_int), _llp, _dp, _dp]),
+    "lgf_slab_history_length": (_ll, [_vp]),
+    "lgf_slab_history": (_i, [_vp, _ll, _ll, _dp, _dp]),
     "lgf_slab_get_field": (_i, [_vp, _vp]),
     "lgf_slab_launch_count": (_ll, [_vp]),
     "lgf_slab_last_error": (ctypes.c_char_p, [_vp]),
@@ -388,6 +394,33 @@ class SlabContext:
 
     def sweep(self, sums):
         self._ck(load().lgf_slab_sweep(self._h, _dev_ptr(sums, LGF_FP64, 2)))
+
+    def finalize(self, sums, tol, after_sweep, record):
+        self._ck(load().lgf_slab_finalize(self._h, _dev_ptr(sums, LGF_FP64, 2), float(tol), int(after_sweep), int(record)))
+
+    def clear_done(self):
+        self._ck(load().lgf_slab_clear_done(self._h))
+
+    def poll(self):
+        self._ck(load().lgf_slab_poll(self._h))
+
+    def poll_wait(self):
+        """(done, nan_seen, n_updates, F, theta) of the oldest outstanding look"""
+        done, nan, n = ctypes.c_int(), ctypes.c_int(), ctypes.c_longlong()
+        F, th = ctypes.c_double(), ctypes.c_double()
+        self._ck(load().lgf_slab_poll_wait(self._h, ctypes.byref(done), ctypes.byref(nan), ctypes.byref(n), ctypes.byref(F),
+                                           ctypes.byref(th)))
+        return bool(done.value), bool(nan.value), int(n.value), F.value, th.value
+
+    def history_length(self):
+        return int(self._ck(load().lgf_slab_history_length(self._h)))
+
+    def history(self, first=0, count=None):
+        if count is None:
+            count = self.history_length() - first
+        F, th = np.zeros(count), np.zeros(count)
+        self._ck(load().lgf_slab_history(self._h, int(first), int(count), F.ctypes.data_as(_dp), th.ctypes.data_as(_dp)))
+        return F, th
 
     def get_field(self, out):
         self._ck(load().lgf_slab_get_field(self._h, _dev_ptr(out, self.precision, self.V * 18)))

@@ -40,42 +40,10 @@ __device__ __forceinline__ void slab_load_g(const C<R> *__restrict__ G, long lon
     reconstruct_row2(gx);
 }
 
-// a1 on a slab.  g = local geometry (Lx, Ly, Lz, T); the backward t neighbour of the first local slice is read
-// from `halo` (U_t of the slice below, C<R>[3 NR][S3]); x, y, z wrap inside the slab.
-template <class R, int NR>
-__global__ void __launch_bounds__(SLAB_THREADS) k_slab_delta(const C<R> *__restrict__ links, const C<R> *__restrict__ halo,
-                                                             C<R> *__restrict__ W, Geom g, double *__restrict__ partial) {
-    __shared__ double scratch[SLAB_THREADS / 32][2];
-    const long long s = (long long)blockIdx.x * SLAB_THREADS + threadIdx.x;
-    double f = 0.0, t = 0.0;
-    if (s < g.V) {
-        int c[4];
-        site_coords(g, s, c);
-        Herm<R> d = herm_zero<R>();
-        R retr = 0;
-#pragma unroll
-        for (int mu = 0; mu < 4; mu++) {
-            C<R> u[9];
-            load_link<R, NR>(links, g.V, mu, s, u);
-            retr += u[0].x + u[4].x + u[8].x;                       // eq. 3: Re tr U_mu(x)
-            herm_sub(d, algebra_part(u));                           // - A_mu(x)
-            if (mu == 3 && c[3] == 0) load_link<R, NR>(halo, g.S[3], 0, s, u);      // s < S3 here: the (x, y, z) index
-            else load_link<R, NR>(links, g.V, mu, site_bwd(g, s, c, mu), u);
-            herm_add(d, algebra_part(u));                           // + A_mu(x - mu)      (eq. 5)
-        }
-        store_herm(W, g.V, s, d);
-        f = (double)retr;
-        t = (double)herm_norm2(d);                                  // eq. 6: tr(Delta Delta^dag)
-    }
-    block_sum2(f, t, scratch);
-    if (threadIdx.x == 0) {
-        partial[2 * blockIdx.x] = f;
-        partial[2 * blockIdx.x + 1] = t;
-    }
-}
-
 // fixed-order sum of the per-block partial sums: out[0] = sum Re tr U, out[1] = sum tr(Delta Delta^dag) of the slab
-__global__ void __launch_bounds__(SLAB_THREADS) k_slab_sum2(const double *__restrict__ partial, int nb, double *__restrict__ out) {
+__global__ void __launch_bounds__(SLAB_THREADS) k_slab_sum2(const double *__restrict__ partial, int nb, double *__restrict__ out,
+                                                            const int *__restrict__ stop) {
+    if (*stop) return;
     __shared__ double scratch[SLAB_THREADS / 32][2];
     double f = 0.0, t = 0.0;
     for (int i = threadIdx.x; i < nb; i += SLAB_THREADS) { f += partial[2 * i]; t += partial[2 * i + 1]; }
@@ -86,8 +54,11 @@ __global__ void __launch_bounds__(SLAB_THREADS) k_slab_sum2(const double *__rest
 // a6 on a slab, in place: U_mu(x) <- g(x) U_mu(x) g(x + mu)^dag (eq. 2, Alg. 1 line 14); g(x + t) of the last local
 // slice comes from `ghalo` (rows 0, 1 of g on the slice above, C<R>[6][S3]).
 template <class R, int NR>
-__global__ void __launch_bounds__(SLAB_THREADS) k_slab_update(C<R> *__restrict__ links, const C<R> *__restrict__ G,
-                                                              const C<R> *__restrict__ ghalo, Geom g) {
+__global__ void __launch_bounds__(SLAB_THREADS) k_slab_update(LinkPair<R> lp, const C<R> *__restrict__ G,
+                                                              const C<R> *__restrict__ ghalo, Geom g,
+                                                              const DevState *__restrict__ st) {
+    if (st->done) return;
+    C<R> *__restrict__ links = st->cur ? lp.buf[1] : lp.buf[0];
     const long long s = (long long)blockIdx.x * SLAB_THREADS + threadIdx.x;
     if (s >= g.V) return;
     int c[4];
@@ -106,71 +77,15 @@ __global__ void __launch_bounds__(SLAB_THREADS) k_slab_update(C<R> *__restrict__
     }
 }
 
-// a6 + a1 fused on a slab (the slab form of k_sweep, lgf_links.cu): every site writes its own new links
-// U'_mu(x) = g(x) U_mu(x) g(x + mu)^dag into the OTHER link buffer and recomputes the new links of its backward
-// neighbours, U'_mu(x - mu) = g(x - mu) U_mu(x - mu) g(x)^dag, for Delta, F, theta of the new configuration
-// (Alg. 1 lines 14, 17) -- the links are read once and written once per iteration, and no separate Delta pass runs.
-// Across the slab boundary it needs g of the slice above (ghi) and of the slice below (glo), and the OLD U_t of the
-// slice below (uhalo); the first local slice also stores the new U_t(x - t) back into uhalo, which thereby stays
-// the neighbour's current U_t without ever being exchanged again.
-constexpr int SLAB_SWEEP_THREADS = 128;
-template <class R, int NR>
-__global__ void __launch_bounds__(SLAB_SWEEP_THREADS, 3)
-    k_slab_sweep(const C<R> *__restrict__ src, C<R> *__restrict__ dst, const C<R> *__restrict__ G,
-                 const C<R> *__restrict__ ghi, const C<R> *__restrict__ glo, C<R> *__restrict__ uhalo,
-                 C<R> *__restrict__ W, Geom g, double *__restrict__ partial) {
-    __shared__ double scratch[SLAB_SWEEP_THREADS / 32][2];
-    const long long s = (long long)blockIdx.x * SLAB_SWEEP_THREADS + threadIdx.x;
-    double f = 0.0, t = 0.0;
-    if (s < g.V) {
-        int c[4];
-        site_coords(g, s, c);
-        const long long S3 = g.S[3];
-        C<R> gx[9];
-        slab_load_g(G, g.V, s, gx);
-        Herm<R> d = herm_zero<R>();
-        R retr = 0;
-#pragma unroll
-        for (int mu = 0; mu < 4; mu++) {
-            {   // the site's own new link
-                C<R> u[9], gn[9], tmp[9], p[9];
-                load_link<R, NR>(src, g.V, mu, s, u);
-                if (mu == 3 && c[3] == g.L[3] - 1) slab_load_g(ghi, S3, s - S3 * (long long)(g.L[3] - 1), gn);
-                else slab_load_g(G, g.V, site_fwd(g, s, c, mu), gn);
-                mat_mul<NR>(gx, u, tmp);
-                mat_mul_dag<NR>(tmp, gn, p);
-                if constexpr (NR == 2) reconstruct_row2(p);        // as whoever loads the stored link will see it (eq. 8)
-                store_link<R, NR>(dst, g.V, mu, s, p);
-                retr += p[0].x + p[4].x + p[8].x;                   // eq. 3 on the new link
-                herm_sub(d, algebra_part(p));                       // - A'_mu(x)
-            }
-            {   // + A'_mu(x - mu): the backward neighbour's new link recomputed
-                C<R> u[9], gb[9], tmp[9], p[9];
-                const bool below = (mu == 3 && c[3] == 0);          // the neighbour is on the rank below
-                if (below) {
-                    load_link<R, NR>(uhalo, S3, 0, s, u);           // s < S3: the (x, y, z) index
-                    slab_load_g(glo, S3, s, gb);
-                } else {
-                    const long long sb = site_bwd(g, s, c, mu);
-                    load_link<R, NR>(src, g.V, mu, sb, u);
-                    slab_load_g(G, g.V, sb, gb);
-                }
-                mat_mul<NR>(gb, u, tmp);
-                mat_mul_dag<NR>(tmp, gx, p);
-                if constexpr (NR == 2) reconstruct_row2(p);
-                if (below) store_link<R, NR>(uhalo, S3, 0, s, p);   // keep the halo copy of U_t current
-                herm_add(d, algebra_part(p));                       // eq. 5
-            }
-        }
-        store_herm(W, g.V, s, d);
-        f = (double)retr;
-        t = (double)herm_norm2(d);                                  // eq. 6
-    }
-    block_sum2(f, t, scratch);
-    if (threadIdx.x == 0) {
-        partial[2 * blockIdx.x] = f;
-        partial[2 * blockIdx.x + 1] = t;
-    }
+// U_t of the slab's last slice, from whichever link buffer is current, into a contiguous send buffer [3 NR][S3]
+template <class R>
+__global__ void __launch_bounds__(SLAB_THREADS) k_slab_pack_ut(LinkPair<R> lp, C<R> *__restrict__ out, long long V, long long S3,
+                                                               int nplanes, long long first, const DevState *__restrict__ st) {
+    const C<R> *__restrict__ links = st->cur ? lp.buf[1] : lp.buf[0];
+    const long long i = (long long)blockIdx.x * SLAB_THREADS + threadIdx.x;
+    if (i >= S3 * nplanes) return;
+    const long long e = i / S3, sx = i % S3;
+    out[i] = links[(3LL * nplanes + e) * V + first + sx];
 }
 
 // Where element n of a line lives: base + (n / D) strideQ + (n % D) strideN.  The all-to-all buffers are ordered
@@ -334,9 +249,9 @@ struct lgf_slab {
     Geom gl{};                   // the slab: (Lx, Ly, Lz, T)
     long long Vglobal = 0;
     cudaStream_t stream = nullptr;
-    void *lbuf[2] = {nullptr, nullptr};   // C<R>[4][3 nr][Vl] each: the fused sweep reads one and writes the other
-    int cur = 0;                 // which one holds the current configuration (`links` below points at it)
-    void *links = nullptr;
+    void *lbuf[2] = {nullptr, nullptr};   // C<R>[4][3 nr][Vl] each: the fused sweep reads one and writes the other;
+                                          // which one is current is st->cur, on the device (k_finalize flips it)
+    int device = 0;              // the CUDA device the buffers live on
     void *uhalo = nullptr;       // C<R>[3 nr][S3]   U_t of the slice below the slab
     void *W = nullptr;           // C<R>[4][Vl]      packed Delta / w, t-slab order
     void *G = nullptr;           // C<R>[6][Vl]
@@ -345,7 +260,12 @@ struct lgf_slab {
     bool uhalo_valid = false;    // uhalo holds U_t of the slice below for the CURRENT configuration
     double *partial = nullptr;
     int nb = 0;
-    DevState *st = nullptr;      // all zero: the kernels shared with the one-GPU path look at st->done
+    DevState *st = nullptr;      // device-resident control block (lgf_state.cuh): done / nan flags, counters, F, theta, cur
+    DevState *h_poll = nullptr;  // pinned: two slots for the asynchronous looks at the state (lgf_slab_poll)
+    cudaEvent_t poll_ev[2] = {nullptr, nullptr};
+    int polls_enq = 0, polls_seen = 0;
+    double *hist = nullptr;      // (F, theta) pairs, device
+    long long hist_cap = 0;
     void *twiddle[4] = {nullptr, nullptr, nullptr, nullptr};
     void *p2tab = nullptr;       // R[4][64], z section shifted to this rank's z-slab
     AxisPass pass_fwd[2], pass_inv[2];   // x, y one axis per pass (any supported length), used unless xy_reg
@@ -372,6 +292,13 @@ static int sfail(lgf_slab *ctx, int code, const std::string &msg) {
         if (e_ != cudaSuccess)                                                                        \
             return sfail(ctx, e_ == cudaErrorMemoryAllocation ? LGF_ENOMEM : LGF_ECUDA,               \
                          std::string(#call) + ": " + cudaGetErrorString(e_));                         \
+    } while (0)
+
+// every entry point runs on the device the context was created on (the caller may have another one current)
+#define SLAB_ENTER(ctx)                                                                               \
+    do {                                                                                              \
+        cudaError_t e_ = cudaSetDevice((ctx)->device);                                                \
+        if (e_ != cudaSuccess) return sfail(ctx, LGF_ECUDA, std::string("cudaSetDevice: ") + cudaGetErrorString(e_)); \
     } while (0)
 
 static long long divisor_le(long long n, long long cap) {
@@ -517,15 +444,27 @@ static int slab_fft_inverse(lgf_slab *ctx, const void *d_recv, bool with_g, doub
 }
 
 template <class R>
-static int slab_delta(lgf_slab *ctx, double *d_sums) {
-    if (ctx->nr == 3)
-        k_slab_delta<R, 3><<<ctx->nb, SLAB_THREADS, 0, ctx->stream>>>((const C<R> *)ctx->links, (const C<R> *)ctx->uhalo,
-                                                                      (C<R> *)ctx->W, ctx->gl, ctx->partial);
-    else
-        k_slab_delta<R, 2><<<ctx->nb, SLAB_THREADS, 0, ctx->stream>>>((const C<R> *)ctx->links, (const C<R> *)ctx->uhalo,
-                                                                      (C<R> *)ctx->W, ctx->gl, ctx->partial);
-    SCK(cudaGetLastError());
-    k_slab_sum2<<<1, SLAB_THREADS, 0, ctx->stream>>>(ctx->partial, ctx->nb, d_sums);
+static LinkPair<R> slab_links(lgf_slab *ctx) {
+    LinkPair<R> lp;
+    lp.buf[0] = (C<R> *)ctx->lbuf[0];
+    lp.buf[1] = (C<R> *)ctx->lbuf[1];
+    return lp;
+}
+template <class R>
+static SweepHalo<R> slab_halo(lgf_slab *ctx) {
+    SweepHalo<R> h;
+    h.ghi = (const C<R> *)ctx->ghalo;
+    h.glo = (const C<R> *)ctx->glo;
+    h.uhalo = (C<R> *)ctx->uhalo;
+    return h;
+}
+// a1 on the slab: the one-GPU path's k_delta with the U_t halo (lgf_links.cu); `stop` = the word that makes it return
+template <class R>
+static int slab_delta(lgf_slab *ctx, double *d_sums, const int *stop) {
+    int nb = 0;
+    SCK(launch_delta<R>(ctx->nr, slab_links<R>(ctx), (C<R> *)ctx->W, ctx->gl, ctx->partial, &nb, stop, ctx->st, ctx->stream,
+                        slab_halo<R>(ctx)));
+    k_slab_sum2<<<1, SLAB_THREADS, 0, ctx->stream>>>(ctx->partial, nb, d_sums, stop);
     SCK(cudaGetLastError());
     ctx->launches += 2;
     return LGF_OK;
@@ -534,34 +473,25 @@ static int slab_delta(lgf_slab *ctx, double *d_sums) {
 template <class R>
 static int slab_update(lgf_slab *ctx) {
     if (ctx->nr == 3)
-        k_slab_update<R, 3><<<ctx->nb, SLAB_THREADS, 0, ctx->stream>>>((C<R> *)ctx->links, (const C<R> *)ctx->G,
-                                                                       (const C<R> *)ctx->ghalo, ctx->gl);
+        k_slab_update<R, 3><<<ctx->nb, SLAB_THREADS, 0, ctx->stream>>>(slab_links<R>(ctx), (const C<R> *)ctx->G,
+                                                                       (const C<R> *)ctx->ghalo, ctx->gl, ctx->st);
     else
-        k_slab_update<R, 2><<<ctx->nb, SLAB_THREADS, 0, ctx->stream>>>((C<R> *)ctx->links, (const C<R> *)ctx->G,
-                                                                       (const C<R> *)ctx->ghalo, ctx->gl);
+        k_slab_update<R, 2><<<ctx->nb, SLAB_THREADS, 0, ctx->stream>>>(slab_links<R>(ctx), (const C<R> *)ctx->G,
+                                                                       (const C<R> *)ctx->ghalo, ctx->gl, ctx->st);
     SCK(cudaGetLastError());
     ctx->launches++;
     return LGF_OK;
 }
 
+// a6 + a1 fused: the one-GPU path's k_sweep with the halo policy (g of both neighbouring slices, U_t of the slice
+// below read from and stored back into its halo copy); new links into the other buffer -- lgf_slab_finalize flips
 template <class R>
 static int slab_sweep(lgf_slab *ctx, double *d_sums) {
-    const int nb = (int)((ctx->gl.V + SLAB_SWEEP_THREADS - 1) / SLAB_SWEEP_THREADS);      // <= 2 * ctx->nb: partial is sized for it
-    const C<R> *src = (const C<R> *)ctx->lbuf[ctx->cur];
-    C<R> *dst = (C<R> *)ctx->lbuf[1 - ctx->cur];
-    if (ctx->nr == 3)
-        k_slab_sweep<R, 3><<<nb, SLAB_SWEEP_THREADS, 0, ctx->stream>>>(src, dst, (const C<R> *)ctx->G, (const C<R> *)ctx->ghalo,
-                                                                       (const C<R> *)ctx->glo, (C<R> *)ctx->uhalo, (C<R> *)ctx->W,
-                                                                       ctx->gl, ctx->partial);
-    else
-        k_slab_sweep<R, 2><<<nb, SLAB_SWEEP_THREADS, 0, ctx->stream>>>(src, dst, (const C<R> *)ctx->G, (const C<R> *)ctx->ghalo,
-                                                                       (const C<R> *)ctx->glo, (C<R> *)ctx->uhalo, (C<R> *)ctx->W,
-                                                                       ctx->gl, ctx->partial);
+    int nb = 0;
+    SCK(launch_sweep<R>(ctx->nr, slab_links<R>(ctx), (const C<R> *)ctx->G, (C<R> *)ctx->W, ctx->gl, ctx->partial, &nb, ctx->st,
+                        LaunchStream(ctx->stream, false), 1, false, -1, 0, 3, slab_halo<R>(ctx)));
+    k_slab_sum2<<<1, SLAB_THREADS, 0, ctx->stream>>>(ctx->partial, nb, d_sums, &ctx->st->done);
     SCK(cudaGetLastError());
-    k_slab_sum2<<<1, SLAB_THREADS, 0, ctx->stream>>>(ctx->partial, nb, d_sums);
-    SCK(cudaGetLastError());
-    ctx->cur = 1 - ctx->cur;
-    ctx->links = ctx->lbuf[ctx->cur];
     ctx->launches += 2;
     return LGF_OK;
 }
@@ -572,10 +502,13 @@ const char *lgf_slab_last_error(const lgf_slab *ctx) { return ctx ? ctx->err.c_s
 
 int lgf_slab_destroy(lgf_slab *ctx) {
     if (!ctx) return LGF_EINVAL;
+    cudaSetDevice(ctx->device);
     cudaStreamSynchronize(ctx->stream);
     void *bufs[] = {ctx->lbuf[0], ctx->lbuf[1], ctx->uhalo, ctx->W, ctx->G, ctx->ghalo, ctx->glo, ctx->partial, ctx->st, ctx->p2tab,
-                    ctx->twiddle[0], ctx->twiddle[1], ctx->twiddle[2], ctx->twiddle[3]};
+                    ctx->twiddle[0], ctx->twiddle[1], ctx->twiddle[2], ctx->twiddle[3], ctx->hist};
     for (void *b : bufs) cudaFree(b);
+    if (ctx->h_poll) cudaFreeHost(ctx->h_poll);
+    for (int k = 0; k < 2; k++) if (ctx->poll_ev[k]) cudaEventDestroy(ctx->poll_ev[k]);
     cudaGetLastError();
     delete ctx;
     return LGF_OK;
@@ -600,6 +533,7 @@ int lgf_slab_create(const int dims[4], int precision, int link_storage, int rank
     }
     lgf_slab *ctx = new (std::nothrow) lgf_slab();
     if (!ctx) return sfail(nullptr, LGF_ENOMEM, "lgf_slab_create: host allocation failed");
+    cudaGetDevice(&ctx->device);                              // every later call runs on this device (slab_enter)
     ctx->prec = precision;
     ctx->nr = link_storage == LGF_LINKS_18 ? 3 : 2;
     ctx->rank = rank;
@@ -637,7 +571,6 @@ int lgf_slab_create(const int dims[4], int precision, int link_storage, int rank
     };
     alloc(&ctx->lbuf[0], V * 4 * 3 * ctx->nr * cb);
     alloc(&ctx->lbuf[1], V * 4 * 3 * ctx->nr * cb);
-    ctx->links = ctx->lbuf[0];
     alloc(&ctx->uhalo, S3 * 3 * ctx->nr * cb);
     alloc(&ctx->W, V * 4 * cb);
     alloc(&ctx->G, V * 6 * cb);
@@ -645,9 +578,13 @@ int lgf_slab_create(const int dims[4], int precision, int link_storage, int rank
     alloc(&ctx->glo, S3 * 6 * cb);
     alloc((void **)&ctx->partial, sizeof(double) * 2 * (2 * ctx->nb + 1));
     alloc((void **)&ctx->st, sizeof(DevState));
+    ctx->hist_cap = 1 << 20;
+    alloc((void **)&ctx->hist, sizeof(double) * 2 * ctx->hist_cap);
     if (rc == LGF_OK) {
         cudaError_t ee = cudaMemset(ctx->st, 0, sizeof(DevState));
-        if (ee != cudaSuccess) rc = sfail(ctx, LGF_ECUDA, std::string("cudaMemset: ") + cudaGetErrorString(ee));
+        if (ee == cudaSuccess) ee = cudaMallocHost((void **)&ctx->h_poll, 2 * sizeof(DevState));
+        for (int k = 0; k < 2 && ee == cudaSuccess; k++) ee = cudaEventCreateWithFlags(&ctx->poll_ev[k], cudaEventDisableTiming);
+        if (ee != cudaSuccess) rc = sfail(ctx, LGF_ECUDA, std::string("state / poll buffers: ") + cudaGetErrorString(ee));
     }
     if (rc == LGF_OK) rc = precision == LGF_FP64 ? slab_tables<double>(ctx) : slab_tables<float>(ctx);
     if (rc != LGF_OK) {
@@ -665,18 +602,20 @@ int lgf_slab_create(const int dims[4], int precision, int link_storage, int rank
 
 int lgf_slab_set_stream(lgf_slab *ctx, void *cuda_stream) {
     if (!ctx) return LGF_EINVAL;
+    SLAB_ENTER(ctx);
+    SCK(cudaStreamSynchronize(ctx->stream));             // work enqueued on the old stream is not ordered with the new one
     ctx->stream = (cudaStream_t)cuda_stream;
     return LGF_OK;
 }
 
 int lgf_slab_set_links(lgf_slab *ctx, const void *d_links) {
     if (!ctx || !d_links) return sfail(ctx, LGF_EINVAL, "lgf_slab_set_links: null argument");
-    ctx->cur = 0;
-    ctx->links = ctx->lbuf[0];
+    SLAB_ENTER(ctx);
     ctx->uhalo_valid = false;
-    if (ctx->prec == LGF_FP64) SCK(launch_convert_in<double>(ctx->nr, (const double *)d_links, (C<double> *)ctx->links, ctx->gl, ctx->stream));
-    else SCK(launch_convert_in<float>(ctx->nr, (const float *)d_links, (C<float> *)ctx->links, ctx->gl, ctx->stream));
-    ctx->launches++;
+    if (ctx->prec == LGF_FP64) SCK(launch_convert_in<double>(ctx->nr, (const double *)d_links, (C<double> *)ctx->lbuf[0], ctx->gl, ctx->stream));
+    else SCK(launch_convert_in<float>(ctx->nr, (const float *)d_links, (C<float> *)ctx->lbuf[0], ctx->gl, ctx->stream));
+    SCK(launch_reset_state(ctx->st, ctx->stream));       // buffer 0 current, counters, history and flags cleared
+    ctx->launches += 2;
     ctx->have_links = true;
     return LGF_OK;
 }
@@ -684,13 +623,11 @@ int lgf_slab_set_links(lgf_slab *ctx, const void *d_links) {
 int lgf_slab_get_links(lgf_slab *ctx, void *d_links) {
     if (!ctx || !d_links) return sfail(ctx, LGF_EINVAL, "lgf_slab_get_links: null argument");
     if (!ctx->have_links) return sfail(ctx, LGF_ESTATE, "lgf_slab_get_links: no configuration loaded");
-    if (ctx->prec == LGF_FP64) {
-        LinkPair<double> lp{{(C<double> *)ctx->links, (C<double> *)ctx->links}};
-        SCK(launch_convert_out<double>(ctx->nr, lp, (double *)d_links, ctx->gl, ctx->st, ctx->stream));
-    } else {
-        LinkPair<float> lp{{(C<float> *)ctx->links, (C<float> *)ctx->links}};
-        SCK(launch_convert_out<float>(ctx->nr, lp, (float *)d_links, ctx->gl, ctx->st, ctx->stream));
-    }
+    SLAB_ENTER(ctx);
+    if (ctx->prec == LGF_FP64)
+        SCK(launch_convert_out<double>(ctx->nr, slab_links<double>(ctx), (double *)d_links, ctx->gl, ctx->st, ctx->stream));
+    else
+        SCK(launch_convert_out<float>(ctx->nr, slab_links<float>(ctx), (float *)d_links, ctx->gl, ctx->st, ctx->stream));
     ctx->launches++;
     return LGF_OK;
 }
@@ -703,10 +640,19 @@ long long lgf_slab_halo_elems(const lgf_slab *ctx, int which) {
 int lgf_slab_halo_pack(lgf_slab *ctx, int which, void *d_send) {
     if (!ctx || !d_send) return sfail(ctx, LGF_EINVAL, "lgf_slab_halo_pack: null argument");
     if (!ctx->have_links) return sfail(ctx, LGF_ESTATE, "lgf_slab_halo_pack: no configuration loaded");
+    SLAB_ENTER(ctx);
     const size_t cb = 2 * (size_t)ctx->prec, S3 = (size_t)ctx->gl.S[3], V = (size_t)ctx->gl.V;
-    if (which == LGF_HALO_LINKS) {          // U_t of the LAST local slice, for the rank above
-        const char *src = (const char *)ctx->links + ((size_t)3 * 3 * ctx->nr * V + S3 * (ctx->T - 1)) * cb;
-        SCK(cudaMemcpy2DAsync(d_send, S3 * cb, src, V * cb, S3 * cb, 3 * ctx->nr, cudaMemcpyDeviceToDevice, ctx->stream));
+    if (which == LGF_HALO_LINKS) {          // U_t of the LAST local slice of the current buffer, for the rank above
+        const int np = 3 * ctx->nr;
+        const int nb = (int)((S3 * np + SLAB_THREADS - 1) / SLAB_THREADS);
+        if (ctx->prec == LGF_FP64)
+            k_slab_pack_ut<double><<<nb, SLAB_THREADS, 0, ctx->stream>>>(slab_links<double>(ctx), (C<double> *)d_send, (long long)V,
+                                                                       (long long)S3, np, (long long)(S3 * (ctx->T - 1)), ctx->st);
+        else
+            k_slab_pack_ut<float><<<nb, SLAB_THREADS, 0, ctx->stream>>>(slab_links<float>(ctx), (C<float> *)d_send, (long long)V,
+                                                                      (long long)S3, np, (long long)(S3 * (ctx->T - 1)), ctx->st);
+        SCK(cudaGetLastError());
+        ctx->launches++;
     } else if (which == LGF_HALO_G) {       // g of the FIRST local slice, for the rank below
         SCK(cudaMemcpy2DAsync(d_send, S3 * cb, ctx->G, V * cb, S3 * cb, 6, cudaMemcpyDeviceToDevice, ctx->stream));
     } else if (which == LGF_HALO_G_UP) {    // g of the LAST local slice, for the rank above (fused sweep)
@@ -718,6 +664,7 @@ int lgf_slab_halo_pack(lgf_slab *ctx, int which, void *d_send) {
 
 int lgf_slab_halo_unpack(lgf_slab *ctx, int which, const void *d_recv) {
     if (!ctx || !d_recv) return sfail(ctx, LGF_EINVAL, "lgf_slab_halo_unpack: null argument");
+    SLAB_ENTER(ctx);
     const size_t cb = 2 * (size_t)ctx->prec, S3 = (size_t)ctx->gl.S[3];
     if (which == LGF_HALO_LINKS) {
         SCK(cudaMemcpyAsync(ctx->uhalo, d_recv, S3 * 3 * ctx->nr * cb, cudaMemcpyDeviceToDevice, ctx->stream));
@@ -731,31 +678,37 @@ int lgf_slab_halo_unpack(lgf_slab *ctx, int which, const void *d_recv) {
 int lgf_slab_delta(lgf_slab *ctx, double *d_sums) {
     if (!ctx || !d_sums) return sfail(ctx, LGF_EINVAL, "lgf_slab_delta: null argument");
     if (!ctx->have_links) return sfail(ctx, LGF_ESTATE, "lgf_slab_delta: no configuration loaded");
-    return ctx->prec == LGF_FP64 ? slab_delta<double>(ctx, d_sums) : slab_delta<float>(ctx, d_sums);
+    SLAB_ENTER(ctx);
+    return ctx->prec == LGF_FP64 ? slab_delta<double>(ctx, d_sums, &ctx->st->zero) : slab_delta<float>(ctx, d_sums, &ctx->st->zero);
 }
 
 int lgf_slab_fft_forward(lgf_slab *ctx, void *d_send) {
     if (!ctx || !d_send) return sfail(ctx, LGF_EINVAL, "lgf_slab_fft_forward: null argument");
+    SLAB_ENTER(ctx);
     return ctx->prec == LGF_FP64 ? slab_fft_forward<double>(ctx, d_send) : slab_fft_forward<float>(ctx, d_send);
 }
 
 int lgf_slab_fft_t(lgf_slab *ctx, const void *d_recv, void *d_send) {
     if (!ctx || !d_recv || !d_send || d_recv == d_send) return sfail(ctx, LGF_EINVAL, "lgf_slab_fft_t: bad argument");
+    SLAB_ENTER(ctx);
     return ctx->prec == LGF_FP64 ? slab_fft_t<double>(ctx, d_recv, d_send) : slab_fft_t<float>(ctx, d_recv, d_send);
 }
 
 int lgf_slab_fft_inverse(lgf_slab *ctx, const void *d_recv) {
     if (!ctx || !d_recv) return sfail(ctx, LGF_EINVAL, "lgf_slab_fft_inverse: null argument");
+    SLAB_ENTER(ctx);
     return ctx->prec == LGF_FP64 ? slab_fft_inverse<double>(ctx, d_recv, false, 0.0) : slab_fft_inverse<float>(ctx, d_recv, false, 0.0);
 }
 
 int lgf_slab_fft_inverse_g(lgf_slab *ctx, const void *d_recv, double alpha) {
     if (!ctx || !d_recv) return sfail(ctx, LGF_EINVAL, "lgf_slab_fft_inverse_g: null argument");
+    SLAB_ENTER(ctx);
     return ctx->prec == LGF_FP64 ? slab_fft_inverse<double>(ctx, d_recv, true, alpha) : slab_fft_inverse<float>(ctx, d_recv, true, alpha);
 }
 
 int lgf_slab_gbuild(lgf_slab *ctx, double alpha) {
     if (!ctx) return LGF_EINVAL;
+    SLAB_ENTER(ctx);
     if (ctx->prec == LGF_FP64)
         SCK(launch_gbuild<double>((const C<double> *)ctx->W, (C<double> *)ctx->G, ctx->gl, 0.5 * alpha, ctx->st, ctx->stream));
     else
@@ -767,6 +720,7 @@ int lgf_slab_gbuild(lgf_slab *ctx, double alpha) {
 int lgf_slab_update(lgf_slab *ctx) {
     if (!ctx) return LGF_EINVAL;
     if (!ctx->have_links) return sfail(ctx, LGF_ESTATE, "lgf_slab_update: no configuration loaded");
+    SLAB_ENTER(ctx);
     ctx->uhalo_valid = false;                // the neighbour's U_t changed too: exchange it again before the next delta
     return ctx->prec == LGF_FP64 ? slab_update<double>(ctx) : slab_update<float>(ctx);
 }
@@ -776,14 +730,88 @@ int lgf_slab_sweep(lgf_slab *ctx, double *d_sums) {
     if (!ctx->have_links) return sfail(ctx, LGF_ESTATE, "lgf_slab_sweep: no configuration loaded");
     if (!ctx->uhalo_valid)
         return sfail(ctx, LGF_ESTATE, "lgf_slab_sweep: the U_t halo is not current (halo_unpack(LGF_HALO_LINKS) after set_links / update)");
+    SLAB_ENTER(ctx);
     return ctx->prec == LGF_FP64 ? slab_sweep<double>(ctx, d_sums) : slab_sweep<float>(ctx, d_sums);
 }
 
 int lgf_slab_get_field(lgf_slab *ctx, void *d_field) {
     if (!ctx || !d_field) return sfail(ctx, LGF_EINVAL, "lgf_slab_get_field: null argument");
+    SLAB_ENTER(ctx);
     if (ctx->prec == LGF_FP64) SCK(launch_field_get<double>((const C<double> *)ctx->W, (double *)d_field, ctx->gl, ctx->stream));
     else SCK(launch_field_get<float>((const C<float> *)ctx->W, (float *)d_field, ctx->gl, ctx->stream));
     ctx->launches++;
+    return LGF_OK;
+}
+
+/* ---- Algorithm 1's control on the device: the slab twin of the one-GPU path's finalize ---- */
+int lgf_slab_finalize(lgf_slab *ctx, const double *d_sums, double tol, int after_sweep, int record) {
+    if (!ctx || !d_sums) return sfail(ctx, LGF_EINVAL, "lgf_slab_finalize: null argument");
+    SLAB_ENTER(ctx);
+    // k_finalize (lgf_links.cu) over ONE pair of sums, the all-reduced ones, normalised with the GLOBAL volume
+    SCK(launch_finalize(d_sums, 1, ctx->Vglobal, tol, after_sweep, record, ctx->st, ctx->hist, ctx->hist_cap,
+                        LaunchStream(ctx->stream, false)));
+    ctx->launches++;
+    return LGF_OK;
+}
+
+int lgf_slab_clear_done(lgf_slab *ctx) {
+    if (!ctx) return LGF_EINVAL;
+    SLAB_ENTER(ctx);
+    SCK(launch_clear_done(ctx->st, ctx->stream));
+    ctx->launches++;
+    return LGF_OK;
+}
+
+int lgf_slab_poll(lgf_slab *ctx) {
+    if (!ctx) return LGF_EINVAL;
+    SLAB_ENTER(ctx);
+    if (ctx->polls_enq - ctx->polls_seen >= 2) return sfail(ctx, LGF_ESTATE, "lgf_slab_poll: two looks are already outstanding");
+    const int k = ctx->polls_enq & 1;
+    SCK(cudaMemcpyAsync(&ctx->h_poll[k], ctx->st, sizeof(DevState), cudaMemcpyDeviceToHost, ctx->stream));
+    SCK(cudaEventRecord(ctx->poll_ev[k], ctx->stream));
+    ctx->polls_enq++;
+    return LGF_OK;
+}
+
+int lgf_slab_poll_wait(lgf_slab *ctx, int *done, int *nan, long long *n_updates, double *F, double *theta) {
+    if (!ctx) return LGF_EINVAL;
+    SLAB_ENTER(ctx);
+    if (ctx->polls_enq == ctx->polls_seen) return sfail(ctx, LGF_ESTATE, "lgf_slab_poll_wait: no look outstanding");
+    const int k = ctx->polls_seen & 1;
+    SCK(cudaEventSynchronize(ctx->poll_ev[k]));
+    ctx->polls_seen++;
+    const DevState &h = ctx->h_poll[k];
+    if (done) *done = h.done;
+    if (nan) *nan = h.nan;
+    if (n_updates) *n_updates = h.n_updates;
+    if (F) *F = h.F;
+    if (theta) *theta = h.theta;
+    return LGF_OK;
+}
+
+long long lgf_slab_history_length(lgf_slab *ctx) {
+    if (!ctx) return LGF_EINVAL;
+    SLAB_ENTER(ctx);
+    DevState h;
+    SCK(cudaMemcpyAsync(&h, ctx->st, sizeof(DevState), cudaMemcpyDeviceToHost, ctx->stream));
+    SCK(cudaStreamSynchronize(ctx->stream));
+    return h.n_hist;
+}
+
+int lgf_slab_history(lgf_slab *ctx, long long first, long long count, double *F, double *theta) {
+    if (!ctx || first < 0 || count < 0) return sfail(ctx, LGF_EINVAL, "lgf_slab_history: bad argument");
+    const long long n = lgf_slab_history_length(ctx);
+    if (n < 0) return (int)n;
+    const long long have = n < ctx->hist_cap ? n : ctx->hist_cap;
+    if (first + count > have) return sfail(ctx, LGF_EINVAL, "lgf_slab_history: range beyond the recorded entries");
+    if (count == 0) return LGF_OK;
+    std::vector<double> buf(2 * (size_t)count);
+    SCK(cudaMemcpyAsync(buf.data(), ctx->hist + 2 * first, sizeof(double) * 2 * count, cudaMemcpyDeviceToHost, ctx->stream));
+    SCK(cudaStreamSynchronize(ctx->stream));
+    for (long long i = 0; i < count; i++) {
+        if (F) F[i] = buf[2 * i];
+        if (theta) theta[i] = buf[2 * i + 1];
+    }
     return LGF_OK;
 }
 

@@ -3,7 +3,8 @@
 SURVEY.md section 8(e) / 8(f) NEXT-3; the paper's stated future work (its CPU code does the same
 decomposition with PFFT over MPI, :124).  Rank r of N owns the slices t = r T .. (r+1) T - 1 of the lattice.
 Every arithmetic step runs in liblgf's kernels through the per-rank entry points ``lgf_slab_*`` (include/lgf.h);
-this module only sequences them and moves the buffers between ranks.  The exchanges (the U_t halo only once per
+this module only sequences them and moves the buffers between ranks: the F / theta normalisation, the history and
+Algorithm 1's loop test are the library's too (``lgf_slab_finalize``, a device-side flag).  The exchanges (the U_t halo only once per
 loaded configuration -- the fused sweep keeps it current -- the others once per iteration):
 
   halo LINKS  U_t of a rank's last slice     -> rank r+1   (a1: A_t(x - t), eq. 5)          S3 * n_l reals
@@ -134,9 +135,8 @@ class SlabFixer:
         self._g2_send, self._g2_recv = mk(c0.halo_elems(B.LGF_HALO_G_UP)), mk(c0.halo_elems(B.LGF_HALO_G_UP))
         self._a_send, self._a_recv = mk(c0.V * 8), mk(c0.V * 8)
         self._sums = mk(2, torch.float64)
-        self._hist = []                 # device tensors [2]: (sum Re tr U, sum tr Delta Delta^dag), all-reduced
-        self._measured = False          # W of every rank holds Delta of the current links and _hist[-1] their sums
-        self.updates = 0
+        self._w_is_delta = False        # W of every rank holds Delta of the current links (and _sums their all-reduced sums)
+        self._recorded = False          # ... and that configuration's (F, theta) is in the history
         self.exchanged_bytes = 0        # per rank, what the last iterate() sent (bench / DESIGN.md figures)
 
     # -- configuration ----------------------------------------------------------------------------
@@ -146,7 +146,7 @@ class SlabFixer:
             raise ValueError("expected %d slab(s)" % len(self.ranks))
         for c, s in zip(self.ranks, slabs):
             c.set_links(s.contiguous())
-        self._hist, self._measured, self.updates = [], False, 0
+        self._w_is_delta, self._recorded = False, False
 
     def set_links_global(self, links) -> None:
         self.set_links([slab_of(links, r, self.ex.world) for r in self.ex.local_ranks])
@@ -160,8 +160,9 @@ class SlabFixer:
         return out
 
     # -- the steps of one iteration ---------------------------------------------------------------
-    def _step_delta(self) -> None:
-        """a1 (+ halo of U_t, all-reduce of the sums): Delta into every rank's work field, sums into the history."""
+    def _step_delta(self, tol: float, record: bool) -> None:
+        """a1 (+ halo of U_t, all-reduce of the sums, finalize on the device): Delta into every rank's work field;
+        F, theta into the state, and with `record` into the history together with the loop test theta < tol."""
         for c, s in zip(self.ranks, self._u_send):
             c.halo_pack(B.LGF_HALO_LINKS, s)
         self.ex.shift(self._u_send, self._u_recv, +1)
@@ -169,8 +170,10 @@ class SlabFixer:
             c.halo_unpack(B.LGF_HALO_LINKS, r)
             c.delta(sm)
         self.ex.all_reduce_sum(self._sums)
-        self._hist.append(self._sums[0].clone())
-        self._measured = True
+        for c, sm in zip(self.ranks, self._sums):
+            c.finalize(sm, tol, False, record)
+        self._w_is_delta = True
+        self._recorded = self._recorded or record
 
     def _fft_to_second_exchange(self) -> None:
         for c, s in zip(self.ranks, self._a_send):
@@ -196,13 +199,14 @@ class SlabFixer:
         for c, r in zip(self.ranks, self._g_recv):
             c.halo_unpack(B.LGF_HALO_G, r)
             c.update()
-        self._measured = False
-        self.updates += 1
+        self._w_is_delta, self._recorded = False, False
 
-    def _step_iteration(self, alpha: float) -> None:
+    def _step_iteration(self, alpha: float, tol: float) -> None:
         """a2-a6 + a1 of the new links, as iterate / fix run them: the g-build at the end of the last FFT sweep, g halos
-        both ways, the fused sweep (new links, their Delta and sums in one pass), all-reduce.  Wants the work fields
-        to hold Delta of the current links (``_measured``), which also means the U_t halos are current."""
+        both ways, the fused sweep (new links, their Delta and sums in one pass), all-reduce, finalize on the device
+        (new buffer current, history, loop test).  Wants the work fields to hold Delta of the current links, which
+        also means the U_t halos are current.  Nothing is read back: once the device-side `done` flag is set the
+        kernels of later iterations return at once."""
         self._fft_to_second_exchange()
         for c, r, dn, up in zip(self.ranks, self._a_recv, self._g_send, self._g2_send):
             c.fft_inverse_g(r, alpha)
@@ -215,9 +219,9 @@ class SlabFixer:
             c.halo_unpack(B.LGF_HALO_G_UP, up)
             c.sweep(sm)
         self.ex.all_reduce_sum(self._sums)
-        self._hist.append(self._sums[0].clone())
-        self._measured = True
-        self.updates += 1
+        for c, sm in zip(self.ranks, self._sums):
+            c.finalize(sm, tol, True, True)
+        self._w_is_delta, self._recorded = True, True
 
     def _bytes_per_iteration(self) -> int:
         n, es = self.ex.world, self._a_send[0].element_size()
@@ -227,50 +231,68 @@ class SlabFixer:
         return a2a + (self._g_send[0].numel() + self._g2_send[0].numel()) * es + 16
 
     # -- public: same meaning as lgf_measure / lgf_iterate / lgf_fix ---------------------------------
+    def _look(self):
+        """(done, nan, n_updates, F, theta) as the device state stands after everything enqueued so far."""
+        for c in self.ranks:
+            c.poll()
+        return [c.poll_wait() for c in self.ranks][0]
+
+    def _first_measure(self, tol: float) -> None:
+        """Alg. 1 line 1: Delta, F, theta of the loaded configuration as history entry 0, with the first loop test."""
+        if not (self._w_is_delta and self._recorded):
+            self._step_delta(tol, True)
+
     def measure(self):
-        """(F, theta) of the current configuration (eqs. 3, 6); synchronises."""
-        if not self._measured:
-            self._step_delta()
-            sums = self._hist.pop()           # a measurement records nothing ...
-            self._measured = False            # ... so the next iterate measures (and records) again
-        else:
-            sums = self._hist[-1]
-        f, t = sums.tolist()
-        return f / (12.0 * self.V), t / (3.0 * self.V)
+        """(F, theta) of the current configuration (eqs. 3, 6), computed by the library; records nothing; synchronises."""
+        self._step_delta(-1.0, False)
+        _, _, _, F, theta = self._look()
+        return F, theta
 
     def iterate(self, alpha: float, n: int) -> None:
         """n updates regardless of theta; leaves n + 1 history entries from a fresh configuration.  Never reads
         a value back to the host."""
+        for c in self.ranks:
+            c.clear_done()
+        self._first_measure(-1.0)
         for _ in range(int(n)):
-            if not self._measured:
-                self._step_delta()
-            self._step_iteration(alpha)
-        if not self._measured:
-            self._step_delta()
+            self._step_iteration(alpha, -1.0)
         self.exchanged_bytes = self._bytes_per_iteration() * int(n)
 
-    def fix(self, alpha: float, tol: float, max_iter: int) -> int:
-        """measure; while theta >= tol and it < max_iter: update; measure.  Returns the number of updates."""
-        it = 0
-        while True:
-            if not self._measured:
-                self._step_delta()
-            theta = float(self._hist[-1][1].item()) / (3.0 * self.V)
-            if theta != theta:
-                raise B.LgfError(B.LGF_ENAN, "theta became NaN")
-            if theta < tol or it >= max_iter:
-                return it
-            self._step_iteration(alpha)
-            it += 1
+    def fix(self, alpha: float, tol: float, max_iter: int, chunk: int = 16) -> int:
+        """measure; while theta >= tol and it < max_iter: update; measure (Alg. 1).  Returns the number of updates.
+        The loop test is taken on the device (lgf_slab_finalize); the host enqueues `chunk` iterations at a time and
+        looks at the state one chunk behind, so the GPU never waits for the host."""
+        for c in self.ranks:
+            c.clear_done()
+        self._first_measure(tol)
+        issued, outstanding, done = 0, 0, False
+        while not done and issued < max_iter:
+            n = min(chunk, max_iter - issued)
+            for _ in range(n):
+                self._step_iteration(alpha, tol)
+            issued += n
+            for c in self.ranks:
+                c.poll()
+            outstanding += 1
+            if outstanding >= 2:            # the look taken one chunk ago; the chunk just enqueued keeps the GPU busy
+                done = [c.poll_wait() for c in self.ranks][0][0]
+                outstanding -= 1
+        while outstanding:
+            for c in self.ranks:
+                c.poll_wait()
+            outstanding -= 1
+        done, nan, updates, _, _ = self._look()
+        if nan:
+            raise B.LgfError(B.LGF_ENAN, "theta became NaN")
+        return updates
 
     def history(self):
-        """(F[], theta[]) numpy arrays of the recorded entries; synchronises."""
-        import numpy as np
+        """(F[], theta[]) numpy arrays of the recorded entries (every rank holds the same); synchronises."""
+        return self.ranks[0].history()
 
-        if not self._hist:
-            return np.zeros(0), np.zeros(0)
-        h = self.torch.stack(self._hist).cpu().numpy()
-        return h[:, 0] / (12.0 * self.V), h[:, 1] / (3.0 * self.V)
+    @property
+    def updates(self) -> int:
+        return self._look()[2]
 
     def work_field(self) -> list:
         """Every local rank's work field (Delta after a measurement) as [T, Lz, Ly, Lx, 3, 3, 2] tensors."""

@@ -61,7 +61,7 @@ def test_slab_delta_and_accelerate(slab, dims, world, prec, storage):
     tol = TOL[prec]
     assert abs(F - F_o) <= tol["scalar"] * abs(F_o)
     assert abs(th - th_o) <= tol["scalar"] * abs(th_o)
-    fx._step_delta()
+    fx._step_delta(-1.0, False)
     D = gathered(fx.work_field())
     assert np.max(np.abs(D - D_o)) < tol["field"] * max(1.0, np.max(np.abs(D_o)))
     fx._step_accelerate()
@@ -103,15 +103,13 @@ def test_slab_single_steps_make_the_same_trajectory(slab, dims, world, prec, sto
     fx = slab.SlabFixer(dims, prec, storage, slab.LocalExchange(world))
     fx.set_links_global(to_dev(U, prec))
     for k in range(n):
-        fx._step_delta()
+        fx._step_delta(-1.0, not fx._recorded)     # (the fused sweep has recorded its result itself)
         if k % 3 == 2:
-            fx._step_iteration(ALPHA)          # fused sweep in between: records the next entry itself
-            fx._hist.pop()
-            fx._measured = False
+            fx._step_iteration(ALPHA, -1.0)        # fused sweep in between: records the next entry itself
         else:
             fx._step_accelerate()
             fx._step_update(ALPHA)
-    fx._step_delta()
+    fx._step_delta(-1.0, not fx._recorded)
     Fh, Th = fx.history()
     tol = TOL[prec]
     assert len(Th) == n + 1
@@ -129,7 +127,7 @@ def test_slab_sweep_refuses_a_stale_link_halo(slab):
     fx.set_links_global(to_dev(inputs.make_config("C1"), 8))
     with pytest.raises(binding.LgfError):
         fx.ranks[0].sweep(fx._sums[0])         # no U_t halo yet
-    fx._step_delta()
+    fx._step_delta(-1.0, True)
     fx._step_accelerate()
     fx._step_update(ALPHA)                      # in-place update: the halo is stale again
     with pytest.raises(binding.LgfError):
