@@ -210,6 +210,11 @@ int lgf_set_profiling(lgf_ctx *ctx, int on);
  * profiling was switched on (arrays of LGF_K_COUNT entries, either may be NULL).  Synchronises. */
 int lgf_kernel_times(lgf_ctx *ctx, double *ms, long long *launches);
 /* Total number of kernels this context has launched since creation. */
+/* The kernel instantiations this context launches for one iteration, as a profiler names them:
+ * "update=k_sweep<double, 3, 0, 0, 3>;fft=k_fftr2_xy<...>|k_fftr2_zt<...>|...;gbuild=...;delta=..." into buf (cap bytes
+ * including the terminator; LGF_EINVAL if too small).  bench.py uses it to refuse a stored ncu capture of a kernel
+ * this build no longer launches. */
+int lgf_kernel_names(const lgf_ctx *ctx, char *buf, int cap);
 long long lgf_launch_count(const lgf_ctx *ctx);
 /* Algorithmic bytes one launch-set of the given kernel class must move for ONE iteration
  * (DESIGN.md "Algorithmic bytes"): e.g. LGF_K_DELTA -> V * (4*n_l + 8) * bytes_per_real;

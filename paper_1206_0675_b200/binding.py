@@ -60,6 +60,7 @@ SIGNATURES = {
     "lgf_fft_passes": (_i, [_vp]),
     "lgf_set_profiling": (_i, [_vp, _i]),
     "lgf_kernel_times": (_i, [_vp, _dp, _llp]),
+    "lgf_kernel_names": (_i, [_vp, ctypes.c_char_p, _i]),
     "lgf_launch_count": (_ll, [_vp]),
     "lgf_algorithmic_bytes": (_d, [_vp, _i]),
     "lgf_last_error": (ctypes.c_char_p, [_vp]),
@@ -307,6 +308,12 @@ class Context:
 
     def launch_count(self):
         return int(load().lgf_launch_count(self._h))
+
+    def kernel_names(self):
+        """{kernel class: [instantiation names]} of one iteration, as a profiler prints them"""
+        buf = ctypes.create_string_buffer(1024)
+        _check(self._h, load().lgf_kernel_names(self._h, buf, 1024))
+        return {k: v.split("|") for k, v in (kv.split("=", 1) for kv in buf.value.decode().split(";"))}
 
     def algorithmic_bytes(self, kernel_class):
         return float(load().lgf_algorithmic_bytes(self._h, int(kernel_class)))

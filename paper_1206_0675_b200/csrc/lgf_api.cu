@@ -15,6 +15,7 @@ using namespace lgf;
 
 struct lgf_ctx {
     Geom g{};
+    int device = 0;      // the CUDA device the context's buffers live on; every entry point makes it current
     int prec = 0;        // bytes per real
     int nr = 3;          // stored rows per link
     cudaStream_t stream = nullptr;
@@ -79,6 +80,13 @@ static int cuda_fail(lgf_ctx *ctx, cudaError_t e, const char *what) {
     do {                                                             \
         cudaError_t e_ = (call);                                     \
         if (e_ != cudaSuccess) return cuda_fail(ctx, e_, #call);     \
+    } while (0)
+
+// every entry point runs on the device the context was created on (the caller may have another one current)
+#define ENTER(ctx)                                                                                    \
+    do {                                                                                              \
+        cudaError_t e_ = cudaSetDevice((ctx)->device);                                                \
+        if (e_ != cudaSuccess) return cuda_fail(ctx, e_, "cudaSetDevice");                            \
     } while (0)
 
 // the context's stream with its dependent-launch setting, for the launchers
@@ -501,6 +509,7 @@ int lgf_create(const int dims[4], int precision, int link_storage, lgf_ctx **out
     }
     lgf_ctx *ctx = new (std::nothrow) lgf_ctx();
     if (!ctx) return fail(nullptr, LGF_ENOMEM, "lgf_create: host allocation failed");
+    cudaGetDevice(&ctx->device);
     ctx->prec = precision;
     ctx->nr = link_storage == LGF_LINKS_18 ? 3 : 2;
     long long S = 1;
@@ -550,6 +559,7 @@ int lgf_create(const int dims[4], int precision, int link_storage, lgf_ctx **out
 
 int lgf_destroy(lgf_ctx *ctx) {
     if (!ctx) return LGF_EINVAL;
+    cudaSetDevice(ctx->device);
     cudaStreamSynchronize(ctx->stream);
     drain_stamps(ctx);
     cudaFree(ctx->links[0]);
@@ -574,6 +584,7 @@ int lgf_destroy(lgf_ctx *ctx) {
 
 int lgf_set_stream(lgf_ctx *ctx, void *cuda_stream) {
     if (!ctx) return LGF_EINVAL;
+    ENTER(ctx);
     CK(cudaStreamSynchronize(ctx->stream));
     ctx->stream = (cudaStream_t)cuda_stream;
     return LGF_OK;
@@ -581,6 +592,7 @@ int lgf_set_stream(lgf_ctx *ctx, void *cuda_stream) {
 
 int lgf_set_links(lgf_ctx *ctx, const void *d_links) {
     if (!ctx || !d_links) return fail(ctx, LGF_EINVAL, "lgf_set_links: null argument");
+    ENTER(ctx);
     {
         Bracket br(ctx, LGF_K_CONVERT);
         if (ctx->prec == LGF_FP64)
@@ -608,6 +620,7 @@ int lgf_set_links(lgf_ctx *ctx, const void *d_links) {
 int lgf_get_links(lgf_ctx *ctx, void *d_links) {
     if (!ctx || !d_links) return fail(ctx, LGF_EINVAL, "lgf_get_links: null argument");
     if (!ctx->have_links) return fail(ctx, LGF_ESTATE, "lgf_get_links: no configuration loaded");
+    ENTER(ctx);
     Bracket br(ctx, LGF_K_CONVERT);
     if (ctx->prec == LGF_FP64)
         CK(launch_convert_out<double>(ctx->nr, link_pair<double>(ctx), (double *)d_links, ctx->g, ctx->st, STRM(ctx)));
@@ -623,6 +636,7 @@ static int ensure_staging(lgf_ctx *ctx) {
 
 int lgf_set_links_host(lgf_ctx *ctx, const void *h_links) {
     if (!ctx || !h_links) return fail(ctx, LGF_EINVAL, "lgf_set_links_host: null argument");
+    ENTER(ctx);
     int rc = ensure_staging(ctx);
     if (rc != LGF_OK) return rc;
     CK(cudaMemcpyAsync(ctx->staging, h_links, (size_t)ctx->g.V * 72 * ctx->prec, cudaMemcpyHostToDevice, ctx->stream));
@@ -634,6 +648,7 @@ int lgf_set_links_host(lgf_ctx *ctx, const void *h_links) {
 
 int lgf_get_links_host(lgf_ctx *ctx, void *h_links) {
     if (!ctx || !h_links) return fail(ctx, LGF_EINVAL, "lgf_get_links_host: null argument");
+    ENTER(ctx);
     int rc = ensure_staging(ctx);
     if (rc != LGF_OK) return rc;
     rc = lgf_get_links(ctx, ctx->staging);
@@ -646,6 +661,7 @@ int lgf_get_links_host(lgf_ctx *ctx, void *h_links) {
 int lgf_iterate(lgf_ctx *ctx, double alpha, int n) {
     if (!ctx || n < 0) return fail(ctx, LGF_EINVAL, "lgf_iterate: bad argument");
     if (!ctx->have_links) return fail(ctx, LGF_ESTATE, "lgf_iterate: no configuration loaded");
+    ENTER(ctx);
     ctx->launches++;
     CK(launch_clear_done(ctx->st, STRM(ctx)));
     // tol = -1: theta >= 0 never stops the loop; only a NaN does
@@ -659,6 +675,7 @@ int lgf_iterate(lgf_ctx *ctx, double alpha, int n) {
 int lgf_measure(lgf_ctx *ctx, double *F, double *theta, double *plaquette) {
     if (!ctx) return LGF_EINVAL;
     if (!ctx->have_links) return fail(ctx, LGF_ESTATE, "lgf_measure: no configuration loaded");
+    ENTER(ctx);
     if (plaquette) {                 // uses the second half of the partial-sum buffer
         int nb = 0;
         double *part = ctx->partial + 2 * ctx->partial_cap;
@@ -715,12 +732,16 @@ static long long fix_loaded(lgf_ctx *ctx, double alpha, double tol, long long ma
         }
     }
     if ((rc = fetch_state(ctx)) != LGF_OK) return rc;
+    // iterations enqueued past convergence were no-ops: the projection schedule ("reunit_every") of a later call
+    // must count the updates that were applied, not the ones that were enqueued
+    ctx->updates_enqueued = ctx->h_st->n_updates;
     if (ctx->h_st->nan) return fail(ctx, LGF_ENAN, "lgf_fix: theta is NaN/Inf");
     return ctx->h_st->n_updates;
 }
 
 long long lgf_fix(lgf_ctx *ctx, void *d_links, double alpha, double tol, long long max_iter) {
     if (!ctx || !d_links || max_iter < 0) return fail(ctx, LGF_EINVAL, "lgf_fix: bad argument");
+    ENTER(ctx);
     int rc = lgf_set_links(ctx, d_links);
     if (rc != LGF_OK) return rc;
     const long long it = fix_loaded(ctx, alpha, tol, max_iter);
@@ -732,6 +753,7 @@ long long lgf_fix(lgf_ctx *ctx, void *d_links, double alpha, double tol, long lo
 
 long long lgf_fix_host(lgf_ctx *ctx, void *h_links, double alpha, double tol, long long max_iter) {
     if (!ctx || !h_links || max_iter < 0) return fail(ctx, LGF_EINVAL, "lgf_fix_host: bad argument");
+    ENTER(ctx);
     int rc = lgf_set_links_host(ctx, h_links);
     if (rc != LGF_OK) return rc;
     const long long it = fix_loaded(ctx, alpha, tol, max_iter);
@@ -742,6 +764,7 @@ long long lgf_fix_host(lgf_ctx *ctx, void *h_links, double alpha, double tol, lo
 
 int lgf_history(lgf_ctx *ctx, long long first, long long count, double *F, double *theta) {
     if (!ctx || first < 0 || count < 0) return fail(ctx, LGF_EINVAL, "lgf_history: bad argument");
+    ENTER(ctx);
     int rc = fetch_state(ctx);
     if (rc != LGF_OK) return rc;
     const long long have = ctx->h_st->n_hist < ctx->hist_cap ? ctx->h_st->n_hist : ctx->hist_cap;
@@ -759,6 +782,7 @@ int lgf_history(lgf_ctx *ctx, long long first, long long count, double *F, doubl
 
 long long lgf_iterations(lgf_ctx *ctx) {
     if (!ctx) return LGF_EINVAL;
+    ENTER(ctx);
     const int rc = fetch_state(ctx);
     if (rc != LGF_OK) return rc;
     return ctx->h_st->n_updates;
@@ -766,6 +790,7 @@ long long lgf_iterations(lgf_ctx *ctx) {
 
 long long lgf_history_length(lgf_ctx *ctx) {
     if (!ctx) return LGF_EINVAL;
+    ENTER(ctx);
     const int rc = fetch_state(ctx);
     if (rc != LGF_OK) return rc;
     return ctx->h_st->n_hist;
@@ -774,6 +799,7 @@ long long lgf_history_length(lgf_ctx *ctx) {
 int lgf_step_delta(lgf_ctx *ctx, double *F, double *theta) {
     if (!ctx) return LGF_EINVAL;
     if (!ctx->have_links) return fail(ctx, LGF_ESTATE, "lgf_step_delta: no configuration loaded");
+    ENTER(ctx);
     int rc = DISPATCH(measure_only, ctx);
     if (rc != LGF_OK) return rc;
     ctx->w_is_delta = true;
@@ -787,6 +813,7 @@ int lgf_step_delta(lgf_ctx *ctx, double *F, double *theta) {
 
 int lgf_step_accelerate(lgf_ctx *ctx) {
     if (!ctx) return LGF_EINVAL;
+    ENTER(ctx);
     ctx->launches++;
     CK(launch_clear_done(ctx->st, STRM(ctx)));
     ctx->w_is_delta = false;
@@ -796,6 +823,7 @@ int lgf_step_accelerate(lgf_ctx *ctx) {
 int lgf_step_update(lgf_ctx *ctx, double alpha) {
     if (!ctx) return LGF_EINVAL;
     if (!ctx->have_links) return fail(ctx, LGF_ESTATE, "lgf_step_update: no configuration loaded");
+    ENTER(ctx);
     ctx->launches++;
     CK(launch_clear_done(ctx->st, STRM(ctx)));
     const int rc = DISPATCH(step_update, ctx, alpha, -1.0, 0, false);
@@ -807,6 +835,7 @@ int lgf_step_update(lgf_ctx *ctx, double alpha) {
 
 int lgf_get_field(lgf_ctx *ctx, void *d_field) {
     if (!ctx || !d_field) return fail(ctx, LGF_EINVAL, "lgf_get_field: null argument");
+    ENTER(ctx);
     ctx->launches++;
     if (ctx->prec == LGF_FP64) CK(launch_field_get<double>((const C<double> *)ctx->W, (double *)d_field, ctx->g, STRM(ctx)));
     else CK(launch_field_get<float>((const C<float> *)ctx->W, (float *)d_field, ctx->g, STRM(ctx)));
@@ -815,6 +844,7 @@ int lgf_get_field(lgf_ctx *ctx, void *d_field) {
 
 int lgf_set_field(lgf_ctx *ctx, const void *d_field) {
     if (!ctx || !d_field) return fail(ctx, LGF_EINVAL, "lgf_set_field: null argument");
+    ENTER(ctx);
     ctx->launches++;
     if (ctx->prec == LGF_FP64) CK(launch_field_set<double>((C<double> *)ctx->W, (const double *)d_field, ctx->g, STRM(ctx)));
     else CK(launch_field_set<float>((C<float> *)ctx->W, (const float *)d_field, ctx->g, STRM(ctx)));
@@ -859,17 +889,20 @@ static int monte_carlo_sweeps(lgf_ctx *ctx, double beta, int nsweeps, unsigned l
 int lgf_thermalize(lgf_ctx *ctx, double beta, int nsweeps, unsigned long long seed) {
     if (!ctx || nsweeps < 0 || !(beta > 0.0)) return fail(ctx, LGF_EINVAL, "lgf_thermalize: bad argument");
     if (!ctx->have_links) return fail(ctx, LGF_ESTATE, "lgf_thermalize: no configuration loaded");
+    ENTER(ctx);
     return monte_carlo_sweeps(ctx, beta, nsweeps, seed, false);
 }
 
 int lgf_overrelax(lgf_ctx *ctx, int nsweeps) {
     if (!ctx || nsweeps < 0) return fail(ctx, LGF_EINVAL, "lgf_overrelax: bad argument");
     if (!ctx->have_links) return fail(ctx, LGF_ESTATE, "lgf_overrelax: no configuration loaded");
+    ENTER(ctx);
     return monte_carlo_sweeps(ctx, 0.0, nsweeps, 0, true);
 }
 
 int lgf_track_transform(lgf_ctx *ctx, int on) {
     if (!ctx) return LGF_EINVAL;
+    ENTER(ctx);
     CK(cudaStreamSynchronize(ctx->stream));
     if (!on) {
         cudaFree(ctx->Gacc);
@@ -888,6 +921,7 @@ int lgf_track_transform(lgf_ctx *ctx, int on) {
 int lgf_get_transform(lgf_ctx *ctx, void *d_transform) {
     if (!ctx || !d_transform) return fail(ctx, LGF_EINVAL, "lgf_get_transform: null argument");
     if (!ctx->Gacc) return fail(ctx, LGF_ESTATE, "lgf_get_transform: tracking is off (lgf_track_transform)");
+    ENTER(ctx);
     ctx->launches++;
     if (ctx->prec == LGF_FP64)
         CK(launch_gacc<double>(2, nullptr, (C<double> *)ctx->Gacc, (double *)d_transform, ctx->g, ctx->st, STRM(ctx)));
@@ -899,17 +933,20 @@ int lgf_get_transform(lgf_ctx *ctx, void *d_transform) {
 int lgf_gluon_field(lgf_ctx *ctx, int mu, void *d_out) {
     if (!ctx || !d_out || mu < 0 || mu > 3) return fail(ctx, LGF_EINVAL, "lgf_gluon_field: bad argument");
     if (!ctx->have_links) return fail(ctx, LGF_ESTATE, "lgf_gluon_field: no configuration loaded");
+    ENTER(ctx);
     return ctx->prec == LGF_FP64 ? gluon_field<double>(ctx, mu, d_out) : gluon_field<float>(ctx, mu, d_out);
 }
 
 int lgf_apply_transform(lgf_ctx *ctx, const void *d_transform) {
     if (!ctx || !d_transform) return fail(ctx, LGF_EINVAL, "lgf_apply_transform: null argument");
     if (!ctx->have_links) return fail(ctx, LGF_ESTATE, "lgf_apply_transform: no configuration loaded");
+    ENTER(ctx);
     return ctx->prec == LGF_FP64 ? apply_transform<double>(ctx, d_transform) : apply_transform<float>(ctx, d_transform);
 }
 
 int lgf_tune(lgf_ctx *ctx, const char *key, int value) {
     if (!ctx || !key) return fail(ctx, LGF_EINVAL, "lgf_tune: null argument");
+    ENTER(ctx);
     const std::string k(key);
     if (k == "fft_two_axis") ctx->tune_two_axis = value;
     else if (k == "fft_reg") ctx->tune_reg = value;
@@ -933,6 +970,7 @@ int lgf_fft_passes(const lgf_ctx *ctx) { return ctx ? (int)ctx->passes.size() : 
 
 int lgf_set_profiling(lgf_ctx *ctx, int on) {
     if (!ctx) return LGF_EINVAL;
+    ENTER(ctx);
     CK(cudaStreamSynchronize(ctx->stream));
     drain_stamps(ctx);
     ctx->profiling = on != 0;
@@ -942,12 +980,31 @@ int lgf_set_profiling(lgf_ctx *ctx, int on) {
 
 int lgf_kernel_times(lgf_ctx *ctx, double *ms, long long *launches) {
     if (!ctx) return LGF_EINVAL;
+    ENTER(ctx);
     CK(cudaStreamSynchronize(ctx->stream));
     drain_stamps(ctx);
     for (int k = 0; k < LGF_K_COUNT; k++) {
         if (ms) ms[k] = ctx->prof_ms[k];
         if (launches) launches[k] = ctx->prof_n[k];
     }
+    return LGF_OK;
+}
+
+int lgf_kernel_names(const lgf_ctx *ctx, char *buf, int cap) {
+    if (!ctx || !buf || cap <= 0) return LGF_EINVAL;
+    std::string s = "update=" + sweep_kernel_name(ctx->g, ctx->nr, ctx->prec, false, ctx->tune_sweep_share, ctx->tune_sweep_minb) + ";fft=";
+    const bool fuse = can_fuse_g(ctx);
+    for (size_t i = 0; i < ctx->passes.size(); i++) {
+        const AxisPass &p = ctx->passes[i];
+        if (i) s += "|";
+        if (p.kind == PASS_REG2) s += fft_reg2_kernel_name((fuse && p.axis == 2) ? 3 : p.axis, ctx->g, ctx->prec);
+        else if (p.kind == PASS_REG) s += p.axis == 1 ? "k_fftr_zt<" : "k_fftr_xy<";
+        else s += p.kind == PASS_XY ? "k_fft_xy<" : (p.kind == PASS_ZT ? "k_fft_zt<" : "k_fft_axis<");
+    }
+    s += std::string(";gbuild=k_gbuild<") + (ctx->prec == 8 ? "double>" : "float>");
+    s += std::string(";delta=k_delta<") + (ctx->prec == 8 ? "double, " : "float, ") + std::to_string(ctx->nr) + ">";
+    if ((int)s.size() + 1 > cap) return LGF_EINVAL;
+    memcpy(buf, s.c_str(), s.size() + 1);
     return LGF_OK;
 }
 

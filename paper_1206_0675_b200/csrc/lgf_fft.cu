@@ -163,8 +163,7 @@ __global__ void __launch_bounds__(256) k_fft_zt(C<R> *__restrict__ W, Geom g, in
 // ---- launchers ------------------------------------------------------------------------------------
 template <class K>
 static cudaError_t set_smem(K kern, size_t smem) {
-    if (smem <= 48 * 1024) return cudaSuccess;
-    return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    return ensure_dynamic_smem(kern, smem);
 }
 
 template <class R, int L>

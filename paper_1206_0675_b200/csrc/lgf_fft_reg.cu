@@ -228,8 +228,8 @@ cudaError_t launch_fft_reg(int which, const Geom &g, C<R> *W, const R *twiddle_t
         auto ki = k_fftr_xy<R, LEN, FFT_INV, P, false>;                                                    \
         auto kg = k_fftr_xy<R, LEN, FFT_INV, P, true>;                                                     \
         auto kern = which == 0 ? kf : (which == 2 ? ki : kg);                                              \
-        if (SM > 48 * 1024) {                                                                            \
-            cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SM); \
+        {                                                                                                \
+            cudaError_t e = ensure_dynamic_smem(kern, SM);                                               \
             if (e != cudaSuccess) return e;                                                              \
         }                                                                                                \
         return launch_pdl(kern, dim3((unsigned)(planes / P)), dim3(P * LEN), SM, stream, W, st, G, g.V, nzt, half_alpha); \
@@ -243,8 +243,8 @@ cudaError_t launch_fft_reg(int which, const Geom &g, C<R> *W, const R *twiddle_t
     if (g.L[2] == A && g.L[3] == B) {                                                                         \
         using S = ZtShape<R, A, B, XC, T>;                                                                    \
         auto kern = k_fftr_zt<R, A, B, XC, T>;                                                                \
-        if (S::SMEM > 48 * 1024) {                                                                            \
-            cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S::SMEM); \
+        {                                                                                                     \
+            cudaError_t e = ensure_dynamic_smem(kern, S::SMEM);                                               \
             if (e != cudaSuccess) return e;                                                                   \
         }                                                                                                     \
         dim3 grid((unsigned)(g.S[2] / XC), 4);                                                                \

@@ -8,6 +8,9 @@
 //   k_finalize  final fixed-order sum, F / theta normalisation, history, stop test (Alg. 1 line 2)
 //   layout conversion canonical AoS <-> internal SoA, packed field <-> full 3x3 field
 // Part of liblgf (CUDA path).  Shares nothing with oracle/.
+#include <cstdio>
+#include <string>
+
 #include "lgf_state.cuh"
 #include "lgf_pdl.cuh"
 
@@ -472,34 +475,53 @@ template <class R>
 cudaError_t launch_gbuild(const C<R> *W, C<R> *G, const Geom &g, R half_alpha, const DevState *st, LaunchStream stream) {
     return launch_pdl(k_gbuild<R>, dim3(site_blocks(g)), dim3(SITE_THREADS), 0, stream, W, G, g, half_alpha, st);
 }
+// one t slice of sweep traffic against L2 (the t-backward neighbours are that far behind in the plain order)
+static bool sweep_slice_beyond_l2(const Geom &g, int nr, int prec) {
+    const long long plane = (long long)g.L[0] * g.L[1];
+    return (double)plane * (8.0 * 6.0 * nr + 28.0) * prec * g.L[2] > 64.0e6;
+}
+// A'_x, A'_y through shared memory (SHARE): automatic where it measured faster on B200 -- 18-real storage,
+// x lines that divide the CTA, and fp32 (32^4: 0.1718 -> 0.1601 ms; 64^4: 2.61 -> 2.42 ms) or a lattice beyond
+// L2 (64^4 fp64: 4.42 -> 4.26 ms); neutral within 1.5 % otherwise, +1.7 % at 24^3 x 48.
+bool sweep_uses_share(const Geom &g, int nr, int prec, int share_mode) {
+    return share_mode >= 0 ? share_mode != 0
+                           : (nr == 3 && SWEEP_THREADS % g.L[0] == 0 && (prec == 4 || sweep_slice_beyond_l2(g, nr, prec)));
+}
+// the instantiation launch_sweep picks, as a profiler prints it (bench.py matches ncu captures against it)
+std::string sweep_kernel_name(const Geom &g, int nr, int prec, bool reunit, int share_mode, int minb) {
+    char buf[96];
+    const bool share = sweep_uses_share(g, nr, prec, share_mode);
+    snprintf(buf, sizeof buf, "k_sweep<%s, %d, %d, %d, %d>", prec == 8 ? "double" : "float", nr, (minb == 2 ? 0 : (reunit ? 1 : 0)),
+             share ? 1 : 0, minb == 2 ? 2 : SWEEP_MINB);
+    return buf;
+}
+// (z, t)-tiled block order when the (x, y) plane is a whole number of CTAs of `nt` sites; TZ: about 24 MB of traffic
+// (1.3 kB per site in fp64 / 18-real) between a site and its t-neighbour
+BlockOrder sweep_block_order(const Geom &g, int nr, int prec, int order_tz, int nt) {
+    BlockOrder bo{0, 1, g.L[2], g.L[3]};
+    const long long plane = (long long)g.L[0] * g.L[1];
+    if (order_tz != 1 && plane % nt == 0) {
+        int tz = order_tz;
+        if (tz <= 0) {
+            // automatic: only when one t slice of traffic does not fit in L2 (measured on B200: neutral at
+            // 32^4 where it fits, -4 % sweep time at 64^4 where it does not)
+            const double per_plane = (double)plane * (8.0 * 6.0 * nr + 28.0) * prec;
+            tz = 1;
+            if (sweep_slice_beyond_l2(g, nr, prec))
+                while (tz * 2 <= g.L[2] && g.L[2] % (tz * 2) == 0 && per_plane * tz * 2 <= 24.0e6) tz *= 2;
+        }
+        if (tz > 1 && g.L[2] % tz == 0) { bo.nxy = (int)(plane / nt); bo.tz = tz; }
+    }
+    return bo;
+}
 template <class R>
 cudaError_t launch_sweep(int nr, LinkPair<R> links, const C<R> *G, C<R> *W, const Geom &g, double *partial,
                          int *nblocks, const DevState *st, LaunchStream stream, int order_tz, bool reunit, int share_mode,
                          int ahead, int minb, const SweepHalo<R> &halo) {
     const int nb = (int)((g.V + SWEEP_THREADS - 1) / SWEEP_THREADS);
     *nblocks = nb;
-    // (z, t)-tiled block order when the (x, y) plane is a whole number of CTAs; TZ: about 24 MB of traffic
-    // (1.3 kB per site in fp64 / 18-real) between a site and its t-neighbour
-    BlockOrder bo{0, 1, g.L[2], g.L[3]};
-    const long long plane = (long long)g.L[0] * g.L[1];
-    const bool beyond_l2 = (double)plane * (8.0 * 6.0 * nr + 28.0) * sizeof(R) * g.L[2] > 64.0e6;   // one t slice of traffic
-    // A'_x, A'_y through shared memory (SHARE): automatic where it measured faster on B200 -- 18-real storage,
-    // x lines that divide the CTA, and fp32 (32^4: 0.1718 -> 0.1601 ms; 64^4: 2.61 -> 2.42 ms) or a lattice beyond
-    // L2 (64^4 fp64: 4.42 -> 4.26 ms); neutral within 1.5 % otherwise, +1.7 % at 24^3 x 48.
-    const bool share = share_mode >= 0 ? share_mode != 0
-                                       : (nr == 3 && SWEEP_THREADS % g.L[0] == 0 && (sizeof(R) == 4 || beyond_l2));
-    if (order_tz != 1 && plane % SWEEP_THREADS == 0) {
-        int tz = order_tz;
-        if (tz <= 0) {
-            // automatic: only when one t slice of traffic does not fit in L2 (measured on B200: neutral at
-            // 32^4 where it fits, -4 % sweep time at 64^4 where it does not)
-            const double per_plane = (double)plane * (8.0 * 6.0 * nr + 28.0) * sizeof(R);
-            tz = 1;
-            if (beyond_l2)
-                while (tz * 2 <= g.L[2] && g.L[2] % (tz * 2) == 0 && per_plane * tz * 2 <= 24.0e6) tz *= 2;
-        }
-        if (tz > 1 && g.L[2] % tz == 0) { bo.nxy = (int)(plane / SWEEP_THREADS); bo.tz = tz; }
-    }
+    const BlockOrder bo = sweep_block_order(g, nr, (int)sizeof(R), order_tz, SWEEP_THREADS);
+    const bool share = sweep_uses_share(g, nr, (int)sizeof(R), share_mode);
 #define LGF_SWK(RU, SH, MB)                                                                              \
     if (nr == 3) return launch_pdl(k_sweep<R, 3, RU, SH, MB>, dim3(nb), dim3(SWEEP_THREADS), 0, stream, links, G, W, g, partial, st, bo, ahead, halo); \
     else return launch_pdl(k_sweep<R, 2, RU, SH, MB>, dim3(nb), dim3(SWEEP_THREADS), 0, stream, links, G, W, g, partial, st, bo, ahead, halo);

@@ -15,12 +15,39 @@
 #pragma once
 #include <cuda_runtime.h>
 
+#include <mutex>
+#include <tuple>
+#include <vector>
+
 namespace lgf {
 
 __device__ __forceinline__ void pdl_enter() {
 #if defined(__CUDA_ARCH__) && __CUDA_ARCH__ >= 900
     cudaGridDependencySynchronize();
 #endif
+}
+
+// Opt a kernel in to more than 48 KB of dynamic shared memory ONCE per (kernel, device), not on every launch: the
+// attribute call is a runtime round trip, and the small lattices are launch-bound.
+template <class K>
+cudaError_t ensure_dynamic_smem(K kern, size_t bytes) {
+    if (bytes <= 48 * 1024) return cudaSuccess;
+    static std::mutex mu;
+    static std::vector<std::tuple<const void *, int, size_t>> seen;
+    int dev = 0;
+    cudaGetDevice(&dev);
+    const void *key = reinterpret_cast<const void *>(kern);
+    std::lock_guard<std::mutex> lock(mu);
+    for (auto &e : seen)
+        if (std::get<0>(e) == key && std::get<1>(e) == dev) {
+            if (std::get<2>(e) >= bytes) return cudaSuccess;
+            const cudaError_t err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+            if (err == cudaSuccess) std::get<2>(e) = bytes;
+            return err;
+        }
+    const cudaError_t err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+    if (err == cudaSuccess) seen.emplace_back(key, dev, bytes);
+    return err;
 }
 
 // A stream plus the context's programmatic-dependent-launch setting (lgf_tune "pdl", per context).  Converts from

@@ -215,10 +215,7 @@ static cudaError_t launch_line_L(int mode, const C<R> *src, C<R> *dst, const Lin
     const size_t smem = (64 + (size_t)L * nlo) * sizeof(C<R>);
     const C<R> *tw = reinterpret_cast<const C<R> *>(twiddle);
     auto go = [&](auto kern) {
-        if (smem > 48 * 1024) {
-            cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-            if (e != cudaSuccess) return e;
-        }
+        if (cudaError_t e = ensure_dynamic_smem(kern, smem); e != cudaSuccess) return e;
         kern<<<grid, 256, smem, stream>>>(src, dst, as, ad, nlo, Lx, tw, p2tab, scale);
         return cudaGetLastError();
     };

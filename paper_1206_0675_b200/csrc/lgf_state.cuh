@@ -2,6 +2,8 @@
 // shared by the translation units of liblgf.  Part of the CUDA path; shares nothing with oracle/.
 #pragma once
 #include <cuda_runtime.h>
+
+#include <string>
 #include "lgf_su3.cuh"
 #include "lgf_pdl.cuh"
 
@@ -134,6 +136,13 @@ cudaError_t launch_heatbath(int nr, LinkPair<R> links, const Geom &g, const DevS
                             bool overrelax /* R28: alpha = (V^dag)^2, no random numbers */,
                             int order_tz /* z-planes per (z, t) tile of the thread order: 0 = automatic */);
 cudaError_t launch_reset_counters(DevState *st, LaunchStream stream);
+
+// kernel instantiations as a profiler names them (lgf_kernel_names)
+std::string fft_reg2_kernel_name(int which, const Geom &g, int prec);
+std::string sweep_kernel_name(const Geom &g, int nr, int prec, bool reunit, int share_mode, int minb);
+bool sweep_uses_share(const Geom &g, int nr, int prec, int share_mode);
+// block order of a sweep whose CTAs take `nt` consecutive sites: (z, t)-tiled when a t slice of traffic exceeds L2
+BlockOrder sweep_block_order(const Geom &g, int nr, int prec, int order_tz, int nt);
 
 // F / theta finalisation (precision independent)
 // after_sweep: the partial sums come from a sweep (flip `cur`, count the update); record: append (F, theta)

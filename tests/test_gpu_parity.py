@@ -285,6 +285,45 @@ def test_fix_pure_gauge_reaches_F1(lgf, config_cache):
     assert np.max(np.abs(to_np(d) - eye)) < 1e-6
 
 
+@pytest.mark.parametrize("storage", [18, 12])
+def test_fix_c2_iteration_count(lgf, config_cache, storage):
+    """BASELINE.json configs[1]: 16^4 fp64 to theta < 1e-15 -- the iteration count within 2 % of the oracle's
+    (north_star), the oracle's whole (F, theta) history and its final links."""
+    dims = inputs.CONFIGS["C2"]["dims"]
+    U = config_cache("C2")
+    U_o, it_o, F_o, T_o = oracle.fix(dims, U, ALPHA, 1e-15, 2000)
+    with lgf.Context(dims, 8, storage) as ctx:
+        d = to_dev(U, 8)
+        it = ctx.fix(d, ALPHA, 1e-15, 2000)
+        Fh, Th = ctx.history()
+    assert abs(it - it_o) <= max(1, round(0.02 * it_o))
+    n = min(it, it_o, 40)                      # well above the rounding floor of theta
+    assert np.max(np.abs(Fh[:n] - F_o[:n]) / np.abs(F_o[:n])) < 1e-12
+    assert np.max(np.abs(Th[:n] - T_o[:n]) / np.abs(T_o[:n])) < 1e-11
+    assert Th[it] < 1e-15 and np.all(Th[:it] >= 1e-15)
+    if it == it_o:
+        assert np.max(np.abs(to_np(d) - U_o)) < 1e-11
+
+
+def test_c2pg_golden_trajectory(lgf, config_cache):
+    """The CUDA path against the stored oracle trajectory of the pure-gauge C2 variant
+    (tests/golden/c2pg_trajectory.txt, written by tests/golden/make_golden.py from oracle/ alone)."""
+    from test_oracle_golden import read_trajectory
+
+    it_g, plaq, rows, final = read_trajectory("c2pg_trajectory.txt")
+    dims = inputs.CONFIGS["C2pg"]["dims"]
+    U = config_cache("C2pg")
+    with lgf.Context(dims, 8, 18) as ctx:
+        d = to_dev(U, 8)
+        it = ctx.fix(d, ALPHA, 1e-15, 2000)
+        Fh, Th = ctx.history()
+        _, _, P = ctx.measure()
+    for n, F, th in rows:
+        assert abs(Fh[n] - F) <= 1e-12 * abs(F) and abs(Th[n] - th) <= 1e-12 * abs(th)
+    assert abs(it - it_g) <= 1 and abs(P - plaq) < 1e-12
+    assert abs(Fh[-1] - final[1]) < 1e-12
+
+
 def test_fix_fp32_c2(lgf, config_cache):
     """fp32 runs stop at theta < 1e-12 (BASELINE.json config C2); count close to the fp64 oracle's."""
     dims = inputs.CONFIGS["C2"]["dims"]

@@ -29,7 +29,7 @@ def read_trajectory(name):
     return it, plaq, rows, final
 
 
-@pytest.mark.parametrize("name,cfg", [("c1_trajectory.txt", "C1")])
+@pytest.mark.parametrize("name,cfg", [("c1_trajectory.txt", "C1"), ("c2pg_trajectory.txt", "C2pg")])
 def test_oracle_reproduces_golden_trajectory(name, cfg):
     it, plaq, rows, final = read_trajectory(name)
     c = inputs.CONFIGS[cfg]
