@@ -48,25 +48,95 @@ def measured_peak():
         return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
 
 
-def captured_traffic(workload, precision, storage, kernel_class):
-    """DRAM bytes per launch of the dominant kernel from the committed ncu --set full capture
-    (profiles/*_traffic.csv: dram__bytes_read.sum + dram__bytes_write.sum), or None if that workload /
-    variant / kernel has not been captured.  A stored measurement, read as data; nothing here runs ncu."""
+NOMINAL_HBM_GBS = 8000.0           # north_star's "~8 TB/s" (nominal; the measured copy rate is the roofline denominator)
+KERNEL_CLASS_OF = (("k_sweep", "update"), ("k_fft", "fft"), ("k_gbuild", "gbuild"), ("k_delta", "delta"))
+
+
+def kernel_class_of(name):
+    for prefix, cls in KERNEL_CLASS_OF:
+        if ("lgf::" + prefix) in name or name.startswith(prefix) or (" " + prefix) in name:
+            return cls
+    return None
+
+
+def short_kernel_name(name):
+    """'void lgf::k_sweep<double, 3, 0, 0, 3>(lgf::LinkPair<T1>, ...)' -> 'k_sweep<double, 3, 0, 0, 3>'"""
+    n = name.replace("void ", "").replace("lgf::", "").replace("(int)", "").replace("(bool)", "")
+    depth, out = 0, []
+    for ch in n:
+        if ch == "(" and depth == 0:
+            break
+        depth += ch == "<"
+        depth -= ch == ">"
+        out.append(ch)
+    return "".join(out).strip()
+
+
+def captured_traffic(workload, precision, storage, launched):
+    """DRAM bytes per launch of the iteration's kernels from the newest committed ncu capture
+    (profiles/*_traffic.csv: dram__bytes_read.sum + dram__bytes_write.sum per launch), keyed by kernel class.
+    `launched` = {class: [instantiation names]} from lgf_kernel_names: a stored row whose kernel is not one this
+    build launches is REFUSED (listed under "stale").  A stored measurement, read as data; nothing here runs ncu."""
     import csv
     import glob
 
-    best = None
+    rows, stale = {}, []
     for path in sorted(glob.glob(os.path.join(ROOT, "profiles", "*_traffic.csv"))):
         try:
             with open(path, newline="") as f:
+                found = {}
                 for row in csv.DictReader(f):
                     if (row["workload"] == workload and row["precision"] == precision
-                            and int(row["link_storage"]) == int(storage) and row["kernel_class"] == kernel_class):
-                        best = {"bytes": float(row["dram_bytes_per_launch"]), "kernel": row["kernel"],
-                                "source": "profiles/" + os.path.basename(path)}
+                            and int(row["link_storage"]) == int(storage)):
+                        ok = any(row["kernel"].startswith(nm) for nm in launched.get(row["kernel_class"], []))
+                        rec = {"bytes": float(row["dram_bytes_per_launch"]), "kernel": row["kernel"],
+                               "launches_per_step": float(row.get("launches_per_step") or 1.0),
+                               "duration_us": float(row.get("duration_us") or 0.0),
+                               "source": "profiles/" + os.path.basename(path)}
+                        if ok:
+                            found.setdefault(row["kernel_class"], []).append(rec)
+                        else:
+                            stale.append(rec["source"] + ": " + row["kernel"])
+                if found:
+                    rows = found               # a newer file with matching rows replaces an older one
         except Exception:  # noqa: BLE001
             continue
-    return best
+    return rows, stale
+
+
+def reduce_ncu(args):
+    """--reduce-ncu FILE: an `ncu --metrics dram__bytes_read.sum,dram__bytes_write.sum,gpu__time_duration.sum --csv`
+    launch list of `bench.py --steps K ...` -> rows of a profiles/*_traffic.csv (per kernel instantiation: launches per
+    step, mean DRAM bytes and mean duration per launch over the LAST K iterations' launches)."""
+    import csv
+
+    per = {}
+    with open(args.reduce_ncu, newline="") as f:
+        lines = [ln for ln in f if ln.startswith('"')]
+    for row in csv.DictReader(lines):
+        name = short_kernel_name(row["Kernel Name"])
+        cls = kernel_class_of(name)
+        if cls is None:
+            continue
+        d = per.setdefault(int(row["ID"]), {"name": name, "cls": cls})
+        val = float(row["Metric Value"].replace(",", ""))
+        unit = row["Metric Unit"]
+        scale = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "ns": 1e-3, "us": 1.0, "ms": 1e3, "s": 1e6}.get(unit, 1.0)
+        d[row["Metric Name"]] = val * scale
+    ids = sorted(per)
+    by_name = {}
+    for i in ids:
+        by_name.setdefault(per[i]["name"], []).append(per[i])
+    print("workload,precision,link_storage,kernel_class,kernel,launches_per_step,dram_bytes_per_launch,duration_us,capture")
+    n_iter = max([len(ls) for name, ls in by_name.items() if ls[0]["cls"] == "update"] or [1])   # one sweep per iteration
+    for name, ls in by_name.items():
+        per_step = max(1, round(len(ls) / n_iter))
+        last = ls[-per_step * min(args.steps, max(1, len(ls) // per_step)):]
+        b = np.mean([x.get("dram__bytes_read.sum", 0.0) + x.get("dram__bytes_write.sum", 0.0) for x in last])
+        t = np.mean([x.get("gpu__time_duration.sum", 0.0) for x in last])
+        print("%s,%s,%d,%s,\"%s\",%d,%.0f,%.3f,%s" % (args.workload, args.precision, args.storage, ls[0]["cls"], name, per_step, b, t,
+                                                      os.path.basename(args.reduce_ncu)))
+    return 0
 
 
 class ClockSampler:
@@ -212,9 +282,41 @@ def time_variant(binding, torch, U0, dims, prec_name, storage, steps, warmup, di
         F, th, P = ctx.measure()
         out["F"], out["theta"], out["plaquette"] = F, th, P
         out["iter_bytes"] = ctx.algorithmic_bytes(binding.LGF_K_ITERATION)
+        out["kernel_names"] = ctx.kernel_names()
     del d
     torch.cuda.empty_cache()
     return out
+
+
+def time_sustained(binding, torch, U0, dims, prec_name, storage, seconds, ms_guess, index):
+    """The same step run back to back for at least `seconds` of device time (a beta = 5.8 configuration needs
+    ~10^4 iterations): the number a long fix sees once the board settles at its power cap."""
+    prec = PREC[prec_name]
+    cdt = torch.complex128 if prec == 8 else torch.complex64
+    stream = torch.cuda.current_stream()
+    sampler = ClockSampler(index, period=0.05)
+    with binding.Context(dims, prec, storage, stream=stream) as ctx:
+        apply_tune(ctx)
+        d = torch.from_numpy(U0).to(cdt).cuda()
+        ctx.set_links(d)
+        chunk = max(50, int(0.25 * 1e3 / ms_guess))        # about a quarter of a second per call
+        ctx.iterate(ALPHA, chunk)
+        torch.cuda.synchronize()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        n, t0 = 0, time.perf_counter()
+        with sampler:
+            a.record(stream)
+            while True:
+                ctx.iterate(ALPHA, chunk)
+                n += chunk
+                if time.perf_counter() - t0 > seconds and n * ms_guess * 1e-3 > 0.8 * seconds:
+                    break
+            b.record(stream)
+            torch.cuda.synchronize()
+        ms = a.elapsed_time(b)
+    del d
+    torch.cuda.empty_cache()
+    return {"seconds": ms * 1e-3, "steps": n, "ms_per_step": ms / n, "value": 1e3 * n / ms, "unit": UNIT, "clocks": sampler.summary()}
 
 
 def time_e2e(binding, torch, U0, dims, prec_name, storage, tol, max_iter, dist):
@@ -523,12 +625,18 @@ def main():
     ap.add_argument("--shard", type=int, default=0, metavar="K",
                     help="ONE configuration sharded over t-slabs: K emulated ranks in a single process; under torchrun the "
                          "ranks are the processes (any K > 0)")
+    ap.add_argument("--sustained-seconds", type=float, default=5.0,
+                    help="also run the step back to back for this long (device time) and report it as `sustained` (0 = skip)")
+    ap.add_argument("--reduce-ncu", default=None, metavar="CSV",
+                    help="turn an ncu --csv launch list of this script (dram bytes + duration metrics) into profiles/*_traffic.csv rows")
     ap.add_argument("--mixed", action="store_true", help="--thermal (fp64 only): also time fp32 iterations + fp64 polish")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)
     for kv in [x for x in args.tune.split(",") if x]:
         k, v = kv.split("=")
         TUNE[k.strip()] = int(v)
+    if args.reduce_ncu:
+        return reduce_ncu(args)
     if args.impl == "reference":
         return run_reference(args)
     if args.thermal is not None:
@@ -577,16 +685,32 @@ def main():
     dk = hot[dom]
     bytes_per_launch = dk["algorithmic_bytes_per_step"] / dk["launches_per_step"]
     achieved = bytes_per_launch / (dk["avg_launch_us"] * 1e-6) / 1e9
-    cap = captured_traffic(args.workload, args.precision, args.storage, dom)
+    caps, stale = captured_traffic(args.workload, args.precision, args.storage, head["kernel_names"])
+    cap = (caps.get(dom) or [None])[0]
+    # whole iteration in REAL DRAM bytes: the ncu capture of every kernel of one iteration, summed
+    dram_iter = sum(r["bytes"] * r["launches_per_step"] for rows in caps.values() for r in rows) if caps else None
+    complete = bool(caps) and all(k in caps for k in hot)
+    yard = head["iter_bytes"] / (head["ms_per_step"] * 1e-3) / 1e9
     roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "traffic": cap["bytes"] if cap else None,
-                "traffic_source": cap["source"] if cap else None, "peak_source": peak_src,
+                "frac": achieved / peak, "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS,
+                "traffic": cap["bytes"] if cap else None,
+                "traffic_source": cap["source"] if cap else None, "traffic_kernel": cap["kernel"] if cap else None,
+                "stale_captures_refused": stale[:8], "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": bytes_per_launch, "avg_launch_us": dk["avg_launch_us"],
-                "iteration": {"algorithmic_bytes": head["iter_bytes"],
-                              "achieved": head["iter_bytes"] / (head["ms_per_step"] * 1e-3) / 1e9,
-                              "frac": head["iter_bytes"] / (head["ms_per_step"] * 1e-3) / 1e9 / peak},
+                "launched_kernels": head["kernel_names"],
+                "iteration": {"yardstick_bytes": head["iter_bytes"], "yardstick_rate": yard, "yardstick_frac": yard / peak,
+                              "yardstick_note": "SURVEY 8(d) UNFUSED budget (12 n_l + 64 reals/site) / time: an effective rate, "
+                                                "not DRAM traffic -- the fused path moves fewer bytes",
+                              "dram_bytes": dram_iter if complete else None,
+                              "dram_rate": dram_iter / (head["ms_per_step"] * 1e-3) / 1e9 if complete else None,
+                              "dram_frac": dram_iter / (head["ms_per_step"] * 1e-3) / 1e9 / peak if complete else None,
+                              "dram_frac_of_nominal_8TBs": dram_iter / (head["ms_per_step"] * 1e-3) / 1e9 / NOMINAL_HBM_GBS if complete else None,
+                              "dram_note": "sum over the iteration's kernels of ncu dram__bytes_read + write per launch "
+                                           "(committed capture, cold L2 per kernel) / this run's ms_per_step"},
                 "kernels": {k: {"ms_per_step": round(v["ms_per_step"], 6), "launches_per_step": v["launches_per_step"],
-                                "gbs": v["gbs"], "frac": v["gbs"] / peak} for k, v in hot.items()}}
+                                "algorithmic_gbs": v["gbs"], "algorithmic_frac": v["gbs"] / peak,
+                                "dram_bytes_per_step": (sum(r["bytes"] * r["launches_per_step"] for r in caps[k]) if k in caps else None)}
+                            for k, v in hot.items()}}
 
     variants = {}
     if not args.no_variants:
@@ -597,10 +721,18 @@ def main():
                 else:
                     r = time_variant(binding, torch, U0, dims, pn, st, args.steps, args.warmup, dist)
                 gbs = r["iter_bytes"] / (r["ms_per_step"] * 1e-3) / 1e9
+                vcaps, _ = captured_traffic(args.workload, pn, st, r["kernel_names"])
+                vhot = [k for k in r["kernels"] if k in ("delta", "fft", "update", "gbuild")]
+                vdram = (sum(x["bytes"] * x["launches_per_step"] for rows in vcaps.values() for x in rows)
+                         if vcaps and all(k in vcaps for k in vhot) else None)
                 variants["%s/%d" % (pn, st)] = {"iterations_per_s": world * 1e3 / r["ms_per_step"],
                                                 "site_updates_per_s": world * V * 1e3 / r["ms_per_step"],
-                                                "ms_per_step": r["ms_per_step"], "algorithmic_gbs": gbs,
-                                                "frac_of_peak": gbs / peak}
+                                                "ms_per_step": r["ms_per_step"], "yardstick_gbs": gbs,
+                                                "yardstick_frac": gbs / peak,
+                                                "dram_bytes_per_step": vdram,
+                                                "dram_frac": vdram / (r["ms_per_step"] * 1e-3) / 1e9 / peak if vdram else None,
+                                                "update_ms": r["kernels"].get("update", {}).get("ms_per_step"),
+                                                "fft_ms": r["kernels"].get("fft", {}).get("ms_per_step")}
 
     e2e = None
     if not args.no_e2e:
@@ -613,6 +745,13 @@ def main():
                "h2d_bytes_per_step": r["bytes_each_way"] / its, "d2h_bytes_per_step": r["bytes_each_way"] / its,
                "call": "lgf_fix_host(pinned host links, alpha=0.08, tol=%g, max_iter=%d): H2D + %d iterations + D2H in %.1f ms"
                        % (tol, max_iter, r["iterations"], r["ms"]), "final_theta": r["theta"]}
+
+    sustained = None
+    if world == 1 and args.sustained_seconds > 0:
+        sustained = time_sustained(binding, torch, U0, dims, args.precision, args.storage, args.sustained_seconds,
+                                   head["ms_per_step"], physical_gpu_index(local))
+        if roofline["iteration"]["dram_bytes"]:
+            sustained["dram_frac"] = roofline["iteration"]["dram_bytes"] / (sustained["ms_per_step"] * 1e-3) / 1e9 / peak
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
@@ -627,6 +766,7 @@ def main():
                            "l2": "inputs larger than L2: one step streams %.0f MB of links and fields"
                                  % (head["iter_bytes"] / 1e6)},
                 "site_updates_per_s": value * V, "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e,
+                "sustained": sustained,
                 "gpu_launches": head["launches"], "clocks": sampler.summary(), "remeasured": head.get("remeasured"),
                 "variants": variants,
                 "state_after_timing": {"F": head["F"], "theta": head["theta"], "plaquette": head["plaquette"]}}

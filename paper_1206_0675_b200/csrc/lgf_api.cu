@@ -37,6 +37,7 @@ struct lgf_ctx {
     double *d_scalar = nullptr;
     void *twiddle[4] = {nullptr, nullptr, nullptr, nullptr};   // C<R>[64] per axis, exp(-2 pi i m / L_mu)
     void *p2tab = nullptr;                                     // R[4][64]
+    SweepMaps *sweep_maps = nullptr;   // TMA tensor maps of the staged sweep (lgf_sweep_tma.cu); null = k_sweep only
     void *staging = nullptr;     // canonical-layout device buffer for the *_host entry points
     std::vector<AxisPass> passes;
     unsigned long long hb_sweeps = 0;   // heat-bath sweeps applied since the last set_links (selects the random stream)
@@ -54,6 +55,8 @@ struct lgf_ctx {
     int tune_reunit = 0;         // lgf_tune "reunit_every": project the new links onto SU(3) in every N-th update (0 = never)
     long long updates_enqueued = 0;   // host-side count of updates enqueued since the last set_links / thermalize
     int tune_pdl = 1;            // lgf_tune "pdl": launch the iteration's kernels with programmatic stream serialization
+    int tune_sweep_tma = -1;     // lgf_tune "sweep_tma" (see use_sweep_tma)
+    int tune_sweep_rsplit = 1;   // lgf_tune "sweep_rsplit": register split between producer and compute warps (fp64 staged sweep)
     int tune_sweep_ahead = 0;    // lgf_tune "sweep_prefetch": CTAs ahead of which the sweep prefetches its tile into L2 (0 = off)
     int tune_sweep_minb = 3;     // lgf_tune "sweep_minb": resident CTAs per SM the sweep's register allocation allows (3 / 2)
     int tune_sweep_tz = 0;       // lgf_tune: z-planes per (z, t) tile of the sweep's block order (0 = automatic, 1 = plain)
@@ -368,6 +371,11 @@ static int step_accelerate(lgf_ctx *ctx, bool with_g = false, double alpha = 0.0
     }
     return LGF_OK;
 }
+// the staged (TMA) sweep or the register sweep?  "sweep_tma": 1 = wherever it applies, 0 = never, -1 = where it
+// measured faster than k_sweep on B200 (12-real storage; lgf_sweep_tma.cu has the numbers)
+static bool use_sweep_tma(const lgf_ctx *ctx) {
+    return ctx->sweep_maps && (ctx->tune_sweep_tma > 0 || (ctx->tune_sweep_tma < 0 && ctx->nr == 2));
+}
 // a5 then a6 + a1: g from the current W, then the fused sweep (new links into the other buffer, Delta of
 // the new links into W, partial sums of F and theta)
 static int step_finalize(lgf_ctx *ctx, double tol, int after_sweep, int record) {
@@ -390,7 +398,12 @@ static int step_update(lgf_ctx *ctx, double alpha, double tol, int record, bool 
     }
     ctx->updates_enqueued++;
     const bool reunit = ctx->tune_reunit > 0 && ctx->updates_enqueued % ctx->tune_reunit == 0;
-    {
+    if (use_sweep_tma(ctx)) {
+        Bracket br(ctx, LGF_K_UPDATE);
+        CK(launch_sweep_tma<R>(ctx->sweep_maps, ctx->nr, link_pair<R>(ctx), (const C<R> *)ctx->G, (C<R> *)ctx->W, ctx->g, ctx->partial,
+                               &ctx->nb_partial, ctx->st, STRM(ctx), ctx->tune_sweep_tz, reunit, SweepHalo<R>(),
+                               ctx->tune_sweep_rsplit != 0));
+    } else {
         Bracket br(ctx, LGF_K_UPDATE);
         CK(launch_sweep<R>(ctx->nr, link_pair<R>(ctx), (const C<R> *)ctx->G, (C<R> *)ctx->W, ctx->g, ctx->partial,
                            &ctx->nb_partial, ctx->st, STRM(ctx), ctx->tune_sweep_tz, reunit, ctx->tune_sweep_share,
@@ -543,6 +556,7 @@ int lgf_create(const int dims[4], int precision, int link_storage, lgf_ctx **out
     }
     if (rc == LGF_OK) rc = precision == LGF_FP64 ? upload_twiddles<double>(ctx) : upload_twiddles<float>(ctx);
     if (rc == LGF_OK) rc = plan_passes(ctx);
+    if (rc == LGF_OK) ctx->sweep_maps = sweep_tma_maps_create(ctx->g, ctx->nr, ctx->prec, ctx->links[0], ctx->links[1], ctx->G);
     if (rc == LGF_OK) {
         cudaError_t ee = launch_reset_state(ctx->st, STRM(ctx));
         if (ee == cudaSuccess) ee = cudaStreamSynchronize(ctx->stream);
@@ -573,6 +587,7 @@ int lgf_destroy(lgf_ctx *ctx) {
     cudaFree(ctx->d_scalar);
     cudaFree(ctx->p2tab);
     cudaFree(ctx->staging);
+    sweep_tma_maps_destroy(ctx->sweep_maps);
     for (int mu = 0; mu < 4; mu++) cudaFree(ctx->twiddle[mu]);
     if (ctx->h_st) cudaFreeHost(ctx->h_st);
     if (ctx->h_poll) cudaFreeHost(ctx->h_poll);
@@ -958,6 +973,8 @@ int lgf_tune(lgf_ctx *ctx, const char *key, int value) {
     else if (k == "sweep_tz") ctx->tune_sweep_tz = value;
     else if (k == "hb_tz") ctx->tune_hb_tz = value;
     else if (k == "sweep_share") ctx->tune_sweep_share = value;
+    else if (k == "sweep_tma") ctx->tune_sweep_tma = value;
+    else if (k == "sweep_rsplit") ctx->tune_sweep_rsplit = value;
     else if (k == "sweep_prefetch") ctx->tune_sweep_ahead = value < 0 ? 0 : value;
     else if (k == "sweep_minb") ctx->tune_sweep_minb = value == 2 ? 2 : 3;
     else if (k == "reunit_every") ctx->tune_reunit = value < 0 ? 0 : value;
@@ -992,7 +1009,9 @@ int lgf_kernel_times(lgf_ctx *ctx, double *ms, long long *launches) {
 
 int lgf_kernel_names(const lgf_ctx *ctx, char *buf, int cap) {
     if (!ctx || !buf || cap <= 0) return LGF_EINVAL;
-    std::string s = "update=" + sweep_kernel_name(ctx->g, ctx->nr, ctx->prec, false, ctx->tune_sweep_share, ctx->tune_sweep_minb) + ";fft=";
+    std::string s = "update=" + (use_sweep_tma(ctx) ? sweep_tma_kernel_name(ctx->g, ctx->nr, ctx->prec, false, ctx->tune_sweep_rsplit != 0)
+                                                  : sweep_kernel_name(ctx->g, ctx->nr, ctx->prec, false, ctx->tune_sweep_share,
+                                                                      ctx->tune_sweep_minb)) + ";fft=";
     const bool fuse = can_fuse_g(ctx);
     for (size_t i = 0; i < ctx->passes.size(); i++) {
         const AxisPass &p = ctx->passes[i];

@@ -137,6 +137,17 @@ cudaError_t launch_heatbath(int nr, LinkPair<R> links, const Geom &g, const DevS
                             int order_tz /* z-planes per (z, t) tile of the thread order: 0 = automatic */);
 cudaError_t launch_reset_counters(DevState *st, LaunchStream stream);
 
+// the staged sweep (lgf_sweep_tma.cu): TMA tensor copies into a shared-memory ring, persistent warp-specialised CTAs
+bool sweep_tma_supported(const Geom &g, int nr, int prec);
+struct SweepMaps;     // the TMA tensor maps over a context's two link buffers and its g field
+SweepMaps *sweep_tma_maps_create(const Geom &g, int nr, int prec, void *links0, void *links1, void *G);   // null: does not apply
+void sweep_tma_maps_destroy(SweepMaps *m);
+template <class R>
+cudaError_t launch_sweep_tma(const SweepMaps *maps, int nr, LinkPair<R> links, const C<R> *G, C<R> *W, const Geom &g, double *partial,
+                             int *nblocks, const DevState *st, LaunchStream stream, int order_tz, bool reunit, const SweepHalo<R> &halo,
+                             bool rsplit = true /* fp64: move the producer warps' registers to the compute warps (setmaxnreg) */);
+std::string sweep_tma_kernel_name(const Geom &g, int nr, int prec, bool reunit, bool rsplit);
+
 // kernel instantiations as a profiler names them (lgf_kernel_names)
 std::string fft_reg2_kernel_name(int which, const Geom &g, int prec);
 std::string sweep_kernel_name(const Geom &g, int nr, int prec, bool reunit, int share_mode, int minb);

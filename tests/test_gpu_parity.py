@@ -223,6 +223,34 @@ def test_trajectory_shared_neighbour_sweep(lgf, config_cache, name, dims, prec, 
     assert np.max(np.abs(out - U_o)) < tol["links"]
 
 
+@pytest.mark.parametrize("name,dims", [("C1", (8, 8, 8, 8)), ("x24", (24, 12, 4, 6)), ("x16", (16, 8, 6, 4)), ("x64", (64, 4, 4, 2)),
+                                       ("C2", (16, 16, 16, 16))])
+@pytest.mark.parametrize("prec,storage", VARIANTS)
+def test_trajectory_staged_sweep(lgf, config_cache, name, dims, prec, storage):
+    """lgf_tune("sweep_tma", 1): the persistent sweep fed by TMA tensor copies through a shared-memory ring
+    (lgf_sweep_tma.cu) in every precision x storage variant -- tiles of 2 x 64, 4 x 24, 8 x 16 and 8 x 8 sites, tiles
+    that are a whole (x, y) plane, with and without the fp64 register split.  Same parity bar as the default sweep;
+    and the run is repeated: the new links must be the same bit for bit (the kernel once handed a ring slot back
+    while its loads were still in flight)."""
+    import torch
+
+    U = config_cache("C2") if name == "C2" else small_config(name, dims)
+    n = 12
+    U_o, F_o, T_o = oracle.iterate(dims, U, ALPHA, n)
+    tol = TOL[prec]
+    outs = []
+    for rsplit in (1, 0, 1):
+        Fh, Th, P, out = run_trajectory(lgf, dims, U, prec, storage, n, tune={"sweep_tma": 1, "sweep_rsplit": rsplit})
+        assert np.max(np.abs(Fh - F_o) / np.abs(F_o)) < tol["scalar"]
+        assert np.max(np.abs(Th - T_o) / np.abs(T_o)) < tol["scalar"]
+        assert np.max(np.abs(out - U_o)) < tol["links"]
+        outs.append(out)
+    assert np.array_equal(outs[0], outs[2])
+    with lgf.Context(dims, prec, storage) as ctx:
+        ctx.tune("sweep_tma", 1)
+        assert ctx.kernel_names()["update"][0].startswith("k_sweep_tma<")     # the lattice does take the staged sweep
+
+
 @pytest.mark.parametrize("prec,storage", VARIANTS)
 def test_trajectory_time_extent_twice_the_spatial_one(lgf, prec, storage):
     """16^3 x 32 -- the usual shape of a lattice QCD volume (the paper tunes on 32^3 x n): 20
