@@ -688,7 +688,7 @@ def main():
     caps, stale = captured_traffic(args.workload, args.precision, args.storage, head["kernel_names"])
     cap = (caps.get(dom) or [None])[0]
     # whole iteration in REAL DRAM bytes: the ncu capture of every kernel of one iteration, summed
-    dram_iter = sum(r["bytes"] * r["launches_per_step"] for rows in caps.values() for r in rows) if caps else None
+    dram_iter = sum(r["bytes"] * r["launches_per_step"] for k in hot for r in caps.get(k, [])) if caps else None
     complete = bool(caps) and all(k in caps for k in hot)
     yard = head["iter_bytes"] / (head["ms_per_step"] * 1e-3) / 1e9
     roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
@@ -723,7 +723,7 @@ def main():
                 gbs = r["iter_bytes"] / (r["ms_per_step"] * 1e-3) / 1e9
                 vcaps, _ = captured_traffic(args.workload, pn, st, r["kernel_names"])
                 vhot = [k for k in r["kernels"] if k in ("delta", "fft", "update", "gbuild")]
-                vdram = (sum(x["bytes"] * x["launches_per_step"] for rows in vcaps.values() for x in rows)
+                vdram = (sum(x["bytes"] * x["launches_per_step"] for k in vhot for x in vcaps[k])
                          if vcaps and all(k in vcaps for k in vhot) else None)
                 variants["%s/%d" % (pn, st)] = {"iterations_per_s": world * 1e3 / r["ms_per_step"],
                                                 "site_updates_per_s": world * V * 1e3 / r["ms_per_step"],

@@ -38,7 +38,12 @@ struct lgf_ctx {
     void *twiddle[4] = {nullptr, nullptr, nullptr, nullptr};   // C<R>[64] per axis, exp(-2 pi i m / L_mu)
     void *p2tab = nullptr;                                     // R[4][64]
     SweepMaps *sweep_maps = nullptr;   // TMA tensor maps of the staged sweep (lgf_sweep_tma.cu); null = k_sweep only
-    void *staging = nullptr;     // canonical-layout device buffer for the *_host entry points
+    // the *_host entry points: two chunk buffers in canonical layout, a copy stream and events, so that the PCIe copy of
+    // chunk k + 1 overlaps the layout conversion of chunk k (no configuration-sized staging buffer)
+    void *stage[2] = {nullptr, nullptr};
+    long long stage_sites = 0;
+    cudaStream_t copy_stream = nullptr;
+    cudaEvent_t ev_full[2] = {nullptr, nullptr}, ev_free[2] = {nullptr, nullptr}, ev_start = nullptr;
     std::vector<AxisPass> passes;
     unsigned long long hb_sweeps = 0;   // heat-bath sweeps applied since the last set_links (selects the random stream)
     bool have_links = false;
@@ -372,9 +377,9 @@ static int step_accelerate(lgf_ctx *ctx, bool with_g = false, double alpha = 0.0
     return LGF_OK;
 }
 // the staged (TMA) sweep or the register sweep?  "sweep_tma": 1 = wherever it applies, 0 = never, -1 = where it
-// measured faster than k_sweep on B200 (12-real storage; lgf_sweep_tma.cu has the numbers)
+// measured faster than k_sweep on B200 (sweep_tma_auto, lgf_sweep_tma.cu, has the numbers)
 static bool use_sweep_tma(const lgf_ctx *ctx) {
-    return ctx->sweep_maps && (ctx->tune_sweep_tma > 0 || (ctx->tune_sweep_tma < 0 && ctx->nr == 2));
+    return ctx->sweep_maps && (ctx->tune_sweep_tma > 0 || (ctx->tune_sweep_tma < 0 && sweep_tma_auto(ctx->g, ctx->nr, ctx->prec)));
 }
 // a5 then a6 + a1: g from the current W, then the fused sweep (new links into the other buffer, Delta of
 // the new links into W, partial sums of F and theta)
@@ -586,7 +591,14 @@ int lgf_destroy(lgf_ctx *ctx) {
     cudaFree(ctx->hist);
     cudaFree(ctx->d_scalar);
     cudaFree(ctx->p2tab);
-    cudaFree(ctx->staging);
+    cudaFree(ctx->stage[0]);
+    cudaFree(ctx->stage[1]);
+    if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
+    for (int k = 0; k < 2; k++) {
+        if (ctx->ev_full[k]) cudaEventDestroy(ctx->ev_full[k]);
+        if (ctx->ev_free[k]) cudaEventDestroy(ctx->ev_free[k]);
+    }
+    if (ctx->ev_start) cudaEventDestroy(ctx->ev_start);
     sweep_tma_maps_destroy(ctx->sweep_maps);
     for (int mu = 0; mu < 4; mu++) cudaFree(ctx->twiddle[mu]);
     if (ctx->h_st) cudaFreeHost(ctx->h_st);
@@ -605,6 +617,25 @@ int lgf_set_stream(lgf_ctx *ctx, void *cuda_stream) {
     return LGF_OK;
 }
 
+// after the internal link buffer 0 has been filled: accumulated transformation, state and host-side flags start again
+static int links_loaded(lgf_ctx *ctx) {
+    if (ctx->Gacc) {
+        ctx->launches++;
+        if (ctx->prec == LGF_FP64)
+            CK(launch_gacc<double>(0, nullptr, (C<double> *)ctx->Gacc, nullptr, ctx->g, ctx->st, STRM(ctx)));
+        else
+            CK(launch_gacc<float>(0, nullptr, (C<float> *)ctx->Gacc, nullptr, ctx->g, ctx->st, STRM(ctx)));
+    }
+    ctx->launches++;
+    CK(launch_reset_state(ctx->st, STRM(ctx)));          // also makes buffer 0 the current one
+    ctx->have_links = true;
+    ctx->w_is_delta = false;
+    ctx->recorded = false;
+    ctx->hb_sweeps = 0;
+    ctx->updates_enqueued = 0;
+    return LGF_OK;
+}
+
 int lgf_set_links(lgf_ctx *ctx, const void *d_links) {
     if (!ctx || !d_links) return fail(ctx, LGF_EINVAL, "lgf_set_links: null argument");
     ENTER(ctx);
@@ -615,21 +646,7 @@ int lgf_set_links(lgf_ctx *ctx, const void *d_links) {
         else
             CK(launch_convert_in<float>(ctx->nr, (const float *)d_links, (C<float> *)ctx->links[0], ctx->g, STRM(ctx)));
     }
-    if (ctx->Gacc) {
-        ctx->launches++;
-        if (ctx->prec == LGF_FP64)
-            CK(launch_gacc<double>(0, nullptr, (C<double> *)ctx->Gacc, nullptr, ctx->g, ctx->st, STRM(ctx)));
-        else
-            CK(launch_gacc<float>(0, nullptr, (C<float> *)ctx->Gacc, nullptr, ctx->g, ctx->st, STRM(ctx)));
-    }
-    ctx->launches++;
-    CK(launch_reset_state(ctx->st, STRM(ctx)));        // also makes buffer 0 the current one
-    ctx->have_links = true;
-    ctx->w_is_delta = false;
-    ctx->recorded = false;
-    ctx->hb_sweeps = 0;
-    ctx->updates_enqueued = 0;
-    return LGF_OK;
+    return links_loaded(ctx);
 }
 
 int lgf_get_links(lgf_ctx *ctx, void *d_links) {
@@ -645,7 +662,16 @@ int lgf_get_links(lgf_ctx *ctx, void *d_links) {
 }
 
 static int ensure_staging(lgf_ctx *ctx) {
-    if (!ctx->staging) CK(cudaMalloc(&ctx->staging, (size_t)ctx->g.V * 72 * ctx->prec));
+    if (ctx->stage[0]) return LGF_OK;
+    const long long CH = 1LL << 16;                        // sites per chunk: 37.7 MB in fp64
+    ctx->stage_sites = ctx->g.V < CH ? ctx->g.V : CH;
+    for (int k = 0; k < 2; k++) {
+        CK(cudaMalloc(&ctx->stage[k], (size_t)ctx->stage_sites * 72 * ctx->prec));
+        CK(cudaEventCreateWithFlags(&ctx->ev_full[k], cudaEventDisableTiming));
+        CK(cudaEventCreateWithFlags(&ctx->ev_free[k], cudaEventDisableTiming));
+    }
+    CK(cudaEventCreateWithFlags(&ctx->ev_start, cudaEventDisableTiming));
+    CK(cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking));
     return LGF_OK;
 }
 
@@ -654,8 +680,28 @@ int lgf_set_links_host(lgf_ctx *ctx, const void *h_links) {
     ENTER(ctx);
     int rc = ensure_staging(ctx);
     if (rc != LGF_OK) return rc;
-    CK(cudaMemcpyAsync(ctx->staging, h_links, (size_t)ctx->g.V * 72 * ctx->prec, cudaMemcpyHostToDevice, ctx->stream));
-    rc = lgf_set_links(ctx, ctx->staging);
+    const size_t site_bytes = (size_t)72 * ctx->prec;
+    CK(cudaEventRecord(ctx->ev_start, ctx->stream));       // the copies start after whatever the stream still does
+    CK(cudaStreamWaitEvent(ctx->copy_stream, ctx->ev_start, 0));
+    int c = 0;
+    for (long long s0 = 0; s0 < ctx->g.V; s0 += ctx->stage_sites, c++) {
+        const int b = c & 1;
+        const long long n = ctx->g.V - s0 < ctx->stage_sites ? ctx->g.V - s0 : ctx->stage_sites;
+        if (c >= 2) CK(cudaStreamWaitEvent(ctx->copy_stream, ctx->ev_free[b], 0));     // its conversion has read the buffer
+        CK(cudaMemcpyAsync(ctx->stage[b], (const char *)h_links + (size_t)s0 * site_bytes, (size_t)n * site_bytes,
+                           cudaMemcpyHostToDevice, ctx->copy_stream));
+        CK(cudaEventRecord(ctx->ev_full[b], ctx->copy_stream));
+        CK(cudaStreamWaitEvent(ctx->stream, ctx->ev_full[b], 0));
+        {
+            Bracket br(ctx, LGF_K_CONVERT);
+            if (ctx->prec == LGF_FP64)
+                CK(launch_convert_in<double>(ctx->nr, (const double *)ctx->stage[b], (C<double> *)ctx->links[0], ctx->g, STRM(ctx), s0, n));
+            else
+                CK(launch_convert_in<float>(ctx->nr, (const float *)ctx->stage[b], (C<float> *)ctx->links[0], ctx->g, STRM(ctx), s0, n));
+        }
+        CK(cudaEventRecord(ctx->ev_free[b], ctx->stream));
+    }
+    rc = links_loaded(ctx);
     if (rc != LGF_OK) return rc;
     CK(cudaStreamSynchronize(ctx->stream));
     return LGF_OK;
@@ -663,12 +709,30 @@ int lgf_set_links_host(lgf_ctx *ctx, const void *h_links) {
 
 int lgf_get_links_host(lgf_ctx *ctx, void *h_links) {
     if (!ctx || !h_links) return fail(ctx, LGF_EINVAL, "lgf_get_links_host: null argument");
+    if (!ctx->have_links) return fail(ctx, LGF_ESTATE, "lgf_get_links_host: no configuration loaded");
     ENTER(ctx);
     int rc = ensure_staging(ctx);
     if (rc != LGF_OK) return rc;
-    rc = lgf_get_links(ctx, ctx->staging);
-    if (rc != LGF_OK) return rc;
-    CK(cudaMemcpyAsync(h_links, ctx->staging, (size_t)ctx->g.V * 72 * ctx->prec, cudaMemcpyDeviceToHost, ctx->stream));
+    const size_t site_bytes = (size_t)72 * ctx->prec;
+    int c = 0;
+    for (long long s0 = 0; s0 < ctx->g.V; s0 += ctx->stage_sites, c++) {
+        const int b = c & 1;
+        const long long n = ctx->g.V - s0 < ctx->stage_sites ? ctx->g.V - s0 : ctx->stage_sites;
+        if (c >= 2) CK(cudaStreamWaitEvent(ctx->stream, ctx->ev_free[b], 0));          // its copy has left the buffer
+        {
+            Bracket br(ctx, LGF_K_CONVERT);
+            if (ctx->prec == LGF_FP64)
+                CK(launch_convert_out<double>(ctx->nr, link_pair<double>(ctx), (double *)ctx->stage[b], ctx->g, ctx->st, STRM(ctx), s0, n));
+            else
+                CK(launch_convert_out<float>(ctx->nr, link_pair<float>(ctx), (float *)ctx->stage[b], ctx->g, ctx->st, STRM(ctx), s0, n));
+        }
+        CK(cudaEventRecord(ctx->ev_full[b], ctx->stream));
+        CK(cudaStreamWaitEvent(ctx->copy_stream, ctx->ev_full[b], 0));
+        CK(cudaMemcpyAsync((char *)h_links + (size_t)s0 * site_bytes, ctx->stage[b], (size_t)n * site_bytes, cudaMemcpyDeviceToHost,
+                           ctx->copy_stream));
+        CK(cudaEventRecord(ctx->ev_free[b], ctx->copy_stream));
+    }
+    CK(cudaStreamSynchronize(ctx->copy_stream));
     CK(cudaStreamSynchronize(ctx->stream));
     return LGF_OK;
 }

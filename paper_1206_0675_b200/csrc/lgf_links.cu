@@ -404,12 +404,14 @@ __global__ void k_clear_done(DevState *st) { st->done = 0; }
 
 // ---- layout conversion ----------------------------------------------------------------------------
 // canonical: canon[((s*4 + mu)*9 + e)*2 + re/im]      (include/lgf.h)
+// `canon` holds the n sites s0 .. s0 + n - 1 (a chunk of the configuration, or all of it)
 template <class R, int NR>
 __global__ void __launch_bounds__(SITE_THREADS) k_convert_in(const R *__restrict__ canon, C<R> *__restrict__ links,
-                                                              Geom g) {
-    const long long s = (long long)blockIdx.x * SITE_THREADS + threadIdx.x;
-    if (s >= g.V) return;
-    const C<R> *src = reinterpret_cast<const C<R> *>(canon) + s * 36;
+                                                              Geom g, long long s0, long long n) {
+    const long long i = (long long)blockIdx.x * SITE_THREADS + threadIdx.x;
+    if (i >= n) return;
+    const long long s = s0 + i;
+    const C<R> *src = reinterpret_cast<const C<R> *>(canon) + i * 36;
 #pragma unroll
     for (int mu = 0; mu < 4; mu++)
 #pragma unroll
@@ -417,11 +419,12 @@ __global__ void __launch_bounds__(SITE_THREADS) k_convert_in(const R *__restrict
 }
 template <class R, int NR>
 __global__ void __launch_bounds__(SITE_THREADS) k_convert_out(LinkPair<R> lp, R *__restrict__ canon, Geom g,
-                                                               const DevState *__restrict__ st) {
-    const C<R> *__restrict__ links = lp.buf[st->cur];
-    const long long s = (long long)blockIdx.x * SITE_THREADS + threadIdx.x;
-    if (s >= g.V) return;
-    C<R> *dst = reinterpret_cast<C<R> *>(canon) + s * 36;
+                                                               const DevState *__restrict__ st, long long s0, long long n) {
+    const C<R> *__restrict__ links = st->cur ? lp.buf[1] : lp.buf[0];
+    const long long i = (long long)blockIdx.x * SITE_THREADS + threadIdx.x;
+    if (i >= n) return;
+    const long long s = s0 + i;
+    C<R> *dst = reinterpret_cast<C<R> *>(canon) + i * 36;
 #pragma unroll
     for (int mu = 0; mu < 4; mu++) {
         C<R> u[9];
@@ -546,18 +549,20 @@ cudaError_t launch_plaquette(int nr, LinkPair<R> links, const Geom &g, double *p
     return cudaGetLastError();
 }
 template <class R>
-cudaError_t launch_convert_in(int nr, const R *canon, C<R> *links0, const Geom &g, LaunchStream stream) {
-    const int nb = site_blocks(g);
-    if (nr == 3) k_convert_in<R, 3><<<nb, SITE_THREADS, 0, stream>>>(canon, links0, g);
-    else k_convert_in<R, 2><<<nb, SITE_THREADS, 0, stream>>>(canon, links0, g);
+cudaError_t launch_convert_in(int nr, const R *canon, C<R> *links0, const Geom &g, LaunchStream stream, long long s0, long long n) {
+    if (n < 0) n = g.V - s0;
+    const int nb = (int)((n + SITE_THREADS - 1) / SITE_THREADS);
+    if (nr == 3) k_convert_in<R, 3><<<nb, SITE_THREADS, 0, stream>>>(canon, links0, g, s0, n);
+    else k_convert_in<R, 2><<<nb, SITE_THREADS, 0, stream>>>(canon, links0, g, s0, n);
     return cudaGetLastError();
 }
 template <class R>
 cudaError_t launch_convert_out(int nr, LinkPair<R> links, R *canon, const Geom &g, const DevState *st,
-                               LaunchStream stream) {
-    const int nb = site_blocks(g);
-    if (nr == 3) k_convert_out<R, 3><<<nb, SITE_THREADS, 0, stream>>>(links, canon, g, st);
-    else k_convert_out<R, 2><<<nb, SITE_THREADS, 0, stream>>>(links, canon, g, st);
+                               LaunchStream stream, long long s0, long long n) {
+    if (n < 0) n = g.V - s0;
+    const int nb = (int)((n + SITE_THREADS - 1) / SITE_THREADS);
+    if (nr == 3) k_convert_out<R, 3><<<nb, SITE_THREADS, 0, stream>>>(links, canon, g, st, s0, n);
+    else k_convert_out<R, 2><<<nb, SITE_THREADS, 0, stream>>>(links, canon, g, st, s0, n);
     return cudaGetLastError();
 }
 template <class R>
@@ -620,8 +625,8 @@ cudaError_t launch_clear_done(DevState *st, LaunchStream stream) {
                                          const DevState *, LaunchStream, int, bool, int, int, int, const SweepHalo<R> &);                                   \
     template cudaError_t launch_plaquette<R>(int, LinkPair<R>, const Geom &, double *, int *, const DevState *,       \
                                              LaunchStream);                                                           \
-    template cudaError_t launch_convert_in<R>(int, const R *, C<R> *, const Geom &, LaunchStream);                    \
-    template cudaError_t launch_convert_out<R>(int, LinkPair<R>, R *, const Geom &, const DevState *, LaunchStream);  \
+    template cudaError_t launch_convert_in<R>(int, const R *, C<R> *, const Geom &, LaunchStream, long long, long long); \
+    template cudaError_t launch_convert_out<R>(int, LinkPair<R>, R *, const Geom &, const DevState *, LaunchStream, long long, long long); \
     template cudaError_t launch_gacc<R>(int, const C<R> *, C<R> *, R *, const Geom &, const DevState *, LaunchStream); \
     template cudaError_t launch_algebra<R>(int, LinkPair<R>, C<R> *, const Geom &, int, const DevState *, LaunchStream); \
     template cudaError_t launch_gluon_unpack<R>(const C<R> *, R *, const Geom &, const int[4], const int[4], LaunchStream); \

@@ -486,7 +486,7 @@ static int slab_update(lgf_slab *ctx) {
 template <class R>
 static int slab_sweep(lgf_slab *ctx, double *d_sums) {
     int nb = 0;
-    if (ctx->sweep_maps && ctx->nr == 2)      // as the one-GPU context: the staged sweep where it measured faster
+    if (ctx->sweep_maps && sweep_tma_auto(ctx->gl, ctx->nr, ctx->prec))      // as the one-GPU context: where it measured faster
         SCK(launch_sweep_tma<R>(ctx->sweep_maps, ctx->nr, slab_links<R>(ctx), (const C<R> *)ctx->G, (C<R> *)ctx->W, ctx->gl,
                                 ctx->partial, &nb, ctx->st, LaunchStream(ctx->stream, false), 1, false, slab_halo<R>(ctx)));
     else

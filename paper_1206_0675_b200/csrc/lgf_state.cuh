@@ -110,10 +110,11 @@ template <class R>
 cudaError_t launch_plaquette(int nr, LinkPair<R> links, const Geom &g, double *partial, int *nblocks,
                              const DevState *st, LaunchStream stream);
 template <class R>
-cudaError_t launch_convert_in(int nr, const R *canon, C<R> *links0, const Geom &g, LaunchStream stream);
+cudaError_t launch_convert_in(int nr, const R *canon, C<R> *links0, const Geom &g, LaunchStream stream, long long s0 = 0,
+                              long long n = -1 /* sites s0 .. s0 + n - 1 from a chunk buffer; -1: all from s0 on */);
 template <class R>
 cudaError_t launch_convert_out(int nr, LinkPair<R> links, R *canon, const Geom &g, const DevState *st,
-                               LaunchStream stream);
+                               LaunchStream stream, long long s0 = 0, long long n = -1);
 // accumulated gauge transformation: op 0 = set to identity, 1 = Gacc <- g Gacc, 2 = copy out (canonical [s][3][3]),
 // 3 = (A = G, out = canonical input field) rows 0, 1 of the SU(3) projection of a given transformation into G
 template <class R>
@@ -139,6 +140,7 @@ cudaError_t launch_reset_counters(DevState *st, LaunchStream stream);
 
 // the staged sweep (lgf_sweep_tma.cu): TMA tensor copies into a shared-memory ring, persistent warp-specialised CTAs
 bool sweep_tma_supported(const Geom &g, int nr, int prec);
+bool sweep_tma_auto(const Geom &g, int nr, int prec);      // ... and measured faster than k_sweep for this lattice / variant
 struct SweepMaps;     // the TMA tensor maps over a context's two link buffers and its g field
 SweepMaps *sweep_tma_maps_create(const Geom &g, int nr, int prec, void *links0, void *links1, void *G);   // null: does not apply
 void sweep_tma_maps_destroy(SweepMaps *m);

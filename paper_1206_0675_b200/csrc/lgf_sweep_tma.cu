@@ -11,9 +11,9 @@
 // the bytes in flight live in shared memory instead of registers: one producer thread keeps the ring full while
 // four compute warps work, every operand is read from shared memory, and a tile's x / y neighbours are served from
 // the staged planes instead of being loaded again (4 + 1/R + 2 link transforms per site instead of 8).
-// Result: as fast as k_sweep in fp64 / 18-real (280 vs 282 us), faster with 12-real storage (fp64 220 vs 224 us,
-// fp32 120 vs 129 us), slower in fp32 / 18-real (171 vs 155 us) -- so the context uses it for 12-real storage
-// (lgf_tune "sweep_tma": 1 = always, 0 = never).  What it took to get there, each step measured:
+// Result at 32^4 (sweep time, staged / register): fp64/18 269 / 283 us, fp64/12 212 / 227, fp32/12 114 / 134, but
+// fp32/18 164 / 160; it loses at 64^4 and 24^3 x 48 (table at sweep_tma_auto) -- the context uses it where it won
+// (lgf_tune "sweep_tma": -1 = that rule, 1 = wherever it applies, 0 = never).  What it took to get there, each step measured:
 //   * 1-D bulk copies (one per plane, 105 per tile) cost the issuing warp 73 cycles each, whatever their size:
 //     tensor maps (14 copies per tile) removed that bottleneck;
 //   * the producer is ONE thread (about one instruction per five cycles): 64-bit index arithmetic and a byte-granular
@@ -388,6 +388,19 @@ static bool sweep_tma_config(const Geom &g, int nr, int prec, int minb, SweepTil
 bool sweep_tma_supported(const Geom &g, int nr, int prec) {
     SweepTileCfg tc;
     return sweep_tma_config(g, nr, prec, prec == 8 ? 2 : 3, &tc);
+}
+
+// Where the staged sweep measured faster than k_sweep on B200 (sweep time in us, staged / register):
+//   32^4    fp64/18 269 / 283   fp64/12 212 / 227   fp32/12 114 / 134   but fp32/18 164 / 160
+//   64^4    fp32/12 1880 / 2038                      but fp64/18 5005 / 4464, fp64/12 3863 / 3738, fp32/18 2652 / 2457
+//           (x lines of 64 sites: tiles of two lines, half of the y neighbours recomputed)
+//   24^3 x 48 (tiles of 96 sites, no register split)  fp64/18 232 / 175, fp32/18 124 / 115;   16^4: equal
+// i.e. tiles of 128 sites in at least 4 lines, except fp32 / 18-real; and fp32 / 12-real on any 128-site tile.
+bool sweep_tma_auto(const Geom &g, int nr, int prec) {
+    SweepTileCfg tc;
+    if (!sweep_tma_config(g, nr, prec, prec == 8 ? 2 : 3, &tc) || tc.NT != 128) return false;
+    if (prec == 4) return nr == 2;
+    return tc.R >= 4;
 }
 
 // cuTensorMapEncodeTiled is a driver entry point; liblgf links only the runtime, so it is looked up at run time.

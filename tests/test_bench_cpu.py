@@ -40,15 +40,28 @@ def test_reference_arm_other_ranks_exit_quietly():
     assert r.returncode == 0 and r.stdout.strip() == ""
 
 
-def test_traffic_comes_from_the_newest_capture():
+def test_traffic_comes_from_the_newest_matching_capture():
     sys.path.insert(0, ROOT)
     import bench
 
-    cap = bench.captured_traffic("C3", "fp64", 18, "update")
-    assert cap is not None and cap["bytes"] > 1.3e9 and cap["kernel"].startswith("k_sweep<double")
-    newest = sorted(f for f in os.listdir(os.path.join(ROOT, "profiles")) if f.endswith("_traffic.csv"))[-1]
-    assert cap["source"] == "profiles/" + newest
-    assert bench.captured_traffic("C3", "fp64", 18, "no_such_class") is None
+    launched = {"update": ["k_sweep_tma<double, 3, 0, 1>"], "fft": ["k_fftr2_xy<double, 32, 0, 2, 0>", "k_fftr2_zt<double, 32, 32, 4>",
+                                                                  "k_fftr2_xy<double, 32, 1, 4, 1>"]}
+    caps, stale = bench.captured_traffic("C3", "fp64", 18, launched)
+    up = caps["update"][0]
+    assert up["bytes"] > 1.3e9 and up["kernel"].startswith("k_sweep_tma<double") and up["source"].startswith("profiles/r2")
+    assert len(caps["fft"]) == 3 and all(r["bytes"] > 5e7 for r in caps["fft"])
+    # a capture of a kernel this build does not launch is refused, not quoted
+    caps2, stale2 = bench.captured_traffic("C3", "fp64", 18, {"update": ["k_sweep<double, 3, 3, 0, 0>"]})
+    assert "update" not in caps2 and any("k_sweep_tma" in x for x in stale2)     # (refused: named under "stale")
+
+
+def test_reduce_ncu_names_and_classes():
+    sys.path.insert(0, ROOT)
+    import bench
+
+    n = bench.short_kernel_name("void lgf::k_sweep<double, (int)3, (bool)0, (bool)1, (int)3>(lgf::LinkPair<T1>, const lgf::C<T1> *)")
+    assert n == "k_sweep<double, 3, 0, 1, 3>" and bench.kernel_class_of(n) == "update"
+    assert bench.kernel_class_of("k_fftr2_zt<float, 32, 32, 4>") == "fft" and bench.kernel_class_of("k_finalize") is None
 
 
 def test_cuda_arm_fails_loudly_without_a_device():
