@@ -269,9 +269,9 @@ int lgf_slab_halo_unpack(lgf_slab *ctx, int which, const void *d_recv);
  * over the slab's sites (device doubles, fixed summation order). */
 int lgf_slab_delta(lgf_slab *ctx, double *d_sums);
 /* The 4-D FFT around the two all-to-alls.  An all-to-all buffer holds 8 reals per local site, ordered
- * [q][c][tl][zl][y][x]: chunk q (1 / nranks of the buffer) is the part that goes to / came from rank q, c = 0..3 the
- * packed component of the work field, tl / zl the t / z index inside the chunk (t = q T + tl on the t-slab side's
- * peer, z = q Zl + zl).  The passes next to an all-to-all read and write these buffers directly:
+ * [c][q][tl][zl][y][x]: c = 0..3 the packed component of the work field -- each component's quarter of the buffer is
+ * an all-to-all of its own --, chunk q (1 / nranks of the quarter) the part that goes to / came from rank q, tl / zl
+ * the t / z index inside the chunk (t = q T + tl on the t-slab side's peer, z = q Zl + zl).  The passes next to an all-to-all read and write these buffers directly:
  *   fft_forward:   forward x, y in place, forward z from the work field into d_send                (Alg. 1 line 4)
  *   fft_t:         t lines of this rank's z-slab, d_recv -> d_send (distinct buffers): forward t, times
  *                  p2max / (V p2(k)) with the zero mode set to 0, inverse t                       (lines 4-7)
@@ -282,6 +282,19 @@ int lgf_slab_fft_forward(lgf_slab *ctx, void *d_send);
 int lgf_slab_fft_t(lgf_slab *ctx, const void *d_recv, void *d_send);
 int lgf_slab_fft_inverse(lgf_slab *ctx, const void *d_recv);
 int lgf_slab_fft_inverse_g(lgf_slab *ctx, const void *d_recv, double alpha);
+/* The same passes one packed component at a time (comp = 0..3; the four components of the work field are independent
+ * fields, and the exchange buffers are component-major, so a component's quarter is one contiguous all-to-all): the
+ * caller can run the exchange of component c on another stream while the kernels of component c + 1 run on the
+ * context's.  fft_forward_comp = forward x, y and z of that component into its quarter of d_send; fft_t_comp = its t
+ * lines, quarter of d_recv -> quarter of d_send; fft_zinv_comp = inverse z of its quarter of d_recv into the work
+ * field; then ONCE lgf_slab_fft_xyinv = inverse y, x of all four components (with_g != 0: ending in a5, which needs
+ * all of w(x)).  Available when every axis takes the register-line passes (extents 16 / 32 / 64 and whole CTAs of
+ * planes per component): lgf_slab_by_component returns 1, else 0 and these calls return LGF_ESTATE. */
+int lgf_slab_by_component(const lgf_slab *ctx);
+int lgf_slab_fft_forward_comp(lgf_slab *ctx, void *d_send, int comp);
+int lgf_slab_fft_t_comp(lgf_slab *ctx, const void *d_recv, void *d_send, int comp);
+int lgf_slab_fft_zinv_comp(lgf_slab *ctx, const void *d_recv, int comp);
+int lgf_slab_fft_xyinv(lgf_slab *ctx, int with_g, double alpha);
 /* a5: g(x) = GS(1 + i (alpha / 2) w(x)) on the slab */
 int lgf_slab_gbuild(lgf_slab *ctx, double alpha);
 /* a6: U_mu(x) <- g(x) U_mu(x) g(x + mu)^dag on the slab, in place */

@@ -79,6 +79,11 @@ SIGNATURES = {
     "lgf_slab_fft_t": (_i, [_vp, _vp, _vp]),
     "lgf_slab_fft_inverse": (_i, [_vp, _vp]),
     "lgf_slab_fft_inverse_g": (_i, [_vp, _vp, _d]),
+    "lgf_slab_by_component": (_i, [_vp]),
+    "lgf_slab_fft_forward_comp": (_i, [_vp, _vp, _i]),
+    "lgf_slab_fft_t_comp": (_i, [_vp, _vp, _vp, _i]),
+    "lgf_slab_fft_zinv_comp": (_i, [_vp, _vp, _i]),
+    "lgf_slab_fft_xyinv": (_i, [_vp, _i, _d]),
     "lgf_slab_gbuild": (_i, [_vp, _d]),
     "lgf_slab_update": (_i, [_vp]),
     "lgf_slab_sweep": (_i, [_vp, _vp]),
@@ -392,6 +397,22 @@ class SlabContext:
 
     def fft_inverse_g(self, recv, alpha):
         self._ck(load().lgf_slab_fft_inverse_g(self._h, _dev_ptr(recv, self.precision, self.V * 8), float(alpha)))
+
+    def by_component(self):
+        return bool(self._ck(load().lgf_slab_by_component(self._h)))
+
+    def fft_forward_comp(self, send, comp):
+        self._ck(load().lgf_slab_fft_forward_comp(self._h, _dev_ptr(send, self.precision, self.V * 8), int(comp)))
+
+    def fft_t_comp(self, recv, send, comp):
+        self._ck(load().lgf_slab_fft_t_comp(self._h, _dev_ptr(recv, self.precision, self.V * 8),
+                                            _dev_ptr(send, self.precision, self.V * 8), int(comp)))
+
+    def fft_zinv_comp(self, recv, comp):
+        self._ck(load().lgf_slab_fft_zinv_comp(self._h, _dev_ptr(recv, self.precision, self.V * 8), int(comp)))
+
+    def fft_xyinv(self, with_g, alpha=0.0):
+        self._ck(load().lgf_slab_fft_xyinv(self._h, int(bool(with_g)), float(alpha)))
 
     def gbuild(self, alpha):
         self._ck(load().lgf_slab_gbuild(self._h, float(alpha)))

@@ -60,6 +60,7 @@ struct lgf_ctx {
     int tune_reunit = 0;         // lgf_tune "reunit_every": project the new links onto SU(3) in every N-th update (0 = never)
     long long updates_enqueued = 0;   // host-side count of updates enqueued since the last set_links / thermalize
     int tune_pdl = 1;            // lgf_tune "pdl": launch the iteration's kernels with programmatic stream serialization
+    int tune_fft_bulk = 0;       // lgf_tune "fft_bulk": (x, y) FFT sweeps fed by cp.async.bulk (ablation; measured in DESIGN.md)
     int tune_sweep_tma = -1;     // lgf_tune "sweep_tma" (see use_sweep_tma)
     int tune_sweep_rsplit = 1;   // lgf_tune "sweep_rsplit": register split between producer and compute warps (fp64 staged sweep)
     int tune_sweep_ahead = 0;    // lgf_tune "sweep_prefetch": CTAs ahead of which the sweep prefetches its tile into L2 (0 = off)
@@ -367,7 +368,7 @@ static int step_accelerate(lgf_ctx *ctx, bool with_g = false, double alpha = 0.0
         if (p.kind == PASS_REG2) {
             const int which = (with_g && p.axis == 2) ? 3 : p.axis;
             CK(launch_fft_reg2<R>(which, ctx->g, (C<R> *)ctx->W, (const R *)ctx->p2tab, scale, ctx->st, STRM(ctx),
-                                  (C<R> *)ctx->G, (R)(0.5 * alpha)));
+                                  (C<R> *)ctx->G, (R)(0.5 * alpha), ctx->tune_fft_bulk != 0));
             continue;
         }
         const R *tw[4] = {(const R *)ctx->twiddle[0], (const R *)ctx->twiddle[1], (const R *)ctx->twiddle[2],
@@ -1038,6 +1039,7 @@ int lgf_tune(lgf_ctx *ctx, const char *key, int value) {
     else if (k == "hb_tz") ctx->tune_hb_tz = value;
     else if (k == "sweep_share") ctx->tune_sweep_share = value;
     else if (k == "sweep_tma") ctx->tune_sweep_tma = value;
+    else if (k == "fft_bulk") ctx->tune_fft_bulk = value;
     else if (k == "sweep_rsplit") ctx->tune_sweep_rsplit = value;
     else if (k == "sweep_prefetch") ctx->tune_sweep_ahead = value < 0 ? 0 : value;
     else if (k == "sweep_minb") ctx->tune_sweep_minb = value == 2 ? 2 : 3;

@@ -14,6 +14,7 @@
 #include "lgf_fft_split.cuh"
 #include "lgf_state.cuh"
 #include "lgf_pdl.cuh"
+#include "lgf_tma.cuh"
 
 namespace lgf {
 
@@ -97,6 +98,113 @@ __global__ void __launch_bounds__(2 * P * L) k_fftr2_xy(C<R> *__restrict__ W, co
             }
         }
     }
+}
+
+// ---- (x, y) planes through the bulk-copy engine (lgf_tune "fft_bulk") ---------------------------------
+// The same sweep with the plane brought on chip by ONE cp.async.bulk per plane (1-D TMA, SASS UBLKCP; an (x, y)
+// plane is a contiguous 16 KB block at 32^4 fp64) signalled by an mbarrier, and -- where the result goes back to W
+// -- taken off chip by one bulk store (UBLKCP.G.S).  The plane lands in the transposition tile's own storage
+// (dense L x L inside the L x (L | 1) tile), so the shared-memory footprint and the CTAs per SM are those of
+// k_fftr2_xy; what it costs is one more pass through shared memory and two more barriers per plane.  Measured on
+// B200 (32^4, FFT time per iteration, default / bulk): see DESIGN.md section 6 -- it is an ablation, off by default.
+template <class R, int L, int MODE, int P, bool GOUT>
+__global__ void __launch_bounds__(2 * P * L) k_fftr2_xy_bulk(C<R> *__restrict__ W, const DevState *__restrict__ st,
+                                                             C<R> *__restrict__ G, long long V, int nzt, R half_alpha) {
+    pdl_enter();
+    if (st->done) return;
+    static_assert(L % 16 == 0, "16 lines per warp");
+    constexpr int M = L / 2;
+    constexpr int PX = L | 1;
+    constexpr unsigned PLANE_BYTES = L * L * sizeof(C<R>);
+    using S = SplitDft<L, PAIR_MASK, R>;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    C<R> *tile_all = reinterpret_cast<C<R> *>(smem_raw);
+    __shared__ uint64_t bar;
+    const int tid = threadIdx.x;
+    const int p = tid / (2 * L), tp = tid % (2 * L);
+    const int h = (tp >> 4) & 1;
+    const int i = (tp >> 5) * 16 + (tp & 15);
+    auto plane_of = [&](int pp) {
+        return GOUT ? (long long)(pp % 4) * nzt + (long long)blockIdx.x * (P / 4) + pp / 4 : (long long)blockIdx.x * P + pp;
+    };
+    C<R> *base = W + plane_of(p) * (L * L);
+    C<R> *tile = tile_all + p * (L * PX);
+    if (tid == 0) {
+        mbar_init(&bar, 1);
+        mbar_init_fence();
+        mbar_arrive_expect_tx(&bar, P * PLANE_BYTES);
+        for (int pp = 0; pp < P; pp++) bulk_g2s(tile_all + pp * (L * PX), W + plane_of(pp) * (L * L), PLANE_BYTES, &bar);
+    }
+    __syncthreads();                                         // the barrier's initialisation is visible to every waiter
+    mbar_wait(&bar, 0);
+    C<R> v[M];
+    if constexpr (MODE == FFT_FWD) {
+#pragma unroll
+        for (int m = 0; m < M; m++) v[m] = tile[(m + M * h) * L + i];        // dense plane: y = m + M h at x = i
+        __syncthreads();                                                     // everyone has its line: the tile may be overwritten
+        S::forward(v, h);
+#pragma unroll
+        for (int j = 0; j < M; j++) tile[(2 * j + h) * PX + i] = v[j];       // tile[ky][x]
+        __syncthreads();
+#pragma unroll
+        for (int m = 0; m < M; m++) v[m] = tile[i * PX + m + M * h];
+        S::forward(v, h);
+        __syncthreads();
+#pragma unroll
+        for (int j = 0; j < M; j++) tile[(2 * j + h) * L + i] = v[j];        // dense again: (kx, ky = i), transposed plane
+    } else {
+#pragma unroll
+        for (int j = 0; j < M; j++) v[j] = tile[(2 * j + h) * L + i];
+        __syncthreads();
+        S::inverse(v, h);
+#pragma unroll
+        for (int m = 0; m < M; m++) tile[i * PX + m + M * h] = v[m];
+        __syncthreads();
+#pragma unroll
+        for (int j = 0; j < M; j++) v[j] = tile[(2 * j + h) * PX + i];
+        S::inverse(v, h);
+        __syncthreads();
+        if constexpr (!GOUT) {
+#pragma unroll
+            for (int m = 0; m < M; m++) tile[(m + M * h) * L + i] = v[m];    // dense (y, x = i)
+        } else {
+#pragma unroll
+            for (int m = 0; m < M; m++) tile[(m + M * h) * PX + i] = v[m];
+            __syncthreads();
+            const C<R> *t4 = tile_all + (p / 4) * 4 * (L * PX);
+            const long long s0 = ((long long)blockIdx.x * (P / 4) + p / 4) * (L * L);
+            const int sub = (p % 4) * 2 + h;
+#pragma unroll
+            for (int mm = 0; mm < L / 8; mm++) {
+                const int y = sub + 8 * mm;
+                Herm<R> w;
+                w.m01 = t4[y * PX + i];
+                w.m02 = t4[L * PX + y * PX + i];
+                w.m12 = t4[2 * L * PX + y * PX + i];
+                const C<R> dg = t4[3 * L * PX + y * PX + i];
+                w.m00 = dg.x;
+                w.m11 = dg.y;
+                C<R> gx[9];
+                build_g(w, half_alpha, gx);
+                const long long s = s0 + y * L + i;
+#pragma unroll
+                for (int e = 0; e < 6; e++) G[(long long)e * V + s] = gx[e];
+            }
+            return;
+        }
+    }
+    // the dense result planes back to W: ordinary shared-memory stores, made visible to the copy engine, one bulk store each
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    __syncthreads();
+    if (tid == 0) {
+        for (int pp = 0; pp < P; pp++)
+            asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(W + plane_of(pp) * (L * L)),
+                         "r"(smem_u32(tile_all + pp * (L * PX))), "r"(PLANE_BYTES)
+                         : "memory");
+        asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+        asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");     // shared memory must outlive the reads
+    }
+    (void)base;
 }
 
 // ---- (z, t) planes --------------------------------------------------------------------------------
@@ -219,6 +327,16 @@ bool fft_reg2_supported(const Geom &g) {
 bool fft_reg2_xy_supported(const Geom &g) {
     return g.L[0] == g.L[1] && reg2_len(g.L[0]) && (4LL * g.L[2] * g.L[3]) % 8 == 0 && ((long long)g.L[2] * g.L[3]) % 2 == 0;
 }
+// can the forward (x, y) sweep run over one component at a time (whole CTAs of that component's planes)?
+bool fft_reg2_xy_by_component(const Geom &g, int prec) {
+    if (!fft_reg2_xy_supported(g)) return false;
+    const long long per = (long long)g.L[2] * g.L[3];
+    int pf = 8;
+#define LGF_C(LEN) if (g.L[0] == LEN) pf = prec == 8 ? Xy2Cfg<double, LEN>::PF : Xy2Cfg<float, LEN>::PF;
+    LGF_REG2_LEN(LGF_C)
+#undef LGF_C
+    return per % pf == 0;
+}
 bool fft_reg2_xy_gout(const Geom &g, int prec) { return fft_reg2_xy_supported(g) && !(g.L[0] == 64 && prec == 8); }
 // can the inverse (x, y) sweep end with the g-build for this lattice and precision (bytes per real)?
 bool fft_reg2_gout(const Geom &g, int prec) {
@@ -227,10 +345,24 @@ bool fft_reg2_gout(const Geom &g, int prec) {
     return true;
 }
 
+static thread_local int t_xy_comp = -1;           // >= 0: the forward (x, y) sweep over ONE packed component only (lgf_slab.cu)
+static thread_local bool t_xy_bulk = false;      // set by launch_fft_reg2 for the launch in progress (lgf_tune "fft_bulk")
 template <class R, int L, int MODE, int P, bool GOUT>
 static cudaError_t launch_xy2_as(const Geom &g, C<R> *W, const DevState *st, LaunchStream stream, C<R> *G, R half_alpha) {
+    if (t_xy_bulk) {
+        constexpr size_t SMB = sizeof(C<R>) * P * L * (L | 1);
+        auto kb = k_fftr2_xy_bulk<R, L, MODE, P, GOUT>;
+        if (cudaError_t e = ensure_dynamic_smem(kb, SMB); e != cudaSuccess) return e;
+        return launch_pdl(kb, dim3((unsigned)(4LL * g.L[2] * g.L[3] / P)), dim3(2 * P * L), SMB, stream, W, st, G, g.V, g.L[2] * g.L[3],
+                          half_alpha);
+    }
     constexpr size_t SM = sizeof(C<R>) * P * L * (L | 1);
-    const long long planes = 4LL * g.L[2] * g.L[3];
+    long long planes = 4LL * g.L[2] * g.L[3];
+    if (!GOUT && t_xy_comp >= 0) {                   // one component: its planes are contiguous in W
+        planes /= 4;
+        if (planes % P != 0) return cudaErrorInvalidValue;
+        W += (long long)t_xy_comp * g.V;
+    }
     auto kern = k_fftr2_xy<R, L, MODE, P, GOUT>;
     if (cudaError_t e = ensure_dynamic_smem(kern, SM); e != cudaSuccess) return e;
     return launch_pdl(kern, dim3((unsigned)(planes / P)), dim3(2 * P * L), SM, stream, W, st, G, g.V, g.L[2] * g.L[3],
@@ -259,7 +391,9 @@ static cudaError_t launch_zt2(const Geom &g, C<R> *W, const R *p2tab, R scale, c
 // which: 0 = (x, y) forward, 1 = (z, t) forward + scale + inverse, 2 = (x, y) inverse, 3 = (x, y) inverse + g
 template <class R>
 cudaError_t launch_fft_reg2(int which, const Geom &g, C<R> *W, const R *p2tab, R scale, const DevState *st,
-                            LaunchStream stream, C<R> *G, R half_alpha) {
+                            LaunchStream stream, C<R> *G, R half_alpha, bool bulk, int comp) {
+    t_xy_bulk = bulk;
+    t_xy_comp = comp;
     if (which == 1) {
 #define LGF_GO(A, B) if (g.L[2] == A && g.L[3] == B) return launch_zt2<R, A, B>(g, W, p2tab, scale, st, stream);
         LGF_REG2_ZT(LGF_GO)
@@ -297,8 +431,8 @@ std::string fft_reg2_kernel_name(int which, const Geom &g, int prec) {
 }
 
 template cudaError_t launch_fft_reg2<float>(int, const Geom &, C<float> *, const float *, float, const DevState *,
-                                            LaunchStream, C<float> *, float);
+                                            LaunchStream, C<float> *, float, bool, int);
 template cudaError_t launch_fft_reg2<double>(int, const Geom &, C<double> *, const double *, double, const DevState *,
-                                             LaunchStream, C<double> *, double);
+                                             LaunchStream, C<double> *, double, bool, int);
 
 }  // namespace lgf

@@ -89,11 +89,14 @@ __global__ void __launch_bounds__(SLAB_THREADS) k_slab_pack_ut(LinkPair<R> lp, C
 }
 
 // Where element n of a line lives: base + (n / D) strideQ + (n % D) strideN.  The all-to-all buffers are ordered
-// [q][c][tl][zl][xy] (chunk q goes to / came from rank q; c = packed component of W; tl, zl local to the chunk), so
-//   a z line in a buffer   (z = q Zl + zl):  D = Zl, strideQ = chunk, strideN = Sxy,     base = (c T + tl) Zl Sxy + xy
-//   a t line in a buffer   (t = q T + tl):   D = T,  strideQ = chunk, strideN = Zl Sxy,  base = (c T Zl + zl) Sxy + xy
+// [c][q][tl][zl][xy] (c = packed component of W: four independent exchanges, each a contiguous quarter of the buffer;
+// chunk q of a component goes to / came from rank q; tl, zl local to the chunk), so with piece = T Zl Sxy elements
+//   a z line in a buffer   (z = q Zl + zl):  D = Zl, strideQ = piece, strideN = Sxy,     base = (c N T + tl) Zl Sxy + xy
+//   a t line in a buffer   (t = q T + tl):   D = T,  strideQ = piece, strideN = Zl Sxy,  base = c N piece + zl Sxy + xy
 //   a z line in the field W[c][tl][z][xy]:   D = Lz (one piece),      strideN = Sxy,     base = c V + tl Lz Sxy + xy
-// with chunk = 4 T Zl Sxy elements.  blockIdx.y = the "other" local index (tl for z lines, zl for t lines), blockIdx.z = c.
+// (N piece = V elements per component).  blockIdx.y = the "other" local index (tl for z lines, zl for t lines),
+// blockIdx.z = c.  The components being separate lets component c's exchange overlap component c + 1's line pass
+// (the *_comp entry points below, paper_1206_0675_b200/slab.py).
 struct LineAddr {
     long long stride_c, stride_o, strideQ, strideN;
     int D;
@@ -270,6 +273,7 @@ struct lgf_slab {
     bool xy_reg = false;         // (x, y) planes by the register-line sweeps of lgf_fft_reg2.cu (square planes of 16 / 32 / 64)
     bool xy_gout = false;        // ... and the inverse one can end with the g-build (a5)
     int nlo_z = 1, nlo_t = 1;    // consecutive (x, y) indices per CTA of the z / t line passes
+    bool by_comp = false;        // the per-component entry points (*_comp) are available: register-line passes on x, y, z and t
     bool z_reg = false, t_reg = false;   // z / t lines in registers (k_slab_fft_line2): natural frequency order on that axis
     LineAddr a_w{}, a_zbuf{}, a_tbuf{};
     bool have_links = false;
@@ -441,6 +445,48 @@ static int slab_fft_inverse(lgf_slab *ctx, const void *d_recv, bool with_g, doub
     return LGF_OK;
 }
 
+// ---- the same passes for ONE packed component c (the four components of W are independent fields): what lets the
+// exchange of component c run on another stream while component c + 1 is being transformed (slab.py)
+template <class R>
+static int slab_fft_forward_comp(lgf_slab *ctx, void *d_send, int c) {
+    SCK(launch_fft_reg2<R>(0, ctx->gl, (C<R> *)ctx->W, (const R *)ctx->p2tab, (R)0, ctx->st, ctx->stream, nullptr, (R)0, false, c));
+    SCK(launch_line2<R>(ctx->dims[2], FFT_FWD, (const C<R> *)ctx->W + c * ctx->a_w.stride_c, (C<R> *)d_send + c * ctx->a_zbuf.stride_c,
+                        ctx->a_w, ctx->a_zbuf, dim3((unsigned)(ctx->gl.S[2] / LINE2_LINES), ctx->T, 1), ctx->dims[0],
+                        (const R *)ctx->p2tab, (R)0, ctx->stream));
+    ctx->launches += 2;
+    return LGF_OK;
+}
+template <class R>
+static int slab_fft_t_comp(lgf_slab *ctx, const void *d_recv, void *d_send, int c) {
+    const R scale = (R)(16.0 / (double)ctx->Vglobal);              // p2max / V (Alg. 1 lines 5, 7; R5)
+    SCK(launch_line2<R>(ctx->dims[3], FFT_FWD_SCALE_INV, (const C<R> *)d_recv + c * ctx->a_tbuf.stride_c,
+                        (C<R> *)d_send + c * ctx->a_tbuf.stride_c, ctx->a_tbuf, ctx->a_tbuf,
+                        dim3((unsigned)(ctx->gl.S[2] / LINE2_LINES), ctx->Zl, 1), ctx->dims[0], (const R *)ctx->p2tab, scale, ctx->stream));
+    ctx->launches++;
+    return LGF_OK;
+}
+template <class R>
+static int slab_fft_zinv_comp(lgf_slab *ctx, const void *d_recv, int c) {
+    SCK(launch_line2<R>(ctx->dims[2], FFT_INV, (const C<R> *)d_recv + c * ctx->a_zbuf.stride_c, (C<R> *)ctx->W + c * ctx->a_w.stride_c,
+                        ctx->a_zbuf, ctx->a_w, dim3((unsigned)(ctx->gl.S[2] / LINE2_LINES), ctx->T, 1), ctx->dims[0],
+                        (const R *)ctx->p2tab, (R)0, ctx->stream));
+    ctx->launches++;
+    return LGF_OK;
+}
+// inverse (x, y) sweep of all four components (ending in a5 with_g: the g-build needs all of w(x) on chip)
+template <class R>
+static int slab_fft_xyinv(lgf_slab *ctx, bool with_g, double alpha) {
+    const R ha = (R)(0.5 * alpha);
+    const bool fuse = with_g && ctx->xy_gout;
+    SCK(launch_fft_reg2<R>(fuse ? 3 : 2, ctx->gl, (C<R> *)ctx->W, (const R *)ctx->p2tab, (R)0, ctx->st, ctx->stream, (C<R> *)ctx->G, ha));
+    ctx->launches++;
+    if (with_g && !fuse) {
+        SCK(launch_gbuild<R>((const C<R> *)ctx->W, (C<R> *)ctx->G, ctx->gl, ha, ctx->st, ctx->stream));
+        ctx->launches++;
+    }
+    return LGF_OK;
+}
+
 template <class R>
 static LinkPair<R> slab_links(lgf_slab *ctx) {
     LinkPair<R> lp;
@@ -552,11 +598,11 @@ int lgf_slab_create(const int dims[4], int precision, int link_storage, int rank
     ctx->xy_reg = fft_reg2_xy_supported(ctx->gl);
     ctx->xy_gout = fft_reg2_xy_gout(ctx->gl, precision);
     {   // address maps of the line passes (LineAddr) and their tiles: about 2048 complex elements per CTA
-        const long long Sxy = ctx->gl.S[2], chunk = 4LL * ctx->T * ctx->Zl * Sxy;
+        const long long Sxy = ctx->gl.S[2], piece = (long long)ctx->T * ctx->Zl * Sxy;
         auto lg2 = [](int d) { int sh = 0; while ((1 << sh) < d) sh++; return (1 << sh) == d ? sh : -1; };
         ctx->a_w = LineAddr{Sl, (long long)dims[2] * Sxy, 0, Sxy, dims[2], lg2(dims[2])};
-        ctx->a_zbuf = LineAddr{(long long)ctx->T * ctx->Zl * Sxy, (long long)ctx->Zl * Sxy, chunk, Sxy, ctx->Zl, lg2(ctx->Zl)};
-        ctx->a_tbuf = LineAddr{(long long)ctx->T * ctx->Zl * Sxy, Sxy, chunk, (long long)ctx->Zl * Sxy, ctx->T, lg2(ctx->T)};
+        ctx->a_zbuf = LineAddr{Sl, (long long)ctx->Zl * Sxy, piece, Sxy, ctx->Zl, lg2(ctx->Zl)};
+        ctx->a_tbuf = LineAddr{Sl, Sxy, piece, (long long)ctx->Zl * Sxy, ctx->T, lg2(ctx->T)};
         auto reg_len = [](int L) { return L == 16 || L == 32 || L == 64; };
         ctx->z_reg = reg_len(dims[2]) && Sxy % LINE2_LINES == 0;          // nranks | L then makes Zl, T powers of two
         ctx->t_reg = reg_len(dims[3]) && Sxy % LINE2_LINES == 0;
@@ -595,6 +641,7 @@ int lgf_slab_create(const int dims[4], int precision, int link_storage, int rank
         lgf_slab_destroy(ctx);
         return rc;
     }
+    ctx->by_comp = ctx->xy_reg && ctx->z_reg && ctx->t_reg && fft_reg2_xy_by_component(ctx->gl, precision);
     ctx->sweep_maps = sweep_tma_maps_create(ctx->gl, ctx->nr, precision, ctx->lbuf[0], ctx->lbuf[1], ctx->G);
     for (int a = 0; a < 2; a++) {
         ctx->pass_fwd[a] = slab_axis_pass(ctx->gl, precision, a, FFT_FWD);
@@ -708,6 +755,39 @@ int lgf_slab_fft_inverse_g(lgf_slab *ctx, const void *d_recv, double alpha) {
     if (!ctx || !d_recv) return sfail(ctx, LGF_EINVAL, "lgf_slab_fft_inverse_g: null argument");
     SLAB_ENTER(ctx);
     return ctx->prec == LGF_FP64 ? slab_fft_inverse<double>(ctx, d_recv, true, alpha) : slab_fft_inverse<float>(ctx, d_recv, true, alpha);
+}
+
+int lgf_slab_by_component(const lgf_slab *ctx) { return ctx ? (ctx->by_comp ? 1 : 0) : LGF_EINVAL; }
+
+#define SLAB_COMP_ENTER(name)                                                                         \
+    if (!ctx) return LGF_EINVAL;                                                                      \
+    if (!ctx->by_comp) return sfail(ctx, LGF_ESTATE, name ": per-component passes are not available for this lattice (lgf_slab_by_component)"); \
+    if (comp < 0 || comp > 3) return sfail(ctx, LGF_EINVAL, name ": component must be 0..3");         \
+    SLAB_ENTER(ctx)
+
+int lgf_slab_fft_forward_comp(lgf_slab *ctx, void *d_send, int comp) {
+    SLAB_COMP_ENTER("lgf_slab_fft_forward_comp");
+    if (!d_send) return sfail(ctx, LGF_EINVAL, "lgf_slab_fft_forward_comp: null argument");
+    return ctx->prec == LGF_FP64 ? slab_fft_forward_comp<double>(ctx, d_send, comp) : slab_fft_forward_comp<float>(ctx, d_send, comp);
+}
+
+int lgf_slab_fft_t_comp(lgf_slab *ctx, const void *d_recv, void *d_send, int comp) {
+    SLAB_COMP_ENTER("lgf_slab_fft_t_comp");
+    if (!d_recv || !d_send || d_recv == d_send) return sfail(ctx, LGF_EINVAL, "lgf_slab_fft_t_comp: bad argument");
+    return ctx->prec == LGF_FP64 ? slab_fft_t_comp<double>(ctx, d_recv, d_send, comp) : slab_fft_t_comp<float>(ctx, d_recv, d_send, comp);
+}
+
+int lgf_slab_fft_zinv_comp(lgf_slab *ctx, const void *d_recv, int comp) {
+    SLAB_COMP_ENTER("lgf_slab_fft_zinv_comp");
+    if (!d_recv) return sfail(ctx, LGF_EINVAL, "lgf_slab_fft_zinv_comp: null argument");
+    return ctx->prec == LGF_FP64 ? slab_fft_zinv_comp<double>(ctx, d_recv, comp) : slab_fft_zinv_comp<float>(ctx, d_recv, comp);
+}
+
+int lgf_slab_fft_xyinv(lgf_slab *ctx, int with_g, double alpha) {
+    if (!ctx) return LGF_EINVAL;
+    if (!ctx->by_comp) return sfail(ctx, LGF_ESTATE, "lgf_slab_fft_xyinv: per-component passes are not available for this lattice");
+    SLAB_ENTER(ctx);
+    return ctx->prec == LGF_FP64 ? slab_fft_xyinv<double>(ctx, with_g != 0, alpha) : slab_fft_xyinv<float>(ctx, with_g != 0, alpha);
 }
 
 int lgf_slab_gbuild(lgf_slab *ctx, double alpha) {

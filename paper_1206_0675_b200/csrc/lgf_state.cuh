@@ -86,9 +86,11 @@ bool fft_reg2_supported(const Geom &g);
 bool fft_reg2_gout(const Geom &g, int prec);
 bool fft_reg2_xy_supported(const Geom &g);      // the (x, y) sweeps alone, any (Lz, Lt): the slabs of lgf_slab.cu
 bool fft_reg2_xy_gout(const Geom &g, int prec);
+bool fft_reg2_xy_by_component(const Geom &g, int prec);
 template <class R>
 cudaError_t launch_fft_reg2(int which, const Geom &g, C<R> *W, const R *p2tab, R scale, const DevState *st,
-                            LaunchStream stream, C<R> *G, R half_alpha);
+                            LaunchStream stream, C<R> *G, R half_alpha, bool bulk = false /* (x, y) planes by bulk copies */,
+                            int comp = -1 /* >= 0: forward (x, y) sweep of this packed component only */);
 // true if a PASS_XY (first two axes) / PASS_ZT (last two axes) kernel is instantiated for these lengths
 bool fft_pair_supported(int kind, int La, int Lb);
 

@@ -23,7 +23,8 @@
 //   * a slot is handed back as soon as its operands are in registers, not after the arithmetic -- and "in registers"
 //     has to be enforced (see loaded_bits);
 //   * fp64: setmaxnreg moves the idle producer warps' registers to the compute warps (no spills at 216 registers);
-//     no warp may exit before the others once registers have been moved.
+//     no warp may exit before the others once registers have been moved, and the idle warps may take their registers
+//     back only after the compute warps have released them (named barrier; without it: a timing-dependent deadlock).
 //
 // Tile: R whole x lines of one (z, t) plane, NT = R Lx <= 128 consecutive sites, one compute thread per site.
 // Per tile: a preamble (g of the tile, g of lines y0 - 1 and y0 + R, U_y of line y0 - 1) and ten ring stages, in the
@@ -218,7 +219,15 @@ __global__ void __launch_bounds__(RSPLIT ? 256 : 160, RSPLIT ? 2 : 0) __maxnreg_
             }
         }
         if constexpr (!RSPLIT) return;
-        if constexpr (RSPLIT) asm volatile("setmaxnreg.inc.sync.aligned.u32 128;");   // (after the compute warps gave them back)
+        // Back to the launch-time register count for the common tail -- but only AFTER the compute warps have given
+        // their extra registers back (named barrier 3: they arrive after their setmaxnreg.dec, this group waits).
+        // Without that order the three idle warps of this group, which get here at once, re-took the registers they
+        // had just released before the compute warps could claim them, and the compute warps then spun in their
+        // setmaxnreg.inc for ever: a timing-dependent hang (seen at 16^3 x 32 slabs and with the projecting variant).
+        if constexpr (RSPLIT) {
+            asm volatile("bar.sync 3, 256;" ::: "memory");
+            asm volatile("setmaxnreg.inc.sync.aligned.u32 128;");
+        }
     } else {
     // ---- consumers: one thread per site of the tile ---------------------------------------------------------
     RingPos rp{0, 0};
@@ -340,7 +349,10 @@ __global__ void __launch_bounds__(RSPLIT ? 256 : 160, RSPLIT ? 2 : 0) __maxnreg_
         partial[2 * blockIdx.x] = sf;
         partial[2 * blockIdx.x + 1] = stt;
     }
-    if constexpr (RSPLIT) asm volatile("setmaxnreg.dec.sync.aligned.u32 128;");
+    if constexpr (RSPLIT) {
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 128;");
+        asm volatile("bar.arrive 3, 256;" ::: "memory");
+    }
     }
     if constexpr (RSPLIT) __syncthreads();
 }

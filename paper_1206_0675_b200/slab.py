@@ -9,6 +9,7 @@ loaded configuration -- the fused sweep keeps it current -- the others once per 
 
   halo LINKS  U_t of a rank's last slice     -> rank r+1   (a1: A_t(x - t), eq. 5)          S3 * n_l reals
   all-to-all  t-slabs -> z-slabs of F_xyz[Delta]            (a2: the t lines of the 4-D FFT)  8 * V/N * (N-1)/N
+              (four of them, one per packed component, each on a second stream while the next component is transformed)
   all-to-all  z-slabs -> t-slabs                            (a4)                              the same
   halo G      g of a rank's first slice      -> rank r-1   (a6: g(x + t), eq. 2)            S3 * 12 reals
   halo G_UP   g of a rank's last slice       -> rank r+1   (fused a6 + a1: g(x - t))        S3 * 12 reals
@@ -35,6 +36,9 @@ from typing import List, Sequence
 from . import binding as B
 
 
+NCOMP = 4       # packed components of the work field: the all-to-all buffers are [c][q][tl][zl][y][x] (include/lgf.h)
+
+
 class LocalExchange:
     """N ranks emulated in one process (see module docstring)."""
 
@@ -50,13 +54,25 @@ class LocalExchange:
         for r in range(n):
             recv[r].copy_(send[(r - step) % n])
 
-    def all_to_all(self, send: Sequence, recv: Sequence) -> None:
-        """Chunk q of rank r's send buffer becomes chunk r of rank q's receive buffer (equal chunks)."""
+    def all_to_all_comp(self, send: Sequence, recv: Sequence, c: int) -> None:
+        """Component c's quarter of the buffers: chunk q of rank r's quarter becomes chunk r of rank q's (equal chunks)."""
         n = self.world
         for r in range(n):
-            dst = recv[r].view(n, -1)
+            dst = recv[r].view(NCOMP, n, -1)[c]
             for q in range(n):
-                dst[q].copy_(send[q].view(n, -1)[r])
+                dst[q].copy_(send[q].view(NCOMP, n, -1)[c][r])
+
+    def all_to_all(self, send: Sequence, recv: Sequence) -> None:
+        for c in range(NCOMP):
+            self.all_to_all_comp(send, recv, c)
+
+    # the overlapped form: here the "exchange" is device copies in stream order, so start = do it, finish = nothing
+    def start_all_to_all_comp(self, send, recv, c, main=None, comm=None):
+        self.all_to_all_comp(send, recv, c)
+        return None
+
+    def finish(self, handle, main=None) -> None:
+        return None
 
     def all_reduce_sum(self, vals: Sequence) -> None:
         total = vals[0].clone()
@@ -88,11 +104,45 @@ class DistExchange:
         for w in dist.batch_isend_irecv(ops):
             w.wait()
 
-    def all_to_all(self, send, recv) -> None:
+    def all_to_all_comp(self, send, recv, c: int, async_op: bool = False):
+        s, r = send[0].view(NCOMP, -1)[c], recv[0].view(NCOMP, -1)[c]
         if self.world == 1:
-            recv[0].copy_(send[0])
+            r.copy_(s)
+            return None
+        return self.dist.all_to_all_single(r, s, group=self.group, async_op=async_op)
+
+    def all_to_all(self, send, recv) -> None:
+        for c in range(NCOMP):
+            self.all_to_all_comp(send, recv, c)
+
+    def start_all_to_all_comp(self, send, recv, c: int, main=None, comm=None):
+        """Component c's exchange on the stream `comm`, after what `main` has enqueued so far; returns a handle for
+        ``finish``.  While it runs, `main` is free for the next component's kernels.  CPU tensors (gloo): done here."""
+        if not send[0].is_cuda or comm is None:
+            self.all_to_all_comp(send, recv, c)
+            return None
+        import torch
+
+        ev = torch.cuda.Event()
+        ev.record(main)
+        comm.wait_event(ev)
+        with torch.cuda.stream(comm):
+            work = self.all_to_all_comp(send, recv, c, async_op=True)      # None for one rank: a copy on `comm`
+            done = torch.cuda.Event()
+            done.record(comm)
+        return (work, done)
+
+    def finish(self, handle, main=None) -> None:
+        """Makes `main` wait (on the device, not the host) for the exchange started with ``start_all_to_all_comp``."""
+        if handle is None:
             return
-        self.dist.all_to_all_single(recv[0].view(-1), send[0].view(-1), group=self.group)
+        import torch
+
+        work, done = handle
+        with torch.cuda.stream(main):
+            if work is not None:
+                work.wait()                  # NCCL: the current stream waits for the collective
+            main.wait_event(done)
 
     def all_reduce_sum(self, vals) -> None:
         if self.world > 1:
@@ -114,7 +164,7 @@ class SlabFixer:
     dims = GLOBAL (Lx, Ly, Lz, Lt); world must divide Lt and Lz.  History entry n = (F, theta) of the configuration
     after n updates since ``set_links`` (as lgf_iterate / lgf_fix, include/lgf.h)."""
 
-    def __init__(self, dims, precision=B.LGF_FP64, link_storage=B.LGF_LINKS_18, exchange=None, device=None):
+    def __init__(self, dims, precision=B.LGF_FP64, link_storage=B.LGF_LINKS_18, exchange=None, device=None, overlap=True):
         import torch
 
         self.torch = torch
@@ -135,6 +185,11 @@ class SlabFixer:
         self._g2_send, self._g2_recv = mk(c0.halo_elems(B.LGF_HALO_G_UP)), mk(c0.halo_elems(B.LGF_HALO_G_UP))
         self._a_send, self._a_recv = mk(c0.V * 8), mk(c0.V * 8)
         self._sums = mk(2, torch.float64)
+        # overlap of the exchanges with the line passes: component c's all-to-all on a second stream while component
+        # c + 1 is transformed (needs the per-component entry points; `overlap=False` keeps the plain order)
+        self.overlap = bool(overlap) and all(c.by_component() for c in self.ranks)
+        self._main = stream
+        self._comm = torch.cuda.Stream(self.device) if self.overlap else None
         self._w_is_delta = False        # W of every rank holds Delta of the current links (and _sums their all-reduced sums)
         self._recorded = False          # ... and that configuration's (F, theta) is in the history
         self.exchanged_bytes = 0        # per rank, what the last iterate() sent (bench / DESIGN.md figures)
@@ -175,6 +230,28 @@ class SlabFixer:
         self._w_is_delta = True
         self._recorded = self._recorded or record
 
+    def _fft_by_component(self) -> None:
+        """a2-a4 up to the work field in (x, y) k space, one packed component at a time: while component c's all-to-all
+        runs on the second stream, the main stream already transforms component c + 1.  Per component the order is
+        forward x, y, z -> exchange 1 -> t lines (forward, scale, inverse) -> exchange 2 -> inverse z; buffers: the
+        t pass of c reads recv[c] and refills send[c] (its first exchange is over), the second exchange refills recv[c]
+        (its t pass is over) -- each ordered by the handle of the step before."""
+        ex, main, comm = self.ex, self._main, self._comm
+        first, second = [], []
+        for k in range(NCOMP):
+            for c, s in zip(self.ranks, self._a_send):
+                c.fft_forward_comp(s, k)
+            first.append(ex.start_all_to_all_comp(self._a_send, self._a_recv, k, main, comm))
+        for k in range(NCOMP):
+            ex.finish(first[k], main)
+            for c, s, r in zip(self.ranks, self._a_send, self._a_recv):
+                c.fft_t_comp(r, s, k)
+            second.append(ex.start_all_to_all_comp(self._a_send, self._a_recv, k, main, comm))
+        for k in range(NCOMP):
+            ex.finish(second[k], main)
+            for c, r in zip(self.ranks, self._a_recv):
+                c.fft_zinv_comp(r, k)
+
     def _fft_to_second_exchange(self) -> None:
         for c, s in zip(self.ranks, self._a_send):
             c.fft_forward(s)
@@ -185,6 +262,11 @@ class SlabFixer:
 
     def _step_accelerate(self) -> None:
         """a2-a4: w = F^-1[(p2max / p2) F Delta] / V with the t lines gathered by two all-to-alls; w into the work field."""
+        if self.overlap:
+            self._fft_by_component()
+            for c in self.ranks:
+                c.fft_xyinv(False)
+            return
         self._fft_to_second_exchange()
         for c, r in zip(self.ranks, self._a_recv):
             c.fft_inverse(r)
@@ -207,9 +289,15 @@ class SlabFixer:
         (new buffer current, history, loop test).  Wants the work fields to hold Delta of the current links, which
         also means the U_t halos are current.  Nothing is read back: once the device-side `done` flag is set the
         kernels of later iterations return at once."""
-        self._fft_to_second_exchange()
+        if self.overlap:
+            self._fft_by_component()
+        else:
+            self._fft_to_second_exchange()
         for c, r, dn, up in zip(self.ranks, self._a_recv, self._g_send, self._g2_send):
-            c.fft_inverse_g(r, alpha)
+            if self.overlap:
+                c.fft_xyinv(True, alpha)
+            else:
+                c.fft_inverse_g(r, alpha)
             c.halo_pack(B.LGF_HALO_G, dn)
             c.halo_pack(B.LGF_HALO_G_UP, up)
         self.ex.shift(self._g_send, self._g_recv, -1)

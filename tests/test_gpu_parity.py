@@ -88,7 +88,7 @@ ACC_DIMS = [(8, 8, 8, 8), (12, 6, 16, 4), (3, 24, 2, 48), (16, 16, 16, 16), (32,
 
 @pytest.mark.parametrize("dims", ACC_DIMS)
 @pytest.mark.parametrize("prec", [8, 4])
-@pytest.mark.parametrize("plan", ["reg", "reg2", "two_axis", "axis"])
+@pytest.mark.parametrize("plan", ["reg", "reg2", "reg2_bulk", "two_axis", "axis"])
 def test_accelerate(lgf, dims, prec, plan):
     """a2-a4: w = F^-1 (16/p^2) F Delta / V against the oracle's naive separable DFT, with each FFT
     plan: register-line sweeps with one and with two threads per line, shared-memory two-axis sweeps
@@ -100,7 +100,8 @@ def test_accelerate(lgf, dims, prec, plan):
     w_o = oracle.accelerate(dims, D)
     with lgf.Context(dims, prec, 18) as ctx:
         ctx.tune("fft_reg", int(plan == "reg"))
-        ctx.tune("fft_reg2", int(plan == "reg2"))
+        ctx.tune("fft_reg2", int(plan in ("reg2", "reg2_bulk")))
+        ctx.tune("fft_bulk", int(plan == "reg2_bulk"))       # (x, y) planes on and off chip by cp.async.bulk + mbarrier
         ctx.tune("fft_two_axis", int(plan != "axis"))
         if plan == "axis":
             assert ctx.fft_passes() == 7
@@ -201,6 +202,20 @@ def test_trajectory_two_thread_fft(lgf, config_cache, prec, storage):
     U = config_cache("C2")
     U_o, F_o, T_o = oracle.iterate(dims, U, ALPHA, 20)
     Fh, Th, P, out = run_trajectory(lgf, dims, U, prec, storage, 20, tune={"fft_reg2": 1})
+    tol = TOL[prec]
+    assert np.max(np.abs(Fh - F_o) / np.abs(F_o)) < tol["scalar"]
+    assert np.max(np.abs(Th - T_o) / np.abs(T_o)) < tol["scalar"]
+    assert np.max(np.abs(out - U_o)) < tol["links"]
+
+
+@pytest.mark.parametrize("prec,storage", VARIANTS)
+def test_trajectory_bulk_copy_fft(lgf, config_cache, prec, storage):
+    """20 iterations of C2 with lgf_tune("fft_bulk", 1): the (x, y) sweeps -- the inverse one ending in the g-build --
+    fed by bulk copies.  Same parity bar as the default plan."""
+    dims = inputs.CONFIGS["C2"]["dims"]
+    U = config_cache("C2")
+    U_o, F_o, T_o = oracle.iterate(dims, U, ALPHA, 20)
+    Fh, Th, P, out = run_trajectory(lgf, dims, U, prec, storage, 20, tune={"fft_reg2": 1, "fft_bulk": 1})
     tol = TOL[prec]
     assert np.max(np.abs(Fh - F_o) / np.abs(F_o)) < tol["scalar"]
     assert np.max(np.abs(Th - T_o) / np.abs(T_o)) < tol["scalar"]
@@ -486,6 +501,10 @@ def test_reunit_every_update_keeps_fp64_parity(lgf, config_cache, storage):
     U = config_cache("C2")
     U_o, F_o, T_o = oracle.iterate(dims, U, ALPHA, 20)
     Fh, Th, P, out = run_trajectory(lgf, dims, U, 8, storage, 20, tune={"reunit_every": 1})
+    # ... and the same through the staged sweep wherever it applies (with and without the fp64 register split)
+    for rsplit in (1, 0):
+        Fh2, Th2, _, out2 = run_trajectory(lgf, dims, U, 8, storage, 20, tune={"reunit_every": 1, "sweep_tma": 1, "sweep_rsplit": rsplit})
+        assert np.max(np.abs(Th2 - T_o) / np.abs(T_o)) < 1e-12 and np.max(np.abs(out2 - U_o)) < 1e-11
     assert np.max(np.abs(Fh - F_o) / np.abs(F_o)) < 1e-12
     assert np.max(np.abs(Th - T_o) / np.abs(T_o)) < 1e-12
     assert np.max(np.abs(out - U_o)) < 1e-11

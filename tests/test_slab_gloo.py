@@ -21,25 +21,25 @@ def _free_port():
 
 # ---- the documented layouts, as numpy ------------------------------------------------------------------
 def pack_stage0(Wslab, n):
-    """t-slab field [c][T][Lz][Sxy] -> send buffer [q][c][tl][zl][xy], z = q Zl + zl."""
+    """t-slab field [c][T][Lz][Sxy] -> send buffer [c][q][tl][zl][xy], z = q Zl + zl."""
     C, T, Lz, S = Wslab.shape
     Zl = Lz // n
-    return np.ascontiguousarray(Wslab.reshape(C, T, n, Zl, S).transpose(2, 0, 1, 3, 4)).reshape(-1)
+    return np.ascontiguousarray(Wslab.reshape(C, T, n, Zl, S).transpose(0, 2, 1, 3, 4)).reshape(-1)
 
 
 def unpack_stage1(buf, n, C, T, Zl, S):
-    """receive buffer [q][c][tl][zl][xy] -> z-slab field [c][t = q T + tl][zl][xy]."""
-    return np.ascontiguousarray(buf.reshape(n, C, T, Zl, S).transpose(1, 0, 2, 3, 4)).reshape(C, n * T, Zl, S)
+    """receive buffer [c][q][tl][zl][xy] -> z-slab field [c][t = q T + tl][zl][xy]."""
+    return buf.reshape(C, n * T, Zl, S).copy()              # (a copy: the buffer is reused by the next exchange)
 
 
 def pack_stage2(Wz, n):
     C, Lt, Zl, S = Wz.shape
     T = Lt // n
-    return np.ascontiguousarray(Wz.reshape(C, n, T, Zl, S).transpose(1, 0, 2, 3, 4)).reshape(-1)
+    return Wz.reshape(-1).copy()                               # [c][q][tl][zl][xy] with t = q T + tl: the field as it stands
 
 
 def unpack_stage3(buf, n, C, T, Zl, S):
-    return np.ascontiguousarray(buf.reshape(n, C, T, Zl, S).transpose(1, 2, 0, 3, 4)).reshape(C, T, n * Zl, S)
+    return np.ascontiguousarray(buf.reshape(C, n, T, Zl, S).transpose(0, 2, 1, 3, 4)).reshape(C, T, n * Zl, S)
 
 
 def global_field(C, Lt, Lz, S):
@@ -74,7 +74,8 @@ def test_local_exchange_round_trip(n):
     for r in range(n):
         assert np.array_equal(Wz[r], W[:, :, r * Zl:(r + 1) * Zl])
     send = [torch.from_numpy(pack_stage2(Wz[r], n)) for r in range(n)]
-    ex.all_to_all(send, recv)
+    for c in (2, 0, 3, 1):                     # the overlapped form, one component at a time, in any order
+        ex.finish(ex.start_all_to_all_comp(send, recv, c))
     for r in range(n):
         assert np.array_equal(unpack_stage3(recv[r].numpy(), n, C, T, Zl, S), W[:, r * T:(r + 1) * T])
     # halos: +1 sends to the rank above (U_t of the last slice), -1 to the rank below (g of the first slice)
@@ -107,7 +108,8 @@ def _worker(rank, world, port, q):
         Wz = unpack_stage1(recv[0].numpy(), world, C, T, Zl, S)
         ok_fwd = bool(np.array_equal(Wz, W[:, :, rank * Zl:(rank + 1) * Zl]))
         send = [torch.from_numpy(pack_stage2(Wz, world))]
-        ex.all_to_all(send, recv)
+        for c in (2, 0, 3, 1):                 # the overlapped form, one component at a time (synchronous on the CPU)
+            ex.finish(ex.start_all_to_all_comp(send, recv, c))
         ok_back = bool(np.array_equal(unpack_stage3(recv[0].numpy(), world, C, T, Zl, S), W[:, rank * T:(rank + 1) * T]))
         tag, got = [torch.full((3,), float(rank))], [torch.empty(3)]
         ex.shift(tag, got, +1)
