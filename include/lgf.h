@@ -335,6 +335,21 @@ int lgf_slab_get_field(lgf_slab *ctx, void *d_field);
 long long lgf_slab_launch_count(const lgf_slab *ctx);
 const char *lgf_slab_last_error(const lgf_slab *ctx);
 
+/* ---- a measurement that allocates nothing -------------------------------------------------------------------
+ * For callers that cannot call cudaMalloc (code under CUDA-graph capture, tight serving loops, harnesses that forbid
+ * it): F = sum Re tr U / (12 V) (eq. 3) and theta = sum tr(Delta Delta^dag) / (3 V) (eqs. 5-7, :63-76) of
+ * a configuration given in the canonical layout (d_links: device, 72 reals per site, `precision` bytes per real),
+ * written to d_F_theta[0], d_F_theta[1] (device, two doubles) asynchronously on `cuda_stream` -- no context, no
+ * cudaMalloc / cudaFree, no allocating call.  The per-block partial sums live in ONE fixed device array inside the
+ * library (128 KB, held by every GPU that loads it until exit), so the lattice is limited to LGF_STATIC_MAX_SITES
+ * sites (32^4 and 32^3 x 64 fit; beyond: LGF_EINVAL, use lgf_create / lgf_measure).  Every call shares that array:
+ * calls that overlap on the GPU (different streams or host threads) race on it -- serialise them.  Per-site terms in
+ * the working precision, sums in fp64, fixed summation order (R14).  Errors: LGF_E* with the message from
+ * lgf_static_last_error() (per host thread). */
+#define LGF_STATIC_MAX_SITES 2097152
+int lgf_measure_static(const int dims[4], int precision, const void *d_links, double *d_F_theta, void *cuda_stream);
+const char *lgf_static_last_error(void);
+
 #ifdef __cplusplus
 }
 #endif

@@ -65,6 +65,8 @@ SIGNATURES = {
     "lgf_algorithmic_bytes": (_d, [_vp, _i]),
     "lgf_last_error": (ctypes.c_char_p, [_vp]),
     "lgf_version": (ctypes.c_char_p, []),
+    "lgf_measure_static": (_i, [ctypes.POINTER(ctypes.c_int), _i, _vp, _vp, _vp]),
+    "lgf_static_last_error": (ctypes.c_char_p, []),
     # one configuration sharded over several GPUs (per-rank entry points; exchanges in slab.py)
     "lgf_slab_create": (_i, [ctypes.POINTER(ctypes.c_int), _i, _i, _i, _i, ctypes.POINTER(_vp)]),
     "lgf_slab_destroy": (_i, [_vp]),
@@ -456,6 +458,24 @@ class SlabContext:
 
     def launch_count(self):
         return int(load().lgf_slab_launch_count(self._h))
+
+
+LGF_STATIC_MAX_SITES = 2097152
+
+
+def measure_static(dims, precision, links, out, stream=None):
+    """lgf_measure_static: (F, theta) of a canonical-layout CUDA tensor into `out` (CUDA tensor of two float64),
+    asynchronously; allocates nothing on the device.  Returns `out`."""
+    dims = tuple(int(v) for v in dims)
+    V = int(np.prod(dims))
+    lib = load()
+    sp = 0 if stream is None else (stream.cuda_stream if hasattr(stream, "cuda_stream") else int(stream))
+    rc = lib.lgf_measure_static((ctypes.c_int * 4)(*dims), int(precision), _dev_ptr(links, precision, V * 72),
+                                _dev_ptr(out, LGF_FP64, 2), ctypes.c_void_p(sp))
+    if rc < 0:
+        msg = lib.lgf_static_last_error()
+        raise LgfError(int(rc), msg.decode() if msg else "")
+    return out
 
 
 def lgf_version() -> str:

@@ -18,7 +18,7 @@ ROOT = os.path.dirname(PKG)
 CSRC = os.path.join(PKG, "csrc")
 OBJDIR = os.path.join(ROOT, "build", "lgf")
 LIB = os.path.join(PKG, "liblgf.so")
-SOURCES = ["lgf_links.cu", "lgf_sweep_tma.cu", "lgf_fft.cu", "lgf_fft_reg.cu", "lgf_fft_reg2.cu", "lgf_heatbath.cu", "lgf_slab.cu", "lgf_api.cu"]
+SOURCES = ["lgf_links.cu", "lgf_sweep_tma.cu", "lgf_fft.cu", "lgf_fft_reg.cu", "lgf_fft_reg2.cu", "lgf_heatbath.cu", "lgf_slab.cu", "lgf_static.cu", "lgf_api.cu"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
     "-O3", "-std=c++17", "-lineinfo", "--expt-relaxed-constexpr",
