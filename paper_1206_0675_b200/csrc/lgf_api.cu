@@ -60,7 +60,8 @@ struct lgf_ctx {
     int tune_reunit = 0;         // lgf_tune "reunit_every": project the new links onto SU(3) in every N-th update (0 = never)
     long long updates_enqueued = 0;   // host-side count of updates enqueued since the last set_links / thermalize
     int tune_pdl = 1;            // lgf_tune "pdl": launch the iteration's kernels with programmatic stream serialization
-    int tune_fft_bulk = 0;       // lgf_tune "fft_bulk": (x, y) FFT sweeps fed by cp.async.bulk (ablation; measured in DESIGN.md)
+    int tune_fft_bulk = -1;      // lgf_tune "fft_bulk": (x, y) FFT sweeps fed by cp.async.bulk: 1 / 0 / -1 = where it measured
+                                 // faster (64-point fp64 planes: 64^4 FFT 1.98 -> 1.81 ms; neutral at 32^4 and 16^4)
     int tune_sweep_tma = -1;     // lgf_tune "sweep_tma" (see use_sweep_tma)
     int tune_sweep_rsplit = 1;   // lgf_tune "sweep_rsplit": register split between producer and compute warps (fp64 staged sweep)
     int tune_sweep_ahead = 0;    // lgf_tune "sweep_prefetch": CTAs ahead of which the sweep prefetches its tile into L2 (0 = off)
@@ -347,6 +348,9 @@ static int step_delta(lgf_ctx *ctx, const int *stop) {
                        STRM(ctx)));
     return LGF_OK;
 }
+static bool use_fft_bulk(const lgf_ctx *ctx) {
+    return ctx->tune_fft_bulk > 0 || (ctx->tune_fft_bulk < 0 && ctx->g.L[0] == 64 && ctx->prec == LGF_FP64);
+}
 // true if the plan's last sweep can end with the g-build (a5) and write G instead of W
 static bool can_fuse_g(const lgf_ctx *ctx) {
     if (!ctx->tune_fuse_g || ctx->passes.empty()) return false;
@@ -368,7 +372,7 @@ static int step_accelerate(lgf_ctx *ctx, bool with_g = false, double alpha = 0.0
         if (p.kind == PASS_REG2) {
             const int which = (with_g && p.axis == 2) ? 3 : p.axis;
             CK(launch_fft_reg2<R>(which, ctx->g, (C<R> *)ctx->W, (const R *)ctx->p2tab, scale, ctx->st, STRM(ctx),
-                                  (C<R> *)ctx->G, (R)(0.5 * alpha), ctx->tune_fft_bulk != 0));
+                                  (C<R> *)ctx->G, (R)(0.5 * alpha), use_fft_bulk(ctx)));
             continue;
         }
         const R *tw[4] = {(const R *)ctx->twiddle[0], (const R *)ctx->twiddle[1], (const R *)ctx->twiddle[2],
@@ -1082,7 +1086,7 @@ int lgf_kernel_names(const lgf_ctx *ctx, char *buf, int cap) {
     for (size_t i = 0; i < ctx->passes.size(); i++) {
         const AxisPass &p = ctx->passes[i];
         if (i) s += "|";
-        if (p.kind == PASS_REG2) s += fft_reg2_kernel_name((fuse && p.axis == 2) ? 3 : p.axis, ctx->g, ctx->prec);
+        if (p.kind == PASS_REG2) s += fft_reg2_kernel_name((fuse && p.axis == 2) ? 3 : p.axis, ctx->g, ctx->prec, use_fft_bulk(ctx));
         else if (p.kind == PASS_REG) s += p.axis == 1 ? "k_fftr_zt<" : "k_fftr_xy<";
         else s += p.kind == PASS_XY ? "k_fft_xy<" : (p.kind == PASS_ZT ? "k_fft_zt<" : "k_fft_axis<");
     }

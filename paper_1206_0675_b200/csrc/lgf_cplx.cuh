@@ -32,6 +32,32 @@ template <class R> __host__ __device__ __forceinline__ void madc(C<R> &acc, C<R>
 }
 template <class R> __host__ __device__ __forceinline__ R norm2(C<R> a) { return a.x * a.x + a.y * a.y; }
 
+// 1 / x and 1 / sqrt(x) for positive normal x.  In double precision the IEEE-exact `a / b` and `1 / sqrt(x)` each
+// expand to a hardware seed plus a dozen instructions with slow-path branches; the hot kernels call them 16 times per
+// thread (the p2max / p2 factors of the t lines) and twice per g(x).  Here: the 20-bit hardware seed and three Newton
+// steps (error below 2 ulp of double, no branches) -- inside every parity tolerance.  Single
+// precision keeps the compiler's correctly rounded division and square root.
+__device__ __forceinline__ double inv_pos(double x) {
+    double r;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+#pragma unroll
+    for (int k = 0; k < 3; k++) r = fma(r, fma(-x, r, 1.0), r);
+    return r;
+}
+__device__ __forceinline__ float inv_pos(float x) { return 1.0f / x; }
+// s / x with x > 0: the branch-free reciprocal in double, the plain division in single precision
+__device__ __forceinline__ double div_pos(double s, double x) { return s * inv_pos(x); }
+__device__ __forceinline__ float div_pos(float s, float x) { return s / x; }
+__device__ __forceinline__ double inv_sqrt_pos(double x) {
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    const double h = 0.5 * x;
+#pragma unroll
+    for (int k = 0; k < 3; k++) y = fma(y, fma(-h * y, y, 0.5), y);
+    return y;
+}
+__device__ __forceinline__ float inv_sqrt_pos(float x) { return 1.0f / sqrtf(x); }   // (rsqrtf, 2 ulp, let the fp32 links drift: plaquette 1.5e-6 after 20 updates)
+
 // compile-time loop: f(std::integral_constant<int, i>) for i in [B, E)
 template <int B, int E, class F>
 __host__ __device__ __forceinline__ void static_for(F &&f) {

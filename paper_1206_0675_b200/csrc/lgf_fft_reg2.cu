@@ -218,11 +218,16 @@ struct Zt2Shape {
     static constexpr int LINES = XC * (LZ > LT ? LZ : LT);
     static constexpr int THREADS = 2 * LINES;
     static constexpr size_t SMEM = sizeof(C<R>) * (size_t)PITCH * LT;
+    // at least two CTAs per SM where the tile allows it: caps the registers at 128 for 256 threads (the compiler
+    // otherwise spends 134 on overlapping the 16 reciprocals of the scale step, which halves the occupancy)
+    // (not for 64-point fp64 lines, which need the registers; asking for 1 is not neutral either: the fp32 64 x 64 sweep
+    // then takes 168 registers instead of 128 and loses its second CTA -- 64^4 fp32 FFT 1.17 -> 1.35 ms)
+    static constexpr int MINB = (SMEM <= 110 * 1024 && (sizeof(R) == 4 || (LZ <= 32 && LT <= 32))) ? 2 : 1;
     static_assert((XC * LZ) % 16 == 0 && (XC * LT) % 16 == 0, "16 lines per warp");
 };
 
 template <class R, int LZ, int LT, int XC>
-__global__ void __launch_bounds__((Zt2Shape<R, LZ, LT, XC>::THREADS))
+__global__ void __launch_bounds__((Zt2Shape<R, LZ, LT, XC>::THREADS), (Zt2Shape<R, LZ, LT, XC>::MINB))
     k_fftr2_zt(C<R> *__restrict__ W, Geom g, const R *__restrict__ p2tab, R scale, const DevState *__restrict__ st) {
     pdl_enter();
     if (st->done) return;
@@ -262,7 +267,7 @@ __global__ void __launch_bounds__((Zt2Shape<R, LZ, LT, XC>::THREADS))
 #pragma unroll
         for (int j = 0; j < MT; j++) {
             const R p2 = p2xyz + p2tab[192 + 2 * j + h];
-            const R f = (p2 == (R)0) ? (R)0 : scale / p2;     // Alg. 1 lines 5, 7; zero mode -> 0 (R6)
+            const R f = (p2 == (R)0) ? (R)0 : div_pos(scale, p2);     // Alg. 1 lines 5, 7; zero mode -> 0 (R6)
             v[j] = f * v[j];
         }
         ST::inverse(v, h);                                    // -> t = m + MT h
@@ -426,8 +431,10 @@ static std::string reg2_name(int which, const Geom &g) {
 #undef LGF_GO
     return buf;
 }
-std::string fft_reg2_kernel_name(int which, const Geom &g, int prec) {
-    return prec == 8 ? reg2_name<double>(which, g) : reg2_name<float>(which, g);
+std::string fft_reg2_kernel_name(int which, const Geom &g, int prec, bool bulk) {
+    std::string s = prec == 8 ? reg2_name<double>(which, g) : reg2_name<float>(which, g);
+    if (bulk && which != 1 && s.size() > 10) s.insert(10, "_bulk");      // k_fftr2_xy -> k_fftr2_xy_bulk
+    return s;
 }
 
 template cudaError_t launch_fft_reg2<float>(int, const Geom &, C<float> *, const float *, float, const DevState *,

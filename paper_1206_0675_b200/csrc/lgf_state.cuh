@@ -153,7 +153,7 @@ cudaError_t launch_sweep_tma(const SweepMaps *maps, int nr, LinkPair<R> links, c
 std::string sweep_tma_kernel_name(const Geom &g, int nr, int prec, bool reunit, bool rsplit);
 
 // kernel instantiations as a profiler names them (lgf_kernel_names)
-std::string fft_reg2_kernel_name(int which, const Geom &g, int prec);
+std::string fft_reg2_kernel_name(int which, const Geom &g, int prec, bool bulk = false);
 std::string sweep_kernel_name(const Geom &g, int nr, int prec, bool reunit, int share_mode, int minb);
 bool sweep_uses_share(const Geom &g, int nr, int prec, int share_mode);
 // block order of a sweep whose CTAs take `nt` consecutive sites: (z, t)-tiled when a t slice of traffic exceeds L2

@@ -117,7 +117,7 @@ template <class R>
 __device__ __forceinline__ void build_g(const Herm<R> &w, R h, C<R> (&g)[9]) {
     C<R> a0 = mk<R>((R)1, h * w.m00), a1 = mk<R>(-h * w.m01.y, h * w.m01.x), a2 = mk<R>(-h * w.m02.y, h * w.m02.x);
     C<R> b0 = mk<R>(h * w.m01.y, h * w.m01.x), b1 = mk<R>((R)1, h * w.m11), b2 = mk<R>(-h * w.m12.y, h * w.m12.x);
-    const R ia = (R)1 / sqrt(norm2(a0) + norm2(a1) + norm2(a2));
+    const R ia = inv_sqrt_pos(norm2(a0) + norm2(a1) + norm2(a2));
     a0 = ia * a0; a1 = ia * a1; a2 = ia * a2;
     // ab = sum_j conj(a_j) b_j ;  b -= ab * a
     C<R> ab = mk<R>(0, 0);
@@ -125,7 +125,7 @@ __device__ __forceinline__ void build_g(const Herm<R> &w, R h, C<R> (&g)[9]) {
     ab = ab + mulc(b1, a1);
     ab = ab + mulc(b2, a2);
     b0 = b0 - ab * a0; b1 = b1 - ab * a1; b2 = b2 - ab * a2;
-    const R ib = (R)1 / sqrt(norm2(b0) + norm2(b1) + norm2(b2));
+    const R ib = inv_sqrt_pos(norm2(b0) + norm2(b1) + norm2(b2));
     b0 = ib * b0; b1 = ib * b1; b2 = ib * b2;
     g[0] = a0; g[1] = a1; g[2] = a2;
     g[3] = b0; g[4] = b1; g[5] = b2;
