@@ -220,9 +220,9 @@ struct Zt2Shape {
     static constexpr size_t SMEM = sizeof(C<R>) * (size_t)PITCH * LT;
     // at least two CTAs per SM where the tile allows it: caps the registers at 128 for 256 threads (the compiler
     // otherwise spends 134 on overlapping the 16 reciprocals of the scale step, which halves the occupancy)
-    // (not for 64-point fp64 lines, which need the registers; asking for 1 is not neutral either: the fp32 64 x 64 sweep
-    // then takes 168 registers instead of 128 and loses its second CTA -- 64^4 fp32 FFT 1.17 -> 1.35 ms)
-    static constexpr int MINB = (SMEM <= 110 * 1024 && (sizeof(R) == 4 || (LZ <= 32 && LT <= 32))) ? 2 : 1;
+    // (fp64 lines of up to 32 points only; 0 = no request, which is NOT the same as asking for 1: with "1" the fp32
+    // 64 x 64 sweep took 168 registers instead of 128 and lost its second CTA -- 64^4 fp32 FFT 1.17 -> 1.35 ms)
+    static constexpr int MINB = (sizeof(R) == 8 && SMEM <= 110 * 1024 && LZ <= 32 && LT <= 32) ? 2 : 0;
     static_assert((XC * LZ) % 16 == 0 && (XC * LT) % 16 == 0, "16 lines per warp");
 };
 
