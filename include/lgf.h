@@ -188,8 +188,14 @@ int lgf_apply_transform(lgf_ctx *ctx, const void *d_transform);
  * same for the thread order of lgf_thermalize / lgf_overrelax, 0 = automatic),
  * "sweep_share" (1 / 0 / -1 = automatic: backward x, y neighbours of the same CTA hand over their algebra parts
  * through shared memory instead of being recomputed), "pdl" (1 / 0: programmatic dependent launch of the
- * iteration's kernels, so that each kernel's launch overlaps the tail of the one before -- the one key that is
- * process-wide rather than per context), "reunit_every" (N > 0: in every
+ * iteration's kernels, so that each kernel's launch overlaps the tail of the one before),
+ * "sweep_tma" (1 / 0 / -1 = where it measured faster: the persistent staged sweep fed by TMA tensor copies,
+ * k_sweep_tma, instead of the register sweep), "sweep_rsplit" (1 / 0: the staged sweep's fp64 register split by
+ * setmaxnreg), "sweep_prefetch" (CTAs ahead of which the register sweep prefetches its tile into L2, 0 = off), "sweep_minb"
+ * (3 / 2: resident CTAs per SM the register sweep's register allocation allows), "fft_bulk" (1 / 0 / -1 = where it measured faster: (x, y) FFT
+ * sweeps fed by cp.async.bulk), "fft_zt_cluster" (2 / 4: a 64 x 64 (z, t) FFT tile split over a thread-block
+ * cluster of that many CTAs with the transposition through distributed shared memory, k_fftr2_zt_cluster; 0 /
+ * -1 = the one-CTA tile, which measured faster), "reunit_every" (N > 0: in every
  * N-th update the new links are projected back onto SU(3) inside the sweep; 0 = never, the method as the
  * paper states it -- this key DOES change the result, by the rounding drift it removes; meant for fp32 runs
  * of thousands of iterations).

@@ -60,6 +60,7 @@ struct lgf_ctx {
     int tune_reunit = 0;         // lgf_tune "reunit_every": project the new links onto SU(3) in every N-th update (0 = never)
     long long updates_enqueued = 0;   // host-side count of updates enqueued since the last set_links / thermalize
     int tune_pdl = 1;            // lgf_tune "pdl": launch the iteration's kernels with programmatic stream serialization
+    int tune_fft_zt_cluster = -1; // lgf_tune "fft_zt_cluster": (z, t) tile split over a cluster of 2 / 4 CTAs; 0 = off; -1 = where it measured
     int tune_fft_bulk = -1;      // lgf_tune "fft_bulk": (x, y) FFT sweeps fed by cp.async.bulk: 1 / 0 / -1 = where it measured
                                  // faster (64-point fp64 planes: 64^4 FFT 1.98 -> 1.81 ms; neutral at 32^4 and 16^4)
     int tune_sweep_tma = -1;     // lgf_tune "sweep_tma" (see use_sweep_tma)
@@ -351,6 +352,11 @@ static int step_delta(lgf_ctx *ctx, const int *stop) {
 static bool use_fft_bulk(const lgf_ctx *ctx) {
     return ctx->tune_fft_bulk > 0 || (ctx->tune_fft_bulk < 0 && ctx->g.L[0] == 64 && ctx->prec == LGF_FP64);
 }
+static int use_zt_cluster(const lgf_ctx *ctx) {
+    const int nc = ctx->tune_fft_zt_cluster;
+    if (nc > 0) return fft_reg2_zt_cluster_supported(ctx->g, nc) ? nc : 0;
+    return 0;                                                // automatic = off: it measured slower
+}
 // true if the plan's last sweep can end with the g-build (a5) and write G instead of W
 static bool can_fuse_g(const lgf_ctx *ctx) {
     if (!ctx->tune_fuse_g || ctx->passes.empty()) return false;
@@ -372,7 +378,7 @@ static int step_accelerate(lgf_ctx *ctx, bool with_g = false, double alpha = 0.0
         if (p.kind == PASS_REG2) {
             const int which = (with_g && p.axis == 2) ? 3 : p.axis;
             CK(launch_fft_reg2<R>(which, ctx->g, (C<R> *)ctx->W, (const R *)ctx->p2tab, scale, ctx->st, STRM(ctx),
-                                  (C<R> *)ctx->G, (R)(0.5 * alpha), use_fft_bulk(ctx)));
+                                  (C<R> *)ctx->G, (R)(0.5 * alpha), use_fft_bulk(ctx), -1, use_zt_cluster(ctx)));
             continue;
         }
         const R *tw[4] = {(const R *)ctx->twiddle[0], (const R *)ctx->twiddle[1], (const R *)ctx->twiddle[2],
@@ -1044,6 +1050,7 @@ int lgf_tune(lgf_ctx *ctx, const char *key, int value) {
     else if (k == "sweep_share") ctx->tune_sweep_share = value;
     else if (k == "sweep_tma") ctx->tune_sweep_tma = value;
     else if (k == "fft_bulk") ctx->tune_fft_bulk = value;
+    else if (k == "fft_zt_cluster") ctx->tune_fft_zt_cluster = value;
     else if (k == "sweep_rsplit") ctx->tune_sweep_rsplit = value;
     else if (k == "sweep_prefetch") ctx->tune_sweep_ahead = value < 0 ? 0 : value;
     else if (k == "sweep_minb") ctx->tune_sweep_minb = value == 2 ? 2 : 3;
@@ -1086,7 +1093,7 @@ int lgf_kernel_names(const lgf_ctx *ctx, char *buf, int cap) {
     for (size_t i = 0; i < ctx->passes.size(); i++) {
         const AxisPass &p = ctx->passes[i];
         if (i) s += "|";
-        if (p.kind == PASS_REG2) s += fft_reg2_kernel_name((fuse && p.axis == 2) ? 3 : p.axis, ctx->g, ctx->prec, use_fft_bulk(ctx));
+        if (p.kind == PASS_REG2) s += fft_reg2_kernel_name((fuse && p.axis == 2) ? 3 : p.axis, ctx->g, ctx->prec, use_fft_bulk(ctx), use_zt_cluster(ctx));
         else if (p.kind == PASS_REG) s += p.axis == 1 ? "k_fftr_zt<" : "k_fftr_xy<";
         else s += p.kind == PASS_XY ? "k_fft_xy<" : (p.kind == PASS_ZT ? "k_fft_zt<" : "k_fft_axis<");
     }

@@ -207,6 +207,78 @@ __global__ void __launch_bounds__(2 * P * L) k_fftr2_xy_bulk(C<R> *__restrict__ 
     (void)base;
 }
 
+// ---- inverse (x, y) sweep ending in the g-build where the four component planes do NOT fit in one SM ----------
+// 64^4 fp64: a plane is 64 KB, so a CTA holds one component of one (z, t) slice and a5 -- which needs all of w(x) --
+// used to be a separate pass over the field (k_gbuild: 1.07 GB read + 1.6 GB written, 0.39 ms of a 6.5 ms iteration,
+// and the sweep before it wrote w only for that pass to read it back).  Here the four CTAs that hold the four
+// components of a slice form a THREAD-BLOCK CLUSTER: each transforms its plane (brought on chip by one bulk copy),
+// the cluster synchronises, and every CTA builds g for a quarter of the slice's sites, reading the other three
+// components out of its neighbours' shared memory (distributed shared memory, ld.shared::cluster: 3 x 16 KB per CTA and
+// plane).  w is never written; rows 0, 1 of g go straight to G.
+template <class R, int L>
+__global__ void __cluster_dims__(4, 1, 1) __launch_bounds__(2 * L, 3)
+    k_fftr2_xy_gcluster(C<R> *__restrict__ W, const DevState *__restrict__ st, C<R> *__restrict__ G, long long V, int nzt, R half_alpha) {
+    pdl_enter();
+    if (st->done) return;                                    // (the same decision in all four CTAs of a cluster)
+    constexpr int M = L / 2;
+    constexpr int PX = L | 1;
+    constexpr unsigned PLANE_BYTES = L * L * sizeof(C<R>);
+    using S = SplitDft<L, PAIR_MASK, R>;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    C<R> *tile = reinterpret_cast<C<R> *>(smem_raw);
+    __shared__ uint64_t bar;
+    const int tid = threadIdx.x;
+    const int h = (tid >> 4) & 1;
+    const int i = (tid >> 5) * 16 + (tid & 15);
+    const unsigned c = cluster_ctarank();                    // packed component = rank in the cluster
+    const long long slice = blockIdx.x / 4;
+    if (tid == 0) {
+        mbar_init(&bar, 1);
+        mbar_init_fence();
+        mbar_arrive_expect_tx(&bar, PLANE_BYTES);
+        bulk_g2s(tile, W + ((long long)c * nzt + slice) * (L * L), PLANE_BYTES, &bar);
+    }
+    __syncthreads();
+    mbar_wait(&bar, 0);
+    C<R> v[M];
+#pragma unroll
+    for (int j = 0; j < M; j++) v[j] = tile[(2 * j + h) * L + i];            // kx = 2 j + h at ky = i (dense plane)
+    __syncthreads();
+    S::inverse(v, h);
+#pragma unroll
+    for (int m = 0; m < M; m++) tile[i * PX + m + M * h] = v[m];             // tile[ky][x]
+    __syncthreads();
+#pragma unroll
+    for (int j = 0; j < M; j++) v[j] = tile[(2 * j + h) * PX + i];           // column x = i, ky = 2 j + h
+    S::inverse(v, h);
+    __syncthreads();
+#pragma unroll
+    for (int m = 0; m < M; m++) tile[(m + M * h) * PX + i] = v[m];           // tile[y][x] of this component
+    cluster_sync_all();                                                      // all four components are in place
+    const uint32_t t0 = smem_u32(tile);
+    uint32_t tk[4];
+#pragma unroll
+    for (int k = 0; k < 4; k++) tk[k] = dsmem_map(t0, k);
+    const long long s0 = slice * (L * L);
+    const int sub = (int)c * 2 + h;                                          // 0 .. 7: this thread's rows y = sub + 8 mm
+#pragma unroll 2
+    for (int mm = 0; mm < L / 8; mm++) {
+        const int y = sub + 8 * mm;
+        const uint32_t off = (uint32_t)((y * PX + i) * sizeof(C<R>));
+        Herm<R> w;
+        dsmem_ld(tk[0] + off, w.m01.x, w.m01.y);
+        dsmem_ld(tk[1] + off, w.m02.x, w.m02.y);
+        dsmem_ld(tk[2] + off, w.m12.x, w.m12.y);
+        dsmem_ld(tk[3] + off, w.m00, w.m11);
+        C<R> gx[9];
+        build_g(w, half_alpha, gx);
+        const long long s = s0 + y * L + i;
+#pragma unroll
+        for (int e = 0; e < 6; e++) G[(long long)e * V + s] = gx[e];
+    }
+    cluster_sync_all();                                                      // nobody leaves while its tile is being read
+}
+
 // ---- (z, t) planes --------------------------------------------------------------------------------
 // grid = ((Lx Ly) / XC, 4 components).  Shared-memory element (xc, z, t) at xc + XC z + PITCH t, PITCH =
 // XC LZ + padding (the 8-lane phases of the z-line stores, lanes (xc, t), land on distinct banks).
@@ -286,6 +358,90 @@ __global__ void __launch_bounds__((Zt2Shape<R, LZ, LT, XC>::THREADS), (Zt2Shape<
     }
 }
 
+// ---- (z, t) tile split over a thread-block cluster ----------------------------------------------------
+// 64 x 64 fp64: the tile of XC = 2 consecutive (kx, ky) indices is 128 KB, so k_fftr2_zt runs ONE CTA of 256 threads per
+// SM and its load, transform and store phases cannot overlap with anything (ncu at 64^4: 0.99 ms for 2.09 GB,
+// fp64 pipe 32 % busy, DRAM 33 %).  Here NC CTAs of a cluster share the tile: CTA q holds the z lines of t in
+// [q Lt / NC, (q + 1) Lt / NC) and, for the t lines, the rows kz in [q Lz / NC, (q + 1) Lz / NC) -- a 1 / NC part
+// either way, 64 KB + padding, so three CTAs of different clusters are resident per SM and their phases overlap.
+// The transposition z lines <-> t lines crosses the cluster through distributed shared memory: after the forward z
+// transform a thread stores its kz values into the tile of the CTA that owns them (st.shared::cluster), and before
+// the inverse z transform it loads them from there (ld.shared::cluster); the t-line round trip (forward, scale,
+// inverse) is local.  Element (xc, kz_local, t) of a CTA's part at t PITCH + kz_local XC + xc.
+template <class R, int LZ, int XC, int NC>
+struct Zt2ClusterShape {
+    static constexpr int PHASE = 128 / (int)sizeof(C<R>);
+    static constexpr int ROW = XC * LZ / NC;                                  // t-line lines of one CTA = elements per t
+    static constexpr int PITCH = ROW + ((XC < PHASE && ROW % PHASE == 0) ? XC : 0);
+    static constexpr int THREADS = 2 * ROW;
+    static constexpr size_t SMEM = sizeof(C<R>) * (size_t)PITCH * LZ;         // (Lt = Lz)
+    static constexpr int MINB = sizeof(R) == 8 ? 3 : 2;
+    static_assert(ROW % 16 == 0 && (LZ / 2) % NC == 0, "16 lines per warp; whole kz ranges per thread half");
+};
+
+template <class R, int LZ, int XC, int NC>
+__global__ void __cluster_dims__(NC, 1, 1)
+    __launch_bounds__((Zt2ClusterShape<R, LZ, XC, NC>::THREADS), (Zt2ClusterShape<R, LZ, XC, NC>::MINB))
+        k_fftr2_zt_cluster(C<R> *__restrict__ W, Geom g, const R *__restrict__ p2tab, R scale, const DevState *__restrict__ st) {
+    pdl_enter();
+    if (st->done) return;                                    // (the same decision in every CTA of a cluster)
+    cluster_arrive();                                        // "I have started": waited for before the first remote store
+    using Sh = Zt2ClusterShape<R, LZ, XC, NC>;
+    constexpr int PITCH = Sh::PITCH, M = LZ / 2, LQ = LZ / NC;
+    using S = SplitDft<LZ, PAIR_MASK, R>;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    C<R> *tile = reinterpret_cast<C<R> *>(smem_raw);
+    const long long plane = g.S[2];
+    const int q = (int)cluster_ctarank();
+    const int lo0 = (blockIdx.x / NC) * XC;
+    C<R> *Wc = W + (long long)blockIdx.y * g.V + lo0;
+    const int tid = threadIdx.x;
+    const int h = (tid >> 4) & 1;
+    const int l = (tid >> 5) * 16 + (tid & 15);               // line number within this CTA's part
+    const int xc = l % XC, r = l / XC;                        // z lines: t = q LQ + r;  t lines: kz = q LQ + r
+    const int t = q * LQ + r;
+    // shared::cluster address of (xc, kz = 2 j + h, t) in the part that owns kz -- part (2 j + h) / LQ = 2 j / LQ (LQ is
+    // even), at kz_local = (2 j) % LQ + h: a per-part base for this thread plus a compile-time offset
+    uint32_t tk[NC];
+#pragma unroll
+    for (int k = 0; k < NC; k++) tk[k] = dsmem_map(smem_u32(tile), k) + (uint32_t)((t * PITCH + h * XC + xc) * sizeof(C<R>));
+    auto addr_of = [&](int j) { return tk[(2 * j) / LQ] + (uint32_t)(((2 * j) % LQ) * XC * sizeof(C<R>)); };
+
+    C<R> v[M];
+    C<R> *col = Wc + xc + plane * ((long long)LZ * t);
+#pragma unroll
+    for (int m = 0; m < M; m++) v[m] = col[plane * (m + M * h)];
+    S::forward(v, h);                                         // -> kz = 2 j + h
+    cluster_wait();                                           // every CTA of the cluster is resident
+#pragma unroll
+    for (int j = 0; j < M; j++) dsmem_st(addr_of(j), v[j].x, v[j].y);
+    cluster_sync_all();                                       // the parts are complete
+    {                                                         // t line at (xc, kz = q LQ + r): forward, scale, inverse
+#pragma unroll
+        for (int m = 0; m < M; m++) v[m] = tile[(m + M * h) * PITCH + l];
+        S::forward(v, h);                                     // -> kt = 2 j + h
+        const int lo = lo0 + xc, kx = lo / g.L[1], ky = lo % g.L[1];
+        const R p2xyz = p2tab[kx] + p2tab[64 + ky] + p2tab[128 + t];       // (kz = q LQ + r, the same number as t)
+#pragma unroll
+        for (int j = 0; j < M; j++) {
+            const R p2 = p2xyz + p2tab[192 + 2 * j + h];
+            const R f = (p2 == (R)0) ? (R)0 : div_pos(scale, p2);     // Alg. 1 lines 5, 7; zero mode -> 0 (R6)
+            v[j] = f * v[j];
+        }
+        S::inverse(v, h);                                     // -> t = m + M h
+#pragma unroll
+        for (int m = 0; m < M; m++) tile[(m + M * h) * PITCH + l] = v[m];
+    }
+    cluster_sync_all();
+#pragma unroll
+    for (int j = 0; j < M; j++) dsmem_ld(addr_of(j), v[j].x, v[j].y);
+    S::inverse(v, h);                                         // -> z = m + M h   (the loads have landed: their values are used)
+    cluster_arrive();                                         // "I no longer read anyone's part"
+#pragma unroll
+    for (int m = 0; m < M; m++) col[plane * (m + M * h)] = v[m];
+    cluster_wait();                                           // nobody leaves while its part may still be read
+}
+
 // ---- configuration and launchers --------------------------------------------------------------------
 // planes per CTA of the inverse (P; a multiple of 4 allows the g output) and of the forward (PF) (x, y) sweep,
 // and consecutive (kx, ky) indices per CTA of the (z, t) sweep.  Measured at 32^4 on B200 (FFT time per
@@ -345,9 +501,7 @@ bool fft_reg2_xy_by_component(const Geom &g, int prec) {
 bool fft_reg2_xy_gout(const Geom &g, int prec) { return fft_reg2_xy_supported(g) && !(g.L[0] == 64 && prec == 8); }
 // can the inverse (x, y) sweep end with the g-build for this lattice and precision (bytes per real)?
 bool fft_reg2_gout(const Geom &g, int prec) {
-    if (!fft_reg2_supported(g)) return false;
-    if (g.L[0] == 64) return prec == 4;
-    return true;
+    return fft_reg2_supported(g);                            // (64-point fp64 planes: by a 4-CTA cluster, k_fftr2_xy_gcluster)
 }
 
 static thread_local int t_xy_comp = -1;           // >= 0: the forward (x, y) sweep over ONE packed component only (lgf_slab.cu)
@@ -380,7 +534,13 @@ static cudaError_t launch_xy2(int which, const Geom &g, C<R> *W, const DevState 
     if (which == 0) return launch_xy2_as<R, L, FFT_FWD, PF, false>(g, W, st, stream, G, half_alpha);
     if (which == 2) return launch_xy2_as<R, L, FFT_INV, P, false>(g, W, st, stream, G, half_alpha);
     if constexpr (P % 4 == 0) return launch_xy2_as<R, L, FFT_INV, P, true>(g, W, st, stream, G, half_alpha);
-    return cudaErrorInvalidValue;
+    else {                                                   // one plane per CTA: the four components of a slice as a cluster
+        constexpr size_t SM = sizeof(C<R>) * L * (L | 1);
+        auto kern = k_fftr2_xy_gcluster<R, L>;
+        if (cudaError_t e = ensure_dynamic_smem(kern, SM); e != cudaSuccess) return e;
+        return launch_pdl(kern, dim3((unsigned)(4LL * g.L[2] * g.L[3])), dim3(2 * L), SM, stream, W, st, G, g.V, g.L[2] * g.L[3],
+                          half_alpha);
+    }
 }
 
 template <class R, int LZ, int LT>
@@ -393,13 +553,34 @@ static cudaError_t launch_zt2(const Geom &g, C<R> *W, const R *p2tab, R scale, c
     return launch_pdl(kern, grid, dim3(Sh::THREADS), Sh::SMEM, stream, W, g, p2tab, scale, st);
 }
 
+// the cluster-split (z, t) sweep: 64 x 64 (z, t) planes, NC = 2 or 4 CTAs per tile of XC = NC (fp64) / 2 NC (fp32)
+// consecutive (kx, ky) indices -- 32 / 64 contiguous bytes per line element either way
+template <class R, int NC> struct Zt2ClusterCfg { static constexpr int XC = (sizeof(R) == 8 ? 1 : 2) * NC; };
+bool fft_reg2_zt_cluster_supported(const Geom &g, int nc) {
+    return fft_reg2_supported(g) && g.L[2] == 64 && g.L[3] == 64 && (nc == 2 || nc == 4) && g.S[2] % 8 == 0;
+}
+template <class R, int NC>
+static cudaError_t launch_zt2_cluster(const Geom &g, C<R> *W, const R *p2tab, R scale, const DevState *st, LaunchStream stream) {
+    constexpr int XC = Zt2ClusterCfg<R, NC>::XC;
+    using Sh = Zt2ClusterShape<R, 64, XC, NC>;
+    auto kern = k_fftr2_zt_cluster<R, 64, XC, NC>;
+    if (cudaError_t e = ensure_dynamic_smem(kern, Sh::SMEM); e != cudaSuccess) return e;
+    dim3 grid((unsigned)(g.S[2] / XC * NC), 4);
+    return launch_pdl(kern, grid, dim3(Sh::THREADS), Sh::SMEM, stream, W, g, p2tab, scale, st);
+}
+
 // which: 0 = (x, y) forward, 1 = (z, t) forward + scale + inverse, 2 = (x, y) inverse, 3 = (x, y) inverse + g
 template <class R>
 cudaError_t launch_fft_reg2(int which, const Geom &g, C<R> *W, const R *p2tab, R scale, const DevState *st,
-                            LaunchStream stream, C<R> *G, R half_alpha, bool bulk, int comp) {
+                            LaunchStream stream, C<R> *G, R half_alpha, bool bulk, int comp, int zt_cluster) {
     t_xy_bulk = bulk;
     t_xy_comp = comp;
     if (which == 1) {
+        if (zt_cluster > 0) {
+            if (!fft_reg2_zt_cluster_supported(g, zt_cluster)) return cudaErrorInvalidValue;
+            return zt_cluster == 2 ? launch_zt2_cluster<R, 2>(g, W, p2tab, scale, st, stream)
+                                   : launch_zt2_cluster<R, 4>(g, W, p2tab, scale, st, stream);
+        }
 #define LGF_GO(A, B) if (g.L[2] == A && g.L[3] == B) return launch_zt2<R, A, B>(g, W, p2tab, scale, st, stream);
         LGF_REG2_ZT(LGF_GO)
 #undef LGF_GO
@@ -413,10 +594,14 @@ cudaError_t launch_fft_reg2(int which, const Geom &g, C<R> *W, const R *p2tab, R
 
 // the instantiation launch_fft_reg2 picks, as a profiler prints it (bench.py matches ncu captures against it)
 template <class R>
-static std::string reg2_name(int which, const Geom &g) {
+static std::string reg2_name(int which, const Geom &g, int zt_cluster) {
     const char *rn = sizeof(R) == 8 ? "double" : "float";
     char buf[96] = "";
     if (which == 1) {
+        if (zt_cluster > 0) {
+            snprintf(buf, sizeof buf, "k_fftr2_zt_cluster<%s, 64, %d, %d>", rn, (sizeof(R) == 8 ? 1 : 2) * zt_cluster, zt_cluster);
+            return buf;
+        }
 #define LGF_GO(A, B) if (g.L[2] == A && g.L[3] == B) snprintf(buf, sizeof buf, "k_fftr2_zt<%s, %d, %d, %d>", rn, A, B, Zt2Cfg<R, A, B>::XC);
         LGF_REG2_ZT(LGF_GO)
 #undef LGF_GO
@@ -425,21 +610,22 @@ static std::string reg2_name(int which, const Geom &g) {
 #define LGF_GO(LEN)                                                                                           \
     if (g.L[0] == LEN) {                                                                                       \
         if (which == 0) snprintf(buf, sizeof buf, "k_fftr2_xy<%s, %d, 0, %d, 0>", rn, LEN, Xy2Cfg<R, LEN>::PF);  \
+        else if (which == 3 && Xy2Cfg<R, LEN>::P % 4 != 0) snprintf(buf, sizeof buf, "k_fftr2_xy_gcluster<%s, %d>", rn, LEN); \
         else snprintf(buf, sizeof buf, "k_fftr2_xy<%s, %d, 1, %d, %d>", rn, LEN, Xy2Cfg<R, LEN>::P, which == 3 ? 1 : 0); \
     }
     LGF_REG2_LEN(LGF_GO)
 #undef LGF_GO
     return buf;
 }
-std::string fft_reg2_kernel_name(int which, const Geom &g, int prec, bool bulk) {
-    std::string s = prec == 8 ? reg2_name<double>(which, g) : reg2_name<float>(which, g);
-    if (bulk && which != 1 && s.size() > 10) s.insert(10, "_bulk");      // k_fftr2_xy -> k_fftr2_xy_bulk
+std::string fft_reg2_kernel_name(int which, const Geom &g, int prec, bool bulk, int zt_cluster) {
+    std::string s = prec == 8 ? reg2_name<double>(which, g, zt_cluster) : reg2_name<float>(which, g, zt_cluster);
+    if (bulk && which != 1 && s.size() > 10 && s.compare(0, 11, "k_fftr2_xy<") == 0) s.insert(10, "_bulk");      // k_fftr2_xy -> k_fftr2_xy_bulk
     return s;
 }
 
 template cudaError_t launch_fft_reg2<float>(int, const Geom &, C<float> *, const float *, float, const DevState *,
-                                            LaunchStream, C<float> *, float, bool, int);
+                                            LaunchStream, C<float> *, float, bool, int, int);
 template cudaError_t launch_fft_reg2<double>(int, const Geom &, C<double> *, const double *, double, const DevState *,
-                                             LaunchStream, C<double> *, double, bool, int);
+                                             LaunchStream, C<double> *, double, bool, int, int);
 
 }  // namespace lgf

@@ -90,7 +90,9 @@ bool fft_reg2_xy_by_component(const Geom &g, int prec);
 template <class R>
 cudaError_t launch_fft_reg2(int which, const Geom &g, C<R> *W, const R *p2tab, R scale, const DevState *st,
                             LaunchStream stream, C<R> *G, R half_alpha, bool bulk = false /* (x, y) planes by bulk copies */,
-                            int comp = -1 /* >= 0: forward (x, y) sweep of this packed component only */);
+                            int comp = -1 /* >= 0: forward (x, y) sweep of this packed component only */,
+                            int zt_cluster = 0 /* 2 / 4: the (z, t) tile split over a cluster of that many CTAs */);
+bool fft_reg2_zt_cluster_supported(const Geom &g, int nc);
 // true if a PASS_XY (first two axes) / PASS_ZT (last two axes) kernel is instantiated for these lengths
 bool fft_pair_supported(int kind, int La, int Lb);
 
@@ -153,7 +155,7 @@ cudaError_t launch_sweep_tma(const SweepMaps *maps, int nr, LinkPair<R> links, c
 std::string sweep_tma_kernel_name(const Geom &g, int nr, int prec, bool reunit, bool rsplit);
 
 // kernel instantiations as a profiler names them (lgf_kernel_names)
-std::string fft_reg2_kernel_name(int which, const Geom &g, int prec, bool bulk = false);
+std::string fft_reg2_kernel_name(int which, const Geom &g, int prec, bool bulk = false, int zt_cluster = 0);
 std::string sweep_kernel_name(const Geom &g, int nr, int prec, bool reunit, int share_mode, int minb);
 bool sweep_uses_share(const Geom &g, int nr, int prec, int share_mode);
 // block order of a sweep whose CTAs take `nt` consecutive sites: (z, t)-tiled when a t slice of traffic exceeds L2
