@@ -537,7 +537,7 @@ static int slab_sweep(lgf_slab *ctx, double *d_sums) {
                                 ctx->partial, &nb, ctx->st, LaunchStream(ctx->stream, false), 1, false, slab_halo<R>(ctx)));
     else
     SCK(launch_sweep<R>(ctx->nr, slab_links<R>(ctx), (const C<R> *)ctx->G, (C<R> *)ctx->W, ctx->gl, ctx->partial, &nb, ctx->st,
-                        LaunchStream(ctx->stream, false), 1, false, -1, 0, 3, slab_halo<R>(ctx)));
+                        LaunchStream(ctx->stream, false), 1, false, -1, 0, 0, slab_halo<R>(ctx)));
     k_slab_sum2<<<1, SLAB_THREADS, 0, ctx->stream>>>(ctx->partial, nb, d_sums, &ctx->st->done);
     SCK(cudaGetLastError());
     ctx->launches += 2;

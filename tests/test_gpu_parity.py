@@ -226,6 +226,30 @@ def test_trajectory_cluster_gbuild(lgf, storage):
         assert any(k.startswith("k_fftr2_xy_gcluster<double, 64>") for k in ctx.kernel_names()["fft"])
 
 
+@pytest.mark.parametrize("name,dims", [("C2", (16, 16, 16, 16)), ("mixed", (12, 6, 16, 4))])
+@pytest.mark.parametrize("storage", [18, 12])
+@pytest.mark.parametrize("share", [0, 1])
+def test_trajectory_fp32_sweep_five_ctas(lgf, config_cache, name, dims, storage, share):
+    """lgf_tune("sweep_minb", 5): the fp32 register sweep compiled for five CTAs per SM (96 registers) -- the automatic
+    choice on lattices of 740 CTAs and more, forced here on small ones.  Same arithmetic in the same order as the
+    three-CTA build: the oracle's parity bar, and bit-equal links."""
+    U = config_cache("C2") if name == "C2" else small_config(name, dims)
+    n = 12
+    U_o, F_o, T_o = oracle.iterate(dims, U, ALPHA, n)
+    tune = {"sweep_tma": 0, "sweep_share": share}
+    Fh, Th, P, out = run_trajectory(lgf, dims, U, 4, storage, n, tune=dict(tune, sweep_minb=5))
+    tol = TOL[4]
+    assert np.max(np.abs(Fh - F_o) / np.abs(F_o)) < tol["scalar"]
+    assert np.max(np.abs(Th - T_o) / np.abs(T_o)) < tol["scalar"]
+    assert np.max(np.abs(out - U_o)) < tol["links"]
+    Fh3, Th3, _, out3 = run_trajectory(lgf, dims, U, 4, storage, n, tune=dict(tune, sweep_minb=3))
+    assert np.array_equal(out, out3) and np.array_equal(Th, Th3)
+    with lgf.Context(dims, 4, storage) as ctx:
+        for k, v in dict(tune, sweep_minb=5).items():
+            ctx.tune(k, v)
+        assert ctx.kernel_names()["update"][0].endswith(", 5>")
+
+
 @pytest.mark.parametrize("nc", [2, 4])
 @pytest.mark.parametrize("prec", [8, 4])
 def test_trajectory_cluster_zt_tile(lgf, prec, nc):
