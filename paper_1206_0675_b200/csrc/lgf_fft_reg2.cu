@@ -294,7 +294,7 @@ struct Zt2Shape {
     // otherwise spends 134 on overlapping the 16 reciprocals of the scale step, which halves the occupancy)
     // (fp64 lines of up to 32 points only; 0 = no request, which is NOT the same as asking for 1: with "1" the fp32
     // 64 x 64 sweep took 168 registers instead of 128 and lost its second CTA -- 64^4 fp32 FFT 1.17 -> 1.35 ms)
-    static constexpr int MINB = (sizeof(R) == 8 && SMEM <= 110 * 1024 && LZ <= 32 && LT <= 32) ? 2 : 0;
+    static constexpr int MINB = (LZ <= 32 && LT <= 32 && SMEM <= 110 * 1024) ? (sizeof(R) == 8 ? 2 : 3) : 0;
     static_assert((XC * LZ) % 16 == 0 && (XC * LT) % 16 == 0, "16 lines per warp");
 };
 
