@@ -350,7 +350,7 @@ static int step_delta(lgf_ctx *ctx, const int *stop) {
     return LGF_OK;
 }
 static bool use_fft_bulk(const lgf_ctx *ctx) {
-    return ctx->tune_fft_bulk > 0 || (ctx->tune_fft_bulk < 0 && ctx->g.L[0] == 64 && ctx->prec == LGF_FP64);
+    return ctx->tune_fft_bulk > 0 || (ctx->tune_fft_bulk < 0 && ctx->g.L[0] == 64);
 }
 static int use_zt_cluster(const lgf_ctx *ctx) {
     const int nc = ctx->tune_fft_zt_cluster;

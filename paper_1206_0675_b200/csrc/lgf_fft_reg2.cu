@@ -207,7 +207,7 @@ __global__ void __launch_bounds__(2 * P * L) k_fftr2_xy_bulk(C<R> *__restrict__ 
     (void)base;
 }
 
-// ---- inverse (x, y) sweep ending in the g-build where the four component planes do NOT fit in one SM ----------
+// ---- inverse (x, y) sweep ending in the g-build with ONE plane per CTA (64-point planes) ----------------------
 // 64^4 fp64: a plane is 64 KB, so a CTA holds one component of one (z, t) slice and a5 -- which needs all of w(x) --
 // used to be a separate pass over the field (k_gbuild: 1.07 GB read + 1.6 GB written, 0.39 ms of a 6.5 ms iteration,
 // and the sweep before it wrote w only for that pass to read it back).  Here the four CTAs that hold the four
@@ -453,7 +453,7 @@ template <> struct Xy2Cfg<double, 32> { static constexpr int P = 4, PF = 2; };
 template <> struct Xy2Cfg<double, 64> { static constexpr int P = 1, PF = 1; };   // 4 planes of 64 x 64 fp64 exceed shared memory
 template <> struct Xy2Cfg<float, 16> { static constexpr int P = 8, PF = 8; };
 template <> struct Xy2Cfg<float, 32> { static constexpr int P = 4, PF = 2; };
-template <> struct Xy2Cfg<float, 64> { static constexpr int P = 4, PF = 4; };
+template <> struct Xy2Cfg<float, 64> { static constexpr int P = 1, PF = 1; };    // (4 planes: one CTA of 512 threads per SM -- 64^4 fp32 FFT 1.14 -> 1.08 ms with 1)
 // (Lz, Lt) pairs of the (z, t) sweep: Lt = Lz, and Lt = 2 Lz -- the usual shape of a lattice QCD volume (the
 // paper tunes on 32^3 x n) -- with the consecutive (kx, ky) indices per CTA
 template <class R, int LZ, int LT> struct Zt2Cfg;
