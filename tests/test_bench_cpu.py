@@ -48,7 +48,7 @@ def test_traffic_comes_from_the_newest_matching_capture():
                                                                   "k_fftr2_xy<double, 32, 1, 4, 1>"]}
     caps, stale = bench.captured_traffic("C3", "fp64", 18, launched)
     up = caps["update"][0]
-    assert up["bytes"] > 1.3e9 and up["kernel"].startswith("k_sweep_tma<double") and up["source"] == "profiles/r2b_traffic.csv"
+    assert up["bytes"] > 1.3e9 and up["kernel"].startswith("k_sweep_tma<double") and up["source"] == "profiles/r2c_traffic.csv"
     assert len(caps["fft"]) == 3 and all(r["bytes"] > 5e7 for r in caps["fft"])
     # a capture of a kernel this build does not launch is refused, not quoted
     caps2, stale2 = bench.captured_traffic("C3", "fp64", 18, {"update": ["k_sweep<double, 3, 3, 0, 0>"]})

@@ -210,9 +210,10 @@ def test_trajectory_two_thread_fft(lgf, config_cache, prec, storage):
 
 @pytest.mark.parametrize("prec,storage", VARIANTS)
 def test_trajectory_cluster_gbuild(lgf, prec, storage):
-    """64-point planes, one per CTA: the inverse (x, y) sweep runs as clusters of four CTAs, one per packed
-    component, and builds g out of the neighbours' shared memory (k_fftr2_xy_gcluster) -- no separate g-build pass.
-    Four iterations of a 64 x 64 x 16 x 16 lattice against the oracle, and against the unfused plan."""
+    """64-point planes: in fp64 (64 KB a plane, one per CTA) the inverse (x, y) sweep runs as clusters of four CTAs,
+    one per packed component, and builds g out of the neighbours' shared memory (k_fftr2_xy_gcluster) -- no separate
+    g-build pass; in fp32 the four planes share a CTA.  Four iterations of a 64 x 64 x 16 x 16 lattice against the
+    oracle, and against the unfused plan."""
     dims, n = (64, 64, 16, 16), 4
     U = inputs.smooth_config(dims, 0.3, 6416, haar=True)
     U_o, F_o, T_o = oracle.iterate(dims, U, ALPHA, n)
@@ -223,8 +224,9 @@ def test_trajectory_cluster_gbuild(lgf, prec, storage):
     assert np.max(np.abs(out - U_o)) < tol["links"]
     Fh2, Th2, _, out2 = run_trajectory(lgf, dims, U, prec, storage, n, tune={"fuse_g": 0})
     assert np.max(np.abs(out2 - out)) < (1e-13 if prec == 8 else 1e-5)
-    with lgf.Context(dims, prec, storage) as ctx:
-        assert any(k.startswith("k_fftr2_xy_gcluster<%s, 64>" % ("double" if prec == 8 else "float")) for k in ctx.kernel_names()["fft"])
+    with lgf.Context(dims, prec, storage) as ctx:       # (fp32: four 32 KB planes fit one CTA, no cluster needed)
+        last = "k_fftr2_xy_gcluster<double, 64>" if prec == 8 else "k_fftr2_xy_bulk<float, 64, 1, 4, 1>"
+        assert ctx.kernel_names()["fft"][-1].startswith(last)
 
 
 @pytest.mark.parametrize("name,dims", [("C2", (16, 16, 16, 16)), ("mixed", (12, 6, 16, 4))])
