@@ -276,7 +276,10 @@ __global__ void __cluster_dims__(4, 1, 1) __launch_bounds__(2 * L, 3)
 #pragma unroll
         for (int e = 0; e < 6; e++) G[(long long)e * V + s] = gx[e];
     }
-    cluster_sync_all();                                                      // nobody leaves while its tile is being read
+    // nobody leaves while its tile is being read.  The loads above have returned (the G stores used their values), so
+    // the arrival needs no fence -- a releasing one would wait for those stores to reach memory
+    cluster_arrive_relaxed();
+    cluster_wait();
 }
 
 // ---- (z, t) planes --------------------------------------------------------------------------------

@@ -85,6 +85,9 @@ __device__ __forceinline__ void dsmem_st(uint32_t addr, float x, float y) {
 }
 // the two halves of cluster_sync_all, for work that can sit between "my part is done" and "I need the others'"
 __device__ __forceinline__ void cluster_arrive() { asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory"); }
+// arrival without the release fence (SASS: no MEMBAR.ALL.GPU, which would wait for this thread's global stores): for a
+// barrier that only says "I have finished READING the others' shared memory" -- loads whose values have been used
+__device__ __forceinline__ void cluster_arrive_relaxed() { asm volatile("barrier.cluster.arrive.relaxed.aligned;" ::: "memory"); }
 __device__ __forceinline__ void cluster_wait() { asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory"); }
 
 // named barrier over `nthreads` threads of the CTA (whole warps), id 1..15; barrier 0 is __syncthreads
