@@ -16,6 +16,37 @@ struct alignas(2 * sizeof(R)) C {
 template <class R> __host__ __device__ __forceinline__ C<R> mk(R x, R y) { C<R> r; r.x = x; r.y = y; return r; }
 template <class R> __host__ __device__ __forceinline__ C<R> operator+(C<R> a, C<R> b) { return mk<R>(a.x + b.x, a.y + b.y); }
 template <class R> __host__ __device__ __forceinline__ C<R> operator-(C<R> a, C<R> b) { return mk<R>(a.x - b.x, a.y - b.y); }
+// Single precision on sm_100: complex add / subtract as ONE packed instruction (FADD2 / FFMA2, add.f32x2 / fma.rn.f32x2) --
+// the real and imaginary parts already sit in adjacent registers.  Each lane rounds to nearest like the scalar
+// instruction, so the results are the scalar ones bit for bit; what it buys is issue slots: the fp32 FFT sweeps are
+// issue-bound (ncu: 47-61 % of the issue slots, FMA pipe 33-41 %), and 27 % of their instructions were scalar adds.
+// (Non-template overloads: preferred over the templates above for C<float>.)
+__host__ __device__ __forceinline__ C<float> operator+(C<float> a, C<float> b) {
+#ifdef __CUDA_ARCH__
+    const float2 r = __fadd2_rn(make_float2(a.x, a.y), make_float2(b.x, b.y));
+    return mk<float>(r.x, r.y);
+#else
+    return mk<float>(a.x + b.x, a.y + b.y);
+#endif
+}
+__host__ __device__ __forceinline__ C<float> operator-(C<float> a, C<float> b) {
+#ifdef __CUDA_ARCH__
+    const float2 r = __ffma2_rn(make_float2(b.x, b.y), make_float2(-1.0f, -1.0f), make_float2(a.x, a.y));   // a - b, exact product
+    return mk<float>(r.x, r.y);
+#else
+    return mk<float>(a.x - b.x, a.y - b.y);
+#endif
+}
+// s * v + o with a real s (the radix-2 stage of the split line transforms); one packed FFMA2 in single precision
+template <class R> __host__ __device__ __forceinline__ C<R> fma_rc(R s, C<R> v, C<R> o) { return mk<R>(fma(s, v.x, o.x), fma(s, v.y, o.y)); }
+__host__ __device__ __forceinline__ C<float> fma_rc(float s, C<float> v, C<float> o) {
+#ifdef __CUDA_ARCH__
+    const float2 r = __ffma2_rn(make_float2(s, s), make_float2(v.x, v.y), make_float2(o.x, o.y));
+    return mk<float>(r.x, r.y);
+#else
+    return mk<float>(fmaf(s, v.x, o.x), fmaf(s, v.y, o.y));
+#endif
+}
 template <class R> __host__ __device__ __forceinline__ C<R> operator-(C<R> a) { return mk<R>(-a.x, -a.y); }
 template <class R> __host__ __device__ __forceinline__ C<R> operator*(C<R> a, C<R> b) { return mk<R>(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
 template <class R> __host__ __device__ __forceinline__ C<R> operator*(R s, C<R> a) { return mk<R>(s * a.x, s * a.y); }
@@ -31,6 +62,7 @@ template <class R> __host__ __device__ __forceinline__ void madc(C<R> &acc, C<R>
     acc.x += a.x * b.x; acc.x += a.y * b.y; acc.y += a.y * b.x; acc.y -= a.x * b.y;
 }
 template <class R> __host__ __device__ __forceinline__ R norm2(C<R> a) { return a.x * a.x + a.y * a.y; }
+
 
 // 1 / x and 1 / sqrt(x) for positive normal x.  In double precision the IEEE-exact `a / b` and `1 / sqrt(x)` each
 // expand to a hardware seed plus a dozen instructions with slow-path branches; the hot kernels call them 16 times per

@@ -38,7 +38,7 @@ struct SplitDft {
         static_for<0, M>([&](auto mc) {
             constexpr int m = decltype(mc)::value;
             const C<R> o = shfl_xor_c(v[m], PMASK);
-            const C<R> t = mk<R>(fma(s, v[m].x, o.x), fma(s, v[m].y, o.y));
+            const C<R> t = fma_rc(s, v[m], o);
             if constexpr (m == 0) v[m] = t;
             else v[m] = h ? twiddle_mul<L, m, -1, R>(t) : t;             // thread 1: (x[m] - x[m + M]) w^m
         });
@@ -52,7 +52,7 @@ struct SplitDft {
             C<R> y = v[m];
             if constexpr (m != 0) y = h ? twiddle_mul<L, m, +1, R>(v[m]) : v[m];   // thread 1: y1[m] conj(w)^m
             const C<R> o = shfl_xor_c(y, PMASK);
-            v[m] = mk<R>(fma(s, y.x, o.x), fma(s, y.y, o.y));           // y0 + y1  /  y0 - y1
+            v[m] = fma_rc(s, y, o);                                     // y0 + y1  /  y0 - y1
         });
     }
 };
