@@ -192,8 +192,8 @@ int lgf_apply_transform(lgf_ctx *ctx, const void *d_transform);
  * "sweep_tma" (1 / 0 / -1 = where it measured faster: the persistent staged sweep fed by TMA tensor copies,
  * k_sweep_tma, instead of the register sweep), "sweep_rsplit" (1 / 0: the staged sweep's fp64 register split by
  * setmaxnreg), "sweep_prefetch" (CTAs ahead of which the register sweep prefetches its tile into L2, 0 = off), "sweep_minb"
- * (resident CTAs per SM the register sweep's register allocation allows: 0 = automatic -- 3 in fp64, 5 in fp32 on
- * lattices that fill them -- or 2 / 3 / 5), "fft_bulk" (1 / 0 / -1 = where it measured faster: (x, y) FFT
+ * (resident CTAs per SM the register sweep's register allocation allows: 0 = automatic -- 3 in fp64, 4 or 5 in fp32 on
+ * lattices that fill them -- or 2 / 3 / 4 / 5), "fft_bulk" (1 / 0 / -1 = where it measured faster: (x, y) FFT
  * sweeps fed by cp.async.bulk), "fft_zt_cluster" (2 / 4: a 64 x 64 (z, t) FFT tile split over a thread-block
  * cluster of that many CTAs with the transposition through distributed shared memory, k_fftr2_zt_cluster; 0 /
  * -1 = the one-CTA tile, which measured faster), "reunit_every" (N > 0: in every

@@ -66,7 +66,7 @@ struct lgf_ctx {
     int tune_sweep_tma = -1;     // lgf_tune "sweep_tma" (see use_sweep_tma)
     int tune_sweep_rsplit = 1;   // lgf_tune "sweep_rsplit": register split between producer and compute warps (fp64 staged sweep)
     int tune_sweep_ahead = 0;    // lgf_tune "sweep_prefetch": CTAs ahead of which the sweep prefetches its tile into L2 (0 = off)
-    int tune_sweep_minb = 0;     // lgf_tune "sweep_minb": resident CTAs per SM the sweep's register allocation allows (0 = automatic, 2, 3, 5)
+    int tune_sweep_minb = 0;     // lgf_tune "sweep_minb": resident CTAs per SM the sweep's register allocation allows (0 = automatic, 2, 3, 4, 5)
     int tune_sweep_tz = 0;       // lgf_tune: z-planes per (z, t) tile of the sweep's block order (0 = automatic, 1 = plain)
     struct Stamp { cudaEvent_t a, b; int cls; };
     std::vector<Stamp> stamps;
@@ -1053,7 +1053,7 @@ int lgf_tune(lgf_ctx *ctx, const char *key, int value) {
     else if (k == "fft_zt_cluster") ctx->tune_fft_zt_cluster = value;
     else if (k == "sweep_rsplit") ctx->tune_sweep_rsplit = value;
     else if (k == "sweep_prefetch") ctx->tune_sweep_ahead = value < 0 ? 0 : value;
-    else if (k == "sweep_minb") ctx->tune_sweep_minb = (value == 2 || value == 3 || value == 5) ? value : 0;
+    else if (k == "sweep_minb") ctx->tune_sweep_minb = (value == 2 || value == 3 || value == 4 || value == 5) ? value : 0;
     else if (k == "reunit_every") ctx->tune_reunit = value < 0 ? 0 : value;
     else return fail(ctx, LGF_EINVAL, "lgf_tune: unknown key " + k);
     CK(cudaStreamSynchronize(ctx->stream));

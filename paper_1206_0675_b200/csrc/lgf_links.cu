@@ -491,15 +491,20 @@ bool sweep_uses_share(const Geom &g, int nr, int prec, int share_mode) {
                            : (nr == 3 && SWEEP_THREADS % g.L[0] == 0 && (prec == 4 || sweep_slice_beyond_l2(g, nr, prec)));
 }
 // Resident CTAs per SM the sweep is compiled for (its register cap).  minb = 0: automatic -- 3 (168 registers) in fp64;
-// in fp32, where a thread's loads carry half the bytes and the sweep is short of bytes in flight, 5 (96 registers, no
-// spills) once the grid fills five CTAs per SM.  Measured on B200, iteration time 3 -> 5 CTAs: 32^4 fp32/18 0.2115 ->
-// 0.2051 ms, 24^3 x 48 0.1613 -> 0.1508 ms, 64^4 3.57 -> 3.48 ms; 16^4 (512 CTAs) 0.0208 -> 0.0210 ms; 6 CTAs (80
-// registers, spills) 0.2111 ms.  The SU(3)-projecting variant (REUNIT) exists for 3 only.
-int sweep_minb_of(const Geom &g, int prec, bool reunit, int minb) {
+// in fp32, where a thread's loads carry half the bytes and the sweep is short of bytes in flight, 5 (96 registers) for
+// the SHARE variant and 4 (128 registers) for the plain one, once the grid fills them.  Measured on B200, iteration
+// time at 3 / 4 / 5 CTAs: 32^4 fp32/18 (SHARE) 0.2029 / 0.2018 / 0.1964 ms; 24^3 x 48 fp32/18 (plain) 0.1590 / 0.1484 /
+// 0.1583 ms (at 96 registers the plain variant spills); 64^4 fp32/18 3.57 -> 3.48 ms at 5; 16^4 (512 CTAs) 0.0208 ->
+// 0.0210 ms at 5, so small lattices keep 3; 6 CTAs (80 registers, spills) lost everywhere.  The SU(3)-projecting
+// variant (REUNIT) exists for 3 only.
+int sweep_minb_of(const Geom &g, int prec, bool reunit, bool share, int minb) {
     if (reunit) return SWEEP_MINB;
     if (minb == 2) return 2;
+    if (prec != 4) return SWEEP_MINB;
+    if (minb == 4 || minb == 5) return minb;
     const long long nb = (g.V + SWEEP_THREADS - 1) / SWEEP_THREADS;
-    if (prec == 4 && (minb == 5 || (minb <= 0 && nb >= 5 * 148))) return 5;
+    if (minb <= 0 && share && nb >= 5 * 148) return 5;
+    if (minb <= 0 && !share && nb >= 4 * 148) return 4;
     return SWEEP_MINB;
 }
 // the instantiation launch_sweep picks, as a profiler prints it (bench.py matches ncu captures against it)
@@ -507,7 +512,7 @@ std::string sweep_kernel_name(const Geom &g, int nr, int prec, bool reunit, int 
     char buf[96];
     const bool share = sweep_uses_share(g, nr, prec, share_mode);
     snprintf(buf, sizeof buf, "k_sweep<%s, %d, %d, %d, %d>", prec == 8 ? "double" : "float", nr, reunit ? 1 : 0, share ? 1 : 0,
-             sweep_minb_of(g, prec, reunit, minb));
+             sweep_minb_of(g, prec, reunit, share, minb));
     return buf;
 }
 // (z, t)-tiled block order when the (x, y) plane is a whole number of CTAs of `nt` sites; TZ: about 24 MB of traffic
@@ -540,11 +545,15 @@ cudaError_t launch_sweep(int nr, LinkPair<R> links, const C<R> *G, C<R> *W, cons
 #define LGF_SWK(RU, SH, MB)                                                                              \
     if (nr == 3) return launch_pdl(k_sweep<R, 3, RU, SH, MB>, dim3(nb), dim3(SWEEP_THREADS), 0, stream, links, G, W, g, partial, st, bo, ahead, halo); \
     else return launch_pdl(k_sweep<R, 2, RU, SH, MB>, dim3(nb), dim3(SWEEP_THREADS), 0, stream, links, G, W, g, partial, st, bo, ahead, halo);
-    const int mb = sweep_minb_of(g, (int)sizeof(R), reunit, minb);
+    const int mb = sweep_minb_of(g, (int)sizeof(R), reunit, share, minb);
     if constexpr (sizeof(R) == 4) {
         if (mb == 5) {
             if (share) { LGF_SWK(false, true, 5) }
             else { LGF_SWK(false, false, 5) }
+        }
+        if (mb == 4) {
+            if (share) { LGF_SWK(false, true, 4) }
+            else { LGF_SWK(false, false, 4) }
         }
     }
     if (mb == 2) {

@@ -108,7 +108,7 @@ cudaError_t launch_sweep(int nr, LinkPair<R> links, const C<R> *G, C<R> *W, cons
                          bool reunit /* project every new link onto SU(3) */,
                          int share_mode /* A'_x, A'_y through shared memory: 1 / 0 / -1 = where it measured faster */,
                          int ahead /* L2 bulk prefetch of the tile `ahead` CTAs later (0 = none) */,
-                         int minb /* resident CTAs per SM the register allocation allows: 0 = automatic (sweep_minb_of), 2, 3, 5 (fp32) */,
+                         int minb /* resident CTAs per SM the register allocation allows: 0 = automatic (sweep_minb_of), 2, 3, 4 / 5 (fp32) */,
                          const SweepHalo<R> &halo = SweepHalo<R>());
 template <class R>
 cudaError_t launch_plaquette(int nr, LinkPair<R> links, const Geom &g, double *partial, int *nblocks,
@@ -156,7 +156,7 @@ std::string sweep_tma_kernel_name(const Geom &g, int nr, int prec, bool reunit, 
 
 // kernel instantiations as a profiler names them (lgf_kernel_names)
 std::string fft_reg2_kernel_name(int which, const Geom &g, int prec, bool bulk = false, int zt_cluster = 0);
-int sweep_minb_of(const Geom &g, int prec, bool reunit, int minb);
+int sweep_minb_of(const Geom &g, int prec, bool reunit, bool share, int minb);
 std::string sweep_kernel_name(const Geom &g, int nr, int prec, bool reunit, int share_mode, int minb);
 bool sweep_uses_share(const Geom &g, int nr, int prec, int share_mode);
 // block order of a sweep whose CTAs take `nt` consecutive sites: (z, t)-tiled when a t slice of traffic exceeds L2

@@ -232,15 +232,16 @@ def test_trajectory_cluster_gbuild(lgf, prec, storage):
 @pytest.mark.parametrize("name,dims", [("C2", (16, 16, 16, 16)), ("mixed", (12, 6, 16, 4))])
 @pytest.mark.parametrize("storage", [18, 12])
 @pytest.mark.parametrize("share", [0, 1])
-def test_trajectory_fp32_sweep_five_ctas(lgf, config_cache, name, dims, storage, share):
-    """lgf_tune("sweep_minb", 5): the fp32 register sweep compiled for five CTAs per SM (96 registers) -- the automatic
-    choice on lattices of 740 CTAs and more, forced here on small ones.  Same arithmetic in the same order as the
-    three-CTA build: the oracle's parity bar, and bit-equal links."""
+@pytest.mark.parametrize("minb", [4, 5])
+def test_trajectory_fp32_sweep_five_ctas(lgf, config_cache, name, dims, storage, share, minb):
+    """lgf_tune("sweep_minb", 4 | 5): the fp32 register sweep compiled for four / five CTAs per SM (128 / 96 registers) --
+    the automatic choices on lattices that fill them, forced here on small ones.  Same arithmetic in the same order as
+    the three-CTA build: the oracle's parity bar, and bit-equal links."""
     U = config_cache("C2") if name == "C2" else small_config(name, dims)
     n = 12
     U_o, F_o, T_o = oracle.iterate(dims, U, ALPHA, n)
     tune = {"sweep_tma": 0, "sweep_share": share}
-    Fh, Th, P, out = run_trajectory(lgf, dims, U, 4, storage, n, tune=dict(tune, sweep_minb=5))
+    Fh, Th, P, out = run_trajectory(lgf, dims, U, 4, storage, n, tune=dict(tune, sweep_minb=minb))
     tol = TOL[4]
     assert np.max(np.abs(Fh - F_o) / np.abs(F_o)) < tol["scalar"]
     assert np.max(np.abs(Th - T_o) / np.abs(T_o)) < tol["scalar"]
@@ -248,9 +249,9 @@ def test_trajectory_fp32_sweep_five_ctas(lgf, config_cache, name, dims, storage,
     Fh3, Th3, _, out3 = run_trajectory(lgf, dims, U, 4, storage, n, tune=dict(tune, sweep_minb=3))
     assert np.array_equal(out, out3) and np.array_equal(Th, Th3)
     with lgf.Context(dims, 4, storage) as ctx:
-        for k, v in dict(tune, sweep_minb=5).items():
+        for k, v in dict(tune, sweep_minb=minb).items():
             ctx.tune(k, v)
-        assert ctx.kernel_names()["update"][0].endswith(", 5>")
+        assert ctx.kernel_names()["update"][0].endswith(", %d>" % minb)
 
 
 @pytest.mark.parametrize("nc", [2, 4])
